@@ -1,0 +1,113 @@
+"""ctypes view of oracle/acx_oracle.c — the plain single-threaded CPU decoder of FORMAT.md (§2).
+
+ORACLE: test infrastructure, not product code.  It imports nothing from paper_2606_18900_b200."""
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_DIR = os.path.dirname(os.path.abspath(__file__))
+_lib = None
+
+ERRORS = {0: "OK", -1: "E_MAGIC", -2: "E_VERSION", -3: "E_TRUNCATED", -4: "E_CORRUPT", -5: "E_RANGE", -6: "E_LEVEL",
+          -7: "E_NOMEM"}
+
+HEADER_FIELDS = ["N", "n_blocks", "log2_bs", "min_match", "W", "prob_bits", "n_tables", "max_level", "max_cmds", "flags",
+                 "tables_off", "dir_off", "fnv_off", "payload_off", "archive_bytes", "total_lit", "total_match_bytes",
+                 "total_matches", "total_cmds", "src_window"]
+
+
+class OracleError(Exception):
+    def __init__(self, rc):
+        super().__init__(ERRORS.get(rc, str(rc)))
+        self.code = rc
+        self.name = ERRORS.get(rc, str(rc))
+
+
+def build(force=False):
+    src = os.path.join(_DIR, "acx_oracle.c")
+    out = os.path.join(_DIR, "libacx_oracle.so")
+    if force or not os.path.exists(out) or os.path.getmtime(out) < os.path.getmtime(src):
+        subprocess.run(["gcc", "-O2", "-std=c11", "-Wall", "-shared", "-fPIC", "-o", out, src], check=True)
+    return out
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        _lib = ctypes.CDLL(build())
+        p, u64 = ctypes.c_void_p, ctypes.c_uint64
+        _lib.acx_oracle_header.argtypes = [p, u64, p]
+        _lib.acx_oracle_decode.argtypes = [p, u64, p, u64, ctypes.c_int]
+        _lib.acx_oracle_block.argtypes = [p, u64, u64] + [p] * 9
+        _lib.acx_oracle_rans.argtypes = [p, ctypes.c_uint32, ctypes.c_uint32, p, u64, p, p, u64, p, p]
+        _lib.acx_oracle_fnv1a64.argtypes = [p, u64]
+        _lib.acx_oracle_fnv1a64.restype = u64
+    return _lib
+
+
+def _arr(a):
+    a = np.frombuffer(a, dtype=np.uint8) if isinstance(a, (bytes, bytearray)) else a
+    return np.ascontiguousarray(a, dtype=np.uint8)
+
+
+def header(archive):
+    a = _arr(archive)
+    f = np.zeros(20, dtype=np.uint64)
+    rc = _load().acx_oracle_header(a.ctypes.data, a.size, f.ctypes.data)
+    if rc:
+        raise OracleError(rc)
+    return {k: int(v) for k, v in zip(HEADER_FIELDS, f)}
+
+
+def decode(archive, check_levels=True):
+    """The whole decompressed output (uint8 array).  Raises OracleError on any format violation."""
+    a = _arr(archive)
+    n = header(a)["N"]
+    out = np.zeros(max(n, 1), dtype=np.uint8)
+    rc = _load().acx_oracle_decode(a.ctypes.data, a.size, out.ctypes.data, n, 1 if check_levels else 0)
+    if rc:
+        raise OracleError(rc)
+    return out[:n]
+
+
+def block(archive, b):
+    """Stage-level view of block b: dict of tokens, literals, sources, lengths and positions."""
+    a = _arr(archive)
+    lib = _load()
+    counts = np.zeros(6, dtype=np.uint32)
+    rc = lib.acx_oracle_block(a.ctypes.data, a.size, b, counts.ctypes.data, *([None] * 8))
+    if rc:
+        raise OracleError(rc)
+    n_cmd, n_match, n_lit = int(counts[0]), int(counts[1]), int(counts[2])
+    r = dict(n_cmd=n_cmd, n_match=n_match, n_lit=n_lit, n_words=int(counts[3]), n_ext=int(counts[4]), level=int(counts[5]),
+             cmd=np.zeros(n_cmd, np.uint8), mlen=np.zeros(n_match, np.uint8), lit=np.zeros(n_lit, np.uint8),
+             src=np.zeros(n_match, np.uint64), lit_len=np.zeros(n_cmd, np.uint32), match_len=np.zeros(n_cmd, np.uint32),
+             lit_pos=np.zeros(n_cmd, np.uint32), out_pos=np.zeros(n_cmd, np.uint64))
+    rc = lib.acx_oracle_block(a.ctypes.data, a.size, b, counts.ctypes.data, *[r[k].ctypes.data for k in
+                              ("cmd", "mlen", "lit", "src", "lit_len", "match_len", "lit_pos", "out_pos")])
+    if rc:
+        raise OracleError(rc)
+    return r
+
+
+def rans_decode(freq, tid, states, words, prob_bits=11):
+    """FORMAT.md §1.5 alone.  freq: (n_tables, 256) u16; tid: table id per symbol; states: 32 u32; words: u16 array.
+    Returns (symbols, final_states, words_used)."""
+    freq = np.ascontiguousarray(freq, dtype=np.uint16).reshape(-1, 256)
+    tid = np.ascontiguousarray(tid, dtype=np.uint8)
+    st = np.ascontiguousarray(states, dtype=np.uint32).copy()
+    w = np.ascontiguousarray(words, dtype="<u2")
+    sym = np.zeros(max(tid.size, 1), dtype=np.uint8)
+    used = ctypes.c_uint64()
+    rc = _load().acx_oracle_rans(freq.ctypes.data, freq.shape[0], prob_bits, tid.ctypes.data, tid.size, st.ctypes.data,
+                                 w.ctypes.data, w.size, sym.ctypes.data, ctypes.byref(used))
+    if rc:
+        raise OracleError(rc)
+    return sym[:tid.size], st, used.value
+
+
+def fnv1a64(data):
+    a = _arr(data)
+    return int(_load().acx_oracle_fnv1a64(a.ctypes.data, a.size))

@@ -1,0 +1,98 @@
+"""Pins of the oracle's rANS step (FORMAT.md §1.5) against an independent pure-Python encoder (tests/acx_build.py),
+closed forms and the final-state invariant."""
+import math
+
+import numpy as np
+import pytest
+
+from acx_build import M, normalise, rans_encode
+from oracle import acx_oracle as O
+
+
+def roundtrip(symbols, tids, freqs):
+    states, words = rans_encode(list(symbols), list(tids), freqs)
+    sym, final, used = O.rans_decode(np.array(freqs, dtype=np.uint16), np.array(tids, dtype=np.uint8),
+                                     np.array(states, dtype=np.uint32), np.array(words, dtype=np.uint16))
+    assert used == len(words)                       # word count consumed == stored count
+    assert (final == (1 << 16)).all()               # encoder started at 2^16 -> decoder ends there
+    assert list(sym) == list(symbols)
+    return states, words
+
+
+@pytest.mark.parametrize("n", [0, 1, 31, 32, 33, 64, 1000])
+def test_identity_random(n):
+    rng = np.random.default_rng(n)
+    s = rng.integers(0, 256, n)
+    hist = np.bincount(s, minlength=256).tolist()
+    roundtrip(s.tolist(), [0] * n, [normalise(hist)])
+
+
+def test_single_symbol_alphabet_needs_no_words():
+    f = [0] * 256
+    f[65] = M
+    states, words = roundtrip([65] * 500, [0] * 500, [f])
+    assert words == [] and states == [1 << 16] * 32     # x = M * (x >> 11) + (x & (M-1)) is the identity
+
+
+def test_two_symbols_freq_1_and_M_minus_1():
+    f = [0] * 256
+    f[0], f[1] = 1, M - 1
+    rng = np.random.default_rng(7)
+    s = (rng.random(5000) < 0.999).astype(int)
+    s[::700] = 0
+    roundtrip(s.tolist(), [0] * len(s), [f])
+
+
+def test_worked_example_by_hand():
+    # One symbol 'a' (freq 512, cum 0 in a table {a:512, b:1536}) on state 0, encoder side by hand:
+    #   x = 2^16 = 65536; f << 21 = 2^30 > x -> no word; x' = (65536 // 512) << 11 + 65536 % 512 + 0 = 128 * 2048 = 262144
+    # Decoder: slot = 262144 & 2047 = 0 -> 'a'; x = 512 * (262144 >> 11) + 0 - 0 = 65536.
+    f = [0] * 256
+    f[97], f[98] = 512, 1536
+    states, words = rans_encode([97], [0], [f])
+    assert states[0] == 262144 and states[1:] == [65536] * 31 and words == []
+    sym, final, used = O.rans_decode(np.array([f], np.uint16), np.array([0], np.uint8), np.array(states, np.uint32),
+                                     np.zeros(0, np.uint16))
+    assert list(sym) == [97] and final[0] == 65536 and used == 0
+    # 'b' (freq 1536, cum 512): x' = (65536 // 1536) << 11 + 65536 % 1536 + 512 = 42 * 2048 + 1024 + 512 = 87552
+    states, words = rans_encode([98], [0], [f])
+    assert states[0] == 87552 and words == []
+    sym, final, used = O.rans_decode(np.array([f], np.uint16), np.array([0], np.uint8), np.array(states, np.uint32),
+                                     np.zeros(0, np.uint16))
+    assert list(sym) == [98] and final[0] == 65536
+
+
+def test_closed_form_size():
+    # compressed bits = sum -log2(f_s / M) + 32 x 16 bits of initial-state slack, within a small additive slack
+    rng = np.random.default_rng(11)
+    p = np.array([0.5, 0.25, 0.125, 0.0625, 0.0625])
+    s = rng.choice(5, size=20000, p=p)
+    f = [0] * 256
+    for k, q in enumerate(p):
+        f[k] = int(q * M)
+    states, words = roundtrip(s.tolist(), [0] * len(s), [f])
+    ideal = sum(-math.log2(f[v] / M) for v in s)
+    bits = 16 * len(words) + sum(math.log2(x) - 16 for x in states)
+    assert abs(bits - ideal) < 64            # rANS loses far less than one bit per state here
+
+
+def test_several_tables_interleaved_on_the_same_states():
+    rng = np.random.default_rng(3)
+    a = rng.integers(0, 4, 333)
+    b = rng.integers(100, 256, 777)
+    s = np.concatenate([a, b])
+    t = [0] * len(a) + [1] * len(b)
+    fa = normalise(np.bincount(a, minlength=256).tolist())
+    fb = normalise(np.bincount(b, minlength=256).tolist())
+    roundtrip(s.tolist(), t, [fa, fb])
+
+
+def test_truncated_word_stream_is_an_error():
+    rng = np.random.default_rng(5)
+    s = rng.integers(0, 256, 400)
+    f = normalise(np.bincount(s, minlength=256).tolist())
+    states, words = rans_encode(s.tolist(), [0] * 400, [f])
+    with pytest.raises(O.OracleError) as e:
+        O.rans_decode(np.array([f], np.uint16), np.zeros(400, np.uint8), np.array(states, np.uint32),
+                      np.array(words[:-1], np.uint16))
+    assert e.value.name == "E_TRUNCATED"
