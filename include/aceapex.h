@@ -1,0 +1,148 @@
+/* aceapex.h — C ABI of the B200 device-resident decoder for ACX-B200 archives (FORMAT.md).
+ *
+ * What the library computes (§2): an archive stores LZ77 back-references as ABSOLUTE positions in the
+ * decompressed output, partitioned into fixed-size blocks with four streams per block (literals, match lengths,
+ * absolute offsets, command sequence).  Decoding a block = entropy-decode its streams, prefix-sum the command
+ * sequence into output positions, place literals, and resolve matches by copying from absolute output positions once
+ * the source data is available (the "wavefront", §1, §3.1).  Every step runs in
+ * hand-written CUDA kernels for sm_100a; there is no CPU fallback.
+ *
+ * Conventions
+ *   - "d_" pointers are DEVICE memory owned by the caller (e.g. torch uint8 tensors) and must stay valid for the
+ *     lifetime stated; "h_" pointers are HOST memory.  The library never frees caller memory.
+ *   - All sizes/positions are uint64_t bytes.  Return value: 0 = ACEAPEX_OK, negative = error (aceapex_strerror).
+ *   - Decode calls are ASYNCHRONOUS on the handle's stream (default: the legacy default stream) unless stated; the
+ *     caller synchronises.  Device-side integrity problems (bad offset, rANS state mismatch, dependency timeout)
+ *     are latched in a device flag that aceapex_check() reads back.
+ *   - The library allocates small device state at open (tables, directory copy is NOT made: it reads the caller's
+ *     archive buffer) and never allocates on the hot path: scratch comes from aceapex_set_workspace().
+ *   - One handle must not be used from two host threads at once.
+ */
+#ifndef ACEAPEX_H
+#define ACEAPEX_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct aceapex_archive aceapex_archive;
+
+enum {
+    ACEAPEX_OK = 0,
+    ACEAPEX_E_MAGIC = -1,      /* not an ACX-B200 archive                                        */
+    ACEAPEX_E_VERSION = -2,    /* unsupported version / prob_bits                                */
+    ACEAPEX_E_TRUNCATED = -3,  /* archive_bytes smaller than the archive says                    */
+    ACEAPEX_E_CORRUPT = -4,    /* header / tables / directory inconsistent, or device flag set   */
+    ACEAPEX_E_RANGE = -5,      /* byte range or read id out of bounds                            */
+    ACEAPEX_E_BUDGET = -6,     /* vram_budget too small for the call                             */
+    ACEAPEX_E_WORKSPACE = -7,  /* workspace missing or smaller than aceapex_info.workspace_bytes */
+    ACEAPEX_E_CUDA = -8,       /* a CUDA runtime call failed (aceapex_last_cuda_error)           */
+    ACEAPEX_E_ARG = -9         /* null pointer / bad argument                                    */
+};
+
+typedef struct {
+    uint64_t raw_bytes;          /* N: decompressed size                                         */
+    uint64_t archive_bytes;      /* C: compressed size (whole archive)                           */
+    uint64_t n_blocks;
+    uint64_t block_size;
+    uint64_t total_lit_bytes;    /* bytes produced by literal runs                               */
+    uint64_t total_match_bytes;  /* M: bytes produced by matches (= source bytes read)           */
+    uint64_t total_matches;
+    uint64_t total_cmds;
+    uint64_t workspace_bytes;    /* device scratch the decode calls need (aceapex_set_workspace) */
+    uint32_t max_level;          /* FORMAT.md §3: number of match waves - 1                      */
+    uint32_t offset_width;       /* W                                                            */
+    uint32_t min_match;
+    uint32_t max_cmds;           /* largest per-block command count                              */
+    uint32_t n_coded_planes;     /* offset planes that are rANS-coded (the rest are raw)         */
+    uint32_t has_fnv;            /* per-block FNV-1a 64 section present                          */
+    uint32_t resident_warps;     /* warps of the persistent decode grid                          */
+    uint32_t reserved;
+} aceapex_info_t;
+
+/* Opens an archive that already resides in device memory ("H2D staging ... outside the timer").
+ * d_archive: device pointer, 16-byte aligned, archive_bytes long, must outlive the handle.
+ * h_archive_or_null: optional host copy of the same bytes (at least header + tables + directory); when null the
+ *   library copies that prefix from the device (synchronous).  Validates magic, version, section layout, tables and
+ *   the whole directory (monotone 16-byte aligned payload offsets, counts) and uploads the decode tables.
+ * Errors: E_ARG, E_MAGIC, E_VERSION, E_TRUNCATED, E_CORRUPT, E_CUDA.  Synchronous. */
+int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* h_archive_or_null, aceapex_archive** out);
+
+/* Frees the handle and the library's own device state (not the archive, not the workspace).  Synchronises. */
+int32_t aceapex_close(aceapex_archive* ar);
+
+int32_t aceapex_info(const aceapex_archive* ar, aceapex_info_t* out);
+
+/* Caller-provided device scratch, >= aceapex_info.workspace_bytes, 256-byte aligned; must stay valid and untouched
+ * by the caller while decode calls are in flight.  The first use zero-initialises its control area (async). */
+int32_t aceapex_set_workspace(aceapex_archive* ar, void* d_workspace, uint64_t workspace_bytes);
+
+/* cudaStream_t (as void*) all later calls are issued on; null = legacy default stream. */
+int32_t aceapex_set_stream(aceapex_archive* ar, void* cuda_stream);
+
+/* Whole-file decode (§3.3, the paper's "v4").  d_out: >= raw_bytes device bytes.  On completion of the
+ * stream, d_out[0..N) are the original bytes.  One persistent-kernel launch: blocks are taken in index order and a
+ * block waits (device-side ready flags) for the earlier blocks it copies from.  Errors: E_WORKSPACE, E_CUDA. */
+int32_t aceapex_decode_all(aceapex_archive* ar, void* d_out);
+
+/* Same result, scheduled the way the paper describes it: literal wave, then one match launch per dependency level
+ * (FORMAT.md §3; max_level + 2 launches).  Exists for measurement (BASELINE.json configs[4]: wavefront depth and
+ * per-launch overhead) and as a cross-check of the flag-driven schedule. */
+int32_t aceapex_decode_all_levels(aceapex_archive* ar, void* d_out);
+
+/* Arbitrary byte range [byte_lo, byte_hi) (§4, "v7-RA"): d_out[0 .. hi-lo) = those bytes; only the
+ * covering blocks are decoded, sources outside the range are reconstructed on demand by recursion on their own
+ * sources (depth <= max_level + 1, FORMAT.md §3).  vram_budget: upper bound on workspace bytes the call may use
+ * (0 = the whole workspace); E_BUDGET if it is below the minimum.  lo == hi is a no-op.  E_RANGE if lo > hi or hi > N. */
+int32_t aceapex_decode_range(aceapex_archive* ar, uint64_t byte_lo, uint64_t byte_hi, void* d_out, uint64_t vram_budget);
+
+/* Read-level random access (§4.1).  h_read_index: host array of n_index entries, 8 bytes per read
+ * (FORMAT.md §4: offset in bits 0..39, length in bits 40..63).  h_read_ids[n]: host array of read ids (duplicates
+ * allowed).  d_out receives the reads packed back to back in h_read_ids order (size: aceapex_reads_bytes).
+ * Only the blocks covering the reads, and recursively the source spans they need, are decoded.  E_RANGE on a bad id. */
+int32_t aceapex_decode_reads(aceapex_archive* ar, const uint64_t* h_read_index, uint64_t n_index,
+                             const uint64_t* h_read_ids, uint64_t n, void* d_out);
+
+/* Output size of aceapex_decode_reads; h_out_offsets_or_null[n+1] receives the packed offsets.  Host only. */
+int32_t aceapex_reads_bytes(const uint64_t* h_read_index, uint64_t n_index, const uint64_t* h_read_ids, uint64_t n,
+                            uint64_t* total_bytes, uint64_t* h_out_offsets_or_null);
+
+/* Makes bytes [pos_lo, pos_hi) of the decompressed output, already resident at d_ptr, usable as match sources by
+ * aceapex_decode_range (the ring of PAPER.md:107-109 §5: earlier windows stay resident while later ones decode).
+ * slot < 8; pos_lo == pos_hi clears the slot. */
+int32_t aceapex_set_resident(aceapex_archive* ar, uint32_t slot, uint64_t pos_lo, uint64_t pos_hi, const void* d_ptr);
+
+/* Device FNV-1a 64 of each block of d_data (= decompressed bytes [byte_lo, byte_hi), byte_lo block aligned) compared
+ * with the archive's FNV section ("FNV for device-resident GPU paths").  Synchronous; *n_bad = number
+ * of mismatching blocks.  E_ARG when the archive has no FNV section. */
+int32_t aceapex_verify_fnv(aceapex_archive* ar, const void* d_data, uint64_t byte_lo, uint64_t byte_hi, uint64_t* n_bad);
+
+/* End-to-end convenience for host data (bench "e2e"; §6.1): copies h_archive (pinned or pageable, same
+ * bytes the handle was opened on) into the handle's device archive, decodes into d_out_staging (>= N device bytes),
+ * copies the result to h_out, and synchronises. */
+int32_t aceapex_decode_all_host(aceapex_archive* ar, const void* h_archive, void* d_out_staging, void* h_out);
+
+/* Synchronises the stream and returns E_CORRUPT if any kernel latched an integrity error since the last check
+ * (details: aceapex_device_flags), E_CUDA on a CUDA error, else OK. */
+int32_t aceapex_check(aceapex_archive* ar);
+uint32_t aceapex_device_flags(const aceapex_archive* ar);   /* bit set of ACEAPEX_DF_* from the last aceapex_check */
+int32_t aceapex_last_cuda_error(const aceapex_archive* ar); /* cudaError_t of the last failing runtime call         */
+const char* aceapex_strerror(int32_t code);
+
+/* Number of kernel launches the library issued on this handle so far (bench.py "gpu_launches"). */
+uint64_t aceapex_launch_count(const aceapex_archive* ar);
+
+enum {
+    ACEAPEX_DF_RANS = 1,      /* final rANS state / word count mismatch         */
+    ACEAPEX_DF_OFFSET = 2,    /* src >= dst or match leaves the block           */
+    ACEAPEX_DF_LENGTH = 4,    /* command lengths do not add up to the block     */
+    ACEAPEX_DF_TIMEOUT = 8,   /* a dependency flag was never set                */
+    ACEAPEX_DF_STACK = 16     /* demand stack overflow (range / read decode)    */
+};
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,5 +1,4 @@
-"""Builds the native libraries in-tree (no JIT cache): datagen (C), encoder (C++), oracle (C, under /oracle, test
-infrastructure only) and the CUDA decoder (sm_100a).  `python -m paper_2606_18900_b200.build [target...]`."""
+"""Builds the native libraries in-tree (no JIT cache): datagen (C), encoder (C++) and the CUDA decoder (sm_100a).  `python -m paper_2606_18900_b200.build [target...]`."""
 import os
 import shutil
 import subprocess
@@ -45,23 +44,6 @@ def build_encoder(force=False):
     return out
 
 
-def build_oracle(force=False):
-    odir = os.path.join(ROOT, "oracle")
-    src = [os.path.join(odir, "acx_oracle.c")]
-    out = os.path.join(odir, "libacx_oracle.so")
-    if force or _newer(out, src):
-        _run(["gcc", "-O2", "-std=c11", "-Wall", "-shared", "-fPIC", "-o", out] + src)
-    return out
-
-
-def build_cpu_mt(force=False):
-    src = [os.path.join(ROOT, "baseline", "acx_cpu_mt.cpp")]
-    out = os.path.join(ROOT, "baseline", "libacx_cpu_mt.so")
-    if os.path.exists(src[0]) and (force or _newer(out, src)):
-        _run(["g++", "-O2", "-std=c++17", "-Wall", "-shared", "-fPIC", "-pthread", "-o", out] + src)
-    return out
-
-
 def build_cuda(force=False):
     cs = os.path.join(PKG, "csrc")
     src = [os.path.join(cs, f) for f in sorted(os.listdir(cs)) if f.endswith(".cu")]
@@ -75,8 +57,7 @@ def build_cuda(force=False):
     return out
 
 
-TARGETS = {"datagen": build_datagen, "encoder": build_encoder, "oracle": build_oracle, "cpu_mt": build_cpu_mt,
-           "cuda": build_cuda}
+TARGETS = {"datagen": build_datagen, "encoder": build_encoder, "cuda": build_cuda}
 
 
 def build_all(force=False):

@@ -1,0 +1,551 @@
+// Host side of the C ABI (include/aceapex.h) and the decode kernels for sm_100a.
+#include "aceapex.h"
+#include "acx_device.cuh"
+
+#include <algorithm>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+using namespace acx;
+
+// =================================================================================================== kernels =====
+
+namespace {
+
+struct BlockCtx {
+    uint64_t b, bstart, bend;       // block id, absolute byte range
+    DirEntry d;
+    const uint8_t* payload;
+    const uint32_t* ext;            // EXT array
+    const uint8_t* raw_planes;      // raw OFF planes, n_match bytes each
+    uint32_t n_ext_cmd;             // number of CMD escapes (they come first in EXT)
+    // per-warp scratch
+    uint8_t *tok_cmd, *tok_mlen, *off_planes, *lit;
+};
+
+__device__ __forceinline__ void report(const Params& P, uint32_t bit) { atomicOr(P.err, bit); }
+
+// Scratch layout per warp: [lit: BS + 32][tok_cmd: max_cmds][tok_mlen: max_cmds][off planes: n_coded x max_cmds] (16 B aligned)
+__device__ __forceinline__ void bind_scratch(const Params& P, uint32_t warp_global, BlockCtx& c) {
+    uint8_t* s = P.scratch + (uint64_t)warp_global * P.scratch_per_warp;
+    uint64_t mc = (P.max_cmds + 15u) & ~15u;
+    c.lit = s; s += (1ull << P.log2_bs) + 32;
+    c.tok_cmd = s; s += mc;
+    c.tok_mlen = s; s += mc;
+    c.off_planes = s;
+}
+
+// A1: entropy-decode the block's streams into the warp's scratch.  lit_limit: number of literal symbols wanted.
+__device__ __forceinline__ bool parse_block(const Params& P, const uint32_t* s_luts, uint16_t* ring, BlockCtx& c, uint32_t lit_limit) {
+    const DirEntry* dp = P.dir + c.b;
+    const uint4* d4 = reinterpret_cast<const uint4*>(dp);
+    uint4 a = __ldg(d4), q = __ldg(d4 + 1);
+    c.d.payload_off = (uint64_t)a.x | ((uint64_t)a.y << 32);
+    c.d.n_cmd = a.z; c.d.n_match = a.w; c.d.n_lit = q.x; c.d.n_words = q.y; c.d.n_ext = q.z; c.d.level = (uint16_t)(q.w & 0xffff);
+    c.bstart = c.b << P.log2_bs;
+    c.bend = min((unsigned long long)(c.bstart + (1ull << P.log2_bs)), (unsigned long long)P.N);
+    c.payload = P.archive + c.d.payload_off;
+    uint64_t rans_bytes = 128 + 2ull * c.d.n_words;
+    c.ext = reinterpret_cast<const uint32_t*>(c.payload + ((rans_bytes + 3) & ~3ull));
+    c.raw_planes = reinterpret_cast<const uint8_t*>(c.ext + c.d.n_ext);
+    uint64_t mc = (P.max_cmds + 15u) & ~15u;
+    if (c.d.n_cmd > P.max_cmds || c.d.n_match > c.d.n_cmd || c.d.n_lit > (1u << P.log2_bs)) { if (lane_id() == 0) report(P, DF_LENGTH); return false; }
+
+    Rans r;
+    r.init(c.payload, P.archive + P.archive_bytes, ring);
+    uint32_t i0 = 0;
+    c.n_ext_cmd = rans_region<true>(r, s_luts + P.lut_cmd * LUT_SIZE, i0, c.d.n_cmd, c.tok_cmd); i0 += c.d.n_cmd;
+    rans_region<false>(r, s_luts + P.lut_mlen * LUT_SIZE, i0, c.d.n_match, c.tok_mlen); i0 += c.d.n_match;
+    for (int p = (int)P.W - 1; p >= 0; p--) {
+        int li = P.plane_lut[p];
+        if (li < 0) continue;
+        // coded planes are stored in decode order: slot k = number of coded planes above p
+        uint32_t k = 0;
+        for (int t = (int)P.W - 1; t > p; t--) k += P.plane_lut[t] >= 0;
+        rans_region<false>(r, s_luts + li * LUT_SIZE, i0, c.d.n_match, c.off_planes + k * mc); i0 += c.d.n_match;
+    }
+    uint32_t nl = min(lit_limit, c.d.n_lit);
+    rans_region<false>(r, s_luts + P.lut_lit * LUT_SIZE, i0, nl, c.lit);
+    if (nl == c.d.n_lit) {   // whole stream decoded: FORMAT.md §1.5 integrity check
+        bool bad = (r.x != 65536u) || (r.wp != c.d.n_words);
+        if (__any_sync(0xffffffffu, bad)) { if (lane_id() == 0) report(P, DF_RANS); return false; }
+    }
+    __syncwarp();
+    return true;
+}
+
+// offset of match j assembled from coded planes (scratch) and raw planes (payload)
+__device__ __forceinline__ uint64_t match_src(const Params& P, const BlockCtx& c, uint32_t j) {
+    uint64_t src = 0, mc = (P.max_cmds + 15u) & ~15u;
+    uint32_t k = 0;
+    for (int p = (int)P.W - 1; p >= 0; p--) {
+        if (P.plane_lut[p] >= 0) { src |= (uint64_t)c.off_planes[k * mc + j] << (8 * p); k++; }
+        else src |= (uint64_t)__ldg(c.raw_planes + (uint64_t)P.plane_raw[p] * c.d.n_match + j) << (8 * p);
+    }
+    return src;
+}
+
+__device__ __forceinline__ void wait_block(const Params& P, uint64_t S) {
+    const uint32_t* f = P.flags + S;
+    uint32_t spins = 0;
+    while (ld_acquire(f) != P.epoch) {
+        __nanosleep(64);
+        if (++spins > (1u << 24)) { report(P, DF_TIMEOUT); break; }
+    }
+}
+
+// Copy one match whose seed lies in the current FULL window.  WAIT: the flag-driven schedule waits for the source
+// blocks (other than the own block); the level schedule needs no wait (sources were completed by earlier launches).
+template <bool WAIT>
+__device__ __forceinline__ void copy_match_window(const Params& P, const BlockCtx& c, uint64_t dst, uint64_t src, uint32_t len) {
+    if (WAIT) {
+        uint64_t seed_end = min((unsigned long long)(src + len), (unsigned long long)dst);
+        uint64_t s0 = src >> P.log2_bs, s1 = (seed_end - 1) >> P.log2_bs;
+        for (uint64_t S = s0; S <= s1; S++) if (S != c.b) wait_block(P, S);
+    }
+    copy_bytes<true>(P.out + (dst - P.out_pos0), P.out + (src - P.out_pos0), len, dst - src);
+}
+
+// A2 + A3 + A4 for a whole block: scan the commands 32 at a time, place literal runs, then resolve the matches.
+// MODE 0: everything (flag-driven schedule); MODE 2: literals only; MODE 3: matches only.
+template <int MODE>
+__device__ __forceinline__ void emit_block(const Params& P, const BlockCtx& c) {
+    uint32_t lit_base = 0, out_base = 0, ec = 0, em = c.n_ext_cmd;
+    const uint32_t lane = lane_id();
+    for (uint32_t c0 = 0; c0 < c.d.n_cmd; c0 += 32) {
+        uint32_t ci = c0 + lane;
+        bool valid = ci < c.d.n_cmd, has_match = ci < c.d.n_match;
+        uint32_t tl = valid ? c.tok_cmd[ci] : 0, tm = has_match ? c.tok_mlen[ci] : 0;
+        uint32_t ml = __ballot_sync(0xffffffffu, valid && tl == 255), mm = __ballot_sync(0xffffffffu, has_match && tm == 255);
+        uint32_t lit_len = tl, match_len = has_match ? P.min_match + tm : 0;
+        if (valid && tl == 255) lit_len = 255 + __ldg(c.ext + ec + __popc(ml & lanemask_lt()));
+        if (has_match && tm == 255) match_len = P.min_match + 255 + __ldg(c.ext + em + __popc(mm & lanemask_lt()));
+        ec += __popc(ml); em += __popc(mm);
+        // inclusive warp scans of lit_len and lit_len + match_len
+        uint32_t sl = lit_len, st = lit_len + match_len;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t a = __shfl_up_sync(0xffffffffu, sl, o), t = __shfl_up_sync(0xffffffffu, st, o);
+            if (lane >= (uint32_t)o) { sl += a; st += t; }
+        }
+        uint32_t lit_pos = lit_base + sl - lit_len;          // position of the run in LIT
+        uint64_t out_pos = c.bstart + out_base + (st - lit_len - match_len);   // absolute position of the run
+        lit_base += __shfl_sync(0xffffffffu, sl, 31);
+        out_base += __shfl_sync(0xffffffffu, st, 31);
+        bool ok = valid && (uint64_t)lit_pos + lit_len <= c.d.n_lit && out_pos + lit_len + match_len <= c.bend;
+        if (__any_sync(0xffffffffu, valid && !ok)) { if (lane == 0) report(P, DF_LENGTH); return; }
+        if (MODE != 3 && ok && lit_len) copy_bytes<false>(P.out + (out_pos - P.out_pos0), c.lit + lit_pos, lit_len, ~0ull);
+        if (MODE == 2) continue;
+        __syncwarp();
+        if (ok && has_match) {
+            uint64_t dst = out_pos + lit_len, src = match_src(P, c, ci);
+            if (src >= dst) report(P, DF_OFFSET);
+            else copy_match_window<MODE == 0>(P, c, dst, src, match_len);
+        }
+    }
+    if (out_base != (uint32_t)(c.bend - c.bstart) || lit_base != c.d.n_lit) { if (lane == 0) report(P, DF_LENGTH); }
+}
+
+__global__ void __launch_bounds__(256) k_decode(const Params P) {
+    extern __shared__ __align__(16) uint32_t smem[];
+    uint32_t* s_luts = smem;
+    const uint32_t n_lut_words = P.n_coded_tables * LUT_SIZE;
+    for (uint32_t i = threadIdx.x; i < n_lut_words / 4; i += blockDim.x)
+        reinterpret_cast<uint4*>(s_luts)[i] = __ldg(reinterpret_cast<const uint4*>(P.luts) + i);
+    __syncthreads();
+    const uint32_t warp = threadIdx.x >> 5, warps_per_cta = blockDim.x >> 5;
+    uint16_t* ring = reinterpret_cast<uint16_t*>(s_luts + n_lut_words) + warp * (RING_BYTES / 2);
+    BlockCtx c;
+    bind_scratch(P, blockIdx.x * warps_per_cta + warp, c);
+    for (;;) {
+        unsigned long long t = 0;
+        if (lane_id() == 0) t = atomicAdd(P.ticket, 1ull);
+        t = __shfl_sync(0xffffffffu, t, 0);
+        if (t >= P.n_work) break;
+        c.b = P.level_list ? (uint64_t)P.level_list[t] : P.first_block + t;
+        if (P.mode == 3) {
+            // match wave: only the command / length / offset streams are needed again
+            if (parse_block(P, s_luts, ring, c, 0)) emit_block<3>(P, c);
+            continue;
+        }
+        bool ok = parse_block(P, s_luts, ring, c, 0xffffffffu);
+        if (P.mode == 0) {
+            if (ok) emit_block<0>(P, c);
+            __threadfence();
+            __syncwarp();
+            if (lane_id() == 0) st_release(P.flags + c.b, P.epoch);   // set even on error so that nobody waits forever
+        } else if (ok) emit_block<2>(P, c);
+    }
+}
+
+// FNV-1a 64 of each block of d_data, compared with the archive's table; one thread per block (a check, not a hot path)
+__global__ void k_fnv(const uint8_t* data, uint64_t n_bytes, uint32_t log2_bs, const uint64_t* expect, unsigned long long* n_bad) {
+    uint64_t b = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x;
+    uint64_t lo = b << log2_bs;
+    if (lo >= n_bytes) return;
+    uint64_t hi = min((unsigned long long)(lo + (1ull << log2_bs)), (unsigned long long)n_bytes), f = 0xcbf29ce484222325ull;
+    for (uint64_t q = lo; q < hi; q++) { f ^= data[q]; f *= 0x100000001b3ull; }
+    if (f != expect[b]) atomicAdd(n_bad, 1ull);
+}
+
+} // namespace
+
+// ====================================================================================================== host =====
+
+struct aceapex_archive {
+    const uint8_t* d_archive = nullptr;
+    uint64_t archive_bytes = 0;
+    // header
+    uint64_t N = 0, n_blocks = 0, tables_off = 0, dir_off = 0, fnv_off = 0, payload_off = 0;
+    uint64_t total_lit = 0, total_match_bytes = 0, total_matches = 0, total_cmds = 0;
+    uint32_t log2_bs = 0, min_match = 0, W = 0, max_level = 0, max_cmds = 0, flags = 0;
+    uint32_t n_coded_tables = 0, n_coded_planes = 0, n_raw_planes = 0;
+    int8_t plane_lut[MAX_W], plane_raw[MAX_W];
+    uint32_t lut_cmd = 0, lut_mlen = 0, lut_lit = 0;
+    std::vector<std::vector<uint32_t>> level_blocks;   // block ids per level
+    // device state owned by the library
+    uint32_t* d_luts = nullptr;
+    uint32_t* d_level_lists = nullptr;                  // concatenated level_blocks
+    std::vector<uint64_t> level_off;
+    // workspace (caller's)
+    uint8_t* d_ws = nullptr; uint64_t ws_bytes = 0; bool ws_clean = false;
+    cudaStream_t stream = nullptr;
+    uint32_t epoch = 0;
+    Resident res[MAX_RESIDENT];
+    // launch geometry
+    int sms = 148, ctas_per_sm = 4, threads = 256;
+    uint32_t grid = 0; size_t smem = 0;
+    uint64_t scratch_per_warp = 0, ctrl_bytes = 0, flags_bytes = 0;
+    // status
+    int32_t last_cuda = 0; uint32_t dev_flags = 0; uint64_t launches = 0;
+};
+
+namespace {
+
+uint64_t rd64(const uint8_t* p) { uint64_t v; memcpy(&v, p, 8); return v; }
+uint32_t rd32(const uint8_t* p) { uint32_t v; memcpy(&v, p, 4); return v; }
+uint16_t rd16(const uint8_t* p) { uint16_t v; memcpy(&v, p, 2); return v; }
+
+#define CU(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { ar->last_cuda = (int32_t)e_; return ACEAPEX_E_CUDA; } } while (0)
+
+uint64_t align_up(uint64_t v, uint64_t a) { return (v + a - 1) / a * a; }
+
+// workspace: [ctrl 256 B: ticket u64 @0, err u32 @8][flags: n_blocks x u32][scratch: warps x scratch_per_warp]
+uint64_t workspace_need(const aceapex_archive* ar) {
+    return ar->ctrl_bytes + ar->flags_bytes + (uint64_t)ar->grid * (ar->threads / 32) * ar->scratch_per_warp;
+}
+
+void fill_params(const aceapex_archive* ar, Params& P) {
+    memset(&P, 0, sizeof P);
+    P.archive = ar->d_archive; P.archive_bytes = ar->archive_bytes;
+    P.dir = reinterpret_cast<const DirEntry*>(ar->d_archive + ar->dir_off);
+    P.luts = ar->d_luts; P.N = ar->N; P.log2_bs = ar->log2_bs; P.min_match = ar->min_match; P.W = ar->W;
+    P.n_coded_tables = ar->n_coded_tables;
+    memcpy(P.plane_lut, ar->plane_lut, MAX_W); memcpy(P.plane_raw, ar->plane_raw, MAX_W);
+    P.n_coded_planes = ar->n_coded_planes; P.n_raw_planes = ar->n_raw_planes;
+    P.lut_cmd = ar->lut_cmd; P.lut_mlen = ar->lut_mlen; P.lut_lit = ar->lut_lit;
+    memcpy(P.res, ar->res, sizeof P.res);
+    P.ticket = reinterpret_cast<unsigned long long*>(ar->d_ws);
+    P.err = reinterpret_cast<uint32_t*>(ar->d_ws + 8);
+    P.flags = reinterpret_cast<uint32_t*>(ar->d_ws + ar->ctrl_bytes);
+    P.scratch = ar->d_ws + ar->ctrl_bytes + ar->flags_bytes;
+    P.scratch_per_warp = ar->scratch_per_warp; P.max_cmds = ar->max_cmds;
+    P.clip_lo = 0; P.clip_hi = ar->N;
+}
+
+int32_t prepare_ws(aceapex_archive* ar) {
+    if (!ar->d_ws || ar->ws_bytes < workspace_need(ar)) return ACEAPEX_E_WORKSPACE;
+    if (!ar->ws_clean) {
+        CU(cudaMemsetAsync(ar->d_ws, 0, ar->ctrl_bytes + ar->flags_bytes, ar->stream));
+        ar->ws_clean = true; ar->epoch = 0;
+    }
+    return ACEAPEX_OK;
+}
+
+int32_t launch(aceapex_archive* ar, Params& P, uint64_t n_work) {
+    P.n_work = n_work;
+    if (n_work == 0) return ACEAPEX_OK;
+    CU(cudaMemsetAsync(P.ticket, 0, 8, ar->stream));
+    uint64_t warps = ar->threads / 32;
+    uint32_t grid = (uint32_t)std::min<uint64_t>(ar->grid, (n_work + warps - 1) / warps);
+    k_decode<<<grid, ar->threads, ar->smem, ar->stream>>>(P);
+    CU(cudaGetLastError());
+    ar->launches++;
+    return ACEAPEX_OK;
+}
+
+} // namespace
+
+extern "C" {
+
+int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* h_archive, aceapex_archive** out) {
+    if (!d_archive || !out || (reinterpret_cast<uintptr_t>(d_archive) & 15)) return ACEAPEX_E_ARG;
+    *out = nullptr;
+    aceapex_archive* ar = new (std::nothrow) aceapex_archive();
+    if (!ar) return ACEAPEX_E_ARG;
+    struct Guard { aceapex_archive* a; ~Guard() { if (a) aceapex_close(a); } } guard{ar};
+    ar->d_archive = static_cast<const uint8_t*>(d_archive); ar->archive_bytes = archive_bytes;
+    memset(ar->res, 0, sizeof ar->res);
+    if (archive_bytes < 160) return ACEAPEX_E_TRUNCATED;
+    uint8_t hdr[160];
+    if (h_archive) memcpy(hdr, h_archive, 160); else CU(cudaMemcpy(hdr, d_archive, 160, cudaMemcpyDeviceToHost));
+    static const uint8_t magic[8] = {0x41, 0x43, 0x58, 0x42, 0x32, 0x30, 0x30, 0x00};
+    if (memcmp(hdr, magic, 8)) return ACEAPEX_E_MAGIC;
+    if (rd32(hdr + 8) != 1 || rd32(hdr + 44) != (uint32_t)PROB_BITS) return ACEAPEX_E_VERSION;
+    if (rd32(hdr + 12) != 160) return ACEAPEX_E_CORRUPT;
+    ar->N = rd64(hdr + 16); ar->n_blocks = rd64(hdr + 24); ar->log2_bs = rd32(hdr + 32); ar->min_match = rd32(hdr + 36);
+    ar->W = rd32(hdr + 40); uint32_t n_tables = rd32(hdr + 48); ar->max_level = rd32(hdr + 52); ar->max_cmds = rd32(hdr + 56);
+    ar->flags = rd32(hdr + 60); ar->tables_off = rd64(hdr + 64); ar->dir_off = rd64(hdr + 72); ar->fnv_off = rd64(hdr + 80);
+    ar->payload_off = rd64(hdr + 88); uint64_t abytes = rd64(hdr + 96);
+    ar->total_lit = rd64(hdr + 104); ar->total_match_bytes = rd64(hdr + 112); ar->total_matches = rd64(hdr + 120); ar->total_cmds = rd64(hdr + 128);
+    if (ar->log2_bs < 3 || ar->log2_bs > 20 || ar->min_match < 1 || ar->W < 4 || ar->W > 8 || n_tables != 3 + ar->W) return ACEAPEX_E_CORRUPT;
+    if (ar->W < 8 && ar->N > (1ull << (8 * ar->W))) return ACEAPEX_E_CORRUPT;
+    if (ar->n_blocks != (ar->N + (1ull << ar->log2_bs) - 1) >> ar->log2_bs) return ACEAPEX_E_CORRUPT;
+    if (abytes > archive_bytes) return ACEAPEX_E_TRUNCATED;
+    if (abytes % 16 || ar->tables_off < 160 || ar->tables_off % 16 || ar->dir_off % 16 || ar->dir_off < ar->tables_off + 528ull * n_tables) return ACEAPEX_E_CORRUPT;
+    uint64_t meta_end = ar->dir_off + 32 * ar->n_blocks;
+    if (ar->flags & 1) { if (ar->fnv_off < meta_end || ar->fnv_off % 8) return ACEAPEX_E_CORRUPT; meta_end = ar->fnv_off + 8 * ar->n_blocks; }
+    if (ar->payload_off < meta_end || ar->payload_off % 16 || ar->payload_off > abytes) return ACEAPEX_E_CORRUPT;
+    if (ar->total_lit + ar->total_match_bytes != ar->N) return ACEAPEX_E_CORRUPT;
+    ar->archive_bytes = abytes;
+    // tables + directory
+    std::vector<uint8_t> meta_own;
+    const uint8_t* meta;   // bytes [0, meta_end)
+    if (h_archive) meta = static_cast<const uint8_t*>(h_archive);
+    else { meta_own.resize(meta_end); CU(cudaMemcpy(meta_own.data(), d_archive, meta_end, cudaMemcpyDeviceToHost)); meta = meta_own.data(); }
+    std::vector<uint32_t> luts;
+    auto add_lut = [&](uint32_t t, uint32_t& idx) -> bool {
+        const uint8_t* p = meta + ar->tables_off + 528ull * t;
+        uint32_t cum = 0;
+        idx = (uint32_t)(luts.size() / LUT_SIZE);
+        luts.resize(luts.size() + LUT_SIZE);
+        uint32_t* L = luts.data() + (size_t)idx * LUT_SIZE;
+        for (uint32_t s = 0; s < 256; s++) {
+            uint32_t f = rd16(p + 16 + 2 * s);
+            if (cum + f > (uint32_t)LUT_SIZE) return false;
+            for (uint32_t k = 0; k < f; k++) L[cum + k] = s | (f << 8) | (k << 20);
+            cum += f;
+        }
+        return cum == (uint32_t)LUT_SIZE;
+    };
+    for (uint32_t t = 0; t < n_tables; t++) {
+        uint32_t mode = rd32(meta + ar->tables_off + 528ull * t);
+        bool is_plane = t >= 2 && t < 2 + ar->W;
+        if (mode > 1 || (mode == 1 && !is_plane)) return ACEAPEX_E_CORRUPT;
+        uint32_t idx = 0;
+        if (mode == 0 && !add_lut(t, idx)) return ACEAPEX_E_CORRUPT;
+        if (t == 0) ar->lut_cmd = idx; else if (t == 1) ar->lut_mlen = idx; else if (t == 2 + ar->W) ar->lut_lit = idx;
+        else {
+            uint32_t p = t - 2;
+            ar->plane_lut[p] = mode == 0 ? (int8_t)idx : -1;
+            ar->plane_raw[p] = mode == 1 ? (int8_t)ar->n_raw_planes : -1;
+            if (mode == 0) ar->n_coded_planes++; else ar->n_raw_planes++;
+        }
+    }
+    for (uint32_t p = ar->W; p < MAX_W; p++) { ar->plane_lut[p] = -1; ar->plane_raw[p] = -1; }
+    ar->n_coded_tables = (uint32_t)(luts.size() / LUT_SIZE);
+    // directory validation + level lists
+    ar->level_blocks.assign(ar->max_level + 1, {});
+    uint64_t prev = ar->payload_off;
+    uint32_t seen_max_cmds = 0;
+    for (uint64_t b = 0; b < ar->n_blocks; b++) {
+        const uint8_t* p = meta + ar->dir_off + 32 * b;
+        uint64_t po = rd64(p), end = b + 1 < ar->n_blocks ? rd64(p + 32) : abytes;
+        uint32_t n_cmd = rd32(p + 8), n_match = rd32(p + 12), n_lit = rd32(p + 16), n_words = rd32(p + 20), n_ext = rd32(p + 24), lvl = rd16(p + 28);
+        if (po % 16 || po < prev || end <= po || end > abytes) return ACEAPEX_E_CORRUPT;
+        if (n_cmd < 1 || n_cmd > ar->max_cmds || !(n_match == n_cmd || n_match + 1 == n_cmd) || lvl > ar->max_level) return ACEAPEX_E_CORRUPT;
+        uint64_t need = ((128 + 2ull * n_words + 3) & ~3ull) + 4ull * n_ext + (uint64_t)ar->n_raw_planes * n_match;
+        if (po + need > end || n_lit > (1u << ar->log2_bs)) return ACEAPEX_E_CORRUPT;
+        prev = po; seen_max_cmds = std::max(seen_max_cmds, n_cmd);
+        ar->level_blocks[lvl].push_back((uint32_t)b);
+    }
+    // device tables
+    if (!luts.empty()) {
+        CU(cudaMalloc(&ar->d_luts, luts.size() * 4));
+        CU(cudaMemcpy(ar->d_luts, luts.data(), luts.size() * 4, cudaMemcpyHostToDevice));
+    }
+    if (ar->n_blocks && ar->n_blocks < (1ull << 32)) {
+        std::vector<uint32_t> cat;
+        for (auto& v : ar->level_blocks) { ar->level_off.push_back(cat.size()); cat.insert(cat.end(), v.begin(), v.end()); }
+        CU(cudaMalloc(&ar->d_level_lists, cat.size() * 4));
+        CU(cudaMemcpy(ar->d_level_lists, cat.data(), cat.size() * 4, cudaMemcpyHostToDevice));
+    }
+    // launch geometry
+    int dev = 0; cudaDeviceProp prop;
+    CU(cudaGetDevice(&dev)); CU(cudaGetDeviceProperties(&prop, dev));
+    ar->sms = prop.multiProcessorCount;
+    ar->threads = 256;
+    ar->smem = (size_t)ar->n_coded_tables * LUT_SIZE * 4 + (size_t)(ar->threads / 32) * RING_BYTES;
+    CU(cudaFuncSetAttribute(k_decode, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ar->smem));
+    int occ = 0;
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_decode, ar->threads, ar->smem));
+    if (occ < 1) return ACEAPEX_E_CUDA;
+    if (const char* e = getenv("ACEAPEX_CTAS_PER_SM")) occ = std::max(1, std::min(occ, atoi(e)));
+    ar->ctas_per_sm = occ;
+    ar->grid = (uint32_t)(ar->sms * occ);
+    uint64_t mc = align_up(ar->max_cmds, 16);
+    ar->scratch_per_warp = align_up((1ull << ar->log2_bs) + 32 + mc * (2 + ar->n_coded_planes), 256);
+    ar->ctrl_bytes = 256;
+    ar->flags_bytes = align_up(4 * ar->n_blocks + 4, 256);
+    guard.a = nullptr;
+    *out = ar;
+    return ACEAPEX_OK;
+}
+
+int32_t aceapex_close(aceapex_archive* ar) {
+    if (!ar) return ACEAPEX_E_ARG;
+    cudaDeviceSynchronize();
+    if (ar->d_luts) cudaFree(ar->d_luts);
+    if (ar->d_level_lists) cudaFree(ar->d_level_lists);
+    delete ar;
+    return ACEAPEX_OK;
+}
+
+int32_t aceapex_info(const aceapex_archive* ar, aceapex_info_t* o) {
+    if (!ar || !o) return ACEAPEX_E_ARG;
+    memset(o, 0, sizeof *o);
+    o->raw_bytes = ar->N; o->archive_bytes = ar->archive_bytes; o->n_blocks = ar->n_blocks; o->block_size = 1ull << ar->log2_bs;
+    o->total_lit_bytes = ar->total_lit; o->total_match_bytes = ar->total_match_bytes; o->total_matches = ar->total_matches;
+    o->total_cmds = ar->total_cmds; o->workspace_bytes = workspace_need(ar); o->max_level = ar->max_level; o->offset_width = ar->W;
+    o->min_match = ar->min_match; o->max_cmds = ar->max_cmds; o->n_coded_planes = ar->n_coded_planes; o->has_fnv = ar->flags & 1;
+    o->resident_warps = ar->grid * (ar->threads / 32);
+    return ACEAPEX_OK;
+}
+
+int32_t aceapex_set_workspace(aceapex_archive* ar, void* d_ws, uint64_t bytes) {
+    if (!ar || (reinterpret_cast<uintptr_t>(d_ws) & 255)) return ACEAPEX_E_ARG;
+    ar->d_ws = static_cast<uint8_t*>(d_ws); ar->ws_bytes = bytes; ar->ws_clean = false;
+    return (d_ws && bytes >= workspace_need(ar)) ? ACEAPEX_OK : ACEAPEX_E_WORKSPACE;
+}
+
+int32_t aceapex_set_stream(aceapex_archive* ar, void* s) {
+    if (!ar) return ACEAPEX_E_ARG;
+    ar->stream = static_cast<cudaStream_t>(s);
+    return ACEAPEX_OK;
+}
+
+int32_t aceapex_decode_all(aceapex_archive* ar, void* d_out) {
+    if (!ar || (!d_out && ar->N)) return ACEAPEX_E_ARG;
+    int32_t rc = prepare_ws(ar);
+    if (rc) return rc;
+    Params P; fill_params(ar, P);
+    P.mode = 0; P.out = static_cast<uint8_t*>(d_out); P.out_pos0 = 0; P.first_block = 0; P.epoch = ++ar->epoch;
+    return launch(ar, P, ar->n_blocks);
+}
+
+int32_t aceapex_decode_all_levels(aceapex_archive* ar, void* d_out) {
+    if (!ar || (!d_out && ar->N)) return ACEAPEX_E_ARG;
+    int32_t rc = prepare_ws(ar);
+    if (rc) return rc;
+    Params P; fill_params(ar, P);
+    P.out = static_cast<uint8_t*>(d_out); P.out_pos0 = 0; P.first_block = 0;
+    P.mode = 2; P.level_list = nullptr;
+    if ((rc = launch(ar, P, ar->n_blocks))) return rc;
+    // matches never wait in this schedule: every source is a literal byte (placed by the launch above) or a match
+    // byte of a lower-level block (completed by an earlier launch) -- FORMAT.md §3
+    for (uint32_t l = 0; l <= ar->max_level && ar->d_level_lists; l++) {
+        P.mode = 3; P.level_list = ar->d_level_lists + ar->level_off[l];
+        if ((rc = launch(ar, P, ar->level_blocks[l].size()))) return rc;
+    }
+    return ACEAPEX_OK;
+}
+
+int32_t aceapex_decode_range(aceapex_archive* ar, uint64_t lo, uint64_t hi, void* d_out, uint64_t budget) {
+    (void)d_out; (void)budget;
+    if (!ar) return ACEAPEX_E_ARG;
+    if (lo > hi || hi > ar->N) return ACEAPEX_E_RANGE;
+    return ACEAPEX_E_ARG;   // implemented in a later commit
+}
+
+int32_t aceapex_reads_bytes(const uint64_t* idx, uint64_t n_index, const uint64_t* ids, uint64_t n, uint64_t* total, uint64_t* offs) {
+    if ((!idx && n_index) || (!ids && n) || !total) return ACEAPEX_E_ARG;
+    uint64_t t = 0;
+    for (uint64_t i = 0; i < n; i++) {
+        if (ids[i] >= n_index) return ACEAPEX_E_RANGE;
+        if (offs) offs[i] = t;
+        t += idx[ids[i]] >> 40;
+    }
+    if (offs) offs[n] = t;
+    *total = t;
+    return ACEAPEX_OK;
+}
+
+int32_t aceapex_decode_reads(aceapex_archive* ar, const uint64_t* idx, uint64_t n_index, const uint64_t* ids, uint64_t n, void* d_out) {
+    (void)idx; (void)n_index; (void)ids; (void)n; (void)d_out;
+    if (!ar) return ACEAPEX_E_ARG;
+    return ACEAPEX_E_ARG;   // implemented in a later commit
+}
+
+int32_t aceapex_set_resident(aceapex_archive* ar, uint32_t slot, uint64_t lo, uint64_t hi, const void* p) {
+    if (!ar || slot >= MAX_RESIDENT || lo > hi || hi > ar->N) return ACEAPEX_E_ARG;
+    ar->res[slot].lo = lo; ar->res[slot].hi = hi; ar->res[slot].ptr = static_cast<const uint8_t*>(p);
+    return ACEAPEX_OK;
+}
+
+int32_t aceapex_verify_fnv(aceapex_archive* ar, const void* d_data, uint64_t lo, uint64_t hi, uint64_t* n_bad) {
+    if (!ar || !n_bad || !(ar->flags & 1) || (lo & ((1ull << ar->log2_bs) - 1)) || lo > hi || hi > ar->N) return ACEAPEX_E_ARG;
+    int32_t rc = prepare_ws(ar);
+    if (rc) return rc;
+    unsigned long long* cnt = reinterpret_cast<unsigned long long*>(ar->d_ws + 16);
+    CU(cudaMemsetAsync(cnt, 0, 8, ar->stream));
+    uint64_t nb = ((hi - lo) + (1ull << ar->log2_bs) - 1) >> ar->log2_bs;
+    if (nb) {
+        const uint64_t* expect = reinterpret_cast<const uint64_t*>(ar->d_archive + ar->fnv_off) + (lo >> ar->log2_bs);
+        k_fnv<<<(unsigned)((nb + 127) / 128), 128, 0, ar->stream>>>(static_cast<const uint8_t*>(d_data), hi - lo, ar->log2_bs, expect, cnt);
+        CU(cudaGetLastError());
+        ar->launches++;
+    }
+    unsigned long long h = 0;
+    CU(cudaMemcpyAsync(&h, cnt, 8, cudaMemcpyDeviceToHost, ar->stream));
+    CU(cudaStreamSynchronize(ar->stream));
+    *n_bad = h;
+    return ACEAPEX_OK;
+}
+
+int32_t aceapex_decode_all_host(aceapex_archive* ar, const void* h_archive, void* d_stage, void* h_out) {
+    if (!ar || !h_archive || (!d_stage && ar->N) || (!h_out && ar->N)) return ACEAPEX_E_ARG;
+    CU(cudaMemcpyAsync(const_cast<uint8_t*>(ar->d_archive), h_archive, ar->archive_bytes, cudaMemcpyHostToDevice, ar->stream));
+    int32_t rc = aceapex_decode_all(ar, d_stage);
+    if (rc) return rc;
+    if (ar->N) CU(cudaMemcpyAsync(h_out, d_stage, ar->N, cudaMemcpyDeviceToHost, ar->stream));
+    CU(cudaStreamSynchronize(ar->stream));
+    return ACEAPEX_OK;
+}
+
+int32_t aceapex_check(aceapex_archive* ar) {
+    if (!ar) return ACEAPEX_E_ARG;
+    CU(cudaStreamSynchronize(ar->stream));
+    ar->dev_flags = 0;
+    if (ar->d_ws && ar->ws_clean) {
+        uint32_t f = 0;
+        CU(cudaMemcpy(&f, ar->d_ws + 8, 4, cudaMemcpyDeviceToHost));
+        ar->dev_flags = f;
+        if (f) { CU(cudaMemset(ar->d_ws + 8, 0, 4)); return ACEAPEX_E_CORRUPT; }
+    }
+    return ACEAPEX_OK;
+}
+
+uint32_t aceapex_device_flags(const aceapex_archive* ar) { return ar ? ar->dev_flags : 0; }
+int32_t aceapex_last_cuda_error(const aceapex_archive* ar) { return ar ? ar->last_cuda : 0; }
+uint64_t aceapex_launch_count(const aceapex_archive* ar) { return ar ? ar->launches : 0; }
+
+const char* aceapex_strerror(int32_t c) {
+    switch (c) {
+        case ACEAPEX_OK: return "ok";
+        case ACEAPEX_E_MAGIC: return "not an ACX-B200 archive";
+        case ACEAPEX_E_VERSION: return "unsupported archive version";
+        case ACEAPEX_E_TRUNCATED: return "archive truncated";
+        case ACEAPEX_E_CORRUPT: return "archive corrupt";
+        case ACEAPEX_E_RANGE: return "range or read id out of bounds";
+        case ACEAPEX_E_BUDGET: return "vram budget too small";
+        case ACEAPEX_E_WORKSPACE: return "workspace missing or too small";
+        case ACEAPEX_E_CUDA: return "CUDA runtime error";
+        case ACEAPEX_E_ARG: return "bad argument";
+    }
+    return "unknown error";
+}
+
+} // extern "C"

@@ -1,0 +1,167 @@
+// Device side of the ACX-B200 decoder (FORMAT.md): per-block entropy decode (A1), command scan (A2), literal
+// placement (A3) and match resolution (A4) — SURVEY §8(a).  One warp owns one block at a time.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace acx {
+
+constexpr int PROB_BITS = 11;
+constexpr int LUT_SIZE = 1 << PROB_BITS;          // u32 entries per coded table: sym | freq << 8 | bias << 20
+constexpr int RING_BYTES = 1024;                  // per-warp ring of rANS words in shared memory (two 512 B halves)
+constexpr int MAX_W = 8;
+constexpr int MAX_RESIDENT = 8;
+
+enum : uint32_t { DF_RANS = 1, DF_OFFSET = 2, DF_LENGTH = 4, DF_TIMEOUT = 8, DF_STACK = 16 };
+
+struct DirEntry {            // FORMAT.md §1.3, 32 bytes
+    uint64_t payload_off;
+    uint32_t n_cmd, n_match, n_lit, n_words, n_ext;
+    uint16_t level, flags;
+};
+
+struct Resident { uint64_t lo, hi; const uint8_t* ptr; };
+
+struct Demand { uint64_t pos; uint64_t dst; uint32_t len; uint32_t pad; };   // dst = byte offset into Params::out2
+
+struct Params {
+    const uint8_t* archive;      // device archive
+    uint64_t archive_bytes;
+    const DirEntry* dir;         // = archive + dir_off
+    const uint32_t* luts;        // n_coded_tables x LUT_SIZE
+    uint64_t N;
+    uint32_t log2_bs, min_match, W, n_coded_tables;
+    int8_t plane_lut[MAX_W];     // coded OFF plane p -> lut index, -1 if raw
+    int8_t plane_raw[MAX_W];     // raw OFF plane p -> index among raw planes, -1 if coded
+    uint32_t n_coded_planes, n_raw_planes;
+    uint32_t lut_cmd, lut_mlen, lut_lit;
+    // work
+    uint64_t first_block, n_work;       // FULL mode: blocks [first_block, first_block + n_work)
+    uint8_t* out;                        // FULL mode: byte at absolute position p is out[p - out_pos0]
+    uint64_t out_pos0;                   // absolute position of out[0]  (window start, block aligned)
+    uint64_t clip_lo, clip_hi;           // only bytes of [clip_lo, clip_hi) are stored (unaligned range ends)
+    const Demand* demands; uint64_t n_demands; uint8_t* out2;    // SPAN mode top-level work
+    Resident res[MAX_RESIDENT];
+    // workspace
+    uint32_t* flags;                     // per block: epoch when done
+    uint32_t epoch;
+    unsigned long long* ticket;
+    uint32_t* err;
+    uint8_t* scratch; uint64_t scratch_per_warp; uint32_t max_cmds; uint32_t stack_cap;
+    uint32_t mode;                       // 0 = FULL blocks with flags, 1 = SPAN demands, 2 = literal wave, 3 = match wave
+    const uint32_t* level_list;          // mode 2/3: block ids to process (n_work entries), null = first_block + i
+};
+
+__device__ __forceinline__ uint32_t lane_id() { return threadIdx.x & 31; }
+__device__ __forceinline__ uint32_t lanemask_lt() { uint32_t m; asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m)); return m; }
+
+__device__ __forceinline__ uint32_t ld_acquire(const uint32_t* p) {
+    uint32_t v; asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory"); return v;
+}
+__device__ __forceinline__ void st_release(uint32_t* p, uint32_t v) {
+    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+// data that other SMs may have written during this kernel: read at L2, never from a stale L1 line
+__device__ __forceinline__ uint8_t ldcg8(const uint8_t* p) { return __ldcg(p); }
+__device__ __forceinline__ uint64_t ldcg64(const uint8_t* p) { return __ldcg(reinterpret_cast<const unsigned long long*>(p)); }
+
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
+    uint32_t s = (uint32_t)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+// ------------------------------------------------------------------------------------------------ rANS ----------
+// FORMAT.md §1.5.  32 states, one per lane; symbol i lives on lane i & 31.  The word stream is staged through a
+// 1 KB per-warp shared-memory ring filled with 16-byte cp.async copies (one coalesced 512 B request per half).
+struct Rans {
+    uint32_t x;              // this lane's state
+    uint32_t wp;             // words consumed so far
+    uint32_t issued;         // bytes of the word stream requested into the ring
+    uint32_t ready;          // bytes known to have landed
+    const uint8_t* words;    // global address of word 0 (16-byte aligned)
+    const uint8_t* limit;    // archive end (loads are clamped)
+    uint16_t* ring;          // shared memory, RING_BYTES
+
+    __device__ __forceinline__ void fill_half() {
+        const uint8_t* g = words + issued + 16 * lane_id();
+        uint8_t* s = reinterpret_cast<uint8_t*>(ring) + ((issued + 16 * lane_id()) & (RING_BYTES - 1));
+        if (g + 16 <= limit) cp_async16(s, g);
+        issued += 512;
+    }
+    __device__ __forceinline__ void init(const uint8_t* payload, const uint8_t* lim, uint16_t* r) {
+        ring = r; limit = lim; words = payload + 128; wp = 0; issued = 0; ready = 0;
+        x = reinterpret_cast<const uint32_t*>(payload)[lane_id()];
+        __syncwarp();        // the previous block's ring reads are done
+        fill_half(); fill_half();
+    }
+    // make sure the next 32 words are in the ring, and request the half that has been fully consumed
+    __device__ __forceinline__ void prepare() {
+        if (2 * wp + 64 > ready) { cp_async_wait_all(); __syncwarp(); ready = issued; }
+        if (issued - 2 * wp <= 512) { __syncwarp(); fill_half(); }   // every lane is past its ring reads of the last round
+    }
+    // decode one symbol on the lanes with active == true; all 32 lanes must call
+    __device__ __forceinline__ uint32_t step(const uint32_t* lut, bool active) {
+        uint32_t e = lut[x & (LUT_SIZE - 1)];
+        uint32_t nx = ((e >> 8) & 0xfff) * (x >> PROB_BITS) + (e >> 20);
+        if (active) x = nx;
+        bool need = active && x < 65536u;
+        uint32_t m = __ballot_sync(0xffffffffu, need);
+        if (need) {
+            uint32_t k = wp + __popc(m & lanemask_lt());
+            x = (x << 16) | ring[k & (RING_BYTES / 2 - 1)];
+        }
+        wp += __popc(m);
+        return e & 0xff;
+    }
+};
+
+// Decodes `count` symbols whose global symbol indices start at i0, storing them to dst[0..count) (byte stores,
+// consecutive lanes -> consecutive bytes).  Returns the number of symbols equal to 255 when COUNT_ESC.
+template <bool COUNT_ESC>
+__device__ __forceinline__ uint32_t rans_region(Rans& r, const uint32_t* lut, uint32_t i0, uint32_t count, uint8_t* dst) {
+    uint32_t esc = 0;
+    if (count == 0) return 0;
+    uint32_t i1 = i0 + count;
+    for (uint32_t base = i0 & ~31u; base < i1; base += 32) {
+        uint32_t i = base + lane_id();
+        bool active = i >= i0 && i < i1;
+        r.prepare();
+        uint32_t s = r.step(lut, active);
+        if (active) dst[i - i0] = (uint8_t)s;
+        if (COUNT_ESC) esc += __popc(__ballot_sync(0xffffffffu, active && s == 255));
+    }
+    return esc;
+}
+
+// ------------------------------------------------------------------------------------------------ copies --------
+// dst/src may have any alignment.  `period` = dst position - src position for a match (UINT64_MAX when the two
+// buffers are unrelated).  period >= 16 (incl. every non-overlapping copy): 8-byte words, two aligned loads + funnel
+// shift on the source side, byte head/tail on the destination side; never reads past src + len.  Smaller periods:
+// ascending byte-serial copy, which is the definition (FORMAT.md §2).
+// SRC_CG: the source may have been written by other SMs during this kernel -> read at L2, not from L1.
+template <bool SRC_CG>
+__device__ __forceinline__ void copy_bytes(uint8_t* dst, const uint8_t* src, uint32_t len, uint64_t period) {
+    if (len >= 24 && period >= 16) {
+        while ((reinterpret_cast<uintptr_t>(dst) & 7) != 0) { *dst++ = SRC_CG ? ldcg8(src) : *src; src++; len--; }
+        uint32_t sh = (uint32_t)(reinterpret_cast<uintptr_t>(src) & 7) * 8;
+        if (sh == 0) {
+            while (len >= 8) {
+                uint64_t v = SRC_CG ? ldcg64(src) : *reinterpret_cast<const uint64_t*>(src);
+                *reinterpret_cast<uint64_t*>(dst) = v; dst += 8; src += 8; len -= 8;
+            }
+        } else {
+            const uint8_t* sa = src - (sh >> 3);
+            uint64_t lo = SRC_CG ? ldcg64(sa) : *reinterpret_cast<const uint64_t*>(sa);
+            while (len >= 16) {   // the look-ahead word [sa+8, sa+16) stays inside [src, src+len)
+                uint64_t hi = SRC_CG ? ldcg64(sa + 8) : *reinterpret_cast<const uint64_t*>(sa + 8);
+                *reinterpret_cast<uint64_t*>(dst) = (lo >> sh) | (hi << (64 - sh));
+                lo = hi; dst += 8; sa += 8; len -= 8;
+            }
+            src = sa + (sh >> 3);
+        }
+    }
+    for (uint32_t i = 0; i < len; i++) dst[i] = SRC_CG ? ldcg8(src + i) : src[i];
+}
+
+} // namespace acx

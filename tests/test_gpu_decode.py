@@ -1,0 +1,126 @@
+"""Parity of the CUDA path (through the C ABI, include/aceapex.h) with the oracle and the original bytes."""
+import numpy as np
+import pytest
+import torch
+
+from acx_build import build
+from oracle import acx_oracle as O
+
+pytestmark = pytest.mark.gpu
+
+
+def gpu_decode(archive, levels=False):
+    from paper_2606_18900_b200.aceapex import Archive
+    ar = Archive(archive)
+    out = ar.decode_all(levels=levels)
+    ar.check()
+    res = out.cpu().numpy().copy()
+    ar.close()
+    return res
+
+
+HAND = [
+    ([[(b"hello", None)]], 5, 3, {}),
+    ([[(b"a", (0, 7))], [(b"", (7, 8))], [(b"", (15, 8))], [(b"", (23, 3))]], 27, 3, dict(min_match=3, levels=[0, 1, 2, 3])),
+    ([[(b"abc", (0, 10))]], 13, 4, {}),
+    ([[(b"wxyz", (0, 4))]], 8, 3, {}),
+    ([[(b"abcd", (0, 4))], [(b"", (2, 5)), (b"XYZ", None)]], 16, 3, dict(levels=[0, 1])),
+    ([[(b"01234567", None)], [(b"89ab", (6, 4))], [(b"", (6, 5)), (b"!!!", None)]], 24, 3, {}),
+    ([[(b"ACGTACGT", None)], [(b"", (0, 4)), (b"", (4, 4))]], 16, 3, {}),
+    ([[(b"ABCDEFGH", None)], [(b"", (0, 8))], [(b"", (8, 8))]], 24, 3, dict(levels=[0, 0, 1])),
+    ([[(b"xy", (0, 9)), (b"END", None)]], 14, 4, {}),
+]
+
+
+@pytest.mark.parametrize("case", range(len(HAND)))
+@pytest.mark.parametrize("levels", [False, True])
+def test_hand_built(case, levels):
+    blocks, N, lb, kw = HAND[case]
+    a = build(blocks, N, lb, **kw)
+    exp = O.decode(a)
+    got = gpu_decode(a, levels=levels)
+    assert got.tobytes() == exp.tobytes()
+
+
+def test_hand_built_escapes_and_planes():
+    lit = bytes((i * 7 + 3) % 251 for i in range(300))
+    blocks = [[(lit, (0, 300)), (b"", (10, 4 + 255)), (lit[:255], (1, 4 + 254)), (b"q", None)]]
+    N = 300 + 300 + 259 + 255 + 258 + 1
+    for raw in [(), (0,), (0, 1), (0, 1, 2, 3)]:
+        a = build(blocks, N, 11, raw_planes=raw)
+        assert gpu_decode(a).tobytes() == O.decode(a).tobytes()
+
+
+@pytest.mark.parametrize("levels", [False, True])
+def test_config0_fastq(fastq_4m, fastq_4m_archive, levels):
+    got = gpu_decode(fastq_4m_archive, levels=levels)
+    assert np.array_equal(got, O.decode(fastq_4m_archive))      # bit-exact vs the oracle
+    assert np.array_equal(got, fastq_4m)                         # and vs the original bytes
+
+
+def test_fasta(fasta_2m, fasta_2m_archive):
+    got = gpu_decode(fasta_2m_archive)
+    assert np.array_equal(got, fasta_2m)
+
+
+@pytest.mark.parametrize("bs", [4096, 8192, 65536, 262144, 1 << 20])
+def test_block_sizes(fastq_4m, bs):
+    from paper_2606_18900_b200 import encoder
+    x = fastq_4m[:(3 << 20) + 12345]            # ragged tail
+    a = encoder.encode(x, block_size=bs)
+    assert np.array_equal(gpu_decode(a), x)
+    assert np.array_equal(gpu_decode(a, levels=True), x)
+
+
+def test_runs_and_periods():
+    from paper_2606_18900_b200 import encoder
+    for data in (b"N" * 100000, (b"ACGTTGCA" * 7 + b"\n") * 3000, b"x" + b"\0" * 70000 + b"y", b"", b"q"):
+        x = np.frombuffer(data, dtype=np.uint8)
+        a = encoder.encode(x, block_size=4096)
+        assert gpu_decode(a).tobytes()[:len(data)] == data
+
+
+def test_repeated_calls_and_fnv(fastq_4m, fastq_4m_archive):
+    from paper_2606_18900_b200.aceapex import Archive
+    ar = Archive(fastq_4m_archive)
+    out = ar.new_output()
+    for _ in range(3):
+        out.zero_()
+        ar.decode_all(out)
+        ar.check()
+        assert ar.verify_fnv(out) == 0
+    out[12345] ^= 1
+    assert ar.verify_fnv(out) == 1
+    assert torch.equal(out.cpu()[:12345], torch.from_numpy(fastq_4m[:12345]))
+    ar.close()
+
+
+def test_open_errors(fastq_4m_archive):
+    from paper_2606_18900_b200.aceapex import AceapexError, Archive
+    bad = fastq_4m_archive.copy()
+    bad[0] = 0
+    with pytest.raises(AceapexError) as e:
+        Archive(bad)
+    assert e.value.name == "E_MAGIC"
+    with pytest.raises(AceapexError) as e:
+        Archive(fastq_4m_archive[:-4096].copy())
+    assert e.value.name == "E_TRUNCATED"
+    bad = fastq_4m_archive.copy()
+    h = O.header(fastq_4m_archive)
+    bad[h["dir_off"] + 8:h["dir_off"] + 12] = 0          # n_cmd = 0
+    with pytest.raises(AceapexError) as e:
+        Archive(bad)
+    assert e.value.name == "E_CORRUPT"
+
+
+def test_device_integrity_flag(fastq_4m_archive):
+    from paper_2606_18900_b200.aceapex import AceapexError, Archive
+    bad = fastq_4m_archive.copy()
+    h = O.header(fastq_4m_archive)
+    bad[h["payload_off"] + 200] ^= 0x55                  # inside block 0's word stream
+    ar = Archive(bad)
+    ar.decode_all()
+    with pytest.raises(AceapexError) as e:
+        ar.check()
+    assert e.value.name == "E_CORRUPT"
+    ar.close()
