@@ -1,0 +1,249 @@
+#!/usr/bin/env python
+"""bench.py — BASELINE.json metric on configs[1]: whole-file device-resident decode of the 1 GiB synthetic FASTQ
+(seed 2, 50 Mbp reference, 16 KB blocks).  A step = one aceapex_decode_all over the whole archive.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--size BYTES]
+
+Prints one JSON line.  N > 1: replicas only: every rank decodes
+its own copy of the same archive, no data-path collective; value = bytes of all ranks / max time over ranks."""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "decompressed GB/s (whole-file, range) vs HBM roofline; random-read latency ms"
+WORKLOAD = "configs[1]: 1 GiB synthetic FASTQ (seed 2, 50 Mbp reference), 16 KB blocks, whole-file decode_all"
+
+
+def make_input(size):
+    from paper_2606_18900_b200 import datagen, encoder
+    x = datagen.fastq(2, size, 50_000_000)
+    a = encoder.encode(x, block_size=16384)
+    return x, a
+
+
+class ClockSampler(threading.Thread):
+    """Samples nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md clocks line)."""
+    Q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap,power.draw"
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.rows, self.stop_flag = index, [], False
+
+    def run(self):
+        while not self.stop_flag:
+            try:
+                o = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits"],
+                                   stdout=subprocess.PIPE, text=True, timeout=5).stdout.strip()
+                self.rows.append([c.strip() for c in o.split(",")])
+            except Exception:
+                pass
+            time.sleep(0.05)
+
+    def summary(self):
+        sm = sorted(int(r[0]) for r in self.rows if r and r[0].isdigit())
+        reasons = []
+        for name, col in (("hw_slowdown", 2), ("hw_thermal_slowdown", 3), ("sw_thermal_slowdown", 4), ("sw_power_cap", 5)):
+            if any(len(r) > col and r[col] == "Active" for r in self.rows):
+                reasons.append(name)
+        mx = max([int(r[1]) for r in self.rows if len(r) > 1 and r[1].isdigit()] or [0])
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx or None, "reasons": reasons, "samples": len(sm)}
+
+
+def oracle_sample(archive, n_bytes_total, target_s=12.0):
+    """Times the oracle (as it stands, one thread) on a bounded prefix of the same archive."""
+    from oracle import acx_oracle
+    import numpy as np
+    h = acx_oracle.header(archive)
+    bs = 1 << h["log2_bs"]
+    probe = min(h["n_blocks"], max(1, (32 << 20) // bs))
+    out = np.zeros(min(h["N"], h["n_blocks"] * bs) + 1, dtype=np.uint8)   # pre-faulted output
+    t = time.perf_counter()
+    acx_oracle.decode_prefix(archive, probe, out=out)
+    dt = time.perf_counter() - t
+    rate = probe * bs / dt
+    nblk = int(min(h["n_blocks"], max(probe, target_s * rate // bs)))
+    t = time.perf_counter()
+    got = acx_oracle.decode_prefix(archive, nblk, out=out)
+    dt = time.perf_counter() - t
+    return got, dt, "first %d of %d blocks (%.0f MiB of %.0f MiB) of the same archive, 1 thread" % (
+        nblk, h["n_blocks"], got.size / 2**20, n_bytes_total / 2**20)
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import numpy as np
+    x, a = make_input(args.size)
+    times, nbytes, sample = [], 0, ""
+    for i in range(args.warmup + args.steps):
+        got, dt, sample = oracle_sample(a, x.size, target_s=max(2.0, min(12.0, 150.0 / (args.warmup + args.steps))))
+        assert np.array_equal(got, x[:got.size])
+        if i >= args.warmup:
+            times.append(dt)
+            nbytes = got.size
+    ms = 1e3 * sum(times) / len(times)
+    v = nbytes / (ms * 1e-3) / 1e9
+    line = {"metric": METRIC, "value": v, "unit": "GB/s", "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8",
+            "data": "synthetic", "impl": "reference", "config": {"workload": WORKLOAD, "size_bytes": int(x.size)},
+            "cpu_baseline": {"value": v, "unit": "GB/s", "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": v, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_2606_18900_b200.aceapex import Archive
+    x, a = make_input(args.size)
+    ar = Archive(a, device="cuda:%d" % local)
+    info = ar.info()
+    out = ar.new_output()
+    stream = torch.cuda.current_stream()
+    ar.set_stream(stream)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident metric: archive and output in HBM, K steps between two events
+    for _ in range(args.warmup):
+        ar.decode_all(out)
+    ar.check()
+    sampler = ClockSampler(local)
+    sampler.start()
+    barrier()
+    l0 = ar.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    per_step = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    e0.record(stream)
+    for a_ev, b_ev in per_step:
+        a_ev.record(stream)
+        ar.decode_all(out)
+        b_ev.record(stream)
+    e1.record(stream)
+    barrier()
+    launches = ar.launch_count() - l0
+    total_ms = e0.elapsed_time(e1)
+    kernel_ms = sum(p.elapsed_time(q) for p, q in per_step) / args.steps
+    sampler.stop_flag = True
+    sampler.join()
+    ar.check()
+    ok = bool(torch.equal(out[:x.size].cpu(), torch.from_numpy(x)))
+    fnv_bad = ar.verify_fnv(out) if info["has_fnv"] else 0
+    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms = float(t.item())
+    ms = total_ms / args.steps
+    value = world * x.size / (ms * 1e-3) / 1e9
+
+    # ---- the same decode scheduled level by level (literal wave + one match launch per level), for comparison
+    ar.decode_all(out, levels=True)
+    l0 = ar.launch_count()
+    p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    p0.record(stream)
+    for _ in range(3):
+        ar.decode_all(out, levels=True)
+    p1.record(stream)
+    torch.cuda.synchronize()
+    lv_ms = p0.elapsed_time(p1) / 3
+    ar.check()
+    ok = ok and bool(torch.equal(out[:x.size].cpu(), torch.from_numpy(x)))
+    levels_info = {"ms_per_step": lv_ms, "value": x.size / (lv_ms * 1e-3) / 1e9, "unit": "GB/s",
+                   "launches_per_step": (ar.launch_count() - l0) // 3}
+
+    # ---- end to end through the C ABI with HOST buffers (pinned): H2D archive + decode + D2H output per step
+    h_arch = torch.from_numpy(a).pin_memory()
+    h_out = torch.empty(x.size, dtype=torch.uint8).pin_memory()
+    for _ in range(2):
+        ar.decode_all_host(h_arch, out, h_out)
+    barrier()
+    n_e2e = max(2, min(args.steps, 5))
+    t0 = time.perf_counter()
+    for _ in range(n_e2e):
+        ar.decode_all_host(h_arch, out, h_out)
+    torch.cuda.synchronize()
+    e2e_s = (time.perf_counter() - t0) / n_e2e
+    t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_s = float(t.item())
+    ok = ok and bool(torch.equal(h_out, torch.from_numpy(x)))
+    e2e = {"value": world * x.size / e2e_s / 1e9, "unit": "GB/s", "h2d_bytes_per_step": int(a.size), "d2h_bytes_per_step": int(x.size)}
+
+    if rank != 0:
+        return
+    # ---- roofline of the dominant (only) kernel: algorithmic bytes C + M + N per launch / measured launch time
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    peak = float(peaks.get("hbm_gbs", 6650.0))
+    alg_bytes = info["archive_bytes"] + info["total_match_bytes"] + info["raw_bytes"]
+    achieved = alg_bytes / (kernel_ms * 1e-3) / 1e9
+    traffic = None
+    try:
+        traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get("k_decode_bytes_per_launch")
+    except Exception:
+        pass
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
+                "peak_source": "MEASURED_PEAKS.json hbm_gbs (measured)" if peaks else "fallback 6650 GB/s",
+                "kernel": "k_decode", "kernel_ms": kernel_ms,
+                "algorithmic_bytes": {"C": info["archive_bytes"], "M": info["total_match_bytes"], "N": info["raw_bytes"]}}
+    cpu = None
+    if args.cpu_baseline:
+        got, dt, sample = oracle_sample(a, x.size)
+        assert np.array_equal(got, x[:got.size])
+        cpu = {"value": got.size / dt / 1e9, "unit": "GB/s", "cores": 1, "kind": "oracle", "sample": sample}
+    line = {"metric": METRIC, "value": value, "unit": "GB/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8",
+            "data": "synthetic",
+            "config": {"workload": WORKLOAD, "size_bytes": int(x.size), "archive_bytes": int(a.size),
+                       "ratio": x.size / a.size, "n_blocks": info["n_blocks"], "max_level": info["max_level"],
+                       "l2": "output (1 GiB) and archive are larger than the 126 MB L2; no flush needed",
+                       "parallelism": "replicas only" if world > 1 else "1 GPU", "resident_warps": info["resident_warps"]},
+            "bit_exact": ok and fnv_bad == 0, "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": int(launches),
+            "roofline": roofline, "cpu_baseline": cpu, "level_schedule": levels_info}
+    print(json.dumps(line))
+    if not (ok and fnv_bad == 0):
+        sys.exit(1)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--size", type=int, default=1 << 30, help="bytes of FASTQ (default: configs[1], 1 GiB)")
+    ap.add_argument("--no-cpu-baseline", dest="cpu_baseline", action="store_false")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

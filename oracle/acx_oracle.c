@@ -255,14 +255,23 @@ int acx_oracle_header(const uint8_t* a, uint64_t n, uint64_t* f) {
     return OK;
 }
 
-/* Whole-archive decode, blocks in index order.  check_levels != 0 also verifies FORMAT.md §3 and the optional FNV
- * section.  out must hold N bytes. */
+/* Decode of blocks [0, n_prefix_blocks) in index order (n_prefix_blocks = 0 or >= n_blocks: the whole archive; a
+ * prefix is self-sufficient because every source precedes its destination).  check_levels != 0 also verifies
+ * FORMAT.md §3 and the optional FNV section.  out must hold min(N, n_prefix_blocks * BS) bytes. */
+int acx_oracle_decode_prefix(const uint8_t* a, uint64_t n, uint8_t* out, uint64_t out_cap, int check_levels, uint64_t n_prefix_blocks);
+
 int acx_oracle_decode(const uint8_t* a, uint64_t n, uint8_t* out, uint64_t out_cap, int check_levels) {
+    return acx_oracle_decode_prefix(a, n, out, out_cap, check_levels, 0);
+}
+
+int acx_oracle_decode_prefix(const uint8_t* a, uint64_t n, uint8_t* out, uint64_t out_cap, int check_levels, uint64_t n_prefix_blocks) {
     hdr_t h; table_t T[11]; scratch_t s; dir_t d;
     memset(&s, 0, sizeof s);
     int rc = parse_header(a, n, &h);
     if (rc) return rc;
-    if (out_cap < h.N) return E_RANGE;
+    uint64_t nb = (n_prefix_blocks == 0 || n_prefix_blocks > h.n_blocks) ? h.n_blocks : n_prefix_blocks;
+    uint64_t need_out = (nb << h.log2_bs) < h.N ? (nb << h.log2_bs) : h.N;
+    if (out_cap < need_out) return E_RANGE;
     if ((rc = parse_tables(a, &h, T))) return rc;
     uint8_t* matchmap = NULL; uint16_t* levels = NULL;
     if (check_levels) {
@@ -270,7 +279,7 @@ int acx_oracle_decode(const uint8_t* a, uint64_t n, uint8_t* out, uint64_t out_c
         if (!matchmap || !levels) { free(matchmap); free(levels); return E_NOMEM; }
     }
     uint64_t sums[4] = {0, 0, 0, 0}; uint32_t max_level = 0, max_cmds = 0;
-    for (uint64_t b = 0; b < h.n_blocks && !rc; b++) {
+    for (uint64_t b = 0; b < nb && !rc; b++) {
         uint64_t pend;
         if ((rc = read_dir(a, &h, b, &d, &pend))) break;
         if ((rc = decode_streams(a, &h, T, &d, pend, &s))) break;
@@ -286,7 +295,7 @@ int acx_oracle_decode(const uint8_t* a, uint64_t n, uint8_t* out, uint64_t out_c
             if (f != rd64(a + h.fnv_off + 8 * b)) rc = E_CORRUPT;
         }
     }
-    if (!rc && (sums[0] != h.total_lit || sums[1] != h.total_matches || sums[2] != h.total_cmds || sums[3] != h.total_match_bytes ||
+    if (!rc && nb == h.n_blocks && (sums[0] != h.total_lit || sums[1] != h.total_matches || sums[2] != h.total_cmds || sums[3] != h.total_match_bytes ||
                 max_level != h.max_level || max_cmds != h.max_cmds)) rc = E_CORRUPT;
     free(matchmap); free(levels); release(&s);
     return rc;

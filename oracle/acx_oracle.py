@@ -40,6 +40,7 @@ def _load():
         p, u64 = ctypes.c_void_p, ctypes.c_uint64
         _lib.acx_oracle_header.argtypes = [p, u64, p]
         _lib.acx_oracle_decode.argtypes = [p, u64, p, u64, ctypes.c_int]
+        _lib.acx_oracle_decode_prefix.argtypes = [p, u64, p, u64, ctypes.c_int, u64]
         _lib.acx_oracle_block.argtypes = [p, u64, u64] + [p] * 9
         _lib.acx_oracle_rans.argtypes = [p, ctypes.c_uint32, ctypes.c_uint32, p, u64, p, p, u64, p, p]
         _lib.acx_oracle_fnv1a64.argtypes = [p, u64]
@@ -67,6 +68,18 @@ def decode(archive, check_levels=True):
     n = header(a)["N"]
     out = np.zeros(max(n, 1), dtype=np.uint8)
     rc = _load().acx_oracle_decode(a.ctypes.data, a.size, out.ctypes.data, n, 1 if check_levels else 0)
+    if rc:
+        raise OracleError(rc)
+    return out[:n]
+
+
+def decode_prefix(archive, n_blocks, check_levels=False, out=None):
+    """The first n_blocks blocks (a prefix is self-sufficient: sources precede destinations)."""
+    a = _arr(archive)
+    h = header(a)
+    n = min(h["N"], n_blocks << h["log2_bs"])
+    out = np.zeros(max(n, 1), dtype=np.uint8) if out is None else out
+    rc = _load().acx_oracle_decode_prefix(a.ctypes.data, a.size, out.ctypes.data, n, 1 if check_levels else 0, n_blocks)
     if rc:
         raise OracleError(rc)
     return out[:n]

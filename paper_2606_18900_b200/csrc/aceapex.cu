@@ -88,10 +88,12 @@ __device__ __forceinline__ uint64_t match_src(const Params& P, const BlockCtx& c
     return src;
 }
 
-__device__ __forceinline__ void wait_block(const Params& P, uint64_t S) {
+// flag[S] = 2 * epoch once block S has placed its literal bytes, 2 * epoch + 1 once it is complete
+__device__ __forceinline__ void wait_block(const Params& P, uint64_t S, bool need_full) {
     const uint32_t* f = P.flags + S;
+    const uint32_t want = 2 * P.epoch + (need_full ? 1u : 0u);
     uint32_t spins = 0;
-    while (ld_acquire(f) != P.epoch) {
+    while (ld_flag(f) < want) {
         __nanosleep(64);
         if (++spins > (1u << 24)) { report(P, DF_TIMEOUT); break; }
     }
@@ -99,18 +101,21 @@ __device__ __forceinline__ void wait_block(const Params& P, uint64_t S) {
 
 // Copy one match whose seed lies in the current FULL window.  WAIT: the flag-driven schedule waits for the source
 // blocks (other than the own block); the level schedule needs no wait (sources were completed by earlier launches).
+// By FORMAT.md §3 a source block S with level(S) >= level(B) can only contribute literal bytes, so B waits for S's
+// literal phase only; S with level(S) < level(B) may contribute match bytes, so B waits for S to complete.  Waits for
+// completion therefore go to strictly lower levels and chain at most max_level deep, whatever the distance.
 template <bool WAIT>
 __device__ __forceinline__ void copy_match_window(const Params& P, const BlockCtx& c, uint64_t dst, uint64_t src, uint32_t len) {
     if (WAIT) {
         uint64_t seed_end = min((unsigned long long)(src + len), (unsigned long long)dst);
         uint64_t s0 = src >> P.log2_bs, s1 = (seed_end - 1) >> P.log2_bs;
-        for (uint64_t S = s0; S <= s1; S++) if (S != c.b) wait_block(P, S);
+        for (uint64_t S = s0; S <= s1; S++) if (S != c.b) wait_block(P, S, __ldg(P.levels + S) < c.d.level);
     }
     copy_bytes<true>(P.out + (dst - P.out_pos0), P.out + (src - P.out_pos0), len, dst - src);
 }
 
 // A2 + A3 + A4 for a whole block: scan the commands 32 at a time, place literal runs, then resolve the matches.
-// MODE 0: everything (flag-driven schedule); MODE 2: literals only; MODE 3: matches only.
+// MODE 2: literals only; MODE 0: matches only, waiting on source-block flags; MODE 3: matches only, no waits.
 template <int MODE>
 __device__ __forceinline__ void emit_block(const Params& P, const BlockCtx& c) {
     uint32_t lit_base = 0, out_base = 0, ec = 0, em = c.n_ext_cmd;
@@ -137,9 +142,8 @@ __device__ __forceinline__ void emit_block(const Params& P, const BlockCtx& c) {
         out_base += __shfl_sync(0xffffffffu, st, 31);
         bool ok = valid && (uint64_t)lit_pos + lit_len <= c.d.n_lit && out_pos + lit_len + match_len <= c.bend;
         if (__any_sync(0xffffffffu, valid && !ok)) { if (lane == 0) report(P, DF_LENGTH); return; }
-        if (MODE != 3 && ok && lit_len) copy_bytes<false>(P.out + (out_pos - P.out_pos0), c.lit + lit_pos, lit_len, ~0ull);
+        if (MODE == 2 && ok && lit_len) copy_bytes<false>(P.out + (out_pos - P.out_pos0), c.lit + lit_pos, lit_len, ~0ull);
         if (MODE == 2) continue;
-        __syncwarp();
         if (ok && has_match) {
             uint64_t dst = out_pos + lit_len, src = match_src(P, c, ci);
             if (src >= dst) report(P, DF_OFFSET);
@@ -172,12 +176,16 @@ __global__ void __launch_bounds__(256) k_decode(const Params P) {
             continue;
         }
         bool ok = parse_block(P, s_luts, ring, c, 0xffffffffu);
+        if (ok) emit_block<2>(P, c);                                  // A3: all literal bytes of the block
         if (P.mode == 0) {
-            if (ok) emit_block<0>(P, c);
             __threadfence();
             __syncwarp();
-            if (lane_id() == 0) st_release(P.flags + c.b, P.epoch);   // set even on error so that nobody waits forever
-        } else if (ok) emit_block<2>(P, c);
+            if (lane_id() == 0) st_release(P.flags + c.b, 2 * P.epoch);       // literals placed
+            if (ok) emit_block<0>(P, c);                              // A4: matches (waits on source blocks)
+            __threadfence();
+            __syncwarp();
+            if (lane_id() == 0) st_release(P.flags + c.b, 2 * P.epoch + 1);   // complete (set even on error: nobody waits forever)
+        }
     }
 }
 
@@ -209,6 +217,7 @@ struct aceapex_archive {
     // device state owned by the library
     uint32_t* d_luts = nullptr;
     uint32_t* d_level_lists = nullptr;                  // concatenated level_blocks
+    uint16_t* d_levels = nullptr;                       // level per block (compact copy of the directory field)
     std::vector<uint64_t> level_off;
     // workspace (caller's)
     uint8_t* d_ws = nullptr; uint64_t ws_bytes = 0; bool ws_clean = false;
@@ -242,7 +251,7 @@ void fill_params(const aceapex_archive* ar, Params& P) {
     memset(&P, 0, sizeof P);
     P.archive = ar->d_archive; P.archive_bytes = ar->archive_bytes;
     P.dir = reinterpret_cast<const DirEntry*>(ar->d_archive + ar->dir_off);
-    P.luts = ar->d_luts; P.N = ar->N; P.log2_bs = ar->log2_bs; P.min_match = ar->min_match; P.W = ar->W;
+    P.luts = ar->d_luts; P.levels = ar->d_levels; P.N = ar->N; P.log2_bs = ar->log2_bs; P.min_match = ar->min_match; P.W = ar->W;
     P.n_coded_tables = ar->n_coded_tables;
     memcpy(P.plane_lut, ar->plane_lut, MAX_W); memcpy(P.plane_raw, ar->plane_raw, MAX_W);
     P.n_coded_planes = ar->n_coded_planes; P.n_raw_planes = ar->n_raw_planes;
@@ -367,6 +376,12 @@ int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* 
         CU(cudaMalloc(&ar->d_luts, luts.size() * 4));
         CU(cudaMemcpy(ar->d_luts, luts.data(), luts.size() * 4, cudaMemcpyHostToDevice));
     }
+    if (ar->n_blocks) {
+        std::vector<uint16_t> lv(ar->n_blocks);
+        for (uint64_t b = 0; b < ar->n_blocks; b++) lv[b] = rd16(meta + ar->dir_off + 32 * b + 28);
+        CU(cudaMalloc(&ar->d_levels, lv.size() * 2));
+        CU(cudaMemcpy(ar->d_levels, lv.data(), lv.size() * 2, cudaMemcpyHostToDevice));
+    }
     if (ar->n_blocks && ar->n_blocks < (1ull << 32)) {
         std::vector<uint32_t> cat;
         for (auto& v : ar->level_blocks) { ar->level_off.push_back(cat.size()); cat.insert(cat.end(), v.begin(), v.end()); }
@@ -400,6 +415,7 @@ int32_t aceapex_close(aceapex_archive* ar) {
     cudaDeviceSynchronize();
     if (ar->d_luts) cudaFree(ar->d_luts);
     if (ar->d_level_lists) cudaFree(ar->d_level_lists);
+    if (ar->d_levels) cudaFree(ar->d_levels);
     delete ar;
     return ACEAPEX_OK;
 }

@@ -29,6 +29,7 @@ struct Params {
     uint64_t archive_bytes;
     const DirEntry* dir;         // = archive + dir_off
     const uint32_t* luts;        // n_coded_tables x LUT_SIZE
+    const uint16_t* levels;      // level per block
     uint64_t N;
     uint32_t log2_bs, min_match, W, n_coded_tables;
     int8_t plane_lut[MAX_W];     // coded OFF plane p -> lut index, -1 if raw
@@ -43,7 +44,7 @@ struct Params {
     const Demand* demands; uint64_t n_demands; uint8_t* out2;    // SPAN mode top-level work
     Resident res[MAX_RESIDENT];
     // workspace
-    uint32_t* flags;                     // per block: epoch when done
+    uint32_t* flags;                     // per block: 2 * epoch = literals placed, 2 * epoch + 1 = complete
     uint32_t epoch;
     unsigned long long* ticket;
     uint32_t* err;
@@ -55,8 +56,11 @@ struct Params {
 __device__ __forceinline__ uint32_t lane_id() { return threadIdx.x & 31; }
 __device__ __forceinline__ uint32_t lanemask_lt() { uint32_t m; asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m)); return m; }
 
-__device__ __forceinline__ uint32_t ld_acquire(const uint32_t* p) {
-    uint32_t v; asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory"); return v;
+// Flag poll.  Relaxed on purpose: an acquire load makes ptxas invalidate the whole L1 (CCTL.IVALL) on every poll.
+// The data guarded by a flag is only ever read with ld.cg (L2, the coherence point) and the reads are issued after
+// the poll has returned (control dependency), so no L1 invalidation is needed.
+__device__ __forceinline__ uint32_t ld_flag(const uint32_t* p) {
+    uint32_t v; asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory"); return v;
 }
 __device__ __forceinline__ void st_release(uint32_t* p, uint32_t v) {
     asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
@@ -135,33 +139,84 @@ __device__ __forceinline__ uint32_t rans_region(Rans& r, const uint32_t* lut, ui
 }
 
 // ------------------------------------------------------------------------------------------------ copies --------
+// SRC_CG: the source may have been written by other SMs during this kernel -> read at L2 (ld.cg), never from L1.
+template <bool SRC_CG> __device__ __forceinline__ uint64_t ld64a(const uint8_t* p) {   // p is 8-byte aligned
+    return SRC_CG ? ldcg64(p) : *reinterpret_cast<const uint64_t*>(p);
+}
+// 8 bytes starting at any address: the aligned word(s) that hold them (never touches a word without a wanted byte
+// when n_valid bytes are wanted)
+template <bool SRC_CG> __device__ __forceinline__ uint64_t ld64u(const uint8_t* p, uint32_t n_valid) {
+    uint32_t sh = (uint32_t)(reinterpret_cast<uintptr_t>(p) & 7);
+    const uint8_t* a = p - sh;
+    uint64_t lo = ld64a<SRC_CG>(a);
+    if (sh == 0) return lo;
+    uint64_t hi = (sh + n_valid > 8) ? ld64a<SRC_CG>(a + 8) : 0;
+    return (lo >> (8 * sh)) | (hi << (64 - 8 * sh));
+}
+// store the low n (<= 8) bytes of v at any address, using the widest naturally aligned stores
+__device__ __forceinline__ void st_small(uint8_t* d, uint64_t v, uint32_t n) {
+    if (n >= 8 && (reinterpret_cast<uintptr_t>(d) & 7) == 0) { *reinterpret_cast<uint64_t*>(d) = v; return; }
+    if (n && (reinterpret_cast<uintptr_t>(d) & 1)) { *d = (uint8_t)v; v >>= 8; d++; n--; }
+    if (n >= 2 && (reinterpret_cast<uintptr_t>(d) & 2)) { *reinterpret_cast<uint16_t*>(d) = (uint16_t)v; v >>= 16; d += 2; n -= 2; }
+    if (n >= 4) { *reinterpret_cast<uint32_t*>(d) = (uint32_t)v; v >>= 32; d += 4; n -= 4; }   // d is 4-aligned here or n < 2
+    if (n >= 4) { *reinterpret_cast<uint32_t*>(d) = (uint32_t)v; d += 4; n -= 4; v = 0; }
+    if (n >= 2) { *reinterpret_cast<uint16_t*>(d) = (uint16_t)v; v >>= 16; d += 2; n -= 2; }
+    if (n) *d = (uint8_t)v;
+}
+
 // dst/src may have any alignment.  `period` = dst position - src position for a match (UINT64_MAX when the two
-// buffers are unrelated).  period >= 16 (incl. every non-overlapping copy): 8-byte words, two aligned loads + funnel
-// shift on the source side, byte head/tail on the destination side; never reads past src + len.  Smaller periods:
-// ascending byte-serial copy, which is the definition (FORMAT.md §2).
-// SRC_CG: the source may have been written by other SMs during this kernel -> read at L2, not from L1.
+// buffers are unrelated).  period >= len (non-overlapping): loads are issued ahead of the stores that depend on
+// them, 8 bytes at a time.  Self-overlap: ascending 8-byte steps when period >= 8, else the byte-serial copy that
+// is the definition (FORMAT.md §2).
 template <bool SRC_CG>
 __device__ __forceinline__ void copy_bytes(uint8_t* dst, const uint8_t* src, uint32_t len, uint64_t period) {
-    if (len >= 24 && period >= 16) {
-        while ((reinterpret_cast<uintptr_t>(dst) & 7) != 0) { *dst++ = SRC_CG ? ldcg8(src) : *src; src++; len--; }
-        uint32_t sh = (uint32_t)(reinterpret_cast<uintptr_t>(src) & 7) * 8;
-        if (sh == 0) {
-            while (len >= 8) {
-                uint64_t v = SRC_CG ? ldcg64(src) : *reinterpret_cast<const uint64_t*>(src);
-                *reinterpret_cast<uint64_t*>(dst) = v; dst += 8; src += 8; len -= 8;
-            }
-        } else {
-            const uint8_t* sa = src - (sh >> 3);
-            uint64_t lo = SRC_CG ? ldcg64(sa) : *reinterpret_cast<const uint64_t*>(sa);
-            while (len >= 16) {   // the look-ahead word [sa+8, sa+16) stays inside [src, src+len)
-                uint64_t hi = SRC_CG ? ldcg64(sa + 8) : *reinterpret_cast<const uint64_t*>(sa + 8);
-                *reinterpret_cast<uint64_t*>(dst) = (lo >> sh) | (hi << (64 - sh));
-                lo = hi; dst += 8; sa += 8; len -= 8;
-            }
-            src = sa + (sh >> 3);
+    if (period < len) {   // self-overlapping match (src + len > dst): ascending order matters
+        if (period < 8) { for (uint32_t i = 0; i < len; i++) dst[i] = SRC_CG ? ldcg8(src + i) : src[i]; return; }
+        for (uint32_t i = 0; i < len; i += 8) {   // bytes [src+i, src+i+8) lie below dst+i: already written
+            uint32_t n = len - i < 8 ? len - i : 8;
+            st_small(dst + i, ld64u<SRC_CG>(src + i, n), n);
+        }
+        return;
+    }
+    if (len <= 16) {
+        uint64_t lo = ld64u<SRC_CG>(src, len < 8 ? len : 8);
+        uint64_t hi = len > 8 ? ld64u<SRC_CG>(src + 8, len - 8) : 0;
+        st_small(dst, lo, len < 8 ? len : 8);
+        if (len > 8) st_small(dst + 8, hi, len - 8);
+        return;
+    }
+    // head: bring dst to 8-byte alignment; tail: the last (< 8) bytes.  Both are loaded before any store.
+    uint32_t head = (uint32_t)(-reinterpret_cast<intptr_t>(dst)) & 7;
+    uint64_t hv = head ? ld64u<SRC_CG>(src, head) : 0;
+    uint32_t body = (len - head) & ~7u, tail = len - head - body;
+    uint64_t tv = tail ? ld64u<SRC_CG>(src + head + body, tail) : 0;
+    const uint8_t* s = src + head;
+    uint8_t* d = dst + head;
+    uint32_t sh = (uint32_t)(reinterpret_cast<uintptr_t>(s) & 7) * 8;
+    if (sh == 0) {
+        uint32_t i = 0;
+        for (; i + 16 <= body; i += 16) {
+            uint64_t a = ld64a<SRC_CG>(s + i), b = ld64a<SRC_CG>(s + i + 8);
+            *reinterpret_cast<uint64_t*>(d + i) = a; *reinterpret_cast<uint64_t*>(d + i + 8) = b;
+        }
+        if (i < body) *reinterpret_cast<uint64_t*>(d + i) = ld64a<SRC_CG>(s + i);
+    } else {
+        const uint8_t* sa = s - (sh >> 3);
+        uint64_t lo = ld64a<SRC_CG>(sa);
+        uint32_t i = 0;
+        for (; i + 16 <= body; i += 16) {   // words sa+8 .. sa+16 hold wanted bytes: i + 16 <= body <= len - head
+            uint64_t m = ld64a<SRC_CG>(sa + i + 8), h2 = ld64a<SRC_CG>(sa + i + 16);
+            *reinterpret_cast<uint64_t*>(d + i) = (lo >> sh) | (m << (64 - sh));
+            *reinterpret_cast<uint64_t*>(d + i + 8) = (m >> sh) | (h2 << (64 - sh));
+            lo = h2;
+        }
+        if (i < body) {
+            uint64_t m = ld64a<SRC_CG>(sa + i + 8);
+            *reinterpret_cast<uint64_t*>(d + i) = (lo >> sh) | (m << (64 - sh));
         }
     }
-    for (uint32_t i = 0; i < len; i++) dst[i] = SRC_CG ? ldcg8(src + i) : src[i];
+    if (head) st_small(dst, hv, head);
+    if (tail) st_small(d + body, tv, tail);
 }
 
 } // namespace acx

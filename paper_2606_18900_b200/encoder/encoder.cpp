@@ -39,7 +39,11 @@ struct Block {
 inline uint64_t ld64(const uint8_t* p) { uint64_t v; memcpy(&v, p, 8); return v; }
 inline uint32_t ld32(const uint8_t* p) { uint32_t v; memcpy(&v, p, 4); return v; }
 inline uint32_t hash4(uint32_t v, int bits) { return (v * 2654435761u) >> (32 - bits); }
-inline uint64_t hash8(uint64_t v, int bits) { return (v * 0x9E3779B97F4A7C15ull) >> (64 - bits); }
+constexpr uint64_t GKEY = 16;   // bytes of the global-table key: long enough to be near-unique in DNA (4^16 keys)
+inline uint64_t hash16(const uint8_t* p, int bits) {
+    uint64_t a = ld64(p) * 0x9E3779B97F4A7C15ull, b = ld64(p + 8) * 0xC2B2AE3D27D4EB4Full;
+    return ((a ^ (b >> 29) ^ (b << 35)) * 0x9E3779B97F4A7C15ull) >> (64 - bits);
+}
 
 struct Enc {
     const uint8_t* x; uint64_t N; Opts o;
@@ -47,7 +51,7 @@ struct Enc {
     std::vector<uint64_t> litmap;            // bit = 1: literal byte
     std::vector<uint16_t> level;
     std::vector<Block> blocks;
-    std::vector<std::atomic<uint64_t>> gtab; // first occurrence of an 8-byte key, positions of earlier batches only
+    std::vector<std::atomic<uint64_t>> gtab; // first occurrence of a GKEY-byte key, positions of earlier batches only
     int gbits;
     uint32_t cost[256];                      // literal cost in 1/16 bit
     uint32_t match_cost;
@@ -76,6 +80,7 @@ struct Enc {
     // Longest valid match of source p for destination i (dst limited to bend); returns false if unusable.
     bool evaluate(uint64_t p, uint64_t i, uint64_t bstart, uint64_t bend, uint64_t cs, uint64_t batch_start, Cand& c) const {
         if (p >= i) return false;
+        if (i + 4 <= N && ld32(x + p) != ld32(x + i)) return false;   // hash collision
         if (o.src_window && i - p > o.src_window) return false;
         uint64_t maxlen = bend - i, l = 0;
         // sources may only touch [0, batch_start) and [cs, i): other chunks of this batch are being parsed concurrently
@@ -104,6 +109,7 @@ struct Enc {
         if (l < o.min_match) return false;
         int64_t g = -(int64_t)match_cost;
         for (uint64_t k = 0; k < l; k++) g += cost[x[i + k]];
+        g -= (int64_t)lvl * 8 * 16;   // prefer shallow sources: 8 bits per level
         c.p = p; c.len = (uint32_t)l; c.lvl = lvl; c.gain = g;
         return true;
     }
@@ -134,8 +140,8 @@ struct Enc {
                     if (c.gain <= 0) return;
                     if (!have || c.gain > best.gain || (c.gain == best.gain && (c.lvl < best.lvl || (c.lvl == best.lvl && c.p < best.p)))) { best = c; have = true; }
                 };
-                if (i + 8 <= N && batch_start > 0) {
-                    uint64_t p = gtab[hash8(ld64(x + i), gbits)].load(std::memory_order_relaxed);
+                if (i + GKEY <= N && batch_start > 0) {
+                    uint64_t p = gtab[hash16(x + i, gbits)].load(std::memory_order_relaxed);
                     if (p != ~0ull && p < batch_start) consider(p);
                 }
                 if (i + 4 <= N) {
@@ -144,7 +150,11 @@ struct Enc {
                     uint32_t r = head[h];
                     for (uint32_t d = 0; d < o.chain_depth && r != 0xffffffffu; d++) { consider(cs + r); r = prev[r]; }
                 }
-                if (!have) { insert(i); i++; continue; }
+                if (!have) { // no match: step faster through incompressible stretches (back-extension recovers match starts)
+                    uint64_t step = 1 + (std::min<uint64_t>(i - lit_start, 1024) >> 6);
+                    for (uint64_t k = 0; k < step && i < bend; k++) { insert(i); i++; }
+                    continue;
+                }
                 // extend backwards over pending literals while the source byte is a literal byte
                 uint64_t p = best.p, len = best.len;
                 while (i > lit_start && p > 0 && x[i - 1] == x[p - 1] && (p - 1 >= cs || p - 1 < batch_start) && is_lit(p - 1)) {
@@ -167,10 +177,11 @@ struct Enc {
         }
     }
 
-    void insert_global(uint64_t a, uint64_t b) { // positions [a, b) whose 8-byte key is made of literal bytes only
-        for (uint64_t p = a; p < b && p + 8 <= N; p++) {
-            if (first_nonlit(p, p + 8) != p + 8) continue;
-            std::atomic<uint64_t>& s = gtab[hash8(ld64(x + p), gbits)];
+    void insert_global(uint64_t a, uint64_t b) { // positions [a, b) whose key is made of literal bytes only
+        for (uint64_t p = a; p < b && p + GKEY <= N; p++) {
+            uint64_t q = first_nonlit(p, p + GKEY);
+            if (q != p + GKEY) { p = q; continue; }   // no key starting in [p, q] is all-literal
+            std::atomic<uint64_t>& s = gtab[hash16(x + p, gbits)];
             uint64_t cur = s.load(std::memory_order_relaxed);
             while (p < cur && !s.compare_exchange_weak(cur, p, std::memory_order_relaxed)) {}
         }
@@ -250,7 +261,7 @@ struct acx_enc_opts {
 void acx_enc_default_opts(acx_enc_opts* o) {
     memset(o, 0, sizeof *o);
     o->log2_bs = 14; o->min_match = 4; o->max_level = 3; o->threads = 0; o->src_window = 0;
-    o->chunk_log2 = 22; o->batch_chunks = 16; o->chain_depth = 8; o->hash_log2 = 0; o->with_fnv = 1;
+    o->chunk_log2 = 22; o->batch_chunks = 16; o->chain_depth = 2; o->hash_log2 = 0; o->with_fnv = 1;
 }
 
 void acx_enc_free(void* p) { free(p); }
