@@ -39,7 +39,7 @@ __device__ __forceinline__ void bind_scratch(const Params& P, uint32_t warp_glob
 }
 
 // A1: entropy-decode the block's streams into the warp's scratch.  lit_limit: number of literal symbols wanted.
-__device__ __forceinline__ bool parse_block(const Params& P, const uint32_t* s_luts, uint16_t* ring, BlockCtx& c, uint32_t lit_limit) {
+__device__ __forceinline__ bool parse_block(const Params& P, uint32_t s_luts, uint32_t ring, BlockCtx& c, uint32_t lit_limit) {
     const DirEntry* dp = P.dir + c.b;
     const uint4* d4 = reinterpret_cast<const uint4*>(dp);
     uint4 a = __ldg(d4), q = __ldg(d4 + 1);
@@ -57,18 +57,18 @@ __device__ __forceinline__ bool parse_block(const Params& P, const uint32_t* s_l
     Rans r;
     r.init(c.payload, P.archive + P.archive_bytes, ring);
     uint32_t i0 = 0;
-    c.n_ext_cmd = rans_region<true>(r, s_luts + P.lut_cmd * LUT_SIZE, i0, c.d.n_cmd, c.tok_cmd); i0 += c.d.n_cmd;
-    rans_region<false>(r, s_luts + P.lut_mlen * LUT_SIZE, i0, c.d.n_match, c.tok_mlen); i0 += c.d.n_match;
+    c.n_ext_cmd = rans_region<true>(r, s_luts + P.lut_cmd * (4 * LUT_SIZE), i0, c.d.n_cmd, c.tok_cmd); i0 += c.d.n_cmd;
+    rans_region<false>(r, s_luts + P.lut_mlen * (4 * LUT_SIZE), i0, c.d.n_match, c.tok_mlen); i0 += c.d.n_match;
     for (int p = (int)P.W - 1; p >= 0; p--) {
         int li = P.plane_lut[p];
         if (li < 0) continue;
         // coded planes are stored in decode order: slot k = number of coded planes above p
         uint32_t k = 0;
         for (int t = (int)P.W - 1; t > p; t--) k += P.plane_lut[t] >= 0;
-        rans_region<false>(r, s_luts + li * LUT_SIZE, i0, c.d.n_match, c.off_planes + k * mc); i0 += c.d.n_match;
+        rans_region<false>(r, s_luts + li * (4 * LUT_SIZE), i0, c.d.n_match, c.off_planes + k * mc); i0 += c.d.n_match;
     }
     uint32_t nl = min(lit_limit, c.d.n_lit);
-    rans_region<false>(r, s_luts + P.lut_lit * LUT_SIZE, i0, nl, c.lit);
+    rans_region<false>(r, s_luts + P.lut_lit * (4 * LUT_SIZE), i0, nl, c.lit);
     if (nl == c.d.n_lit) {   // whole stream decoded: FORMAT.md §1.5 integrity check
         bool bad = (r.x != 65536u) || (r.wp != c.d.n_words);
         if (__any_sync(0xffffffffu, bad)) { if (lane_id() == 0) report(P, DF_RANS); return false; }
@@ -153,15 +153,20 @@ __device__ __forceinline__ void emit_block(const Params& P, const BlockCtx& c) {
     if (out_base != (uint32_t)(c.bend - c.bstart) || lit_base != c.d.n_lit) { if (lane == 0) report(P, DF_LENGTH); }
 }
 
-__global__ void __launch_bounds__(256) k_decode(const Params P) {
-    extern __shared__ __align__(16) uint32_t smem[];
-    uint32_t* s_luts = smem;
+__global__ void __launch_bounds__(512, 2) k_decode(const Params P) {
+    // shared memory: [pad to 8 KB][tables: n_coded_tables x 8 KB][rings: warps x 2 KB]  (absolute shared addresses)
+    extern __shared__ __align__(16) uint8_t smem_raw[];
+    const uint32_t smem0 = (uint32_t)__cvta_generic_to_shared(smem_raw);
+    const uint32_t pad = (8192u - (smem0 & 8191u)) & 8191u;
+    const uint32_t s_luts = smem0 + pad;
     const uint32_t n_lut_words = P.n_coded_tables * LUT_SIZE;
-    for (uint32_t i = threadIdx.x; i < n_lut_words / 4; i += blockDim.x)
-        reinterpret_cast<uint4*>(s_luts)[i] = __ldg(reinterpret_cast<const uint4*>(P.luts) + i);
+    {
+        uint4* dstv = reinterpret_cast<uint4*>(smem_raw + pad);
+        for (uint32_t i = threadIdx.x; i < n_lut_words / 4; i += blockDim.x) dstv[i] = __ldg(reinterpret_cast<const uint4*>(P.luts) + i);
+    }
     __syncthreads();
     const uint32_t warp = threadIdx.x >> 5, warps_per_cta = blockDim.x >> 5;
-    uint16_t* ring = reinterpret_cast<uint16_t*>(s_luts + n_lut_words) + warp * (RING_BYTES / 2);
+    const uint32_t ring = s_luts + n_lut_words * 4 + warp * RING_BYTES;
     BlockCtx c;
     bind_scratch(P, blockIdx.x * warps_per_cta + warp, c);
     for (;;) {
@@ -225,7 +230,7 @@ struct aceapex_archive {
     uint32_t epoch = 0;
     Resident res[MAX_RESIDENT];
     // launch geometry
-    int sms = 148, ctas_per_sm = 4, threads = 256;
+    int sms = 148, ctas_per_sm = 2, threads = 512;
     uint32_t grid = 0; size_t smem = 0;
     uint64_t scratch_per_warp = 0, ctrl_bytes = 0, flags_bytes = 0;
     // status
@@ -335,7 +340,7 @@ int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* 
         for (uint32_t s = 0; s < 256; s++) {
             uint32_t f = rd16(p + 16 + 2 * s);
             if (cum + f > (uint32_t)LUT_SIZE) return false;
-            for (uint32_t k = 0; k < f; k++) L[cum + k] = s | (f << 8) | (k << 20);
+            for (uint32_t k = 0; k < f; k++) L[cum + k] = s | (k << 8) | (f << 20);
             cum += f;
         }
         return cum == (uint32_t)LUT_SIZE;
@@ -392,8 +397,8 @@ int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* 
     int dev = 0; cudaDeviceProp prop;
     CU(cudaGetDevice(&dev)); CU(cudaGetDeviceProperties(&prop, dev));
     ar->sms = prop.multiProcessorCount;
-    ar->threads = 256;
-    ar->smem = (size_t)ar->n_coded_tables * LUT_SIZE * 4 + (size_t)(ar->threads / 32) * RING_BYTES;
+    ar->threads = 512;
+    ar->smem = 8192 + (size_t)ar->n_coded_tables * LUT_SIZE * 4 + (size_t)(ar->threads / 32) * RING_BYTES;
     CU(cudaFuncSetAttribute(k_decode, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ar->smem));
     int occ = 0;
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_decode, ar->threads, ar->smem));

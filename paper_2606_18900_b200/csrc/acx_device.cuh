@@ -7,8 +7,8 @@
 namespace acx {
 
 constexpr int PROB_BITS = 11;
-constexpr int LUT_SIZE = 1 << PROB_BITS;          // u32 entries per coded table: sym | freq << 8 | bias << 20
-constexpr int RING_BYTES = 1024;                  // per-warp ring of rANS words in shared memory (two 512 B halves)
+constexpr int LUT_SIZE = 1 << PROB_BITS;          // u32 entries per coded table: sym | bias << 8 | freq << 20
+constexpr int RING_BYTES = 2048;                  // per-warp ring of rANS words in shared memory (four 512 B quarters)
 constexpr int MAX_W = 8;
 constexpr int MAX_RESIDENT = 8;
 
@@ -69,71 +69,109 @@ __device__ __forceinline__ void st_release(uint32_t* p, uint32_t v) {
 __device__ __forceinline__ uint8_t ldcg8(const uint8_t* p) { return __ldcg(p); }
 __device__ __forceinline__ uint64_t ldcg64(const uint8_t* p) { return __ldcg(reinterpret_cast<const unsigned long long*>(p)); }
 
-__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
-    uint32_t s = (uint32_t)__cvta_generic_to_shared(smem);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
-}
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 // ------------------------------------------------------------------------------------------------ rANS ----------
 // FORMAT.md §1.5.  32 states, one per lane; symbol i lives on lane i & 31.  The word stream is staged through a
-// 1 KB per-warp shared-memory ring filled with 16-byte cp.async copies (one coalesced 512 B request per half).
+// 2 KB per-warp shared-memory ring (four 512 B quarters) filled with 16-byte cp.async copies: one coalesced 512 B
+// request per quarter, issued two quarters ahead of its use.  Both the ring (2 KB aligned) and every table
+// (8 KB aligned) sit at aligned shared addresses so that an index folds into an address with one LOP3.
+__device__ __forceinline__ uint32_t lds32(uint32_t a) { uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a)); return v; }
+__device__ __forceinline__ uint32_t lds16(uint32_t a) { uint32_t v; asm volatile("ld.shared.u16 %0, [%1];" : "=r"(v) : "r"(a)); return v; }
+__device__ __forceinline__ void cp_async16s(uint32_t saddr, const void* gmem) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(saddr), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait_group() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
 struct Rans {
     uint32_t x;              // this lane's state
     uint32_t wp;             // words consumed so far
-    uint32_t issued;         // bytes of the word stream requested into the ring
-    uint32_t ready;          // bytes known to have landed
+    uint32_t issued;         // bytes of the word stream requested into the ring (multiple of 512)
+    uint32_t ring;           // shared address of the ring, RING_BYTES aligned
     const uint8_t* words;    // global address of word 0 (16-byte aligned)
     const uint8_t* limit;    // archive end (loads are clamped)
-    uint16_t* ring;          // shared memory, RING_BYTES
 
-    __device__ __forceinline__ void fill_half() {
+    __device__ __forceinline__ void fill_quarter() {
         const uint8_t* g = words + issued + 16 * lane_id();
-        uint8_t* s = reinterpret_cast<uint8_t*>(ring) + ((issued + 16 * lane_id()) & (RING_BYTES - 1));
-        if (g + 16 <= limit) cp_async16(s, g);
+        if (g + 16 <= limit) cp_async16s(ring | ((issued + 16 * lane_id()) & (RING_BYTES - 1)), g);
+        cp_async_commit();
         issued += 512;
     }
-    __device__ __forceinline__ void init(const uint8_t* payload, const uint8_t* lim, uint16_t* r) {
-        ring = r; limit = lim; words = payload + 128; wp = 0; issued = 0; ready = 0;
-        x = reinterpret_cast<const uint32_t*>(payload)[lane_id()];
+    __device__ __forceinline__ void init(const uint8_t* payload, const uint8_t* lim, uint32_t ring_addr) {
+        ring = ring_addr; limit = lim; words = payload + 128; wp = 0; issued = 0;
+        x = __ldg(reinterpret_cast<const uint32_t*>(payload) + lane_id());
         __syncwarp();        // the previous block's ring reads are done
-        fill_half(); fill_half();
+        fill_quarter(); fill_quarter(); fill_quarter(); fill_quarter();
     }
-    // make sure the next 32 words are in the ring, and request the half that has been fully consumed
-    __device__ __forceinline__ void prepare() {
-        if (2 * wp + 64 > ready) { cp_async_wait_all(); __syncwarp(); ready = issued; }
-        if (issued - 2 * wp <= 512) { __syncwarp(); fill_half(); }   // every lane is past its ring reads of the last round
+    // Call before every group of <= 8 rounds (<= 512 B of words).  Invariant after the call: more than 1536 B are
+    // requested beyond the read position and all but the two most recent quarters have landed, so >= 512 B are readable.
+    __device__ __forceinline__ void prepare8() {
+        if (issued - 2 * wp <= RING_BYTES - 512) { __syncwarp(); fill_quarter(); }   // that quarter is fully consumed
+        cp_async_wait_group<2>();
+        __syncwarp();
     }
-    // decode one symbol on the lanes with active == true; all 32 lanes must call
-    __device__ __forceinline__ uint32_t step(const uint32_t* lut, bool active) {
-        uint32_t e = lut[x & (LUT_SIZE - 1)];
-        uint32_t nx = ((e >> 8) & 0xfff) * (x >> PROB_BITS) + (e >> 20);
+    // one symbol on every lane (full round).  lut = shared address of the table (8 KB aligned).
+    __device__ __forceinline__ uint32_t step_full(uint32_t lut) {
+        uint32_t e = lds32(lut | ((x << 2) & (4 * LUT_SIZE - 4)));
+        x = (e >> 20) * (x >> PROB_BITS) + ((e >> 8) & 0xfff);
+        bool need = x < 65536u;
+        uint32_t m = __ballot_sync(0xffffffffu, need);
+        uint32_t w = lds16(ring | ((2 * (wp + __popc(m & lanemask_lt()))) & (RING_BYTES - 1)));
+        if (need) x = (x << 16) | w;
+        wp += __popc(m);
+        return e;
+    }
+    // one symbol on the lanes with active == true; all 32 lanes must call
+    __device__ __forceinline__ uint32_t step(uint32_t lut, bool active) {
+        uint32_t e = lds32(lut | ((x << 2) & (4 * LUT_SIZE - 4)));
+        uint32_t nx = (e >> 20) * (x >> PROB_BITS) + ((e >> 8) & 0xfff);
         if (active) x = nx;
         bool need = active && x < 65536u;
         uint32_t m = __ballot_sync(0xffffffffu, need);
-        if (need) {
-            uint32_t k = wp + __popc(m & lanemask_lt());
-            x = (x << 16) | ring[k & (RING_BYTES / 2 - 1)];
-        }
+        uint32_t w = lds16(ring | ((2 * (wp + __popc(m & lanemask_lt()))) & (RING_BYTES - 1)));
+        if (need) x = (x << 16) | w;
         wp += __popc(m);
-        return e & 0xff;
+        return e;
     }
 };
 
 // Decodes `count` symbols whose global symbol indices start at i0, storing them to dst[0..count) (byte stores,
 // consecutive lanes -> consecutive bytes).  Returns the number of symbols equal to 255 when COUNT_ESC.
+// Table entries: sym | bias << 8 | freq << 20  (the low byte is what gets stored).
 template <bool COUNT_ESC>
-__device__ __forceinline__ uint32_t rans_region(Rans& r, const uint32_t* lut, uint32_t i0, uint32_t count, uint8_t* dst) {
+__device__ __forceinline__ uint32_t rans_region(Rans& r, uint32_t lut, uint32_t i0, uint32_t count, uint8_t* dst) {
     uint32_t esc = 0;
     if (count == 0) return 0;
-    uint32_t i1 = i0 + count;
-    for (uint32_t base = i0 & ~31u; base < i1; base += 32) {
-        uint32_t i = base + lane_id();
+    const uint32_t i1 = i0 + count, lane = lane_id();
+    uint32_t base = i0 & ~31u;
+    uint8_t* p = dst + lane - (i0 - base);           // address of symbol base + lane
+    if (base != i0) {                                // ragged first round
+        uint32_t i = base + lane;
         bool active = i >= i0 && i < i1;
-        r.prepare();
-        uint32_t s = r.step(lut, active);
-        if (active) dst[i - i0] = (uint8_t)s;
-        if (COUNT_ESC) esc += __popc(__ballot_sync(0xffffffffu, active && s == 255));
+        r.prepare8();
+        uint32_t e = r.step(lut, active);
+        if (active) *p = (uint8_t)e;
+        if (COUNT_ESC) esc += __popc(__ballot_sync(0xffffffffu, active && (e & 0xff) == 255));
+        base += 32; p += 32;
+    }
+    while (base + 256 <= i1) {                       // eight full rounds per ring check
+        r.prepare8();
+#pragma unroll
+        for (int k = 0; k < 8; k++) {
+            uint32_t e = r.step_full(lut);
+            p[32 * k] = (uint8_t)e;
+            if (COUNT_ESC) esc += __popc(__ballot_sync(0xffffffffu, (e & 0xff) == 255));
+        }
+        base += 256; p += 256;
+    }
+    if (base < i1) {                                 // fewer than eight rounds left, the last may be ragged
+        r.prepare8();
+        for (; base < i1; base += 32, p += 32) {
+            bool active = base + lane < i1;
+            uint32_t e = r.step(lut, active);
+            if (active) *p = (uint8_t)e;
+            if (COUNT_ESC) esc += __popc(__ballot_sync(0xffffffffu, active && (e & 0xff) == 255));
+        }
     }
     return esc;
 }
