@@ -83,9 +83,15 @@ int32_t aceapex_set_workspace(aceapex_archive* ar, void* d_workspace, uint64_t w
 int32_t aceapex_set_stream(aceapex_archive* ar, void* cuda_stream);
 
 /* Whole-file decode (§3.3, the paper's "v4").  d_out: >= raw_bytes device bytes.  On completion of the
- * stream, d_out[0..N) are the original bytes.  One persistent-kernel launch: blocks are taken in index order and a
- * block waits (device-side ready flags) for the earlier blocks it copies from.  Errors: E_WORKSPACE, E_CUDA. */
+ * stream, d_out[0..N) are the original bytes.  Two persistent-kernel launches: (1) every block: entropy decode,
+ * command scan, literal placement; (2) every block, sorted by (level, index): match resolution, a block waiting on a
+ * device-side ready flag only for source blocks of a strictly lower level (FORMAT.md §3).  Errors: E_WORKSPACE, E_CUDA. */
 int32_t aceapex_decode_all(aceapex_archive* ar, void* d_out);
+
+/* Same result in ONE launch: blocks are taken in index order; each block places its literals, publishes a
+ * "literals placed" flag, then resolves its matches, waiting for the literal flag of same-or-higher-level source
+ * blocks and for the completion flag of lower-level ones.  Kept for comparison. */
+int32_t aceapex_decode_all_fused(aceapex_archive* ar, void* d_out);
 
 /* Same result, scheduled the way the paper describes it: literal wave, then one match launch per dependency level
  * (FORMAT.md §3; max_level + 2 launches).  Exists for measurement (BASELINE.json configs[4]: wavefront depth and

@@ -47,6 +47,7 @@ def load():
             "aceapex_set_stream": ([p, p], i32),
             "aceapex_decode_all": ([p, p], i32),
             "aceapex_decode_all_levels": ([p, p], i32),
+            "aceapex_decode_all_fused": ([p, p], i32),
             "aceapex_decode_range": ([p, u64, u64, p, u64], i32),
             "aceapex_decode_reads": ([p, p, u64, p, u64, p], i32),
             "aceapex_reads_bytes": ([p, u64, p, u64, ctypes.POINTER(u64), p], i32),
@@ -134,9 +135,12 @@ class Archive:
             pass
 
     # -- the calls of include/aceapex.h
-    def decode_all(self, out=None, levels=False):
+    def decode_all(self, out=None, levels=False, schedule=None):
+        """schedule: None (default two-launch schedule), "levels" (one launch per level) or "fused" (one launch)."""
         out = self.new_output() if out is None else out
-        f = self.L.aceapex_decode_all_levels if levels else self.L.aceapex_decode_all
+        schedule = "levels" if levels else schedule
+        f = {None: self.L.aceapex_decode_all, "levels": self.L.aceapex_decode_all_levels,
+             "fused": self.L.aceapex_decode_all_fused}[schedule]
         _chk(f(self.h, out.data_ptr()), "decode_all")
         return out[:self.raw_bytes]
 

@@ -38,6 +38,30 @@ __device__ __forceinline__ void bind_scratch(const Params& P, uint32_t warp_glob
     c.off_planes = s;
 }
 
+// offset of match j assembled from coded planes (scratch) and raw planes (payload)
+__device__ __forceinline__ uint64_t match_src(const Params& P, const BlockCtx& c, uint32_t j) {
+    uint64_t src = 0, mc = (P.max_cmds + 15u) & ~15u;
+    uint32_t k = 0;
+    for (int p = (int)P.W - 1; p >= 0; p--) {
+        if (P.plane_lut[p] >= 0) { src |= (uint64_t)c.off_planes[k * mc + j] << (8 * p); k++; }
+        else src |= (uint64_t)__ldg(c.raw_planes + (uint64_t)P.plane_raw[p] * c.d.n_match + j) << (8 * p);
+    }
+    return src;
+}
+
+// Warm L2 with the source lines of every match of the block (issued before the literal stream is decoded, so the
+// HBM latency of the scattered sources overlaps the entropy decode).
+__device__ __forceinline__ void prefetch_sources(const Params& P, const BlockCtx& c) {
+    for (uint32_t j = lane_id(); j < c.d.n_match; j += 32) {
+        uint64_t src = match_src(P, c, j);
+        if (src >= P.out_pos0 && src < c.bstart) {
+            const uint8_t* p = P.out + (src - P.out_pos0);
+            prefetch_l2(p);
+            prefetch_l2(p + 64);
+        }
+    }
+}
+
 // A1: entropy-decode the block's streams into the warp's scratch.  lit_limit: number of literal symbols wanted.
 __device__ __forceinline__ bool parse_block(const Params& P, uint32_t s_luts, uint32_t ring, BlockCtx& c, uint32_t lit_limit) {
     const DirEntry* dp = P.dir + c.b;
@@ -67,6 +91,8 @@ __device__ __forceinline__ bool parse_block(const Params& P, uint32_t s_luts, ui
         for (int t = (int)P.W - 1; t > p; t--) k += P.plane_lut[t] >= 0;
         rans_region<false>(r, s_luts + li * (4 * LUT_SIZE), i0, c.d.n_match, c.off_planes + k * mc); i0 += c.d.n_match;
     }
+    __syncwarp();
+    if (P.mode != 2) prefetch_sources(P, c);
     uint32_t nl = min(lit_limit, c.d.n_lit);
     rans_region<false>(r, s_luts + P.lut_lit * (4 * LUT_SIZE), i0, nl, c.lit);
     if (nl == c.d.n_lit) {   // whole stream decoded: FORMAT.md §1.5 integrity check
@@ -77,45 +103,41 @@ __device__ __forceinline__ bool parse_block(const Params& P, uint32_t s_luts, ui
     return true;
 }
 
-// offset of match j assembled from coded planes (scratch) and raw planes (payload)
-__device__ __forceinline__ uint64_t match_src(const Params& P, const BlockCtx& c, uint32_t j) {
-    uint64_t src = 0, mc = (P.max_cmds + 15u) & ~15u;
-    uint32_t k = 0;
-    for (int p = (int)P.W - 1; p >= 0; p--) {
-        if (P.plane_lut[p] >= 0) { src |= (uint64_t)c.off_planes[k * mc + j] << (8 * p); k++; }
-        else src |= (uint64_t)__ldg(c.raw_planes + (uint64_t)P.plane_raw[p] * c.d.n_match + j) << (8 * p);
-    }
-    return src;
-}
-
 // flag[S] = 2 * epoch once block S has placed its literal bytes, 2 * epoch + 1 once it is complete
 __device__ __forceinline__ void wait_block(const Params& P, uint64_t S, bool need_full) {
     const uint32_t* f = P.flags + S;
     const uint32_t want = 2 * P.epoch + (need_full ? 1u : 0u);
-    uint32_t spins = 0;
+    uint32_t spins = 0, ns = 128;
     while (ld_flag(f) < want) {
-        __nanosleep(64);
-        if (++spins > (1u << 24)) { report(P, DF_TIMEOUT); break; }
+        __nanosleep(ns);
+        if (ns < 2048) ns *= 2;          // back off: thousands of lanes polling one L2 line slow everybody down
+        if (++spins > (1u << 21)) { report(P, DF_TIMEOUT); break; }
     }
+#ifdef ACX_WAIT_STATS
+    if (spins) { atomicAdd(P.err + 4 + (need_full ? 2 : 0), 1u); atomicAdd(P.err + 5 + (need_full ? 2 : 0), spins); }
+#endif
 }
 
-// Copy one match whose seed lies in the current FULL window.  WAIT: the flag-driven schedule waits for the source
-// blocks (other than the own block); the level schedule needs no wait (sources were completed by earlier launches).
+// Flag-driven schedule: wait for the blocks that hold the seed of a match (other than the own block).
 // By FORMAT.md §3 a source block S with level(S) >= level(B) can only contribute literal bytes, so B waits for S's
 // literal phase only; S with level(S) < level(B) may contribute match bytes, so B waits for S to complete.  Waits for
 // completion therefore go to strictly lower levels and chain at most max_level deep, whatever the distance.
-template <bool WAIT>
-__device__ __forceinline__ void copy_match_window(const Params& P, const BlockCtx& c, uint64_t dst, uint64_t src, uint32_t len) {
-    if (WAIT) {
-        uint64_t seed_end = min((unsigned long long)(src + len), (unsigned long long)dst);
-        uint64_t s0 = src >> P.log2_bs, s1 = (seed_end - 1) >> P.log2_bs;
-        for (uint64_t S = s0; S <= s1; S++) if (S != c.b) wait_block(P, S, __ldg(P.levels + S) < c.d.level);
+// LIT_WAITS = false: all literals were placed by an earlier launch, only completion waits remain.
+template <bool LIT_WAITS>
+__device__ __forceinline__ void wait_sources(const Params& P, const BlockCtx& c, uint64_t dst, uint64_t src, uint32_t len) {
+    uint64_t seed_end = min((unsigned long long)(src + len), (unsigned long long)dst);
+    uint64_t s0 = src >> P.log2_bs, s1 = (seed_end - 1) >> P.log2_bs;
+    for (uint64_t S = s0; S <= s1; S++) if (S != c.b) {
+        bool full = __ldg(P.levels + S) < c.d.level;
+        if (full || LIT_WAITS) wait_block(P, S, full);
     }
-    copy_bytes<true>(P.out + (dst - P.out_pos0), P.out + (src - P.out_pos0), len, dst - src);
 }
 
+constexpr uint32_t LONG_RUN = 64;   // runs at least this long are copied by the whole warp
+
 // A2 + A3 + A4 for a whole block: scan the commands 32 at a time, place literal runs, then resolve the matches.
-// MODE 2: literals only; MODE 0: matches only, waiting on source-block flags; MODE 3: matches only, no waits.
+// MODE 2: literals only; MODE 0: matches, waiting on literal and completion flags; MODE 4: matches, waiting on
+// completion flags only; MODE 3: matches only, no waits.
 template <int MODE>
 __device__ __forceinline__ void emit_block(const Params& P, const BlockCtx& c) {
     uint32_t lit_base = 0, out_base = 0, ec = 0, em = c.n_ext_cmd;
@@ -142,12 +164,31 @@ __device__ __forceinline__ void emit_block(const Params& P, const BlockCtx& c) {
         out_base += __shfl_sync(0xffffffffu, st, 31);
         bool ok = valid && (uint64_t)lit_pos + lit_len <= c.d.n_lit && out_pos + lit_len + match_len <= c.bend;
         if (__any_sync(0xffffffffu, valid && !ok)) { if (lane == 0) report(P, DF_LENGTH); return; }
-        if (MODE == 2 && ok && lit_len) copy_bytes<false>(P.out + (out_pos - P.out_pos0), c.lit + lit_pos, lit_len, ~0ull);
-        if (MODE == 2) continue;
-        if (ok && has_match) {
-            uint64_t dst = out_pos + lit_len, src = match_src(P, c, ci);
-            if (src >= dst) report(P, DF_OFFSET);
-            else copy_match_window<MODE == 0>(P, c, dst, src, match_len);
+        if (MODE == 2) {   // A3: literal runs.  Long runs (quality strings) are copied by the whole warp, short ones per lane.
+            uint32_t longs = __ballot_sync(0xffffffffu, ok && lit_len >= LONG_RUN);
+            if (ok && lit_len && lit_len < LONG_RUN) copy_bytes<false>(P.out + (out_pos - P.out_pos0), c.lit + lit_pos, lit_len, ~0ull);
+            while (longs) {
+                int l = __ffs(longs) - 1; longs &= longs - 1;
+                uint64_t op = __shfl_sync(0xffffffffu, out_pos, l);
+                uint32_t lp = __shfl_sync(0xffffffffu, lit_pos, l), n = __shfl_sync(0xffffffffu, lit_len, l);
+                warp_copy<false>(P.out + (op - P.out_pos0), c.lit + lp, n);
+            }
+            continue;
+        }
+        // A4: matches.  Non-overlapping long matches by the whole warp, the rest per lane.
+        uint64_t dst = out_pos + lit_len, src = (ok && has_match) ? match_src(P, c, ci) : 0;
+        bool good = ok && has_match && src < dst;
+        if (ok && has_match && !good) report(P, DF_OFFSET);
+        if (good && MODE == 0) wait_sources<true>(P, c, dst, src, match_len);
+        if (good && MODE == 4) wait_sources<false>(P, c, dst, src, match_len);
+        bool is_long = good && match_len >= LONG_RUN && src + match_len <= dst;
+        uint32_t longs = __ballot_sync(0xffffffffu, is_long);
+        if (good && !is_long) copy_bytes<true>(P.out + (dst - P.out_pos0), P.out + (src - P.out_pos0), match_len, dst - src);
+        while (longs) {
+            int l = __ffs(longs) - 1; longs &= longs - 1;
+            uint64_t d2 = __shfl_sync(0xffffffffu, dst, l), s2 = __shfl_sync(0xffffffffu, src, l);
+            uint32_t n = __shfl_sync(0xffffffffu, match_len, l);
+            warp_copy<true>(P.out + (d2 - P.out_pos0), P.out + (s2 - P.out_pos0), n);
         }
     }
     if (out_base != (uint32_t)(c.bend - c.bstart) || lit_base != c.d.n_lit) { if (lane == 0) report(P, DF_LENGTH); }
@@ -178,6 +219,15 @@ __global__ void __launch_bounds__(512, 2) k_decode(const Params P) {
         if (P.mode == 3) {
             // match wave: only the command / length / offset streams are needed again
             if (parse_block(P, s_luts, ring, c, 0)) emit_block<3>(P, c);
+            continue;
+        }
+        if (P.mode == 4) {
+            // all match waves in one launch: blocks arrive sorted by (level, index), a block waits for the completion
+            // of lower-level source blocks, which were dispatched before it
+            if (parse_block(P, s_luts, ring, c, 0)) emit_block<4>(P, c);
+            __threadfence();
+            __syncwarp();
+            if (lane_id() == 0) st_release(P.flags + c.b, 2 * P.epoch + 1);
             continue;
         }
         bool ok = parse_block(P, s_luts, ring, c, 0xffffffffu);
@@ -449,6 +499,19 @@ int32_t aceapex_set_stream(aceapex_archive* ar, void* s) {
 }
 
 int32_t aceapex_decode_all(aceapex_archive* ar, void* d_out) {
+    if (!ar || (!d_out && ar->N)) return ACEAPEX_E_ARG;
+    int32_t rc = prepare_ws(ar);
+    if (rc) return rc;
+    Params P; fill_params(ar, P);
+    P.out = static_cast<uint8_t*>(d_out); P.out_pos0 = 0; P.first_block = 0; P.epoch = ++ar->epoch;
+    if (!ar->d_level_lists) return ACEAPEX_OK;      // no blocks
+    P.mode = 2; P.level_list = nullptr;             // launch 1: entropy decode + literal placement, every block
+    if ((rc = launch(ar, P, ar->n_blocks))) return rc;
+    P.mode = 4; P.level_list = ar->d_level_lists;   // launch 2: matches, blocks sorted by (level, index)
+    return launch(ar, P, ar->n_blocks);
+}
+
+int32_t aceapex_decode_all_fused(aceapex_archive* ar, void* d_out) {
     if (!ar || (!d_out && ar->N)) return ACEAPEX_E_ARG;
     int32_t rc = prepare_ws(ar);
     if (rc) return rc;

@@ -257,4 +257,29 @@ __device__ __forceinline__ void copy_bytes(uint8_t* dst, const uint8_t* src, uin
     if (tail) st_small(d + body, tv, tail);
 }
 
+// Warp-cooperative copy of a long non-overlapping run: every lane moves 16 bytes per iteration, destination-aligned
+// 16-byte stores (512 B per warp instruction), byte lanes for the unaligned head and tail.  All 32 lanes must call.
+template <bool SRC_CG>
+__device__ __forceinline__ void warp_copy(uint8_t* dst, const uint8_t* src, uint32_t len) {
+    const uint32_t lane = lane_id();
+    uint32_t head = (uint32_t)(-reinterpret_cast<intptr_t>(dst)) & 15;
+    if (head > len) head = len;
+    if (lane < head) dst[lane] = SRC_CG ? ldcg8(src + lane) : src[lane];
+    uint32_t body = (len - head) & ~15u;
+    for (uint32_t off = head + 16 * lane; off < head + body; off += 512) {
+        const uint8_t* s = src + off;
+        uint32_t sh = (uint32_t)(reinterpret_cast<uintptr_t>(s) & 7) * 8;
+        const uint8_t* sa = s - (sh >> 3);
+        uint64_t w0 = ld64a<SRC_CG>(sa), w1 = ld64a<SRC_CG>(sa + 8), lo, hi;
+        if (sh == 0) { lo = w0; hi = w1; }
+        else { uint64_t w2 = ld64a<SRC_CG>(sa + 16); lo = (w0 >> sh) | (w1 << (64 - sh)); hi = (w1 >> sh) | (w2 << (64 - sh)); }
+        uint2 a = make_uint2((uint32_t)lo, (uint32_t)(lo >> 32)), b2 = make_uint2((uint32_t)hi, (uint32_t)(hi >> 32));
+        *reinterpret_cast<uint4*>(dst + off) = make_uint4(a.x, a.y, b2.x, b2.y);
+    }
+    uint32_t done = head + body;
+    if (done + lane < len) dst[done + lane] = SRC_CG ? ldcg8(src + done + lane) : src[done + lane];
+}
+
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
 } // namespace acx

@@ -9,10 +9,10 @@ from oracle import acx_oracle as O
 pytestmark = pytest.mark.gpu
 
 
-def gpu_decode(archive, levels=False):
+def gpu_decode(archive, levels=False, schedule=None):
     from paper_2606_18900_b200.aceapex import Archive
     ar = Archive(archive)
-    out = ar.decode_all(levels=levels)
+    out = ar.decode_all(levels=levels, schedule=schedule)
     ar.check()
     res = out.cpu().numpy().copy()
     ar.close()
@@ -40,6 +40,8 @@ def test_hand_built(case, levels):
     exp = O.decode(a)
     got = gpu_decode(a, levels=levels)
     assert got.tobytes() == exp.tobytes()
+    if not levels:
+        assert gpu_decode(a, schedule="fused").tobytes() == exp.tobytes()
 
 
 def test_hand_built_escapes_and_planes():
@@ -51,9 +53,9 @@ def test_hand_built_escapes_and_planes():
         assert gpu_decode(a).tobytes() == O.decode(a).tobytes()
 
 
-@pytest.mark.parametrize("levels", [False, True])
-def test_config0_fastq(fastq_4m, fastq_4m_archive, levels):
-    got = gpu_decode(fastq_4m_archive, levels=levels)
+@pytest.mark.parametrize("schedule", [None, "levels", "fused"])
+def test_config0_fastq(fastq_4m, fastq_4m_archive, schedule):
+    got = gpu_decode(fastq_4m_archive, schedule=schedule)
     assert np.array_equal(got, O.decode(fastq_4m_archive))      # bit-exact vs the oracle
     assert np.array_equal(got, fastq_4m)                         # and vs the original bytes
 
@@ -70,6 +72,7 @@ def test_block_sizes(fastq_4m, bs):
     a = encoder.encode(x, block_size=bs)
     assert np.array_equal(gpu_decode(a), x)
     assert np.array_equal(gpu_decode(a, levels=True), x)
+    assert np.array_equal(gpu_decode(a, schedule="fused"), x)
 
 
 def test_runs_and_periods():
