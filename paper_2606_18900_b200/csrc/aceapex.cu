@@ -62,8 +62,9 @@ __device__ __forceinline__ void prefetch_sources(const Params& P, const BlockCtx
     }
 }
 
-// A1: entropy-decode the block's streams into the warp's scratch.  lit_limit: number of literal symbols wanted.
-__device__ __forceinline__ bool parse_block(const Params& P, uint32_t s_luts, uint32_t ring, BlockCtx& c, uint32_t lit_limit) {
+// A1 (first part): directory entry, then the CMD, MLEN and coded OFF streams into the warp's scratch.  Leaves the rANS
+// state positioned at the first literal symbol (global symbol index *lit_i0).
+__device__ __forceinline__ bool parse_tokens(const Params& P, uint32_t s_luts, uint32_t ring, BlockCtx& c, Rans& r, uint32_t* lit_i0) {
     const DirEntry* dp = P.dir + c.b;
     const uint4* d4 = reinterpret_cast<const uint4*>(dp);
     uint4 a = __ldg(d4), q = __ldg(d4 + 1);
@@ -77,8 +78,6 @@ __device__ __forceinline__ bool parse_block(const Params& P, uint32_t s_luts, ui
     c.raw_planes = reinterpret_cast<const uint8_t*>(c.ext + c.d.n_ext);
     uint64_t mc = (P.max_cmds + 15u) & ~15u;
     if (c.d.n_cmd > P.max_cmds || c.d.n_match > c.d.n_cmd || c.d.n_lit > (1u << P.log2_bs)) { if (lane_id() == 0) report(P, DF_LENGTH); return false; }
-
-    Rans r;
     r.init(c.payload, P.archive + P.archive_bytes, ring);
     uint32_t i0 = 0;
     c.n_ext_cmd = rans_region<true>(r, s_luts + P.lut_cmd * (4 * LUT_SIZE), i0, c.d.n_cmd, c.tok_cmd); i0 += c.d.n_cmd;
@@ -92,15 +91,140 @@ __device__ __forceinline__ bool parse_block(const Params& P, uint32_t s_luts, ui
         rans_region<false>(r, s_luts + li * (4 * LUT_SIZE), i0, c.d.n_match, c.off_planes + k * mc); i0 += c.d.n_match;
     }
     __syncwarp();
+    *lit_i0 = i0;
+    return true;
+}
+
+// FORMAT.md §1.5 integrity check once every symbol of the block has been decoded
+__device__ __forceinline__ bool rans_final_ok(const Params& P, const BlockCtx& c, const Rans& r) {
+    bool bad = (r.x != 65536u) || (r.wp != c.d.n_words);
+    if (__any_sync(0xffffffffu, bad)) { if (lane_id() == 0) report(P, DF_RANS); return false; }
+    return true;
+}
+
+// A1, whole block: tokens, then the first min(lit_limit, n_lit) literal symbols into the scratch staging buffer.
+__device__ __forceinline__ bool parse_block(const Params& P, uint32_t s_luts, uint32_t ring, BlockCtx& c, uint32_t lit_limit) {
+    Rans r; uint32_t i0;
+    if (!parse_tokens(P, s_luts, ring, c, r, &i0)) return false;
     if (P.mode != 2) prefetch_sources(P, c);
     uint32_t nl = min(lit_limit, c.d.n_lit);
     rans_region<false>(r, s_luts + P.lut_lit * (4 * LUT_SIZE), i0, nl, c.lit);
-    if (nl == c.d.n_lit) {   // whole stream decoded: FORMAT.md §1.5 integrity check
-        bool bad = (r.x != 65536u) || (r.wp != c.d.n_words);
-        if (__any_sync(0xffffffffu, bad)) { if (lane_id() == 0) report(P, DF_RANS); return false; }
-    }
+    if (nl == c.d.n_lit && !rans_final_ok(P, c, r)) return false;
     __syncwarp();
     return true;
+}
+
+// ---- A2 + A3 fused into the literal decode ("direct placement") --------------------------------------------------
+// The command scan runs BEFORE the literal stream is decoded and leaves, in shared memory, one entry per non-empty
+// literal run: (last literal index of the run) | (out_start - lit_start) << 16.  The literal decode then stores every
+// decoded byte straight to its final position: while a 32-symbol round stays inside one run that is a pointer bump;
+// a round that crosses run boundaries looks its runs up with a 5-step shuffle search over the next 32 entries.
+constexpr uint32_t RUNS_CAP = 512;     // entries per warp (2 KB); blocks with more runs, or > 64 KB, use the staged path
+
+// returns the number of runs, or 0xffffffff when the block does not fit the table / fails validation
+__device__ __forceinline__ uint32_t build_runs(const Params& P, const BlockCtx& c, uint32_t runs /* shared address */) {
+    uint32_t lit_base = 0, out_base = 0, ec = 0, em = c.n_ext_cmd, n_runs = 0;
+    const uint32_t lane = lane_id();
+    bool fits = true;
+    for (uint32_t c0 = 0; c0 < c.d.n_cmd; c0 += 32) {
+        uint32_t ci = c0 + lane;
+        bool valid = ci < c.d.n_cmd, has_match = ci < c.d.n_match;
+        uint32_t tl = valid ? c.tok_cmd[ci] : 0, tm = has_match ? c.tok_mlen[ci] : 0;
+        uint32_t ml = __ballot_sync(0xffffffffu, valid && tl == 255), mm = __ballot_sync(0xffffffffu, has_match && tm == 255);
+        uint32_t lit_len = tl, match_len = has_match ? P.min_match + tm : 0;
+        if (valid && tl == 255) lit_len = 255 + __ldg(c.ext + ec + __popc(ml & lanemask_lt()));
+        if (has_match && tm == 255) match_len = P.min_match + 255 + __ldg(c.ext + em + __popc(mm & lanemask_lt()));
+        ec += __popc(ml); em += __popc(mm);
+        uint32_t sl = lit_len, st = lit_len + match_len;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t a = __shfl_up_sync(0xffffffffu, sl, o), t = __shfl_up_sync(0xffffffffu, st, o);
+            if (lane >= (uint32_t)o) { sl += a; st += t; }
+        }
+        uint32_t lit_pos = lit_base + sl - lit_len, out_rel = out_base + (st - lit_len - match_len);
+        lit_base += __shfl_sync(0xffffffffu, sl, 31);
+        out_base += __shfl_sync(0xffffffffu, st, 31);
+        uint32_t ne = __ballot_sync(0xffffffffu, valid && lit_len > 0);
+        uint32_t k = n_runs + __popc(ne & lanemask_lt());
+        if (valid && lit_len > 0 && k < RUNS_CAP) {
+            uint32_t e = ((lit_pos + lit_len - 1) & 0xffff) | ((out_rel - lit_pos) << 16);
+            asm volatile("st.shared.u32 [%0], %1;" ::"r"(runs + 4 * k), "r"(e) : "memory");
+        }
+        n_runs += __popc(ne);
+    }
+    fits = n_runs <= RUNS_CAP && lit_base == c.d.n_lit && c.bstart + out_base == c.bend;
+    __syncwarp();
+    return fits ? n_runs : 0xffffffffu;
+}
+
+// Literal decode with direct placement.  out_blk = address of the block's first output byte.
+struct RunCursor {
+    uint32_t k;          // run that holds the first literal of the coming round
+    uint32_t last;       // last literal index of run k
+    uint32_t delta;      // out_start - lit_start of run k
+};
+
+// A round whose literals [.., j_hi] are not all strictly inside run k: look the runs up (entries k .. k+31 cover any
+// 32 consecutive literals), store, and move the cursor to the run of the literal after j_hi.
+__device__ __forceinline__ void place_slow(RunCursor& rc, uint32_t runs, uint32_t n_runs, uint8_t* out_blk, uint32_t j, uint32_t j_hi,
+                                           uint32_t lane_hi, bool active, uint32_t e) {
+    uint32_t kk = rc.k + lane_id();
+    uint32_t ent = kk < n_runs ? lds32(runs + 4 * kk) : 0xffffffffu;
+    uint32_t last = kk < n_runs ? (ent & 0xffff) : 0xffffffffu;
+    uint32_t cnt = 0;                                     // number of runs (from k) that end before literal j
+#pragma unroll
+    for (int step = 16; step >= 1; step >>= 1) {
+        uint32_t t = __shfl_sync(0xffffffffu, last, (cnt + step - 1) & 31);
+        if (t < j) cnt += step;
+    }
+    uint32_t mine = __shfl_sync(0xffffffffu, ent, cnt & 31);
+    if (active) out_blk[(mine >> 16) + j] = (uint8_t)e;
+    uint32_t ck = __shfl_sync(0xffffffffu, cnt, lane_hi), ce = __shfl_sync(0xffffffffu, mine, lane_hi);
+    rc.k += ck; rc.last = ce & 0xffff; rc.delta = ce >> 16;
+    if (rc.last == j_hi && rc.k + 1 < n_runs) {           // that run ends with this round: the next literal opens run k + 1
+        rc.k++;
+        uint32_t en = lds32(runs + 4 * rc.k);
+        rc.last = en & 0xffff; rc.delta = en >> 16;
+    }
+}
+
+__device__ __forceinline__ void decode_lit_direct(Rans& r, uint32_t lut, uint32_t i0, uint32_t n_lit, uint32_t runs, uint32_t n_runs, uint8_t* out_blk) {
+    if (n_lit == 0) return;
+    const uint32_t lane = lane_id(), i1 = i0 + n_lit;
+    RunCursor rc;
+    { uint32_t e0 = lds32(runs); rc.k = 0; rc.last = e0 & 0xffff; rc.delta = e0 >> 16; }
+    uint32_t base = i0 & ~31u;
+    if (base != i0) {                                     // ragged first round
+        uint32_t i = base + lane;
+        bool active = i >= i0 && i < i1;
+        r.prepare8();
+        uint32_t e = r.step(lut, active);
+        uint32_t j_hi = min(base + 31, i1 - 1) - i0;
+        place_slow(rc, runs, n_runs, out_blk, i - i0, j_hi, (j_hi + i0 - base) & 31, active, e);
+        base += 32;
+    }
+    uint8_t* pj = out_blk + (base + lane - i0);           // address of literal (base + lane - i0) if delta were 0
+    while (base + 256 <= i1) {                            // eight full rounds per ring check
+        r.prepare8();
+        uint8_t* pd = pj + rc.delta;
+#pragma unroll
+        for (int q = 0; q < 8; q++) {
+            uint32_t e = r.step_full(lut);
+            uint32_t j_hi = base + 32 * q + 31 - i0;
+            if (j_hi < rc.last) pd[32 * q] = (uint8_t)e;   // the whole round lies strictly inside run k: pointer bump
+            else { place_slow(rc, runs, n_runs, out_blk, j_hi - 31 + lane, j_hi, 31, true, e); pd = pj + rc.delta; }
+        }
+        base += 256; pj += 256;
+    }
+    if (base < i1) {                                      // fewer than eight rounds left, the last may be ragged
+        r.prepare8();
+        for (; base < i1; base += 32) {
+            bool active = base + lane < i1;
+            uint32_t e = r.step(lut, active);
+            uint32_t j_hi = min(base + 31, i1 - 1) - i0;
+            place_slow(rc, runs, n_runs, out_blk, base + lane - i0, j_hi, (j_hi + i0 - base) & 31, active, e);
+        }
+    }
 }
 
 // flag[S] = 2 * epoch once block S has placed its literal bytes, 2 * epoch + 1 once it is complete
@@ -194,7 +318,7 @@ __device__ __forceinline__ void emit_block(const Params& P, const BlockCtx& c) {
     if (out_base != (uint32_t)(c.bend - c.bstart) || lit_base != c.d.n_lit) { if (lane == 0) report(P, DF_LENGTH); }
 }
 
-__global__ void __launch_bounds__(512, 2) k_decode(const Params P) {
+__global__ void __launch_bounds__(1024, 1) k_decode(const Params P) {
     // shared memory: [pad to 8 KB][tables: n_coded_tables x 8 KB][rings: warps x 2 KB]  (absolute shared addresses)
     extern __shared__ __align__(16) uint8_t smem_raw[];
     const uint32_t smem0 = (uint32_t)__cvta_generic_to_shared(smem_raw);
@@ -208,6 +332,7 @@ __global__ void __launch_bounds__(512, 2) k_decode(const Params P) {
     __syncthreads();
     const uint32_t warp = threadIdx.x >> 5, warps_per_cta = blockDim.x >> 5;
     const uint32_t ring = s_luts + n_lut_words * 4 + warp * RING_BYTES;
+    const uint32_t runs = s_luts + n_lut_words * 4 + warps_per_cta * RING_BYTES + warp * (4 * RUNS_CAP);
     BlockCtx c;
     bind_scratch(P, blockIdx.x * warps_per_cta + warp, c);
     for (;;) {
@@ -230,7 +355,24 @@ __global__ void __launch_bounds__(512, 2) k_decode(const Params P) {
             if (lane_id() == 0) st_release(P.flags + c.b, 2 * P.epoch + 1);
             continue;
         }
-        bool ok = parse_block(P, s_luts, ring, c, 0xffffffffu);
+        bool ok;
+        if (P.mode == 2 && P.log2_bs <= 16) {
+            // literal launch: scan first, then decode the literal stream straight to its final positions
+            Rans r; uint32_t i0;
+            ok = parse_tokens(P, s_luts, ring, c, r, &i0);
+            if (ok) {
+                uint32_t n_runs = build_runs(P, c, runs);
+                if (n_runs != 0xffffffffu) {
+                    decode_lit_direct(r, s_luts + P.lut_lit * (4 * LUT_SIZE), i0, c.d.n_lit, runs, n_runs, P.out + (c.bstart - P.out_pos0));
+                    rans_final_ok(P, c, r);
+                } else {                                              // too many runs (or a bad scan): staged path
+                    rans_region<false>(r, s_luts + P.lut_lit * (4 * LUT_SIZE), i0, c.d.n_lit, c.lit);
+                    if (rans_final_ok(P, c, r)) { __syncwarp(); emit_block<2>(P, c); }
+                }
+            }
+            continue;
+        }
+        ok = parse_block(P, s_luts, ring, c, 0xffffffffu);
         if (ok) emit_block<2>(P, c);                                  // A3: all literal bytes of the block
         if (P.mode == 0) {
             __threadfence();
@@ -280,7 +422,7 @@ struct aceapex_archive {
     uint32_t epoch = 0;
     Resident res[MAX_RESIDENT];
     // launch geometry
-    int sms = 148, ctas_per_sm = 2, threads = 512;
+    int sms = 148, ctas_per_sm = 1, threads = 1024;
     uint32_t grid = 0; size_t smem = 0;
     uint64_t scratch_per_warp = 0, ctrl_bytes = 0, flags_bytes = 0;
     // status
@@ -447,9 +589,10 @@ int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* 
     int dev = 0; cudaDeviceProp prop;
     CU(cudaGetDevice(&dev)); CU(cudaGetDeviceProperties(&prop, dev));
     ar->sms = prop.multiProcessorCount;
-    ar->threads = 512;
-    ar->smem = 8192 + (size_t)ar->n_coded_tables * LUT_SIZE * 4 + (size_t)(ar->threads / 32) * RING_BYTES;
+    ar->threads = 1024;   // one CTA per SM: the decode tables are staged once per SM, 32 warps share them
+    ar->smem = 8192 + (size_t)ar->n_coded_tables * LUT_SIZE * 4 + (size_t)(ar->threads / 32) * (RING_BYTES + 4 * RUNS_CAP);
     CU(cudaFuncSetAttribute(k_decode, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ar->smem));
+    CU(cudaFuncSetAttribute(k_decode, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
     int occ = 0;
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_decode, ar->threads, ar->smem));
     if (occ < 1) return ACEAPEX_E_CUDA;
