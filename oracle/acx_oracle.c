@@ -226,9 +226,10 @@ static int decode_block(const hdr_t* h, const dir_t* d, const scratch_t* s, uint
             if (!(src < dst) || dst + ml > end) return E_CORRUPT;
             if (matchmap) {
                 uint64_t seed_end = src + ml < dst ? src + ml : dst;
-                for (uint64_t q = src; q < seed_end; q++) if (getbit(matchmap, q)) {
+                for (uint64_t q = src; q < seed_end; q++) {
                     uint64_t S = q >> h->log2_bs;
-                    if (S == b || !(levels[S] < d->level)) return E_LEVEL;
+                    if (getbit(matchmap, q)) { if (S == b || !(levels[S] < d->level)) return E_LEVEL; }  /* §3 (b) */
+                    else if (S != b && !(levels[S] <= d->level)) return E_LEVEL;                          /* §3 (a) */
                 }
             }
             for (uint32_t i = 0; i < ml; i++) out[dst + i] = out[src + i]; /* ascending, one byte at a time */

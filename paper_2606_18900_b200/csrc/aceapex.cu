@@ -24,15 +24,17 @@ struct BlockCtx {
     uint32_t n_ext_cmd;             // number of CMD escapes (they come first in EXT)
     // per-warp scratch
     uint8_t *tok_cmd, *tok_mlen, *off_planes, *lit;
+    uint4* desc;                    // per match: {dst_rel, len, src lo, src hi} (chunked match resolution)
 };
 
 __device__ __forceinline__ void report(const Params& P, uint32_t bit) { atomicOr(P.err, bit); }
 
-// Scratch layout per warp: [lit: BS + 32][tok_cmd: max_cmds][tok_mlen: max_cmds][off planes: n_coded x max_cmds] (16 B aligned)
+// Scratch layout per warp: [lit: BS + 32][desc: 16 B x max_cmds][tok_cmd: max_cmds][tok_mlen: max_cmds][off planes: n_coded x max_cmds]
 __device__ __forceinline__ void bind_scratch(const Params& P, uint32_t warp_global, BlockCtx& c) {
     uint8_t* s = P.scratch + (uint64_t)warp_global * P.scratch_per_warp;
     uint64_t mc = (P.max_cmds + 15u) & ~15u;
     c.lit = s; s += (1ull << P.log2_bs) + 32;
+    c.desc = reinterpret_cast<uint4*>(s); s += 16 * mc;
     c.tok_cmd = s; s += mc;
     c.tok_mlen = s; s += mc;
     c.off_planes = s;
@@ -318,6 +320,125 @@ __device__ __forceinline__ void emit_block(const Params& P, const BlockCtx& c) {
     if (out_base != (uint32_t)(c.bend - c.bstart) || lit_base != c.d.n_lit) { if (lane == 0) report(P, DF_LENGTH); }
 }
 
+// ---- A4, output-centric ("chunked") --------------------------------------------------------------------------------
+// Every lane owns one 16-byte aligned chunk of the block's output at a time: it reads the chunk (the literal bytes are
+// already there), finds the matches that overlap it (binary search over the match end positions in shared memory),
+// fetches their source bytes, merges and writes the chunk back with one aligned 16-byte store.  All lanes run the same
+// code whatever the match lengths are, stores are coalesced, and a self-overlapping match is just a gather from its
+// seed with index (i mod period) -- FORMAT.md §2 -- so it needs no serial path.
+// Shared-memory aux area per warp (4 * RUNS_CAP bytes, shared with the run table of the literal phase):
+//   [0, 2 * CHUNK_MATCH_CAP): u16 end_rel - 1 per match      [.., + 4 * CHUNK_WORDS): bitmap of chunks holding match bytes
+constexpr uint32_t CHUNK_MATCH_CAP = 768;
+constexpr uint32_t CHUNK_WORDS = 128;        // 4096 chunks = 64 KB blocks
+static_assert(2 * CHUNK_MATCH_CAP + 4 * CHUNK_WORDS <= 4 * RUNS_CAP, "aux area");
+
+__device__ __forceinline__ uint64_t ones_bytes(uint32_t n) { return n >= 8 ? ~0ull : ((1ull << (8 * n)) - 1); }   // low n bytes set
+
+// WAIT: 0 none, 1 completion flags of lower-level blocks, 2 literal flags too.  Returns false when the block does not
+// fit (caller falls back to the per-match path).
+template <int WAIT>
+__device__ __forceinline__ bool resolve_chunked(const Params& P, const BlockCtx& c, uint32_t aux) {
+    const uint32_t lane = lane_id();
+    const uint32_t blk_bytes = (uint32_t)(c.bend - c.bstart);
+    if (c.d.n_match > CHUNK_MATCH_CAP || P.log2_bs > 16 || P.log2_bs < 4) return false;
+    if (c.d.n_match == 0) return true;
+    const uint32_t ends = aux, bitmap = aux + 2 * CHUNK_MATCH_CAP;
+    const uint32_t n_chunks = (blk_bytes + 15) >> 4, n_words = (n_chunks + 31) >> 5;
+    for (uint32_t w = lane; w < n_words; w += 32) asm volatile("st.shared.u32 [%0], %1;" ::"r"(bitmap + 4 * w), "r"(0u) : "memory");
+    __syncwarp();
+    // ---- scan: per match {dst_rel, len, src} to scratch, end to shared memory, chunk bitmap
+    uint32_t out_base = 0, lit_total = 0, ec = 0, em = c.n_ext_cmd;
+    bool bad = false;
+    for (uint32_t c0 = 0; c0 < c.d.n_cmd; c0 += 32) {
+        uint32_t ci = c0 + lane;
+        bool valid = ci < c.d.n_cmd, has_match = ci < c.d.n_match;
+        uint32_t tl = valid ? c.tok_cmd[ci] : 0, tm = has_match ? c.tok_mlen[ci] : 0;
+        uint32_t ml = __ballot_sync(0xffffffffu, valid && tl == 255), mm = __ballot_sync(0xffffffffu, has_match && tm == 255);
+        uint32_t lit_len = tl, match_len = has_match ? P.min_match + tm : 0;
+        if (valid && tl == 255) lit_len = 255 + __ldg(c.ext + ec + __popc(ml & lanemask_lt()));
+        if (has_match && tm == 255) match_len = P.min_match + 255 + __ldg(c.ext + em + __popc(mm & lanemask_lt()));
+        ec += __popc(ml); em += __popc(mm);
+        uint32_t st = lit_len + match_len, sl = lit_len;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t t = __shfl_up_sync(0xffffffffu, st, o), a = __shfl_up_sync(0xffffffffu, sl, o);
+            if (lane >= (uint32_t)o) { st += t; sl += a; }
+        }
+        uint32_t dst_rel = out_base + st - match_len, end_rel = out_base + st;
+        out_base += __shfl_sync(0xffffffffu, st, 31);
+        lit_total += __shfl_sync(0xffffffffu, sl, 31);
+        if (has_match) {
+            uint64_t src = match_src(P, c, ci);
+            bool okm = end_rel <= blk_bytes && src < c.bstart + dst_rel && src >= P.out_pos0;
+            if (!okm) { bad = true; match_len = 0; end_rel = min(end_rel, blk_bytes); dst_rel = min(dst_rel, end_rel); }
+            c.desc[ci] = make_uint4(dst_rel, match_len, (uint32_t)src, (uint32_t)(src >> 32));
+            asm volatile("st.shared.u16 [%0], %1;" ::"r"(ends + 2 * ci), "h"((uint16_t)(end_rel - 1)) : "memory");
+            if (match_len) for (uint32_t ch = dst_rel >> 4; ch <= (end_rel - 1) >> 4; ch++)
+                asm volatile("red.shared.or.b32 [%0], %1;" ::"r"(bitmap + 4 * (ch >> 5)), "r"(1u << (ch & 31)) : "memory");
+        }
+    }
+    if (__any_sync(0xffffffffu, bad)) { if (lane == 0) report(P, DF_OFFSET); }
+    if (out_base != blk_bytes || lit_total != c.d.n_lit) { if (lane == 0) report(P, DF_LENGTH); return true; }
+    __syncwarp();
+    // ---- chunks
+    uint8_t* out_blk = P.out + (c.bstart - P.out_pos0);
+    for (uint32_t w = 0; w < n_words; w++) {
+        uint32_t word = lds32(bitmap + 4 * w);
+        if (word == 0) continue;
+        if (!((word >> lane) & 1)) continue;                 // divergent from here on; no warp-level primitives below
+        const uint32_t q = (32 * w + lane) << 4;             // chunk start, block-relative
+        const uint32_t nv = min(16u, blk_bytes - q);         // valid bytes (only the file's last chunk can be short)
+        uint64_t lo = 0, hi = 0;
+        if (nv == 16) { uint4 o = __ldcg(reinterpret_cast<const uint4*>(out_blk + q)); lo = (uint64_t)o.x | ((uint64_t)o.y << 32); hi = (uint64_t)o.z | ((uint64_t)o.w << 32); }
+        else for (uint32_t t = 0; t < nv; t++) { uint64_t v = ldcg8(out_blk + q + t); if (t < 8) lo |= v << (8 * t); else hi |= v << (8 * (t - 8)); }
+        uint32_t a0 = 0, b0 = c.d.n_match;                    // first match with end_rel - 1 >= q
+        while (a0 < b0) { uint32_t mid = (a0 + b0) >> 1; if (lds16(ends + 2 * mid) < q) a0 = mid + 1; else b0 = mid; }
+        for (uint32_t m = a0; m < c.d.n_match; m++) {
+            uint4 d = c.desc[m];
+            if (d.x >= q + 16) break;
+            uint32_t pa = max(d.x, q), pb = min(d.x + d.y, q + nv);
+            if (pa >= pb) continue;
+            uint32_t a = pa - q, n = pb - pa, i = pa - d.x;  // chunk byte offset, byte count, offset inside the match
+            uint64_t src = (uint64_t)d.z | ((uint64_t)d.w << 32), dstpos = c.bstart + d.x, period = dstpos - src;
+            if (WAIT) {
+                uint64_t seed_end = min((unsigned long long)(src + d.y), (unsigned long long)dstpos);
+                uint64_t f0 = period >= d.y ? src + i : src, f1 = period >= d.y ? src + i + n : seed_end;
+                for (uint64_t S = f0 >> P.log2_bs; S <= (f1 - 1) >> P.log2_bs; S++) if (S != c.b) {
+                    bool full = __ldg(P.levels + S) < c.d.level;
+                    if (full || WAIT == 2) wait_block(P, S, full);
+                }
+            }
+            uint64_t vlo, vhi;
+            if (period >= d.y) {                             // non-overlapping: n contiguous source bytes
+                const uint8_t* sp = P.out + (src + i - P.out_pos0);
+                vlo = ld64u<true>(sp, n < 8 ? n : 8);
+                vhi = n > 8 ? ld64u<true>(sp + 8, n - 8) : 0;
+            } else {                                         // self-overlap: byte i of the match = seed[i mod period]
+                vlo = 0; vhi = 0;
+                uint32_t r0 = (uint32_t)(i % period);
+                for (uint32_t t = 0; t < n; t++) {
+                    uint64_t v = ldcg8(P.out + (src + r0 - P.out_pos0));
+                    if (t < 8) vlo |= v << (8 * t); else vhi |= v << (8 * (t - 8));
+                    if (++r0 == period) r0 = 0;
+                }
+            }
+            // place bytes [0, n) of (vlo, vhi) at chunk bytes [a, a + n)
+            uint64_t mlo = ones_bytes(a + n) & ~ones_bytes(a), mhi = (a + n > 8 ? ones_bytes(a + n - 8) : 0) & ~(a > 8 ? ones_bytes(a - 8) : 0);
+            uint64_t slo, shi;
+            if (a == 0) { slo = vlo; shi = vhi; }
+            else if (a < 8) { slo = vlo << (8 * a); shi = (vhi << (8 * a)) | (vlo >> (64 - 8 * a)); }
+            else if (a == 8) { slo = 0; shi = vlo; }
+            else { slo = 0; shi = vlo << (8 * (a - 8)); }
+            lo = (lo & ~mlo) | (slo & mlo);
+            hi = (hi & ~mhi) | (shi & mhi);
+        }
+        if (nv == 16) *reinterpret_cast<uint4*>(out_blk + q) = make_uint4((uint32_t)lo, (uint32_t)(lo >> 32), (uint32_t)hi, (uint32_t)(hi >> 32));
+        else for (uint32_t t = 0; t < nv; t++) out_blk[q + t] = (uint8_t)((t < 8 ? lo >> (8 * t) : hi >> (8 * (t - 8))));
+    }
+    __syncwarp();
+    return true;
+}
+
 __global__ void __launch_bounds__(1024, 1) k_decode(const Params P) {
     // shared memory: [pad to 8 KB][tables: n_coded_tables x 8 KB][rings: warps x 2 KB]  (absolute shared addresses)
     extern __shared__ __align__(16) uint8_t smem_raw[];
@@ -343,42 +464,42 @@ __global__ void __launch_bounds__(1024, 1) k_decode(const Params P) {
         c.b = P.level_list ? (uint64_t)P.level_list[t] : P.first_block + t;
         if (P.mode == 3) {
             // match wave: only the command / length / offset streams are needed again
-            if (parse_block(P, s_luts, ring, c, 0)) emit_block<3>(P, c);
+            if (parse_block(P, s_luts, ring, c, 0) && !(P.chunked && resolve_chunked<0>(P, c, runs))) emit_block<3>(P, c);
             continue;
         }
         if (P.mode == 4) {
             // all match waves in one launch: blocks arrive sorted by (level, index), a block waits for the completion
             // of lower-level source blocks, which were dispatched before it
-            if (parse_block(P, s_luts, ring, c, 0)) emit_block<4>(P, c);
+            if (parse_block(P, s_luts, ring, c, 0) && !(P.chunked && resolve_chunked<1>(P, c, runs))) emit_block<4>(P, c);
             __threadfence();
             __syncwarp();
             if (lane_id() == 0) st_release(P.flags + c.b, 2 * P.epoch + 1);
             continue;
         }
+        // modes 0 (everything, flags) and 2 (literal launch): A1 + A2 + A3
         bool ok;
-        if (P.mode == 2 && P.log2_bs <= 16) {
-            // literal launch: scan first, then decode the literal stream straight to its final positions
+        {
             Rans r; uint32_t i0;
             ok = parse_tokens(P, s_luts, ring, c, r, &i0);
             if (ok) {
-                uint32_t n_runs = build_runs(P, c, runs);
-                if (n_runs != 0xffffffffu) {
+                if (P.mode == 0) prefetch_sources(P, c);              // source lines travel to L2 while the literals decode
+                uint32_t n_runs = P.log2_bs <= 16 ? build_runs(P, c, runs) : 0xffffffffu;
+                if (n_runs != 0xffffffffu) {                          // scan first, literals straight to their positions
                     decode_lit_direct(r, s_luts + P.lut_lit * (4 * LUT_SIZE), i0, c.d.n_lit, runs, n_runs, P.out + (c.bstart - P.out_pos0));
-                    rans_final_ok(P, c, r);
-                } else {                                              // too many runs (or a bad scan): staged path
+                    ok = rans_final_ok(P, c, r);
+                } else {                                              // too many runs / big block / bad scan: staged path
                     rans_region<false>(r, s_luts + P.lut_lit * (4 * LUT_SIZE), i0, c.d.n_lit, c.lit);
-                    if (rans_final_ok(P, c, r)) { __syncwarp(); emit_block<2>(P, c); }
+                    ok = rans_final_ok(P, c, r);
+                    __syncwarp();
+                    if (ok) emit_block<2>(P, c);
                 }
             }
-            continue;
         }
-        ok = parse_block(P, s_luts, ring, c, 0xffffffffu);
-        if (ok) emit_block<2>(P, c);                                  // A3: all literal bytes of the block
         if (P.mode == 0) {
             __threadfence();
             __syncwarp();
             if (lane_id() == 0) st_release(P.flags + c.b, 2 * P.epoch);       // literals placed
-            if (ok) emit_block<0>(P, c);                              // A4: matches (waits on source blocks)
+            if (ok && !(P.chunked && resolve_chunked<2>(P, c, runs))) emit_block<0>(P, c);   // A4 (waits on source blocks)
             __threadfence();
             __syncwarp();
             if (lane_id() == 0) st_release(P.flags + c.b, 2 * P.epoch + 1);   // complete (set even on error: nobody waits forever)
@@ -427,6 +548,7 @@ struct aceapex_archive {
     uint64_t scratch_per_warp = 0, ctrl_bytes = 0, flags_bytes = 0;
     // status
     int32_t last_cuda = 0; uint32_t dev_flags = 0; uint64_t launches = 0;
+    uint32_t chunked = 0;   // match resolver: 0 = one lane per match, 1 = one lane per 16-byte output chunk
 };
 
 namespace {
@@ -460,6 +582,7 @@ void fill_params(const aceapex_archive* ar, Params& P) {
     P.scratch = ar->d_ws + ar->ctrl_bytes + ar->flags_bytes;
     P.scratch_per_warp = ar->scratch_per_warp; P.max_cmds = ar->max_cmds;
     P.clip_lo = 0; P.clip_hi = ar->N;
+    P.chunked = ar->chunked;
 }
 
 int32_t prepare_ws(aceapex_archive* ar) {
@@ -596,11 +719,12 @@ int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* 
     int occ = 0;
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_decode, ar->threads, ar->smem));
     if (occ < 1) return ACEAPEX_E_CUDA;
+    if (const char* e = getenv("ACEAPEX_CHUNKED")) ar->chunked = atoi(e) != 0;
     if (const char* e = getenv("ACEAPEX_CTAS_PER_SM")) occ = std::max(1, std::min(occ, atoi(e)));
     ar->ctas_per_sm = occ;
     ar->grid = (uint32_t)(ar->sms * occ);
     uint64_t mc = align_up(ar->max_cmds, 16);
-    ar->scratch_per_warp = align_up((1ull << ar->log2_bs) + 32 + mc * (2 + ar->n_coded_planes), 256);
+    ar->scratch_per_warp = align_up((1ull << ar->log2_bs) + 32 + mc * (16 + 2 + ar->n_coded_planes), 256);
     ar->ctrl_bytes = 256;
     ar->flags_bytes = align_up(4 * ar->n_blocks + 4, 256);
     guard.a = nullptr;
@@ -660,6 +784,7 @@ int32_t aceapex_decode_all_fused(aceapex_archive* ar, void* d_out) {
     if (rc) return rc;
     Params P; fill_params(ar, P);
     P.mode = 0; P.out = static_cast<uint8_t*>(d_out); P.out_pos0 = 0; P.first_block = 0; P.epoch = ++ar->epoch;
+    P.level_list = ar->d_level_lists;   // blocks sorted by (level, index): everything a block reads from precedes it
     return launch(ar, P, ar->n_blocks);
 }
 

@@ -49,8 +49,9 @@ struct Params {
     unsigned long long* ticket;
     uint32_t* err;
     uint8_t* scratch; uint64_t scratch_per_warp; uint32_t max_cmds; uint32_t stack_cap;
-    uint32_t mode;                       // 0 = FULL blocks with flags, 1 = SPAN demands, 2 = literal wave, 3 = match wave
-    const uint32_t* level_list;          // mode 2/3: block ids to process (n_work entries), null = first_block + i
+    uint32_t mode;                       // 0 = everything with flags, 2 = literal launch, 3 = match wave, 4 = all match waves with flags
+    const uint32_t* level_list;          // block ids to process (n_work entries), null = first_block + i
+    uint32_t chunked;                    // match resolver: 0 = lane per match, 1 = lane per 16-byte output chunk
 };
 
 __device__ __forceinline__ uint32_t lane_id() { return threadIdx.x & 31; }

@@ -2,6 +2,7 @@
 // subsystem 1; the paper's encoder: "global match search", absolute offsets, fixed-size blocks, §2).
 // It shares no code with the decoders (oracle/, csrc/): decoders are checked against the ORIGINAL bytes.
 //
+// Levels (FORMAT.md §3): level(B) >= level(S) for every block S that B reads, > when B reads match bytes of S.
 // Parse: greedy LZ77 with (a) a global first-occurrence table of 8-byte keys filled batch by batch and (b) per-chunk
 // 4-byte hash chains.  A candidate is accepted only if it keeps the FORMAT.md §3 invariant: seed bytes inside the
 // current block must be literal bytes, seed bytes that are match bytes of an earlier block S need
@@ -99,10 +100,11 @@ struct Enc {
         while (a < seed_end) {
             uint64_t S = a / BS, sb_end = std::min(seed_end, (S + 1) * BS);
             uint64_t q = first_nonlit(a, sb_end);
+            if (S * BS != bstart) lvl = std::max(lvl, (uint32_t)level[S]);   // literal bytes of S: level(B) >= level(S)
             if (q < sb_end) {
                 bool ok = (S * BS != bstart) && (uint32_t)level[S] + 1 <= o.max_level;
                 if (!ok) { seed_end = q; l = q - p; break; } // cut the match in front of the offending byte
-                lvl = std::max(lvl, (uint32_t)level[S] + 1);
+                lvl = std::max(lvl, (uint32_t)level[S] + 1);                 // match bytes of S: level(B) > level(S)
             }
             a = sb_end;
         }
@@ -158,8 +160,9 @@ struct Enc {
                 // extend backwards over pending literals while the source byte is a literal byte
                 uint64_t p = best.p, len = best.len;
                 while (i > lit_start && p > 0 && x[i - 1] == x[p - 1] && (p - 1 >= cs || p - 1 < batch_start) && is_lit(p - 1)) {
-                    // the new seed byte p-1 is a literal byte: always allowed by FORMAT.md §3 (a)
+                    // the new seed byte p-1 is a literal byte: allowed by FORMAT.md §3 (a); its block may raise the level
                     i--; p--; len++;
+                    if (p / BS != bi) best.lvl = std::max(best.lvl, (uint32_t)level[p / BS]);
                 }
                 put_lit_token(i - lit_start);
                 uint64_t t = len - o.min_match;
