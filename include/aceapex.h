@@ -117,7 +117,8 @@ int32_t aceapex_reads_bytes(const uint64_t* h_read_index, uint64_t n_index, cons
 
 /* Makes bytes [pos_lo, pos_hi) of the decompressed output, already resident at d_ptr, usable as match sources by
  * aceapex_decode_range (the ring of PAPER.md:107-109 §5: earlier windows stay resident while later ones decode).
- * slot < 8; pos_lo == pos_hi clears the slot. */
+ * slot < 8; pos_lo == pos_hi clears the slot.  A slot must be cleared (or re-pointed) BEFORE its buffer is overwritten,
+ * and d_ptr must be 8-byte aligned. */
 int32_t aceapex_set_resident(aceapex_archive* ar, uint32_t slot, uint64_t pos_lo, uint64_t pos_hi, const void* d_ptr);
 
 /* Device FNV-1a 64 of each block of d_data (= decompressed bytes [byte_lo, byte_hi), byte_lo block aligned) compared

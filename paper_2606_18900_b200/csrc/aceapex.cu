@@ -24,17 +24,15 @@ struct BlockCtx {
     uint32_t n_ext_cmd;             // number of CMD escapes (they come first in EXT)
     // per-warp scratch
     uint8_t *tok_cmd, *tok_mlen, *off_planes, *lit;
-    uint4* desc;                    // per match: {dst_rel, len, src lo, src hi} (chunked match resolution)
 };
 
 __device__ __forceinline__ void report(const Params& P, uint32_t bit) { atomicOr(P.err, bit); }
 
-// Scratch layout per warp: [lit: BS + 32][desc: 16 B x max_cmds][tok_cmd: max_cmds][tok_mlen: max_cmds][off planes: n_coded x max_cmds]
+// Scratch layout per warp: [lit: BS + 32][tok_cmd: max_cmds][tok_mlen: max_cmds][off planes: n_coded x max_cmds]
 __device__ __forceinline__ void bind_scratch(const Params& P, uint32_t warp_global, BlockCtx& c) {
     uint8_t* s = P.scratch + (uint64_t)warp_global * P.scratch_per_warp;
     uint64_t mc = (P.max_cmds + 15u) & ~15u;
     c.lit = s; s += (1ull << P.log2_bs) + 32;
-    c.desc = reinterpret_cast<uint4*>(s); s += 16 * mc;
     c.tok_cmd = s; s += mc;
     c.tok_mlen = s; s += mc;
     c.off_planes = s;
@@ -261,11 +259,71 @@ __device__ __forceinline__ void wait_sources(const Params& P, const BlockCtx& c,
 
 constexpr uint32_t LONG_RUN = 64;   // runs at least this long are copied by the whole warp
 
+struct Stack { Demand* base; uint32_t cap; uint32_t top; /* shared address of the entry count */ };
+
+__device__ __forceinline__ uint32_t lds_top(const Stack& st) { return lds32(st.top); }
+
+__device__ __forceinline__ void push_span(const Params& P, const Stack& st, uint64_t pos, uint64_t len, uint64_t dst) {
+    while (len) {                                   // a demand never crosses a block boundary
+        uint64_t bend = ((pos >> P.log2_bs) + 1) << P.log2_bs;
+        uint64_t n = min((unsigned long long)len, (unsigned long long)(bend - pos));
+        uint32_t idx;
+        asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(idx) : "r"(st.top) : "memory");
+        if (idx < st.cap) { st.base[idx].pos = pos; st.base[idx].dst = dst; st.base[idx].len = n; }
+        else report(P, DF_STACK);
+        pos += n; dst += n; len -= n;
+    }
+}
+
+// n contiguous original bytes from absolute position sp -> dptr (= out2 + dst_off).  Window bytes and resident slots
+// are copied, the rest becomes demands.  WAIT: window sources of a block being decoded in the same launch need flags.
+template <bool WAIT>
+__device__ __forceinline__ void fetch_source(const Params& P, const BlockCtx& c, const Stack& st, uint64_t sp, uint64_t n, uint64_t dst_off) {
+    while (n) {
+        uint64_t m = n;
+        const uint8_t* from = nullptr;
+        if (sp >= P.out_pos0 && sp < P.win_end) {
+            m = min((unsigned long long)n, (unsigned long long)(P.win_end - sp));
+            if (WAIT) for (uint64_t S = sp >> P.log2_bs; S <= (sp + m - 1) >> P.log2_bs; S++) if (S != c.b) wait_block(P, S, __ldg(P.levels + S) < c.d.level);
+            from = P.out + (sp - P.out_pos0);
+        } else {
+            uint64_t next = sp < P.out_pos0 && P.out_pos0 < P.win_end ? P.out_pos0 : ~0ull;   // start of the next known region
+#pragma unroll
+            for (int r = 0; r < MAX_RESIDENT; r++) {
+                if (P.res[r].lo >= P.res[r].hi) continue;
+                if (sp >= P.res[r].lo && sp < P.res[r].hi) { m = min((unsigned long long)n, (unsigned long long)(P.res[r].hi - sp)); from = P.res[r].ptr + (sp - P.res[r].lo); }
+                else if (P.res[r].lo > sp && P.res[r].lo < next) next = P.res[r].lo;
+            }
+            if (!from) m = min((unsigned long long)n, (unsigned long long)(next - sp));
+        }
+        if (from) {
+            uint8_t* d = P.out2 + dst_off;
+            uint64_t left = m; const uint8_t* f = from;
+            while (left) { uint32_t k = (uint32_t)min((unsigned long long)left, 1ull << 30); copy_bytes<true>(d, f, k, ~0ull); d += k; f += k; left -= k; }
+        } else push_span(P, st, sp, m, dst_off);
+        sp += m; dst_off += m; n -= m;
+    }
+}
+
+// source of a match piece: bytes [i, i + n) of the match (dst position md, source src, length mlen) -> out2[dst_off ..)
+template <bool WAIT>
+__device__ __forceinline__ void fetch_match_piece(const Params& P, const BlockCtx& c, const Stack& st, uint64_t md, uint64_t src, uint32_t mlen,
+                                                  uint32_t i, uint32_t n, uint64_t dst_off) {
+    uint64_t period = md - src;
+    if (period >= mlen) { fetch_source<WAIT>(P, c, st, src + i, n, dst_off); return; }
+    uint64_t r = i % period;                       // self-overlap: byte i of the match = seed[i mod period] (FORMAT.md §2)
+    while (n) {
+        uint64_t m = min((unsigned long long)n, (unsigned long long)(period - r));
+        fetch_source<WAIT>(P, c, st, src + r, m, dst_off);
+        dst_off += m; n -= (uint32_t)m; r = 0;
+    }
+}
+
 // A2 + A3 + A4 for a whole block: scan the commands 32 at a time, place literal runs, then resolve the matches.
 // MODE 2: literals only; MODE 0: matches, waiting on literal and completion flags; MODE 4: matches, waiting on
 // completion flags only; MODE 3: matches only, no waits.
-template <int MODE>
-__device__ __forceinline__ void emit_block(const Params& P, const BlockCtx& c) {
+template <int MODE, bool DEMANDS = false>
+__device__ __forceinline__ void emit_block(const Params& P, const BlockCtx& c, const Stack& stk) {
     uint32_t lit_base = 0, out_base = 0, ec = 0, em = c.n_ext_cmd;
     const uint32_t lane = lane_id();
     for (uint32_t c0 = 0; c0 < c.d.n_cmd; c0 += 32) {
@@ -305,6 +363,10 @@ __device__ __forceinline__ void emit_block(const Params& P, const BlockCtx& c) {
         uint64_t dst = out_pos + lit_len, src = (ok && has_match) ? match_src(P, c, ci) : 0;
         bool good = ok && has_match && src < dst;
         if (ok && has_match && !good) report(P, DF_OFFSET);
+        if (MODE == 0 && DEMANDS && good && src < P.out_pos0) {          // the source starts below the window: copy what is here,
+            fetch_match_piece<true>(P, c, stk, dst, src, match_len, 0u, match_len, dst - P.out_pos0);   // demand the rest
+            good = false;
+        }
         if (good && MODE == 0) wait_sources<true>(P, c, dst, src, match_len);
         if (good && MODE == 4) wait_sources<false>(P, c, dst, src, match_len);
         bool is_long = good && match_len >= LONG_RUN && src + match_len <= dst;
@@ -320,35 +382,17 @@ __device__ __forceinline__ void emit_block(const Params& P, const BlockCtx& c) {
     if (out_base != (uint32_t)(c.bend - c.bstart) || lit_base != c.d.n_lit) { if (lane == 0) report(P, DF_LENGTH); }
 }
 
-// ---- A4, output-centric ("chunked") --------------------------------------------------------------------------------
-// Every lane owns one 16-byte aligned chunk of the block's output at a time: it reads the chunk (the literal bytes are
-// already there), finds the matches that overlap it (binary search over the match end positions in shared memory),
-// fetches their source bytes, merges and writes the chunk back with one aligned 16-byte store.  All lanes run the same
-// code whatever the match lengths are, stores are coalesced, and a self-overlapping match is just a gather from its
-// seed with index (i mod period) -- FORMAT.md §2 -- so it needs no serial path.
-// Shared-memory aux area per warp (4 * RUNS_CAP bytes, shared with the run table of the literal phase):
-//   [0, 2 * CHUNK_MATCH_CAP): u16 end_rel - 1 per match      [.., + 4 * CHUNK_WORDS): bitmap of chunks holding match bytes
-constexpr uint32_t CHUNK_MATCH_CAP = 768;
-constexpr uint32_t CHUNK_WORDS = 128;        // 4096 chunks = 64 KB blocks
-static_assert(2 * CHUNK_MATCH_CAP + 4 * CHUNK_WORDS <= 4 * RUNS_CAP, "aux area");
-
-__device__ __forceinline__ uint64_t ones_bytes(uint32_t n) { return n >= 8 ? ~0ull : ((1ull << (8 * n)) - 1); }   // low n bytes set
-
-// WAIT: 0 none, 1 completion flags of lower-level blocks, 2 literal flags too.  Returns false when the block does not
-// fit (caller falls back to the per-match path).
-template <int WAIT>
-__device__ __forceinline__ bool resolve_chunked(const Params& P, const BlockCtx& c, uint32_t aux) {
+// ---- A5-A7: demands ("materialise original bytes [pos, pos+len) at out2[dst..)") ------------------------------------
+// Source bytes that are neither in the current window nor in a resident slot are reconstructed by recursion on their
+// own sources: the block that holds them is parsed and the wanted span is emitted; literal bytes are final, match
+// pieces are forwarded to *their* sources with the same destination.  Recursion depth <= max_level + 1 (FORMAT.md §3).
+// Each warp keeps its pending demands in a private LIFO in the workspace; all pending demands of one block are served
+// from a single parse of that block.
+// Emit the bytes [pos, pos + len) of the parsed block c (tokens + all literals are in the warp's scratch) to out2[dst..).
+__device__ __forceinline__ void emit_span(const Params& P, const BlockCtx& c, const Stack& st, uint64_t pos, uint64_t len, uint64_t dst) {
+    uint32_t lit_base = 0, out_base = 0, ec = 0, em = c.n_ext_cmd;
     const uint32_t lane = lane_id();
-    const uint32_t blk_bytes = (uint32_t)(c.bend - c.bstart);
-    if (c.d.n_match > CHUNK_MATCH_CAP || P.log2_bs > 16 || P.log2_bs < 4) return false;
-    if (c.d.n_match == 0) return true;
-    const uint32_t ends = aux, bitmap = aux + 2 * CHUNK_MATCH_CAP;
-    const uint32_t n_chunks = (blk_bytes + 15) >> 4, n_words = (n_chunks + 31) >> 5;
-    for (uint32_t w = lane; w < n_words; w += 32) asm volatile("st.shared.u32 [%0], %1;" ::"r"(bitmap + 4 * w), "r"(0u) : "memory");
-    __syncwarp();
-    // ---- scan: per match {dst_rel, len, src} to scratch, end to shared memory, chunk bitmap
-    uint32_t out_base = 0, lit_total = 0, ec = 0, em = c.n_ext_cmd;
-    bool bad = false;
+    const uint64_t pend = pos + len;
     for (uint32_t c0 = 0; c0 < c.d.n_cmd; c0 += 32) {
         uint32_t ci = c0 + lane;
         bool valid = ci < c.d.n_cmd, has_match = ci < c.d.n_match;
@@ -358,87 +402,73 @@ __device__ __forceinline__ bool resolve_chunked(const Params& P, const BlockCtx&
         if (valid && tl == 255) lit_len = 255 + __ldg(c.ext + ec + __popc(ml & lanemask_lt()));
         if (has_match && tm == 255) match_len = P.min_match + 255 + __ldg(c.ext + em + __popc(mm & lanemask_lt()));
         ec += __popc(ml); em += __popc(mm);
-        uint32_t st = lit_len + match_len, sl = lit_len;
+        uint32_t sl = lit_len, stt = lit_len + match_len;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
-            uint32_t t = __shfl_up_sync(0xffffffffu, st, o), a = __shfl_up_sync(0xffffffffu, sl, o);
-            if (lane >= (uint32_t)o) { st += t; sl += a; }
+            uint32_t a = __shfl_up_sync(0xffffffffu, sl, o), t = __shfl_up_sync(0xffffffffu, stt, o);
+            if (lane >= (uint32_t)o) { sl += a; stt += t; }
         }
-        uint32_t dst_rel = out_base + st - match_len, end_rel = out_base + st;
-        out_base += __shfl_sync(0xffffffffu, st, 31);
-        lit_total += __shfl_sync(0xffffffffu, sl, 31);
-        if (has_match) {
-            uint64_t src = match_src(P, c, ci);
-            bool okm = end_rel <= blk_bytes && src < c.bstart + dst_rel && src >= P.out_pos0;
-            if (!okm) { bad = true; match_len = 0; end_rel = min(end_rel, blk_bytes); dst_rel = min(dst_rel, end_rel); }
-            c.desc[ci] = make_uint4(dst_rel, match_len, (uint32_t)src, (uint32_t)(src >> 32));
-            asm volatile("st.shared.u16 [%0], %1;" ::"r"(ends + 2 * ci), "h"((uint16_t)(end_rel - 1)) : "memory");
-            if (match_len) for (uint32_t ch = dst_rel >> 4; ch <= (end_rel - 1) >> 4; ch++)
-                asm volatile("red.shared.or.b32 [%0], %1;" ::"r"(bitmap + 4 * (ch >> 5)), "r"(1u << (ch & 31)) : "memory");
-        }
-    }
-    if (__any_sync(0xffffffffu, bad)) { if (lane == 0) report(P, DF_OFFSET); }
-    if (out_base != blk_bytes || lit_total != c.d.n_lit) { if (lane == 0) report(P, DF_LENGTH); return true; }
-    __syncwarp();
-    // ---- chunks
-    uint8_t* out_blk = P.out + (c.bstart - P.out_pos0);
-    for (uint32_t w = 0; w < n_words; w++) {
-        uint32_t word = lds32(bitmap + 4 * w);
-        if (word == 0) continue;
-        if (!((word >> lane) & 1)) continue;                 // divergent from here on; no warp-level primitives below
-        const uint32_t q = (32 * w + lane) << 4;             // chunk start, block-relative
-        const uint32_t nv = min(16u, blk_bytes - q);         // valid bytes (only the file's last chunk can be short)
-        uint64_t lo = 0, hi = 0;
-        if (nv == 16) { uint4 o = __ldcg(reinterpret_cast<const uint4*>(out_blk + q)); lo = (uint64_t)o.x | ((uint64_t)o.y << 32); hi = (uint64_t)o.z | ((uint64_t)o.w << 32); }
-        else for (uint32_t t = 0; t < nv; t++) { uint64_t v = ldcg8(out_blk + q + t); if (t < 8) lo |= v << (8 * t); else hi |= v << (8 * (t - 8)); }
-        uint32_t a0 = 0, b0 = c.d.n_match;                    // first match with end_rel - 1 >= q
-        while (a0 < b0) { uint32_t mid = (a0 + b0) >> 1; if (lds16(ends + 2 * mid) < q) a0 = mid + 1; else b0 = mid; }
-        for (uint32_t m = a0; m < c.d.n_match; m++) {
-            uint4 d = c.desc[m];
-            if (d.x >= q + 16) break;
-            uint32_t pa = max(d.x, q), pb = min(d.x + d.y, q + nv);
-            if (pa >= pb) continue;
-            uint32_t a = pa - q, n = pb - pa, i = pa - d.x;  // chunk byte offset, byte count, offset inside the match
-            uint64_t src = (uint64_t)d.z | ((uint64_t)d.w << 32), dstpos = c.bstart + d.x, period = dstpos - src;
-            if (WAIT) {
-                uint64_t seed_end = min((unsigned long long)(src + d.y), (unsigned long long)dstpos);
-                uint64_t f0 = period >= d.y ? src + i : src, f1 = period >= d.y ? src + i + n : seed_end;
-                for (uint64_t S = f0 >> P.log2_bs; S <= (f1 - 1) >> P.log2_bs; S++) if (S != c.b) {
-                    bool full = __ldg(P.levels + S) < c.d.level;
-                    if (full || WAIT == 2) wait_block(P, S, full);
-                }
+        uint32_t lit_pos = lit_base + sl - lit_len;
+        uint64_t out_pos = c.bstart + out_base + (stt - lit_len - match_len);
+        lit_base += __shfl_sync(0xffffffffu, sl, 31);
+        out_base += __shfl_sync(0xffffffffu, stt, 31);
+        bool ok = valid && (uint64_t)lit_pos + lit_len <= c.d.n_lit && out_pos + lit_len + match_len <= c.bend;
+        if (__any_sync(0xffffffffu, valid && !ok)) { if (lane == 0) report(P, DF_LENGTH); return; }
+        if (c.bstart + out_base <= pos) continue;            // the whole group lies before the span
+        if (ok) {
+            uint64_t a = max((unsigned long long)out_pos, (unsigned long long)pos), b = min((unsigned long long)(out_pos + lit_len), (unsigned long long)pend);
+            if (a < b) copy_bytes<false>(P.out2 + dst + (a - pos), c.lit + lit_pos + (a - out_pos), (uint32_t)(b - a), ~0ull);
+            uint64_t md = out_pos + lit_len;
+            a = max((unsigned long long)md, (unsigned long long)pos); b = min((unsigned long long)(md + match_len), (unsigned long long)pend);
+            if (has_match && a < b) {
+                uint64_t src = match_src(P, c, ci);
+                if (src >= md) report(P, DF_OFFSET);
+                else fetch_match_piece<false>(P, c, st, md, src, match_len, (uint32_t)(a - md), (uint32_t)(b - a), dst + (a - pos));
             }
-            uint64_t vlo, vhi;
-            if (period >= d.y) {                             // non-overlapping: n contiguous source bytes
-                const uint8_t* sp = P.out + (src + i - P.out_pos0);
-                vlo = ld64u<true>(sp, n < 8 ? n : 8);
-                vhi = n > 8 ? ld64u<true>(sp + 8, n - 8) : 0;
-            } else {                                         // self-overlap: byte i of the match = seed[i mod period]
-                vlo = 0; vhi = 0;
-                uint32_t r0 = (uint32_t)(i % period);
-                for (uint32_t t = 0; t < n; t++) {
-                    uint64_t v = ldcg8(P.out + (src + r0 - P.out_pos0));
-                    if (t < 8) vlo |= v << (8 * t); else vhi |= v << (8 * (t - 8));
-                    if (++r0 == period) r0 = 0;
-                }
-            }
-            // place bytes [0, n) of (vlo, vhi) at chunk bytes [a, a + n)
-            uint64_t mlo = ones_bytes(a + n) & ~ones_bytes(a), mhi = (a + n > 8 ? ones_bytes(a + n - 8) : 0) & ~(a > 8 ? ones_bytes(a - 8) : 0);
-            uint64_t slo, shi;
-            if (a == 0) { slo = vlo; shi = vhi; }
-            else if (a < 8) { slo = vlo << (8 * a); shi = (vhi << (8 * a)) | (vlo >> (64 - 8 * a)); }
-            else if (a == 8) { slo = 0; shi = vlo; }
-            else { slo = 0; shi = vlo << (8 * (a - 8)); }
-            lo = (lo & ~mlo) | (slo & mlo);
-            hi = (hi & ~mhi) | (shi & mhi);
         }
-        if (nv == 16) *reinterpret_cast<uint4*>(out_blk + q) = make_uint4((uint32_t)lo, (uint32_t)(lo >> 32), (uint32_t)hi, (uint32_t)(hi >> 32));
-        else for (uint32_t t = 0; t < nv; t++) out_blk[q + t] = (uint8_t)((t < 8 ? lo >> (8 * t) : hi >> (8 * (t - 8))));
+        if (c.bstart + out_base >= pend) break;              // uniform: nothing after this group is wanted
     }
-    __syncwarp();
-    return true;
 }
 
+// Serve every pending demand of the warp's stack (depth-first; all demands of one block from one parse).
+__device__ __forceinline__ void process_demands(const Params& P, uint32_t s_luts, uint32_t ring, BlockCtx& c, const Stack& st) {
+    const uint32_t lane = lane_id();
+    for (;;) {
+        __syncwarp();
+        uint32_t top = min(lds_top(st), st.cap);
+        while (top > 0 && st.base[top - 1].len == 0) top--;  // drop served entries
+        __syncwarp();
+        if (lane == 0) asm volatile("st.shared.u32 [%0], %1;" ::"r"(st.top), "r"(top) : "memory");
+        __syncwarp();
+        if (top == 0) return;
+        c.b = st.base[top - 1].pos >> P.log2_bs;
+        if (c.b >= (P.N + (1ull << P.log2_bs) - 1) >> P.log2_bs) { if (lane == 0) { report(P, DF_OFFSET); st.base[top - 1].len = 0; } continue; }
+        bool ok = parse_block(P, s_luts, ring, c, 0xffffffffu);   // tokens + all literals into the scratch
+        bool found = true;
+        while (found) {                                      // emit_span may push more demands for this same block
+            found = false;
+            uint32_t n = min(lds_top(st), st.cap);
+            for (uint32_t i0 = 0; i0 < n; i0 += 32) {
+                uint32_t idx = i0 + lane;
+                bool mine = idx < n && st.base[idx].len != 0 && (st.base[idx].pos >> P.log2_bs) == c.b;
+                uint32_t m = __ballot_sync(0xffffffffu, mine);
+                while (m) {
+                    uint32_t e = i0 + __ffs(m) - 1; m &= m - 1;
+                    uint64_t pos = st.base[e].pos, len = st.base[e].len, dst = st.base[e].dst;
+                    __syncwarp();
+                    if (lane == 0) st.base[e].len = 0;
+                    __syncwarp();
+                    if (ok) emit_span(P, c, st, pos, len, dst);
+                    found = true;
+                }
+            }
+            __syncwarp();
+        }
+    }
+}
+
+// DEMANDS = false: whole-file schedules (no source can lie outside the output).  true: range / read decode.
+template <bool DEMANDS>
 __global__ void __launch_bounds__(1024, 1) k_decode(const Params P) {
     // shared memory: [pad to 8 KB][tables: n_coded_tables x 8 KB][rings: warps x 2 KB]  (absolute shared addresses)
     extern __shared__ __align__(16) uint8_t smem_raw[];
@@ -456,21 +486,31 @@ __global__ void __launch_bounds__(1024, 1) k_decode(const Params P) {
     const uint32_t runs = s_luts + n_lut_words * 4 + warps_per_cta * RING_BYTES + warp * (4 * RUNS_CAP);
     BlockCtx c;
     bind_scratch(P, blockIdx.x * warps_per_cta + warp, c);
+    Stack st;
+    st.base = P.stacks + (uint64_t)(blockIdx.x * warps_per_cta + warp) * P.stack_cap; st.cap = P.stack_cap;
+    st.top = s_luts + n_lut_words * 4 + warps_per_cta * (RING_BYTES + 4 * RUNS_CAP) + 4 * warp;
+    if (lane_id() == 0) asm volatile("st.shared.u32 [%0], %1;" ::"r"(st.top), "r"(0u) : "memory");
+    __syncwarp();
     for (;;) {
         unsigned long long t = 0;
         if (lane_id() == 0) t = atomicAdd(P.ticket, 1ull);
         t = __shfl_sync(0xffffffffu, t, 0);
         if (t >= P.n_work) break;
+        if (DEMANDS && P.mode == 1) {                        // spans: one top-level demand per ticket
+            if (lane_id() == 0) push_span(P, st, P.demands[t].pos, P.demands[t].len, P.demands[t].dst);
+            process_demands(P, s_luts, ring, c, st);
+            continue;
+        }
         c.b = P.level_list ? (uint64_t)P.level_list[t] : P.first_block + t;
         if (P.mode == 3) {
             // match wave: only the command / length / offset streams are needed again
-            if (parse_block(P, s_luts, ring, c, 0) && !(P.chunked && resolve_chunked<0>(P, c, runs))) emit_block<3>(P, c);
+            if (parse_block(P, s_luts, ring, c, 0)) emit_block<3>(P, c, st);
             continue;
         }
         if (P.mode == 4) {
             // all match waves in one launch: blocks arrive sorted by (level, index), a block waits for the completion
             // of lower-level source blocks, which were dispatched before it
-            if (parse_block(P, s_luts, ring, c, 0) && !(P.chunked && resolve_chunked<1>(P, c, runs))) emit_block<4>(P, c);
+            if (parse_block(P, s_luts, ring, c, 0)) emit_block<4>(P, c, st);
             __threadfence();
             __syncwarp();
             if (lane_id() == 0) st_release(P.flags + c.b, 2 * P.epoch + 1);
@@ -491,7 +531,7 @@ __global__ void __launch_bounds__(1024, 1) k_decode(const Params P) {
                     rans_region<false>(r, s_luts + P.lut_lit * (4 * LUT_SIZE), i0, c.d.n_lit, c.lit);
                     ok = rans_final_ok(P, c, r);
                     __syncwarp();
-                    if (ok) emit_block<2>(P, c);
+                    if (ok) emit_block<2>(P, c, st);
                 }
             }
         }
@@ -499,7 +539,10 @@ __global__ void __launch_bounds__(1024, 1) k_decode(const Params P) {
             __threadfence();
             __syncwarp();
             if (lane_id() == 0) st_release(P.flags + c.b, 2 * P.epoch);       // literals placed
-            if (ok && !(P.chunked && resolve_chunked<2>(P, c, runs))) emit_block<0>(P, c);   // A4 (waits on source blocks)
+            const uint64_t b0 = c.b;
+            if (ok) emit_block<0, DEMANDS>(P, c, st);                         // A4 (waits on source blocks)
+            if (DEMANDS && lds_top(st)) process_demands(P, s_luts, ring, c, st);   // sources below the window (range decode)
+            c.b = b0;
             __threadfence();
             __syncwarp();
             if (lane_id() == 0) st_release(P.flags + c.b, 2 * P.epoch + 1);   // complete (set even on error: nobody waits forever)
@@ -546,9 +589,12 @@ struct aceapex_archive {
     int sms = 148, ctas_per_sm = 1, threads = 1024;
     uint32_t grid = 0; size_t smem = 0;
     uint64_t scratch_per_warp = 0, ctrl_bytes = 0, flags_bytes = 0;
+    uint64_t scratch_off = 0, stacks_off = 0, demands_off = 0, list_off = 0, ws_need = 0;
+    uint32_t stack_cap = 0, demand_cap = 0;
+    std::vector<uint16_t> h_levels;                    // host copy of the per-block levels
+    std::vector<uint32_t> h_list; std::vector<Demand> h_demands;   // host staging for range / read calls
     // status
     int32_t last_cuda = 0; uint32_t dev_flags = 0; uint64_t launches = 0;
-    uint32_t chunked = 0;   // match resolver: 0 = one lane per match, 1 = one lane per 16-byte output chunk
 };
 
 namespace {
@@ -562,8 +608,20 @@ uint16_t rd16(const uint8_t* p) { uint16_t v; memcpy(&v, p, 2); return v; }
 uint64_t align_up(uint64_t v, uint64_t a) { return (v + a - 1) / a * a; }
 
 // workspace: [ctrl 256 B: ticket u64 @0, err u32 @8][flags: n_blocks x u32][scratch: warps x scratch_per_warp]
-uint64_t workspace_need(const aceapex_archive* ar) {
-    return ar->ctrl_bytes + ar->flags_bytes + (uint64_t)ar->grid * (ar->threads / 32) * ar->scratch_per_warp;
+//            [stacks: warps x stack_cap demands][demands: demand_cap][block list: n_blocks x u32]
+uint64_t workspace_need(const aceapex_archive* ar) { return ar->ws_need; }
+
+void layout_workspace(aceapex_archive* ar) {
+    uint64_t warps = (uint64_t)ar->grid * (ar->threads / 32);
+    ar->ctrl_bytes = 256;
+    ar->flags_bytes = align_up(4 * ar->n_blocks + 4, 256);
+    ar->scratch_off = ar->ctrl_bytes + ar->flags_bytes;
+    ar->stack_cap = std::max(1024u, std::min(8192u, 8 * ar->max_cmds));
+    ar->demand_cap = 1u << 16;
+    ar->stacks_off = align_up(ar->scratch_off + warps * ar->scratch_per_warp, 256);
+    ar->demands_off = align_up(ar->stacks_off + warps * ar->stack_cap * sizeof(Demand), 256);
+    ar->list_off = align_up(ar->demands_off + (uint64_t)ar->demand_cap * sizeof(Demand), 256);
+    ar->ws_need = align_up(ar->list_off + 4 * ar->n_blocks + 4, 256);
 }
 
 void fill_params(const aceapex_archive* ar, Params& P) {
@@ -579,10 +637,10 @@ void fill_params(const aceapex_archive* ar, Params& P) {
     P.ticket = reinterpret_cast<unsigned long long*>(ar->d_ws);
     P.err = reinterpret_cast<uint32_t*>(ar->d_ws + 8);
     P.flags = reinterpret_cast<uint32_t*>(ar->d_ws + ar->ctrl_bytes);
-    P.scratch = ar->d_ws + ar->ctrl_bytes + ar->flags_bytes;
+    P.scratch = ar->d_ws + ar->scratch_off;
     P.scratch_per_warp = ar->scratch_per_warp; P.max_cmds = ar->max_cmds;
-    P.clip_lo = 0; P.clip_hi = ar->N;
-    P.chunked = ar->chunked;
+    P.out_pos0 = 0; P.win_end = ar->N;
+    P.stacks = reinterpret_cast<Demand*>(ar->d_ws + ar->stacks_off); P.stack_cap = ar->stack_cap;
 }
 
 int32_t prepare_ws(aceapex_archive* ar) {
@@ -600,7 +658,8 @@ int32_t launch(aceapex_archive* ar, Params& P, uint64_t n_work) {
     CU(cudaMemsetAsync(P.ticket, 0, 8, ar->stream));
     uint64_t warps = ar->threads / 32;
     uint32_t grid = (uint32_t)std::min<uint64_t>(ar->grid, (n_work + warps - 1) / warps);
-    k_decode<<<grid, ar->threads, ar->smem, ar->stream>>>(P);
+    if (P.mode == 1 || P.out_pos0 != 0 || P.win_end != ar->N) k_decode<true><<<grid, ar->threads, ar->smem, ar->stream>>>(P);
+    else k_decode<false><<<grid, ar->threads, ar->smem, ar->stream>>>(P);
     CU(cudaGetLastError());
     ar->launches++;
     return ACEAPEX_OK;
@@ -697,7 +756,8 @@ int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* 
         CU(cudaMemcpy(ar->d_luts, luts.data(), luts.size() * 4, cudaMemcpyHostToDevice));
     }
     if (ar->n_blocks) {
-        std::vector<uint16_t> lv(ar->n_blocks);
+        std::vector<uint16_t>& lv = ar->h_levels;
+        lv.resize(ar->n_blocks);
         for (uint64_t b = 0; b < ar->n_blocks; b++) lv[b] = rd16(meta + ar->dir_off + 32 * b + 28);
         CU(cudaMalloc(&ar->d_levels, lv.size() * 2));
         CU(cudaMemcpy(ar->d_levels, lv.data(), lv.size() * 2, cudaMemcpyHostToDevice));
@@ -713,20 +773,20 @@ int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* 
     CU(cudaGetDevice(&dev)); CU(cudaGetDeviceProperties(&prop, dev));
     ar->sms = prop.multiProcessorCount;
     ar->threads = 1024;   // one CTA per SM: the decode tables are staged once per SM, 32 warps share them
-    ar->smem = 8192 + (size_t)ar->n_coded_tables * LUT_SIZE * 4 + (size_t)(ar->threads / 32) * (RING_BYTES + 4 * RUNS_CAP);
-    CU(cudaFuncSetAttribute(k_decode, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ar->smem));
-    CU(cudaFuncSetAttribute(k_decode, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+    ar->smem = 8192 + (size_t)ar->n_coded_tables * LUT_SIZE * 4 + (size_t)(ar->threads / 32) * (RING_BYTES + 4 * RUNS_CAP + 4);
+    CU(cudaFuncSetAttribute(k_decode<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ar->smem));
+    CU(cudaFuncSetAttribute(k_decode<false>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+    CU(cudaFuncSetAttribute(k_decode<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ar->smem));
+    CU(cudaFuncSetAttribute(k_decode<true>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
     int occ = 0;
-    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_decode, ar->threads, ar->smem));
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_decode<true>, ar->threads, ar->smem));
     if (occ < 1) return ACEAPEX_E_CUDA;
-    if (const char* e = getenv("ACEAPEX_CHUNKED")) ar->chunked = atoi(e) != 0;
     if (const char* e = getenv("ACEAPEX_CTAS_PER_SM")) occ = std::max(1, std::min(occ, atoi(e)));
     ar->ctas_per_sm = occ;
     ar->grid = (uint32_t)(ar->sms * occ);
     uint64_t mc = align_up(ar->max_cmds, 16);
-    ar->scratch_per_warp = align_up((1ull << ar->log2_bs) + 32 + mc * (16 + 2 + ar->n_coded_planes), 256);
-    ar->ctrl_bytes = 256;
-    ar->flags_bytes = align_up(4 * ar->n_blocks + 4, 256);
+    ar->scratch_per_warp = align_up((1ull << ar->log2_bs) + 32 + mc * (2 + ar->n_coded_planes), 256);
+    layout_workspace(ar);
     guard.a = nullptr;
     *out = ar;
     return ACEAPEX_OK;
@@ -805,11 +865,70 @@ int32_t aceapex_decode_all_levels(aceapex_archive* ar, void* d_out) {
     return ACEAPEX_OK;
 }
 
+// launches span-mode work for the demands staged in ar->h_demands (in batches of demand_cap)
+static int32_t run_demands(aceapex_archive* ar, Params& P) {
+    Demand* d_dem = reinterpret_cast<Demand*>(ar->d_ws + ar->demands_off);
+    P.mode = 1; P.level_list = nullptr; P.demands = d_dem;
+    for (size_t i = 0; i < ar->h_demands.size(); i += ar->demand_cap) {
+        size_t n = std::min<size_t>(ar->demand_cap, ar->h_demands.size() - i);
+        CU(cudaMemcpyAsync(d_dem, ar->h_demands.data() + i, n * sizeof(Demand), cudaMemcpyHostToDevice, ar->stream));
+        int32_t rc = launch(ar, P, n);
+        if (rc) return rc;
+        if (i + n < ar->h_demands.size()) CU(cudaStreamSynchronize(ar->stream));   // the staging area is reused
+    }
+    return ACEAPEX_OK;
+}
+
+static void add_demands(aceapex_archive* ar, uint64_t pos, uint64_t len, uint64_t dst) {
+    while (len) {
+        uint64_t bend = ((pos >> ar->log2_bs) + 1) << ar->log2_bs, n = std::min(len, bend - pos);
+        ar->h_demands.push_back(Demand{pos, dst, n});
+        pos += n; dst += n; len -= n;
+    }
+}
+
 int32_t aceapex_decode_range(aceapex_archive* ar, uint64_t lo, uint64_t hi, void* d_out, uint64_t budget) {
-    (void)d_out; (void)budget;
     if (!ar) return ACEAPEX_E_ARG;
     if (lo > hi || hi > ar->N) return ACEAPEX_E_RANGE;
-    return ACEAPEX_E_ARG;   // implemented in a later commit
+    if (lo == hi) return ACEAPEX_OK;
+    if (!d_out) return ACEAPEX_E_ARG;
+    if (budget && budget < workspace_need(ar)) return ACEAPEX_E_BUDGET;
+    int32_t rc = prepare_ws(ar);
+    if (rc) return rc;
+    const uint64_t BS = 1ull << ar->log2_bs;
+    // whole blocks [alo, ahi) are decoded as a window (flag-driven schedule); the ragged ends are spans
+    uint64_t alo = (lo + BS - 1) & ~(BS - 1), ahi = hi == ar->N ? hi : hi & ~(BS - 1);
+    Params P; fill_params(ar, P);
+    uint8_t* out = static_cast<uint8_t*>(d_out);
+    P.out2 = out; P.out_pos0 = 0; P.win_end = 0; P.out = out;
+    if (alo < ahi) {
+        uint64_t b0 = alo >> ar->log2_bs, b1 = (ahi + BS - 1) >> ar->log2_bs, nb = b1 - b0;
+        // blocks of the window sorted by (level, index): counting sort on the host copy of the levels
+        std::vector<uint32_t>& L = ar->h_list;
+        L.resize(nb);
+        std::vector<uint64_t> cnt(ar->max_level + 2, 0);
+        for (uint64_t b = b0; b < b1; b++) cnt[ar->h_levels[b] + 1]++;
+        for (size_t l = 1; l < cnt.size(); l++) cnt[l] += cnt[l - 1];
+        for (uint64_t b = b0; b < b1; b++) L[cnt[ar->h_levels[b]]++] = (uint32_t)b;
+        uint32_t* d_list = reinterpret_cast<uint32_t*>(ar->d_ws + ar->list_off);
+        CU(cudaMemcpyAsync(d_list, L.data(), nb * 4, cudaMemcpyHostToDevice, ar->stream));
+        P.mode = 0; P.level_list = d_list; P.epoch = ++ar->epoch;
+        P.out = out + (alo - lo); P.out2 = P.out; P.out_pos0 = alo; P.win_end = ahi;
+        if ((rc = launch(ar, P, nb))) return rc;
+    }
+    ar->h_demands.clear();
+    if (alo >= ahi) add_demands(ar, lo, hi - lo, 0);
+    else {
+        if (lo < alo) add_demands(ar, lo, alo - lo, 0);
+        if (ahi < hi) add_demands(ar, ahi, hi - ahi, ahi - lo);
+    }
+    if (!ar->h_demands.empty()) {
+        P.out2 = out;          // demand destinations are offsets into d_out; the decoded window is readable as a source
+        CU(cudaStreamSynchronize(ar->stream));   // h_list / earlier staging must be consumed before reuse (small ranges only)
+        if ((rc = run_demands(ar, P))) return rc;
+        CU(cudaStreamSynchronize(ar->stream));   // h_demands is host staging
+    }
+    return ACEAPEX_OK;
 }
 
 int32_t aceapex_reads_bytes(const uint64_t* idx, uint64_t n_index, const uint64_t* ids, uint64_t n, uint64_t* total, uint64_t* offs) {
@@ -826,9 +945,25 @@ int32_t aceapex_reads_bytes(const uint64_t* idx, uint64_t n_index, const uint64_
 }
 
 int32_t aceapex_decode_reads(aceapex_archive* ar, const uint64_t* idx, uint64_t n_index, const uint64_t* ids, uint64_t n, void* d_out) {
-    (void)idx; (void)n_index; (void)ids; (void)n; (void)d_out;
-    if (!ar) return ACEAPEX_E_ARG;
-    return ACEAPEX_E_ARG;   // implemented in a later commit
+    if (!ar || (!idx && n_index) || (!ids && n)) return ACEAPEX_E_ARG;
+    if (n == 0) return ACEAPEX_OK;
+    if (!d_out) return ACEAPEX_E_ARG;
+    int32_t rc = prepare_ws(ar);
+    if (rc) return rc;
+    ar->h_demands.clear();
+    uint64_t off = 0;
+    for (uint64_t i = 0; i < n; i++) {               // index lookup: O(1) per read
+        if (ids[i] >= n_index) return ACEAPEX_E_RANGE;
+        uint64_t e = idx[ids[i]], pos = e & ((1ull << 40) - 1), len = e >> 40;
+        if (pos + len > ar->N) return ACEAPEX_E_RANGE;
+        add_demands(ar, pos, len, off);
+        off += len;
+    }
+    Params P; fill_params(ar, P);
+    P.out = static_cast<uint8_t*>(d_out); P.out2 = P.out; P.out_pos0 = 0; P.win_end = 0;
+    if ((rc = run_demands(ar, P))) return rc;
+    CU(cudaStreamSynchronize(ar->stream));           // h_demands is host staging; the call returns the reads
+    return ACEAPEX_OK;
 }
 
 int32_t aceapex_set_resident(aceapex_archive* ar, uint32_t slot, uint64_t lo, uint64_t hi, const void* p) {

@@ -22,7 +22,8 @@ struct DirEntry {            // FORMAT.md §1.3, 32 bytes
 
 struct Resident { uint64_t lo, hi; const uint8_t* ptr; };
 
-struct Demand { uint64_t pos; uint64_t dst; uint32_t len; uint32_t pad; };   // dst = byte offset into Params::out2
+// "materialise original bytes [pos, pos + len) at out2[dst ..)"; never crosses a block boundary; len == 0: served
+struct Demand { uint64_t pos; uint64_t dst; uint64_t len; };
 
 struct Params {
     const uint8_t* archive;      // device archive
@@ -39,19 +40,19 @@ struct Params {
     // work
     uint64_t first_block, n_work;       // FULL mode: blocks [first_block, first_block + n_work)
     uint8_t* out;                        // FULL mode: byte at absolute position p is out[p - out_pos0]
-    uint64_t out_pos0;                   // absolute position of out[0]  (window start, block aligned)
-    uint64_t clip_lo, clip_hi;           // only bytes of [clip_lo, clip_hi) are stored (unaligned range ends)
-    const Demand* demands; uint64_t n_demands; uint8_t* out2;    // SPAN mode top-level work
+    uint64_t out_pos0, win_end;          // out holds the original bytes [out_pos0, win_end) (the window; block aligned start)
+    const Demand* demands; uint8_t* out2; // span mode (1): top-level work items, destination buffer of every demand
     Resident res[MAX_RESIDENT];
     // workspace
     uint32_t* flags;                     // per block: 2 * epoch = literals placed, 2 * epoch + 1 = complete
     uint32_t epoch;
     unsigned long long* ticket;
     uint32_t* err;
-    uint8_t* scratch; uint64_t scratch_per_warp; uint32_t max_cmds; uint32_t stack_cap;
-    uint32_t mode;                       // 0 = everything with flags, 2 = literal launch, 3 = match wave, 4 = all match waves with flags
+    uint8_t* scratch; uint64_t scratch_per_warp; uint32_t max_cmds;
+    Demand* stacks; uint32_t stack_cap;  // per-warp LIFO of pending demands
+    uint32_t mode;                       // 0 = whole blocks with flags, 1 = spans (demands), 2 = literal launch, 3 = match wave,
+                                         // 4 = all match waves with flags
     const uint32_t* level_list;          // block ids to process (n_work entries), null = first_block + i
-    uint32_t chunked;                    // match resolver: 0 = lane per match, 1 = lane per 16-byte output chunk
 };
 
 __device__ __forceinline__ uint32_t lane_id() { return threadIdx.x & 31; }

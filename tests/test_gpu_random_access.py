@@ -1,0 +1,165 @@
+"""decode_range / decode_reads (§4): bit-exact against slices of the ORIGINAL bytes and against the
+oracle's whole-file output."""
+import numpy as np
+import pytest
+import torch
+
+from acx_build import build
+from oracle import acx_oracle as O
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def fq(fastq_4m, fastq_4m_archive):
+    from paper_2606_18900_b200.aceapex import Archive
+    ar = Archive(fastq_4m_archive)
+    yield ar, fastq_4m
+    ar.close()
+
+
+@pytest.fixture(scope="module")
+def fa(fasta_2m, fasta_2m_archive):
+    from paper_2606_18900_b200.aceapex import Archive
+    ar = Archive(fasta_2m_archive)
+    yield ar, fasta_2m
+    ar.close()
+
+
+def check_range(ar, x, lo, hi):
+    got = ar.decode_range(lo, hi)
+    ar.check()
+    assert got.cpu().numpy().tobytes() == x[lo:hi].tobytes(), (lo, hi)
+
+
+def test_ranges_fastq(fq):
+    ar, x = fq
+    N = x.size
+    rng = np.random.default_rng(0)
+    cases = [(0, 0), (5, 5), (0, 1), (N - 1, N), (0, N), (16384, 32768), (16383, 16385), (100, 200), (1, N - 1),
+             (N - 40000, N), (3 * 16384, 3 * 16384 + 1), (16384 * 100 + 7, 16384 * 101 - 9)]
+    for _ in range(12):
+        lo = int(rng.integers(0, N))
+        hi = int(min(N, lo + rng.integers(0, 400000)))
+        cases.append((lo, hi))
+    for lo, hi in cases:
+        check_range(ar, x, lo, hi)
+
+
+def test_ranges_far_from_start_need_sources_before_lo(fq):
+    ar, x = fq
+    N = x.size
+    # the last quarter of the file reads from everywhere before it
+    check_range(ar, x, 3 * N // 4 + 123, N - 77)
+    check_range(ar, x, N // 2, N // 2 + 5 * 16384)
+
+
+def test_ranges_fasta(fa):
+    ar, x = fa
+    N = x.size
+    rng = np.random.default_rng(1)
+    for _ in range(10):
+        lo = int(rng.integers(0, N))
+        hi = int(min(N, lo + rng.integers(1, 300000)))
+        check_range(ar, x, lo, hi)
+    check_range(ar, x, 0, N)
+
+
+def test_range_errors(fq):
+    from paper_2606_18900_b200.aceapex import AceapexError
+    ar, x = fq
+    with pytest.raises(AceapexError) as e:
+        ar.decode_range(10, 5)
+    assert e.value.name == "E_RANGE"
+    with pytest.raises(AceapexError) as e:
+        ar.decode_range(0, x.size + 1)
+    assert e.value.name == "E_RANGE"
+    with pytest.raises(AceapexError) as e:
+        ar.decode_range(0, 100, vram_budget=4096)
+    assert e.value.name == "E_BUDGET"
+
+
+def test_reads_fastq(fq):
+    from paper_2606_18900_b200 import datagen
+    ar, x = fq
+    idx = datagen.fastq_index(x.size)
+    rng = np.random.default_rng(2)
+    for n in (1, 2, 33, 4096):
+        ids = rng.integers(0, idx.size, n).astype(np.uint64)
+        ids[-1] = ids[0]                                # a duplicate
+        total, offs = ar.reads_bytes(idx, ids)
+        got = ar.decode_reads(idx, ids).cpu().numpy()
+        ar.check()
+        for k, r in enumerate(ids):
+            o, ln = int(idx[r] & np.uint64((1 << 40) - 1)), int(idx[r] >> np.uint64(40))
+            assert got[int(offs[k]):int(offs[k]) + ln].tobytes() == x[o:o + ln].tobytes()
+        assert total == int(offs[-1])
+    # first and last read, and a read that crosses a block boundary
+    off = (idx & np.uint64((1 << 40) - 1)).astype(np.int64)
+    ln = (idx >> np.uint64(40)).astype(np.int64)
+    crossing = np.nonzero((off >> 14) != ((off + ln - 1) >> 14))[0][:5]
+    ids = np.concatenate([[0, idx.size - 1], crossing]).astype(np.uint64)
+    got = ar.decode_reads(idx, ids).cpu().numpy()
+    exp = np.concatenate([x[off[i]:off[i] + ln[i]] for i in ids.astype(np.int64)])
+    assert got[:exp.size].tobytes() == exp.tobytes()
+
+
+def test_reads_regions_fasta(fa):
+    from paper_2606_18900_b200 import datagen
+    ar, x = fa
+    idx = datagen.region_index(3, x.size, 5000, 150)
+    ids = np.arange(5000, dtype=np.uint64)
+    got = ar.decode_reads(idx, ids).cpu().numpy()
+    ar.check()
+    off = (idx & np.uint64((1 << 40) - 1)).astype(np.int64)
+    exp = np.concatenate([x[o:o + 150] for o in off])
+    assert got[:exp.size].tobytes() == exp.tobytes()
+
+
+def test_reads_errors(fq):
+    from paper_2606_18900_b200 import datagen
+    from paper_2606_18900_b200.aceapex import AceapexError
+    ar, x = fq
+    idx = datagen.fastq_index(x.size)
+    with pytest.raises(AceapexError) as e:
+        ar.decode_reads(idx, np.array([idx.size], dtype=np.uint64))
+    assert e.value.name == "E_RANGE"
+
+
+def test_resident_window_serves_as_source(fq):
+    """PAPER.md:107-109 §5: consecutive windows through a ring; an earlier window stays resident as a match source."""
+    ar, x = fq
+    W = 64 * 16384
+    ring = [ar.new_output(W) for _ in range(2)]
+    for w in range(x.size // W):
+        buf = ring[w % 2]
+        ar.set_resident(w % 2, 0, 0, None)          # this buffer is about to be overwritten: no longer a source
+        got = ar.decode_range(w * W, (w + 1) * W, out=buf)
+        ar.check()
+        assert torch.equal(got.cpu(), torch.from_numpy(x[w * W:(w + 1) * W]))
+        ar.set_resident(w % 2, w * W, (w + 1) * W, buf)
+    ar.set_resident(0, 0, 0, None)
+    ar.set_resident(1, 0, 0, None)
+
+
+HAND = [
+    ([[(b"a", (0, 7))], [(b"", (7, 8))], [(b"", (15, 8))], [(b"", (23, 3))]], 27, 3, dict(min_match=3, levels=[0, 1, 2, 3])),
+    ([[(b"abc", (0, 10)), (b"XYZ", None)], [(b"", (1, 9)), (b"0123456", None)]], 32, 4, dict(levels=[0, 1])),
+    ([[(b"01234567", None)], [(b"89ab", (6, 4))], [(b"", (6, 5)), (b"!!!", None)]], 24, 3, {}),
+    ([[(b"ABCDEFGH", None)], [(b"", (0, 8))], [(b"", (8, 8))]], 24, 3, dict(levels=[0, 0, 1])),
+]
+
+
+@pytest.mark.parametrize("case", range(len(HAND)))
+def test_hand_built_every_range(case):
+    from paper_2606_18900_b200.aceapex import Archive
+    blocks, N, lb, kw = HAND[case]
+    a = build(blocks, N, lb, **kw)
+    exp = O.decode(a).tobytes()
+    ar = Archive(a)
+    for lo in range(0, N + 1):
+        for hi in range(lo, N + 1, 3):
+            got = ar.decode_range(lo, hi).cpu().numpy().tobytes()[:hi - lo]
+            assert got == exp[lo:hi], (lo, hi)
+    ar.check()
+    ar.close()
