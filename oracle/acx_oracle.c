@@ -36,7 +36,7 @@ static int parse_header(const uint8_t* a, uint64_t n, hdr_t* h) {
     static const uint8_t magic[8] = {0x41, 0x43, 0x58, 0x42, 0x32, 0x30, 0x30, 0x00};
     if (n < 160) return E_TRUNCATED;
     if (memcmp(a, magic, 8)) return E_MAGIC;
-    if (rd32(a + 8) != 1) return E_VERSION;
+    if (rd32(a + 8) != 2) return E_VERSION;
     if (rd32(a + 12) != 160) return E_CORRUPT;
     h->N = rd64(a + 16); h->n_blocks = rd64(a + 24);
     h->log2_bs = rd32(a + 32); h->min_match = rd32(a + 36); h->W = rd32(a + 40); h->prob_bits = rd32(a + 44);
@@ -96,27 +96,28 @@ static int read_dir(const uint8_t* a, const hdr_t* h, uint64_t b, dir_t* d, uint
     return OK;
 }
 
-/* FORMAT.md §1.5: decode n_sym symbols; tid[i] = table of symbol i.  Scalar loop over symbols, 32 states.
- * Returns OK, or E_TRUNCATED when more than n_words words would be consumed. */
+/* FORMAT.md §1.5: decode n_sym symbols; tid[i] = table of symbol i.  Scalar loop over symbols, 32 states; state k
+ * renormalises from its own stream words[word_off[k] .. word_off[k+1]) (word_off has 33 entries).  used[k] = number of
+ * words state k consumed.  Returns OK, or E_TRUNCATED when a state would read past the end of its stream. */
 static int rans_decode(const table_t* T, const uint8_t* tid, uint64_t n_sym, uint32_t prob_bits, uint32_t X[32],
-                       const uint8_t* words, uint64_t n_words, uint8_t* sym, uint64_t* words_used) {
+                       const uint8_t* words, const uint64_t word_off[33], uint8_t* sym, uint64_t used[32]) {
     uint32_t M = 1u << prob_bits;
-    uint64_t wp = 0;
+    for (int k = 0; k < 32; k++) used[k] = 0;
     for (uint64_t i = 0; i < n_sym; i++) {
+        int k = (int)(i & 31);
         const table_t* t = &T[tid[i]];
-        uint32_t x = X[i & 31];
+        uint32_t x = X[k];
         uint32_t slot = x & (M - 1);
         int s = t->sym_of_slot[slot];
         x = t->freq[s] * (x >> prob_bits) + slot - t->cum[s];
         if (x < (1u << 16)) {
-            if (wp >= n_words) return E_TRUNCATED;
-            x = (x << 16) | rd16(words + 2 * wp);
-            wp++;
+            if (word_off[k] + used[k] >= word_off[k + 1]) return E_TRUNCATED;
+            x = (x << 16) | rd16(words + 2 * (word_off[k] + used[k]));
+            used[k]++;
         }
-        X[i & 31] = x;
+        X[k] = x;
         sym[i] = (uint8_t)s;
     }
-    *words_used = wp;
     return OK;
 }
 
@@ -157,7 +158,7 @@ static int decode_streams(const uint8_t* a, const hdr_t* h, const table_t* T, co
     int rc = ensure(s, d->n_cmd, d->n_lit, n_sym);
     if (rc) return rc;
     /* payload geometry */
-    uint64_t rans_bytes = 128 + 2ull * d->n_words;
+    uint64_t rans_bytes = 256 + 2ull * d->n_words;   /* head: 32 x (state, word_off) */
     uint64_t ext_off = d->payload_off + ((rans_bytes + 3) & ~3ull);
     uint64_t raw_off = ext_off + 4ull * d->n_ext;
     uint64_t need = raw_off + (uint64_t)n_raw * d->n_match;
@@ -168,13 +169,15 @@ static int decode_streams(const uint8_t* a, const hdr_t* h, const table_t* T, co
     for (uint32_t i = 0; i < d->n_match; i++) s->tid[k++] = 1;
     for (int p = (int)W - 1; p >= 0; p--) if (T[2 + p].mode == 0) for (uint32_t i = 0; i < d->n_match; i++) s->tid[k++] = (uint8_t)(2 + p);
     for (uint32_t i = 0; i < d->n_lit; i++) s->tid[k++] = (uint8_t)(2 + W);
-    uint32_t X[32];
-    for (int j = 0; j < 32; j++) X[j] = rd32(a + d->payload_off + 4 * j);
+    uint32_t X[32]; uint64_t woff[33], used[32];
+    for (int j = 0; j < 32; j++) { X[j] = rd32(a + d->payload_off + 8 * j); woff[j] = rd32(a + d->payload_off + 8 * j + 4); }
+    woff[32] = d->n_words;
+    if (woff[0] != 0) return E_CORRUPT;
+    for (int j = 0; j < 32; j++) if (woff[j] > woff[j + 1]) return E_CORRUPT;
     for (int j = 0; j < 32; j++) if (X[j] < (1u << 16)) return E_CORRUPT;
-    uint64_t used = 0;
-    rc = rans_decode(T, s->tid, n_sym, h->prob_bits, X, a + d->payload_off + 128, d->n_words, s->sym, &used);
+    rc = rans_decode(T, s->tid, n_sym, h->prob_bits, X, a + d->payload_off + 256, woff, s->sym, used);
     if (rc) return rc;
-    if (used != d->n_words) return E_CORRUPT;
+    for (int j = 0; j < 32; j++) if (used[j] != woff[j + 1] - woff[j]) return E_CORRUPT; /* every stream fully consumed */
     for (int j = 0; j < 32; j++) if (X[j] != (1u << 16)) return E_CORRUPT; /* encoder started every state at 2^16 */
     /* split */
     k = 0;
@@ -330,9 +333,9 @@ int acx_oracle_block(const uint8_t* a, uint64_t n, uint64_t b, uint32_t* counts,
 }
 
 /* The rANS step alone (FORMAT.md §1.5), for the rANS pins: freq is n_tables x 256 u16 (each row sums to 2^prob_bits).
- * states: 32 initial states in, final states out. */
+ * states: 32 initial states in, final states out.  word_off: 33 entries (u64); words_used: 32 entries out. */
 int acx_oracle_rans(const uint16_t* freq, uint32_t n_tables, uint32_t prob_bits, const uint8_t* tid, uint64_t n_sym,
-                    uint32_t* states, const uint8_t* words, uint64_t n_words, uint8_t* sym, uint64_t* words_used) {
+                    uint32_t* states, const uint8_t* words, const uint64_t* word_off, uint8_t* sym, uint64_t* words_used) {
     if (n_tables > 11) return E_RANGE;
     table_t T[11];
     for (uint32_t t = 0; t < n_tables; t++) {
@@ -341,7 +344,8 @@ int acx_oracle_rans(const uint16_t* freq, uint32_t n_tables, uint32_t prob_bits,
         if (sum != (1u << prob_bits) || prob_bits > 11) return E_CORRUPT;
         fill_slots(&T[t]);
     }
-    return rans_decode(T, tid, n_sym, prob_bits, states, words, n_words, sym, words_used);
+    for (int k = 0; k < 32; k++) if (word_off[k] > word_off[k + 1]) return E_CORRUPT;
+    return rans_decode(T, tid, n_sym, prob_bits, states, words, word_off, sym, words_used);
 }
 
 /* FNV-1a 64 (FORMAT.md §5; "FNV for device-resident GPU paths"). */

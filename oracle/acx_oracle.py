@@ -42,7 +42,7 @@ def _load():
         _lib.acx_oracle_decode.argtypes = [p, u64, p, u64, ctypes.c_int]
         _lib.acx_oracle_decode_prefix.argtypes = [p, u64, p, u64, ctypes.c_int, u64]
         _lib.acx_oracle_block.argtypes = [p, u64, u64] + [p] * 9
-        _lib.acx_oracle_rans.argtypes = [p, ctypes.c_uint32, ctypes.c_uint32, p, u64, p, p, u64, p, p]
+        _lib.acx_oracle_rans.argtypes = [p, ctypes.c_uint32, ctypes.c_uint32, p, u64, p, p, p, p, p]
         _lib.acx_oracle_fnv1a64.argtypes = [p, u64]
         _lib.acx_oracle_fnv1a64.restype = u64
     return _lib
@@ -105,20 +105,23 @@ def block(archive, b):
     return r
 
 
-def rans_decode(freq, tid, states, words, prob_bits=11):
-    """FORMAT.md §1.5 alone.  freq: (n_tables, 256) u16; tid: table id per symbol; states: 32 u32; words: u16 array.
-    Returns (symbols, final_states, words_used)."""
+def rans_decode(freq, tid, states, streams, prob_bits=11):
+    """FORMAT.md §1.5 alone.  freq: (n_tables, 256) u16; tid: table id per symbol; states: 32 u32; streams: 32 lists of
+    u16 words (state k's own stream).  Returns (symbols, final_states, words_used[32])."""
     freq = np.ascontiguousarray(freq, dtype=np.uint16).reshape(-1, 256)
     tid = np.ascontiguousarray(tid, dtype=np.uint8)
     st = np.ascontiguousarray(states, dtype=np.uint32).copy()
-    w = np.ascontiguousarray(words, dtype="<u2")
+    assert len(streams) == 32
+    off = np.zeros(33, dtype=np.uint64)
+    off[1:] = np.cumsum([len(s) for s in streams])
+    w = np.ascontiguousarray(np.concatenate([np.asarray(s, dtype="<u2") for s in streams] + [np.zeros(1, "<u2")]))
     sym = np.zeros(max(tid.size, 1), dtype=np.uint8)
-    used = ctypes.c_uint64()
+    used = np.zeros(32, dtype=np.uint64)
     rc = _load().acx_oracle_rans(freq.ctypes.data, freq.shape[0], prob_bits, tid.ctypes.data, tid.size, st.ctypes.data,
-                                 w.ctypes.data, w.size, sym.ctypes.data, ctypes.byref(used))
+                                 w.ctypes.data, off.ctypes.data, sym.ctypes.data, used.ctypes.data)
     if rc:
         raise OracleError(rc)
-    return sym[:tid.size], st, used.value
+    return sym[:tid.size], st, used.astype(np.int64)
 
 
 def fnv1a64(data):

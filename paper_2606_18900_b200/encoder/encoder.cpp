@@ -235,20 +235,20 @@ struct Out {
     void pad(size_t a) { while (b.size() % a) b.push_back(0); }
 };
 
-// rANS-encode the block's symbol sequence (FORMAT.md §1.5); returns states + words
+// rANS-encode the block's symbol sequence (FORMAT.md §1.5); returns the 32 initial decoder states and, per state, its
+// own word stream in the order the decoder consumes it
 void rans_block(const std::vector<uint8_t>& sym, const std::vector<uint8_t>& tid, const std::vector<Table>& T,
-                uint32_t X[32], std::vector<uint16_t>& words) {
-    for (int k = 0; k < 32; k++) X[k] = RANS_L;
-    words.clear();
+                uint32_t X[32], std::vector<uint16_t> words[32]) {
+    for (int k = 0; k < 32; k++) { X[k] = RANS_L; words[k].clear(); }
     for (size_t i = sym.size(); i-- > 0;) {
         const Table& t = T[tid[i]];
         uint32_t f = t.freq[sym[i]], c = t.cum[sym[i]];
         uint32_t& xs = X[i & 31];
         uint32_t xv = xs;
-        if ((uint64_t)xv >= ((uint64_t)f << (32 - PROB_BITS))) { words.push_back((uint16_t)(xv & 0xffff)); xv >>= 16; }
+        if ((uint64_t)xv >= ((uint64_t)f << (32 - PROB_BITS))) { words[i & 31].push_back((uint16_t)(xv & 0xffff)); xv >>= 16; }
         xs = ((xv / f) << PROB_BITS) + (xv % f) + c;
     }
-    std::reverse(words.begin(), words.end());
+    for (int k = 0; k < 32; k++) std::reverse(words[k].begin(), words[k].end());
 }
 
 } // namespace
@@ -358,17 +358,18 @@ int acx_encode(const uint8_t* in, uint64_t N, const acx_enc_opts* uo, uint8_t** 
         for (int p = (int)W - 1; p >= 0; p--) if (T[2 + p].mode == 0)
             for (uint64_t v : B.off) { sym.push_back((uint8_t)(v >> (8 * p))); tid.push_back((uint8_t)(2 + p)); }
         for (uint8_t v : B.lit) { sym.push_back(v); tid.push_back((uint8_t)(2 + W)); }
-        uint32_t X[32]; std::vector<uint16_t> words;
+        uint32_t X[32]; std::vector<uint16_t> words[32];
         rans_block(sym, tid, T, X, words);
         Out o2;
-        for (int k = 0; k < 32; k++) o2.u32(X[k]);
-        for (uint16_t w : words) { o2.b.push_back((uint8_t)w); o2.b.push_back((uint8_t)(w >> 8)); }
+        uint32_t woff = 0;
+        for (int k = 0; k < 32; k++) { o2.u32(X[k]); o2.u32(woff); woff += (uint32_t)words[k].size(); }   // head
+        for (int k = 0; k < 32; k++) for (uint16_t w : words[k]) { o2.b.push_back((uint8_t)w); o2.b.push_back((uint8_t)(w >> 8)); }
         o2.pad(4);
         for (uint32_t v : B.ext_cmd) o2.u32(v);
         for (uint32_t v : B.ext_mlen) o2.u32(v);
         for (uint32_t p = 0; p < W; p++) if (T[2 + p].mode == 1) for (uint64_t v : B.off) o2.b.push_back((uint8_t)(v >> (8 * p)));
         o2.pad(16);
-        pay[bi].swap(o2.b); n_words[bi] = (uint32_t)words.size();
+        pay[bi].swap(o2.b); n_words[bi] = woff;
         uint64_t h = 0xcbf29ce484222325ull, a = bi * e.BS, b = std::min(N, a + e.BS);
         for (uint64_t q = a; q < b; q++) { h ^= in[q]; h *= 0x100000001b3ull; }
         fnv[bi] = h;
@@ -384,7 +385,7 @@ int acx_encode(const uint8_t* in, uint64_t N, const acx_enc_opts* uo, uint8_t** 
     Out h;
     const uint8_t magic[8] = {0x41, 0x43, 0x58, 0x42, 0x32, 0x30, 0x30, 0x00};
     h.b.insert(h.b.end(), magic, magic + 8);
-    h.u32(1); h.u32(160); h.u64(N); h.u64(e.n_blocks); h.u32(o.log2_bs); h.u32(o.min_match); h.u32(W); h.u32(PROB_BITS);
+    h.u32(2); h.u32(160); h.u64(N); h.u64(e.n_blocks); h.u32(o.log2_bs); h.u32(o.min_match); h.u32(W); h.u32(PROB_BITS);
     h.u32(n_tables); h.u32(max_level); h.u32(max_cmds); h.u32(o.with_fnv ? 1 : 0);
     h.u64(tables_off); h.u64(dir_off); h.u64(o.with_fnv ? fnv_off : 0); h.u64(payload_off); h.u64(total);
     h.u64(tot_lit); h.u64(tot_mb); h.u64(tot_m); h.u64(tot_c); h.u64(o.src_window); h.u64(0); h.u64(0);

@@ -23,7 +23,8 @@ def normalise(hist):
 
 
 def rans_encode(symbols, tids, freqs):
-    """symbols[i] coded with table tids[i] on state i % 32.  Returns (32 initial decoder states, list of u16 words)."""
+    """symbols[i] coded with table tids[i] on state i % 32.  Returns (32 initial decoder states, 32 lists of u16 words:
+    state k's own stream in the order the decoder consumes it)."""
     cums = []
     for f in freqs:
         c = [0]
@@ -31,19 +32,20 @@ def rans_encode(symbols, tids, freqs):
             c.append(c[-1] + v)
         cums.append(c)
     x = [1 << 16] * 32
-    words = []
+    streams = [[] for _ in range(32)]
     for i in range(len(symbols) - 1, -1, -1):
         f = freqs[tids[i]][symbols[i]]
         c = cums[tids[i]][symbols[i]]
         assert f > 0, "symbol with zero frequency"
         s = i % 32
         if x[s] >= (f << (32 - M_BITS)):
-            words.append(x[s] & 0xFFFF)
+            streams[s].append(x[s] & 0xFFFF)
             x[s] >>= 16
         x[s] = ((x[s] // f) << M_BITS) + (x[s] % f) + c
         assert (1 << 16) <= x[s] < (1 << 32)
-    words.reverse()
-    return x, words
+    for st in streams:
+        st.reverse()
+    return x, streams
 
 
 def build(blocks, N, log2_bs, min_match=4, W=4, levels=None, raw_planes=(0, 1), with_fnv=False, expected=None,
@@ -103,8 +105,13 @@ def build(blocks, N, log2_bs, min_match=4, W=4, levels=None, raw_planes=(0, 1), 
                 tids += [2 + p] * len(off)
         syms += list(lit)
         tids += [2 + W] * len(lit)
-        states, words = rans_encode(syms, tids, freqs)
-        pl = b"".join(struct.pack("<I", s) for s in states) + b"".join(struct.pack("<H", w) for w in words)
+        states, streams = rans_encode(syms, tids, freqs)
+        words = [w for st in streams for w in st]
+        pl, woff = b"", 0
+        for k in range(32):                                   # head: (initial state, word_off) per state
+            pl += struct.pack("<II", states[k], woff)
+            woff += len(streams[k])
+        pl += b"".join(struct.pack("<H", w) for w in words)
         pl += b"\0" * (-len(pl) % 4)
         pl += b"".join(struct.pack("<I", e) for e in ext)
         for p in range(W):
@@ -120,7 +127,7 @@ def build(blocks, N, log2_bs, min_match=4, W=4, levels=None, raw_planes=(0, 1), 
     payload_off += -payload_off % 16
     total = payload_off + sum(len(p) for p in payloads)
     tot_lit = sum(d[2] for d in dirs)
-    hdr = MAGIC + struct.pack("<IIQQIIIIIIIIQQQQQQQQQQQQ", 1, 160, N, len(blocks), log2_bs, min_match, W, M_BITS, n_tables,
+    hdr = MAGIC + struct.pack("<IIQQIIIIIIIIQQQQQQQQQQQQ", 2, 160, N, len(blocks), log2_bs, min_match, W, M_BITS, n_tables,
                               max(levels) if levels else 0, max([d[0] for d in dirs] or [0]), 1 if with_fnv else 0,
                               tables_off, dir_off, fnv_off if with_fnv else 0, payload_off, total, tot_lit, N - tot_lit,
                               sum(d[1] for d in dirs), sum(d[0] for d in dirs), 0, 0, 0)

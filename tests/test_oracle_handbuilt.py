@@ -135,7 +135,7 @@ def test_corrupt_archives_are_rejected():
         O.decode(build(blocks, 16, 3, levels=[0, 1], mutate=_mut(0, 0x42)))
     assert e.value.name == "E_MAGIC"
     with pytest.raises(O.OracleError) as e:
-        O.decode(build(blocks, 16, 3, levels=[0, 1], mutate=_mut(8, 2)))
+        O.decode(build(blocks, 16, 3, levels=[0, 1], mutate=_mut(8, 1)))   # version 1 archives are not readable
     assert e.value.name == "E_VERSION"
     with pytest.raises(O.OracleError) as e:
         O.decode(good[:-16])
@@ -155,3 +155,25 @@ def test_corrupt_archives_are_rejected():
     bad[h["payload_off"] + 1] ^= 0x5A  # inside the initial state of lane 0
     with pytest.raises(O.OracleError):
         O.decode(bytes(bad))
+
+
+def test_word_offsets_of_the_rans_head_are_checked():
+    # FORMAT.md §1.5: word_off[0] = 0, non-decreasing, word_off[32] = n_words; every state consumes exactly its stream
+    lit0, lit1 = bytes((i * 37 + 11) % 251 for i in range(252)), bytes((i * 91 + 5) % 241 for i in range(232))
+    blocks = [[(lit0, (0, 4))], [(b"", (2, 24)), (lit1, None)]]
+    N = 512
+    good = build(blocks, N, 8, levels=[0, 0])
+    exp = O.decode(good).tobytes()
+    assert exp == lit0 + lit0[:4] + lit0[2:26] + lit1
+    h = O.header(good)
+    po = h["payload_off"]
+    offs = [int.from_bytes(good[po + 8 * k + 4:po + 8 * k + 8], "little") for k in range(32)]
+    assert offs[0] == 0 and offs == sorted(offs) and offs[-1] > 0      # the block does use words
+    for k, delta in ((0, 1), (5, 1), (31, -1)):
+        bad = bytearray(good)
+        v = offs[k] + delta
+        if v < 0:
+            continue
+        bad[po + 8 * k + 4:po + 8 * k + 8] = v.to_bytes(4, "little")
+        with pytest.raises(O.OracleError):
+            O.decode(bytes(bad))

@@ -10,13 +10,13 @@ from oracle import acx_oracle as O
 
 
 def roundtrip(symbols, tids, freqs):
-    states, words = rans_encode(list(symbols), list(tids), freqs)
+    states, streams = rans_encode(list(symbols), list(tids), freqs)
     sym, final, used = O.rans_decode(np.array(freqs, dtype=np.uint16), np.array(tids, dtype=np.uint8),
-                                     np.array(states, dtype=np.uint32), np.array(words, dtype=np.uint16))
-    assert used == len(words)                       # word count consumed == stored count
+                                     np.array(states, dtype=np.uint32), streams)
+    assert used.tolist() == [len(s) for s in streams]   # every state consumed exactly its own stream
     assert (final == (1 << 16)).all()               # encoder started at 2^16 -> decoder ends there
     assert list(sym) == list(symbols)
-    return states, words
+    return states, [w for s in streams for w in s]
 
 
 @pytest.mark.parametrize("n", [0, 1, 31, 32, 33, 64, 1000])
@@ -49,16 +49,14 @@ def test_worked_example_by_hand():
     # Decoder: slot = 262144 & 2047 = 0 -> 'a'; x = 512 * (262144 >> 11) + 0 - 0 = 65536.
     f = [0] * 256
     f[97], f[98] = 512, 1536
-    states, words = rans_encode([97], [0], [f])
-    assert states[0] == 262144 and states[1:] == [65536] * 31 and words == []
-    sym, final, used = O.rans_decode(np.array([f], np.uint16), np.array([0], np.uint8), np.array(states, np.uint32),
-                                     np.zeros(0, np.uint16))
-    assert list(sym) == [97] and final[0] == 65536 and used == 0
+    states, streams = rans_encode([97], [0], [f])
+    assert states[0] == 262144 and states[1:] == [65536] * 31 and streams == [[]] * 32
+    sym, final, used = O.rans_decode(np.array([f], np.uint16), np.array([0], np.uint8), np.array(states, np.uint32), streams)
+    assert list(sym) == [97] and final[0] == 65536 and used.sum() == 0
     # 'b' (freq 1536, cum 512): x' = (65536 // 1536) << 11 + 65536 % 1536 + 512 = 42 * 2048 + 1024 + 512 = 87552
-    states, words = rans_encode([98], [0], [f])
-    assert states[0] == 87552 and words == []
-    sym, final, used = O.rans_decode(np.array([f], np.uint16), np.array([0], np.uint8), np.array(states, np.uint32),
-                                     np.zeros(0, np.uint16))
+    states, streams = rans_encode([98], [0], [f])
+    assert states[0] == 87552 and streams == [[]] * 32
+    sym, final, used = O.rans_decode(np.array([f], np.uint16), np.array([0], np.uint8), np.array(states, np.uint32), streams)
     assert list(sym) == [98] and final[0] == 65536
 
 
@@ -87,12 +85,51 @@ def test_several_tables_interleaved_on_the_same_states():
     roundtrip(s.tolist(), t, [fa, fb])
 
 
+def test_worked_example_with_words_on_two_states():
+    # Table {a: 1, b: 2047}.  Decoding by hand, FORMAT.md §1.5, symbols i = 0, 1, 32 (states 0, 1, 0):
+    #   state 0 starts at x = 65536 * 2048 + 0 = 134217728: slot 0 -> 'a' (cum 0, freq 1); x = 1 * (x >> 11) + 0 = 65536.
+    #   state 1 starts at 65537 * 2048 = 134219776: slot 0 -> 'a'; x = 65537.
+    #   i = 32 (state 0): x = 65536: slot 0 -> 'a'; x = 1 * 32 + 0 = 32 < 2^16 -> x = (32 << 16) | w with w from state 0's stream.
+    # Choose w0 = 0x1234 for state 0 and give state 1 a different word 0xBEEF that must NOT be touched:
+    f = [0] * 256
+    f[97], f[98] = 1, 2047
+    streams = [[0x1234], [0xBEEF]] + [[] for _ in range(30)]
+    states = [134217728, 134219776] + [65536] * 30
+    tids = [0] * 33
+    # symbols 2..31 are decoded on states 2..31 = 65536: slot 0 -> 'a', x = 32 -> needs a word: give each a stream of one word
+    for k in range(2, 32):
+        streams[k] = [k]
+    sym, final, used = O.rans_decode(np.array([f], np.uint16), np.array(tids, np.uint8), np.array(states, np.uint32), streams)
+    assert list(sym) == [97] * 33
+    assert final[0] == (32 << 16) | 0x1234          # state 0 read its own word, after its second symbol
+    assert final[1] == 65537                         # state 1 never renormalised
+    assert [int(final[k]) for k in range(2, 32)] == [(32 << 16) | k for k in range(2, 32)]
+    assert used.tolist() == [1, 0] + [1] * 30
+
+
+def test_states_do_not_share_words():
+    # the same symbols coded twice; swapping two states' streams must change the output (streams are per state)
+    rng = np.random.default_rng(9)
+    s = rng.integers(0, 256, 2000)
+    f = normalise(np.bincount(s, minlength=256).tolist())
+    states, streams = rans_encode(s.tolist(), [0] * len(s), [f])
+    assert streams[3] != streams[4]
+    swapped = list(streams)
+    swapped[3], swapped[4] = streams[4], streams[3]
+    try:
+        sym, final, used = O.rans_decode(np.array([f], np.uint16), np.zeros(len(s), np.uint8), np.array(states, np.uint32), swapped)
+        assert list(sym) != s.tolist()
+    except O.OracleError as e:
+        assert e.name == "E_TRUNCATED"
+
+
 def test_truncated_word_stream_is_an_error():
     rng = np.random.default_rng(5)
     s = rng.integers(0, 256, 400)
     f = normalise(np.bincount(s, minlength=256).tolist())
-    states, words = rans_encode(s.tolist(), [0] * 400, [f])
+    states, streams = rans_encode(s.tolist(), [0] * 400, [f])
+    k = max(range(32), key=lambda q: len(streams[q]))
+    streams[k] = streams[k][:-1]                       # one state's stream is one word short
     with pytest.raises(O.OracleError) as e:
-        O.rans_decode(np.array([f], np.uint16), np.zeros(400, np.uint8), np.array(states, np.uint32),
-                      np.array(words[:-1], np.uint16))
+        O.rans_decode(np.array([f], np.uint16), np.zeros(400, np.uint8), np.array(states, np.uint32), streams)
     assert e.value.name == "E_TRUNCATED"
