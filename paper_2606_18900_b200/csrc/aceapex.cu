@@ -38,26 +38,28 @@ __device__ __forceinline__ void bind_scratch(const Params& P, uint32_t warp_glob
     c.off_planes = s;
 }
 
-// offset of match j assembled from coded planes (scratch) and raw planes (payload)
+// offset of match j assembled from coded planes (scratch, decode order = high plane first) and raw planes (payload)
 __device__ __forceinline__ uint64_t match_src(const Params& P, const BlockCtx& c, uint32_t j) {
-    uint64_t src = 0, mc = (P.max_cmds + 15u) & ~15u;
-    uint32_t k = 0;
-    for (int p = (int)P.W - 1; p >= 0; p--) {
-        if (P.plane_lut[p] >= 0) { src |= (uint64_t)c.off_planes[k * mc + j] << (8 * p); k++; }
-        else src |= (uint64_t)__ldg(c.raw_planes + (uint64_t)P.plane_raw[p] * c.d.n_match + j) << (8 * p);
-    }
+    uint64_t src = 0;
+    const uint32_t mc = (P.max_cmds + 15u) & ~15u;
+    for (uint32_t k = 0; k < P.n_coded_planes; k++) src |= (uint64_t)c.off_planes[k * mc + j] << P.coded_shift[k];
+    for (uint32_t r = 0; r < P.n_raw_planes; r++) src |= (uint64_t)__ldg(c.raw_planes + (uint64_t)r * c.d.n_match + j) << P.raw_shift[r];
     return src;
 }
 
-// Warm L2 with the source lines of every match of the block (issued before the literal stream is decoded, so the
-// HBM latency of the scattered sources overlaps the entropy decode).
+// Warm L2 with the source sectors of every match of the block (issued before the copies, so the HBM latency of the
+// scattered sources is paid once per block, not once per match).  Only sectors the match really touches are requested.
 __device__ __forceinline__ void prefetch_sources(const Params& P, const BlockCtx& c) {
     for (uint32_t j = lane_id(); j < c.d.n_match; j += 32) {
         uint64_t src = match_src(P, c, j);
         if (src >= P.out_pos0 && src < c.bstart) {
             const uint8_t* p = P.out + (src - P.out_pos0);
+            uint32_t len = P.min_match + c.tok_mlen[j];                  // escapes (>= 259 bytes) are served by the copy itself
+            uint32_t span = (uint32_t)(reinterpret_cast<uintptr_t>(p) & 31) + len;
             prefetch_l2(p);
-            prefetch_l2(p + 64);
+            if (span > 32) prefetch_l2(p + 32);
+            if (span > 64) prefetch_l2(p + 64);
+            if (span > 96) prefetch_l2(p + len - 1);
         }
     }
 }
@@ -73,12 +75,12 @@ __device__ __forceinline__ bool parse_tokens(const Params& P, uint32_t s_luts, u
     c.bstart = c.b << P.log2_bs;
     c.bend = min((unsigned long long)(c.bstart + (1ull << P.log2_bs)), (unsigned long long)P.N);
     c.payload = P.archive + c.d.payload_off;
-    uint64_t rans_bytes = 128 + 2ull * c.d.n_words;
+    uint64_t rans_bytes = 256 + 2ull * c.d.n_words;
     c.ext = reinterpret_cast<const uint32_t*>(c.payload + ((rans_bytes + 3) & ~3ull));
     c.raw_planes = reinterpret_cast<const uint8_t*>(c.ext + c.d.n_ext);
     uint64_t mc = (P.max_cmds + 15u) & ~15u;
     if (c.d.n_cmd > P.max_cmds || c.d.n_match > c.d.n_cmd || c.d.n_lit > (1u << P.log2_bs)) { if (lane_id() == 0) report(P, DF_LENGTH); return false; }
-    r.init(c.payload, P.archive + P.archive_bytes, ring);
+    r.init(c.payload, c.d.n_words, P.archive + P.archive_bytes, ring);
     uint32_t i0 = 0;
     c.n_ext_cmd = rans_region<true>(r, s_luts + P.lut_cmd * (4 * LUT_SIZE), i0, c.d.n_cmd, c.tok_cmd); i0 += c.d.n_cmd;
     rans_region<false>(r, s_luts + P.lut_mlen * (4 * LUT_SIZE), i0, c.d.n_match, c.tok_mlen); i0 += c.d.n_match;
@@ -97,7 +99,7 @@ __device__ __forceinline__ bool parse_tokens(const Params& P, uint32_t s_luts, u
 
 // FORMAT.md §1.5 integrity check once every symbol of the block has been decoded
 __device__ __forceinline__ bool rans_final_ok(const Params& P, const BlockCtx& c, const Rans& r) {
-    bool bad = (r.x != 65536u) || (r.wp != c.d.n_words);
+    bool bad = !r.finished();
     if (__any_sync(0xffffffffu, bad)) { if (lane_id() == 0) report(P, DF_RANS); return false; }
     return true;
 }
@@ -152,7 +154,8 @@ __device__ __forceinline__ uint32_t build_runs(const Params& P, const BlockCtx& 
         }
         n_runs += __popc(ne);
     }
-    fits = n_runs <= RUNS_CAP && lit_base == c.d.n_lit && c.bstart + out_base == c.bend;
+    fits = n_runs < RUNS_CAP && c.d.n_lit < 0xffffu && lit_base == c.d.n_lit && c.bstart + out_base == c.bend;
+    if (fits && lane == 0) asm volatile("st.shared.u32 [%0], %1;" ::"r"(runs + 4 * n_runs), "r"(0xffffu) : "memory");   // sentinel
     __syncwarp();
     return fits ? n_runs : 0xffffffffu;
 }
@@ -164,31 +167,22 @@ struct RunCursor {
     uint32_t delta;      // out_start - lit_start of run k
 };
 
-// A round whose literals [.., j_hi] are not all strictly inside run k: look the runs up (entries k .. k+31 cover any
-// 32 consecutive literals), store, and move the cursor to the run of the literal after j_hi.
-__device__ __forceinline__ void place_slow(RunCursor& rc, uint32_t runs, uint32_t n_runs, uint8_t* out_blk, uint32_t j, uint32_t j_hi,
-                                           uint32_t lane_hi, bool active, uint32_t e) {
-    uint32_t kk = rc.k + lane_id();
-    uint32_t ent = kk < n_runs ? lds32(runs + 4 * kk) : 0xffffffffu;
-    uint32_t last = kk < n_runs ? (ent & 0xffff) : 0xffffffffu;
-    uint32_t cnt = 0;                                     // number of runs (from k) that end before literal j
-#pragma unroll
-    for (int step = 16; step >= 1; step >>= 1) {
-        uint32_t t = __shfl_sync(0xffffffffu, last, (cnt + step - 1) & 31);
-        if (t < j) cnt += step;
-    }
-    uint32_t mine = __shfl_sync(0xffffffffu, ent, cnt & 31);
-    if (active) out_blk[(mine >> 16) + j] = (uint8_t)e;
-    uint32_t ck = __shfl_sync(0xffffffffu, cnt, lane_hi), ce = __shfl_sync(0xffffffffu, mine, lane_hi);
-    rc.k += ck; rc.last = ce & 0xffff; rc.delta = ce >> 16;
-    if (rc.last == j_hi && rc.k + 1 < n_runs) {           // that run ends with this round: the next literal opens run k + 1
+// A round whose literals [.., j_hi] are not all strictly inside run k: walk the cursor over the runs that end inside
+// the round (one broadcast table read per boundary; the table ends with a sentinel whose `last` is 0xffff).  Returns the
+// delta of this lane's literal j and leaves the cursor on the run of literal j_hi + 1.
+__device__ __forceinline__ uint32_t walk_runs(RunCursor& rc, uint32_t runs, uint32_t j, uint32_t j_hi) {
+    uint32_t mine = rc.delta;
+    while (rc.last <= j_hi) {
+        const uint32_t prev = rc.last;
         rc.k++;
-        uint32_t en = lds32(runs + 4 * rc.k);
-        rc.last = en & 0xffff; rc.delta = en >> 16;
+        const uint32_t e = lds32(runs + 4 * rc.k);
+        rc.last = e & 0xffff; rc.delta = e >> 16;
+        if (j > prev) mine = rc.delta;
     }
+    return mine;
 }
 
-__device__ __forceinline__ void decode_lit_direct(Rans& r, uint32_t lut, uint32_t i0, uint32_t n_lit, uint32_t runs, uint32_t n_runs, uint8_t* out_blk) {
+__device__ __forceinline__ void decode_lit_direct(Rans& r, uint32_t lut, uint32_t i0, uint32_t n_lit, uint32_t runs, uint8_t* out_blk) {
     if (n_lit == 0) return;
     const uint32_t lane = lane_id(), i1 = i0 + n_lit;
     RunCursor rc;
@@ -200,7 +194,8 @@ __device__ __forceinline__ void decode_lit_direct(Rans& r, uint32_t lut, uint32_
         r.prepare8();
         uint32_t e = r.step(lut, active);
         uint32_t j_hi = min(base + 31, i1 - 1) - i0;
-        place_slow(rc, runs, n_runs, out_blk, i - i0, j_hi, (j_hi + i0 - base) & 31, active, e);
+        uint32_t d = walk_runs(rc, runs, i - i0, j_hi);
+        if (active) out_blk[d + (i - i0)] = (uint8_t)e;
         base += 32;
     }
     uint8_t* pj = out_blk + (base + lane - i0);           // address of literal (base + lane - i0) if delta were 0
@@ -212,7 +207,7 @@ __device__ __forceinline__ void decode_lit_direct(Rans& r, uint32_t lut, uint32_
             uint32_t e = r.step_full(lut);
             uint32_t j_hi = base + 32 * q + 31 - i0;
             if (j_hi < rc.last) pd[32 * q] = (uint8_t)e;   // the whole round lies strictly inside run k: pointer bump
-            else { place_slow(rc, runs, n_runs, out_blk, j_hi - 31 + lane, j_hi, 31, true, e); pd = pj + rc.delta; }
+            else { uint32_t d = walk_runs(rc, runs, j_hi - 31 + lane, j_hi); pj[32 * q + d] = (uint8_t)e; pd = pj + rc.delta; }
         }
         base += 256; pj += 256;
     }
@@ -222,7 +217,8 @@ __device__ __forceinline__ void decode_lit_direct(Rans& r, uint32_t lut, uint32_
             bool active = base + lane < i1;
             uint32_t e = r.step(lut, active);
             uint32_t j_hi = min(base + 31, i1 - 1) - i0;
-            place_slow(rc, runs, n_runs, out_blk, base + lane - i0, j_hi, (j_hi + i0 - base) & 31, active, e);
+            uint32_t d = walk_runs(rc, runs, base + lane - i0, j_hi);
+            if (active) out_blk[d + (base + lane - i0)] = (uint8_t)e;
         }
     }
 }
@@ -382,6 +378,117 @@ __device__ __forceinline__ void emit_block(const Params& P, const BlockCtx& c, c
     if (out_base != (uint32_t)(c.bend - c.bstart) || lit_base != c.d.n_lit) { if (lane == 0) report(P, DF_LENGTH); }
 }
 
+// ---- A4 for the whole-file schedules: matches of one block, 32 commands at a time ---------------------------------------
+// Short non-overlapping matches of a group are flattened into one run of T match bytes and copied 32 consecutive bytes
+// per warp instruction (one coalesced byte load + one coalesced byte store; the entry that owns a byte is found by
+// walking a 32-entry table in shared memory, one broadcast read per match boundary).  The loads of four steps are in
+// flight before the first store: by FORMAT.md §3 no match reads match bytes of its own block, so the loads of a block
+// never depend on its stores.  Long matches use the 16-byte warp copy, self-overlapping ones read src + (i mod period).
+constexpr uint32_t LONG_MATCH = 192;
+constexpr uint32_t MTAB_BYTES = 33 * 16;   // per warp: 32 entries + sentinel; entry = {last, dst_delta, src_ptr lo, hi}
+
+__device__ __forceinline__ void sts128(uint32_t a, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
+    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
+}
+__device__ __forceinline__ uint4 lds128(uint32_t a) {
+    uint4 v; asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a)); return v;
+}
+
+// MODE 3: no waits (one launch per level); MODE 4: completion waits for lower-level source blocks
+template <int MODE>
+__device__ __forceinline__ void emit_matches(const Params& P, const BlockCtx& c, uint32_t mtab) {
+    uint32_t lit_base = 0, out_base = 0, ec = 0, em = c.n_ext_cmd;
+    const uint32_t lane = lane_id();
+    uint8_t* const out_blk = P.out + (c.bstart - P.out_pos0);
+    for (uint32_t c0 = 0; c0 < c.d.n_cmd; c0 += 32) {
+        uint32_t ci = c0 + lane;
+        bool valid = ci < c.d.n_cmd, has_match = ci < c.d.n_match;
+        uint32_t tl = valid ? c.tok_cmd[ci] : 0, tm = has_match ? c.tok_mlen[ci] : 0;
+        uint32_t ml = __ballot_sync(0xffffffffu, valid && tl == 255), mm = __ballot_sync(0xffffffffu, has_match && tm == 255);
+        uint32_t lit_len = tl, match_len = has_match ? P.min_match + tm : 0;
+        if (valid && tl == 255) lit_len = 255 + __ldg(c.ext + ec + __popc(ml & lanemask_lt()));
+        if (has_match && tm == 255) match_len = P.min_match + 255 + __ldg(c.ext + em + __popc(mm & lanemask_lt()));
+        ec += __popc(ml); em += __popc(mm);
+        uint32_t sl = lit_len, st = lit_len + match_len;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t a = __shfl_up_sync(0xffffffffu, sl, o), t = __shfl_up_sync(0xffffffffu, st, o);
+            if (lane >= (uint32_t)o) { sl += a; st += t; }
+        }
+        uint32_t lit_pos = lit_base + sl - lit_len;
+        uint32_t dst_rel = out_base + (st - match_len);      // block-relative position of the match
+        lit_base += __shfl_sync(0xffffffffu, sl, 31);
+        out_base += __shfl_sync(0xffffffffu, st, 31);
+        bool ok = valid && (uint64_t)lit_pos + lit_len <= c.d.n_lit && c.bstart + dst_rel + match_len <= c.bend;
+        if (__any_sync(0xffffffffu, valid && !ok)) { if (lane == 0) report(P, DF_LENGTH); return; }
+        uint64_t dst = c.bstart + dst_rel, src = (ok && has_match) ? match_src(P, c, ci) : 0;
+        bool good = ok && has_match && src < dst;
+        if (ok && has_match && !good) report(P, DF_OFFSET);
+        if (MODE == 4 && good && c.d.level) wait_sources<false>(P, c, dst, src, match_len);
+        const bool ovl = good && src + match_len > dst;
+        const bool lng = good && !ovl && match_len >= LONG_MATCH;
+        const bool sht = good && !ovl && !lng;
+        // flatten the short matches of the group
+        uint32_t fi = sht ? match_len : 0;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { uint32_t a = __shfl_up_sync(0xffffffffu, fi, o); if (lane >= (uint32_t)o) fi += a; }
+        const uint32_t T = __shfl_sync(0xffffffffu, fi, 31);
+        const uint32_t smask = __ballot_sync(0xffffffffu, sht);
+        if (sht) {
+            uint32_t f0 = fi - match_len;
+            uint64_t sp = reinterpret_cast<uint64_t>(P.out) + (src - P.out_pos0) - f0;
+            sts128(mtab + 16 * __popc(smask & lanemask_lt()), fi - 1, dst_rel - f0, (uint32_t)sp, (uint32_t)(sp >> 32));
+        }
+        if (lane == 0) sts128(mtab + 16 * __popc(smask), 0xffffffffu, 0, 0, 0);
+        __syncwarp();
+        if (T) {
+            uint32_t k = 0;
+            uint4 cur = lds128(mtab);
+            for (uint32_t fb = 0; fb < T; fb += 128) {
+                uint8_t v[4]; uint32_t dd[4];
+#pragma unroll
+                for (int u = 0; u < 4; u++) {
+                    const uint32_t f = fb + 32 * u + lane, f_hi = fb + 32 * u + 31;
+                    uint4 mine = cur;
+                    while (cur.x <= f_hi) {                  // uniform: the current match ends inside this step
+                        const uint32_t prev = cur.x;
+                        k++;
+                        cur = lds128(mtab + 16 * k);
+                        if (f > prev) mine = cur;
+                    }
+                    dd[u] = mine.y + f;
+                    v[u] = 0;
+                    if (f < T) v[u] = __ldcg(reinterpret_cast<const uint8_t*>(((uint64_t)mine.w << 32 | mine.z) + f));
+                }
+#pragma unroll
+                for (int u = 0; u < 4; u++) if (fb + 32 * u + lane < T) out_blk[dd[u]] = v[u];
+            }
+        }
+        __syncwarp();                                        // the table is rewritten by the next group
+        uint32_t longs = __ballot_sync(0xffffffffu, lng);
+        while (longs) {
+            int l = __ffs(longs) - 1; longs &= longs - 1;
+            uint32_t d2 = __shfl_sync(0xffffffffu, dst_rel, l), n = __shfl_sync(0xffffffffu, match_len, l);
+            uint64_t s2 = __shfl_sync(0xffffffffu, src, l);
+            warp_copy<true>(out_blk + d2, P.out + (s2 - P.out_pos0), n);
+        }
+        uint32_t ovls = __ballot_sync(0xffffffffu, ovl);
+        while (ovls) {                                       // byte i of the match = seed[i mod period] (FORMAT.md §2)
+            int l = __ffs(ovls) - 1; ovls &= ovls - 1;
+            uint32_t d2 = __shfl_sync(0xffffffffu, dst_rel, l), n = __shfl_sync(0xffffffffu, match_len, l);
+            uint64_t s2 = __shfl_sync(0xffffffffu, src, l);
+            const uint32_t per = (uint32_t)(c.bstart + d2 - s2);
+            const uint8_t* sp = P.out + (s2 - P.out_pos0);
+            uint32_t r = lane % per; const uint32_t stp = 32 % per;
+            for (uint32_t i = lane; i < n; i += 32) {
+                out_blk[d2 + i] = __ldcg(sp + r);
+                r += stp; if (r >= per) r -= per;
+            }
+        }
+    }
+    if (out_base != (uint32_t)(c.bend - c.bstart) || lit_base != c.d.n_lit) { if (lane == 0) report(P, DF_LENGTH); }
+}
+
 // ---- A5-A7: demands ("materialise original bytes [pos, pos+len) at out2[dst..)") ------------------------------------
 // Source bytes that are neither in the current window nor in a resident slot are reconstructed by recursion on their
 // own sources: the block that holds them is parsed and the wanted span is emitted; literal bytes are final, match
@@ -489,6 +596,7 @@ __global__ void __launch_bounds__(1024, 1) k_decode(const Params P) {
     Stack st;
     st.base = P.stacks + (uint64_t)(blockIdx.x * warps_per_cta + warp) * P.stack_cap; st.cap = P.stack_cap;
     st.top = s_luts + n_lut_words * 4 + warps_per_cta * (RING_BYTES + 4 * RUNS_CAP) + 4 * warp;
+    const uint32_t mtab = s_luts + n_lut_words * 4 + warps_per_cta * (RING_BYTES + 4 * RUNS_CAP + 4) + warp * MTAB_BYTES;
     if (lane_id() == 0) asm volatile("st.shared.u32 [%0], %1;" ::"r"(st.top), "r"(0u) : "memory");
     __syncwarp();
     for (;;) {
@@ -504,13 +612,13 @@ __global__ void __launch_bounds__(1024, 1) k_decode(const Params P) {
         c.b = P.level_list ? (uint64_t)P.level_list[t] : P.first_block + t;
         if (P.mode == 3) {
             // match wave: only the command / length / offset streams are needed again
-            if (parse_block(P, s_luts, ring, c, 0)) emit_block<3>(P, c, st);
+            if (parse_block(P, s_luts, ring, c, 0)) emit_matches<3>(P, c, mtab);
             continue;
         }
         if (P.mode == 4) {
             // all match waves in one launch: blocks arrive sorted by (level, index), a block waits for the completion
             // of lower-level source blocks, which were dispatched before it
-            if (parse_block(P, s_luts, ring, c, 0)) emit_block<4>(P, c, st);
+            if (parse_block(P, s_luts, ring, c, 0)) emit_matches<4>(P, c, mtab);
             __threadfence();
             __syncwarp();
             if (lane_id() == 0) st_release(P.flags + c.b, 2 * P.epoch + 1);
@@ -525,7 +633,7 @@ __global__ void __launch_bounds__(1024, 1) k_decode(const Params P) {
                 if (P.mode == 0) prefetch_sources(P, c);              // source lines travel to L2 while the literals decode
                 uint32_t n_runs = P.log2_bs <= 16 ? build_runs(P, c, runs) : 0xffffffffu;
                 if (n_runs != 0xffffffffu) {                          // scan first, literals straight to their positions
-                    decode_lit_direct(r, s_luts + P.lut_lit * (4 * LUT_SIZE), i0, c.d.n_lit, runs, n_runs, P.out + (c.bstart - P.out_pos0));
+                    decode_lit_direct(r, s_luts + P.lut_lit * (4 * LUT_SIZE), i0, c.d.n_lit, runs, P.out + (c.bstart - P.out_pos0));
                     ok = rans_final_ok(P, c, r);
                 } else {                                              // too many runs / big block / bad scan: staged path
                     rans_region<false>(r, s_luts + P.lut_lit * (4 * LUT_SIZE), i0, c.d.n_lit, c.lit);
@@ -632,6 +740,8 @@ void fill_params(const aceapex_archive* ar, Params& P) {
     P.n_coded_tables = ar->n_coded_tables;
     memcpy(P.plane_lut, ar->plane_lut, MAX_W); memcpy(P.plane_raw, ar->plane_raw, MAX_W);
     P.n_coded_planes = ar->n_coded_planes; P.n_raw_planes = ar->n_raw_planes;
+    for (int p = (int)ar->W - 1, k = 0; p >= 0; p--) if (ar->plane_lut[p] >= 0) P.coded_shift[k++] = (uint8_t)(8 * p);
+    for (uint32_t p = 0; p < ar->W; p++) if (ar->plane_raw[p] >= 0) P.raw_shift[ar->plane_raw[p]] = (uint8_t)(8 * p);
     P.lut_cmd = ar->lut_cmd; P.lut_mlen = ar->lut_mlen; P.lut_lit = ar->lut_lit;
     memcpy(P.res, ar->res, sizeof P.res);
     P.ticket = reinterpret_cast<unsigned long long*>(ar->d_ws);
@@ -682,7 +792,7 @@ int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* 
     if (h_archive) memcpy(hdr, h_archive, 160); else CU(cudaMemcpy(hdr, d_archive, 160, cudaMemcpyDeviceToHost));
     static const uint8_t magic[8] = {0x41, 0x43, 0x58, 0x42, 0x32, 0x30, 0x30, 0x00};
     if (memcmp(hdr, magic, 8)) return ACEAPEX_E_MAGIC;
-    if (rd32(hdr + 8) != 1 || rd32(hdr + 44) != (uint32_t)PROB_BITS) return ACEAPEX_E_VERSION;
+    if (rd32(hdr + 8) != 2 || rd32(hdr + 44) != (uint32_t)PROB_BITS) return ACEAPEX_E_VERSION;
     if (rd32(hdr + 12) != 160) return ACEAPEX_E_CORRUPT;
     ar->N = rd64(hdr + 16); ar->n_blocks = rd64(hdr + 24); ar->log2_bs = rd32(hdr + 32); ar->min_match = rd32(hdr + 36);
     ar->W = rd32(hdr + 40); uint32_t n_tables = rd32(hdr + 48); ar->max_level = rd32(hdr + 52); ar->max_cmds = rd32(hdr + 56);
@@ -745,7 +855,7 @@ int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* 
         uint32_t n_cmd = rd32(p + 8), n_match = rd32(p + 12), n_lit = rd32(p + 16), n_words = rd32(p + 20), n_ext = rd32(p + 24), lvl = rd16(p + 28);
         if (po % 16 || po < prev || end <= po || end > abytes) return ACEAPEX_E_CORRUPT;
         if (n_cmd < 1 || n_cmd > ar->max_cmds || !(n_match == n_cmd || n_match + 1 == n_cmd) || lvl > ar->max_level) return ACEAPEX_E_CORRUPT;
-        uint64_t need = ((128 + 2ull * n_words + 3) & ~3ull) + 4ull * n_ext + (uint64_t)ar->n_raw_planes * n_match;
+        uint64_t need = ((256 + 2ull * n_words + 3) & ~3ull) + 4ull * n_ext + (uint64_t)ar->n_raw_planes * n_match;
         if (po + need > end || n_lit > (1u << ar->log2_bs)) return ACEAPEX_E_CORRUPT;
         prev = po; seen_max_cmds = std::max(seen_max_cmds, n_cmd);
         ar->level_blocks[lvl].push_back((uint32_t)b);
@@ -772,8 +882,14 @@ int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* 
     int dev = 0; cudaDeviceProp prop;
     CU(cudaGetDevice(&dev)); CU(cudaGetDeviceProperties(&prop, dev));
     ar->sms = prop.multiProcessorCount;
-    ar->threads = 1024;   // one CTA per SM: the decode tables are staged once per SM, 32 warps share them
-    ar->smem = 8192 + (size_t)ar->n_coded_tables * LUT_SIZE * 4 + (size_t)(ar->threads / 32) * (RING_BYTES + 4 * RUNS_CAP + 4);
+    // one CTA per SM: the decode tables are staged once per SM and shared by all its warps (fewer warps when many
+    // offset planes are coded and the tables leave less room)
+    auto smem_for = [&](int threads) {
+        return (size_t)8192 + (size_t)ar->n_coded_tables * LUT_SIZE * 4 + (size_t)(threads / 32) * (RING_BYTES + 4 * RUNS_CAP + 4 + MTAB_BYTES);
+    };
+    ar->threads = 1024;
+    while (ar->threads > 128 && smem_for(ar->threads) > (size_t)prop.sharedMemPerBlockOptin) ar->threads -= 128;
+    ar->smem = smem_for(ar->threads);
     CU(cudaFuncSetAttribute(k_decode<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ar->smem));
     CU(cudaFuncSetAttribute(k_decode<false>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
     CU(cudaFuncSetAttribute(k_decode<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ar->smem));

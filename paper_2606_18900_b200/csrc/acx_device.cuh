@@ -8,7 +8,7 @@ namespace acx {
 
 constexpr int PROB_BITS = 11;
 constexpr int LUT_SIZE = 1 << PROB_BITS;          // u32 entries per coded table: sym | bias << 8 | freq << 20
-constexpr int RING_BYTES = 2048;                  // per-warp ring of rANS words in shared memory (four 512 B quarters)
+constexpr int RING_BYTES = 2048;                  // per warp: 32 lanes x 64-byte ring of rANS words in shared memory
 constexpr int MAX_W = 8;
 constexpr int MAX_RESIDENT = 8;
 
@@ -36,6 +36,8 @@ struct Params {
     int8_t plane_lut[MAX_W];     // coded OFF plane p -> lut index, -1 if raw
     int8_t plane_raw[MAX_W];     // raw OFF plane p -> index among raw planes, -1 if coded
     uint32_t n_coded_planes, n_raw_planes;
+    uint8_t coded_shift[MAX_W];  // bit position of the k-th coded plane in decode order (high plane first)
+    uint8_t raw_shift[MAX_W];    // bit position of the r-th raw plane (ascending p)
     uint32_t lut_cmd, lut_mlen, lut_lit;
     // work
     uint64_t first_block, n_work;       // FULL mode: blocks [first_block, first_block + n_work)
@@ -73,10 +75,11 @@ __device__ __forceinline__ uint64_t ldcg64(const uint8_t* p) { return __ldcg(rei
 
 
 // ------------------------------------------------------------------------------------------------ rANS ----------
-// FORMAT.md §1.5.  32 states, one per lane; symbol i lives on lane i & 31.  The word stream is staged through a
-// 2 KB per-warp shared-memory ring (four 512 B quarters) filled with 16-byte cp.async copies: one coalesced 512 B
-// request per quarter, issued two quarters ahead of its use.  Both the ring (2 KB aligned) and every table
-// (8 KB aligned) sit at aligned shared addresses so that an index folds into an address with one LOP3.
+// FORMAT.md §1.5 (version 2).  32 states, one per lane; symbol i lives on lane i & 31; every state renormalises from
+// its OWN word stream, so the decode step needs no ballot, no prefix and no shared cursor.  Each lane stages its stream
+// through a private 64-byte ring in shared memory (four 16-byte chunks, filled with cp.async two chunks ahead of their
+// use).  Every table (8 KB aligned) and every ring (64 B aligned) sits at an aligned shared address so that an index
+// folds into an address with one LOP3.
 __device__ __forceinline__ uint32_t lds32(uint32_t a) { uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a)); return v; }
 __device__ __forceinline__ uint32_t lds16(uint32_t a) { uint32_t v; asm volatile("ld.shared.u16 %0, [%1];" : "=r"(v) : "r"(a)); return v; }
 __device__ __forceinline__ void cp_async16s(uint32_t saddr, const void* gmem) {
@@ -87,54 +90,65 @@ template <int N> __device__ __forceinline__ void cp_async_wait_group() { asm vol
 
 struct Rans {
     uint32_t x;              // this lane's state
-    uint32_t wp;             // words consumed so far
-    uint32_t issued;         // bytes of the word stream requested into the ring (multiple of 512)
-    uint32_t ring;           // shared address of the ring, RING_BYTES aligned
-    const uint8_t* words;    // global address of word 0 (16-byte aligned)
+    uint32_t rp;             // byte offset of this lane's next word, relative to gbase; ring slot = rp & 63
+    uint32_t fp;             // bytes of the stream requested into the ring so far (relative to gbase, multiple of 16)
+    uint32_t ring;           // shared address of this lane's ring, 64-byte aligned
+    uint32_t end;            // rp after the lane's last word (integrity check)
+    const uint8_t* gbase;    // 16-byte aligned global address that offsets are relative to
     const uint8_t* limit;    // archive end (loads are clamped)
 
-    __device__ __forceinline__ void fill_quarter() {
-        const uint8_t* g = words + issued + 16 * lane_id();
-        if (g + 16 <= limit) cp_async16s(ring | ((issued + 16 * lane_id()) & (RING_BYTES - 1)), g);
-        cp_async_commit();
-        issued += 512;
+    __device__ __forceinline__ void fetch() {
+        const uint8_t* g = gbase + fp;
+        if (g + 16 <= limit) cp_async16s(ring | (fp & 63), g);
+        fp += 16;
     }
-    __device__ __forceinline__ void init(const uint8_t* payload, const uint8_t* lim, uint32_t ring_addr) {
-        ring = ring_addr; limit = lim; words = payload + 128; wp = 0; issued = 0;
-        x = __ldg(reinterpret_cast<const uint32_t*>(payload) + lane_id());
-        __syncwarp();        // the previous block's ring reads are done
-        fill_quarter(); fill_quarter(); fill_quarter(); fill_quarter();
+    // payload: [32 x (u32 state, u32 word_off)][words]; n_words = total words of the block
+    __device__ __forceinline__ void init(const uint8_t* payload, uint32_t n_words, const uint8_t* lim, uint32_t ring_warp) {
+        const uint32_t lane = lane_id();
+        uint2 h = __ldg(reinterpret_cast<const uint2*>(payload) + lane);
+        x = h.x;
+        uint32_t next = __shfl_down_sync(0xffffffffu, h.y, 1);
+        if (lane == 31) next = n_words;
+        const uint8_t* start = payload + 256 + 2ull * h.y;
+        // bias the base by a lane-dependent multiple of 16 so that lanes in lockstep sit in different ring slots (banks)
+        const uint32_t bias = 16u * ((lane >> 1) & 3u);
+        gbase = start - (reinterpret_cast<uintptr_t>(start) & 15) - bias;
+        rp = (uint32_t)(start - gbase);
+        end = rp + 2u * (next - h.y);
+        fp = bias;
+        ring = ring_warp + 64u * lane;
+        limit = lim;
+        cp_async_wait_group<0>();            // chunks still in flight from the previous block must not land after ours
+        fetch(); cp_async_commit(); fetch(); cp_async_commit(); fetch(); cp_async_commit(); fetch(); cp_async_commit();
     }
-    // Call before every group of <= 8 rounds (<= 512 B of words).  Invariant after the call: more than 1536 B are
-    // requested beyond the read position and all but the two most recent quarters have landed, so >= 512 B are readable.
+    // Call before every group of <= 8 symbols per lane (<= 16 B of words).  Invariant after the call: fp - rp >= 50 and
+    // everything but the two most recent chunks has landed, so the next 16 bytes are readable.
     __device__ __forceinline__ void prepare8() {
-        if (issued - 2 * wp <= RING_BYTES - 512) { __syncwarp(); fill_quarter(); }   // that quarter is fully consumed
+        if (fp - rp <= 48) fetch();          // the slot being refilled holds bytes below rp
+        cp_async_commit();
         cp_async_wait_group<2>();
-        __syncwarp();
     }
-    // one symbol on every lane (full round).  lut = shared address of the table (8 KB aligned).
+    // one symbol on this lane.  lut = shared address of the table (8 KB aligned).  Returns the table entry
+    // (sym | bias << 8 | freq << 20).
     __device__ __forceinline__ uint32_t step_full(uint32_t lut) {
         uint32_t e = lds32(lut | ((x << 2) & (4 * LUT_SIZE - 4)));
+        uint32_t w = lds16(ring | (rp & 63));
         x = (e >> 20) * (x >> PROB_BITS) + ((e >> 8) & 0xfff);
-        bool need = x < 65536u;
-        uint32_t m = __ballot_sync(0xffffffffu, need);
-        uint32_t w = lds16(ring | ((2 * (wp + __popc(m & lanemask_lt()))) & (RING_BYTES - 1)));
-        if (need) x = (x << 16) | w;
-        wp += __popc(m);
+        if (x < 65536u) { x = (x << 16) | w; rp += 2; }
         return e;
     }
-    // one symbol on the lanes with active == true; all 32 lanes must call
+    // one symbol on the lanes with active == true
     __device__ __forceinline__ uint32_t step(uint32_t lut, bool active) {
         uint32_t e = lds32(lut | ((x << 2) & (4 * LUT_SIZE - 4)));
+        uint32_t w = lds16(ring | (rp & 63));
         uint32_t nx = (e >> 20) * (x >> PROB_BITS) + ((e >> 8) & 0xfff);
-        if (active) x = nx;
-        bool need = active && x < 65536u;
-        uint32_t m = __ballot_sync(0xffffffffu, need);
-        uint32_t w = lds16(ring | ((2 * (wp + __popc(m & lanemask_lt()))) & (RING_BYTES - 1)));
-        if (need) x = (x << 16) | w;
-        wp += __popc(m);
+        if (active) {
+            x = nx;
+            if (x < 65536u) { x = (x << 16) | w; rp += 2; }
+        }
         return e;
     }
+    __device__ __forceinline__ bool finished() const { return x == 65536u && rp == end; }
 };
 
 // Decodes `count` symbols whose global symbol indices start at i0, storing them to dst[0..count) (byte stores,
