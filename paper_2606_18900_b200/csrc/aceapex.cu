@@ -52,7 +52,7 @@ __device__ __forceinline__ uint64_t match_src(const Params& P, const BlockCtx& c
 __device__ __forceinline__ void prefetch_sources(const Params& P, const BlockCtx& c) {
     for (uint32_t j = lane_id(); j < c.d.n_match; j += 32) {
         uint64_t src = match_src(P, c, j);
-        if (src >= P.out_pos0 && src < c.bstart) {
+        if (src >= P.out_pos0 && src < c.bstart && src < P.win_end) {
             const uint8_t* p = P.out + (src - P.out_pos0);
             uint32_t len = P.min_match + c.tok_mlen[j];                  // escapes (>= 259 bytes) are served by the copy itself
             uint32_t span = (uint32_t)(reinterpret_cast<uintptr_t>(p) & 31) + len;
@@ -105,10 +105,10 @@ __device__ __forceinline__ bool rans_final_ok(const Params& P, const BlockCtx& c
 }
 
 // A1, whole block: tokens, then the first min(lit_limit, n_lit) literal symbols into the scratch staging buffer.
-__device__ __forceinline__ bool parse_block(const Params& P, uint32_t s_luts, uint32_t ring, BlockCtx& c, uint32_t lit_limit) {
+__device__ __forceinline__ bool parse_block(const Params& P, uint32_t s_luts, uint32_t ring, BlockCtx& c, uint32_t lit_limit, bool prefetch = true) {
     Rans r; uint32_t i0;
     if (!parse_tokens(P, s_luts, ring, c, r, &i0)) return false;
-    if (P.mode != 2) prefetch_sources(P, c);
+    if (prefetch) prefetch_sources(P, c);
     uint32_t nl = min(lit_limit, c.d.n_lit);
     rans_region<false>(r, s_luts + P.lut_lit * (4 * LUT_SIZE), i0, nl, c.lit);
     if (nl == c.d.n_lit && !rans_final_ok(P, c, r)) return false;
@@ -379,16 +379,19 @@ __device__ __forceinline__ void emit_block(const Params& P, const BlockCtx& c, c
 }
 
 // ---- A4 for the whole-file schedules: matches of one block, 32 commands at a time ---------------------------------------
-// Short non-overlapping matches of a group are flattened into one run of T match bytes and copied 32 consecutive bytes
-// per warp instruction (one coalesced byte load + one coalesced byte store; the entry that owns a byte is found by
-// walking a 32-entry table in shared memory, one broadcast read per match boundary).  The loads of four steps are in
-// flight before the first store: by FORMAT.md §3 no match reads match bytes of its own block, so the loads of a block
-// never depend on its stores.  Long matches use the 16-byte warp copy, self-overlapping ones read src + (i mod period).
+// Short non-overlapping matches are staged through shared memory (see below); matches of LONG_MATCH bytes and more use
+// the 16-byte warp copy; self-overlapping ones read src + (i mod period).  By FORMAT.md §3 no match reads match bytes of
+// its own block, so the loads of a block never depend on its stores.
 constexpr uint32_t LONG_MATCH = 192;
-constexpr uint32_t MTAB_BYTES = 33 * 16;   // per warp: 32 entries + sentinel; entry = {last, dst_delta, src_ptr lo, hi}
+constexpr uint32_t MTAB_BYTES = 32 * 16;   // per warp: 32 entries {destination pointer | len << 56, shared address of the staged source}
+constexpr uint32_t STAGE_CHUNKS = 160;     // per warp: 2560 bytes of staged source data
+static_assert(LONG_MATCH < 256 && (15 + LONG_MATCH + 15) / 16 <= STAGE_CHUNKS, "a short match has an 8-bit length and fits the stage");
 
 __device__ __forceinline__ void sts128(uint32_t a, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
     asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
+}
+__device__ __forceinline__ uint2 lds64(uint32_t a) {
+    uint2 v; asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(a)); return v;
 }
 __device__ __forceinline__ uint4 lds128(uint32_t a) {
     uint4 v; asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a)); return v;
@@ -396,7 +399,7 @@ __device__ __forceinline__ uint4 lds128(uint32_t a) {
 
 // MODE 3: no waits (one launch per level); MODE 4: completion waits for lower-level source blocks
 template <int MODE>
-__device__ __forceinline__ void emit_matches(const Params& P, const BlockCtx& c, uint32_t mtab) {
+__device__ __forceinline__ void emit_matches(const Params& P, const BlockCtx& c, uint32_t mtab, uint32_t stage) {
     uint32_t lit_base = 0, out_base = 0, ec = 0, em = c.n_ext_cmd;
     const uint32_t lane = lane_id();
     uint8_t* const out_blk = P.out + (c.bstart - P.out_pos0);
@@ -428,43 +431,47 @@ __device__ __forceinline__ void emit_matches(const Params& P, const BlockCtx& c,
         const bool ovl = good && src + match_len > dst;
         const bool lng = good && !ovl && match_len >= LONG_MATCH;
         const bool sht = good && !ovl && !lng;
-        // flatten the short matches of the group
-        uint32_t fi = sht ? match_len : 0;
+        // Short matches: their source bytes travel global -> shared memory with 16-byte cp.async (issued by the lane that
+        // owns the match, all matches of the group at once: one exposed memory latency per group instead of one per
+        // match), then the warp copies match after match from the stage to the output: lane i moves bytes i, i + 32, ...
+        // A group whose sources do not fit the stage is served in several rounds.
+        const uint64_t sp = reinterpret_cast<uint64_t>(P.out) + (src - P.out_pos0);
+        const uint32_t mis = (uint32_t)sp & 15u;
+        // a chunk may not reach past the end of the output buffer (only possible for sources in its last 16 bytes)
+        const bool stg = sht && ((sp - mis) + 16ull * ((mis + match_len + 15u) >> 4) <= reinterpret_cast<uint64_t>(P.out) + (P.win_end - P.out_pos0));
+        const bool direct = (sht && !stg) || ovl;
+        uint32_t pending = __ballot_sync(0xffffffffu, stg);
+        while (pending) {
+            const bool mine = (pending >> lane) & 1u;
+            const uint32_t need = mine ? (mis + match_len + 15u) >> 4 : 0u;
+            uint32_t ce = need;
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) { uint32_t a = __shfl_up_sync(0xffffffffu, fi, o); if (lane >= (uint32_t)o) fi += a; }
-        const uint32_t T = __shfl_sync(0xffffffffu, fi, 31);
-        const uint32_t smask = __ballot_sync(0xffffffffu, sht);
-        if (sht) {
-            uint32_t f0 = fi - match_len;
-            uint64_t sp = reinterpret_cast<uint64_t>(P.out) + (src - P.out_pos0) - f0;
-            sts128(mtab + 16 * __popc(smask & lanemask_lt()), fi - 1, dst_rel - f0, (uint32_t)sp, (uint32_t)(sp >> 32));
-        }
-        if (lane == 0) sts128(mtab + 16 * __popc(smask), 0xffffffffu, 0, 0, 0);
-        __syncwarp();
-        if (T) {
-            uint32_t k = 0;
-            uint4 cur = lds128(mtab);
-            for (uint32_t fb = 0; fb < T; fb += 128) {
-                uint8_t v[4]; uint32_t dd[4];
-#pragma unroll
-                for (int u = 0; u < 4; u++) {
-                    const uint32_t f = fb + 32 * u + lane, f_hi = fb + 32 * u + 31;
-                    uint4 mine = cur;
-                    while (cur.x <= f_hi) {                  // uniform: the current match ends inside this step
-                        const uint32_t prev = cur.x;
-                        k++;
-                        cur = lds128(mtab + 16 * k);
-                        if (f > prev) mine = cur;
-                    }
-                    dd[u] = mine.y + f;
-                    v[u] = 0;
-                    if (f < T) v[u] = __ldcg(reinterpret_cast<const uint8_t*>(((uint64_t)mine.w << 32 | mine.z) + f));
-                }
-#pragma unroll
-                for (int u = 0; u < 4; u++) if (fb + 32 * u + lane < T) out_blk[dd[u]] = v[u];
+            for (int o = 1; o < 32; o <<= 1) { uint32_t a = __shfl_up_sync(0xffffffffu, ce, o); if (lane >= (uint32_t)o) ce += a; }
+            const bool fits = mine && ce <= STAGE_CHUNKS;
+            const uint32_t fmask = __ballot_sync(0xffffffffu, fits);
+            if (fits) {
+                const uint32_t so = 16u * (ce - need);
+                const uint8_t* g = reinterpret_cast<const uint8_t*>(sp - mis);
+                for (uint32_t q = 0; q < need; q++) cp_async16s(stage + so + 16 * q, g + 16 * q);
+                const uint64_t dp = reinterpret_cast<uint64_t>(out_blk) + dst_rel;
+                sts128(mtab + 16 * __popc(fmask & lanemask_lt()), (uint32_t)dp, (uint32_t)(dp >> 32) | (match_len << 24), stage + so + mis, 0);
             }
+            cp_async_commit();
+            cp_async_wait_group<0>();
+            __syncwarp();
+            const uint32_t n_ent = __popc(fmask);
+            for (uint32_t k = 0; k < n_ent; k++) {
+                const uint4 e = lds128(mtab + 16 * k);
+                const uint32_t len = e.y >> 24;
+                uint8_t* dp = reinterpret_cast<uint8_t*>((uint64_t)(e.y & 0xffffffu) << 32 | e.x) + lane;
+                const uint32_t sa = e.z + lane;
+                if (lane < len) dp[0] = (uint8_t)lds8(sa);
+                if (lane + 32 < len) dp[32] = (uint8_t)lds8(sa + 32);
+                for (uint32_t o = 64 + lane; o < len; o += 32) dp[o - lane] = (uint8_t)lds8(sa + o - lane);
+            }
+            __syncwarp();                                    // table and stage are rewritten by the next round
+            pending &= ~fmask;
         }
-        __syncwarp();                                        // the table is rewritten by the next group
         uint32_t longs = __ballot_sync(0xffffffffu, lng);
         while (longs) {
             int l = __ffs(longs) - 1; longs &= longs - 1;
@@ -472,7 +479,7 @@ __device__ __forceinline__ void emit_matches(const Params& P, const BlockCtx& c,
             uint64_t s2 = __shfl_sync(0xffffffffu, src, l);
             warp_copy<true>(out_blk + d2, P.out + (s2 - P.out_pos0), n);
         }
-        uint32_t ovls = __ballot_sync(0xffffffffu, ovl);
+        uint32_t ovls = __ballot_sync(0xffffffffu, direct);
         while (ovls) {                                       // byte i of the match = seed[i mod period] (FORMAT.md §2)
             int l = __ffs(ovls) - 1; ovls &= ovls - 1;
             uint32_t d2 = __shfl_sync(0xffffffffu, dst_rel, l), n = __shfl_sync(0xffffffffu, match_len, l);
@@ -574,63 +581,123 @@ __device__ __forceinline__ void process_demands(const Params& P, uint32_t s_luts
     }
 }
 
-// DEMANDS = false: whole-file schedules (no source can lie outside the output).  true: range / read decode.
-template <bool DEMANDS>
-__global__ void __launch_bounds__(1024, 1) k_decode(const Params P) {
-    // shared memory: [pad to 8 KB][tables: n_coded_tables x 8 KB][rings: warps x 2 KB]  (absolute shared addresses)
-    extern __shared__ __align__(16) uint8_t smem_raw[];
+// shared memory of every decode kernel: [pad to 8 KB][tables: n_coded_tables x 8 KB][rings: warps x 2 KB]
+// [run tables: warps x 2 KB][stack tops: warps x 4]   (absolute shared addresses)
+struct CtaSmem { uint32_t luts, ring, runs, top; };
+
+__device__ __forceinline__ CtaSmem setup_cta(const Params& P, uint8_t* smem_raw) {
     const uint32_t smem0 = (uint32_t)__cvta_generic_to_shared(smem_raw);
     const uint32_t pad = (8192u - (smem0 & 8191u)) & 8191u;
-    const uint32_t s_luts = smem0 + pad;
     const uint32_t n_lut_words = P.n_coded_tables * LUT_SIZE;
     {
         uint4* dstv = reinterpret_cast<uint4*>(smem_raw + pad);
         for (uint32_t i = threadIdx.x; i < n_lut_words / 4; i += blockDim.x) dstv[i] = __ldg(reinterpret_cast<const uint4*>(P.luts) + i);
     }
     __syncthreads();
-    const uint32_t warp = threadIdx.x >> 5, warps_per_cta = blockDim.x >> 5;
-    const uint32_t ring = s_luts + n_lut_words * 4 + warp * RING_BYTES;
-    const uint32_t runs = s_luts + n_lut_words * 4 + warps_per_cta * RING_BYTES + warp * (4 * RUNS_CAP);
+    const uint32_t warp = threadIdx.x >> 5, warps = blockDim.x >> 5;
+    CtaSmem m;
+    m.luts = smem0 + pad;
+    uint32_t base = m.luts + n_lut_words * 4;
+    m.ring = base + warp * RING_BYTES; base += warps * RING_BYTES;
+    m.runs = base + warp * (4 * RUNS_CAP); base += warps * (4 * RUNS_CAP);
+    m.top = base + 4 * warp;
+    return m;
+}
+
+__device__ __forceinline__ bool next_ticket(const Params& P, unsigned long long& t) {
+    t = 0;
+    if (lane_id() == 0) t = atomicAdd(P.ticket, 1ull);
+    t = __shfl_sync(0xffffffffu, t, 0);
+    return t < P.n_work;
+}
+
+// Whole-file literal launch (mode 2): A1 + A2 + A3 for every block, no dependencies.
+template <int MAXT>
+__global__ void __launch_bounds__(MAXT, 1) k_literals(const Params P) {
+    extern __shared__ __align__(16) uint8_t smem_raw[];
+    const CtaSmem m = setup_cta(P, smem_raw);
     BlockCtx c;
-    bind_scratch(P, blockIdx.x * warps_per_cta + warp, c);
+    bind_scratch(P, blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), c);
+    Stack st{nullptr, 0, m.top};
+    unsigned long long t;
+    while (next_ticket(P, t)) {
+        c.b = P.first_block + t;
+        Rans r; uint32_t i0;
+        if (!parse_tokens(P, m.luts, m.ring, c, r, &i0)) continue;
+        uint32_t n_runs = P.log2_bs <= 16 ? build_runs(P, c, m.runs) : 0xffffffffu;
+        if (n_runs != 0xffffffffu) {                          // scan first, literals straight to their positions
+            decode_lit_direct(r, m.luts + P.lut_lit * (4 * LUT_SIZE), i0, c.d.n_lit, m.runs, P.out + (c.bstart - P.out_pos0));
+            rans_final_ok(P, c, r);
+        } else {                                              // too many runs / big block / bad scan: staged path
+            rans_region<false>(r, m.luts + P.lut_lit * (4 * LUT_SIZE), i0, c.d.n_lit, c.lit);
+            bool ok = rans_final_ok(P, c, r);
+            __syncwarp();
+            if (ok) emit_block<2>(P, c, st);
+        }
+    }
+}
+
+// Whole-file match launches.  WAIT = false (mode 3): one dependency level per launch, nothing to wait for.
+// WAIT = true (mode 4): all levels in one launch; blocks arrive sorted by (level, index) and a block waits for the
+// completion of lower-level source blocks, which were dispatched before it.
+template <bool WAIT, int MAXT>
+__global__ void __launch_bounds__(MAXT, 1) k_matches(const Params P) {
+    // shared memory: [pad to 8 KB][tables without LIT (the last one): (n_coded_tables - 1) x 8 KB]
+    //                [per warp: ring 2 KB | match table MTAB_BYTES | stage 16 x STAGE_CHUNKS]
+    extern __shared__ __align__(16) uint8_t smem_raw[];
+    const uint32_t smem0 = (uint32_t)__cvta_generic_to_shared(smem_raw);
+    const uint32_t pad = (8192u - (smem0 & 8191u)) & 8191u;
+    const uint32_t n_lut_words = (P.n_coded_tables - 1) * LUT_SIZE;
+    {
+        uint4* dstv = reinterpret_cast<uint4*>(smem_raw + pad);
+        for (uint32_t i = threadIdx.x; i < n_lut_words / 4; i += blockDim.x) dstv[i] = __ldg(reinterpret_cast<const uint4*>(P.luts) + i);
+    }
+    __syncthreads();
+    const uint32_t warp = threadIdx.x >> 5;
+    const uint32_t luts = smem0 + pad;
+    const uint32_t ring = luts + n_lut_words * 4 + warp * (RING_BYTES + MTAB_BYTES + 16 * STAGE_CHUNKS);
+    const uint32_t mtab = ring + RING_BYTES, stage = mtab + MTAB_BYTES;
+    BlockCtx c;
+    bind_scratch(P, blockIdx.x * (blockDim.x >> 5) + warp, c);
+    unsigned long long t;
+    while (next_ticket(P, t)) {
+        c.b = P.level_list ? (uint64_t)P.level_list[t] : P.first_block + t;
+        if (parse_block(P, luts, ring, c, 0, false)) emit_matches<WAIT ? 4 : 3>(P, c, mtab, stage);
+        if (WAIT) {
+            __threadfence();
+            __syncwarp();
+            if (lane_id() == 0) st_release(P.flags + c.b, 2 * P.epoch + 1);
+        }
+    }
+}
+
+template <bool DEMANDS>
+__global__ void __launch_bounds__(1024, 1) k_decode(const Params P) {
+    extern __shared__ __align__(16) uint8_t smem_raw[];
+    const CtaSmem m = setup_cta(P, smem_raw);
+    const uint32_t s_luts = m.luts, ring = m.ring, runs = m.runs;
+    const uint32_t gw = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    BlockCtx c;
+    bind_scratch(P, gw, c);
     Stack st;
-    st.base = P.stacks + (uint64_t)(blockIdx.x * warps_per_cta + warp) * P.stack_cap; st.cap = P.stack_cap;
-    st.top = s_luts + n_lut_words * 4 + warps_per_cta * (RING_BYTES + 4 * RUNS_CAP) + 4 * warp;
-    const uint32_t mtab = s_luts + n_lut_words * 4 + warps_per_cta * (RING_BYTES + 4 * RUNS_CAP + 4) + warp * MTAB_BYTES;
+    st.base = P.stacks + (uint64_t)gw * P.stack_cap; st.cap = P.stack_cap; st.top = m.top;
     if (lane_id() == 0) asm volatile("st.shared.u32 [%0], %1;" ::"r"(st.top), "r"(0u) : "memory");
     __syncwarp();
-    for (;;) {
-        unsigned long long t = 0;
-        if (lane_id() == 0) t = atomicAdd(P.ticket, 1ull);
-        t = __shfl_sync(0xffffffffu, t, 0);
-        if (t >= P.n_work) break;
+    unsigned long long t;
+    while (next_ticket(P, t)) {
         if (DEMANDS && P.mode == 1) {                        // spans: one top-level demand per ticket
             if (lane_id() == 0) push_span(P, st, P.demands[t].pos, P.demands[t].len, P.demands[t].dst);
             process_demands(P, s_luts, ring, c, st);
             continue;
         }
         c.b = P.level_list ? (uint64_t)P.level_list[t] : P.first_block + t;
-        if (P.mode == 3) {
-            // match wave: only the command / length / offset streams are needed again
-            if (parse_block(P, s_luts, ring, c, 0)) emit_matches<3>(P, c, mtab);
-            continue;
-        }
-        if (P.mode == 4) {
-            // all match waves in one launch: blocks arrive sorted by (level, index), a block waits for the completion
-            // of lower-level source blocks, which were dispatched before it
-            if (parse_block(P, s_luts, ring, c, 0)) emit_matches<4>(P, c, mtab);
-            __threadfence();
-            __syncwarp();
-            if (lane_id() == 0) st_release(P.flags + c.b, 2 * P.epoch + 1);
-            continue;
-        }
-        // modes 0 (everything, flags) and 2 (literal launch): A1 + A2 + A3
+        // mode 0: everything for one block (A1 + A2 + A3, then A4 with flags)
         bool ok;
         {
             Rans r; uint32_t i0;
             ok = parse_tokens(P, s_luts, ring, c, r, &i0);
             if (ok) {
-                if (P.mode == 0) prefetch_sources(P, c);              // source lines travel to L2 while the literals decode
+                prefetch_sources(P, c);                               // source lines travel to L2 while the literals decode
                 uint32_t n_runs = P.log2_bs <= 16 ? build_runs(P, c, runs) : 0xffffffffu;
                 if (n_runs != 0xffffffffu) {                          // scan first, literals straight to their positions
                     decode_lit_direct(r, s_luts + P.lut_lit * (4 * LUT_SIZE), i0, c.d.n_lit, runs, P.out + (c.bstart - P.out_pos0));
@@ -643,18 +710,16 @@ __global__ void __launch_bounds__(1024, 1) k_decode(const Params P) {
                 }
             }
         }
-        if (P.mode == 0) {
-            __threadfence();
-            __syncwarp();
-            if (lane_id() == 0) st_release(P.flags + c.b, 2 * P.epoch);       // literals placed
-            const uint64_t b0 = c.b;
-            if (ok) emit_block<0, DEMANDS>(P, c, st);                         // A4 (waits on source blocks)
-            if (DEMANDS && lds_top(st)) process_demands(P, s_luts, ring, c, st);   // sources below the window (range decode)
-            c.b = b0;
-            __threadfence();
-            __syncwarp();
-            if (lane_id() == 0) st_release(P.flags + c.b, 2 * P.epoch + 1);   // complete (set even on error: nobody waits forever)
-        }
+        __threadfence();
+        __syncwarp();
+        if (lane_id() == 0) st_release(P.flags + c.b, 2 * P.epoch);       // literals placed
+        const uint64_t b0 = c.b;
+        if (ok) emit_block<0, DEMANDS>(P, c, st);                         // A4 (waits on source blocks)
+        if (DEMANDS && lds_top(st)) process_demands(P, s_luts, ring, c, st);   // sources below the window (range decode)
+        c.b = b0;
+        __threadfence();
+        __syncwarp();
+        if (lane_id() == 0) st_release(P.flags + c.b, 2 * P.epoch + 1);   // complete (set even on error: nobody waits forever)
     }
 }
 
@@ -694,7 +759,7 @@ struct aceapex_archive {
     uint32_t epoch = 0;
     Resident res[MAX_RESIDENT];
     // launch geometry
-    int sms = 148, ctas_per_sm = 1, threads = 1024;
+    int sms = 148, ctas_per_sm = 1, threads = 1024, threads_lit = 1024, threads_match = 1024;
     uint32_t grid = 0; size_t smem = 0;
     uint64_t scratch_per_warp = 0, ctrl_bytes = 0, flags_bytes = 0;
     uint64_t scratch_off = 0, stacks_off = 0, demands_off = 0, list_off = 0, ws_need = 0;
@@ -718,6 +783,13 @@ uint64_t align_up(uint64_t v, uint64_t a) { return (v + a - 1) / a * a; }
 // workspace: [ctrl 256 B: ticket u64 @0, err u32 @8][flags: n_blocks x u32][scratch: warps x scratch_per_warp]
 //            [stacks: warps x stack_cap demands][demands: demand_cap][block list: n_blocks x u32]
 uint64_t workspace_need(const aceapex_archive* ar) { return ar->ws_need; }
+
+size_t smem_for(const aceapex_archive* ar, int threads) {
+    return (size_t)8192 + (size_t)ar->n_coded_tables * LUT_SIZE * 4 + (size_t)(threads / 32) * (RING_BYTES + 4 * RUNS_CAP + 4);
+}
+size_t smem_matches(const aceapex_archive* ar, int threads) {
+    return (size_t)8192 + (size_t)(ar->n_coded_tables - 1) * LUT_SIZE * 4 + (size_t)(threads / 32) * (RING_BYTES + MTAB_BYTES + 16 * STAGE_CHUNKS);
+}
 
 void layout_workspace(aceapex_archive* ar) {
     uint64_t warps = (uint64_t)ar->grid * (ar->threads / 32);
@@ -768,7 +840,17 @@ int32_t launch(aceapex_archive* ar, Params& P, uint64_t n_work) {
     CU(cudaMemsetAsync(P.ticket, 0, 8, ar->stream));
     uint64_t warps = ar->threads / 32;
     uint32_t grid = (uint32_t)std::min<uint64_t>(ar->grid, (n_work + warps - 1) / warps);
-    if (P.mode == 1 || P.out_pos0 != 0 || P.win_end != ar->N) k_decode<true><<<grid, ar->threads, ar->smem, ar->stream>>>(P);
+    const bool whole = P.out_pos0 == 0 && P.win_end == ar->N;
+    if (whole && P.mode >= 2) {                               // specialised whole-file kernels
+        const int T = P.mode == 2 ? ar->threads_lit : ar->threads_match;
+        const size_t sm = P.mode == 2 ? smem_for(ar, T) : smem_matches(ar, T);
+        uint64_t w = T / 32;
+        uint32_t g = (uint32_t)std::min<uint64_t>(ar->sms, (n_work + w - 1) / w);
+        if (P.mode == 2) { if (T == 768) k_literals<768><<<g, T, sm, ar->stream>>>(P); else k_literals<1024><<<g, T, sm, ar->stream>>>(P); }
+        else if (P.mode == 3) { if (T == 768) k_matches<false, 768><<<g, T, sm, ar->stream>>>(P); else k_matches<false, 1024><<<g, T, sm, ar->stream>>>(P); }
+        else { if (T == 768) k_matches<true, 768><<<g, T, sm, ar->stream>>>(P); else k_matches<true, 1024><<<g, T, sm, ar->stream>>>(P); }
+    }
+    else if (P.mode == 1 || !whole) k_decode<true><<<grid, ar->threads, ar->smem, ar->stream>>>(P);
     else k_decode<false><<<grid, ar->threads, ar->smem, ar->stream>>>(P);
     CU(cudaGetLastError());
     ar->launches++;
@@ -884,16 +966,23 @@ int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* 
     ar->sms = prop.multiProcessorCount;
     // one CTA per SM: the decode tables are staged once per SM and shared by all its warps (fewer warps when many
     // offset planes are coded and the tables leave less room)
-    auto smem_for = [&](int threads) {
-        return (size_t)8192 + (size_t)ar->n_coded_tables * LUT_SIZE * 4 + (size_t)(threads / 32) * (RING_BYTES + 4 * RUNS_CAP + 4 + MTAB_BYTES);
-    };
     ar->threads = 1024;
-    while (ar->threads > 128 && smem_for(ar->threads) > (size_t)prop.sharedMemPerBlockOptin) ar->threads -= 128;
-    ar->smem = smem_for(ar->threads);
-    CU(cudaFuncSetAttribute(k_decode<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ar->smem));
-    CU(cudaFuncSetAttribute(k_decode<false>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
-    CU(cudaFuncSetAttribute(k_decode<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ar->smem));
-    CU(cudaFuncSetAttribute(k_decode<true>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+    while (ar->threads > 128 && std::max(smem_for(ar, ar->threads), smem_matches(ar, ar->threads)) > (size_t)prop.sharedMemPerBlockOptin) ar->threads -= 128;
+    ar->smem = smem_for(ar, ar->threads);
+    ar->threads_lit = ar->threads_match = ar->threads;
+    if (ar->threads == 1024) {                                // 768-thread variants trade occupancy for registers (80 vs 64)
+        if (const char* e = getenv("ACEAPEX_LIT_THREADS")) if (atoi(e) == 768) ar->threads_lit = 768;
+        if (const char* e = getenv("ACEAPEX_MATCH_THREADS")) if (atoi(e) == 768) ar->threads_match = 768;
+    }
+    {
+        const void* fns[] = {(const void*)k_decode<false>, (const void*)k_decode<true>, (const void*)k_literals<1024>, (const void*)k_literals<768>,
+                             (const void*)k_matches<false, 1024>, (const void*)k_matches<false, 768>, (const void*)k_matches<true, 1024>,
+                             (const void*)k_matches<true, 768>};
+        for (const void* f : fns) {
+            CU(cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max(ar->smem, smem_matches(ar, ar->threads))));
+            CU(cudaFuncSetAttribute(f, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+        }
+    }
     int occ = 0;
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_decode<true>, ar->threads, ar->smem));
     if (occ < 1) return ACEAPEX_E_CUDA;

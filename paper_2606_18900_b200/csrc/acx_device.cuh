@@ -71,6 +71,12 @@ __device__ __forceinline__ void st_release(uint32_t* p, uint32_t v) {
 }
 // data that other SMs may have written during this kernel: read at L2, never from a stale L1 line
 __device__ __forceinline__ uint8_t ldcg8(const uint8_t* p) { return __ldcg(p); }
+// predicated byte load at L2; the result is unspecified (0) when pred is false
+__device__ __forceinline__ uint32_t ldcg8_if(const uint8_t* p, bool pred) {
+    uint32_t v = 0;
+    asm volatile("{ .reg .pred q; setp.ne.u32 q, %2, 0; @q ld.global.cg.u8 %0, [%1]; }" : "+r"(v) : "l"(p), "r"((uint32_t)pred) : "memory");
+    return v;
+}
 __device__ __forceinline__ uint64_t ldcg64(const uint8_t* p) { return __ldcg(reinterpret_cast<const unsigned long long*>(p)); }
 
 
@@ -81,6 +87,7 @@ __device__ __forceinline__ uint64_t ldcg64(const uint8_t* p) { return __ldcg(rei
 // use).  Every table (8 KB aligned) and every ring (64 B aligned) sits at an aligned shared address so that an index
 // folds into an address with one LOP3.
 __device__ __forceinline__ uint32_t lds32(uint32_t a) { uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a)); return v; }
+__device__ __forceinline__ uint32_t lds8(uint32_t a) { uint32_t v; asm volatile("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(a)); return v; }
 __device__ __forceinline__ uint32_t lds16(uint32_t a) { uint32_t v; asm volatile("ld.shared.u16 %0, [%1];" : "=r"(v) : "r"(a)); return v; }
 __device__ __forceinline__ void cp_async16s(uint32_t saddr, const void* gmem) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(saddr), "l"(gmem) : "memory");
