@@ -383,8 +383,9 @@ __device__ __forceinline__ void emit_block(const Params& P, const BlockCtx& c, c
 // the 16-byte warp copy; self-overlapping ones read src + (i mod period).  By FORMAT.md §3 no match reads match bytes of
 // its own block, so the loads of a block never depend on its stores.
 constexpr uint32_t LONG_MATCH = 192;
-constexpr uint32_t MTAB_BYTES = 32 * 16;   // per warp: 32 entries {destination pointer | len << 56, shared address of the staged source}
+constexpr uint32_t MTAB_BYTES = 36 * 16;   // per warp: 32 entries (+ 1 empty; a multiple of 64 bytes keeps the rings aligned) {destination pointer | len << 56, shared address of the staged source}
 constexpr uint32_t STAGE_CHUNKS = 160;     // per warp: 2560 bytes of staged source data
+static_assert((RING_BYTES + MTAB_BYTES + 16 * STAGE_CHUNKS) % 64 == 0, "per-warp shared memory must keep 64-byte ring alignment");
 static_assert(LONG_MATCH < 256 && (15 + LONG_MATCH + 15) / 16 <= STAGE_CHUNKS, "a short match has an 8-bit length and fits the stage");
 
 __device__ __forceinline__ void sts128(uint32_t a, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
@@ -403,10 +404,15 @@ __device__ __forceinline__ void emit_matches(const Params& P, const BlockCtx& c,
     uint32_t lit_base = 0, out_base = 0, ec = 0, em = c.n_ext_cmd;
     const uint32_t lane = lane_id();
     uint8_t* const out_blk = P.out + (c.bstart - P.out_pos0);
+    // tokens and offsets of a group are loaded one group ahead, so that their latency overlaps the copies
+    uint32_t n_tl = 0, n_tm = 0; uint64_t n_src = 0;
+    { uint32_t ci = lane; if (ci < c.d.n_cmd) n_tl = c.tok_cmd[ci]; if (ci < c.d.n_match) { n_tm = c.tok_mlen[ci]; n_src = match_src(P, c, ci); } }
     for (uint32_t c0 = 0; c0 < c.d.n_cmd; c0 += 32) {
         uint32_t ci = c0 + lane;
         bool valid = ci < c.d.n_cmd, has_match = ci < c.d.n_match;
-        uint32_t tl = valid ? c.tok_cmd[ci] : 0, tm = has_match ? c.tok_mlen[ci] : 0;
+        const uint32_t tl = n_tl, tm = n_tm; const uint64_t src = n_src;
+        { uint32_t cn = ci + 32; n_tl = 0; n_tm = 0; n_src = 0;
+          if (cn < c.d.n_cmd) n_tl = c.tok_cmd[cn]; if (cn < c.d.n_match) { n_tm = c.tok_mlen[cn]; n_src = match_src(P, c, cn); } }
         uint32_t ml = __ballot_sync(0xffffffffu, valid && tl == 255), mm = __ballot_sync(0xffffffffu, has_match && tm == 255);
         uint32_t lit_len = tl, match_len = has_match ? P.min_match + tm : 0;
         if (valid && tl == 255) lit_len = 255 + __ldg(c.ext + ec + __popc(ml & lanemask_lt()));
@@ -424,7 +430,7 @@ __device__ __forceinline__ void emit_matches(const Params& P, const BlockCtx& c,
         out_base += __shfl_sync(0xffffffffu, st, 31);
         bool ok = valid && (uint64_t)lit_pos + lit_len <= c.d.n_lit && c.bstart + dst_rel + match_len <= c.bend;
         if (__any_sync(0xffffffffu, valid && !ok)) { if (lane == 0) report(P, DF_LENGTH); return; }
-        uint64_t dst = c.bstart + dst_rel, src = (ok && has_match) ? match_src(P, c, ci) : 0;
+        uint64_t dst = c.bstart + dst_rel;
         bool good = ok && has_match && src < dst;
         if (ok && has_match && !good) report(P, DF_OFFSET);
         if (MODE == 4 && good && c.d.level) wait_sources<false>(P, c, dst, src, match_len);
@@ -456,18 +462,31 @@ __device__ __forceinline__ void emit_matches(const Params& P, const BlockCtx& c,
                 const uint64_t dp = reinterpret_cast<uint64_t>(out_blk) + dst_rel;
                 sts128(mtab + 16 * __popc(fmask & lanemask_lt()), (uint32_t)dp, (uint32_t)(dp >> 32) | (match_len << 24), stage + so + mis, 0);
             }
+            const uint32_t n_ent = __popc(fmask);
+            if (lane == 0) sts128(mtab + 16 * n_ent, 0, 0, 0, 0);       // empty entry: matches are taken two at a time
             cp_async_commit();
             cp_async_wait_group<0>();
             __syncwarp();
-            const uint32_t n_ent = __popc(fmask);
-            for (uint32_t k = 0; k < n_ent; k++) {
+            uint32_t more = 0;
+            for (uint32_t k = 0; k < n_ent; k += 2) {
+                const uint4 e0 = lds128(mtab + 16 * k), e1 = lds128(mtab + 16 * k + 16);
+                const uint32_t l0 = e0.y >> 24, l1 = e1.y >> 24;
+                const uint32_t a0 = e0.z + lane, a1 = e1.z + lane;
+                const uint32_t v00 = lds8(a0), v01 = lds8(a0 + 32), v10 = lds8(a1), v11 = lds8(a1 + 32);
+                uint8_t* d0 = reinterpret_cast<uint8_t*>((uint64_t)(e0.y & 0xffffffu) << 32 | e0.x) + lane;
+                uint8_t* d1 = reinterpret_cast<uint8_t*>((uint64_t)(e1.y & 0xffffffu) << 32 | e1.x) + lane;
+                if (lane < l0) d0[0] = (uint8_t)v00;
+                if (lane + 32 < l0) d0[32] = (uint8_t)v01;
+                if (lane < l1) d1[0] = (uint8_t)v10;
+                if (lane + 32 < l1) d1[32] = (uint8_t)v11;
+                more |= (l0 > 64 ? 1u : 0u) << k | (l1 > 64 ? 2u : 0u) << k;
+            }
+            while (more) {                                   // bytes 64.. of the longer ones (about one match in nine on FASTQ)
+                const int k = __ffs(more) - 1; more &= more - 1;
                 const uint4 e = lds128(mtab + 16 * k);
-                const uint32_t len = e.y >> 24;
+                const uint32_t len = e.y >> 24, sa = e.z + lane;
                 uint8_t* dp = reinterpret_cast<uint8_t*>((uint64_t)(e.y & 0xffffffu) << 32 | e.x) + lane;
-                const uint32_t sa = e.z + lane;
-                if (lane < len) dp[0] = (uint8_t)lds8(sa);
-                if (lane + 32 < len) dp[32] = (uint8_t)lds8(sa + 32);
-                for (uint32_t o = 64 + lane; o < len; o += 32) dp[o - lane] = (uint8_t)lds8(sa + o - lane);
+                for (uint32_t o = 64; o + lane < len; o += 32) dp[o] = (uint8_t)lds8(sa + o);
             }
             __syncwarp();                                    // table and stage are rewritten by the next round
             pending &= ~fmask;
@@ -663,10 +682,9 @@ __global__ void __launch_bounds__(MAXT, 1) k_matches(const Params P) {
     while (next_ticket(P, t)) {
         c.b = P.level_list ? (uint64_t)P.level_list[t] : P.first_block + t;
         if (parse_block(P, luts, ring, c, 0, false)) emit_matches<WAIT ? 4 : 3>(P, c, mtab, stage);
-        if (WAIT) {
-            __threadfence();
+        if (WAIT) {                                          // publish: the warp's stores happen-before lane 0's fence + release
             __syncwarp();
-            if (lane_id() == 0) st_release(P.flags + c.b, 2 * P.epoch + 1);
+            if (lane_id() == 0) { __threadfence(); st_release(P.flags + c.b, 2 * P.epoch + 1); }
         }
     }
 }
@@ -788,7 +806,7 @@ size_t smem_for(const aceapex_archive* ar, int threads) {
     return (size_t)8192 + (size_t)ar->n_coded_tables * LUT_SIZE * 4 + (size_t)(threads / 32) * (RING_BYTES + 4 * RUNS_CAP + 4);
 }
 size_t smem_matches(const aceapex_archive* ar, int threads) {
-    return (size_t)8192 + (size_t)(ar->n_coded_tables - 1) * LUT_SIZE * 4 + (size_t)(threads / 32) * (RING_BYTES + MTAB_BYTES + 16 * STAGE_CHUNKS);
+    return (size_t)8192 + (size_t)(ar->n_coded_tables - 1) * LUT_SIZE * 4 + (size_t)(threads / 32) * (RING_BYTES + MTAB_BYTES + 16 * STAGE_CHUNKS) + 64;   // + 64: the copy reads bytes i and i + 32 unconditionally
 }
 
 void layout_workspace(aceapex_archive* ar) {
