@@ -1,0 +1,271 @@
+#!/usr/bin/env python
+"""Measurements for BASELINE.json configs[0..4] (one JSON line per measurement).
+
+  python -m paper_2606_18900_b200.report --config 1            # 1 GiB FASTQ: whole-file, range windows, reads
+  python -m paper_2606_18900_b200.report --config 2            # 3.1 GB FASTA + 10^6 region reads (batch 1 / 4096)
+  python -m paper_2606_18900_b200.report --config 3 --size N   # N bytes of FASTA (default 50 GiB) through an 8 GiB ring
+  python -m paper_2606_18900_b200.report --config 4            # block-size sweep on the configs[1] FASTQ
+
+Everything is verified against the ORIGINAL bytes (direct compare where the data fits, per-block FNV-1a otherwise).
+Timing: CUDA events on the handle's stream around the C-ABI calls, after warm-up; GB = 10^9 bytes.
+CPU baselines (oracle, multithreaded decoder) are timed by bench.py, not here: the product never imports oracle/."""
+import argparse
+import json
+import os
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+PEAK_FALLBACK = 6650.0
+
+
+def peak_gbs():
+    try:
+        return float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]), "measured"
+    except Exception:
+        return PEAK_FALLBACK, "fallback"
+
+
+def emit(**kw):
+    print(json.dumps(kw), flush=True)
+
+
+def timed(torch, stream, fn, reps, warmup=1):
+    for _ in range(warmup):
+        fn()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(reps):
+        fn()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / reps
+
+
+def roofline(info, ms, out_bytes=None):
+    peak, how = peak_gbs()
+    n = info["raw_bytes"] if out_bytes is None else out_bytes
+    scale = n / max(info["raw_bytes"], 1)
+    alg = (info["archive_bytes"] + info["total_match_bytes"] + info["raw_bytes"]) * scale
+    ach = alg / (ms * 1e-3) / 1e9
+    return {"bound": "hbm", "achieved": ach, "peak": peak, "peak_source": how, "unit": "GB/s", "frac": ach / peak,
+            "frac_of_8TBs": ach / 8000.0}
+
+
+def whole_file(torch, ar, x, label, reps=5):
+    stream = torch.cuda.current_stream()
+    ar.set_stream(stream)
+    out = ar.new_output()
+    info = ar.info()
+    res = {}
+    xt = torch.from_numpy(x).to(out.device) if x is not None else None
+    for sched in (None, "levels", "fused"):
+        out.zero_()
+        ar.decode_all(out, schedule=sched)
+        ar.check()
+        ok = bool(torch.equal(out[:info["raw_bytes"]], xt)) if xt is not None else None
+        fnv_bad = ar.verify_fnv(out) if info["has_fnv"] else None
+        l0 = ar.launch_count()
+        ms = timed(torch, stream, lambda: ar.decode_all(out, schedule=sched), reps)
+        res[sched or "default"] = {"ms": ms, "GBps": info["raw_bytes"] / ms / 1e6, "bit_exact": ok, "fnv_bad_blocks": fnv_bad,
+                                   "launches": (ar.launch_count() - l0) // (reps + 1)}
+    d = res["default"]
+    emit(config=label, what="decode_all", raw_bytes=info["raw_bytes"], archive_bytes=info["archive_bytes"],
+         ratio=info["raw_bytes"] / info["archive_bytes"], n_blocks=info["n_blocks"], block_size=info["block_size"],
+         max_level=info["max_level"], schedules=res, roofline=roofline(info, d["ms"]))
+    del out, xt
+    return res
+
+
+def windows(torch, ar, x, label, window, ring_slots, reps=1, sample_check=None):
+    """Whole file as consecutive windows through a ring of `ring_slots` buffers that stay resident as sources."""
+    stream = torch.cuda.current_stream()
+    ar.set_stream(stream)
+    info = ar.info()
+    N = info["raw_bytes"]
+    ring = [ar.new_output(window) for _ in range(ring_slots)]
+    nwin = (N + window - 1) // window
+    per_win, bad = [], 0
+    for rep in range(reps + 1):
+        for s in range(ring_slots):
+            ar.set_resident(s, 0, 0, None)
+        t_all = 0.0
+        per_win = []
+        for w in range(nwin):
+            lo, hi = w * window, min(N, (w + 1) * window)
+            s = w % ring_slots
+            ar.set_resident(s, 0, 0, None)             # about to be overwritten
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            ar.decode_range(lo, hi, out=ring[s])
+            e1.record(stream)
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1)
+            t_all += ms
+            per_win.append((hi - lo) / ms / 1e6)
+            if rep == 0:                                # verify once (the consumer of the ring)
+                ar.check()
+                if info["has_fnv"]:
+                    bad += ar.verify_fnv(ring[s], lo, hi)
+                if x is not None and (sample_check is None or w in sample_check):
+                    if not torch.equal(ring[s][:hi - lo].cpu(), torch.from_numpy(x[lo:hi])):
+                        bad += 1
+            ar.set_resident(s, lo, hi, ring[s])
+    for s in range(ring_slots):
+        ar.set_resident(s, 0, 0, None)
+    emit(config=label, what="range_windows_through_ring", window_bytes=window, ring_bytes=window * ring_slots, windows=nwin,
+         total_ms=t_all, GBps=N / t_all / 1e6, GBps_min=min(per_win), GBps_max=max(per_win),
+         GBps_first_mid_last=[per_win[0], per_win[len(per_win) // 2], per_win[-1]], bad=bad,
+         roofline=roofline(info, t_all), peak_vram_bytes=int(torch.cuda.max_memory_allocated()))
+    return bad
+
+
+def isolated_windows(torch, ar, x, label, window):
+    """1 GiB-style windows decoded in isolation (nothing resident): start / middle / end of the file."""
+    stream = torch.cuda.current_stream()
+    info = ar.info()
+    N = info["raw_bytes"]
+    buf = ar.new_output(window)
+    res = {}
+    for name, lo in (("start", 0), ("middle", (N // 2) & ~(window - 1) if N >= 2 * window else 0), ("end", max(0, N - window))):
+        hi = min(N, lo + window)
+        ar.decode_range(lo, hi, out=buf)
+        ar.check()
+        ok = None
+        if x is not None:
+            ok = bool(torch.equal(buf[:hi - lo].cpu(), torch.from_numpy(x[lo:hi])))
+        ms = timed(torch, stream, lambda: ar.decode_range(lo, hi, out=buf), 2, warmup=0)
+        res[name] = {"lo": lo, "hi": hi, "ms": ms, "GBps": (hi - lo) / ms / 1e6, "bit_exact": ok}
+    emit(config=label, what="isolated_windows", window_bytes=window, windows=res)
+
+
+def reads(torch, ar, x, idx, label, n_single=1000, n_batches=20, batch=4096, seed=5):
+    stream = torch.cuda.current_stream()
+    rng = np.random.default_rng(seed)
+    off = (idx & np.uint64((1 << 40) - 1)).astype(np.int64)
+    ln = (idx >> np.uint64(40)).astype(np.int64)
+    out = ar.new_output(int(ln.max()) * batch)
+    # batch 1: sequential single calls (the call synchronises and returns the read); wall clock per call
+    ids = rng.integers(0, idx.size, n_single).astype(np.uint64)
+    for i in ids[:20]:
+        ar.decode_reads(idx, np.array([i], dtype=np.uint64), out=out)
+    lat = []
+    ok = True
+    for i in ids:
+        one = np.array([i], dtype=np.uint64)
+        t = time.perf_counter()
+        ar.decode_reads(idx, one, out=out)
+        lat.append((time.perf_counter() - t) * 1e3)
+    for i in ids[:50]:
+        ar.decode_reads(idx, np.array([i], dtype=np.uint64), out=out)
+        got = out[:ln[i]].cpu().numpy()
+        ok = ok and got.tobytes() == x[off[i]:off[i] + ln[i]].tobytes()
+    ar.check()
+    lat = np.array(lat)
+    b_ms, ok_b = [], True
+    for k in range(n_batches):
+        bi = rng.integers(0, idx.size, batch).astype(np.uint64)
+        if k == 0:
+            ar.decode_reads(idx, bi, out=out)           # warm-up
+        t = time.perf_counter()
+        ar.decode_reads(idx, bi, out=out)
+        b_ms.append((time.perf_counter() - t) * 1e3)
+        if k < 2:
+            total, offs = ar.reads_bytes(idx, bi)
+            got = out[:total].cpu().numpy()
+            for j in range(0, batch, 37):
+                r = int(bi[j])
+                ok_b = ok_b and got[int(offs[j]):int(offs[j]) + ln[r]].tobytes() == x[off[r]:off[r] + ln[r]].tobytes()
+    ar.check()
+    b_ms = np.array(b_ms)
+    emit(config=label, what="random_reads", index_entries=int(idx.size), index_bytes=int(idx.nbytes),
+         batch1={"n": n_single, "ms_median": float(np.median(lat)), "ms_p99": float(np.percentile(lat, 99)), "ms_min": float(lat.min()),
+                 "bit_exact": ok},
+         batched={"batch": batch, "n_batches": n_batches, "ms_per_batch_median": float(np.median(b_ms)),
+                  "us_per_read": float(np.median(b_ms)) * 1e3 / batch, "bit_exact": ok_b})
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--config", type=int, required=True)
+    ap.add_argument("--size", type=int, default=0)
+    args = ap.parse_args()
+    import torch
+    from paper_2606_18900_b200 import datagen, encoder
+    from paper_2606_18900_b200.aceapex import Archive
+    emit(what="box", cores=os.cpu_count(), gpu=torch.cuda.get_device_name(0), peak=peak_gbs())
+    if args.config in (0, 1):
+        size, seed, ref = ((4 << 20), 1, 1_000_000) if args.config == 0 else ((1 << 30), 2, 50_000_000)
+        size = args.size or size
+        x = datagen.fastq(seed, size, ref)
+        t = time.time()
+        a = encoder.encode(x, block_size=16384)
+        emit(config=args.config, what="encode", seconds=time.time() - t, MBps=x.size / (time.time() - t) / 1e6)
+        ar = Archive(a)
+        whole_file(torch, ar, x, args.config)
+        win = min(64 << 20, max(1 << 20, size // 16))
+        windows(torch, ar, x, args.config, win, 2)
+        isolated_windows(torch, ar, x, args.config, win)
+        reads(torch, ar, x, datagen.fastq_index(size), args.config)
+        ar.close()
+    elif args.config == 2:
+        size = args.size or 3_100_000_000
+        t = time.time()
+        x = datagen.fasta(3, size)
+        emit(config=2, what="generate", seconds=time.time() - t)
+        t = time.time()
+        a = encoder.encode(x, block_size=16384)
+        emit(config=2, what="encode", seconds=time.time() - t, MBps=x.size / (time.time() - t) / 1e6)
+        ar = Archive(a)
+        whole_file(torch, ar, x, 2, reps=3)
+        idx = datagen.region_index(3, size, 1_000_000, 150)
+        reads(torch, ar, x, idx, 2, n_single=2000, n_batches=1_000_000 // 4096)
+        isolated_windows(torch, ar, x, 2, 1 << 28)
+        ar.close()
+    elif args.config == 3:
+        size = args.size or (50 << 30)
+        t = time.time()
+        x = datagen.fasta(4, size)
+        emit(config=3, what="generate", seconds=time.time() - t, bytes=size)
+        t = time.time()
+        a = encoder.encode(x, block_size=16384)
+        emit(config=3, what="encode", seconds=time.time() - t, MBps=x.size / (time.time() - t) / 1e6, archive_bytes=int(a.size))
+        ar = Archive(a)
+        info = ar.info()
+        emit(config=3, what="archive", raw_bytes=info["raw_bytes"], archive_bytes=info["archive_bytes"], n_blocks=info["n_blocks"],
+             offset_width=info["offset_width"], max_level=info["max_level"], workspace_bytes=info["workspace_bytes"])
+        window = min(1 << 30, max(1 << 24, size // 8))
+        nwin = (size + window - 1) // window
+        windows(torch, ar, x, 3, window, 8, reps=1, sample_check={0, nwin // 2, nwin - 1})
+        isolated_windows(torch, ar, x, 3, window)
+        ar.close()
+    elif args.config == 4:
+        size = args.size or (1 << 30)
+        x = datagen.fastq(2, size, 50_000_000)
+        for bs in (4096, 8192, 16384, 65536, 262144, 1 << 20):
+            t = time.time()
+            a = encoder.encode(x, block_size=bs)
+            enc_s = time.time() - t
+            ar = Archive(a)
+            res = whole_file(torch, ar, x, "4/bs=%d" % bs, reps=3)
+            n_blocks, dir_off = int(a[24:32].view(np.uint64)[0]), int(a[72:80].view(np.uint64)[0])   # FORMAT.md §1.1
+            lv = np.frombuffer(a[dir_off:dir_off + 32 * n_blocks].tobytes(), dtype=np.uint16).reshape(-1, 16)[:, 14]   # §1.3 level
+            # per-launch overhead (S19): level schedule time minus the two-launch time, per extra launch
+            extra = res["levels"]["launches"] - res["default"]["launches"]
+            emit(config=4, what="block_size_point", block_size=bs, ratio=x.size / a.size, encode_seconds=enc_s,
+                 GBps=res["default"]["GBps"], ms=res["default"]["ms"], mean_level=float(lv.mean()), max_level=int(lv.max()),
+                 launches_default=res["default"]["launches"], launches_levels=res["levels"]["launches"],
+                 ms_levels=res["levels"]["ms"], per_launch_overhead_ms=(res["levels"]["ms"] - res["default"]["ms"]) / max(extra, 1))
+            ar.close()
+            del ar
+            torch.cuda.empty_cache()
+
+
+if __name__ == "__main__":
+    main()
