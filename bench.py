@@ -230,14 +230,14 @@ def run_ours(args):
     sustained_ms = s0.elapsed_time(s1) / n_sus
     ar.check()
 
-    # ---- the same decode scheduled level by level (literal wave + one match launch per level), for comparison
-    ar.decode_all(out, levels=True)
+    # ---- the same decode with the two-launch flag schedule (completion flags instead of one launch per level), for comparison
+    ar.decode_all(out, schedule="flags")
     l0 = ar.launch_count()
     p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
     p0.record(stream)
     for _ in range(3):
-        ar.decode_all(out, levels=True)
+        ar.decode_all(out, schedule="flags")
     p1.record(stream)
     torch.cuda.synchronize()
     lv_ms = p0.elapsed_time(p1) / 3
@@ -327,7 +327,7 @@ def run_ours(args):
                        "parallelism": "replicas only" if world > 1 else "1 GPU", "resident_warps": info["resident_warps"]},
             "bit_exact": ok and fnv_bad == 0,
             "clocks": dict(sampler.summary(), sustained_ms_per_step=sustained_ms, sustained_steps=n_sus), "e2e": e2e, "gpu_launches": int(launches),
-            "roofline": roofline, "cpu_baseline": cpu, "cpu_multithreaded": cpu_mt, "range_and_reads": extra, "level_schedule": levels_info, "fused_schedule": fused_info}
+            "roofline": roofline, "cpu_baseline": cpu, "cpu_multithreaded": cpu_mt, "range_and_reads": extra, "flag_schedule": levels_info, "fused_schedule": fused_info}
     print(json.dumps(line))
     if not (ok and fnv_bad == 0):
         sys.exit(1)

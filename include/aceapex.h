@@ -82,21 +82,23 @@ int32_t aceapex_set_workspace(aceapex_archive* ar, void* d_workspace, uint64_t w
 /* cudaStream_t (as void*) all later calls are issued on; null = legacy default stream. */
 int32_t aceapex_set_stream(aceapex_archive* ar, void* cuda_stream);
 
-/* Whole-file decode (§3.3, the paper's "v4").  d_out: >= raw_bytes device bytes.  On completion of the
- * stream, d_out[0..N) are the original bytes.  Two persistent-kernel launches: (1) every block: entropy decode,
- * command scan, literal placement; (2) every block, sorted by (level, index): match resolution, a block waiting on a
- * device-side ready flag only for source blocks of a strictly lower level (FORMAT.md §3).  Errors: E_WORKSPACE, E_CUDA. */
+/* Whole-file decode (§3.3, the paper's "v4").  d_out: >= raw_bytes device bytes, 16-byte aligned.  On
+ * completion of the stream, d_out[0..N) are the original bytes.  Scheduled the way the paper describes the wavefront
+ * (PAPER.md:17, 25): (1) one launch over every block: entropy decode, command scan, literal placement; (2) one match
+ * launch per dependency level (FORMAT.md §3; max_level + 2 launches in all, max_level <= 3 with the default encoder).
+ * Inside a level nothing waits: every source is a literal byte or belongs to a lower level.  Errors: E_ARG,
+ * E_WORKSPACE, E_CUDA. */
 int32_t aceapex_decode_all(aceapex_archive* ar, void* d_out);
 
-/* Same result in ONE launch: blocks are taken in index order; each block places its literals, publishes a
+/* Same result with TWO launches: the match launch takes the blocks sorted by (level, index) and a block waits on a
+ * device-side completion flag only for source blocks of a strictly lower level (the "device-side ready counter"
+ * variant of BASELINE.json north_star (4)).  Measured slightly slower than one launch per level. */
+int32_t aceapex_decode_all_flags(aceapex_archive* ar, void* d_out);
+
+/* Same result in ONE launch: blocks are taken in (level, index) order; each block places its literals, publishes a
  * "literals placed" flag, then resolves its matches, waiting for the literal flag of same-or-higher-level source
  * blocks and for the completion flag of lower-level ones.  Kept for comparison. */
 int32_t aceapex_decode_all_fused(aceapex_archive* ar, void* d_out);
-
-/* Same result, scheduled the way the paper describes it: literal wave, then one match launch per dependency level
- * (FORMAT.md §3; max_level + 2 launches).  Exists for measurement (BASELINE.json configs[4]: wavefront depth and
- * per-launch overhead) and as a cross-check of the flag-driven schedule. */
-int32_t aceapex_decode_all_levels(aceapex_archive* ar, void* d_out);
 
 /* Arbitrary byte range [byte_lo, byte_hi) (§4, "v7-RA"): d_out[0 .. hi-lo) = those bytes; only the
  * covering blocks are decoded, sources outside the range are reconstructed on demand by recursion on their own

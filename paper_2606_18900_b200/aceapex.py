@@ -46,7 +46,7 @@ def load():
             "aceapex_set_workspace": ([p, p, u64], i32),
             "aceapex_set_stream": ([p, p], i32),
             "aceapex_decode_all": ([p, p], i32),
-            "aceapex_decode_all_levels": ([p, p], i32),
+            "aceapex_decode_all_flags": ([p, p], i32),
             "aceapex_decode_all_fused": ([p, p], i32),
             "aceapex_decode_range": ([p, u64, u64, p, u64], i32),
             "aceapex_decode_reads": ([p, p, u64, p, u64, p], i32),
@@ -136,10 +136,11 @@ class Archive:
 
     # -- the calls of include/aceapex.h
     def decode_all(self, out=None, levels=False, schedule=None):
-        """schedule: None (default two-launch schedule), "levels" (one launch per level) or "fused" (one launch)."""
+        """schedule: None / "levels" (default: literal launch + one match launch per level), "flags" (two launches,
+        completion flags) or "fused" (one launch)."""
         out = self.new_output() if out is None else out
         schedule = "levels" if levels else schedule
-        f = {None: self.L.aceapex_decode_all, "levels": self.L.aceapex_decode_all_levels,
+        f = {None: self.L.aceapex_decode_all, "levels": self.L.aceapex_decode_all, "flags": self.L.aceapex_decode_all_flags,
              "fused": self.L.aceapex_decode_all_fused}[schedule]
         _chk(f(self.h, out.data_ptr()), "decode_all")
         return out[:self.raw_bytes]

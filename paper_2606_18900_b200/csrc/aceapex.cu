@@ -1048,8 +1048,27 @@ int32_t aceapex_set_stream(aceapex_archive* ar, void* s) {
     return ACEAPEX_OK;
 }
 
+// literal launch + one match launch per dependency level (FORMAT.md §3): no waits, no flags, no fences
 int32_t aceapex_decode_all(aceapex_archive* ar, void* d_out) {
-    if (!ar || (!d_out && ar->N)) return ACEAPEX_E_ARG;
+    if (!ar || (!d_out && ar->N) || (reinterpret_cast<uintptr_t>(d_out) & 15)) return ACEAPEX_E_ARG;
+    int32_t rc = prepare_ws(ar);
+    if (rc) return rc;
+    Params P; fill_params(ar, P);
+    P.out = static_cast<uint8_t*>(d_out); P.out_pos0 = 0; P.first_block = 0;
+    P.mode = 2; P.level_list = nullptr;
+    if ((rc = launch(ar, P, ar->n_blocks))) return rc;
+    // matches never wait in this schedule: every source is a literal byte (placed by the launch above) or a match
+    // byte of a lower-level block (completed by an earlier launch) -- FORMAT.md §3
+    for (uint32_t l = 0; l <= ar->max_level && ar->d_level_lists; l++) {
+        P.mode = 3; P.level_list = ar->d_level_lists + ar->level_off[l];
+        if ((rc = launch(ar, P, ar->level_blocks[l].size()))) return rc;
+    }
+    return ACEAPEX_OK;
+}
+
+// literal launch + ONE match launch over the blocks sorted by (level, index) with completion flags
+int32_t aceapex_decode_all_flags(aceapex_archive* ar, void* d_out) {
+    if (!ar || (!d_out && ar->N) || (reinterpret_cast<uintptr_t>(d_out) & 15)) return ACEAPEX_E_ARG;
     int32_t rc = prepare_ws(ar);
     if (rc) return rc;
     Params P; fill_params(ar, P);
@@ -1069,23 +1088,6 @@ int32_t aceapex_decode_all_fused(aceapex_archive* ar, void* d_out) {
     P.mode = 0; P.out = static_cast<uint8_t*>(d_out); P.out_pos0 = 0; P.first_block = 0; P.epoch = ++ar->epoch;
     P.level_list = ar->d_level_lists;   // blocks sorted by (level, index): everything a block reads from precedes it
     return launch(ar, P, ar->n_blocks);
-}
-
-int32_t aceapex_decode_all_levels(aceapex_archive* ar, void* d_out) {
-    if (!ar || (!d_out && ar->N)) return ACEAPEX_E_ARG;
-    int32_t rc = prepare_ws(ar);
-    if (rc) return rc;
-    Params P; fill_params(ar, P);
-    P.out = static_cast<uint8_t*>(d_out); P.out_pos0 = 0; P.first_block = 0;
-    P.mode = 2; P.level_list = nullptr;
-    if ((rc = launch(ar, P, ar->n_blocks))) return rc;
-    // matches never wait in this schedule: every source is a literal byte (placed by the launch above) or a match
-    // byte of a lower-level block (completed by an earlier launch) -- FORMAT.md §3
-    for (uint32_t l = 0; l <= ar->max_level && ar->d_level_lists; l++) {
-        P.mode = 3; P.level_list = ar->d_level_lists + ar->level_off[l];
-        if ((rc = launch(ar, P, ar->level_blocks[l].size()))) return rc;
-    }
-    return ACEAPEX_OK;
 }
 
 // launches span-mode work for the demands staged in ar->h_demands (in batches of demand_cap)

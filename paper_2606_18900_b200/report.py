@@ -65,7 +65,7 @@ def whole_file(torch, ar, x, label, reps=5):
     info = ar.info()
     res = {}
     xt = torch.from_numpy(x).to(out.device) if x is not None else None
-    for sched in (None, "levels", "fused"):
+    for sched in (None, "flags", "fused"):
         out.zero_()
         ar.decode_all(out, schedule=sched)
         ar.check()
@@ -257,11 +257,11 @@ def main():
             n_blocks, dir_off = int(a[24:32].view(np.uint64)[0]), int(a[72:80].view(np.uint64)[0])   # FORMAT.md §1.1
             lv = np.frombuffer(a[dir_off:dir_off + 32 * n_blocks].tobytes(), dtype=np.uint16).reshape(-1, 16)[:, 14]   # §1.3 level
             # per-launch overhead (S19): level schedule time minus the two-launch time, per extra launch
-            extra = res["levels"]["launches"] - res["default"]["launches"]
+            extra = res["default"]["launches"] - res["flags"]["launches"]
             emit(config=4, what="block_size_point", block_size=bs, ratio=x.size / a.size, encode_seconds=enc_s,
                  GBps=res["default"]["GBps"], ms=res["default"]["ms"], mean_level=float(lv.mean()), max_level=int(lv.max()),
-                 launches_default=res["default"]["launches"], launches_levels=res["levels"]["launches"],
-                 ms_levels=res["levels"]["ms"], per_launch_overhead_ms=(res["levels"]["ms"] - res["default"]["ms"]) / max(extra, 1))
+                 launches_default=res["default"]["launches"], launches_flags=res["flags"]["launches"],
+                 ms_flags=res["flags"]["ms"], per_launch_overhead_ms=(res["default"]["ms"] - res["flags"]["ms"]) / max(extra, 1))
             ar.close()
             del ar
             torch.cuda.empty_cache()

@@ -38,7 +38,7 @@ def test_hand_built(case, levels):
     blocks, N, lb, kw = HAND[case]
     a = build(blocks, N, lb, **kw)
     exp = O.decode(a)
-    got = gpu_decode(a, levels=levels)
+    got = gpu_decode(a, schedule="flags" if levels else None)
     assert got.tobytes() == exp.tobytes()
     if not levels:
         assert gpu_decode(a, schedule="fused").tobytes() == exp.tobytes()
@@ -53,7 +53,7 @@ def test_hand_built_escapes_and_planes():
         assert gpu_decode(a).tobytes() == O.decode(a).tobytes()
 
 
-@pytest.mark.parametrize("schedule", [None, "levels", "fused"])
+@pytest.mark.parametrize("schedule", [None, "flags", "fused"])
 def test_config0_fastq(fastq_4m, fastq_4m_archive, schedule):
     got = gpu_decode(fastq_4m_archive, schedule=schedule)
     assert np.array_equal(got, O.decode(fastq_4m_archive))      # bit-exact vs the oracle
@@ -71,7 +71,7 @@ def test_block_sizes(fastq_4m, bs):
     x = fastq_4m[:(3 << 20) + 12345]            # ragged tail
     a = encoder.encode(x, block_size=bs)
     assert np.array_equal(gpu_decode(a), x)
-    assert np.array_equal(gpu_decode(a, levels=True), x)
+    assert np.array_equal(gpu_decode(a, schedule="flags"), x)
     assert np.array_equal(gpu_decode(a, schedule="fused"), x)
 
 
