@@ -227,6 +227,7 @@ static int decode_block(const hdr_t* h, const dir_t* d, const scratch_t* s, uint
         if (c < d->n_match) {
             uint64_t src = s->src[c];
             if (!(src < dst) || dst + ml > end) return E_CORRUPT;
+            if (src + ml > dst && src < b * BS) return E_CORRUPT;   /* FORMAT.md §3 (c): a self-overlapping match starts in its own block */
             if (matchmap) {
                 uint64_t seed_end = src + ml < dst ? src + ml : dst;
                 for (uint64_t q = src; q < seed_end; q++) {

@@ -255,24 +255,44 @@ __device__ __forceinline__ void wait_sources(const Params& P, const BlockCtx& c,
 
 constexpr uint32_t LONG_RUN = 64;   // runs at least this long are copied by the whole warp
 
-struct Stack { Demand* base; uint32_t cap; uint32_t top; /* shared address of the entry count */ };
+// Where source bytes that are neither in the window nor resident go: a per-warp LIFO (read access: depth-first recursion
+// by the warp itself) or the global per-source-block lists of a range decode (gl != null).  policy: see fetch_source.
+struct Stack { Demand* base; uint32_t cap; uint32_t top; /* shared address of the entry count */ const GList* gl; uint32_t policy; };
+enum : uint32_t { SKIP_KNOWN = 1, SKIP_UNKNOWN = 2 };
 
 __device__ __forceinline__ uint32_t lds_top(const Stack& st) { return lds32(st.top); }
+
+// append "original bytes [pos, pos + len) -> out2[dst ..)" (inside one block) to the list of the block that holds them
+__device__ __forceinline__ void gl_append(const Params& P, const GList& gl, uint64_t pos, uint32_t len, uint64_t dst) {
+    uint32_t idx = atomicAdd(gl.count, 1u);
+    if (idx >= gl.cap) { report(P, DF_STACK); return; }
+    const uint64_t blk = pos >> P.log2_bs;
+    uint32_t prev = atomicExch(gl.head + blk, idx);
+    gl.rec[idx].pos = pos; gl.rec[idx].dst = dst; gl.rec[idx].len = len; gl.rec[idx].next = prev;
+    if (prev == GL_NIL) {
+        uint32_t t = atomicAdd(gl.count + 1, 1u);
+        if (t < gl.touched_cap) gl.touched[t] = (uint32_t)blk; else report(P, DF_STACK);
+    }
+}
 
 __device__ __forceinline__ void push_span(const Params& P, const Stack& st, uint64_t pos, uint64_t len, uint64_t dst) {
     while (len) {                                   // a demand never crosses a block boundary
         uint64_t bend = ((pos >> P.log2_bs) + 1) << P.log2_bs;
         uint64_t n = min((unsigned long long)len, (unsigned long long)(bend - pos));
-        uint32_t idx;
-        asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(idx) : "r"(st.top) : "memory");
-        if (idx < st.cap) { st.base[idx].pos = pos; st.base[idx].dst = dst; st.base[idx].len = n; }
-        else report(P, DF_STACK);
+        if (st.gl) gl_append(P, *st.gl, pos, (uint32_t)n, dst);
+        else {
+            uint32_t idx;
+            asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(idx) : "r"(st.top) : "memory");
+            if (idx < st.cap) { st.base[idx].pos = pos; st.base[idx].dst = dst; st.base[idx].len = n; }
+            else report(P, DF_STACK);
+        }
         pos += n; dst += n; len -= n;
     }
 }
 
 // n contiguous original bytes from absolute position sp -> dptr (= out2 + dst_off).  Window bytes and resident slots
-// are copied, the rest becomes demands.  WAIT: window sources of a block being decoded in the same launch need flags.
+// are copied (unless policy SKIP_KNOWN), the rest becomes demands (unless policy SKIP_UNKNOWN).  WAIT: window sources of
+// a block being decoded in the same launch need flags.
 template <bool WAIT>
 __device__ __forceinline__ void fetch_source(const Params& P, const BlockCtx& c, const Stack& st, uint64_t sp, uint64_t n, uint64_t dst_off) {
     while (n) {
@@ -293,10 +313,12 @@ __device__ __forceinline__ void fetch_source(const Params& P, const BlockCtx& c,
             if (!from) m = min((unsigned long long)n, (unsigned long long)(next - sp));
         }
         if (from) {
-            uint8_t* d = P.out2 + dst_off;
-            uint64_t left = m; const uint8_t* f = from;
-            while (left) { uint32_t k = (uint32_t)min((unsigned long long)left, 1ull << 30); copy_bytes<true>(d, f, k, ~0ull); d += k; f += k; left -= k; }
-        } else push_span(P, st, sp, m, dst_off);
+            if (!(st.policy & SKIP_KNOWN)) {
+                uint8_t* d = P.out2 + dst_off;
+                uint64_t left = m; const uint8_t* f = from;
+                while (left) { uint32_t k = (uint32_t)min((unsigned long long)left, 1ull << 30); copy_bytes<true>(d, f, k, ~0ull); d += k; f += k; left -= k; }
+            }
+        } else if (!(st.policy & SKIP_UNKNOWN)) push_span(P, st, sp, m, dst_off);
         sp += m; dst_off += m; n -= m;
     }
 }
@@ -399,7 +421,21 @@ __device__ __forceinline__ uint4 lds128(uint32_t a) {
 }
 
 // MODE 3: no waits (one launch per level); MODE 4: completion waits for lower-level source blocks
-template <int MODE>
+// Where the bytes [src, src + n) live if one known buffer holds them all: the window, or a resident slot (range decode).
+// *end = end of that buffer.  Null when they are unknown or spread over several buffers.
+__device__ __forceinline__ const uint8_t* resolve_src(const Params& P, uint64_t src, uint64_t n, const uint8_t** end) {
+    if (src >= P.out_pos0 && src + n <= P.win_end) { *end = P.out + (P.win_end - P.out_pos0); return P.out + (src - P.out_pos0); }
+#pragma unroll
+    for (int r = 0; r < MAX_RESIDENT; r++)
+        if (src >= P.res[r].lo && src + n <= P.res[r].hi) { *end = P.res[r].ptr + (P.res[r].hi - P.res[r].lo); return P.res[r].ptr + (src - P.res[r].lo); }
+    return nullptr;
+}
+
+// WIN = false: whole file (every source is in P.out).  WIN = true: a window of a range decode: sources are looked up in
+// the window and the resident slots; source bytes that are in neither have been delivered by the demand rounds before
+// this launch and are skipped.  COLLECT = true (range decode, before the demand rounds): nothing is copied, the unknown
+// seed bytes of every match are appended to the demand lists.
+template <int MODE, bool WIN = false, bool COLLECT = false>
 __device__ __forceinline__ void emit_matches(const Params& P, const BlockCtx& c, uint32_t mtab, uint32_t stage) {
     uint32_t lit_base = 0, out_base = 0, ec = 0, em = c.n_ext_cmd;
     const uint32_t lane = lane_id();
@@ -435,17 +471,35 @@ __device__ __forceinline__ void emit_matches(const Params& P, const BlockCtx& c,
         if (ok && has_match && !good) report(P, DF_OFFSET);
         if (MODE == 4 && good && c.d.level) wait_sources<false>(P, c, dst, src, match_len);
         const bool ovl = good && src + match_len > dst;
-        const bool lng = good && !ovl && match_len >= LONG_MATCH;
-        const bool sht = good && !ovl && !lng;
+        const uint32_t seed_len = ovl ? (uint32_t)(dst - src) : match_len;     // source bytes that are not the match's own output
+        const uint8_t* sbase = P.out + (src - P.out_pos0);
+        const uint8_t* send = P.out + (P.win_end - P.out_pos0);
+        if (WIN || COLLECT) sbase = good ? resolve_src(P, src, seed_len, &send) : nullptr;
+        if (COLLECT) {                                       // unknown seed bytes -> demands; nothing else happens here
+            if (good && !sbase) {
+                Stack sk{nullptr, 0, 0, &P.gl_nxt, SKIP_KNOWN};
+                fetch_source<false>(P, c, sk, src, seed_len, dst - P.out_pos0);
+            }
+            continue;
+        }
+        const bool known = good && sbase != nullptr;
+        const bool lng = known && !ovl && match_len >= LONG_MATCH;
+        const bool sht = known && !ovl && !lng;
         // Short matches: their source bytes travel global -> shared memory with 16-byte cp.async (issued by the lane that
         // owns the match, all matches of the group at once: one exposed memory latency per group instead of one per
         // match), then the warp copies match after match from the stage to the output: lane i moves bytes i, i + 32, ...
         // A group whose sources do not fit the stage is served in several rounds.
-        const uint64_t sp = reinterpret_cast<uint64_t>(P.out) + (src - P.out_pos0);
+        const uint64_t sp = reinterpret_cast<uint64_t>(sbase);
         const uint32_t mis = (uint32_t)sp & 15u;
-        // a chunk may not reach past the end of the output buffer (only possible for sources in its last 16 bytes)
-        const bool stg = sht && ((sp - mis) + 16ull * ((mis + match_len + 15u) >> 4) <= reinterpret_cast<uint64_t>(P.out) + (P.win_end - P.out_pos0));
-        const bool direct = (sht && !stg) || ovl;
+        // a chunk may not reach past the end of the buffer (only possible for sources in its last 16 bytes)
+        const bool stg = sht && ((sp - mis) + 16ull * ((mis + match_len + 15u) >> 4) <= reinterpret_cast<uint64_t>(send));
+        const bool direct = (sht && !stg) || (known && ovl);
+        if (WIN && good && !sbase) {                         // seed spread over several buffers or (partly) delivered by demands
+            Stack sk{nullptr, 0, 0, nullptr, SKIP_UNKNOWN};
+            fetch_source<false>(P, c, sk, src, seed_len, dst - P.out_pos0);     // the known pieces of the seed
+            uint8_t* d = P.out + (dst - P.out_pos0);
+            for (uint32_t i = seed_len; i < match_len; i++) d[i] = d[i - seed_len];   // the rest repeats it (FORMAT.md §2)
+        }
         uint32_t pending = __ballot_sync(0xffffffffu, stg);
         while (pending) {
             const bool mine = (pending >> lane) & 1u;
@@ -495,19 +549,18 @@ __device__ __forceinline__ void emit_matches(const Params& P, const BlockCtx& c,
         while (longs) {
             int l = __ffs(longs) - 1; longs &= longs - 1;
             uint32_t d2 = __shfl_sync(0xffffffffu, dst_rel, l), n = __shfl_sync(0xffffffffu, match_len, l);
-            uint64_t s2 = __shfl_sync(0xffffffffu, src, l);
-            warp_copy<true>(out_blk + d2, P.out + (s2 - P.out_pos0), n);
+            uint64_t s2 = __shfl_sync(0xffffffffu, sp, l);
+            warp_copy<true>(out_blk + d2, reinterpret_cast<const uint8_t*>(s2), n);
         }
         uint32_t ovls = __ballot_sync(0xffffffffu, direct);
         while (ovls) {                                       // byte i of the match = seed[i mod period] (FORMAT.md §2)
             int l = __ffs(ovls) - 1; ovls &= ovls - 1;
             uint32_t d2 = __shfl_sync(0xffffffffu, dst_rel, l), n = __shfl_sync(0xffffffffu, match_len, l);
-            uint64_t s2 = __shfl_sync(0xffffffffu, src, l);
-            const uint32_t per = (uint32_t)(c.bstart + d2 - s2);
-            const uint8_t* sp = P.out + (s2 - P.out_pos0);
+            const uint32_t per = __shfl_sync(0xffffffffu, (uint32_t)min((unsigned long long)(dst - src), 0xffffffffull), l);
+            const uint8_t* sq = reinterpret_cast<const uint8_t*>(__shfl_sync(0xffffffffu, sp, l));
             uint32_t r = lane % per; const uint32_t stp = 32 % per;
             for (uint32_t i = lane; i < n; i += 32) {
-                out_blk[d2 + i] = __ldcg(sp + r);
+                out_blk[d2 + i] = __ldcg(sq + r);
                 r += stp; if (r >= per) r -= per;
             }
         }
@@ -637,7 +690,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_literals(const Params P) {
     const CtaSmem m = setup_cta(P, smem_raw);
     BlockCtx c;
     bind_scratch(P, blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), c);
-    Stack st{nullptr, 0, m.top};
+    Stack st{nullptr, 0, m.top, nullptr, 0};
     unsigned long long t;
     while (next_ticket(P, t)) {
         c.b = P.first_block + t;
@@ -659,7 +712,8 @@ __global__ void __launch_bounds__(MAXT, 1) k_literals(const Params P) {
 // Whole-file match launches.  WAIT = false (mode 3): one dependency level per launch, nothing to wait for.
 // WAIT = true (mode 4): all levels in one launch; blocks arrive sorted by (level, index) and a block waits for the
 // completion of lower-level source blocks, which were dispatched before it.
-template <bool WAIT, int MAXT>
+// WIN / COLLECT: the two range-decode variants (see emit_matches); they run one level per launch (WAIT = false).
+template <bool WAIT, int MAXT, bool WIN = false, bool COLLECT = false>
 __global__ void __launch_bounds__(MAXT, 1) k_matches(const Params P) {
     // shared memory: [pad to 8 KB][tables without LIT (the last one): (n_coded_tables - 1) x 8 KB]
     //                [per warp: ring 2 KB | match table MTAB_BYTES | stage 16 x STAGE_CHUNKS]
@@ -681,13 +735,43 @@ __global__ void __launch_bounds__(MAXT, 1) k_matches(const Params P) {
     unsigned long long t;
     while (next_ticket(P, t)) {
         c.b = P.level_list ? (uint64_t)P.level_list[t] : P.first_block + t;
-        if (parse_block(P, luts, ring, c, 0, false)) emit_matches<WAIT ? 4 : 3>(P, c, mtab, stage);
+        if (parse_block(P, luts, ring, c, 0, false)) emit_matches<WAIT ? 4 : 3, WIN, COLLECT>(P, c, mtab, stage);
         if (WAIT) {                                          // publish: the warp's stores happen-before lane 0's fence + release
             __syncwarp();
             if (lane_id() == 0) { __threadfence(); st_release(P.flags + c.b, 2 * P.epoch + 1); }
         }
     }
 }
+
+// One round of the demand lists of a range decode: every block with a non-empty list is parsed ONCE (tokens + all its
+// literals into the warp's scratch) and serves all its records; match pieces whose sources are unknown go to the lists
+// of the next round (recursion depth <= max_level + 1, FORMAT.md §3).
+__global__ void __launch_bounds__(1024, 1) k_serve(const Params P) {
+    extern __shared__ __align__(16) uint8_t smem_raw[];
+    const CtaSmem m = setup_cta(P, smem_raw);
+    BlockCtx c;
+    bind_scratch(P, blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), c);
+    const Stack sk{nullptr, 0, m.top, &P.gl_nxt, 0};
+    const unsigned long long n = min(__ldg(P.gl_cur.count + 1), P.gl_cur.touched_cap);
+    for (;;) {
+        unsigned long long t = 0;
+        if (lane_id() == 0) t = atomicAdd(P.ticket, 1ull);
+        t = __shfl_sync(0xffffffffu, t, 0);
+        if (t >= n) break;
+        c.b = P.gl_cur.touched[t];
+        const bool ok = parse_block(P, m.luts, m.ring, c, 0xffffffffu, false);
+        uint32_t idx = P.gl_cur.head[c.b];
+        __syncwarp();
+        if (lane_id() == 0) P.gl_cur.head[c.b] = GL_NIL;      // the list is consumed: the array is clean for the next use
+        while (idx != GL_NIL && idx < P.gl_cur.cap) {
+            const GDemand d = P.gl_cur.rec[idx];
+            if (ok) emit_span(P, c, sk, d.pos, d.len, d.dst);
+            idx = d.next;
+        }
+    }
+}
+
+__global__ void k_assert_empty(const uint32_t* count, uint32_t* err) { if (*count) atomicOr(err, (uint32_t)DF_STACK); }
 
 template <bool DEMANDS>
 __global__ void __launch_bounds__(1024, 1) k_decode(const Params P) {
@@ -698,7 +782,7 @@ __global__ void __launch_bounds__(1024, 1) k_decode(const Params P) {
     BlockCtx c;
     bind_scratch(P, gw, c);
     Stack st;
-    st.base = P.stacks + (uint64_t)gw * P.stack_cap; st.cap = P.stack_cap; st.top = m.top;
+    st.base = P.stacks + (uint64_t)gw * P.stack_cap; st.cap = P.stack_cap; st.top = m.top; st.gl = nullptr; st.policy = 0;
     if (lane_id() == 0) asm volatile("st.shared.u32 [%0], %1;" ::"r"(st.top), "r"(0u) : "memory");
     __syncwarp();
     unsigned long long t;
@@ -782,6 +866,8 @@ struct aceapex_archive {
     uint64_t scratch_per_warp = 0, ctrl_bytes = 0, flags_bytes = 0;
     uint64_t scratch_off = 0, stacks_off = 0, demands_off = 0, list_off = 0, ws_need = 0;
     uint32_t stack_cap = 0, demand_cap = 0;
+    uint64_t gl_cap = 0, gl_tcap = 0, gl_rec_off[2] = {0, 0}, gl_head_off[2] = {0, 0}, gl_touched_off[2] = {0, 0};   // range decode lists
+    std::vector<uint64_t> h_match_prefix;             // matches in blocks [0, b)
     std::vector<uint16_t> h_levels;                    // host copy of the per-block levels
     std::vector<uint32_t> h_list; std::vector<Demand> h_demands;   // host staging for range / read calls
     // status
@@ -819,7 +905,26 @@ void layout_workspace(aceapex_archive* ar) {
     ar->stacks_off = align_up(ar->scratch_off + warps * ar->scratch_per_warp, 256);
     ar->demands_off = align_up(ar->stacks_off + warps * ar->stack_cap * sizeof(Demand), 256);
     ar->list_off = align_up(ar->demands_off + (uint64_t)ar->demand_cap * sizeof(Demand), 256);
-    ar->ws_need = align_up(ar->list_off + 4 * ar->n_blocks + 4, 256);
+    uint64_t off = align_up(ar->list_off + 4 * ar->n_blocks + 4, 256);
+    // demand lists of range decode (two sets, alternating between rounds); counters live in the control area at +64
+    ar->gl_cap = std::min<uint64_t>(1ull << 24, std::max<uint64_t>(1ull << 20, ar->total_matches / 2));
+    ar->gl_tcap = std::max<uint64_t>(1, std::min<uint64_t>(ar->n_blocks, ar->gl_cap));
+    for (int k = 0; k < 2; k++) {
+        ar->gl_rec_off[k] = off; off = align_up(off + ar->gl_cap * sizeof(GDemand), 256);
+        ar->gl_head_off[k] = off; off = align_up(off + 4 * ar->n_blocks + 4, 256);
+        ar->gl_touched_off[k] = off; off = align_up(off + 4 * ar->gl_tcap, 256);
+    }
+    ar->ws_need = off;
+}
+
+GList glist(const aceapex_archive* ar, int k) {
+    GList g;
+    g.rec = reinterpret_cast<GDemand*>(ar->d_ws + ar->gl_rec_off[k]);
+    g.head = reinterpret_cast<uint32_t*>(ar->d_ws + ar->gl_head_off[k]);
+    g.touched = reinterpret_cast<uint32_t*>(ar->d_ws + ar->gl_touched_off[k]);
+    g.count = reinterpret_cast<uint32_t*>(ar->d_ws + 64 + 8 * k);
+    g.cap = (uint32_t)ar->gl_cap; g.touched_cap = (uint32_t)ar->gl_tcap;
+    return g;
 }
 
 void fill_params(const aceapex_archive* ar, Params& P) {
@@ -847,6 +952,7 @@ int32_t prepare_ws(aceapex_archive* ar) {
     if (!ar->d_ws || ar->ws_bytes < workspace_need(ar)) return ACEAPEX_E_WORKSPACE;
     if (!ar->ws_clean) {
         CU(cudaMemsetAsync(ar->d_ws, 0, ar->ctrl_bytes + ar->flags_bytes, ar->stream));
+        for (int k = 0; k < 2; k++) CU(cudaMemsetAsync(ar->d_ws + ar->gl_head_off[k], 0xff, 4 * ar->n_blocks + 4, ar->stream));   // GL_NIL
         ar->ws_clean = true; ar->epoch = 0;
     }
     return ACEAPEX_OK;
@@ -859,7 +965,15 @@ int32_t launch(aceapex_archive* ar, Params& P, uint64_t n_work) {
     uint64_t warps = ar->threads / 32;
     uint32_t grid = (uint32_t)std::min<uint64_t>(ar->grid, (n_work + warps - 1) / warps);
     const bool whole = P.out_pos0 == 0 && P.win_end == ar->N;
-    if (whole && P.mode >= 2) {                               // specialised whole-file kernels
+    if (P.mode >= 5) {                                        // range decode: collect / window matches / serve
+        const int T = ar->threads;
+        uint64_t w = T / 32;
+        uint32_t g = (uint32_t)std::min<uint64_t>(ar->sms, (n_work + w - 1) / w);
+        if (P.mode == 5) k_matches<false, 1024, true, true><<<g, T, smem_matches(ar, T), ar->stream>>>(P);
+        else if (P.mode == 6) k_matches<false, 1024, true, false><<<g, T, smem_matches(ar, T), ar->stream>>>(P);
+        else k_serve<<<ar->sms, T, ar->smem, ar->stream>>>(P);
+    }
+    else if ((whole || P.mode == 2) && P.mode >= 2) {         // specialised whole-file kernels (the literal launch also serves windows)
         const int T = P.mode == 2 ? ar->threads_lit : ar->threads_match;
         const size_t sm = P.mode == 2 ? smem_for(ar, T) : smem_matches(ar, T);
         uint64_t w = T / 32;
@@ -947,6 +1061,7 @@ int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* 
     ar->n_coded_tables = (uint32_t)(luts.size() / LUT_SIZE);
     // directory validation + level lists
     ar->level_blocks.assign(ar->max_level + 1, {});
+    ar->h_match_prefix.assign(ar->n_blocks + 1, 0);
     uint64_t prev = ar->payload_off;
     uint32_t seen_max_cmds = 0;
     for (uint64_t b = 0; b < ar->n_blocks; b++) {
@@ -959,6 +1074,7 @@ int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* 
         if (po + need > end || n_lit > (1u << ar->log2_bs)) return ACEAPEX_E_CORRUPT;
         prev = po; seen_max_cmds = std::max(seen_max_cmds, n_cmd);
         ar->level_blocks[lvl].push_back((uint32_t)b);
+        ar->h_match_prefix[b + 1] = ar->h_match_prefix[b] + n_match;
     }
     // device tables
     if (!luts.empty()) {
@@ -995,7 +1111,8 @@ int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* 
     {
         const void* fns[] = {(const void*)k_decode<false>, (const void*)k_decode<true>, (const void*)k_literals<1024>, (const void*)k_literals<768>,
                              (const void*)k_matches<false, 1024>, (const void*)k_matches<false, 768>, (const void*)k_matches<true, 1024>,
-                             (const void*)k_matches<true, 768>};
+                             (const void*)k_matches<true, 768>, (const void*)k_matches<false, 1024, true, true>,
+                             (const void*)k_matches<false, 1024, true, false>, (const void*)k_serve};
         for (const void* f : fns) {
             CU(cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max(ar->smem, smem_matches(ar, ar->threads))));
             CU(cudaFuncSetAttribute(f, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
@@ -1137,9 +1254,43 @@ int32_t aceapex_decode_range(aceapex_archive* ar, uint64_t lo, uint64_t hi, void
         for (uint64_t b = b0; b < b1; b++) L[cnt[ar->h_levels[b]]++] = (uint32_t)b;
         uint32_t* d_list = reinterpret_cast<uint32_t*>(ar->d_ws + ar->list_off);
         CU(cudaMemcpyAsync(d_list, L.data(), nb * 4, cudaMemcpyHostToDevice, ar->stream));
-        P.mode = 0; P.level_list = d_list; P.epoch = ++ar->epoch;
         P.out = out + (alo - lo); P.out2 = P.out; P.out_pos0 = alo; P.win_end = ahi;
-        if ((rc = launch(ar, P, nb))) return rc;
+        if (nb < 256 || (reinterpret_cast<uintptr_t>(P.out) & 15)) {
+            // small window (a seek): one launch, every warp reconstructs the foreign sources of its block by recursion
+            P.mode = 0; P.level_list = d_list; P.epoch = ++ar->epoch;
+            if ((rc = launch(ar, P, nb))) return rc;
+        } else {
+            // (1) literals of the window; (2) foreign seed bytes of its matches -> demand lists, served in rounds, every
+            // source block parsed once per round; (3) matches of the window, one launch per dependency level
+            P.mode = 2; P.level_list = nullptr; P.first_block = b0;
+            if ((rc = launch(ar, P, nb))) return rc;
+            const GList g[2] = {glist(ar, 0), glist(ar, 1)};
+            // a span can recurse through max_level + 1 blocks (FORMAT.md §3), and inside each of them once more when a
+            // match piece reads literal bytes of its own block
+            const uint32_t rounds = 2 * (ar->max_level + 1) + 1;
+            for (uint64_t s0 = b0; s0 < b1;) {                // sub-windows whose demands fit the lists
+                uint64_t s1 = s0 + 1;
+                while (s1 < b1 && ar->h_match_prefix[s1 + 1] - ar->h_match_prefix[s0] <= ar->gl_cap / 3) s1++;
+                CU(cudaMemsetAsync(g[0].count, 0, 16, ar->stream));
+                P.mode = 5; P.level_list = nullptr; P.first_block = s0; P.gl_nxt = g[0];
+                if ((rc = launch(ar, P, s1 - s0))) return rc;
+                Params Q = P;                                   // serving knows no window: sources of foreign bytes precede it
+                Q.mode = 7; Q.out_pos0 = 0; Q.win_end = 0;
+                for (uint32_t r = 0; r < rounds; r++) {
+                    Q.gl_cur = g[r & 1]; Q.gl_nxt = g[(r + 1) & 1];
+                    CU(cudaMemsetAsync(Q.gl_nxt.count, 0, 8, ar->stream));
+                    if ((rc = launch(ar, Q, 1))) return rc;
+                }
+                k_assert_empty<<<1, 1, 0, ar->stream>>>(g[rounds & 1].count, Q.err);
+                ar->launches++;
+                s0 = s1;
+            }
+            for (uint32_t l = 0; l <= ar->max_level; l++) {     // cnt[l] = end of level l in the sorted list
+                uint64_t l0 = l ? cnt[l - 1] : 0, l1 = cnt[l];
+                P.mode = 6; P.level_list = d_list + l0; P.first_block = 0;
+                if ((rc = launch(ar, P, l1 - l0))) return rc;
+            }
+        }
     }
     ar->h_demands.clear();
     if (alo >= ahi) add_demands(ar, lo, hi - lo, 0);

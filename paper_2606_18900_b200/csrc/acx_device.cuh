@@ -25,6 +25,17 @@ struct Resident { uint64_t lo, hi; const uint8_t* ptr; };
 // "materialise original bytes [pos, pos + len) at out2[dst ..)"; never crosses a block boundary; len == 0: served
 struct Demand { uint64_t pos; uint64_t dst; uint64_t len; };
 
+// Aggregated demands (range decode): records linked per SOURCE block, so that one parse of a block serves all of them.
+struct GDemand { uint64_t pos; uint64_t dst; uint32_t len; uint32_t next; };
+constexpr uint32_t GL_NIL = 0xffffffffu;
+struct GList {
+    GDemand* rec;            // cap records
+    uint32_t* head;          // per block: index of the first record of its list, GL_NIL when empty
+    uint32_t* touched;       // blocks with a non-empty list, in order of first touch
+    uint32_t* count;         // [0] = records appended, [1] = blocks touched
+    uint32_t cap, touched_cap;
+};
+
 struct Params {
     const uint8_t* archive;      // device archive
     uint64_t archive_bytes;
@@ -55,6 +66,7 @@ struct Params {
     uint32_t mode;                       // 0 = whole blocks with flags, 1 = spans (demands), 2 = literal launch, 3 = match wave,
                                          // 4 = all match waves with flags
     const uint32_t* level_list;          // block ids to process (n_work entries), null = first_block + i
+    GList gl_cur, gl_nxt;                // range decode: demands being served / being collected
 };
 
 __device__ __forceinline__ uint32_t lane_id() { return threadIdx.x & 31; }

@@ -94,6 +94,8 @@ struct Enc {
         while (l < maxlen && x[p + l] == x[i + l]) l++;
     done:
         if (l < o.min_match) return false;
+        if (p + l > i && p < bstart) l = i - p;                 // FORMAT.md §3 (c): a self-overlapping match starts in its own block
+        if (l < o.min_match) return false;
         uint64_t seed_end = std::min(p + l, i);
         uint32_t lvl = 0;
         uint64_t a = p;
@@ -159,7 +161,8 @@ struct Enc {
                 }
                 // extend backwards over pending literals while the source byte is a literal byte
                 uint64_t p = best.p, len = best.len;
-                while (i > lit_start && p > 0 && x[i - 1] == x[p - 1] && (p - 1 >= cs || p - 1 < batch_start) && is_lit(p - 1)) {
+                while (i > lit_start && p > 0 && x[i - 1] == x[p - 1] && (p - 1 >= cs || p - 1 < batch_start) && is_lit(p - 1) &&
+                       !(p + len > i && p - 1 < bstart)) {   // FORMAT.md §3 (c): a self-overlapping match stays in its block
                     // the new seed byte p-1 is a literal byte: allowed by FORMAT.md §3 (a); its block may raise the level
                     i--; p--; len++;
                     if (p / BS != bi) best.lvl = std::max(best.lvl, (uint32_t)level[p / BS]);

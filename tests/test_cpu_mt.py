@@ -13,7 +13,7 @@ def test_fastq_and_fasta(fastq_4m, fastq_4m_archive, fasta_2m, fasta_2m_archive,
 
 
 def test_hand_built_levels_and_overlap():
-    blocks = [[(b"a", (0, 7))], [(b"", (7, 8))], [(b"", (15, 8))], [(b"", (23, 3))]]
+    blocks = [[(b"a", (0, 7))], [(b"", (0, 8))], [(b"", (8, 8))], [(b"", (16, 3))]]
     a = build(blocks, 27, 3, min_match=3, levels=[0, 1, 2, 3])
     assert acx_mt.decode(a, threads=4).tobytes() == O.decode(a).tobytes() == b"a" * 27
     lit = bytes((i * 7 + 3) % 251 for i in range(300))

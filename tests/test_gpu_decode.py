@@ -21,7 +21,7 @@ def gpu_decode(archive, levels=False, schedule=None):
 
 HAND = [
     ([[(b"hello", None)]], 5, 3, {}),
-    ([[(b"a", (0, 7))], [(b"", (7, 8))], [(b"", (15, 8))], [(b"", (23, 3))]], 27, 3, dict(min_match=3, levels=[0, 1, 2, 3])),
+    ([[(b"a", (0, 7))], [(b"", (0, 8))], [(b"", (8, 8))], [(b"", (16, 3))]], 27, 3, dict(min_match=3, levels=[0, 1, 2, 3])),
     ([[(b"abc", (0, 10))]], 13, 4, {}),
     ([[(b"wxyz", (0, 4))]], 8, 3, {}),
     ([[(b"abcd", (0, 4))], [(b"", (2, 5)), (b"XYZ", None)]], 16, 3, dict(levels=[0, 1])),

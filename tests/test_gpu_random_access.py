@@ -143,7 +143,7 @@ def test_resident_window_serves_as_source(fq):
 
 
 HAND = [
-    ([[(b"a", (0, 7))], [(b"", (7, 8))], [(b"", (15, 8))], [(b"", (23, 3))]], 27, 3, dict(min_match=3, levels=[0, 1, 2, 3])),
+    ([[(b"a", (0, 7))], [(b"", (0, 8))], [(b"", (8, 8))], [(b"", (16, 3))]], 27, 3, dict(min_match=3, levels=[0, 1, 2, 3])),
     ([[(b"abc", (0, 10)), (b"XYZ", None)], [(b"", (1, 9)), (b"0123456", None)]], 32, 4, dict(levels=[0, 1])),
     ([[(b"01234567", None)], [(b"89ab", (6, 4))], [(b"", (6, 5)), (b"!!!", None)]], 24, 3, {}),
     ([[(b"ABCDEFGH", None)], [(b"", (0, 8))], [(b"", (8, 8))]], 24, 3, dict(levels=[0, 0, 1])),
@@ -162,4 +162,64 @@ def test_hand_built_every_range(case):
             got = ar.decode_range(lo, hi).cpu().numpy().tobytes()[:hi - lo]
             assert got == exp[lo:hi], (lo, hi)
     ar.check()
+    ar.close()
+
+
+@pytest.fixture(scope="module")
+def big(request):
+    """12 MiB FASTQ (high coverage: most matches reach far back) and 8 MiB FASTA: windows of >= 256 blocks take the
+    aggregated-demand path of decode_range (literals, demand rounds, matches per level)."""
+    from paper_2606_18900_b200 import datagen, encoder
+    from paper_2606_18900_b200.aceapex import Archive
+    xq = datagen.fastq(7, 12 << 20, 300_000)
+    xa = datagen.fasta(9, 8 << 20)
+    aq, aa = Archive(encoder.encode(xq, block_size=16384)), Archive(encoder.encode(xa, block_size=16384))
+    yield (aq, xq), (aa, xa)
+    aq.close()
+    aa.close()
+
+
+def test_large_windows_with_foreign_sources(big):
+    for ar, x in big:
+        N = x.size
+        BS = 16384
+        for lo, hi in ((150 * BS, 450 * BS), (N - 300 * BS - 5, N), (100 * BS + 77, 400 * BS + 99), (0, 256 * BS), (5, N - 5),
+                       (N // 3 - 3, N // 3 + 200 + 257 * BS)):
+            check_range(ar, x, lo, min(hi, N))
+
+
+def test_large_windows_ring(big):
+    """Consecutive 4 MiB windows through a two-slot ring: sources are found in the window, in the resident previous
+    window, or are reconstructed through the demand lists."""
+    for ar, x in big:
+        W = 256 * 16384
+        ring = [ar.new_output(W) for _ in range(2)]
+        for w in range((x.size + W - 1) // W):
+            lo, hi = w * W, min(x.size, (w + 1) * W)
+            buf = ring[w % 2]
+            ar.set_resident(w % 2, 0, 0, None)
+            got = ar.decode_range(lo, hi, out=buf)
+            ar.check()
+            assert torch.equal(got.cpu(), torch.from_numpy(x[lo:hi])), w
+            ar.set_resident(w % 2, lo, hi, buf)
+        ar.set_resident(0, 0, 0, None)
+        ar.set_resident(1, 0, 0, None)
+
+
+def test_large_window_runs_and_overlaps():
+    """RLE runs and short periods that cross block and window boundaries (self-overlapping matches whose seed lies
+    outside the window)."""
+    from paper_2606_18900_b200 import encoder
+    from paper_2606_18900_b200.aceapex import Archive
+    rng = np.random.default_rng(3)
+    parts = []
+    for k in range(120):
+        parts.append(rng.integers(65, 70, 3000 + 17 * k, dtype=np.uint8).tobytes())
+        parts.append(b"N" * (20000 + 999 * (k % 7)))
+        parts.append((b"ACGTTGCA" * 5 + b"\n") * 300)
+    x = np.frombuffer(b"".join(parts), dtype=np.uint8)
+    ar = Archive(encoder.encode(x, block_size=4096))
+    N = x.size
+    for lo, hi in ((300 * 4096, 700 * 4096), (N // 3 + 11, N // 3 + 11 + 300 * 4096), (N - 260 * 4096, N)):
+        check_range(ar, x, lo, hi)
     ar.close()

@@ -18,12 +18,22 @@ def test_literals_only_single_block():
 
 
 def test_rle_one_byte_period_across_blocks():
-    # 'a' then src = dst-1 copies: every later byte equals the previous one.  Blocks of 8 bytes, N = 27 (ragged tail).
-    blocks = [[(b"a", (0, 7))], [(b"", (7, 8))], [(b"", (15, 8))], [(b"", (23, 3))]]
+    # 'a', an in-block run (src = dst-1), then every block copies its predecessor.  Blocks of 8 bytes, N = 27 (ragged tail).
+    blocks = [[(b"a", (0, 7))], [(b"", (0, 8))], [(b"", (8, 8))], [(b"", (16, 3))]]
     # each block reads a match byte of its predecessor -> levels must increase (FORMAT.md §3)
     assert dec(blocks, 27, 3, min_match=3, levels=[0, 1, 2, 3]) == b"a" * 27
     with pytest.raises(O.OracleError):
         dec(blocks, 27, 3, min_match=3, levels=[0, 1, 1, 2])
+
+
+def test_self_overlap_needs_its_seed_in_the_own_block():
+    # FORMAT.md §3 (c): a self-overlapping match (src + len > dst) starts in its own block.  src = 7, dst = 8, len = 8
+    # would continue the run of block 0 from outside block 1: rejected.
+    with pytest.raises(O.OracleError) as e:
+        dec([[(b"a", (0, 7))], [(b"", (7, 8))]], 16, 3, min_match=3, levels=[0, 1])
+    assert e.value.name == "E_CORRUPT"
+    # the same bytes with the run restarted by a literal inside block 1 are fine
+    assert dec([[(b"a", (0, 7))], [(b"a", (8, 7))]], 16, 3, min_match=3, levels=[0, 0]) == b"a" * 16
 
 
 def test_period_three_overlap():
