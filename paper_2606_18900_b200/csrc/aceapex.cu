@@ -471,6 +471,7 @@ __device__ __forceinline__ void emit_matches(const Params& P, const BlockCtx& c,
         if (ok && has_match && !good) report(P, DF_OFFSET);
         if (MODE == 4 && good && c.d.level) wait_sources<false>(P, c, dst, src, match_len);
         const bool ovl = good && src + match_len > dst;
+        if (ovl && src < c.bstart) report(P, DF_OFFSET);     // FORMAT.md §3 (c)
         const uint32_t seed_len = ovl ? (uint32_t)(dst - src) : match_len;     // source bytes that are not the match's own output
         const uint8_t* sbase = P.out + (src - P.out_pos0);
         const uint8_t* send = P.out + (P.win_end - P.out_pos0);
@@ -608,8 +609,16 @@ __device__ __forceinline__ void emit_span(const Params& P, const BlockCtx& c, co
             a = max((unsigned long long)md, (unsigned long long)pos); b = min((unsigned long long)(md + match_len), (unsigned long long)pend);
             if (has_match && a < b) {
                 uint64_t src = match_src(P, c, ci);
+                const uint64_t period = md - src;
                 if (src >= md) report(P, DF_OFFSET);
-                else fetch_match_piece<false>(P, c, st, md, src, match_len, (uint32_t)(a - md), (uint32_t)(b - a), dst + (a - pos));
+                else if (period >= match_len) fetch_source<false>(P, c, st, src + (a - md), b - a, dst + (a - pos));
+                else if (period > lit_len) report(P, DF_OFFSET);      // FORMAT.md §3 (c): the seed is the tail of this literal run
+                else {                                                // byte i of the match = seed[i mod period]
+                    const uint8_t* seed = c.lit + lit_pos + lit_len - period;
+                    uint8_t* d = P.out2 + dst + (a - pos);
+                    uint32_t r = (uint32_t)((a - md) % period);
+                    for (uint32_t k = 0; k < (uint32_t)(b - a); k++) { d[k] = seed[r]; if (++r == period) r = 0; }
+                }
             }
         }
         if (c.bstart + out_base >= pend) break;              // uniform: nothing after this group is wanted
@@ -1265,9 +1274,9 @@ int32_t aceapex_decode_range(aceapex_archive* ar, uint64_t lo, uint64_t hi, void
             P.mode = 2; P.level_list = nullptr; P.first_block = b0;
             if ((rc = launch(ar, P, nb))) return rc;
             const GList g[2] = {glist(ar, 0), glist(ar, 1)};
-            // a span can recurse through max_level + 1 blocks (FORMAT.md §3), and inside each of them once more when a
-            // match piece reads literal bytes of its own block
-            const uint32_t rounds = 2 * (ar->max_level + 1) + 1;
+            // a seed byte is found after at most max_level + 1 source blocks (FORMAT.md §3): one round each, the list
+            // left by the last round must be empty
+            const uint32_t rounds = ar->max_level + 2;
             for (uint64_t s0 = b0; s0 < b1;) {                // sub-windows whose demands fit the lists
                 uint64_t s1 = s0 + 1;
                 while (s1 < b1 && ar->h_match_prefix[s1 + 1] - ar->h_match_prefix[s0] <= ar->gl_cap / 3) s1++;
