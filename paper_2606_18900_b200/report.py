@@ -195,6 +195,7 @@ def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--config", type=int, required=True)
     ap.add_argument("--size", type=int, default=0)
+    ap.add_argument("--src-window", type=int, default=0, help="encoder option: sources at most this far back (0 = unlimited)")
     args = ap.parse_args()
     import torch
     from paper_2606_18900_b200 import datagen, encoder
@@ -234,8 +235,8 @@ def main():
         x = datagen.fasta(4, size)
         emit(config=3, what="generate", seconds=time.time() - t, bytes=size)
         t = time.time()
-        a = encoder.encode(x, block_size=16384)
-        emit(config=3, what="encode", seconds=time.time() - t, MBps=x.size / (time.time() - t) / 1e6, archive_bytes=int(a.size))
+        a = encoder.encode(x, block_size=16384, src_window=args.src_window)
+        emit(config=3, what="encode", src_window=args.src_window, seconds=time.time() - t, MBps=x.size / (time.time() - t) / 1e6, archive_bytes=int(a.size))
         ar = Archive(a)
         info = ar.info()
         emit(config=3, what="archive", raw_bytes=info["raw_bytes"], archive_bytes=info["archive_bytes"], n_blocks=info["n_blocks"],
