@@ -877,6 +877,10 @@ struct aceapex_archive {
     uint32_t stack_cap = 0, demand_cap = 0;
     uint64_t gl_cap = 0, gl_tcap = 0, gl_rec_off[2] = {0, 0}, gl_head_off[2] = {0, 0}, gl_touched_off[2] = {0, 0};   // range decode lists
     std::vector<uint64_t> h_match_prefix;             // matches in blocks [0, b)
+    // end-to-end pipeline (aceapex_decode_all_host): chunks of blocks, per chunk the block ids sorted by level
+    uint64_t chunk_blocks = 0; uint32_t* d_chunk_lists = nullptr; std::vector<uint64_t> chunk_level_off;   // (chunk, level) -> offset
+    std::vector<uint64_t> h_payload_off;               // payload offset of block b (n_blocks + 1 entries)
+    cudaStream_t s_h2d = nullptr, s_d2h = nullptr; std::vector<cudaEvent_t> ev_h2d, ev_dec;
     std::vector<uint16_t> h_levels;                    // host copy of the per-block levels
     std::vector<uint32_t> h_list; std::vector<Demand> h_demands;   // host staging for range / read calls
     // status
@@ -1071,6 +1075,7 @@ int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* 
     // directory validation + level lists
     ar->level_blocks.assign(ar->max_level + 1, {});
     ar->h_match_prefix.assign(ar->n_blocks + 1, 0);
+    ar->h_payload_off.assign(ar->n_blocks + 1, abytes);
     uint64_t prev = ar->payload_off;
     uint32_t seen_max_cmds = 0;
     for (uint64_t b = 0; b < ar->n_blocks; b++) {
@@ -1084,6 +1089,7 @@ int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* 
         prev = po; seen_max_cmds = std::max(seen_max_cmds, n_cmd);
         ar->level_blocks[lvl].push_back((uint32_t)b);
         ar->h_match_prefix[b + 1] = ar->h_match_prefix[b] + n_match;
+        ar->h_payload_off[b] = po;
     }
     // device tables
     if (!luts.empty()) {
@@ -1147,6 +1153,11 @@ int32_t aceapex_close(aceapex_archive* ar) {
     if (ar->d_luts) cudaFree(ar->d_luts);
     if (ar->d_level_lists) cudaFree(ar->d_level_lists);
     if (ar->d_levels) cudaFree(ar->d_levels);
+    if (ar->d_chunk_lists) cudaFree(ar->d_chunk_lists);
+    for (cudaEvent_t e : ar->ev_h2d) cudaEventDestroy(e);
+    for (cudaEvent_t e : ar->ev_dec) cudaEventDestroy(e);
+    if (ar->s_h2d) cudaStreamDestroy(ar->s_h2d);
+    if (ar->s_d2h) cudaStreamDestroy(ar->s_d2h);
     delete ar;
     return ACEAPEX_OK;
 }
@@ -1377,12 +1388,72 @@ int32_t aceapex_verify_fnv(aceapex_archive* ar, const void* d_data, uint64_t lo,
     return ACEAPEX_OK;
 }
 
+// End to end with host buffers, pipelined over chunks of blocks: the payload of chunk k+1 travels host -> device while
+// chunk k decodes and the output of chunk k-1 travels device -> host (a chunk only reads output bytes of lower positions,
+// and inside a chunk the levels are launched in order, FORMAT.md §3).
 int32_t aceapex_decode_all_host(aceapex_archive* ar, const void* h_archive, void* d_stage, void* h_out) {
-    if (!ar || !h_archive || (!d_stage && ar->N) || (!h_out && ar->N)) return ACEAPEX_E_ARG;
-    CU(cudaMemcpyAsync(const_cast<uint8_t*>(ar->d_archive), h_archive, ar->archive_bytes, cudaMemcpyHostToDevice, ar->stream));
-    int32_t rc = aceapex_decode_all(ar, d_stage);
+    if (!ar || !h_archive || (!d_stage && ar->N) || (!h_out && ar->N) || (reinterpret_cast<uintptr_t>(d_stage) & 15)) return ACEAPEX_E_ARG;
+    int32_t rc = prepare_ws(ar);
     if (rc) return rc;
-    if (ar->N) CU(cudaMemcpyAsync(h_out, d_stage, ar->N, cudaMemcpyDeviceToHost, ar->stream));
+    const uint8_t* h_a = static_cast<const uint8_t*>(h_archive);
+    uint8_t* d_a = const_cast<uint8_t*>(ar->d_archive);
+    if (ar->n_blocks == 0) {
+        CU(cudaMemcpyAsync(d_a, h_a, ar->archive_bytes, cudaMemcpyHostToDevice, ar->stream));
+        CU(cudaStreamSynchronize(ar->stream));
+        return ACEAPEX_OK;
+    }
+    const uint32_t n_lv = ar->max_level + 1;
+    if (!ar->s_h2d) {                                      // first use: streams, events, per-chunk level lists
+        CU(cudaStreamCreateWithFlags(&ar->s_h2d, cudaStreamNonBlocking));
+        CU(cudaStreamCreateWithFlags(&ar->s_d2h, cudaStreamNonBlocking));
+        ar->chunk_blocks = std::max<uint64_t>(256, (ar->n_blocks + 15) / 16);
+        const uint64_t n_chunks = (ar->n_blocks + ar->chunk_blocks - 1) / ar->chunk_blocks;
+        std::vector<uint32_t> list(ar->n_blocks);
+        ar->chunk_level_off.assign(n_chunks * n_lv + 1, 0);
+        uint64_t at = 0;
+        for (uint64_t k = 0; k < n_chunks; k++) {
+            const uint64_t b0 = k * ar->chunk_blocks, b1 = std::min(ar->n_blocks, b0 + ar->chunk_blocks);
+            for (uint32_t l = 0; l < n_lv; l++) {
+                ar->chunk_level_off[k * n_lv + l] = at;
+                for (uint64_t b = b0; b < b1; b++) if (ar->h_levels[b] == l) list[at++] = (uint32_t)b;
+            }
+        }
+        ar->chunk_level_off[n_chunks * n_lv] = at;
+        CU(cudaMalloc(&ar->d_chunk_lists, list.size() * 4));
+        CU(cudaMemcpy(ar->d_chunk_lists, list.data(), list.size() * 4, cudaMemcpyHostToDevice));
+        ar->ev_h2d.resize(n_chunks); ar->ev_dec.resize(n_chunks);
+        for (uint64_t k = 0; k < n_chunks; k++) {
+            CU(cudaEventCreateWithFlags(&ar->ev_h2d[k], cudaEventDisableTiming));
+            CU(cudaEventCreateWithFlags(&ar->ev_dec[k], cudaEventDisableTiming));
+        }
+    }
+    const uint64_t n_chunks = ar->ev_h2d.size();
+    // everything queued on the handle's stream so far must be done before the archive bytes are replaced
+    CU(cudaEventRecord(ar->ev_dec[0], ar->stream));
+    CU(cudaStreamWaitEvent(ar->s_h2d, ar->ev_dec[0], 0));
+    CU(cudaStreamWaitEvent(ar->s_d2h, ar->ev_dec[0], 0));
+    CU(cudaMemcpyAsync(d_a, h_a, ar->payload_off, cudaMemcpyHostToDevice, ar->s_h2d));     // header, tables, directory, fnv
+    Params P; fill_params(ar, P);
+    P.out = static_cast<uint8_t*>(d_stage); P.out_pos0 = 0;
+    for (uint64_t k = 0; k < n_chunks; k++) {
+        const uint64_t b0 = k * ar->chunk_blocks, b1 = std::min(ar->n_blocks, b0 + ar->chunk_blocks);
+        const uint64_t p0 = ar->h_payload_off[b0], p1 = b1 < ar->n_blocks ? ar->h_payload_off[b1] : ar->archive_bytes;
+        CU(cudaMemcpyAsync(d_a + p0, h_a + p0, p1 - p0, cudaMemcpyHostToDevice, ar->s_h2d));
+        CU(cudaEventRecord(ar->ev_h2d[k], ar->s_h2d));
+        CU(cudaStreamWaitEvent(ar->stream, ar->ev_h2d[k], 0));
+        P.mode = 2; P.level_list = nullptr; P.first_block = b0;
+        if ((rc = launch(ar, P, b1 - b0))) return rc;
+        for (uint32_t l = 0; l < n_lv; l++) {
+            const uint64_t l0 = ar->chunk_level_off[k * n_lv + l], l1 = ar->chunk_level_off[k * n_lv + l + 1];
+            P.mode = 3; P.level_list = ar->d_chunk_lists + l0; P.first_block = 0;
+            if ((rc = launch(ar, P, l1 - l0))) return rc;
+        }
+        CU(cudaEventRecord(ar->ev_dec[k], ar->stream));
+        CU(cudaStreamWaitEvent(ar->s_d2h, ar->ev_dec[k], 0));
+        const uint64_t o0 = b0 << ar->log2_bs, o1 = std::min(ar->N, b1 << ar->log2_bs);
+        CU(cudaMemcpyAsync(static_cast<uint8_t*>(h_out) + o0, static_cast<uint8_t*>(d_stage) + o0, o1 - o0, cudaMemcpyDeviceToHost, ar->s_d2h));
+    }
+    CU(cudaStreamSynchronize(ar->s_d2h));
     CU(cudaStreamSynchronize(ar->stream));
     return ACEAPEX_OK;
 }

@@ -162,7 +162,8 @@ struct Enc {
                 // extend backwards over pending literals while the source byte is a literal byte
                 uint64_t p = best.p, len = best.len;
                 while (i > lit_start && p > 0 && x[i - 1] == x[p - 1] && (p - 1 >= cs || p - 1 < batch_start) && is_lit(p - 1) &&
-                       !(p + len > i && p - 1 < bstart)) {   // FORMAT.md §3 (c): a self-overlapping match stays in its block
+                       !(len + 1 > i - p && p - 1 < bstart)) {   // FORMAT.md §3 (c): the extended match (len + 1, same period) would
+                    // overlap itself with its source starting outside the block
                     // the new seed byte p-1 is a literal byte: allowed by FORMAT.md §3 (a); its block may raise the level
                     i--; p--; len++;
                     if (p / BS != bi) best.lvl = std::max(best.lvl, (uint32_t)level[p / BS]);

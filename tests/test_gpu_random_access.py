@@ -223,3 +223,18 @@ def test_large_window_runs_and_overlaps():
     for lo, hi in ((300 * 4096, 700 * 4096), (N // 3 + 11, N // 3 + 11 + 300 * 4096), (N - 260 * 4096, N)):
         check_range(ar, x, lo, hi)
     ar.close()
+
+
+def test_end_to_end_host_pipeline(big, fq):
+    """aceapex_decode_all_host: archive from pinned host memory, output to pinned host memory, chunks pipelined."""
+    for ar, x in (big[0], big[1], fq):
+        import torch as T
+        h_arch = ar.d_archive.cpu().pin_memory()
+        ar.d_archive.zero_()                                  # the call must bring every archive byte itself
+        stage = ar.new_output()
+        h_out = T.empty(x.size, dtype=T.uint8).pin_memory()
+        for _ in range(2):
+            h_out.zero_()
+            ar.decode_all_host(h_arch, stage, h_out)
+            ar.check()
+            assert T.equal(h_out, T.from_numpy(x))

@@ -106,3 +106,20 @@ def test_stage_view_is_consistent_with_decode(fastq_4m, fastq_4m_archive):
                     out[dst + i] = out[s + i]
                 dst += ml
         assert bytes(out[b * BS:dst]) == fastq_4m[b * BS:dst].tobytes()
+
+
+def test_periodic_data_small_blocks_keep_overlaps_in_their_block():
+    """FORMAT.md §3 (c) under stress: mutated periodic data, periods around the block size.  The oracle rejects any
+    self-overlapping match whose source starts outside its block, so a clean decode is the check.  (Seeds 8, 12, 29, 39,
+    53 of this recipe caught an encoder that extended a match cut to exactly one period backwards into an overlap.)"""
+    from paper_2606_18900_b200 import encoder
+    for seed in range(120):
+        rng = np.random.default_rng(seed)
+        period, alpha, n = int(rng.integers(3, 40)), int(rng.integers(2, 5)), int(rng.integers(1500, 5000))
+        pat = rng.integers(65, 65 + alpha, period, dtype=np.uint8)
+        x = np.tile(pat, n // period + 1)[:n].copy()
+        m = rng.random(n) < rng.uniform(0.002, 0.03)
+        x[m] = rng.integers(65, 65 + alpha + 1, int(m.sum()), dtype=np.uint8)
+        bs = int(rng.choice([32, 64, 128, 256, 1024]))
+        a = encoder.encode(x, block_size=bs, chunk_log2=11, batch_chunks=2)
+        assert np.array_equal(O.decode(a), x), (seed, bs)
