@@ -83,16 +83,15 @@ int32_t aceapex_set_workspace(aceapex_archive* ar, void* d_workspace, uint64_t w
 int32_t aceapex_set_stream(aceapex_archive* ar, void* cuda_stream);
 
 /* Whole-file decode (§3.3, the paper's "v4").  d_out: >= raw_bytes device bytes, 16-byte aligned.  On
- * completion of the stream, d_out[0..N) are the original bytes.  Scheduled the way the paper describes the wavefront
- * (PAPER.md:17, 25): (1) one launch over every block: entropy decode, command scan, literal placement; (2) one match
- * launch per dependency level (FORMAT.md §3; max_level + 2 launches in all, max_level <= 3 with the default encoder).
- * Inside a level nothing waits: every source is a literal byte or belongs to a lower level.  Errors: E_ARG,
- * E_WORKSPACE, E_CUDA. */
+ * completion of the stream, d_out[0..N) are the original bytes.  Scheduled as the wavefront of PAPER.md:17, 25 over the
+ * dependency levels of FORMAT.md §3, in at most three launches: (1) every block: entropy decode, command scan, literal
+ * placement; (2) the blocks below the top level, sorted by (level, index), a block waiting on a device-side completion
+ * flag only for source blocks of a strictly lower level; (3) the blocks of the top level (the bulk: 97 % on FASTQ),
+ * where nothing waits: every source is a literal byte or belongs to a lower level.  Errors: E_ARG, E_WORKSPACE, E_CUDA. */
 int32_t aceapex_decode_all(aceapex_archive* ar, void* d_out);
 
-/* Same result with TWO launches: the match launch takes the blocks sorted by (level, index) and a block waits on a
- * device-side completion flag only for source blocks of a strictly lower level (the "device-side ready counter"
- * variant of BASELINE.json north_star (4)).  Measured slightly slower than one launch per level. */
+/* Same result with TWO launches: one match launch takes ALL blocks sorted by (level, index) with completion flags (the
+ * "device-side ready counter" variant of BASELINE.json north_star (4)).  Measured slightly slower. */
 int32_t aceapex_decode_all_flags(aceapex_archive* ar, void* d_out);
 
 /* Same result in ONE launch: blocks are taken in (level, index) order; each block places its literals, publishes a
