@@ -262,15 +262,14 @@ enum : uint32_t { SKIP_KNOWN = 1, SKIP_UNKNOWN = 2 };
 
 __device__ __forceinline__ uint32_t lds_top(const Stack& st) { return lds32(st.top); }
 
-// append "original bytes [pos, pos + len) -> out2[dst ..)" (inside one block) to the list of the block that holds them
+// append "original bytes [pos, pos + len) -> out2[dst ..)" (inside one block)
 __device__ __forceinline__ void gl_append(const Params& P, const GList& gl, uint64_t pos, uint32_t len, uint64_t dst) {
-    uint32_t idx = atomicAdd(gl.count, 1u);
+    const uint32_t idx = atomicAdd(gl.count, 1u);
     if (idx >= gl.cap) { report(P, DF_STACK); return; }
+    gl.rec[idx].pos = pos; gl.rec[idx].dst = dst; gl.rec[idx].len = len;
     const uint64_t blk = pos >> P.log2_bs;
-    uint32_t prev = atomicExch(gl.head + blk, idx);
-    gl.rec[idx].pos = pos; gl.rec[idx].dst = dst; gl.rec[idx].len = len; gl.rec[idx].next = prev;
-    if (prev == GL_NIL) {
-        uint32_t t = atomicAdd(gl.count + 1, 1u);
+    if (atomicAdd(gl.cnt + blk, 1u) == 0) {
+        const uint32_t t = atomicAdd(gl.count + 1, 1u);
         if (t < gl.touched_cap) gl.touched[t] = (uint32_t)blk; else report(P, DF_STACK);
     }
 }
@@ -755,27 +754,84 @@ __global__ void __launch_bounds__(MAXT, 1) k_matches(const Params P) {
 // One round of the demand lists of a range decode: every block with a non-empty list is parsed ONCE (tokens + all its
 // literals into the warp's scratch) and serves all its records; match pieces whose sources are unknown go to the lists
 // of the next round (recursion depth <= max_level + 1, FORMAT.md §3).
+// Bucket offsets and work items of the list in P.gl_cur: one CTA scans the touched blocks (their record counts and their
+// numbers of work items) 1024 at a time; cnt[block] becomes the fill pointer of the block's bucket.
+__global__ void __launch_bounds__(1024, 1) k_plan(const Params P) {
+    __shared__ uint32_t s_rec[32], s_item[32], s_base[2];
+    const GList& g = P.gl_cur;
+    const uint32_t n = min(g.count[1], g.touched_cap), lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) { s_base[0] = 0; s_base[1] = 0; }
+    __syncthreads();
+    for (uint32_t t0 = 0; t0 < n; t0 += 1024) {
+        const uint32_t t = t0 + threadIdx.x;
+        uint32_t blk = 0, c = 0;
+        if (t < n) { blk = g.touched[t]; c = g.cnt[blk]; }
+        uint32_t it = (c + GL_ITEM - 1) / GL_ITEM, ps = c, pi = it;      // inclusive warp scans of records and items
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t a = __shfl_up_sync(0xffffffffu, ps, o), b2 = __shfl_up_sync(0xffffffffu, pi, o);
+            if (lane >= (uint32_t)o) { ps += a; pi += b2; }
+        }
+        if (lane == 31) { s_rec[warp] = ps; s_item[warp] = pi; }
+        __syncthreads();
+        if (warp == 0) {
+            uint32_t a = s_rec[lane], b2 = s_item[lane], sa = a, sb = b2;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                uint32_t x = __shfl_up_sync(0xffffffffu, sa, o), y = __shfl_up_sync(0xffffffffu, sb, o);
+                if (lane >= (uint32_t)o) { sa += x; sb += y; }
+            }
+            s_rec[lane] = sa - a; s_item[lane] = sb - b2;                 // exclusive offsets of the warps
+        }
+        __syncthreads();
+        const uint32_t r0 = s_base[0] + s_rec[warp] + ps - c, i0 = s_base[1] + s_item[warp] + pi - it;
+        if (t < n) {
+            g.cnt[blk] = r0;
+            for (uint32_t j = 0; j < it; j++) if (i0 + j < g.work_cap) {
+                g.work[i0 + j] = (unsigned long long)blk << 32 | (r0 + j * GL_ITEM);
+                g.work_n[i0 + j] = min(GL_ITEM, c - j * GL_ITEM);
+            }
+        }
+        __syncthreads();
+        if (threadIdx.x == 1023) { s_base[0] = r0 + c; s_base[1] = i0 + it; }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) g.count[2] = min(s_base[1], g.work_cap);
+}
+
+__global__ void __launch_bounds__(256) k_scatter(const Params P) {
+    const GList& g = P.gl_cur;
+    const uint32_t n = min(g.count[0], g.cap);
+    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const GDemand d = g.rec[i];
+        const uint32_t p = atomicAdd(g.cnt + (d.pos >> P.log2_bs), 1u);
+        if (p < g.cap) g.sorted[p] = d;
+    }
+}
+
+// One round of the demand lists of a range decode: a work item = up to GL_ITEM records of one source block; the block is
+// parsed once (tokens + all its literals into the warp's scratch) and serves them; match pieces whose sources are
+// unknown go to the lists of the next round (recursion depth <= max_level + 1, FORMAT.md §3).
 __global__ void __launch_bounds__(1024, 1) k_serve(const Params P) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
     const CtaSmem m = setup_cta(P, smem_raw);
     BlockCtx c;
     bind_scratch(P, blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), c);
     const Stack sk{nullptr, 0, m.top, &P.gl_nxt, 0};
-    const unsigned long long n = min(__ldg(P.gl_cur.count + 1), P.gl_cur.touched_cap);
+    const unsigned long long n = min(__ldg(P.gl_cur.count + 2), P.gl_cur.work_cap);
     for (;;) {
         unsigned long long t = 0;
         if (lane_id() == 0) t = atomicAdd(P.ticket, 1ull);
         t = __shfl_sync(0xffffffffu, t, 0);
         if (t >= n) break;
-        c.b = P.gl_cur.touched[t];
+        const unsigned long long item = P.gl_cur.work[t];
+        const uint32_t first = (uint32_t)item, cnt = P.gl_cur.work_n[t];
+        c.b = item >> 32;
+        if (lane_id() == 0) P.gl_cur.cnt[c.b] = 0;            // every item of the block writes the same value: the array is idle again
         const bool ok = parse_block(P, m.luts, m.ring, c, 0xffffffffu, false);
-        uint32_t idx = P.gl_cur.head[c.b];
-        __syncwarp();
-        if (lane_id() == 0) P.gl_cur.head[c.b] = GL_NIL;      // the list is consumed: the array is clean for the next use
-        while (idx != GL_NIL && idx < P.gl_cur.cap) {
-            const GDemand d = P.gl_cur.rec[idx];
+        for (uint32_t k = 0; k < cnt && first + k < P.gl_cur.cap; k++) {
+            const GDemand d = P.gl_cur.sorted[first + k];
             if (ok) emit_span(P, c, sk, d.pos, d.len, d.dst);
-            idx = d.next;
         }
     }
 }
@@ -875,7 +931,8 @@ struct aceapex_archive {
     uint64_t scratch_per_warp = 0, ctrl_bytes = 0, flags_bytes = 0;
     uint64_t scratch_off = 0, stacks_off = 0, demands_off = 0, list_off = 0, ws_need = 0;
     uint32_t stack_cap = 0, demand_cap = 0;
-    uint64_t gl_cap = 0, gl_tcap = 0, gl_rec_off[2] = {0, 0}, gl_head_off[2] = {0, 0}, gl_touched_off[2] = {0, 0};   // range decode lists
+    uint64_t gl_cap = 0, gl_tcap = 0, gl_wcap = 0, gl_rec_off[2] = {0, 0}, gl_cnt_off[2] = {0, 0}, gl_touched_off[2] = {0, 0};   // range decode lists
+    uint64_t gl_sorted_off = 0, gl_work_off = 0, gl_workn_off = 0;
     std::vector<uint64_t> h_match_prefix;             // matches in blocks [0, b)
     // end-to-end pipeline (aceapex_decode_all_host): chunks of blocks, per chunk the block ids sorted by level
     uint64_t chunk_blocks = 0; uint32_t* d_chunk_lists = nullptr; std::vector<uint64_t> chunk_level_off;   // (chunk, level) -> offset
@@ -922,21 +979,28 @@ void layout_workspace(aceapex_archive* ar) {
     // demand lists of range decode (two sets, alternating between rounds); counters live in the control area at +64
     ar->gl_cap = std::min<uint64_t>(1ull << 24, std::max<uint64_t>(1ull << 20, ar->total_matches / 2));
     ar->gl_tcap = std::max<uint64_t>(1, std::min<uint64_t>(ar->n_blocks, ar->gl_cap));
+    ar->gl_wcap = ar->gl_tcap + ar->gl_cap / GL_ITEM + 1;
     for (int k = 0; k < 2; k++) {
         ar->gl_rec_off[k] = off; off = align_up(off + ar->gl_cap * sizeof(GDemand), 256);
-        ar->gl_head_off[k] = off; off = align_up(off + 4 * ar->n_blocks + 4, 256);
+        ar->gl_cnt_off[k] = off; off = align_up(off + 4 * ar->n_blocks + 4, 256);
         ar->gl_touched_off[k] = off; off = align_up(off + 4 * ar->gl_tcap, 256);
     }
+    ar->gl_sorted_off = off; off = align_up(off + ar->gl_cap * sizeof(GDemand), 256);
+    ar->gl_work_off = off; off = align_up(off + 8 * ar->gl_wcap, 256);
+    ar->gl_workn_off = off; off = align_up(off + 4 * ar->gl_wcap, 256);
     ar->ws_need = off;
 }
 
 GList glist(const aceapex_archive* ar, int k) {
     GList g;
     g.rec = reinterpret_cast<GDemand*>(ar->d_ws + ar->gl_rec_off[k]);
-    g.head = reinterpret_cast<uint32_t*>(ar->d_ws + ar->gl_head_off[k]);
+    g.sorted = reinterpret_cast<GDemand*>(ar->d_ws + ar->gl_sorted_off);
+    g.cnt = reinterpret_cast<uint32_t*>(ar->d_ws + ar->gl_cnt_off[k]);
     g.touched = reinterpret_cast<uint32_t*>(ar->d_ws + ar->gl_touched_off[k]);
-    g.count = reinterpret_cast<uint32_t*>(ar->d_ws + 64 + 8 * k);
-    g.cap = (uint32_t)ar->gl_cap; g.touched_cap = (uint32_t)ar->gl_tcap;
+    g.work = reinterpret_cast<unsigned long long*>(ar->d_ws + ar->gl_work_off);
+    g.work_n = reinterpret_cast<uint32_t*>(ar->d_ws + ar->gl_workn_off);
+    g.count = reinterpret_cast<uint32_t*>(ar->d_ws + 64 + 16 * k);
+    g.cap = (uint32_t)ar->gl_cap; g.touched_cap = (uint32_t)ar->gl_tcap; g.work_cap = (uint32_t)ar->gl_wcap;
     return g;
 }
 
@@ -965,7 +1029,7 @@ int32_t prepare_ws(aceapex_archive* ar) {
     if (!ar->d_ws || ar->ws_bytes < workspace_need(ar)) return ACEAPEX_E_WORKSPACE;
     if (!ar->ws_clean) {
         CU(cudaMemsetAsync(ar->d_ws, 0, ar->ctrl_bytes + ar->flags_bytes, ar->stream));
-        for (int k = 0; k < 2; k++) CU(cudaMemsetAsync(ar->d_ws + ar->gl_head_off[k], 0xff, 4 * ar->n_blocks + 4, ar->stream));   // GL_NIL
+        for (int k = 0; k < 2; k++) CU(cudaMemsetAsync(ar->d_ws + ar->gl_cnt_off[k], 0, 4 * ar->n_blocks + 4, ar->stream));
         ar->ws_clean = true; ar->epoch = 0;
     }
     return ACEAPEX_OK;
@@ -1297,14 +1361,17 @@ int32_t aceapex_decode_range(aceapex_archive* ar, uint64_t lo, uint64_t hi, void
             for (uint64_t s0 = b0; s0 < b1;) {                // sub-windows whose demands fit the lists
                 uint64_t s1 = s0 + 1;
                 while (s1 < b1 && ar->h_match_prefix[s1 + 1] - ar->h_match_prefix[s0] <= ar->gl_cap / 3) s1++;
-                CU(cudaMemsetAsync(g[0].count, 0, 16, ar->stream));
+                CU(cudaMemsetAsync(g[0].count, 0, 32, ar->stream));
                 P.mode = 5; P.level_list = nullptr; P.first_block = s0; P.gl_nxt = g[0];
                 if ((rc = launch(ar, P, s1 - s0))) return rc;
                 Params Q = P;                                   // serving knows no window: sources of foreign bytes precede it
                 Q.mode = 7; Q.out_pos0 = 0; Q.win_end = 0;
                 for (uint32_t r = 0; r < rounds; r++) {
                     Q.gl_cur = g[r & 1]; Q.gl_nxt = g[(r + 1) & 1];
-                    CU(cudaMemsetAsync(Q.gl_nxt.count, 0, 8, ar->stream));
+                    CU(cudaMemsetAsync(Q.gl_nxt.count, 0, 16, ar->stream));
+                    k_plan<<<1, 1024, 0, ar->stream>>>(Q);       // bucket offsets + work items
+                    k_scatter<<<4 * ar->sms, 256, 0, ar->stream>>>(Q);
+                    ar->launches += 2;
                     if ((rc = launch(ar, Q, 1))) return rc;
                 }
                 k_assert_empty<<<1, 1, 0, ar->stream>>>(g[rounds & 1].count, Q.err);

@@ -25,15 +25,20 @@ struct Resident { uint64_t lo, hi; const uint8_t* ptr; };
 // "materialise original bytes [pos, pos + len) at out2[dst ..)"; never crosses a block boundary; len == 0: served
 struct Demand { uint64_t pos; uint64_t dst; uint64_t len; };
 
-// Aggregated demands (range decode): records linked per SOURCE block, so that one parse of a block serves all of them.
-struct GDemand { uint64_t pos; uint64_t dst; uint32_t len; uint32_t next; };
-constexpr uint32_t GL_NIL = 0xffffffffu;
+// Aggregated demands (range decode).  Records are appended unsorted while a per-block counter counts them; before they
+// are served they are bucketed by SOURCE block (k_plan + k_scatter), so one parse of a block serves its whole bucket and a
+// hot block (thousands of records) is cut into work items of GL_ITEM records that different warps take.
+struct GDemand { uint64_t pos; uint64_t dst; uint32_t len; uint32_t pad; };
+constexpr uint32_t GL_ITEM = 32;
 struct GList {
-    GDemand* rec;            // cap records
-    uint32_t* head;          // per block: index of the first record of its list, GL_NIL when empty
-    uint32_t* touched;       // blocks with a non-empty list, in order of first touch
-    uint32_t* count;         // [0] = records appended, [1] = blocks touched
-    uint32_t cap, touched_cap;
+    GDemand* rec;            // cap records, in order of arrival
+    GDemand* sorted;         // the same records bucketed by block (written by k_scatter)
+    uint32_t* cnt;           // per block: records appended; after k_plan: fill pointer of the block's bucket; 0 when idle
+    uint32_t* touched;       // blocks with at least one record, in order of first touch
+    unsigned long long* work;// work items written by k_plan: block << 32 | first record, then the record count in work_n
+    uint32_t* work_n;
+    uint32_t* count;         // [0] = records appended, [1] = blocks touched, [2] = work items
+    uint32_t cap, touched_cap, work_cap;
 };
 
 struct Params {
