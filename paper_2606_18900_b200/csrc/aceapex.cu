@@ -836,6 +836,12 @@ __global__ void __launch_bounds__(1024, 1) k_serve(const Params P) {
     }
 }
 
+// top-level spans of a range decode (its ragged ends) enter the demand lists like any other record
+__global__ void k_seed(const Params P, uint32_t n) {
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) gl_append(P, P.gl_nxt, P.demands[i].pos, (uint32_t)P.demands[i].len, P.demands[i].dst);
+}
+
 __global__ void k_assert_empty(const uint32_t* count, uint32_t* err) { if (*count) atomicOr(err, (uint32_t)DF_STACK); }
 
 template <bool DEMANDS>
@@ -977,7 +983,7 @@ void layout_workspace(aceapex_archive* ar) {
     ar->list_off = align_up(ar->demands_off + (uint64_t)ar->demand_cap * sizeof(Demand), 256);
     uint64_t off = align_up(ar->list_off + 4 * ar->n_blocks + 4, 256);
     // demand lists of range decode (two sets, alternating between rounds); counters live in the control area at +64
-    ar->gl_cap = std::min<uint64_t>(1ull << 24, std::max<uint64_t>(1ull << 20, ar->total_matches / 2));
+    ar->gl_cap = std::min<uint64_t>(1ull << 24, std::max<uint64_t>(1ull << 16, ar->total_matches / 2));
     ar->gl_tcap = std::max<uint64_t>(1, std::min<uint64_t>(ar->n_blocks, ar->gl_cap));
     ar->gl_wcap = ar->gl_tcap + ar->gl_cap / GL_ITEM + 1;
     for (int k = 0; k < 2; k++) {
@@ -1319,6 +1325,24 @@ static void add_demands(aceapex_archive* ar, uint64_t pos, uint64_t len, uint64_
     }
 }
 
+// Serves the demand list g[0] (filled by the caller) in `rounds` rounds; the list left by the last round must be empty.
+static int32_t serve_rounds(aceapex_archive* ar, Params Q, const GList g[2], uint32_t rounds) {
+    Q.mode = 7;
+    for (uint32_t r = 0; r < rounds; r++) {
+        Q.gl_cur = g[r & 1]; Q.gl_nxt = g[(r + 1) & 1];
+        CU(cudaMemsetAsync(Q.gl_nxt.count, 0, 16, ar->stream));
+        k_plan<<<1, 1024, 0, ar->stream>>>(Q);               // bucket offsets + work items
+        k_scatter<<<4 * ar->sms, 256, 0, ar->stream>>>(Q);
+        ar->launches += 2;
+        int32_t rc = launch(ar, Q, 1);
+        if (rc) return rc;
+    }
+    k_assert_empty<<<1, 1, 0, ar->stream>>>(g[rounds & 1].count, Q.err);
+    CU(cudaGetLastError());
+    ar->launches++;
+    return ACEAPEX_OK;
+}
+
 int32_t aceapex_decode_range(aceapex_archive* ar, uint64_t lo, uint64_t hi, void* d_out, uint64_t budget) {
     if (!ar) return ACEAPEX_E_ARG;
     if (lo > hi || hi > ar->N) return ACEAPEX_E_RANGE;
@@ -1345,8 +1369,8 @@ int32_t aceapex_decode_range(aceapex_archive* ar, uint64_t lo, uint64_t hi, void
         uint32_t* d_list = reinterpret_cast<uint32_t*>(ar->d_ws + ar->list_off);
         CU(cudaMemcpyAsync(d_list, L.data(), nb * 4, cudaMemcpyHostToDevice, ar->stream));
         P.out = out + (alo - lo); P.out2 = P.out; P.out_pos0 = alo; P.win_end = ahi;
-        if (nb < 256 || (reinterpret_cast<uintptr_t>(P.out) & 15)) {
-            // small window (a seek): one launch, every warp reconstructs the foreign sources of its block by recursion
+        if (reinterpret_cast<uintptr_t>(P.out) & 15) {
+            // window not 16-byte aligned in d_out: one launch, every warp reconstructs the foreign sources of its block by recursion
             P.mode = 0; P.level_list = d_list; P.epoch = ++ar->epoch;
             if ((rc = launch(ar, P, nb))) return rc;
         } else {
@@ -1355,9 +1379,6 @@ int32_t aceapex_decode_range(aceapex_archive* ar, uint64_t lo, uint64_t hi, void
             P.mode = 2; P.level_list = nullptr; P.first_block = b0;
             if ((rc = launch(ar, P, nb))) return rc;
             const GList g[2] = {glist(ar, 0), glist(ar, 1)};
-            // a seed byte is found after at most max_level + 1 source blocks (FORMAT.md §3): one round each, the list
-            // left by the last round must be empty
-            const uint32_t rounds = ar->max_level + 2;
             for (uint64_t s0 = b0; s0 < b1;) {                // sub-windows whose demands fit the lists
                 uint64_t s1 = s0 + 1;
                 while (s1 < b1 && ar->h_match_prefix[s1 + 1] - ar->h_match_prefix[s0] <= ar->gl_cap / 3) s1++;
@@ -1365,17 +1386,9 @@ int32_t aceapex_decode_range(aceapex_archive* ar, uint64_t lo, uint64_t hi, void
                 P.mode = 5; P.level_list = nullptr; P.first_block = s0; P.gl_nxt = g[0];
                 if ((rc = launch(ar, P, s1 - s0))) return rc;
                 Params Q = P;                                   // serving knows no window: sources of foreign bytes precede it
-                Q.mode = 7; Q.out_pos0 = 0; Q.win_end = 0;
-                for (uint32_t r = 0; r < rounds; r++) {
-                    Q.gl_cur = g[r & 1]; Q.gl_nxt = g[(r + 1) & 1];
-                    CU(cudaMemsetAsync(Q.gl_nxt.count, 0, 16, ar->stream));
-                    k_plan<<<1, 1024, 0, ar->stream>>>(Q);       // bucket offsets + work items
-                    k_scatter<<<4 * ar->sms, 256, 0, ar->stream>>>(Q);
-                    ar->launches += 2;
-                    if ((rc = launch(ar, Q, 1))) return rc;
-                }
-                k_assert_empty<<<1, 1, 0, ar->stream>>>(g[rounds & 1].count, Q.err);
-                ar->launches++;
+                Q.out_pos0 = 0; Q.win_end = 0;
+                // a seed byte is found after at most max_level + 1 source blocks (FORMAT.md §3): one round each
+                if ((rc = serve_rounds(ar, Q, g, ar->max_level + 2))) return rc;
                 s0 = s1;
             }
             for (uint32_t l = 0; l <= ar->max_level; l++) {     // cnt[l] = end of level l in the sorted list
@@ -1385,6 +1398,7 @@ int32_t aceapex_decode_range(aceapex_archive* ar, uint64_t lo, uint64_t hi, void
             }
         }
     }
+    // the ragged ends: spans that enter the demand lists as top-level records; the finished window is a plain source
     ar->h_demands.clear();
     if (alo >= ahi) add_demands(ar, lo, hi - lo, 0);
     else {
@@ -1392,10 +1406,18 @@ int32_t aceapex_decode_range(aceapex_archive* ar, uint64_t lo, uint64_t hi, void
         if (ahi < hi) add_demands(ar, ahi, hi - ahi, ahi - lo);
     }
     if (!ar->h_demands.empty()) {
-        P.out2 = out;          // demand destinations are offsets into d_out; the decoded window is readable as a source
-        CU(cudaStreamSynchronize(ar->stream));   // h_list / earlier staging must be consumed before reuse (small ranges only)
-        if ((rc = run_demands(ar, P))) return rc;
-        CU(cudaStreamSynchronize(ar->stream));   // h_demands is host staging
+        const GList g[2] = {glist(ar, 0), glist(ar, 1)};
+        Demand* d_dem = reinterpret_cast<Demand*>(ar->d_ws + ar->demands_off);
+        const uint32_t n = (uint32_t)ar->h_demands.size();      // at most a handful: two spans cut at block boundaries
+        CU(cudaMemcpyAsync(d_dem, ar->h_demands.data(), n * sizeof(Demand), cudaMemcpyHostToDevice, ar->stream));
+        CU(cudaMemsetAsync(g[0].count, 0, 32, ar->stream));
+        Params Q = P;
+        if (alo >= ahi) { Q.out_pos0 = 0; Q.win_end = 0; }
+        Q.out2 = out; Q.demands = d_dem; Q.gl_nxt = g[0];
+        k_seed<<<(n + 127) / 128, 128, 0, ar->stream>>>(Q, n);
+        CU(cudaGetLastError());
+        ar->launches++;
+        if ((rc = serve_rounds(ar, Q, g, ar->max_level + 3))) return rc;   // one more round: the span's own block comes first
     }
     return ACEAPEX_OK;
 }

@@ -145,6 +145,35 @@ def isolated_windows(torch, ar, x, label, window):
     emit(config=label, what="isolated_windows", window_bytes=window, windows=res)
 
 
+def seeks(torch, ar, x, label, n=300, seed=11):
+    """PAPER.md:81-91 Table 3: latency of decoding 1 block and 100 consecutive blocks at random positions (host wall clock
+    around decode_range + synchronize, nothing resident)."""
+    info = ar.info()
+    BS, nb = info["block_size"], info["n_blocks"]
+    rng = np.random.default_rng(seed)
+    res = {}
+    for blocks in (1, 100):
+        if nb <= blocks:
+            continue
+        buf = ar.new_output(blocks * BS)
+        lat, ok = [], True
+        for k in range(n + 10):
+            b = int(rng.integers(0, nb - blocks))
+            lo, hi = b * BS, min(info["raw_bytes"], (b + blocks) * BS)
+            t = time.perf_counter()
+            ar.decode_range(lo, hi, out=buf)
+            torch.cuda.synchronize()
+            if k >= 10:
+                lat.append((time.perf_counter() - t) * 1e3)
+            if k < 10:
+                ok = ok and buf[:hi - lo].cpu().numpy().tobytes() == x[lo:hi].tobytes()
+        ar.check()
+        lat = np.array(lat)
+        res["%d_blocks" % blocks] = {"ms_median": float(np.median(lat)), "ms_p99": float(np.percentile(lat, 99)), "ms_min": float(lat.min()),
+                                     "bytes": blocks * BS, "bit_exact": ok}
+    emit(config=label, what="seek_latency", n=n, seeks=res)
+
+
 def reads(torch, ar, x, idx, label, n_single=1000, n_batches=20, batch=4096, seed=5):
     stream = torch.cuda.current_stream()
     rng = np.random.default_rng(seed)
@@ -214,6 +243,7 @@ def main():
         windows(torch, ar, x, args.config, win, 2)
         isolated_windows(torch, ar, x, args.config, win)
         reads(torch, ar, x, datagen.fastq_index(size), args.config)
+        seeks(torch, ar, x, args.config)
         ar.close()
     elif args.config == 2:
         size = args.size or 3_100_000_000
@@ -228,6 +258,7 @@ def main():
         idx = datagen.region_index(3, size, 1_000_000, 150)
         reads(torch, ar, x, idx, 2, n_single=2000, n_batches=1_000_000 // 4096)
         isolated_windows(torch, ar, x, 2, 1 << 28)
+        seeks(torch, ar, x, 2)
         ar.close()
     elif args.config == 3:
         size = args.size or (50 << 30)
