@@ -139,6 +139,21 @@ def range_and_reads(torch, ar, x, stream):
             "bit_exact": ok}
 
 
+def max_over_ranks(dist, value, device):
+    """Replicas only: the job time is the slowest rank's time.  dist = None: single process."""
+    if dist is None:
+        return float(value)
+    import torch
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(world, bytes_per_rank, ms_per_step):
+    """Whole-job throughput in GB/s: every rank decodes its own copy, the step time is the maximum over ranks."""
+    return world * bytes_per_rank / (ms_per_step * 1e-3) / 1e9
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -207,12 +222,9 @@ def run_ours(args):
     ar.check()
     ok = bool(torch.equal(out[:x.size].cpu(), torch.from_numpy(x)))
     fnv_bad = ar.verify_fnv(out) if info["has_fnv"] else 0
-    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms = float(t.item())
+    total_ms = max_over_ranks(dist, total_ms, "cuda")
     ms = total_ms / args.steps
-    value = world * x.size / (ms * 1e-3) / 1e9
+    value = aggregate_value(world, x.size, ms)
     # clocks under the same load: the timed region is a few ms, too short for nvidia-smi, so the identical step is
     # repeated for ~1.5 s while the sampler runs; the sustained rate of that loop is reported beside the clocks
     sampler = ClockSampler(local)
@@ -269,10 +281,7 @@ def run_ours(args):
         ar.decode_all_host(h_arch, out, h_out)
     torch.cuda.synchronize()
     e2e_s = (time.perf_counter() - t0) / n_e2e
-    t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_s = float(t.item())
+    e2e_s = max_over_ranks(dist, e2e_s, "cuda")
     ok = ok and bool(torch.equal(h_out, torch.from_numpy(x)))
     e2e = {"value": world * x.size / e2e_s / 1e9, "unit": "GB/s", "h2d_bytes_per_step": int(a.size), "d2h_bytes_per_step": int(x.size)}
 
