@@ -277,6 +277,22 @@ def main():
         windows(torch, ar, x, 3, window, 8, reps=1, sample_check={0, nwin // 2, nwin - 1})
         isolated_windows(torch, ar, x, 3, window)
         ar.close()
+    elif args.config == 5:
+        # the entropy stage alone on the workload shape of PAPER.md:135 (DietGPU: 256 MB of
+        # exponentially distributed bytes, 4096 x 64 KB).  Random bytes have no matches, so decode_all = rANS literal decode.
+        size = args.size or (256 << 20)
+        rng = np.random.default_rng(6)
+        x = np.minimum(rng.exponential(scale=12.0, size=size), 255).astype(np.uint8)
+        for bs in (65536, 16384):
+            a = encoder.encode(x, block_size=bs)
+            ar = Archive(a)
+            info = ar.info()
+            res = whole_file(torch, ar, x, "5/bs=%d" % bs, reps=10)
+            emit(config=5, what="rans_microbench", block_size=bs, n_blocks=info["n_blocks"], ratio=x.size / a.size,
+                 literal_fraction=info["total_lit_bytes"] / max(info["raw_bytes"], 1), GBps=res["default"]["GBps"],
+                 compressed_GBps=res["default"]["GBps"] * a.size / x.size,
+                 context="DietGPU on H100: decode 592.5 GB/s (PAPER.md:135); not on this box")
+            ar.close()
     elif args.config == 4:
         size = args.size or (1 << 30)
         x = datagen.fastq(2, size, 50_000_000)
