@@ -116,6 +116,44 @@ __device__ __forceinline__ bool parse_block(const Params& P, uint32_t s_luts, ui
     return true;
 }
 
+// Number of literal bytes of the parsed block that lie in front of output position `pend` (counting the whole literal
+// run of a command that starts before pend): the LIT stream has to be decoded only that far to serve spans ending at pend.
+__device__ __forceinline__ uint32_t literals_before(const Params& P, const BlockCtx& c, uint64_t pend) {
+    uint32_t out_base = 0, ec = 0, em = c.n_ext_cmd, lits = 0;
+    const uint32_t lane = lane_id();
+    for (uint32_t c0 = 0; c0 < c.d.n_cmd && c.bstart + out_base < pend; c0 += 32) {
+        uint32_t ci = c0 + lane;
+        bool valid = ci < c.d.n_cmd, has_match = ci < c.d.n_match;
+        uint32_t tl = valid ? c.tok_cmd[ci] : 0, tm = has_match ? c.tok_mlen[ci] : 0;
+        uint32_t ml = __ballot_sync(0xffffffffu, valid && tl == 255), mm = __ballot_sync(0xffffffffu, has_match && tm == 255);
+        uint32_t lit_len = tl, match_len = has_match ? P.min_match + tm : 0;
+        if (valid && tl == 255) lit_len = 255 + __ldg(c.ext + ec + __popc(ml & lanemask_lt()));
+        if (has_match && tm == 255) match_len = P.min_match + 255 + __ldg(c.ext + em + __popc(mm & lanemask_lt()));
+        ec += __popc(ml); em += __popc(mm);
+        uint32_t st = lit_len + match_len;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { uint32_t t = __shfl_up_sync(0xffffffffu, st, o); if (lane >= (uint32_t)o) st += t; }
+        const uint64_t out_pos = c.bstart + out_base + (st - lit_len - match_len);
+        uint32_t mine = (valid && out_pos < pend) ? lit_len : 0;
+#pragma unroll
+        for (int o = 16; o >= 1; o >>= 1) mine += __shfl_xor_sync(0xffffffffu, mine, o);
+        lits += mine;
+        out_base += __shfl_sync(0xffffffffu, st, 31);
+    }
+    return min(lits, c.d.n_lit);
+}
+
+// A1 for span service: tokens, then only the literals in front of `pend` (all of them when pend is past the block)
+__device__ __forceinline__ bool parse_block_upto(const Params& P, uint32_t s_luts, uint32_t ring, BlockCtx& c, uint64_t pend) {
+    Rans r; uint32_t i0;
+    if (!parse_tokens(P, s_luts, ring, c, r, &i0)) return false;
+    const uint32_t nl = pend >= c.bend ? c.d.n_lit : literals_before(P, c, pend);
+    rans_region<false>(r, s_luts + P.lut_lit * (4 * LUT_SIZE), i0, nl, c.lit);
+    if (nl == c.d.n_lit && !rans_final_ok(P, c, r)) return false;
+    __syncwarp();
+    return true;
+}
+
 // ---- A2 + A3 fused into the literal decode ("direct placement") --------------------------------------------------
 // The command scan runs BEFORE the literal stream is decoded and leaves, in shared memory, one entry per non-empty
 // literal run: (last literal index of the run) | (out_start - lit_start) << 16.  The literal decode then stores every
@@ -637,7 +675,15 @@ __device__ __forceinline__ void process_demands(const Params& P, uint32_t s_luts
         if (top == 0) return;
         c.b = st.base[top - 1].pos >> P.log2_bs;
         if (c.b >= (P.N + (1ull << P.log2_bs) - 1) >> P.log2_bs) { if (lane == 0) { report(P, DF_OFFSET); st.base[top - 1].len = 0; } continue; }
-        bool ok = parse_block(P, s_luts, ring, c, 0xffffffffu);   // tokens + all literals into the scratch
+        uint64_t pend = 0;                                   // the literals are needed up to the last pending span of this block
+        for (uint32_t i0 = 0; i0 < top; i0 += 32) {
+            const uint32_t idx = i0 + lane;
+            if (idx < top && st.base[idx].len != 0 && (st.base[idx].pos >> P.log2_bs) == c.b)
+                pend = max((unsigned long long)pend, (unsigned long long)(st.base[idx].pos + st.base[idx].len));
+        }
+#pragma unroll
+        for (int o = 16; o >= 1; o >>= 1) pend = max((unsigned long long)pend, (unsigned long long)__shfl_xor_sync(0xffffffffu, pend, o));
+        bool ok = parse_block_upto(P, s_luts, ring, c, pend);     // tokens + the literals in front of it into the scratch
         bool found = true;
         while (found) {                                      // emit_span may push more demands for this same block
             found = false;
@@ -828,7 +874,11 @@ __global__ void __launch_bounds__(1024, 1) k_serve(const Params P) {
         const uint32_t first = (uint32_t)item, cnt = P.gl_cur.work_n[t];
         c.b = item >> 32;
         if (lane_id() == 0) P.gl_cur.cnt[c.b] = 0;            // every item of the block writes the same value: the array is idle again
-        const bool ok = parse_block(P, m.luts, m.ring, c, 0xffffffffu, false);
+        uint64_t pend = 0;                                    // the literals are needed up to the last span of the item
+        if (lane_id() < cnt && first + lane_id() < P.gl_cur.cap) { const GDemand d = P.gl_cur.sorted[first + lane_id()]; pend = d.pos + d.len; }
+#pragma unroll
+        for (int o = 16; o >= 1; o >>= 1) pend = max((unsigned long long)pend, (unsigned long long)__shfl_xor_sync(0xffffffffu, pend, o));
+        const bool ok = parse_block_upto(P, m.luts, m.ring, c, pend);
         for (uint32_t k = 0; k < cnt && first + k < P.gl_cur.cap; k++) {
             const GDemand d = P.gl_cur.sorted[first + k];
             if (ok) emit_span(P, c, sk, d.pos, d.len, d.dst);
