@@ -24,6 +24,8 @@ struct BlockCtx {
     uint32_t n_ext_cmd;             // number of CMD escapes (they come first in EXT)
     // per-warp scratch
     uint8_t *tok_cmd, *tok_mlen, *off_planes, *lit;
+    uint8_t* off_scratch;           // the warp's own buffer for the coded offset planes
+    uint32_t plane_stride;          // bytes between two coded planes at off_planes
 };
 
 __device__ __forceinline__ void report(const Params& P, uint32_t bit) { atomicOr(P.err, bit); }
@@ -35,15 +37,23 @@ __device__ __forceinline__ void bind_scratch(const Params& P, uint32_t warp_glob
     c.lit = s; s += (1ull << P.log2_bs) + 32;
     c.tok_cmd = s; s += mc;
     c.tok_mlen = s; s += mc;
-    c.off_planes = s;
+    c.off_planes = s; c.off_scratch = s; c.plane_stride = (uint32_t)mc;
 }
 
 // offset of match j assembled from coded planes (scratch, decode order = high plane first) and raw planes (payload)
 __device__ __forceinline__ uint64_t match_src(const Params& P, const BlockCtx& c, uint32_t j) {
+    const uint32_t mc = c.plane_stride;
+    const uint8_t* cp = c.off_planes + j;
+    const uint8_t* rp = c.raw_planes + j;
+    if (P.W <= 4) {                                          // files up to 4 GiB: 32-bit arithmetic
+        uint32_t src = 0;
+        for (uint32_t k = 0; k < P.n_coded_planes; k++, cp += mc) src |= (uint32_t)*cp << P.coded_shift[k];
+        for (uint32_t r = 0; r < P.n_raw_planes; r++, rp += c.d.n_match) src |= (uint32_t)__ldg(rp) << P.raw_shift[r];
+        return src;
+    }
     uint64_t src = 0;
-    const uint32_t mc = (P.max_cmds + 15u) & ~15u;
-    for (uint32_t k = 0; k < P.n_coded_planes; k++) src |= (uint64_t)c.off_planes[k * mc + j] << P.coded_shift[k];
-    for (uint32_t r = 0; r < P.n_raw_planes; r++) src |= (uint64_t)__ldg(c.raw_planes + (uint64_t)r * c.d.n_match + j) << P.raw_shift[r];
+    for (uint32_t k = 0; k < P.n_coded_planes; k++, cp += mc) src |= (uint64_t)*cp << P.coded_shift[k];
+    for (uint32_t r = 0; r < P.n_raw_planes; r++, rp += c.d.n_match) src |= (uint64_t)__ldg(rp) << P.raw_shift[r];
     return src;
 }
 
@@ -79,6 +89,11 @@ __device__ __forceinline__ bool parse_tokens(const Params& P, uint32_t s_luts, u
     c.ext = reinterpret_cast<const uint32_t*>(c.payload + ((rans_bytes + 3) & ~3ull));
     c.raw_planes = reinterpret_cast<const uint8_t*>(c.ext + c.d.n_ext);
     uint64_t mc = (P.max_cmds + 15u) & ~15u;
+    c.off_planes = c.off_scratch; c.plane_stride = (uint32_t)mc;
+    if (P.cplanes) {                                     // whole-file decode: the coded planes are decoded straight into k_copy's input
+        c.off_planes = P.cplanes + (uint64_t)P.n_coded_planes * __ldg(P.match_prefix + c.b);
+        c.plane_stride = c.d.n_match; mc = c.d.n_match;
+    }
     if (c.d.n_cmd > P.max_cmds || c.d.n_match > c.d.n_cmd || c.d.n_lit > (1u << P.log2_bs)) { if (lane_id() == 0) report(P, DF_LENGTH); return false; }
     r.init(c.payload, c.d.n_words, P.archive + P.archive_bytes, ring);
     uint32_t i0 = 0;
@@ -164,6 +179,7 @@ constexpr uint32_t RUNS_CAP = 512;     // entries per warp (2 KB); blocks with m
 // returns the number of runs, or 0xffffffff when the block does not fit the table / fails validation
 __device__ __forceinline__ uint32_t build_runs(const Params& P, const BlockCtx& c, uint32_t runs /* shared address */) {
     uint32_t lit_base = 0, out_base = 0, ec = 0, em = c.n_ext_cmd, n_runs = 0;
+    uint2* const pairs = P.pairs ? P.pairs + __ldg(P.match_prefix + c.b) : nullptr;   // whole-file decode: matches for k_copy
     const uint32_t lane = lane_id();
     bool fits = true;
     for (uint32_t c0 = 0; c0 < c.d.n_cmd; c0 += 32) {
@@ -184,6 +200,7 @@ __device__ __forceinline__ uint32_t build_runs(const Params& P, const BlockCtx& 
         uint32_t lit_pos = lit_base + sl - lit_len, out_rel = out_base + (st - lit_len - match_len);
         lit_base += __shfl_sync(0xffffffffu, sl, 31);
         out_base += __shfl_sync(0xffffffffu, st, 31);
+        if (pairs && has_match) pairs[ci] = make_uint2(out_rel + lit_len, match_len);
         uint32_t ne = __ballot_sync(0xffffffffu, valid && lit_len > 0);
         uint32_t k = n_runs + __popc(ne & lanemask_lt());
         if (valid && lit_len > 0 && k < RUNS_CAP) {
@@ -750,7 +767,8 @@ __global__ void __launch_bounds__(MAXT, 1) k_literals(const Params P) {
         c.b = P.first_block + t;
         Rans r; uint32_t i0;
         if (!parse_tokens(P, m.luts, m.ring, c, r, &i0)) continue;
-        uint32_t n_runs = P.log2_bs <= 16 ? build_runs(P, c, m.runs) : 0xffffffffu;
+        uint32_t n_runs = build_runs(P, c, m.runs);           // also leaves the match descriptors for k_copy
+        if (P.log2_bs > 16) n_runs = 0xffffffffu;
         if (n_runs != 0xffffffffu) {                          // scan first, literals straight to their positions
             decode_lit_direct(r, m.luts + P.lut_lit * (4 * LUT_SIZE), i0, c.d.n_lit, m.runs, P.out + (c.bstart - P.out_pos0));
             rans_final_ok(P, c, r);
@@ -800,6 +818,158 @@ __global__ void __launch_bounds__(MAXT, 1) k_matches(const Params P) {
 // One round of the demand lists of a range decode: every block with a non-empty list is parsed ONCE (tokens + all its
 // literals into the warp's scratch) and serves all its records; match pieces whose sources are unknown go to the lists
 // of the next round (recursion depth <= max_level + 1, FORMAT.md §3).
+// Whole-file match resolution from the descriptors k_literals left (A4).  No entropy decode, no scan: per block the
+// warp walks its descriptors 32 at a time.  The sources of the short non-overlapping matches of a group travel
+// global -> shared memory with 16-byte cp.async issued by the lanes that own them; the stage is double-buffered, so the
+// sources of round r + 1 are in flight while the warp copies round r to the output (lane i moves bytes i, i + 32, ...).
+// Matches of LONG_MATCH bytes and more use the 16-byte warp copy, self-overlapping ones replicate src + (i mod period).
+// WAIT = true: blocks arrive sorted by (level, index) and wait for the completion of lower-level source blocks.
+constexpr uint32_t COPY_WARP_BYTES = 2 * (MTAB_BYTES + 16 * STAGE_CHUNKS);
+static_assert(COPY_WARP_BYTES % 16 == 0, "tables and stages are 16-byte aligned");
+
+template <bool WAIT>
+__global__ void __launch_bounds__(1024, 1) k_copy(const Params P) {
+    extern __shared__ __align__(16) uint8_t smem_raw[];
+    const uint32_t lane = lane_id(), warp = threadIdx.x >> 5;
+    const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(smem_raw) + warp * COPY_WARP_BYTES;
+    const uint8_t* const out_end = P.out + (P.win_end - P.out_pos0);
+    unsigned long long t;
+    while (next_ticket(P, t)) {
+        const uint64_t b = P.level_list ? (uint64_t)P.level_list[t] : P.first_block + t;
+        const uint64_t mp0 = __ldg(P.match_prefix + b);
+        const uint4* d4 = reinterpret_cast<const uint4*>(P.dir + b);
+        const uint4 da = __ldg(d4), dq = __ldg(d4 + 1);       // FORMAT.md §1.3: payload_off, n_cmd, n_match | n_lit, n_words, n_ext, level
+        const uint32_t n = da.w;
+        const uint8_t* const raw = P.archive + ((uint64_t)da.y << 32 | da.x) + ((256 + 2ull * dq.y + 3) & ~3ull) + 4ull * dq.z;
+        const uint8_t* const cpl = P.cplanes + (uint64_t)P.n_coded_planes * mp0;
+        const uint2* const prs = P.pairs + mp0;
+        const uint64_t bstart = b << P.log2_bs;
+        const uint32_t blen = (uint32_t)(min((unsigned long long)(bstart + (1ull << P.log2_bs)), (unsigned long long)P.N) - bstart);
+        const uint32_t lvl = WAIT ? __ldg(P.levels + b) : 0;
+        uint8_t* const out_blk = P.out + (bstart - P.out_pos0);
+        uint32_t g0 = 0, pending = 0, mis = 0, len = 0, dst_rel = 0;
+        uint64_t sp = 0;
+        bool done = n == 0;
+        // (dst_rel, len) from k_literals, the offset from its decoded coded planes and the raw planes of the payload
+        auto load_desc = [&](uint32_t j) -> uint4 {
+            if (j >= n) return make_uint4(0, 0, 0, 0);
+            const uint2 pr = __ldcg(prs + j);
+            uint64_t src = 0;
+            for (uint32_t k = 0; k < P.n_coded_planes; k++) src |= (uint64_t)__ldcg(cpl + (uint64_t)k * n + j) << P.coded_shift[k];
+            for (uint32_t r = 0; r < P.n_raw_planes; r++) src |= (uint64_t)__ldg(raw + (uint64_t)r * n + j) << P.raw_shift[r];
+            return make_uint4((uint32_t)src, (uint32_t)(src >> 32), pr.x, pr.y);
+        };
+        uint4 nd = load_desc(lane);                           // descriptors are loaded one group ahead
+        // one staging round into buffer `buf`: returns the number of staged matches; commits exactly one cp.async group
+        auto issue = [&](uint32_t buf) -> uint32_t {
+            const uint32_t mtab = sbase + buf * (MTAB_BYTES + 16 * STAGE_CHUNKS), stage = mtab + MTAB_BYTES;
+            for (;;) {
+                if (pending == 0) {
+                    if (g0 >= n) { done = true; cp_async_commit(); return 0; }
+                    const uint4 d = nd;
+                    const bool has = g0 + lane < n;
+                    g0 += 32;
+                    nd = load_desc(g0 + lane);
+                    const uint64_t src = (uint64_t)d.y << 32 | d.x, dst = bstart + d.z;
+                    dst_rel = d.z; len = d.w;
+                    const bool good = has && src < dst && d.z + d.w <= blen && d.w != 0;
+                    if (has && !good) report(P, src < dst ? DF_LENGTH : DF_OFFSET);
+                    const bool ovl = good && src + len > dst;
+                    if (ovl && src < bstart) report(P, DF_OFFSET);       // FORMAT.md §3 (c)
+                    if (WAIT && good && lvl) {                            // completion of lower-level source blocks
+                        const uint64_t s1 = (min((unsigned long long)(src + len), (unsigned long long)dst) - 1) >> P.log2_bs;
+                        for (uint64_t S = src >> P.log2_bs; S <= s1; S++) if (S != b && __ldg(P.levels + S) < lvl) wait_block(P, S, true);
+                    }
+                    sp = reinterpret_cast<uint64_t>(P.out) + (src - P.out_pos0);
+                    mis = (uint32_t)sp & 15u;
+                    const bool lng = good && !ovl && len >= LONG_MATCH;
+                    const bool sht = good && !ovl && !lng;
+                    // a chunk may not reach past the end of the output buffer (only possible for sources in its last 16 bytes)
+                    const bool stg = sht && ((sp - mis) + 16ull * ((mis + len + 15u) >> 4) <= reinterpret_cast<uint64_t>(out_end));
+                    uint32_t longs = __ballot_sync(0xffffffffu, lng);
+                    while (longs) {
+                        const int l = __ffs(longs) - 1; longs &= longs - 1;
+                        const uint32_t d2 = __shfl_sync(0xffffffffu, dst_rel, l), m = __shfl_sync(0xffffffffu, len, l);
+                        warp_copy<true>(out_blk + d2, reinterpret_cast<const uint8_t*>(__shfl_sync(0xffffffffu, sp, l)), m);
+                    }
+                    uint32_t direct = __ballot_sync(0xffffffffu, (sht && !stg) || ovl);
+                    while (direct) {                                     // byte i of the match = seed[i mod period] (FORMAT.md §2)
+                        const int l = __ffs(direct) - 1; direct &= direct - 1;
+                        const uint32_t d2 = __shfl_sync(0xffffffffu, dst_rel, l), m = __shfl_sync(0xffffffffu, len, l);
+                        const uint32_t per = __shfl_sync(0xffffffffu, (uint32_t)min((unsigned long long)(dst - src), 0xffffffffull), l);
+                        const uint8_t* sq = reinterpret_cast<const uint8_t*>(__shfl_sync(0xffffffffu, sp, l));
+                        uint32_t r = lane % per; const uint32_t stp = 32 % per;
+                        for (uint32_t i = lane; i < m; i += 32) { out_blk[d2 + i] = __ldcg(sq + r); r += stp; if (r >= per) r -= per; }
+                    }
+                    pending = __ballot_sync(0xffffffffu, stg);
+                    if (pending == 0) continue;
+                }
+                const bool mine = (pending >> lane) & 1u;
+                const uint32_t need = mine ? (mis + len + 15u) >> 4 : 0u;
+                uint32_t ce = need;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) { uint32_t a = __shfl_up_sync(0xffffffffu, ce, o); if (lane >= (uint32_t)o) ce += a; }
+                const bool fits = mine && ce <= STAGE_CHUNKS;
+                const uint32_t fmask = __ballot_sync(0xffffffffu, fits);
+                if (fits) {
+                    const uint32_t so = 16u * (ce - need);
+                    const uint8_t* g = reinterpret_cast<const uint8_t*>(sp - mis);
+                    for (uint32_t q = 0; q < need; q++) cp_async16s(stage + so + 16 * q, g + 16 * q);
+                    const uint64_t dp = reinterpret_cast<uint64_t>(out_blk) + dst_rel;
+                    sts128(mtab + 16 * __popc(fmask & lanemask_lt()), (uint32_t)dp, (uint32_t)(dp >> 32) | (len << 24), stage + so + mis, 0);
+                }
+                const uint32_t n_ent = __popc(fmask);
+                if (lane == 0) sts128(mtab + 16 * n_ent, 0, 0, 0, 0);   // empty entry: matches are taken two at a time
+                cp_async_commit();
+                pending &= ~fmask;
+                return n_ent;
+            }
+        };
+        auto copy_out = [&](uint32_t buf, uint32_t n_ent) {
+            const uint32_t mtab = sbase + buf * (MTAB_BYTES + 16 * STAGE_CHUNKS);
+            uint32_t more = 0;
+            for (uint32_t k = 0; k < n_ent; k += 2) {
+                const uint4 e0 = lds128(mtab + 16 * k), e1 = lds128(mtab + 16 * k + 16);
+                const uint32_t l0 = e0.y >> 24, l1 = e1.y >> 24;
+                const uint32_t a0 = e0.z + lane, a1 = e1.z + lane;
+                const uint32_t v00 = lds8(a0), v01 = lds8(a0 + 32), v10 = lds8(a1), v11 = lds8(a1 + 32);
+                uint8_t* d0 = reinterpret_cast<uint8_t*>((uint64_t)(e0.y & 0xffffffu) << 32 | e0.x) + lane;
+                uint8_t* d1 = reinterpret_cast<uint8_t*>((uint64_t)(e1.y & 0xffffffu) << 32 | e1.x) + lane;
+                if (lane < l0) d0[0] = (uint8_t)v00;
+                if (lane + 32 < l0) d0[32] = (uint8_t)v01;
+                if (lane < l1) d1[0] = (uint8_t)v10;
+                if (lane + 32 < l1) d1[32] = (uint8_t)v11;
+                more |= (l0 > 64 ? 1u : 0u) << k | (l1 > 64 ? 2u : 0u) << k;
+            }
+            while (more) {                                   // bytes 64.. of the longer ones (about one match in nine on FASTQ)
+                const int k = __ffs(more) - 1; more &= more - 1;
+                const uint4 e = lds128(mtab + 16 * k);
+                const uint32_t ln = e.y >> 24, sa = e.z + lane;
+                uint8_t* dp = reinterpret_cast<uint8_t*>((uint64_t)(e.y & 0xffffffu) << 32 | e.x) + lane;
+                for (uint32_t o = 64; o + lane < ln; o += 32) dp[o] = (uint8_t)lds8(sa + o);
+            }
+        };
+        if (!done) {
+            uint32_t cur = 0, n_cur = issue(0);
+            for (;;) {
+                uint32_t n_nxt = 0;
+                if (done) cp_async_commit(); else n_nxt = issue(cur ^ 1);
+                cp_async_wait_group<1>();                    // everything but the round just issued has landed
+                __syncwarp();
+                copy_out(cur, n_cur);
+                __syncwarp();                                // this buffer is refilled by the next round
+                if (done && n_nxt == 0) break;
+                n_cur = n_nxt; cur ^= 1;
+            }
+            cp_async_wait_group<0>();
+        }
+        if (WAIT) {                                          // publish: the warp's stores happen-before lane 0's fence + release
+            __syncwarp();
+            if (lane == 0) { __threadfence(); st_release(P.flags + b, 2 * P.epoch + 1); }
+        }
+    }
+}
+
 // Bucket offsets and work items of the list in P.gl_cur: one CTA scans the touched blocks (their record counts and their
 // numbers of work items) 1024 at a time; cnt[block] becomes the fill pointer of the block's bucket.
 __global__ void __launch_bounds__(1024, 1) k_plan(const Params P) {
@@ -975,6 +1145,8 @@ struct aceapex_archive {
     uint32_t* d_luts = nullptr;
     uint32_t* d_level_lists = nullptr;                  // concatenated level_blocks
     uint16_t* d_levels = nullptr;                       // level per block (compact copy of the directory field)
+    uint64_t* d_match_prefix = nullptr;                 // matches in blocks [0, b), n_blocks + 1 entries
+    uint64_t desc_off = 0, cplanes_off = 0;             // workspace: (dst_rel, len) and coded offset planes of every match
     std::vector<uint64_t> level_off;
     // workspace (caller's)
     uint8_t* d_ws = nullptr; uint64_t ws_bytes = 0; bool ws_clean = false;
@@ -1044,6 +1216,8 @@ void layout_workspace(aceapex_archive* ar) {
     ar->gl_sorted_off = off; off = align_up(off + ar->gl_cap * sizeof(GDemand), 256);
     ar->gl_work_off = off; off = align_up(off + 8 * ar->gl_wcap, 256);
     ar->gl_workn_off = off; off = align_up(off + 4 * ar->gl_wcap, 256);
+    ar->desc_off = off; off = align_up(off + 8 * (ar->total_matches + 1), 256);
+    ar->cplanes_off = off; off = align_up(off + (uint64_t)ar->n_coded_planes * ar->total_matches + 16, 256);
     ar->ws_need = off;
 }
 
@@ -1079,6 +1253,7 @@ void fill_params(const aceapex_archive* ar, Params& P) {
     P.scratch_per_warp = ar->scratch_per_warp; P.max_cmds = ar->max_cmds;
     P.out_pos0 = 0; P.win_end = ar->N;
     P.stacks = reinterpret_cast<Demand*>(ar->d_ws + ar->stacks_off); P.stack_cap = ar->stack_cap;
+    P.pairs = nullptr; P.cplanes = nullptr; P.match_prefix = ar->d_match_prefix;
 }
 
 int32_t prepare_ws(aceapex_archive* ar) {
@@ -1098,7 +1273,14 @@ int32_t launch(aceapex_archive* ar, Params& P, uint64_t n_work) {
     uint64_t warps = ar->threads / 32;
     uint32_t grid = (uint32_t)std::min<uint64_t>(ar->grid, (n_work + warps - 1) / warps);
     const bool whole = P.out_pos0 == 0 && P.win_end == ar->N;
-    if (P.mode >= 5) {                                        // range decode: collect / window matches / serve
+    if (P.mode >= 8) {                                        // whole-file match resolution from descriptors
+        const int T = ar->threads;
+        uint64_t w = T / 32;
+        uint32_t g = (uint32_t)std::min<uint64_t>(ar->sms, (n_work + w - 1) / w);
+        const size_t sm = (size_t)(T / 32) * COPY_WARP_BYTES + 64;
+        if (P.mode == 8) k_copy<false><<<g, T, sm, ar->stream>>>(P); else k_copy<true><<<g, T, sm, ar->stream>>>(P);
+    }
+    else if (P.mode >= 5) {                                        // range decode: collect / window matches / serve
         const int T = ar->threads;
         uint64_t w = T / 32;
         uint32_t g = (uint32_t)std::min<uint64_t>(ar->sms, (n_work + w - 1) / w);
@@ -1211,6 +1393,7 @@ int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* 
         ar->h_match_prefix[b + 1] = ar->h_match_prefix[b] + n_match;
         ar->h_payload_off[b] = po;
     }
+    if (ar->h_match_prefix[ar->n_blocks] != ar->total_matches) return ACEAPEX_E_CORRUPT;
     // device tables
     if (!luts.empty()) {
         CU(cudaMalloc(&ar->d_luts, luts.size() * 4));
@@ -1222,6 +1405,8 @@ int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* 
         for (uint64_t b = 0; b < ar->n_blocks; b++) lv[b] = rd16(meta + ar->dir_off + 32 * b + 28);
         CU(cudaMalloc(&ar->d_levels, lv.size() * 2));
         CU(cudaMemcpy(ar->d_levels, lv.data(), lv.size() * 2, cudaMemcpyHostToDevice));
+        CU(cudaMalloc(&ar->d_match_prefix, ar->h_match_prefix.size() * 8));
+        CU(cudaMemcpy(ar->d_match_prefix, ar->h_match_prefix.data(), ar->h_match_prefix.size() * 8, cudaMemcpyHostToDevice));
     }
     if (ar->n_blocks && ar->n_blocks < (1ull << 32)) {
         std::vector<uint32_t> cat;
@@ -1247,9 +1432,10 @@ int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* 
         const void* fns[] = {(const void*)k_decode<false>, (const void*)k_decode<true>, (const void*)k_literals<1024>, (const void*)k_literals<768>,
                              (const void*)k_matches<false, 1024>, (const void*)k_matches<false, 768>, (const void*)k_matches<true, 1024>,
                              (const void*)k_matches<true, 768>, (const void*)k_matches<false, 1024, true, true>,
-                             (const void*)k_matches<false, 1024, true, false>, (const void*)k_serve};
+                             (const void*)k_matches<false, 1024, true, false>, (const void*)k_serve, (const void*)k_copy<false>,
+                             (const void*)k_copy<true>};
         for (const void* f : fns) {
-            CU(cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max(ar->smem, smem_matches(ar, ar->threads))));
+            CU(cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max(std::max(ar->smem, smem_matches(ar, ar->threads)), (size_t)(ar->threads / 32) * COPY_WARP_BYTES + 64)));
             CU(cudaFuncSetAttribute(f, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
         }
     }
@@ -1273,6 +1459,7 @@ int32_t aceapex_close(aceapex_archive* ar) {
     if (ar->d_luts) cudaFree(ar->d_luts);
     if (ar->d_level_lists) cudaFree(ar->d_level_lists);
     if (ar->d_levels) cudaFree(ar->d_levels);
+    if (ar->d_match_prefix) cudaFree(ar->d_match_prefix);
     if (ar->d_chunk_lists) cudaFree(ar->d_chunk_lists);
     for (cudaEvent_t e : ar->ev_h2d) cudaEventDestroy(e);
     for (cudaEvent_t e : ar->ev_dec) cudaEventDestroy(e);
@@ -1313,19 +1500,20 @@ int32_t aceapex_decode_all(aceapex_archive* ar, void* d_out) {
     if (rc) return rc;
     Params P; fill_params(ar, P);
     P.out = static_cast<uint8_t*>(d_out); P.out_pos0 = 0; P.first_block = 0;
+    P.pairs = reinterpret_cast<uint2*>(ar->d_ws + ar->desc_off);          // k_literals leaves (dst_rel, len) and the coded offset
+    P.cplanes = ar->d_ws + ar->cplanes_off;                               // planes of every match for k_copy
     P.mode = 2; P.level_list = nullptr;
     if ((rc = launch(ar, P, ar->n_blocks))) return rc;
-    // matches never wait in this schedule: every source is a literal byte (placed by the launch above) or a match
-    // byte of a lower-level block (completed by an earlier launch) -- FORMAT.md §3
     if (!ar->d_level_lists) return ACEAPEX_OK;
-    // the top level (on FASTQ 97 % of the blocks sit at the level cap) runs without waits in a launch of its own; the
-    // few blocks of all lower levels share one flag-driven launch instead of one small latency-bound launch per level
+    // the top level (on FASTQ 97 % of the blocks sit at the level cap) runs without waits in a launch of its own: every
+    // source is a literal byte (placed by the launch above) or a match byte of a lower level (FORMAT.md §3); the few
+    // blocks of all lower levels share one flag-driven launch instead of one small latency-bound launch per level
     const uint32_t top = ar->max_level;
     if (top > 0 && ar->level_off[top] > 0) {
-        P.mode = 4; P.level_list = ar->d_level_lists; P.epoch = ++ar->epoch;
+        P.mode = 9; P.level_list = ar->d_level_lists; P.epoch = ++ar->epoch;
         if ((rc = launch(ar, P, ar->level_off[top]))) return rc;
     }
-    P.mode = 3; P.level_list = ar->d_level_lists + ar->level_off[top];
+    P.mode = 8; P.level_list = ar->d_level_lists + ar->level_off[top];
     return launch(ar, P, ar->level_blocks[top].size());
 }
 
@@ -1580,6 +1768,7 @@ int32_t aceapex_decode_all_host(aceapex_archive* ar, const void* h_archive, void
     CU(cudaMemcpyAsync(d_a, h_a, ar->payload_off, cudaMemcpyHostToDevice, ar->s_h2d));     // header, tables, directory, fnv
     Params P; fill_params(ar, P);
     P.out = static_cast<uint8_t*>(d_stage); P.out_pos0 = 0;
+    P.pairs = reinterpret_cast<uint2*>(ar->d_ws + ar->desc_off); P.cplanes = ar->d_ws + ar->cplanes_off;
     for (uint64_t k = 0; k < n_chunks; k++) {
         const uint64_t b0 = k * ar->chunk_blocks, b1 = std::min(ar->n_blocks, b0 + ar->chunk_blocks);
         const uint64_t p0 = ar->h_payload_off[b0], p1 = b1 < ar->n_blocks ? ar->h_payload_off[b1] : ar->archive_bytes;
@@ -1590,7 +1779,7 @@ int32_t aceapex_decode_all_host(aceapex_archive* ar, const void* h_archive, void
         if ((rc = launch(ar, P, b1 - b0))) return rc;
         for (uint32_t l = 0; l < n_lv; l++) {
             const uint64_t l0 = ar->chunk_level_off[k * n_lv + l], l1 = ar->chunk_level_off[k * n_lv + l + 1];
-            P.mode = 3; P.level_list = ar->d_chunk_lists + l0; P.first_block = 0;
+            P.mode = 8; P.level_list = ar->d_chunk_lists + l0; P.first_block = 0;
             if ((rc = launch(ar, P, l1 - l0))) return rc;
         }
         CU(cudaEventRecord(ar->ev_dec[k], ar->stream));

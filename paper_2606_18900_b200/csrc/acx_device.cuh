@@ -41,6 +41,7 @@ struct GList {
     uint32_t cap, touched_cap, work_cap;
 };
 
+
 struct Params {
     const uint8_t* archive;      // device archive
     uint64_t archive_bytes;
@@ -72,6 +73,10 @@ struct Params {
                                          // 4 = all match waves with flags
     const uint32_t* level_list;          // block ids to process (n_work entries), null = first_block + i
     GList gl_cur, gl_nxt;                // range decode: demands being served / being collected
+    uint2* pairs;                        // whole-file decode, left by k_literals for k_copy: (dst_rel, len) of every match,
+                                         // block b at pairs[match_prefix[b] ..]
+    uint8_t* cplanes;                    // ... and its decoded coded offset planes: n_coded_planes x n_match bytes per block
+    const uint64_t* match_prefix;        // n_blocks + 1 entries
 };
 
 __device__ __forceinline__ uint32_t lane_id() { return threadIdx.x & 31; }
