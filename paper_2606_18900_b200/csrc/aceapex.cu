@@ -854,9 +854,16 @@ __global__ void __launch_bounds__(1024, 1) k_copy(const Params P) {
         auto load_desc = [&](uint32_t j) -> uint4 {
             if (j >= n) return make_uint4(0, 0, 0, 0);
             const uint2 pr = __ldcg(prs + j);
+            const uint8_t* cq = cpl + j; const uint8_t* rq = raw + j;
+            if (P.W <= 4) {                                   // files up to 4 GiB: 32-bit arithmetic
+                uint32_t s32 = 0;
+                for (uint32_t k = 0; k < P.n_coded_planes; k++, cq += n) s32 |= (uint32_t)__ldcg(cq) << P.coded_shift[k];
+                for (uint32_t r = 0; r < P.n_raw_planes; r++, rq += n) s32 |= (uint32_t)__ldg(rq) << P.raw_shift[r];
+                return make_uint4(s32, 0, pr.x, pr.y);
+            }
             uint64_t src = 0;
-            for (uint32_t k = 0; k < P.n_coded_planes; k++) src |= (uint64_t)__ldcg(cpl + (uint64_t)k * n + j) << P.coded_shift[k];
-            for (uint32_t r = 0; r < P.n_raw_planes; r++) src |= (uint64_t)__ldg(raw + (uint64_t)r * n + j) << P.raw_shift[r];
+            for (uint32_t k = 0; k < P.n_coded_planes; k++, cq += n) src |= (uint64_t)__ldcg(cq) << P.coded_shift[k];
+            for (uint32_t r = 0; r < P.n_raw_planes; r++, rq += n) src |= (uint64_t)__ldg(rq) << P.raw_shift[r];
             return make_uint4((uint32_t)src, (uint32_t)(src >> 32), pr.x, pr.y);
         };
         uint4 nd = load_desc(lane);                           // descriptors are loaded one group ahead
