@@ -127,9 +127,10 @@ int32_t aceapex_set_resident(aceapex_archive* ar, uint32_t slot, uint64_t pos_lo
  * of mismatching blocks.  E_ARG when the archive has no FNV section. */
 int32_t aceapex_verify_fnv(aceapex_archive* ar, const void* d_data, uint64_t byte_lo, uint64_t byte_hi, uint64_t* n_bad);
 
-/* End-to-end convenience for host data (bench "e2e"; §6.1): copies h_archive (pinned or pageable, same
- * bytes the handle was opened on) into the handle's device archive, decodes into d_out_staging (>= N device bytes),
- * copies the result to h_out, and synchronises. */
+/* End to end with HOST buffers (bench "e2e"; §6.1): h_archive (the same bytes the handle was opened on,
+ * ideally pinned) -> the handle's device archive -> decode into d_out_staging (>= N device bytes, 16-byte aligned) -> h_out
+ * (ideally pinned).  Pipelined over chunks of blocks on three streams: the payload of chunk k+1 travels host -> device
+ * while chunk k decodes and the output of chunk k-1 travels device -> host.  Synchronous: returns when h_out is complete. */
 int32_t aceapex_decode_all_host(aceapex_archive* ar, const void* h_archive, void* d_out_staging, void* h_out);
 
 /* Synchronises the stream and returns E_CORRUPT if any kernel latched an integrity error since the last check
