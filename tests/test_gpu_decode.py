@@ -127,3 +127,34 @@ def test_device_integrity_flag(fastq_4m_archive):
         ar.check()
     assert e.value.name == "E_CORRUPT"
     ar.close()
+
+
+def test_wide_offsets_many_coded_planes_fewer_warps_per_cta():
+    """W = 8 with every offset plane rANS-coded: 11 decode tables (88 KB) leave room for fewer than 32 warps per CTA, so
+    the library launches smaller CTAs; every schedule, a range and reads must still be exact."""
+    from paper_2606_18900_b200.aceapex import Archive
+    lit = bytes((i * 7 + 3) % 251 for i in range(300))
+    blocks = [[(lit, (0, 300)), (b"", (10, 4 + 255)), (lit[:255], (1, 4 + 254)), (b"q", None)]]
+    N = 300 + 300 + 259 + 255 + 258 + 1
+    for W, raw in ((8, ()), (8, (0, 3, 7)), (6, ()), (5, (0,))):
+        a = build(blocks, N, 11, W=W, raw_planes=raw)
+        exp = O.decode(a).tobytes()
+        for sched in (None, "flags", "fused"):
+            assert gpu_decode(a, schedule=sched).tobytes() == exp, (W, raw, sched)
+        ar = Archive(a)
+        assert ar.decode_range(100, 1200).cpu().numpy().tobytes() == exp[100:1200]
+        idx = np.array([(5 | (700 << 40)), (900 | (300 << 40))], dtype=np.uint64)
+        got = ar.decode_reads(idx, np.array([1, 0, 1], dtype=np.uint64)).cpu().numpy().tobytes()
+        assert got[:1300] == exp[900:1200] + exp[5:705] + exp[900:1200]
+        ar.check()
+        ar.close()
+
+
+def test_output_must_be_16_byte_aligned(fastq_4m_archive):
+    from paper_2606_18900_b200.aceapex import AceapexError, Archive
+    ar = Archive(fastq_4m_archive)
+    out = ar.new_output(ar.raw_bytes + 64)
+    with pytest.raises(AceapexError) as e:
+        ar.decode_all(out[8:])
+    assert e.value.name == "E_ARG"
+    ar.close()
