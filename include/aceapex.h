@@ -101,8 +101,10 @@ int32_t aceapex_decode_all_fused(aceapex_archive* ar, void* d_out);
 
 /* Arbitrary byte range [byte_lo, byte_hi) (§4, "v7-RA"): d_out[0 .. hi-lo) = those bytes; only the
  * covering blocks are decoded, sources outside the range are reconstructed on demand by recursion on their own
- * sources (depth <= max_level + 1, FORMAT.md §3).  vram_budget: upper bound on workspace bytes the call may use
- * (0 = the whole workspace); E_BUDGET if it is below the minimum.  lo == hi is a no-op.  E_RANGE if lo > hi or hi > N. */
+ * sources (depth <= max_level + 1, FORMAT.md §3).  vram_budget: upper bound on the workspace bytes the call touches
+ * (0 = the whole workspace): a smaller budget shrinks the demand lists, the window is then served in more sub-windows;
+ * E_BUDGET below the minimum (the fixed part of the workspace + 4096 demand records).  lo == hi is a no-op.  E_RANGE if
+ * lo > hi or hi > N. */
 int32_t aceapex_decode_range(aceapex_archive* ar, uint64_t byte_lo, uint64_t byte_hi, void* d_out, uint64_t vram_budget);
 
 /* Read-level random access (§4.1).  h_read_index: host array of n_index entries, 8 bytes per read

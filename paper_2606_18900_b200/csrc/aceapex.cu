@@ -1168,6 +1168,7 @@ struct aceapex_archive {
     uint32_t stack_cap = 0, demand_cap = 0;
     uint64_t gl_cap = 0, gl_tcap = 0, gl_wcap = 0, gl_rec_off[2] = {0, 0}, gl_cnt_off[2] = {0, 0}, gl_touched_off[2] = {0, 0};   // range decode lists
     uint64_t gl_sorted_off = 0, gl_work_off = 0, gl_workn_off = 0;
+    uint64_t gl_eff = 0;                               // records a range-decode call may use (vram_budget), <= gl_cap
     std::vector<uint64_t> h_match_prefix;             // matches in blocks [0, b)
     // end-to-end pipeline (aceapex_decode_all_host): chunks of blocks, per chunk the block ids sorted by level
     uint64_t chunk_blocks = 0; uint32_t* d_chunk_lists = nullptr; std::vector<uint64_t> chunk_level_off;   // (chunk, level) -> offset
@@ -1237,7 +1238,7 @@ GList glist(const aceapex_archive* ar, int k) {
     g.work = reinterpret_cast<unsigned long long*>(ar->d_ws + ar->gl_work_off);
     g.work_n = reinterpret_cast<uint32_t*>(ar->d_ws + ar->gl_workn_off);
     g.count = reinterpret_cast<uint32_t*>(ar->d_ws + 64 + 16 * k);
-    g.cap = (uint32_t)ar->gl_cap; g.touched_cap = (uint32_t)ar->gl_tcap; g.work_cap = (uint32_t)ar->gl_wcap;
+    g.cap = (uint32_t)(ar->gl_eff ? ar->gl_eff : ar->gl_cap); g.touched_cap = (uint32_t)ar->gl_tcap; g.work_cap = (uint32_t)ar->gl_wcap;
     return g;
 }
 
@@ -1300,9 +1301,9 @@ int32_t launch(aceapex_archive* ar, Params& P, uint64_t n_work) {
         const size_t sm = P.mode == 2 ? smem_for(ar, T) : smem_matches(ar, T);
         uint64_t w = T / 32;
         uint32_t g = (uint32_t)std::min<uint64_t>(ar->sms, (n_work + w - 1) / w);
-        if (P.mode == 2) { if (T == 768) k_literals<768><<<g, T, sm, ar->stream>>>(P); else k_literals<1024><<<g, T, sm, ar->stream>>>(P); }
-        else if (P.mode == 3) { if (T == 768) k_matches<false, 768><<<g, T, sm, ar->stream>>>(P); else k_matches<false, 1024><<<g, T, sm, ar->stream>>>(P); }
-        else { if (T == 768) k_matches<true, 768><<<g, T, sm, ar->stream>>>(P); else k_matches<true, 1024><<<g, T, sm, ar->stream>>>(P); }
+        if (P.mode == 2) k_literals<1024><<<g, T, sm, ar->stream>>>(P);
+        else if (P.mode == 3) k_matches<false, 1024><<<g, T, sm, ar->stream>>>(P);
+        else k_matches<true, 1024><<<g, T, sm, ar->stream>>>(P);
     }
     else if (P.mode == 1 || !whole) k_decode<true><<<grid, ar->threads, ar->smem, ar->stream>>>(P);
     else k_decode<false><<<grid, ar->threads, ar->smem, ar->stream>>>(P);
@@ -1431,14 +1432,9 @@ int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* 
     while (ar->threads > 128 && std::max(smem_for(ar, ar->threads), smem_matches(ar, ar->threads)) > (size_t)prop.sharedMemPerBlockOptin) ar->threads -= 128;
     ar->smem = smem_for(ar, ar->threads);
     ar->threads_lit = ar->threads_match = ar->threads;
-    if (ar->threads == 1024) {                                // 768-thread variants trade occupancy for registers (80 vs 64)
-        if (const char* e = getenv("ACEAPEX_LIT_THREADS")) if (atoi(e) == 768) ar->threads_lit = 768;
-        if (const char* e = getenv("ACEAPEX_MATCH_THREADS")) if (atoi(e) == 768) ar->threads_match = 768;
-    }
     {
-        const void* fns[] = {(const void*)k_decode<false>, (const void*)k_decode<true>, (const void*)k_literals<1024>, (const void*)k_literals<768>,
-                             (const void*)k_matches<false, 1024>, (const void*)k_matches<false, 768>, (const void*)k_matches<true, 1024>,
-                             (const void*)k_matches<true, 768>, (const void*)k_matches<false, 1024, true, true>,
+        const void* fns[] = {(const void*)k_decode<false>, (const void*)k_decode<true>, (const void*)k_literals<1024>,
+                             (const void*)k_matches<false, 1024>, (const void*)k_matches<true, 1024>, (const void*)k_matches<false, 1024, true, true>,
                              (const void*)k_matches<false, 1024, true, false>, (const void*)k_serve, (const void*)k_copy<false>,
                              (const void*)k_copy<true>};
         for (const void* f : fns) {
@@ -1593,7 +1589,15 @@ int32_t aceapex_decode_range(aceapex_archive* ar, uint64_t lo, uint64_t hi, void
     if (lo > hi || hi > ar->N) return ACEAPEX_E_RANGE;
     if (lo == hi) return ACEAPEX_OK;
     if (!d_out) return ACEAPEX_E_ARG;
-    if (budget && budget < workspace_need(ar)) return ACEAPEX_E_BUDGET;
+    // vram_budget bounds the workspace bytes this call touches: everything but the demand lists is fixed, the lists use
+    // 3 x 24 bytes per record (two arrival arrays, one bucketed copy) plus their work items; fewer records mean more
+    // sub-windows, not failure, down to a floor of 4096 records
+    ar->gl_eff = ar->gl_cap;
+    if (budget && budget < workspace_need(ar)) {
+        const uint64_t per_rec = 3 * sizeof(GDemand) + 8, fixed = workspace_need(ar) - std::min<uint64_t>(workspace_need(ar), per_rec * ar->gl_cap);
+        if (budget < fixed + per_rec * 4096) return ACEAPEX_E_BUDGET;
+        ar->gl_eff = std::min<uint64_t>(ar->gl_cap, (budget - fixed) / per_rec);
+    }
     int32_t rc = prepare_ws(ar);
     if (rc) return rc;
     const uint64_t BS = 1ull << ar->log2_bs;
@@ -1626,7 +1630,7 @@ int32_t aceapex_decode_range(aceapex_archive* ar, uint64_t lo, uint64_t hi, void
             const GList g[2] = {glist(ar, 0), glist(ar, 1)};
             for (uint64_t s0 = b0; s0 < b1;) {                // sub-windows whose demands fit the lists
                 uint64_t s1 = s0 + 1;
-                while (s1 < b1 && ar->h_match_prefix[s1 + 1] - ar->h_match_prefix[s0] <= ar->gl_cap / 3) s1++;
+                while (s1 < b1 && ar->h_match_prefix[s1 + 1] - ar->h_match_prefix[s0] <= ar->gl_eff / 3) s1++;
                 CU(cudaMemsetAsync(g[0].count, 0, 32, ar->stream));
                 P.mode = 5; P.level_list = nullptr; P.first_block = s0; P.gl_nxt = g[0];
                 if ((rc = launch(ar, P, s1 - s0))) return rc;

@@ -238,3 +238,22 @@ def test_end_to_end_host_pipeline(big, fq):
             ar.decode_all_host(h_arch, stage, h_out)
             ar.check()
             assert T.equal(h_out, T.from_numpy(x))
+
+
+def test_small_vram_budget_means_more_sub_windows_not_failure(big):
+    """vram_budget below the full workspace shrinks the demand lists: the window is served in several sub-windows."""
+    from paper_2606_18900_b200.aceapex import AceapexError
+    ar, x = big[0]
+    need = ar.info()["workspace_bytes"]
+    lo, hi = 200 * 16384, 700 * 16384
+    served = 0
+    for budget in (need - 1, need - (1 << 20), need - (4 << 20), need - (7 << 20), need // 2):
+        try:
+            got = ar.decode_range(lo, hi, vram_budget=budget)
+        except AceapexError as e:
+            assert e.name == "E_BUDGET"                      # below the floor: refused, never wrong
+            continue
+        ar.check()
+        assert got.cpu().numpy().tobytes() == x[lo:hi].tobytes(), budget
+        served += 1
+    assert served >= 3
