@@ -142,6 +142,13 @@ uint32_t aceapex_device_flags(const aceapex_archive* ar);   /* bit set of ACEAPE
 int32_t aceapex_last_cuda_error(const aceapex_archive* ar); /* cudaError_t of the last failing runtime call         */
 const char* aceapex_strerror(int32_t code);
 
+/* Per-kernel device times of aceapex_decode_all (bench.py "roofline"): when switched on, the call records CUDA events on the
+ * handle's stream around its three launches.  aceapex_phase_times waits for the last aceapex_decode_all and returns, in
+ * milliseconds, ms3[0] = literal launch (entropy decode + scan + literal placement), ms3[1] = match launch of the blocks
+ * below the top level, ms3[2] = match launch of the top level.  E_ARG when timing is off or nothing was decoded. */
+int32_t aceapex_set_phase_timing(aceapex_archive* ar, int32_t on);
+int32_t aceapex_phase_times(aceapex_archive* ar, float* ms3);
+
 /* Number of kernel launches the library issued on this handle so far (bench.py "gpu_launches"). */
 uint64_t aceapex_launch_count(const aceapex_archive* ar);
 

@@ -59,6 +59,8 @@ def load():
             "aceapex_last_cuda_error": ([p], i32),
             "aceapex_strerror": ([i32], ctypes.c_char_p),
             "aceapex_launch_count": ([p], u64),
+            "aceapex_set_phase_timing": ([p, i32], i32),
+            "aceapex_phase_times": ([p, ctypes.POINTER(ctypes.c_float)], i32),
         }
         for name, (args, res) in sig.items():
             f = getattr(L, name)
@@ -119,6 +121,15 @@ class Archive:
         if rc:
             raise AceapexError(rc, "device flags 0x%x cuda %d" % (self.L.aceapex_device_flags(self.h),
                                                                    self.L.aceapex_last_cuda_error(self.h)))
+
+    def set_phase_timing(self, on=True):
+        _chk(self.L.aceapex_set_phase_timing(self.h, 1 if on else 0))
+
+    def phase_times(self):
+        """(literal launch, lower-level match launch, top-level match launch) of the last decode_all, in ms."""
+        ms = (ctypes.c_float * 3)()
+        _chk(self.L.aceapex_phase_times(self.h, ms), "phase_times")
+        return [float(v) for v in ms]
 
     def launch_count(self):
         return int(self.L.aceapex_launch_count(self.h))

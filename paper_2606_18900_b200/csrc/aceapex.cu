@@ -1174,6 +1174,7 @@ struct aceapex_archive {
     uint64_t chunk_blocks = 0; uint32_t* d_chunk_lists = nullptr; std::vector<uint64_t> chunk_level_off;   // (chunk, level) -> offset
     std::vector<uint64_t> h_payload_off;               // payload offset of block b (n_blocks + 1 entries)
     cudaStream_t s_h2d = nullptr, s_d2h = nullptr; std::vector<cudaEvent_t> ev_h2d, ev_dec;
+    bool phase_timing = false; cudaEvent_t ev_phase[4] = {nullptr, nullptr, nullptr, nullptr};   // aceapex_set_phase_timing
     std::vector<uint16_t> h_levels;                    // host copy of the per-block levels
     std::vector<uint32_t> h_list; std::vector<Demand> h_demands;   // host staging for range / read calls
     // status
@@ -1466,6 +1467,7 @@ int32_t aceapex_close(aceapex_archive* ar) {
     if (ar->d_chunk_lists) cudaFree(ar->d_chunk_lists);
     for (cudaEvent_t e : ar->ev_h2d) cudaEventDestroy(e);
     for (cudaEvent_t e : ar->ev_dec) cudaEventDestroy(e);
+    for (cudaEvent_t e : ar->ev_phase) if (e) cudaEventDestroy(e);
     if (ar->s_h2d) cudaStreamDestroy(ar->s_h2d);
     if (ar->s_d2h) cudaStreamDestroy(ar->s_d2h);
     delete ar;
@@ -1505,8 +1507,11 @@ int32_t aceapex_decode_all(aceapex_archive* ar, void* d_out) {
     P.out = static_cast<uint8_t*>(d_out); P.out_pos0 = 0; P.first_block = 0;
     P.pairs = reinterpret_cast<uint2*>(ar->d_ws + ar->desc_off);          // k_literals leaves (dst_rel, len) and the coded offset
     P.cplanes = ar->d_ws + ar->cplanes_off;                               // planes of every match for k_copy
+    const bool tm = ar->phase_timing;
+    if (tm) CU(cudaEventRecord(ar->ev_phase[0], ar->stream));
     P.mode = 2; P.level_list = nullptr;
     if ((rc = launch(ar, P, ar->n_blocks))) return rc;
+    if (tm) CU(cudaEventRecord(ar->ev_phase[1], ar->stream));
     if (!ar->d_level_lists) return ACEAPEX_OK;
     // the top level (on FASTQ 97 % of the blocks sit at the level cap) runs without waits in a launch of its own: every
     // source is a literal byte (placed by the launch above) or a match byte of a lower level (FORMAT.md §3); the few
@@ -1516,8 +1521,25 @@ int32_t aceapex_decode_all(aceapex_archive* ar, void* d_out) {
         P.mode = 9; P.level_list = ar->d_level_lists; P.epoch = ++ar->epoch;
         if ((rc = launch(ar, P, ar->level_off[top]))) return rc;
     }
+    if (tm) CU(cudaEventRecord(ar->ev_phase[2], ar->stream));
     P.mode = 8; P.level_list = ar->d_level_lists + ar->level_off[top];
-    return launch(ar, P, ar->level_blocks[top].size());
+    rc = launch(ar, P, ar->level_blocks[top].size());
+    if (tm && !rc) CU(cudaEventRecord(ar->ev_phase[3], ar->stream));
+    return rc;
+}
+
+int32_t aceapex_set_phase_timing(aceapex_archive* ar, int32_t on) {
+    if (!ar) return ACEAPEX_E_ARG;
+    if (on && !ar->ev_phase[0]) for (int k = 0; k < 4; k++) CU(cudaEventCreate(&ar->ev_phase[k]));
+    ar->phase_timing = on != 0;
+    return ACEAPEX_OK;
+}
+
+int32_t aceapex_phase_times(aceapex_archive* ar, float* ms3) {
+    if (!ar || !ms3 || !ar->phase_timing || !ar->ev_phase[0]) return ACEAPEX_E_ARG;
+    CU(cudaEventSynchronize(ar->ev_phase[3]));
+    for (int k = 0; k < 3; k++) CU(cudaEventElapsedTime(ms3 + k, ar->ev_phase[k], ar->ev_phase[k + 1]));
+    return ACEAPEX_OK;
 }
 
 // literal launch + ONE match launch over the blocks sorted by (level, index) with completion flags

@@ -158,3 +158,17 @@ def test_output_must_be_16_byte_aligned(fastq_4m_archive):
         ar.decode_all(out[8:])
     assert e.value.name == "E_ARG"
     ar.close()
+
+
+def test_phase_times(fastq_4m_archive):
+    from paper_2606_18900_b200.aceapex import AceapexError, Archive
+    ar = Archive(fastq_4m_archive)
+    with pytest.raises(AceapexError):
+        ar.phase_times()                                     # timing is off
+    ar.set_phase_timing(True)
+    out = ar.decode_all()
+    ms = ar.phase_times()
+    ar.check()
+    assert len(ms) == 3 and ms[0] > 0 and ms[2] > 0 and all(v >= 0 for v in ms)
+    ar.set_phase_timing(False)
+    ar.close()
