@@ -747,6 +747,12 @@ __device__ __forceinline__ CtaSmem setup_cta(const Params& P, uint8_t* smem_raw)
     return m;
 }
 
+// Two ticket slots alternate between consecutive launches of a handle: a kernel draws from its own slot and clears the
+// other one, so no memset has to be queued between launches (a seek is ~30 launches).
+__device__ __forceinline__ void clear_next_ticket(const Params& P) {
+    if (blockIdx.x == 0 && threadIdx.x == 0) *P.ticket_next = 0ull;
+}
+
 __device__ __forceinline__ bool next_ticket(const Params& P, unsigned long long& t) {
     t = 0;
     if (lane_id() == 0) t = atomicAdd(P.ticket, 1ull);
@@ -758,6 +764,7 @@ __device__ __forceinline__ bool next_ticket(const Params& P, unsigned long long&
 template <int MAXT>
 __global__ void __launch_bounds__(MAXT, 1) k_literals(const Params P) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
+    clear_next_ticket(P);
     const CtaSmem m = setup_cta(P, smem_raw);
     BlockCtx c;
     bind_scratch(P, blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), c);
@@ -790,6 +797,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_matches(const Params P) {
     // shared memory: [pad to 8 KB][tables without LIT (the last one): (n_coded_tables - 1) x 8 KB]
     //                [per warp: ring 2 KB | match table MTAB_BYTES | stage 16 x STAGE_CHUNKS]
     extern __shared__ __align__(16) uint8_t smem_raw[];
+    clear_next_ticket(P);
     const uint32_t smem0 = (uint32_t)__cvta_generic_to_shared(smem_raw);
     const uint32_t pad = (8192u - (smem0 & 8191u)) & 8191u;
     const uint32_t n_lut_words = (P.n_coded_tables - 1) * LUT_SIZE;
@@ -830,6 +838,7 @@ static_assert(COPY_WARP_BYTES % 16 == 0, "tables and stages are 16-byte aligned"
 template <bool WAIT>
 __global__ void __launch_bounds__(1024, 1) k_copy(const Params P) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
+    clear_next_ticket(P);
     const uint32_t lane = lane_id(), warp = threadIdx.x >> 5;
     const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(smem_raw) + warp * COPY_WARP_BYTES;
     const uint8_t* const out_end = P.out + (P.win_end - P.out_pos0);
@@ -1037,6 +1046,7 @@ __global__ void __launch_bounds__(256) k_scatter(const Params P) {
 // unknown go to the lists of the next round (recursion depth <= max_level + 1, FORMAT.md §3).
 __global__ void __launch_bounds__(1024, 1) k_serve(const Params P) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
+    clear_next_ticket(P);
     const CtaSmem m = setup_cta(P, smem_raw);
     BlockCtx c;
     bind_scratch(P, blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), c);
@@ -1074,6 +1084,7 @@ __global__ void k_assert_empty(const uint32_t* count, uint32_t* err) { if (*coun
 template <bool DEMANDS>
 __global__ void __launch_bounds__(1024, 1) k_decode(const Params P) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
+    clear_next_ticket(P);
     const CtaSmem m = setup_cta(P, smem_raw);
     const uint32_t s_luts = m.luts, ring = m.ring, runs = m.runs;
     const uint32_t gw = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
@@ -1086,7 +1097,10 @@ __global__ void __launch_bounds__(1024, 1) k_decode(const Params P) {
     unsigned long long t;
     while (next_ticket(P, t)) {
         if (DEMANDS && P.mode == 1) {                        // spans: one top-level demand per ticket
-            if (lane_id() == 0) push_span(P, st, P.demands[t].pos, P.demands[t].len, P.demands[t].dst);
+            if (lane_id() == 0) {
+                const Demand d = P.n_inline ? P.inline_dem[t] : P.demands[t];
+                push_span(P, st, d.pos, d.len, d.dst);
+            }
             process_demands(P, s_luts, ring, c, st);
             continue;
         }
@@ -1159,6 +1173,7 @@ struct aceapex_archive {
     uint8_t* d_ws = nullptr; uint64_t ws_bytes = 0; bool ws_clean = false;
     cudaStream_t stream = nullptr;
     uint32_t epoch = 0;
+    uint32_t ticket_slot = 0;                          // which of the two ticket slots the next launch draws from
     Resident res[MAX_RESIDENT];
     // launch geometry
     int sms = 148, ctas_per_sm = 1, threads = 1024, threads_lit = 1024, threads_match = 1024;
@@ -1191,7 +1206,7 @@ uint16_t rd16(const uint8_t* p) { uint16_t v; memcpy(&v, p, 2); return v; }
 
 uint64_t align_up(uint64_t v, uint64_t a) { return (v + a - 1) / a * a; }
 
-// workspace: [ctrl 256 B: ticket u64 @0, err u32 @8][flags: n_blocks x u32][scratch: warps x scratch_per_warp]
+// workspace: [ctrl 256 B: ticket slots u64 @0 and @24, err u32 @8, fnv count @16, list counters @64][flags: n_blocks x u32][scratch: warps x scratch_per_warp]
 //            [stacks: warps x stack_cap demands][demands: demand_cap][block list: n_blocks x u32]
 uint64_t workspace_need(const aceapex_archive* ar) { return ar->ws_need; }
 
@@ -1255,7 +1270,7 @@ void fill_params(const aceapex_archive* ar, Params& P) {
     for (uint32_t p = 0; p < ar->W; p++) if (ar->plane_raw[p] >= 0) P.raw_shift[ar->plane_raw[p]] = (uint8_t)(8 * p);
     P.lut_cmd = ar->lut_cmd; P.lut_mlen = ar->lut_mlen; P.lut_lit = ar->lut_lit;
     memcpy(P.res, ar->res, sizeof P.res);
-    P.ticket = reinterpret_cast<unsigned long long*>(ar->d_ws);
+    P.ticket = nullptr; P.ticket_next = nullptr;            // set per launch
     P.err = reinterpret_cast<uint32_t*>(ar->d_ws + 8);
     P.flags = reinterpret_cast<uint32_t*>(ar->d_ws + ar->ctrl_bytes);
     P.scratch = ar->d_ws + ar->scratch_off;
@@ -1270,7 +1285,7 @@ int32_t prepare_ws(aceapex_archive* ar) {
     if (!ar->ws_clean) {
         CU(cudaMemsetAsync(ar->d_ws, 0, ar->ctrl_bytes + ar->flags_bytes, ar->stream));
         for (int k = 0; k < 2; k++) CU(cudaMemsetAsync(ar->d_ws + ar->gl_cnt_off[k], 0, 4 * ar->n_blocks + 4, ar->stream));
-        ar->ws_clean = true; ar->epoch = 0;
+        ar->ws_clean = true; ar->epoch = 0; ar->ticket_slot = 0;
     }
     return ACEAPEX_OK;
 }
@@ -1278,7 +1293,9 @@ int32_t prepare_ws(aceapex_archive* ar) {
 int32_t launch(aceapex_archive* ar, Params& P, uint64_t n_work) {
     P.n_work = n_work;
     if (n_work == 0) return ACEAPEX_OK;
-    CU(cudaMemsetAsync(P.ticket, 0, 8, ar->stream));
+    P.ticket = reinterpret_cast<unsigned long long*>(ar->d_ws) + (ar->ticket_slot ? 3 : 0);       // bytes 0 and 24 of the control area
+    P.ticket_next = reinterpret_cast<unsigned long long*>(ar->d_ws) + (ar->ticket_slot ? 0 : 3);
+    ar->ticket_slot ^= 1;
     uint64_t warps = ar->threads / 32;
     uint32_t grid = (uint32_t)std::min<uint64_t>(ar->grid, (n_work + warps - 1) / warps);
     const bool whole = P.out_pos0 == 0 && P.win_end == ar->N;
@@ -1569,7 +1586,12 @@ int32_t aceapex_decode_all_fused(aceapex_archive* ar, void* d_out) {
 // launches span-mode work for the demands staged in ar->h_demands (in batches of demand_cap)
 static int32_t run_demands(aceapex_archive* ar, Params& P) {
     Demand* d_dem = reinterpret_cast<Demand*>(ar->d_ws + ar->demands_off);
-    P.mode = 1; P.level_list = nullptr; P.demands = d_dem;
+    P.mode = 1; P.level_list = nullptr; P.demands = d_dem; P.n_inline = 0;
+    if (ar->h_demands.size() <= 4) {                   // a single read: the items travel in the kernel arguments, no copy
+        P.n_inline = (uint32_t)ar->h_demands.size();
+        for (uint32_t i = 0; i < P.n_inline; i++) P.inline_dem[i] = ar->h_demands[i];
+        return launch(ar, P, P.n_inline);
+    }
     for (size_t i = 0; i < ar->h_demands.size(); i += ar->demand_cap) {
         size_t n = std::min<size_t>(ar->demand_cap, ar->h_demands.size() - i);
         CU(cudaMemcpyAsync(d_dem, ar->h_demands.data() + i, n * sizeof(Demand), cudaMemcpyHostToDevice, ar->stream));

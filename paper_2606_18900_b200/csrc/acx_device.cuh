@@ -61,11 +61,13 @@ struct Params {
     uint8_t* out;                        // FULL mode: byte at absolute position p is out[p - out_pos0]
     uint64_t out_pos0, win_end;          // out holds the original bytes [out_pos0, win_end) (the window; block aligned start)
     const Demand* demands; uint8_t* out2; // span mode (1): top-level work items, destination buffer of every demand
+    Demand inline_dem[4]; uint32_t n_inline; // span mode with at most four items: they travel in the kernel arguments
     Resident res[MAX_RESIDENT];
     // workspace
     uint32_t* flags;                     // per block: 2 * epoch = literals placed, 2 * epoch + 1 = complete
     uint32_t epoch;
-    unsigned long long* ticket;
+    unsigned long long* ticket;          // work counter of this launch (zero when the kernel starts)
+    unsigned long long* ticket_next;     // the other slot: every kernel clears it for the launch that follows
     uint32_t* err;
     uint8_t* scratch; uint64_t scratch_per_warp; uint32_t max_cmds;
     Demand* stacks; uint32_t stack_cap;  // per-warp LIFO of pending demands
