@@ -1,6 +1,7 @@
 // Host side of the C ABI (include/aceapex.h) and the decode kernels for sm_100a.
 #include "aceapex.h"
 #include "acx_device.cuh"
+#include <cooperative_groups.h>
 
 #include <algorithm>
 #include <cstdio>
@@ -988,16 +989,24 @@ __global__ void __launch_bounds__(1024, 1) k_copy(const Params P) {
 
 // Bucket offsets and work items of the list in P.gl_cur: one CTA scans the touched blocks (their record counts and their
 // numbers of work items) 1024 at a time; cnt[block] becomes the fill pointer of the block's bucket.
-__global__ void __launch_bounds__(1024, 1) k_plan(const Params P) {
+// The list arrays are written by other CTAs, possibly earlier in the SAME launch (k_rounds): they are read at L2.
+__device__ __forceinline__ GDemand ld_demand(const GDemand* p) {
+    const unsigned long long* q = reinterpret_cast<const unsigned long long*>(p);
+    GDemand d; d.pos = __ldcg(q); d.dst = __ldcg(q + 1);
+    const unsigned long long w = __ldcg(q + 2); d.len = (uint32_t)w; d.pad = (uint32_t)(w >> 32);
+    return d;
+}
+
+__device__ __forceinline__ void plan_body(const GList& g) {      // one CTA (any multiple of 32 threads up to 1024)
     __shared__ uint32_t s_rec[32], s_item[32], s_base[2];
-    const GList& g = P.gl_cur;
-    const uint32_t n = min(g.count[1], g.touched_cap), lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t n = min(__ldcg(g.count + 1), g.touched_cap), lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     if (threadIdx.x == 0) { s_base[0] = 0; s_base[1] = 0; }
     __syncthreads();
-    for (uint32_t t0 = 0; t0 < n; t0 += 1024) {
+    const uint32_t n_warps = blockDim.x >> 5;
+    for (uint32_t t0 = 0; t0 < n; t0 += blockDim.x) {
         const uint32_t t = t0 + threadIdx.x;
         uint32_t blk = 0, c = 0;
-        if (t < n) { blk = g.touched[t]; c = g.cnt[blk]; }
+        if (t < n) { blk = __ldcg(g.touched + t); c = __ldcg(g.cnt + blk); }
         uint32_t it = (c + GL_ITEM - 1) / GL_ITEM, ps = c, pi = it;      // inclusive warp scans of records and items
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
@@ -1007,7 +1016,7 @@ __global__ void __launch_bounds__(1024, 1) k_plan(const Params P) {
         if (lane == 31) { s_rec[warp] = ps; s_item[warp] = pi; }
         __syncthreads();
         if (warp == 0) {
-            uint32_t a = s_rec[lane], b2 = s_item[lane], sa = a, sb = b2;
+            uint32_t a = lane < n_warps ? s_rec[lane] : 0, b2 = lane < n_warps ? s_item[lane] : 0, sa = a, sb = b2;
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
                 uint32_t x = __shfl_up_sync(0xffffffffu, sa, o), y = __shfl_up_sync(0xffffffffu, sb, o);
@@ -1025,51 +1034,92 @@ __global__ void __launch_bounds__(1024, 1) k_plan(const Params P) {
             }
         }
         __syncthreads();
-        if (threadIdx.x == 1023) { s_base[0] = r0 + c; s_base[1] = i0 + it; }
+        if (threadIdx.x == blockDim.x - 1) { s_base[0] = r0 + c; s_base[1] = i0 + it; }
         __syncthreads();
     }
     if (threadIdx.x == 0) g.count[2] = min(s_base[1], g.work_cap);
 }
 
-__global__ void __launch_bounds__(256) k_scatter(const Params P) {
-    const GList& g = P.gl_cur;
-    const uint32_t n = min(g.count[0], g.cap);
-    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
-        const GDemand d = g.rec[i];
+__global__ void __launch_bounds__(1024, 1) k_plan(const Params P) { plan_body(P.gl_cur); }
+
+__device__ __forceinline__ void scatter_body(const Params& P, const GList& g, uint32_t tid, uint32_t n_threads) {
+    const uint32_t n = min(__ldcg(g.count), g.cap);
+    for (uint32_t i = tid; i < n; i += n_threads) {
+        const GDemand d = ld_demand(g.rec + i);
         const uint32_t p = atomicAdd(g.cnt + (d.pos >> P.log2_bs), 1u);
         if (p < g.cap) g.sorted[p] = d;
     }
 }
 
+__global__ void __launch_bounds__(256) k_scatter(const Params P) {
+    scatter_body(P, P.gl_cur, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
+}
+
 // One round of the demand lists of a range decode: a work item = up to GL_ITEM records of one source block; the block is
 // parsed once (tokens + all its literals into the warp's scratch) and serves them; match pieces whose sources are
 // unknown go to the lists of the next round (recursion depth <= max_level + 1, FORMAT.md §3).
+__device__ __forceinline__ void serve_body(const Params& P, const CtaSmem& m, BlockCtx& c, const GList& cur, const GList& nxt,
+                                           unsigned long long* ticket) {
+    const Stack sk{nullptr, 0, m.top, &nxt, 0};
+    const unsigned long long n = min(__ldcg(cur.count + 2), cur.work_cap);
+    for (;;) {
+        unsigned long long t = 0;
+        if (lane_id() == 0) t = atomicAdd(ticket, 1ull);
+        t = __shfl_sync(0xffffffffu, t, 0);
+        if (t >= n) break;
+        const unsigned long long item = __ldcg(cur.work + t);
+        const uint32_t first = (uint32_t)item, cnt = __ldcg(cur.work_n + t);
+        c.b = item >> 32;
+        if (lane_id() == 0) cur.cnt[c.b] = 0;                 // every item of the block writes the same value: the array is idle again
+        uint64_t pend = 0;                                    // the literals are needed up to the last span of the item
+        if (lane_id() < cnt && first + lane_id() < cur.cap) { const GDemand d = ld_demand(cur.sorted + first + lane_id()); pend = d.pos + d.len; }
+#pragma unroll
+        for (int o = 16; o >= 1; o >>= 1) pend = max((unsigned long long)pend, (unsigned long long)__shfl_xor_sync(0xffffffffu, pend, o));
+        const bool ok = parse_block_upto(P, m.luts, m.ring, c, pend);
+        for (uint32_t k = 0; k < cnt && first + k < cur.cap; k++) {
+            const GDemand d = ld_demand(cur.sorted + first + k);
+            if (ok) emit_span(P, c, sk, d.pos, d.len, d.dst);
+        }
+    }
+}
+
 __global__ void __launch_bounds__(1024, 1) k_serve(const Params P) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
     clear_next_ticket(P);
     const CtaSmem m = setup_cta(P, smem_raw);
     BlockCtx c;
     bind_scratch(P, blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), c);
-    const Stack sk{nullptr, 0, m.top, &P.gl_nxt, 0};
-    const unsigned long long n = min(__ldg(P.gl_cur.count + 2), P.gl_cur.work_cap);
-    for (;;) {
-        unsigned long long t = 0;
-        if (lane_id() == 0) t = atomicAdd(P.ticket, 1ull);
-        t = __shfl_sync(0xffffffffu, t, 0);
-        if (t >= n) break;
-        const unsigned long long item = P.gl_cur.work[t];
-        const uint32_t first = (uint32_t)item, cnt = P.gl_cur.work_n[t];
-        c.b = item >> 32;
-        if (lane_id() == 0) P.gl_cur.cnt[c.b] = 0;            // every item of the block writes the same value: the array is idle again
-        uint64_t pend = 0;                                    // the literals are needed up to the last span of the item
-        if (lane_id() < cnt && first + lane_id() < P.gl_cur.cap) { const GDemand d = P.gl_cur.sorted[first + lane_id()]; pend = d.pos + d.len; }
-#pragma unroll
-        for (int o = 16; o >= 1; o >>= 1) pend = max((unsigned long long)pend, (unsigned long long)__shfl_xor_sync(0xffffffffu, pend, o));
-        const bool ok = parse_block_upto(P, m.luts, m.ring, c, pend);
-        for (uint32_t k = 0; k < cnt && first + k < P.gl_cur.cap; k++) {
-            const GDemand d = P.gl_cur.sorted[first + k];
-            if (ok) emit_span(P, c, sk, d.pos, d.len, d.dst);
+    serve_body(P, m, c, P.gl_cur, P.gl_nxt, P.ticket);
+}
+
+// All rounds of a demand list in ONE cooperative launch (every CTA resident, grid-wide barriers between plan, scatter and
+// serve): a seek or the ragged ends of a range need a handful of records per round, and one launch instead of three per
+// round, with an exit as soon as a round leaves nothing, is what their latency is made of.  P.gl_cur = the filled list,
+// P.gl_nxt = the other one; round_tickets = one zeroed counter per round.
+__global__ void __launch_bounds__(1024, 1) k_rounds(const Params P, unsigned long long* round_tickets, uint32_t rounds) {
+    extern __shared__ __align__(16) uint8_t smem_raw[];
+    cooperative_groups::grid_group grid = cooperative_groups::this_grid();
+    const CtaSmem m = setup_cta(P, smem_raw);
+    BlockCtx c;
+    bind_scratch(P, blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), c);
+    for (uint32_t r = 0;; r++) {
+        const GList& cur = (r & 1) ? P.gl_nxt : P.gl_cur;
+        const GList& nxt = (r & 1) ? P.gl_cur : P.gl_nxt;
+        const uint32_t n_rec = *reinterpret_cast<volatile uint32_t*>(cur.count);
+        if (n_rec == 0) break;                                // uniform over the grid: read after a grid-wide barrier
+        if (r == rounds) { if (blockIdx.x == 0 && threadIdx.x == 0) report(P, DF_STACK); break; }
+        if (blockIdx.x == 0) {
+            if (threadIdx.x < 4) nxt.count[threadIdx.x] = 0;
+            plan_body(cur);
         }
+        __threadfence();
+        grid.sync();
+        scatter_body(P, cur, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
+        __threadfence();
+        grid.sync();
+        serve_body(P, m, c, cur, nxt, round_tickets + r);
+        __threadfence();
+        grid.sync();
     }
 }
 
@@ -1173,6 +1223,7 @@ struct aceapex_archive {
     uint8_t* d_ws = nullptr; uint64_t ws_bytes = 0; bool ws_clean = false;
     cudaStream_t stream = nullptr;
     uint32_t epoch = 0;
+    bool cooperative = false;                          // k_rounds can be launched cooperatively (all CTAs resident)
     uint32_t ticket_slot = 0;                          // which of the two ticket slots the next launch draws from
     Resident res[MAX_RESIDENT];
     // launch geometry
@@ -1454,11 +1505,17 @@ int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* 
         const void* fns[] = {(const void*)k_decode<false>, (const void*)k_decode<true>, (const void*)k_literals<1024>,
                              (const void*)k_matches<false, 1024>, (const void*)k_matches<true, 1024>, (const void*)k_matches<false, 1024, true, true>,
                              (const void*)k_matches<false, 1024, true, false>, (const void*)k_serve, (const void*)k_copy<false>,
-                             (const void*)k_copy<true>};
+                             (const void*)k_copy<true>, (const void*)k_rounds};
         for (const void* f : fns) {
             CU(cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max(std::max(ar->smem, smem_matches(ar, ar->threads)), (size_t)(ar->threads / 32) * COPY_WARP_BYTES + 64)));
             CU(cudaFuncSetAttribute(f, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
         }
+    }
+    {
+        int coop = 0, occ_r = 0;
+        CU(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_r, k_rounds, ar->threads, ar->smem));
+        ar->cooperative = coop && occ_r >= 1 && !getenv("ACEAPEX_NO_COOPERATIVE");
     }
     int occ = 0;
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_decode<true>, ar->threads, ar->smem));
@@ -1610,9 +1667,19 @@ static void add_demands(aceapex_archive* ar, uint64_t pos, uint64_t len, uint64_
     }
 }
 
-// Serves the demand list g[0] (filled by the caller) in `rounds` rounds; the list left by the last round must be empty.
+// Serves the demand list g[0] (filled by the caller) in at most `rounds` rounds; the list left by the last round must be
+// empty.  One cooperative launch (k_rounds) where the device supports it, else three launches per round.
 static int32_t serve_rounds(aceapex_archive* ar, Params Q, const GList g[2], uint32_t rounds) {
     Q.mode = 7;
+    if (ar->cooperative && rounds <= 16) {
+        unsigned long long* tickets = reinterpret_cast<unsigned long long*>(ar->d_ws + 128);     // 16 counters in the control area
+        CU(cudaMemsetAsync(tickets, 0, 128, ar->stream));
+        Q.gl_cur = g[0]; Q.gl_nxt = g[1];
+        void* args[] = {&Q, &tickets, &rounds};
+        CU(cudaLaunchCooperativeKernel((const void*)k_rounds, dim3(ar->sms), dim3(ar->threads), args, ar->smem, ar->stream));
+        ar->launches++;
+        return ACEAPEX_OK;
+    }
     for (uint32_t r = 0; r < rounds; r++) {
         Q.gl_cur = g[r & 1]; Q.gl_nxt = g[(r + 1) & 1];
         CU(cudaMemsetAsync(Q.gl_nxt.count, 0, 16, ar->stream));
