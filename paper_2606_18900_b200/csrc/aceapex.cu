@@ -304,6 +304,7 @@ __device__ __forceinline__ void wait_sources(const Params& P, const BlockCtx& c,
     uint64_t seed_end = min((unsigned long long)(src + len), (unsigned long long)dst);
     uint64_t s0 = src >> P.log2_bs, s1 = (seed_end - 1) >> P.log2_bs;
     for (uint64_t S = s0; S <= s1; S++) if (S != c.b) {
+        if ((S << P.log2_bs) < P.out_pos0 || (S << P.log2_bs) >= P.win_end) continue;   // outside the window: final already
         bool full = __ldg(P.levels + S) < c.d.level;
         if (full || LIT_WAITS) wait_block(P, S, full);
     }
@@ -1350,7 +1351,7 @@ int32_t launch(aceapex_archive* ar, Params& P, uint64_t n_work) {
     uint64_t warps = ar->threads / 32;
     uint32_t grid = (uint32_t)std::min<uint64_t>(ar->grid, (n_work + warps - 1) / warps);
     const bool whole = P.out_pos0 == 0 && P.win_end == ar->N;
-    if (P.mode >= 8) {                                        // whole-file match resolution from descriptors
+    if (P.mode == 8 || P.mode == 9) {                         // whole-file match resolution from descriptors
         const int T = ar->threads;
         uint64_t w = T / 32;
         uint32_t g = (uint32_t)std::min<uint64_t>(ar->sms, (n_work + w - 1) / w);
@@ -1363,6 +1364,7 @@ int32_t launch(aceapex_archive* ar, Params& P, uint64_t n_work) {
         uint32_t g = (uint32_t)std::min<uint64_t>(ar->sms, (n_work + w - 1) / w);
         if (P.mode == 5) k_matches<false, 1024, true, true><<<g, T, smem_matches(ar, T), ar->stream>>>(P);
         else if (P.mode == 6) k_matches<false, 1024, true, false><<<g, T, smem_matches(ar, T), ar->stream>>>(P);
+        else if (P.mode == 10) k_matches<true, 1024, true, false><<<g, T, smem_matches(ar, T), ar->stream>>>(P);
         else k_serve<<<ar->sms, T, ar->smem, ar->stream>>>(P);
     }
     else if ((whole || P.mode == 2) && P.mode >= 2) {         // specialised whole-file kernels (the literal launch also serves windows)
@@ -1504,7 +1506,7 @@ int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* 
     {
         const void* fns[] = {(const void*)k_decode<false>, (const void*)k_decode<true>, (const void*)k_literals<1024>,
                              (const void*)k_matches<false, 1024>, (const void*)k_matches<true, 1024>, (const void*)k_matches<false, 1024, true, true>,
-                             (const void*)k_matches<false, 1024, true, false>, (const void*)k_serve, (const void*)k_copy<false>,
+                             (const void*)k_matches<false, 1024, true, false>, (const void*)k_matches<true, 1024, true, false>, (const void*)k_serve, (const void*)k_copy<false>,
                              (const void*)k_copy<true>, (const void*)k_rounds};
         for (const void* f : fns) {
             CU(cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max(std::max(ar->smem, smem_matches(ar, ar->threads)), (size_t)(ar->threads / 32) * COPY_WARP_BYTES + 64)));
@@ -1751,11 +1753,10 @@ int32_t aceapex_decode_range(aceapex_archive* ar, uint64_t lo, uint64_t hi, void
                 if ((rc = serve_rounds(ar, Q, g, ar->max_level + 2))) return rc;
                 s0 = s1;
             }
-            for (uint32_t l = 0; l <= ar->max_level; l++) {     // cnt[l] = end of level l in the sorted list
-                uint64_t l0 = l ? cnt[l - 1] : 0, l1 = cnt[l];
-                P.mode = 6; P.level_list = d_list + l0; P.first_block = 0;
-                if ((rc = launch(ar, P, l1 - l0))) return rc;
-            }
+            // matches of the window: its blocks sorted by (level, index) in one flag-driven launch (a block waits for
+            // lower-level source blocks of the window only; everything outside the window is final)
+            P.mode = 10; P.level_list = d_list; P.first_block = 0; P.epoch = ++ar->epoch;
+            if ((rc = launch(ar, P, nb))) return rc;
         }
     }
     // the ragged ends: spans that enter the demand lists as top-level records; the finished window is a plain source
