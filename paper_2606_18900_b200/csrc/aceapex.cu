@@ -1127,7 +1127,10 @@ __global__ void __launch_bounds__(1024, 1) k_rounds(const Params P, unsigned lon
 // top-level spans of a range decode (its ragged ends) enter the demand lists like any other record
 __global__ void k_seed(const Params P, uint32_t n) {
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) gl_append(P, P.gl_nxt, P.demands[i].pos, (uint32_t)P.demands[i].len, P.demands[i].dst);
+    if (i < n) {
+        const Demand d = P.n_inline ? P.inline_dem[i] : P.demands[i];
+        gl_append(P, P.gl_nxt, d.pos, (uint32_t)d.len, d.dst);
+    }
 }
 
 __global__ void k_assert_empty(const uint32_t* count, uint32_t* err) { if (*count) atomicOr(err, (uint32_t)DF_STACK); }
@@ -1813,7 +1816,30 @@ int32_t aceapex_decode_reads(aceapex_archive* ar, const uint64_t* idx, uint64_t 
     }
     Params P; fill_params(ar, P);
     P.out = static_cast<uint8_t*>(d_out); P.out2 = P.out; P.out_pos0 = 0; P.win_end = 0;
-    if ((rc = run_demands(ar, P))) return rc;
+    static const int force_rounds = getenv("ACEAPEX_READS_ROUNDS") ? atoi(getenv("ACEAPEX_READS_ROUNDS")) : -1;
+    // Medium batches go through the demand lists as top-level records: their blocks, then the source blocks of every
+    // round, are parsed in parallel by different warps.  A single read is served faster by one warp that recurses on its
+    // sources itself (one launch); a batch that fills the machine gains nothing from the extra passes.
+    const bool by_rounds = ar->cooperative && (force_rounds >= 0 ? force_rounds != 0 : (n >= 2 && n <= 1024));
+    if (by_rounds) {
+        const GList g[2] = {glist(ar, 0), glist(ar, 1)};
+        Demand* d_dem = reinterpret_cast<Demand*>(ar->d_ws + ar->demands_off);
+        ar->gl_eff = ar->gl_cap;
+        const size_t chunk = std::max<size_t>(1, std::min<size_t>(ar->demand_cap, ar->gl_cap / 8));
+        for (size_t i = 0; i < ar->h_demands.size(); i += chunk) {
+            const uint32_t m = (uint32_t)std::min<size_t>(chunk, ar->h_demands.size() - i);
+            CU(cudaMemsetAsync(g[0].count, 0, 32, ar->stream));
+            Params Q = P;
+            Q.gl_nxt = g[0]; Q.demands = d_dem; Q.n_inline = 0;
+            if (m <= 4) { Q.n_inline = m; for (uint32_t k = 0; k < m; k++) Q.inline_dem[k] = ar->h_demands[i + k]; }
+            else CU(cudaMemcpyAsync(d_dem, ar->h_demands.data() + i, m * sizeof(Demand), cudaMemcpyHostToDevice, ar->stream));
+            k_seed<<<(m + 127) / 128, 128, 0, ar->stream>>>(Q, m);
+            CU(cudaGetLastError());
+            ar->launches++;
+            if ((rc = serve_rounds(ar, Q, g, ar->max_level + 3))) return rc;
+            if (i + chunk < ar->h_demands.size()) CU(cudaStreamSynchronize(ar->stream));   // the staging area is reused
+        }
+    } else if ((rc = run_demands(ar, P))) return rc;
     CU(cudaStreamSynchronize(ar->stream));           // h_demands is host staging; the call returns the reads
     return ACEAPEX_OK;
 }
