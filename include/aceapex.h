@@ -17,6 +17,9 @@
  *   - The library allocates small device state at open (tables, directory copy is NOT made: it reads the caller's
  *     archive buffer) and never allocates on the hot path: scratch comes from aceapex_set_workspace().
  *   - One handle must not be used from two host threads at once.
+ *   - Environment switches, read at open / first use, for tests and measurements only: ACEAPEX_NO_COOPERATIVE (demand rounds as
+ *     three launches per round instead of one cooperative launch), ACEAPEX_READS_ROUNDS=0|1 (force one of the two read paths),
+ *     ACEAPEX_CTAS_PER_SM (cap on resident CTAs of the generic kernel).
  */
 #ifndef ACEAPEX_H
 #define ACEAPEX_H
