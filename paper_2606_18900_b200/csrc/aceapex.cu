@@ -861,36 +861,54 @@ __global__ void __launch_bounds__(1024, 1) k_copy(const Params P) {
         uint32_t g0 = 0, pending = 0, mis = 0, len = 0, dst_rel = 0;
         uint64_t sp = 0;
         bool done = n == 0;
-        // (dst_rel, len) from k_literals, the offset from its decoded coded planes and the raw planes of the payload
-        auto load_desc = [&](uint32_t j) -> uint4 {
-            if (j >= n) return make_uint4(0, 0, 0, 0);
-            const uint2 pr = __ldcg(prs + j);
+        // (dst_rel, len) from k_literals, the offset bytes from its decoded coded planes and the raw planes of the payload.
+        // The loads of a group are issued one group ahead and their values stay untouched in registers until the group is
+        // staged (any arithmetic on them here would wait for the loads): v[i] = byte of the i-th plane in load order
+        // (coded planes in decode order, then raw planes) for W <= 4, else the assembled 64-bit offset in v[0], v[1].
+        auto load_desc = [&](uint32_t j, uint2& pr, uint32_t (&v)[4]) {
+            pr = make_uint2(0, 0); v[0] = v[1] = v[2] = v[3] = 0;
+            if (j >= n) return;
+            pr = __ldcg(prs + j);
             const uint8_t* cq = cpl + j; const uint8_t* rq = raw + j;
-            if (P.W <= 4) {                                   // files up to 4 GiB: 32-bit arithmetic
-                uint32_t s32 = 0;
-                for (uint32_t k = 0; k < P.n_coded_planes; k++, cq += n) s32 |= (uint32_t)__ldcg(cq) << P.coded_shift[k];
-                for (uint32_t r = 0; r < P.n_raw_planes; r++, rq += n) s32 |= (uint32_t)__ldg(rq) << P.raw_shift[r];
-                return make_uint4(s32, 0, pr.x, pr.y);
+            if (P.W <= 4) {                                   // files up to 4 GiB
+#pragma unroll
+                for (uint32_t i = 0; i < 4; i++) {
+                    if (i < P.n_coded_planes) v[i] = __ldcg(cq + (uint64_t)i * n);
+                    else if (i < P.W) v[i] = __ldg(rq + (uint64_t)(i - P.n_coded_planes) * n);
+                }
+                return;
             }
             uint64_t src = 0;
             for (uint32_t k = 0; k < P.n_coded_planes; k++, cq += n) src |= (uint64_t)__ldcg(cq) << P.coded_shift[k];
             for (uint32_t r = 0; r < P.n_raw_planes; r++, rq += n) src |= (uint64_t)__ldg(rq) << P.raw_shift[r];
-            return make_uint4((uint32_t)src, (uint32_t)(src >> 32), pr.x, pr.y);
+            v[0] = (uint32_t)src; v[1] = (uint32_t)(src >> 32);
         };
-        uint4 nd = load_desc(lane);                           // descriptors are loaded one group ahead
+        auto desc_src = [&](const uint32_t (&v)[4]) -> uint64_t {
+            if (P.W > 4) return (uint64_t)v[1] << 32 | v[0];
+            uint32_t s32 = 0;
+#pragma unroll
+            for (uint32_t i = 0; i < 4; i++)
+                s32 |= v[i] << (i < P.n_coded_planes ? P.coded_shift[i] : P.raw_shift[(i - P.n_coded_planes) & (MAX_W - 1)]);
+            return s32;
+        };
+        // The descriptors of a group are requested when the last staging round of the group before it has been issued (no
+        // value of that group is live any more, so the loads land in the same registers) and travel while the round
+        // before that is copied out.
+        uint2 npr; uint32_t nv[4];
+        bool have = false;
         // one staging round into buffer `buf`: returns the number of staged matches; commits exactly one cp.async group
-        auto issue = [&](uint32_t buf) -> uint32_t {
+        auto issue = [&](uint32_t buf, uint32_t& more) -> uint32_t {
             const uint32_t mtab = sbase + buf * (MTAB_BYTES + 16 * STAGE_CHUNKS), stage = mtab + MTAB_BYTES;
             for (;;) {
                 if (pending == 0) {
-                    if (g0 >= n) { done = true; cp_async_commit(); return 0; }
-                    const uint4 d = nd;
+                    if (g0 >= n) { done = true; more = 0; cp_async_commit(); return 0; }
+                    if (!have) load_desc(g0 + lane, npr, nv);            // head of a block, or a group that staged nothing
+                    have = false;
+                    const uint64_t src = desc_src(nv), dst = bstart + npr.x;
+                    dst_rel = npr.x; len = npr.y;
                     const bool has = g0 + lane < n;
                     g0 += 32;
-                    nd = load_desc(g0 + lane);
-                    const uint64_t src = (uint64_t)d.y << 32 | d.x, dst = bstart + d.z;
-                    dst_rel = d.z; len = d.w;
-                    const bool good = has && src < dst && d.z + d.w <= blen && d.w != 0;
+                    const bool good = has && src < dst && dst_rel + len <= blen && len != 0;
                     if (has && !good) report(P, src < dst ? DF_LENGTH : DF_OFFSET);
                     const bool ovl = good && src + len > dst;
                     if (ovl && src < bstart) report(P, DF_OFFSET);       // FORMAT.md §3 (c)
@@ -929,55 +947,56 @@ __global__ void __launch_bounds__(1024, 1) k_copy(const Params P) {
                 for (int o = 1; o < 32; o <<= 1) { uint32_t a = __shfl_up_sync(0xffffffffu, ce, o); if (lane >= (uint32_t)o) ce += a; }
                 const bool fits = mine && ce <= STAGE_CHUNKS;
                 const uint32_t fmask = __ballot_sync(0xffffffffu, fits);
+                const uint32_t ent = __popc(fmask & lanemask_lt());
+                more = __reduce_or_sync(0xffffffffu, fits && len > 64 ? 1u << ent : 0u);   // entries that need more than two passes
                 if (fits) {
                     const uint32_t so = 16u * (ce - need);
                     const uint8_t* g = reinterpret_cast<const uint8_t*>(sp - mis);
                     for (uint32_t q = 0; q < need; q++) cp_async16s(stage + so + 16 * q, g + 16 * q);
                     const uint64_t dp = reinterpret_cast<uint64_t>(out_blk) + dst_rel;
-                    sts128(mtab + 16 * __popc(fmask & lanemask_lt()), (uint32_t)dp, (uint32_t)(dp >> 32) | (len << 24), stage + so + mis, 0);
+                    sts128(mtab + 16 * ent, (uint32_t)dp, (uint32_t)(dp >> 32), stage + so + mis, len);
                 }
                 const uint32_t n_ent = __popc(fmask);
                 if (lane == 0) sts128(mtab + 16 * n_ent, 0, 0, 0, 0);   // empty entry: matches are taken two at a time
                 cp_async_commit();
                 pending &= ~fmask;
+                if (pending == 0 && g0 < n) { load_desc(g0 + lane, npr, nv); have = true; }
                 return n_ent;
             }
         };
-        auto copy_out = [&](uint32_t buf, uint32_t n_ent) {
+        auto copy_out = [&](uint32_t buf, uint32_t n_ent, uint32_t more) {
             const uint32_t mtab = sbase + buf * (MTAB_BYTES + 16 * STAGE_CHUNKS);
-            uint32_t more = 0;
             for (uint32_t k = 0; k < n_ent; k += 2) {
                 const uint4 e0 = lds128(mtab + 16 * k), e1 = lds128(mtab + 16 * k + 16);
-                const uint32_t l0 = e0.y >> 24, l1 = e1.y >> 24;
+                const uint32_t l0 = e0.w, l1 = e1.w;
                 const uint32_t a0 = e0.z + lane, a1 = e1.z + lane;
                 const uint32_t v00 = lds8(a0), v01 = lds8(a0 + 32), v10 = lds8(a1), v11 = lds8(a1 + 32);
-                uint8_t* d0 = reinterpret_cast<uint8_t*>((uint64_t)(e0.y & 0xffffffu) << 32 | e0.x) + lane;
-                uint8_t* d1 = reinterpret_cast<uint8_t*>((uint64_t)(e1.y & 0xffffffu) << 32 | e1.x) + lane;
+                uint8_t* d0 = reinterpret_cast<uint8_t*>((uint64_t)e0.y << 32 | e0.x) + lane;
+                uint8_t* d1 = reinterpret_cast<uint8_t*>((uint64_t)e1.y << 32 | e1.x) + lane;
                 if (lane < l0) d0[0] = (uint8_t)v00;
                 if (lane + 32 < l0) d0[32] = (uint8_t)v01;
                 if (lane < l1) d1[0] = (uint8_t)v10;
                 if (lane + 32 < l1) d1[32] = (uint8_t)v11;
-                more |= (l0 > 64 ? 1u : 0u) << k | (l1 > 64 ? 2u : 0u) << k;
             }
             while (more) {                                   // bytes 64.. of the longer ones (about one match in nine on FASTQ)
                 const int k = __ffs(more) - 1; more &= more - 1;
                 const uint4 e = lds128(mtab + 16 * k);
-                const uint32_t ln = e.y >> 24, sa = e.z + lane;
-                uint8_t* dp = reinterpret_cast<uint8_t*>((uint64_t)(e.y & 0xffffffu) << 32 | e.x) + lane;
+                const uint32_t ln = e.w, sa = e.z + lane;
+                uint8_t* dp = reinterpret_cast<uint8_t*>((uint64_t)e.y << 32 | e.x) + lane;
                 for (uint32_t o = 64; o + lane < ln; o += 32) dp[o] = (uint8_t)lds8(sa + o);
             }
         };
         if (!done) {
-            uint32_t cur = 0, n_cur = issue(0);
+            uint32_t cur = 0, more_cur = 0, n_cur = issue(0, more_cur);
             for (;;) {
-                uint32_t n_nxt = 0;
-                if (done) cp_async_commit(); else n_nxt = issue(cur ^ 1);
+                uint32_t n_nxt = 0, more_nxt = 0;
+                if (done) cp_async_commit(); else n_nxt = issue(cur ^ 1, more_nxt);
                 cp_async_wait_group<1>();                    // everything but the round just issued has landed
                 __syncwarp();
-                copy_out(cur, n_cur);
+                copy_out(cur, n_cur, more_cur);
                 __syncwarp();                                // this buffer is refilled by the next round
                 if (done && n_nxt == 0) break;
-                n_cur = n_nxt; cur ^= 1;
+                n_cur = n_nxt; more_cur = more_nxt; cur ^= 1;
             }
             cp_async_wait_group<0>();
         }
