@@ -1364,6 +1364,14 @@ int32_t prepare_ws(aceapex_archive* ar) {
     return ACEAPEX_OK;
 }
 
+// Few work items: spread them over all SMs with fewer warps per CTA instead of filling a few CTAs with 32 warps each (a
+// warp that shares its SM with fewer others finishes its block sooner).  T <= max_threads, g <= SMs (all CTAs resident).
+static void spread(const aceapex_archive* ar, uint64_t n_work, int max_threads, uint32_t& g, int& T) {
+    const uint64_t per_sm = (n_work + ar->sms - 1) / ar->sms;
+    T = (int)std::min<uint64_t>((uint64_t)max_threads, 32 * std::max<uint64_t>(per_sm, 1));
+    g = (uint32_t)std::min<uint64_t>(ar->sms, (n_work + T / 32 - 1) / (T / 32));
+}
+
 int32_t launch(aceapex_archive* ar, Params& P, uint64_t n_work) {
     P.n_work = n_work;
     if (n_work == 0) return ACEAPEX_OK;
@@ -1374,26 +1382,23 @@ int32_t launch(aceapex_archive* ar, Params& P, uint64_t n_work) {
     uint32_t grid = (uint32_t)std::min<uint64_t>(ar->grid, (n_work + warps - 1) / warps);
     const bool whole = P.out_pos0 == 0 && P.win_end == ar->N;
     if (P.mode == 8 || P.mode == 9) {                         // whole-file match resolution from descriptors
-        const int T = ar->threads;
-        uint64_t w = T / 32;
-        uint32_t g = (uint32_t)std::min<uint64_t>(ar->sms, (n_work + w - 1) / w);
+        int T; uint32_t g;
+        spread(ar, n_work, ar->threads, g, T);
         const size_t sm = (size_t)(T / 32) * COPY_WARP_BYTES + 64;
         if (P.mode == 8) k_copy<false><<<g, T, sm, ar->stream>>>(P); else k_copy<true><<<g, T, sm, ar->stream>>>(P);
     }
     else if (P.mode >= 5) {                                        // range decode: collect / window matches / serve
-        const int T = ar->threads;
-        uint64_t w = T / 32;
-        uint32_t g = (uint32_t)std::min<uint64_t>(ar->sms, (n_work + w - 1) / w);
+        int T = ar->threads; uint32_t g = ar->sms;
+        if (P.mode != 7) spread(ar, n_work, ar->threads, g, T);
         if (P.mode == 5) k_matches<false, 1024, true, true><<<g, T, smem_matches(ar, T), ar->stream>>>(P);
         else if (P.mode == 6) k_matches<false, 1024, true, false><<<g, T, smem_matches(ar, T), ar->stream>>>(P);
         else if (P.mode == 10) k_matches<true, 1024, true, false><<<g, T, smem_matches(ar, T), ar->stream>>>(P);
         else k_serve<<<ar->sms, T, ar->smem, ar->stream>>>(P);
     }
     else if ((whole || P.mode == 2) && P.mode >= 2) {         // specialised whole-file kernels (the literal launch also serves windows)
-        const int T = P.mode == 2 ? ar->threads_lit : ar->threads_match;
+        int T; uint32_t g;
+        spread(ar, n_work, P.mode == 2 ? ar->threads_lit : ar->threads_match, g, T);
         const size_t sm = P.mode == 2 ? smem_for(ar, T) : smem_matches(ar, T);
-        uint64_t w = T / 32;
-        uint32_t g = (uint32_t)std::min<uint64_t>(ar->sms, (n_work + w - 1) / w);
         if (P.mode == 2) k_literals<1024><<<g, T, sm, ar->stream>>>(P);
         else if (P.mode == 3) k_matches<false, 1024><<<g, T, sm, ar->stream>>>(P);
         else k_matches<true, 1024><<<g, T, sm, ar->stream>>>(P);
