@@ -22,7 +22,8 @@ def _run(cmd, log=None):
     r = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
     if log:
         with open(log, "w") as f:
-            f.write(" ".join(cmd) + "\n" + r.stdout)
+            # without the "Compile time" lines the log is the same for the same source
+            f.write(" ".join(cmd) + "\n" + "".join(ln for ln in r.stdout.splitlines(True) if "Compile time" not in ln))
     if r.returncode != 0:
         raise RuntimeError("build failed: %s\n%s" % (" ".join(cmd), r.stdout))
     return r.stdout
