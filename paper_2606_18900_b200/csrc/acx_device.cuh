@@ -126,15 +126,14 @@ struct Rans {
     uint32_t ring;           // shared address of this lane's ring, 64-byte aligned
     uint32_t end;            // rp after the lane's last word (integrity check)
     const uint8_t* gbase;    // 16-byte aligned global address that offsets are relative to
-    const uint8_t* limit;    // archive end (loads are clamped)
+    uint32_t lim;            // archive end relative to gbase, saturated (loads are clamped)
 
     __device__ __forceinline__ void fetch() {
-        const uint8_t* g = gbase + fp;
-        if (g + 16 <= limit) cp_async16s(ring | (fp & 63), g);
+        if (fp + 16 <= lim) cp_async16s(ring | (fp & 63), gbase + fp);
         fp += 16;
     }
     // payload: [32 x (u32 state, u32 word_off)][words]; n_words = total words of the block
-    __device__ __forceinline__ void init(const uint8_t* payload, uint32_t n_words, const uint8_t* lim, uint32_t ring_warp) {
+    __device__ __forceinline__ void init(const uint8_t* payload, uint32_t n_words, const uint8_t* lim_end, uint32_t ring_warp) {
         const uint32_t lane = lane_id();
         uint2 h = __ldg(reinterpret_cast<const uint2*>(payload) + lane);
         x = h.x;
@@ -148,7 +147,7 @@ struct Rans {
         end = rp + 2u * (next - h.y);
         fp = bias;
         ring = ring_warp + 64u * lane;
-        limit = lim;
+        this->lim = (uint32_t)min((unsigned long long)(lim_end - gbase), 0xfffffff0ull);
         cp_async_wait_group<0>();            // chunks still in flight from the previous block must not land after ours
         fetch(); cp_async_commit(); fetch(); cp_async_commit(); fetch(); cp_async_commit(); fetch(); cp_async_commit();
     }
