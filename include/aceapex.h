@@ -19,7 +19,8 @@
  *   - One handle must not be used from two host threads at once.
  *   - Environment switches, read at open / first use, for tests and measurements only: ACEAPEX_NO_COOPERATIVE (demand rounds as
  *     three launches per round instead of one cooperative launch), ACEAPEX_READS_ROUNDS=0|1 (force one of the two read paths),
- *     ACEAPEX_CTAS_PER_SM (cap on resident CTAs of the generic kernel).
+ *     ACEAPEX_CTAS_PER_SM (cap on resident CTAs of the generic kernel), ACEAPEX_WIN_TOKENS=1 (the collect and match launches of
+ *     a range-decode window re-decode the block's tokens instead of reading the descriptors its literal launch left).
  */
 #ifndef ACEAPEX_H
 #define ACEAPEX_H

@@ -837,7 +837,8 @@ __global__ void __launch_bounds__(MAXT, 1) k_matches(const Params P) {
 constexpr uint32_t COPY_WARP_BYTES = 2 * (MTAB_BYTES + 16 * STAGE_CHUNKS);
 static_assert(COPY_WARP_BYTES % 16 == 0, "tables and stages are 16-byte aligned");
 
-template <bool WAIT>
+// WIN / COLLECT: the windows of a range decode (sources looked up in the window and the resident slots; see emit_matches).
+template <bool WAIT, bool WIN = false, bool COLLECT = false>
 __global__ void __launch_bounds__(1024, 1) k_copy(const Params P) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
     clear_next_ticket(P);
@@ -912,23 +913,45 @@ __global__ void __launch_bounds__(1024, 1) k_copy(const Params P) {
                     if (has && !good) report(P, src < dst ? DF_LENGTH : DF_OFFSET);
                     const bool ovl = good && src + len > dst;
                     if (ovl && src < bstart) report(P, DF_OFFSET);       // FORMAT.md §3 (c)
-                    if (WAIT && good && lvl) {                            // completion of lower-level source blocks
-                        const uint64_t s1 = (min((unsigned long long)(src + len), (unsigned long long)dst) - 1) >> P.log2_bs;
-                        for (uint64_t S = src >> P.log2_bs; S <= s1; S++) if (S != b && __ldg(P.levels + S) < lvl) wait_block(P, S, true);
+                    const uint32_t seed_len = ovl ? (uint32_t)(dst - src) : len;   // source bytes that are not the match's own output
+                    const uint8_t* sbase = P.out + (src - P.out_pos0);
+                    const uint8_t* send = out_end;
+                    if (WIN || COLLECT) sbase = good ? resolve_src(P, src, seed_len, &send) : nullptr;
+                    if (COLLECT) {                                        // unknown seed bytes -> demand lists; nothing is copied
+                        if (g0 < n) { load_desc(g0 + lane, npr, nv); have = true; }
+                        if (good && !sbase) {
+                            const Stack sk{nullptr, 0, 0, &P.gl_nxt, SKIP_KNOWN};
+                            fetch_source<false>(P, BlockCtx{}, sk, src, seed_len, dst - P.out_pos0);
+                        }
+                        continue;
                     }
-                    sp = reinterpret_cast<uint64_t>(P.out) + (src - P.out_pos0);
+                    if (WAIT && good && lvl) {                            // completion of lower-level source blocks (of the window)
+                        const uint64_t s1 = (min((unsigned long long)(src + len), (unsigned long long)dst) - 1) >> P.log2_bs;
+                        for (uint64_t S = src >> P.log2_bs; S <= s1; S++) {
+                            if (WIN && ((S << P.log2_bs) < P.out_pos0 || (S << P.log2_bs) >= P.win_end)) continue;   // final already
+                            if (S != b && __ldg(P.levels + S) < lvl) wait_block(P, S, true);
+                        }
+                    }
+                    const bool known = good && sbase != nullptr;
+                    if (WIN && good && !sbase) {                          // seed spread over several buffers or (partly) delivered by the demand rounds
+                        const Stack sk{nullptr, 0, 0, nullptr, SKIP_UNKNOWN};
+                        fetch_source<false>(P, BlockCtx{}, sk, src, seed_len, dst - P.out_pos0);   // the known pieces of the seed
+                        uint8_t* d = P.out + (dst - P.out_pos0);
+                        for (uint32_t i = seed_len; i < len; i++) d[i] = d[i - seed_len];          // the rest repeats it (FORMAT.md §2)
+                    }
+                    sp = reinterpret_cast<uint64_t>(sbase);
                     mis = (uint32_t)sp & 15u;
-                    const bool lng = good && !ovl && len >= LONG_MATCH;
-                    const bool sht = good && !ovl && !lng;
-                    // a chunk may not reach past the end of the output buffer (only possible for sources in its last 16 bytes)
-                    const bool stg = sht && ((sp - mis) + 16ull * ((mis + len + 15u) >> 4) <= reinterpret_cast<uint64_t>(out_end));
+                    const bool lng = known && !ovl && len >= LONG_MATCH;
+                    const bool sht = known && !ovl && !lng;
+                    // a chunk may not reach past the end of the buffer (only possible for sources in its last 16 bytes)
+                    const bool stg = sht && ((sp - mis) + 16ull * ((mis + len + 15u) >> 4) <= reinterpret_cast<uint64_t>(send));
                     uint32_t longs = __ballot_sync(0xffffffffu, lng);
                     while (longs) {
                         const int l = __ffs(longs) - 1; longs &= longs - 1;
                         const uint32_t d2 = __shfl_sync(0xffffffffu, dst_rel, l), m = __shfl_sync(0xffffffffu, len, l);
                         warp_copy<true>(out_blk + d2, reinterpret_cast<const uint8_t*>(__shfl_sync(0xffffffffu, sp, l)), m);
                     }
-                    uint32_t direct = __ballot_sync(0xffffffffu, (sht && !stg) || ovl);
+                    uint32_t direct = __ballot_sync(0xffffffffu, (sht && !stg) || (known && ovl));
                     while (direct) {                                     // byte i of the match = seed[i mod period] (FORMAT.md §2)
                         const int l = __ffs(direct) - 1; direct &= direct - 1;
                         const uint32_t d2 = __shfl_sync(0xffffffffu, dst_rel, l), m = __shfl_sync(0xffffffffu, len, l);
@@ -1251,6 +1274,7 @@ struct aceapex_archive {
     Resident res[MAX_RESIDENT];
     // launch geometry
     int sms = 148, ctas_per_sm = 1, threads = 1024, threads_lit = 1024, threads_match = 1024;
+    bool win_tokens = false;                             // ACEAPEX_WIN_TOKENS=1: windows re-decode the tokens (k_matches) instead of reading descriptors
     uint32_t grid = 0; size_t smem = 0;
     uint64_t scratch_per_warp = 0, ctrl_bytes = 0, flags_bytes = 0;
     uint64_t scratch_off = 0, stacks_off = 0, demands_off = 0, list_off = 0, ws_need = 0;
@@ -1381,11 +1405,14 @@ int32_t launch(aceapex_archive* ar, Params& P, uint64_t n_work) {
     uint64_t warps = ar->threads / 32;
     uint32_t grid = (uint32_t)std::min<uint64_t>(ar->grid, (n_work + warps - 1) / warps);
     const bool whole = P.out_pos0 == 0 && P.win_end == ar->N;
-    if (P.mode == 8 || P.mode == 9) {                         // whole-file match resolution from descriptors
+    if (P.mode == 8 || P.mode == 9 || P.mode == 11 || P.mode == 12) {   // match resolution from descriptors (11 / 12: windows)
         int T; uint32_t g;
         spread(ar, n_work, ar->threads, g, T);
         const size_t sm = (size_t)(T / 32) * COPY_WARP_BYTES + 64;
-        if (P.mode == 8) k_copy<false><<<g, T, sm, ar->stream>>>(P); else k_copy<true><<<g, T, sm, ar->stream>>>(P);
+        if (P.mode == 8) k_copy<false><<<g, T, sm, ar->stream>>>(P);
+        else if (P.mode == 9) k_copy<true><<<g, T, sm, ar->stream>>>(P);
+        else if (P.mode == 11) k_copy<false, true, true><<<g, T, sm, ar->stream>>>(P);
+        else k_copy<true, true, false><<<g, T, sm, ar->stream>>>(P);
     }
     else if (P.mode >= 5) {                                        // range decode: collect / window matches / serve
         int T = ar->threads; uint32_t g = ar->sms;
@@ -1534,7 +1561,7 @@ int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* 
         const void* fns[] = {(const void*)k_decode<false>, (const void*)k_decode<true>, (const void*)k_literals<1024>,
                              (const void*)k_matches<false, 1024>, (const void*)k_matches<true, 1024>, (const void*)k_matches<false, 1024, true, true>,
                              (const void*)k_matches<false, 1024, true, false>, (const void*)k_matches<true, 1024, true, false>, (const void*)k_serve, (const void*)k_copy<false>,
-                             (const void*)k_copy<true>, (const void*)k_rounds};
+                             (const void*)k_copy<true>, (const void*)k_copy<false, true, true>, (const void*)k_copy<true, true, false>, (const void*)k_rounds};
         for (const void* f : fns) {
             CU(cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max(std::max(ar->smem, smem_matches(ar, ar->threads)), (size_t)(ar->threads / 32) * COPY_WARP_BYTES + 64)));
             CU(cudaFuncSetAttribute(f, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
@@ -1545,6 +1572,7 @@ int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* 
         CU(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
         CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_r, k_rounds, ar->threads, ar->smem));
         ar->cooperative = coop && occ_r >= 1 && !getenv("ACEAPEX_NO_COOPERATIVE");
+        ar->win_tokens = getenv("ACEAPEX_WIN_TOKENS") && atoi(getenv("ACEAPEX_WIN_TOKENS")) != 0;
     }
     int occ = 0;
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_decode<true>, ar->threads, ar->smem));
@@ -1765,6 +1793,8 @@ int32_t aceapex_decode_range(aceapex_archive* ar, uint64_t lo, uint64_t hi, void
         } else {
             // (1) literals of the window; (2) foreign seed bytes of its matches -> demand lists, served in rounds, every
             // source block parsed once per round; (3) matches of the window, one launch per dependency level
+            // the literal launch leaves (dst_rel, len) and the decoded offset planes of the window's matches for (2) and (3)
+            P.pairs = reinterpret_cast<uint2*>(ar->d_ws + ar->desc_off); P.cplanes = ar->d_ws + ar->cplanes_off;
             P.mode = 2; P.level_list = nullptr; P.first_block = b0;
             if ((rc = launch(ar, P, nb))) return rc;
             const GList g[2] = {glist(ar, 0), glist(ar, 1)};
@@ -1772,18 +1802,19 @@ int32_t aceapex_decode_range(aceapex_archive* ar, uint64_t lo, uint64_t hi, void
                 uint64_t s1 = s0 + 1;
                 while (s1 < b1 && ar->h_match_prefix[s1 + 1] - ar->h_match_prefix[s0] <= ar->gl_eff / 3) s1++;
                 CU(cudaMemsetAsync(g[0].count, 0, 32, ar->stream));
-                P.mode = 5; P.level_list = nullptr; P.first_block = s0; P.gl_nxt = g[0];
+                P.mode = ar->win_tokens ? 5 : 11; P.level_list = nullptr; P.first_block = s0; P.gl_nxt = g[0];
                 if ((rc = launch(ar, P, s1 - s0))) return rc;
                 Params Q = P;                                   // serving knows no window: sources of foreign bytes precede it
-                Q.out_pos0 = 0; Q.win_end = 0;
+                Q.out_pos0 = 0; Q.win_end = 0; Q.pairs = nullptr; Q.cplanes = nullptr;
                 // a seed byte is found after at most max_level + 1 source blocks (FORMAT.md §3): one round each
                 if ((rc = serve_rounds(ar, Q, g, ar->max_level + 2))) return rc;
                 s0 = s1;
             }
             // matches of the window: its blocks sorted by (level, index) in one flag-driven launch (a block waits for
             // lower-level source blocks of the window only; everything outside the window is final)
-            P.mode = 10; P.level_list = d_list; P.first_block = 0; P.epoch = ++ar->epoch;
+            P.mode = ar->win_tokens ? 10 : 12; P.level_list = d_list; P.first_block = 0; P.epoch = ++ar->epoch;
             if ((rc = launch(ar, P, nb))) return rc;
+            P.pairs = nullptr; P.cplanes = nullptr;
         }
     }
     // the ragged ends: spans that enter the demand lists as top-level records; the finished window is a plain source

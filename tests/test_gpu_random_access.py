@@ -188,6 +188,19 @@ def test_large_windows_with_foreign_sources(big):
             check_range(ar, x, lo, min(hi, N))
 
 
+def test_large_windows_token_path(monkeypatch):
+    """ACEAPEX_WIN_TOKENS=1 (read at open): the collect and match launches of a window re-decode the block's tokens
+    (k_matches) instead of reading the descriptors the literal launch left (k_copy); same bytes either way."""
+    from paper_2606_18900_b200 import datagen, encoder
+    from paper_2606_18900_b200.aceapex import Archive
+    monkeypatch.setenv("ACEAPEX_WIN_TOKENS", "1")
+    x = datagen.fastq(7, 6 << 20, 300_000)
+    ar = Archive(encoder.encode(x, block_size=16384))
+    for lo, hi in ((100 * 16384, 380 * 16384), (x.size - 300 * 16384 - 5, x.size), (0, 256 * 16384)):
+        check_range(ar, x, lo, hi)
+    ar.close()
+
+
 def test_large_windows_ring(big):
     """Consecutive 4 MiB windows through a two-slot ring: sources are found in the window, in the resident previous
     window, or are reconstructed through the demand lists."""
