@@ -1030,8 +1030,10 @@ __global__ void __launch_bounds__(1024, 1) k_copy(const Params P) {
     }
 }
 
-// Bucket offsets and work items of the list in P.gl_cur: one CTA scans the touched blocks (their record counts and their
-// numbers of work items) 1024 at a time; cnt[block] becomes the fill pointer of the block's bucket.
+// Bucket offsets and work items of the list in P.gl_cur: every warp of the launch takes 32 touched blocks at a time; the
+// bucket offsets and the work-item slots come from two global counters (count[3]: records placed, count[2]: work items),
+// one atomicAdd per warp each (the order of the buckets in the sorted array is irrelevant); cnt[block] becomes the fill
+// pointer of the block's bucket.  Both counters are zero when a list becomes the current one.
 // The list arrays are written by other CTAs, possibly earlier in the SAME launch (k_rounds): they are read at L2.
 __device__ __forceinline__ GDemand ld_demand(const GDemand* p) {
     const unsigned long long* q = reinterpret_cast<const unsigned long long*>(p);
@@ -1040,14 +1042,10 @@ __device__ __forceinline__ GDemand ld_demand(const GDemand* p) {
     return d;
 }
 
-__device__ __forceinline__ void plan_body(const GList& g) {      // one CTA (any multiple of 32 threads up to 1024)
-    __shared__ uint32_t s_rec[32], s_item[32], s_base[2];
-    const uint32_t n = min(__ldcg(g.count + 1), g.touched_cap), lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (threadIdx.x == 0) { s_base[0] = 0; s_base[1] = 0; }
-    __syncthreads();
-    const uint32_t n_warps = blockDim.x >> 5;
-    for (uint32_t t0 = 0; t0 < n; t0 += blockDim.x) {
-        const uint32_t t = t0 + threadIdx.x;
+__device__ __forceinline__ void plan_body(const GList& g, uint32_t warp_global, uint32_t n_warps_global) {
+    const uint32_t n = min(__ldcg(g.count + 1), g.touched_cap), lane = threadIdx.x & 31;
+    for (uint32_t t0 = 32 * warp_global; t0 < n; t0 += 32 * n_warps_global) {
+        const uint32_t t = t0 + lane;
         uint32_t blk = 0, c = 0;
         if (t < n) { blk = __ldcg(g.touched + t); c = __ldcg(g.cnt + blk); }
         uint32_t it = (c + GL_ITEM - 1) / GL_ITEM, ps = c, pi = it;      // inclusive warp scans of records and items
@@ -1056,19 +1054,10 @@ __device__ __forceinline__ void plan_body(const GList& g) {      // one CTA (any
             uint32_t a = __shfl_up_sync(0xffffffffu, ps, o), b2 = __shfl_up_sync(0xffffffffu, pi, o);
             if (lane >= (uint32_t)o) { ps += a; pi += b2; }
         }
-        if (lane == 31) { s_rec[warp] = ps; s_item[warp] = pi; }
-        __syncthreads();
-        if (warp == 0) {
-            uint32_t a = lane < n_warps ? s_rec[lane] : 0, b2 = lane < n_warps ? s_item[lane] : 0, sa = a, sb = b2;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                uint32_t x = __shfl_up_sync(0xffffffffu, sa, o), y = __shfl_up_sync(0xffffffffu, sb, o);
-                if (lane >= (uint32_t)o) { sa += x; sb += y; }
-            }
-            s_rec[lane] = sa - a; s_item[lane] = sb - b2;                 // exclusive offsets of the warps
-        }
-        __syncthreads();
-        const uint32_t r0 = s_base[0] + s_rec[warp] + ps - c, i0 = s_base[1] + s_item[warp] + pi - it;
+        uint32_t rb = 0, ib = 0;
+        if (lane == 31) { rb = atomicAdd(g.count + 3, ps); ib = atomicAdd(g.count + 2, pi); }
+        rb = __shfl_sync(0xffffffffu, rb, 31); ib = __shfl_sync(0xffffffffu, ib, 31);
+        const uint32_t r0 = rb + ps - c, i0 = ib + pi - it;
         if (t < n) {
             g.cnt[blk] = r0;
             for (uint32_t j = 0; j < it; j++) if (i0 + j < g.work_cap) {
@@ -1076,14 +1065,12 @@ __device__ __forceinline__ void plan_body(const GList& g) {      // one CTA (any
                 g.work_n[i0 + j] = min(GL_ITEM, c - j * GL_ITEM);
             }
         }
-        __syncthreads();
-        if (threadIdx.x == blockDim.x - 1) { s_base[0] = r0 + c; s_base[1] = i0 + it; }
-        __syncthreads();
     }
-    if (threadIdx.x == 0) g.count[2] = min(s_base[1], g.work_cap);
 }
 
-__global__ void __launch_bounds__(1024, 1) k_plan(const Params P) { plan_body(P.gl_cur); }
+__global__ void __launch_bounds__(1024, 1) k_plan(const Params P) {
+    plan_body(P.gl_cur, blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), gridDim.x * (blockDim.x >> 5));
+}
 
 __device__ __forceinline__ void scatter_body(const Params& P, const GList& g, uint32_t tid, uint32_t n_threads) {
     const uint32_t n = min(__ldcg(g.count), g.cap);
@@ -1151,10 +1138,8 @@ __global__ void __launch_bounds__(1024, 1) k_rounds(const Params P, unsigned lon
         const uint32_t n_rec = *reinterpret_cast<volatile uint32_t*>(cur.count);
         if (n_rec == 0) break;                                // uniform over the grid: read after a grid-wide barrier
         if (r == rounds) { if (blockIdx.x == 0 && threadIdx.x == 0) report(P, DF_STACK); break; }
-        if (blockIdx.x == 0) {
-            if (threadIdx.x < 4) nxt.count[threadIdx.x] = 0;
-            plan_body(cur);
-        }
+        if (blockIdx.x == 0 && threadIdx.x < 4) nxt.count[threadIdx.x] = 0;
+        plan_body(cur, blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), gridDim.x * (blockDim.x >> 5));
         __threadfence();
         grid.sync();
         scatter_body(P, cur, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
@@ -1740,7 +1725,7 @@ static int32_t serve_rounds(aceapex_archive* ar, Params Q, const GList g[2], uin
     for (uint32_t r = 0; r < rounds; r++) {
         Q.gl_cur = g[r & 1]; Q.gl_nxt = g[(r + 1) & 1];
         CU(cudaMemsetAsync(Q.gl_nxt.count, 0, 16, ar->stream));
-        k_plan<<<1, 1024, 0, ar->stream>>>(Q);               // bucket offsets + work items
+        k_plan<<<ar->sms, 256, 0, ar->stream>>>(Q);          // bucket offsets + work items
         k_scatter<<<4 * ar->sms, 256, 0, ar->stream>>>(Q);
         ar->launches += 2;
         int32_t rc = launch(ar, Q, 1);

@@ -37,7 +37,7 @@ struct GList {
     uint32_t* touched;       // blocks with at least one record, in order of first touch
     unsigned long long* work;// work items written by k_plan: block << 32 | first record, then the record count in work_n
     uint32_t* work_n;
-    uint32_t* count;         // [0] = records appended, [1] = blocks touched, [2] = work items
+    uint32_t* count;         // [0] = records appended, [1] = blocks touched, [2] = work items, [3] = records given a bucket
     uint32_t cap, touched_cap, work_cap;
 };
 
