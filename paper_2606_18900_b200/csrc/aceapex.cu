@@ -1030,6 +1030,80 @@ __global__ void __launch_bounds__(1024, 1) k_copy(const Params P) {
     }
 }
 
+// Command table of a parsed block (demand rounds): entry ci = block-relative output position of command ci | position of
+// its first literal in the literal stream << 16; entry n_cmd is the sentinel (block length, n_lit), so lengths are
+// differences of neighbours.  Lives in the warp's run-table area.  Returns false when the block does not fit (more than
+// RUNS_CAP - 1 commands, blocks above 32 KB) or fails validation (reported); the caller then serves span by span.
+__device__ __forceinline__ bool build_cmd_table(const Params& P, const BlockCtx& c, uint32_t tab /* shared address */) {
+    if (c.d.n_cmd + 1 > RUNS_CAP || P.log2_bs > 15) return false;
+    uint32_t lit_base = 0, out_base = 0, ec = 0, em = c.n_ext_cmd;
+    const uint32_t lane = lane_id();
+    for (uint32_t c0 = 0; c0 < c.d.n_cmd; c0 += 32) {
+        uint32_t ci = c0 + lane;
+        bool valid = ci < c.d.n_cmd, has_match = ci < c.d.n_match;
+        uint32_t tl = valid ? c.tok_cmd[ci] : 0, tm = has_match ? c.tok_mlen[ci] : 0;
+        uint32_t ml = __ballot_sync(0xffffffffu, valid && tl == 255), mm = __ballot_sync(0xffffffffu, has_match && tm == 255);
+        uint32_t lit_len = tl, match_len = has_match ? P.min_match + tm : 0;
+        if (valid && tl == 255) lit_len = 255 + __ldg(c.ext + ec + __popc(ml & lanemask_lt()));
+        if (has_match && tm == 255) match_len = P.min_match + 255 + __ldg(c.ext + em + __popc(mm & lanemask_lt()));
+        ec += __popc(ml); em += __popc(mm);
+        uint32_t sl = lit_len, stt = lit_len + match_len;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t a = __shfl_up_sync(0xffffffffu, sl, o), t = __shfl_up_sync(0xffffffffu, stt, o);
+            if (lane >= (uint32_t)o) { sl += a; stt += t; }
+        }
+        const uint64_t lit_pos = (uint64_t)lit_base + sl - lit_len, out_rel = (uint64_t)out_base + (stt - lit_len - match_len);
+        const bool ok = !valid || (lit_pos + lit_len <= c.d.n_lit && c.bstart + out_rel + lit_len + match_len <= c.bend);
+        if (__any_sync(0xffffffffu, !ok)) { if (lane == 0) report(P, DF_LENGTH); return false; }
+        if (valid) asm volatile("st.shared.u32 [%0], %1;" ::"r"(tab + 4 * ci), "r"((uint32_t)out_rel | (uint32_t)lit_pos << 16) : "memory");
+        lit_base += __shfl_sync(0xffffffffu, sl, 31);
+        out_base += __shfl_sync(0xffffffffu, stt, 31);
+    }
+    if (lit_base != c.d.n_lit || c.bstart + out_base != c.bend) { if (lane == 0) report(P, DF_LENGTH); return false; }
+    if (lane == 0) asm volatile("st.shared.u32 [%0], %1;" ::"r"(tab + 4 * c.d.n_cmd), "r"(out_base | lit_base << 16) : "memory");
+    __syncwarp();
+    return true;
+}
+
+constexpr uint32_t ITEM_LANE_MAX = 96;   // spans up to this many bytes are served by one lane each
+
+// The records of a work item, one per lane: lane l emits bytes [pos, pos + len) of the parsed block c to out2[dst ..).
+// A binary search in the command table finds the first command of the span; the lane then walks its commands (one to
+// three for a 32-byte span): literal bytes come from the warp's scratch, match pieces are forwarded to their sources.
+__device__ __forceinline__ void emit_item(const Params& P, const BlockCtx& c, const Stack& st, uint32_t tab, bool have,
+                                          uint64_t pos, uint32_t len, uint64_t dst) {
+    if (!have || len == 0) return;
+    const uint32_t pr = (uint32_t)(pos - c.bstart), pe = pr + len;
+    uint32_t lo = 0, hi = c.d.n_cmd;
+    while (hi - lo > 1) { const uint32_t mid = (lo + hi) >> 1; if ((lds32(tab + 4 * mid) & 0xffffu) <= pr) lo = mid; else hi = mid; }
+    uint32_t e = lds32(tab + 4 * lo);
+    for (uint32_t k = lo; k < c.d.n_cmd; k++) {
+        const uint32_t e1 = lds32(tab + 4 * k + 4);
+        const uint32_t o0 = e & 0xffffu, lit_pos = e >> 16;
+        if (o0 >= pe) break;
+        const uint32_t lit_len = (e1 >> 16) - lit_pos, match_len = (e1 & 0xffffu) - o0 - lit_len;
+        e = e1;
+        uint32_t a = max(o0, pr), b = min(o0 + lit_len, pe);
+        if (a < b) copy_bytes<false>(P.out2 + dst + (a - pr), c.lit + lit_pos + (a - o0), b - a, ~0ull);
+        const uint32_t mo = o0 + lit_len;
+        a = max(mo, pr); b = min(mo + match_len, pe);
+        if (k < c.d.n_match && a < b) {
+            const uint64_t md = c.bstart + mo, src = match_src(P, c, k);
+            const uint64_t period = md - src;
+            if (src >= md) report(P, DF_OFFSET);
+            else if (period >= match_len) fetch_source<false>(P, c, st, src + (a - mo), b - a, dst + (a - pr));
+            else if (period > lit_len) report(P, DF_OFFSET);          // FORMAT.md §3 (c): the seed is the tail of this literal run
+            else {                                                    // byte i of the match = seed[i mod period]
+                const uint8_t* seed = c.lit + lit_pos + lit_len - period;
+                uint8_t* d = P.out2 + dst + (a - pr);
+                uint32_t r = (uint32_t)((a - mo) % period);
+                for (uint32_t i = 0; i < b - a; i++) { d[i] = seed[r]; if (++r == period) r = 0; }
+            }
+        }
+    }
+}
+
 // Bucket offsets and work items of the list in P.gl_cur: every warp of the launch takes 32 touched blocks at a time; the
 // bucket offsets and the work-item slots come from two global counters (count[3]: records placed, count[2]: work items),
 // one atomicAdd per warp each (the order of the buckets in the sorted array is irrelevant); cnt[block] becomes the fill
@@ -1106,6 +1180,23 @@ __device__ __forceinline__ void serve_body(const Params& P, const CtaSmem& m, Bl
 #pragma unroll
         for (int o = 16; o >= 1; o >>= 1) pend = max((unsigned long long)pend, (unsigned long long)__shfl_xor_sync(0xffffffffu, pend, o));
         const bool ok = parse_block_upto(P, m.luts, m.ring, c, pend);
+        if (ok && build_cmd_table(P, c, m.runs)) {           // one record per lane
+            const bool have = lane_id() < cnt && first + lane_id() < cur.cap;
+            GDemand d; d.pos = c.bstart; d.len = 0; d.dst = 0;
+            if (have) d = ld_demand(cur.sorted + first + lane_id());
+            const bool inside = have && d.pos >= c.bstart && d.pos + d.len <= c.bend;
+            if (have && !inside) report(P, DF_LENGTH);
+            // a long span covers many commands: the whole warp walks it (a lane per command) instead of one lane
+            const bool wide = inside && d.len > ITEM_LANE_MAX;
+            emit_item(P, c, sk, m.runs, inside && !wide, d.pos, (uint32_t)d.len, d.dst);
+            __syncwarp();
+            uint32_t wides = __ballot_sync(0xffffffffu, wide);
+            while (wides) {
+                const int l = __ffs(wides) - 1; wides &= wides - 1;
+                emit_span(P, c, sk, __shfl_sync(0xffffffffu, d.pos, l), __shfl_sync(0xffffffffu, (uint32_t)d.len, l), __shfl_sync(0xffffffffu, d.dst, l));
+            }
+            continue;
+        }
         for (uint32_t k = 0; k < cnt && first + k < cur.cap; k++) {
             const GDemand d = ld_demand(cur.sorted + first + k);
             if (ok) emit_span(P, c, sk, d.pos, d.len, d.dst);
