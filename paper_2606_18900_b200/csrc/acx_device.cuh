@@ -159,22 +159,22 @@ struct Rans {
         cp_async_wait_group<2>();
     }
     // one symbol on this lane.  lut = shared address of the table (8 KB aligned).  Returns the table entry
-    // (sym | bias << 8 | freq << 20).
+    // (sym | bias << 8 | freq << 20).  The ring is read only by the lanes that renormalise (a predicated load: about one
+    // lane in four on quality strings), which costs the step a dependent shared-memory read but takes ~1.7 of ~8.4
+    // wavefronts per 32-symbol round off the shared-memory pipe (k_literals 0.844 -> 0.827 ms on configs[1]).
     __device__ __forceinline__ uint32_t step_full(uint32_t lut) {
         uint32_t e = lds32(lut | ((x << 2) & (4 * LUT_SIZE - 4)));
-        uint32_t w = lds16(ring | (rp & 63));
         x = (e >> 20) * (x >> PROB_BITS) + ((e >> 8) & 0xfff);
-        if (x < 65536u) { x = (x << 16) | w; rp += 2; }
+        if (x < 65536u) { x = (x << 16) | lds16(ring | (rp & 63)); rp += 2; }
         return e;
     }
     // one symbol on the lanes with active == true
     __device__ __forceinline__ uint32_t step(uint32_t lut, bool active) {
         uint32_t e = lds32(lut | ((x << 2) & (4 * LUT_SIZE - 4)));
-        uint32_t w = lds16(ring | (rp & 63));
         uint32_t nx = (e >> 20) * (x >> PROB_BITS) + ((e >> 8) & 0xfff);
         if (active) {
             x = nx;
-            if (x < 65536u) { x = (x << 16) | w; rp += 2; }
+            if (x < 65536u) { x = (x << 16) | lds16(ring | (rp & 63)); rp += 2; }
         }
         return e;
     }
