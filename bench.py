@@ -205,6 +205,7 @@ def run_ours(args):
     for _ in range(args.warmup):
         ar.decode_all(out)
     ar.check()
+    out.fill_(0xA5)           # poison: bit_exact below then proves that the TIMED launches wrote every byte
     barrier()
     l0 = ar.launch_count()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)

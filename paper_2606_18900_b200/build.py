@@ -54,7 +54,7 @@ def build_cuda(force=False):
     if force or _newer(out, deps):
         nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
         _run([nvcc] + CUDA_FLAGS + ["-I", os.path.join(ROOT, "include"), "-o", out] + src + ["-lcudart"],
-             log=os.path.join(cs, "ptxas_v.log"))
+             log=os.path.join(PKG, "ptxas_v.log"))          # build log: registers, spills, shared memory (git-ignored)
     return out
 
 

@@ -289,6 +289,9 @@ __device__ __forceinline__ void wait_block(const Params& P, uint64_t S, bool nee
         if (ns < 2048) ns *= 2;          // back off: thousands of lanes polling one L2 line slow everybody down
         if (++spins > (1u << 21)) { report(P, DF_TIMEOUT); break; }
     }
+    // The polls are relaxed loads; one acquire-release fence once the flag has been seen orders every later read of the
+    // guarded bytes after it (the writer: stores, __threadfence, st.release).  Once per wait, not per poll.
+    asm volatile("fence.acq_rel.gpu;" ::: "memory");
 #ifdef ACX_WAIT_STATS
     if (spins) { atomicAdd(P.err + 4 + (need_full ? 2 : 0), 1u); atomicAdd(P.err + 5 + (need_full ? 2 : 0), spins); }
 #endif

@@ -85,8 +85,9 @@ __device__ __forceinline__ uint32_t lane_id() { return threadIdx.x & 31; }
 __device__ __forceinline__ uint32_t lanemask_lt() { uint32_t m; asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m)); return m; }
 
 // Flag poll.  Relaxed on purpose: an acquire load makes ptxas invalidate the whole L1 (CCTL.IVALL) on every poll.
-// The data guarded by a flag is only ever read with ld.cg (L2, the coherence point) and the reads are issued after
-// the poll has returned (control dependency), so no L1 invalidation is needed.
+// wait_block issues ONE fence.acq_rel.gpu after the loop has seen the value (PTX memory model: the relaxed load that
+// observed the release store, followed by the fence, synchronises with the writer); the guarded data is read with
+// ld.cg / cp.async.cg (L2, the coherence point) after that fence.
 __device__ __forceinline__ uint32_t ld_flag(const uint32_t* p) {
     uint32_t v; asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory"); return v;
 }

@@ -73,6 +73,28 @@ def test_far_source_levels():
     assert e.value.name == "E_LEVEL"
 
 
+def test_literal_bytes_of_a_higher_level_block_violate_levels():
+    # FORMAT.md §3 (a): literal bytes may only be read from blocks whose level is NOT HIGHER than the reader's.  Block 1
+    # copies the eight literal bytes of block 0.  With level(0) = 1 and level(1) = 0 the reader sits below its source: the
+    # (level, index) dispatch order of the flag schedules would start block 1 before block 0 -> rejected.
+    blocks = [[(b"ABCDEFGH", None)], [(b"", (0, 8))]]
+    with pytest.raises(O.OracleError) as e:
+        dec(blocks, 16, 3, levels=[1, 0])
+    assert e.value.name == "E_LEVEL"
+    # the same bytes with legal levels (equal, or the reader higher) decode to the hand-written output
+    for lv in ([0, 0], [1, 1], [0, 1], [2, 3]):
+        assert dec(blocks, 16, 3, levels=lv) == b"ABCDEFGH" * 2
+    # a source two blocks back at a higher level is rejected as well; one literal byte is enough
+    blocks3 = [[(b"ABCDEFGH", None)], [(b"IJKLMNOP", None)], [(b"xyz", (7, 5))]]
+    assert dec(blocks3, 24, 3, levels=[0, 0, 0]) == b"ABCDEFGHIJKLMNOP" + b"xyz" + b"HIJKL"
+    with pytest.raises(O.OracleError) as e:
+        dec(blocks3, 24, 3, levels=[1, 0, 0])       # byte 7 is a literal byte of block 0 (level 1 > 0)
+    assert e.value.name == "E_LEVEL"
+    with pytest.raises(O.OracleError) as e:
+        dec(blocks3, 24, 3, levels=[0, 2, 1])       # bytes 8..11 are literal bytes of block 1 (level 2 > 1)
+    assert e.value.name == "E_LEVEL"
+
+
 def test_in_block_match_bytes_as_source_violate_levels():
     # second match reads bytes produced by the first match of the same block: forbidden by FORMAT.md §3
     blocks = [[(b"abcd", (0, 4)), (b"", (4, 4)), (b"zzzz", None)]]
