@@ -1,11 +1,11 @@
-"""Pins of the oracle's rANS step (FORMAT.md §1.5) against an independent pure-Python encoder (tests/acx_build.py),
+"""Pins of the oracle's rANS step (FORMAT.md §1.7) against an independent pure-Python encoder (tests/acx_build.py),
 closed forms and the final-state invariant."""
 import math
 
 import numpy as np
 import pytest
 
-from acx_build import M, normalise, rans_encode
+from acx_build import M, MQ_BITS, normalise, rans_encode
 from oracle import acx_oracle as O
 
 
@@ -133,3 +133,40 @@ def test_truncated_word_stream_is_an_error():
     with pytest.raises(O.OracleError) as e:
         O.rans_decode(np.array([f], np.uint16), np.zeros(400, np.uint8), np.array(states, np.uint32), streams)
     assert e.value.name == "E_TRUNCATED"
+
+
+def test_worked_example_pair_table_precision_12():
+    # FORMAT.md §1.7: the pair table codes with pb = 12 (M_Q = 4096).  Two entries {A: 1024, B: 3072}, by hand:
+    #   encode A on x = 65536: f << 20 = 2^30 > x -> no word; x' = (65536 // 1024) << 12 + 0 + 0 = 64 * 4096 = 262144
+    #   decode: slot = 262144 & 4095 = 0 -> A; x = 1024 * (262144 >> 12) + 0 = 65536.
+    #   encode B: x' = (65536 // 3072) << 12 + 65536 % 3072 + 1024 = 21 * 4096 + 1024 + 1024 = 88064
+    #   decode: slot = 88064 & 4095 = 2048 -> B (cum 1024); x = 3072 * 21 + 2048 - 1024 = 65536.
+    f = [1024, 3072]
+    for sym, want in ((0, 262144), (1, 88064)):
+        states, streams = rans_encode([sym], [0], [f], [MQ_BITS])
+        assert states[0] == want and states[1:] == [65536] * 31 and streams == [[]] * 32
+        got, final, used = O.rans_decode(np.array([f], np.uint16), np.array([0], np.uint8), np.array(states, np.uint32), streams,
+                                         prob_bits=MQ_BITS)
+        assert list(got) == [sym] and final[0] == 65536 and used.sum() == 0
+    # the same states read with pb = 11 are a different code: 262144 & 2047 = 0 still says A but leaves x = 512 * 128 != 2^16
+    with pytest.raises(O.OracleError):
+        O.rans_decode(np.array([f], np.uint16), np.array([0], np.uint8), np.array([262144] + [65536] * 31, np.uint32), [[]] * 32, prob_bits=11)
+
+
+def test_tables_of_precision_11_and_12_interleaved_on_the_same_states():
+    # a segment's symbol sequence ends with LITA (pb 11) followed by LITQ pairs (pb 12, up to 4096 symbols) on the SAME 32 states
+    rng = np.random.default_rng(21)
+    a = rng.integers(0, 40, 1237)                                   # byte symbols
+    b = rng.integers(0, 900, 2999)                                  # pair-table entries
+    n_sym = 900
+    fa = normalise(np.bincount(a, minlength=n_sym).tolist())        # sums to 2^11
+    fb = normalise(np.bincount(b, minlength=n_sym).tolist(), MQ_BITS)
+    syms = a.tolist() + b.tolist()
+    tids = [0] * len(a) + [1] * len(b)
+    states, streams = rans_encode(syms, tids, [fa, fb], [11, MQ_BITS])
+    got, final, used = O.rans_decode(np.array([fa, fb], np.uint16), np.array(tids, np.uint8), np.array(states, np.uint32), streams,
+                                     prob_bits=[11, MQ_BITS])
+    assert list(got) == syms and (final == 65536).all() and used.tolist() == [len(s) for s in streams]
+    ideal = sum(-math.log2(fa[v] / 2048) for v in a) + sum(-math.log2(fb[v] / 4096) for v in b)
+    bits = 16 * sum(len(s) for s in streams) + sum(math.log2(x) - 16 for x in states)
+    assert abs(bits - ideal) < 64
