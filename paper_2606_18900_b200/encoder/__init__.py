@@ -10,7 +10,7 @@ class EncOpts(ctypes.Structure):
     _fields_ = [("log2_bs", ctypes.c_uint32), ("min_match", ctypes.c_uint32), ("max_level", ctypes.c_uint32),
                 ("threads", ctypes.c_uint32), ("src_window", ctypes.c_uint64), ("chunk_log2", ctypes.c_uint32),
                 ("batch_chunks", ctypes.c_uint32), ("chain_depth", ctypes.c_uint32), ("hash_log2", ctypes.c_uint32),
-                ("with_fnv", ctypes.c_uint32), ("reserved", ctypes.c_uint32 * 3)]
+                ("with_fnv", ctypes.c_uint32), ("log2_seg", ctypes.c_uint32), ("q_min", ctypes.c_uint32), ("q_mode", ctypes.c_uint32)]
 
 
 def _load():
@@ -29,8 +29,9 @@ def _load():
 def encode(data, block_size=16384, **kw):
     """data: uint8 numpy array (or bytes).  Returns the archive as a uint8 numpy array.
 
-    Options (encoder.cpp acx_enc_opts): min_match, max_level, threads, src_window, chunk_log2, batch_chunks,
-    chain_depth, hash_log2, with_fnv."""
+    Options (encoder.cpp acx_enc_opts): min_match, max_level (default 0), threads, src_window, chunk_log2, batch_chunks,
+    chain_depth, hash_log2, with_fnv, log2_seg (segment size, default min(block, 16 KB)), q_min (literal runs of this many
+    bytes or more form the stream LITQ; default 64, 0 = one literal class), q_mode (0 bytes, 1 pairs, 2 = the smaller)."""
     lib = _load()
     data = np.ascontiguousarray(np.frombuffer(data, dtype=np.uint8) if isinstance(data, (bytes, bytearray)) else data)
     assert data.dtype == np.uint8

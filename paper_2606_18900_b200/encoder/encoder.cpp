@@ -23,18 +23,32 @@ constexpr uint32_t PROB_BITS = 11;
 constexpr uint32_t M = 1u << PROB_BITS;
 constexpr uint32_t RANS_L = 1u << 16;
 
+constexpr uint32_t MQ_BITS = 12;
+constexpr uint32_t MAX_SEG_CMDS = 510, MAX_SEG_LITS = 16384;     // FORMAT.md §1.5
+constexpr uint64_t TAIL_PAD = 128;
+
 struct Opts {
     uint32_t log2_bs, min_match, max_level, threads;
     uint64_t src_window;
-    uint32_t chunk_log2, batch_chunks, chain_depth, hash_log2, with_fnv, reserved[3];
+    uint32_t chunk_log2, batch_chunks, chain_depth, hash_log2, with_fnv, log2_seg, q_min, q_mode;
 };
 
+struct Cmd { uint32_t lit_len, match_len; uint64_t off; };       // match_len 0: no match
+
 struct Block {
-    std::vector<uint8_t> cmd, mlen, lit;
-    std::vector<uint64_t> off;
-    std::vector<uint32_t> ext_cmd, ext_mlen;
+    std::vector<Cmd> cmds;
+    std::vector<uint8_t> lit;                                     // the literal runs back to back
     uint16_t level = 0;
     uint64_t match_bytes = 0;
+};
+
+// a segment: commands [c0, c1) of its block after cutting (FORMAT.md §1.5)
+struct Seg {
+    uint64_t block, out_start;
+    std::vector<Cmd> cmds;
+    std::vector<uint8_t> lit_a, lit_q;
+    std::vector<uint16_t> q_sym;                                  // LITQ symbols: bytes, or pairs v0 | v1 << 8
+    std::vector<uint32_t> q_edge;                                 // pair mode: indices into q_sym of the pairs with a filler half
 };
 
 inline uint64_t ld64(const uint8_t* p) { uint64_t v; memcpy(&v, p, 8); return v; }
@@ -79,7 +93,8 @@ struct Enc {
     struct Cand { uint64_t p; uint32_t len; uint32_t lvl; int64_t gain; };
 
     // Longest valid match of source p for destination i (dst limited to bend); returns false if unusable.
-    bool evaluate(uint64_t p, uint64_t i, uint64_t bstart, uint64_t bend, uint64_t cs, uint64_t batch_start, Cand& c) const {
+    // lit_start: start of the pending literal run of the command this match would close
+    bool evaluate(uint64_t p, uint64_t i, uint64_t bstart, uint64_t bend, uint64_t cs, uint64_t batch_start, uint64_t lit_start, Cand& c) const {
         if (p >= i) return false;
         if (i + 4 <= N && ld32(x + p) != ld32(x + i)) return false;   // hash collision
         if (o.src_window && i - p > o.src_window) return false;
@@ -94,7 +109,9 @@ struct Enc {
         while (l < maxlen && x[p + l] == x[i + l]) l++;
     done:
         if (l < o.min_match) return false;
-        if (p + l > i && p < bstart) l = i - p;                 // FORMAT.md §3 (c): a self-overlapping match starts in its own block
+        // FORMAT.md §3 (c): the seed of a self-overlapping match is the tail of its own literal run (and short enough to stay
+        // in one piece when the run is cut at a segment boundary)
+        if (p + l > i && (p < lit_start || i - p > 4096)) l = i - p;
         if (l < o.min_match) return false;
         uint64_t seed_end = std::min(p + l, i);
         uint32_t lvl = 0;
@@ -132,15 +149,12 @@ struct Enc {
             Block& B = blocks[bi];
             uint64_t i = bstart, lit_start = bstart;
             uint32_t blvl = 0;
-            auto put_lit_token = [&](uint64_t n) {
-                if (n < 255) B.cmd.push_back((uint8_t)n); else { B.cmd.push_back(255); B.ext_cmd.push_back((uint32_t)(n - 255)); }
-                B.lit.insert(B.lit.end(), x + lit_start, x + lit_start + n);
-            };
+            auto put_lit = [&](uint64_t n) { B.lit.insert(B.lit.end(), x + lit_start, x + lit_start + n); };
             while (i < bend) {
                 Cand best{0, 0, 0, 0}; bool have = false;
                 auto consider = [&](uint64_t p) {
                     Cand c;
-                    if (!evaluate(p, i, bstart, bend, cs, batch_start, c)) return;
+                    if (!evaluate(p, i, bstart, bend, cs, batch_start, lit_start, c)) return;
                     if (c.gain <= 0) return;
                     if (!have || c.gain > best.gain || (c.gain == best.gain && (c.lvl < best.lvl || (c.lvl == best.lvl && c.p < best.p)))) { best = c; have = true; }
                 };
@@ -162,23 +176,21 @@ struct Enc {
                 // extend backwards over pending literals while the source byte is a literal byte
                 uint64_t p = best.p, len = best.len;
                 while (i > lit_start && p > 0 && x[i - 1] == x[p - 1] && (p - 1 >= cs || p - 1 < batch_start) && is_lit(p - 1) &&
-                       !(len + 1 > i - p && p - 1 < bstart)) {   // FORMAT.md §3 (c): the extended match (len + 1, same period) would
-                    // overlap itself with its source starting outside the block
+                       !(len + 1 > i - p) && !(p + len > i)) {   // FORMAT.md §3 (c): an overlapping match keeps its seed inside the
+                    // literal run in front of it, so it is never extended backwards, and an extension may not create an overlap
                     // the new seed byte p-1 is a literal byte: allowed by FORMAT.md §3 (a); its block may raise the level
                     i--; p--; len++;
                     if (p / BS != bi) best.lvl = std::max(best.lvl, (uint32_t)level[p / BS]);
                 }
-                put_lit_token(i - lit_start);
-                uint64_t t = len - o.min_match;
-                if (t < 255) B.mlen.push_back((uint8_t)t); else { B.mlen.push_back(255); B.ext_mlen.push_back((uint32_t)(t - 255)); }
-                B.off.push_back(p);
+                put_lit(i - lit_start);
+                B.cmds.push_back(Cmd{(uint32_t)(i - lit_start), (uint32_t)len, p});
                 B.match_bytes += len;
                 blvl = std::max(blvl, best.lvl);
                 clear_lit(i, i + len);
                 for (uint64_t k = i + len - best.len; k < i + len; k++) insert(k); // [i, old i) were inserted as literals
                 i += len; lit_start = i;
             }
-            if (lit_start < bend || B.cmd.empty()) put_lit_token(bend - lit_start);
+            if (lit_start < bend || B.cmds.empty()) { put_lit(bend - lit_start); B.cmds.push_back(Cmd{(uint32_t)(bend - lit_start), 0, 0}); }
             B.level = (uint16_t)blvl;
             level[bi] = (uint16_t)blvl;
         }
@@ -205,54 +217,100 @@ template <class F> void parallel_for(uint64_t n, uint32_t threads, F f) {
 }
 
 // ---- static tables --------------------------------------------------------------------------------------------
-struct Table { uint32_t mode = 0; uint16_t freq[256] = {0}; uint16_t cum[257] = {0}; };
+struct Table { uint32_t mode = 0; std::vector<uint16_t> freq, cum; };   // cum has one entry more than freq
 
-void normalise(const uint64_t* h, Table& t) {
-    uint64_t total = 0; int present = 0, top = 0;
-    for (int s = 0; s < 256; s++) { total += h[s]; if (h[s]) present++; if (h[s] > h[top]) top = s; }
-    memset(t.freq, 0, sizeof t.freq);
-    if (total == 0) { t.freq[0] = M; }
+// counts -> frequencies summing to 2^bits, every present symbol >= 1 (needs at most 2^bits present symbols)
+void normalise(const std::vector<uint64_t>& h, uint32_t bits, Table& t) {
+    const int64_t m = 1ll << bits;
+    const size_t n = h.size();
+    uint64_t total = 0;
+    for (size_t s = 0; s < n; s++) total += h[s];
+    t.freq.assign(n, 0);
+    if (total == 0) { t.freq[0] = (uint16_t)m; }
     else {
         int64_t sum = 0;
-        for (int s = 0; s < 256; s++) if (h[s]) {
-            uint64_t f = (h[s] * (uint64_t)M + total / 2) / total;
+        for (size_t s = 0; s < n; s++) if (h[s]) {
+            uint64_t f = (h[s] * (uint64_t)m + total / 2) / total;
             if (f == 0) f = 1;
-            t.freq[s] = (uint16_t)f; sum += (int64_t)f;
+            t.freq[s] = (uint16_t)std::min<uint64_t>(f, 65535); sum += (int64_t)t.freq[s];
         }
         // fix the sum on the symbols that lose least: repeatedly adjust the currently largest frequency
-        while (sum != (int64_t)M) {
-            int best = -1;
-            for (int s = 0; s < 256; s++) if (t.freq[s] > 1 || (sum < (int64_t)M && t.freq[s] >= 1)) if (best < 0 || t.freq[s] > t.freq[best]) best = s;
-            int64_t d = (int64_t)M - sum;
+        while (sum != m) {
+            size_t best = n;
+            for (size_t s = 0; s < n; s++) if (t.freq[s] > 1 || (sum < m && t.freq[s] >= 1)) if (best == n || t.freq[s] > t.freq[best]) best = s;
+            int64_t d = m - sum;
             int64_t room = d > 0 ? d : -std::min<int64_t>(-d, (int64_t)t.freq[best] - 1);
             t.freq[best] = (uint16_t)(t.freq[best] + room); sum += room;
         }
     }
-    t.cum[0] = 0;
-    for (int s = 0; s < 256; s++) t.cum[s + 1] = (uint16_t)(t.cum[s] + t.freq[s]);
+    t.cum.assign(n + 1, 0);
+    for (size_t s = 0; s < n; s++) t.cum[s + 1] = (uint16_t)(t.cum[s] + t.freq[s]);
+}
+
+double coded_bits(const std::vector<uint64_t>& h, const Table& t, uint32_t bits) {
+    double b = 0;
+    for (size_t s = 0; s < h.size(); s++) if (h[s]) b += (double)h[s] * -std::log2(t.freq[s] / (double)(1u << bits));
+    return b;
 }
 
 struct Out {
     std::vector<uint8_t> b;
+    void u16(uint32_t v) { b.push_back((uint8_t)v); b.push_back((uint8_t)(v >> 8)); }
     void u32(uint32_t v) { for (int i = 0; i < 4; i++) b.push_back((uint8_t)(v >> (8 * i))); }
     void u64(uint64_t v) { for (int i = 0; i < 8; i++) b.push_back((uint8_t)(v >> (8 * i))); }
     void pad(size_t a) { while (b.size() % a) b.push_back(0); }
 };
 
-// rANS-encode the block's symbol sequence (FORMAT.md §1.5); returns the 32 initial decoder states and, per state, its
+struct Sym { uint16_t freq, cum; uint8_t pb; };
+
+// rANS-encode the segment's symbol sequence (FORMAT.md §1.7); returns the 32 initial decoder states and, per state, its
 // own word stream in the order the decoder consumes it
-void rans_block(const std::vector<uint8_t>& sym, const std::vector<uint8_t>& tid, const std::vector<Table>& T,
-                uint32_t X[32], std::vector<uint16_t> words[32]) {
+void rans_segment(const std::vector<Sym>& sym, uint32_t X[32], std::vector<uint16_t> words[32]) {
     for (int k = 0; k < 32; k++) { X[k] = RANS_L; words[k].clear(); }
     for (size_t i = sym.size(); i-- > 0;) {
-        const Table& t = T[tid[i]];
-        uint32_t f = t.freq[sym[i]], c = t.cum[sym[i]];
+        const uint32_t f = sym[i].freq, c = sym[i].cum, pb = sym[i].pb;
         uint32_t& xs = X[i & 31];
         uint32_t xv = xs;
-        if ((uint64_t)xv >= ((uint64_t)f << (32 - PROB_BITS))) { words[i & 31].push_back((uint16_t)(xv & 0xffff)); xv >>= 16; }
-        xs = ((xv / f) << PROB_BITS) + (xv % f) + c;
+        if ((uint64_t)xv >= ((uint64_t)f << (32 - pb))) { words[i & 31].push_back((uint16_t)(xv & 0xffff)); xv >>= 16; }
+        xs = ((xv / f) << pb) + (xv % f) + c;
     }
     for (int k = 0; k < 32; k++) std::reverse(words[k].begin(), words[k].end());
+}
+
+// FORMAT.md §1.5: cut the commands of one block into segments.  A command starts only while its segment holds fewer than
+// SEG output bytes; at most 510 commands and 16384 literal bytes per segment; a literal run that does not fit is cut (the
+// segment ends with a match-less command, the run goes on in the next one).  A self-overlapping match keeps at least
+// its period of literal bytes in front of it (FORMAT.md §3 (c)).
+void cut_block(const Block& B, uint64_t bi, uint64_t BS, uint64_t SEG, std::vector<Seg>& out) {
+    uint64_t pos = bi * BS, lp = 0;
+    Seg cur; cur.block = bi; cur.out_start = pos;
+    uint64_t seg_lits = 0;
+    std::vector<std::pair<uint64_t, uint32_t>> runs;     // (position in B.lit, length) of the literal part of each command of cur
+    auto close = [&]() {
+        // literal classes are assigned later (they need q_min); keep the raw run list in lit_a for now
+        out.push_back(std::move(cur));
+        cur = Seg(); cur.block = bi; cur.out_start = pos; seg_lits = 0;
+    };
+    for (const Cmd& c : B.cmds) {
+        if (!cur.cmds.empty() && (pos - cur.out_start >= SEG || cur.cmds.size() == MAX_SEG_CMDS)) close();
+        uint64_t R = c.lit_len;
+        const uint64_t dst = pos + R;
+        const uint64_t period = (c.match_len && c.off + c.match_len > dst) ? dst - c.off : 0;   // self-overlap: keep >= period literals
+        while (seg_lits + R > MAX_SEG_LITS) {
+            uint64_t t = MAX_SEG_LITS - seg_lits;
+            if (R - t < period) t = R > period ? R - period : 0;
+            if (t > 0) {
+                cur.cmds.push_back(Cmd{(uint32_t)t, 0, 0});
+                cur.lit_a.insert(cur.lit_a.end(), B.lit.begin() + lp, B.lit.begin() + lp + t);
+                lp += t; pos += t; R -= t;
+            }
+            close();
+        }
+        cur.cmds.push_back(Cmd{(uint32_t)R, c.match_len, c.off});
+        cur.lit_a.insert(cur.lit_a.end(), B.lit.begin() + lp, B.lit.begin() + lp + R);
+        lp += R; pos += R + c.match_len; seg_lits += R;
+    }
+    if (!cur.cmds.empty()) out.push_back(std::move(cur));
 }
 
 } // namespace
@@ -262,13 +320,17 @@ extern "C" {
 struct acx_enc_opts {
     uint32_t log2_bs, min_match, max_level, threads;
     uint64_t src_window;
-    uint32_t chunk_log2, batch_chunks, chain_depth, hash_log2, with_fnv, reserved[3];
+    uint32_t chunk_log2, batch_chunks, chain_depth, hash_log2, with_fnv, log2_seg, q_min, q_mode;
 };
 
+// q_mode: 0 = LITQ as bytes, 1 = LITQ as aligned pairs (falls back to bytes when the data has more than 4096 distinct
+// pairs), 2 = whichever is smaller, pairs when they cost at most 2 % more (they halve the decode steps).
+// log2_seg 0 = min(log2_bs, 14).  q_min 0 = one literal class.
 void acx_enc_default_opts(acx_enc_opts* o) {
     memset(o, 0, sizeof *o);
-    o->log2_bs = 14; o->min_match = 4; o->max_level = 3; o->threads = 0; o->src_window = 0;
+    o->log2_bs = 14; o->min_match = 4; o->max_level = 0; o->threads = 0; o->src_window = 0;
     o->chunk_log2 = 22; o->batch_chunks = 16; o->chain_depth = 2; o->hash_log2 = 0; o->with_fnv = 1;
+    o->log2_seg = 0; o->q_min = 64; o->q_mode = 2;
 }
 
 void acx_enc_free(void* p) { free(p); }
@@ -280,6 +342,8 @@ int acx_encode(const uint8_t* in, uint64_t N, const acx_enc_opts* uo, uint8_t** 
     memcpy(&e.o, uo, sizeof(Opts));
     Opts& o = e.o;
     if (o.log2_bs < 3 || o.log2_bs > 20 || o.min_match < 4 || o.max_level > 65534) return -1;
+    if (o.log2_seg == 0) o.log2_seg = std::min(o.log2_bs, 14u);
+    if (o.log2_seg < 3 || o.log2_seg > 14 || o.log2_seg > o.log2_bs || o.q_min == 1 || o.q_mode > 2) return -1;
     if (o.chunk_log2 < o.log2_bs) o.chunk_log2 = o.log2_bs;
     if (o.chunk_log2 < 6) o.chunk_log2 = 6; // chunks own whole 64-bit words of the literal bitmap
     if (o.chunk_log2 > 30) return -1;
@@ -326,90 +390,244 @@ int acx_encode(const uint8_t* in, uint64_t N, const acx_enc_opts* uo, uint8_t** 
             });
     }
     { std::vector<std::atomic<uint64_t>> g; e.gtab.swap(g); }
+    { std::vector<uint64_t> g; e.litmap.swap(g); }
 
-    // ---- histograms and tables
-    const uint32_t n_tables = 3 + W;
-    std::vector<std::vector<uint64_t>> H(n_tables, std::vector<uint64_t>(256, 0));
-    uint64_t tot_lit = 0, tot_mb = 0, tot_m = 0, tot_c = 0; uint32_t max_level = 0, max_cmds = 0;
-    for (auto& B : e.blocks) {
-        for (uint8_t v : B.cmd) H[0][v]++;
-        for (uint8_t v : B.mlen) H[1][v]++;
-        for (uint64_t v : B.off) for (uint32_t p = 0; p < W; p++) H[2 + p][(v >> (8 * p)) & 0xff]++;
-        for (uint8_t v : B.lit) H[2 + W][v]++;
-        tot_lit += B.lit.size(); tot_mb += B.match_bytes; tot_m += B.off.size(); tot_c += B.cmd.size();
-        max_level = std::max<uint32_t>(max_level, B.level); max_cmds = std::max<uint32_t>(max_cmds, (uint32_t)B.cmd.size());
+    // ---- segments (FORMAT.md §1.5): cut block by block, in parallel over groups of blocks, concatenated in block order
+    const uint64_t SEG = 1ull << o.log2_seg;
+    std::vector<Seg> segs;
+    std::vector<uint32_t> first_seg(e.n_blocks + 1, 0);
+    {
+        const uint64_t G = 256, n_groups = (e.n_blocks + G - 1) / G;
+        std::vector<std::vector<Seg>> part(n_groups);
+        parallel_for(n_groups, threads, [&](uint64_t g) {
+            for (uint64_t bi = g * G; bi < std::min(e.n_blocks, (g + 1) * G); bi++) {
+                cut_block(e.blocks[bi], bi, e.BS, SEG, part[g]);
+                Block& B = e.blocks[bi];
+                std::vector<Cmd>().swap(B.cmds); std::vector<uint8_t>().swap(B.lit);
+            }
+        });
+        uint64_t total = 0;
+        for (auto& p : part) total += p.size();
+        if (total >= (1ull << 32)) return -3;
+        segs.reserve(total);
+        for (auto& p : part) { for (auto& s : p) segs.push_back(std::move(s)); std::vector<Seg>().swap(p); }
+        uint64_t at = 0;
+        for (uint64_t bi = 0; bi < e.n_blocks; bi++) {
+            first_seg[bi] = (uint32_t)at;
+            while (at < segs.size() && segs[at].block == bi) at++;
+        }
+        first_seg[e.n_blocks] = (uint32_t)segs.size();
     }
-    std::vector<Table> T(n_tables);
-    for (uint32_t t = 0; t < n_tables; t++) {
-        normalise(H[t].data(), T[t]);
-        if (t >= 2 && t < 2 + W) { // raw if coding would save < 3 %
-            double bits = 0; uint64_t n = 0;
-            for (int s = 0; s < 256; s++) if (H[t][s]) { bits += (double)H[t][s] * -std::log2(T[t].freq[s] / (double)M); n += H[t][s]; }
-            if (n && bits > 0.97 * 8.0 * (double)n) { T[t].mode = 1; memset(T[t].freq, 0, sizeof T[t].freq); }
+    const uint64_t n_segs = segs.size();
+
+    // ---- literal classes (FORMAT.md §1.6): runs of q_min bytes or more -> LITQ.  cut_block left every run in lit_a.
+    const uint32_t q_min = o.q_min;
+    parallel_for(n_segs, threads, [&](uint64_t si) {
+        Seg& s = segs[si];
+        if (q_min == 0) return;
+        std::vector<uint8_t> a, q;
+        uint64_t lp = 0;
+        for (const Cmd& c : s.cmds) {
+            std::vector<uint8_t>& dst = c.lit_len >= q_min ? q : a;
+            dst.insert(dst.end(), s.lit_a.begin() + lp, s.lit_a.begin() + lp + c.lit_len);
+            lp += c.lit_len;
+        }
+        s.lit_a.swap(a); s.lit_q.swap(q);
+    });
+
+    // ---- LITQ model: bytes or aligned pairs (FORMAT.md §1.7)
+    // pass 1: histogram of the complete pairs (both halves inside a run) and of the LITQ bytes
+    std::vector<uint64_t> pair_h(65536, 0), qbyte_h(256, 0);
+    uint64_t tot_litq = 0;
+    for (const Seg& s : segs) {
+        uint64_t pos = s.out_start, lq = 0;
+        for (const Cmd& c : s.cmds) {
+            if (q_min && c.lit_len >= q_min) {
+                const uint8_t* r = s.lit_q.data() + lq;
+                for (uint64_t k = (pos + 1) >> 1; 2 * k + 1 < pos + c.lit_len; k++) pair_h[r[2 * k - pos] | r[2 * k + 1 - pos] << 8]++;
+                for (uint32_t i = 0; i < c.lit_len; i++) qbyte_h[r[i]]++;
+                lq += c.lit_len; tot_litq += c.lit_len;
+            }
+            pos += (uint64_t)c.lit_len + c.match_len;
         }
     }
+    // pass 2: a pair with one half outside its run gets the filler that makes it the most frequent complete pair
+    // (ties: the smaller filler); best_lo[v1] = filler for (?, v1), best_hi[v0] = filler for (v0, ?)
+    uint32_t q_mode = (q_min && tot_litq) ? o.q_mode : 0;
+    std::vector<uint16_t> qpair_of;            // table order: sorted pair values
+    Table TQ;                                   // over qpair_of
+    std::vector<uint32_t> qindex(65536, 0);
+    std::vector<uint64_t> qh;
+    if (q_mode >= 1) {
+        uint8_t best_lo[256], best_hi[256];
+        for (int v = 0; v < 256; v++) {
+            int bl = 0, bh = 0;
+            for (int f = 1; f < 256; f++) { if (pair_h[f | v << 8] > pair_h[bl | v << 8]) bl = f; if (pair_h[v | f << 8] > pair_h[v | bh << 8]) bh = f; }
+            best_lo[v] = (uint8_t)bl; best_hi[v] = (uint8_t)bh;
+        }
+        std::vector<uint64_t> edge_h(65536, 0);
+        for (const Seg& s : segs) {
+            uint64_t pos = s.out_start, lq = 0;
+            for (const Cmd& c : s.cmds) {
+                if (c.lit_len >= q_min) {
+                    const uint8_t* r = s.lit_q.data() + lq;
+                    if (pos & 1) edge_h[best_lo[r[0]] | r[0] << 8]++;
+                    if ((pos + c.lit_len) & 1) { uint8_t v0 = r[c.lit_len - 1]; if (!(c.lit_len == 1 && (pos & 1))) edge_h[v0 | best_hi[v0] << 8]++; }
+                    lq += c.lit_len;
+                }
+                pos += (uint64_t)c.lit_len + c.match_len;
+            }
+        }
+        uint64_t distinct = 0;
+        for (uint32_t v = 0; v < 65536; v++) { pair_h[v] += edge_h[v]; distinct += pair_h[v] != 0; }
+        if (distinct > 4096 || distinct == 0) q_mode = 0;
+        else {
+            for (uint32_t v = 0; v < 65536; v++) if (pair_h[v]) { qindex[v] = (uint32_t)qpair_of.size(); qpair_of.push_back((uint16_t)v); qh.push_back(pair_h[v]); }
+            normalise(qh, MQ_BITS, TQ);
+            if (q_mode == 2) {                  // smaller of the two, pairs preferred within 2 %
+                Table tb; std::vector<uint64_t> hb(qbyte_h.begin(), qbyte_h.end());
+                normalise(hb, PROB_BITS, tb);
+                q_mode = coded_bits(qh, TQ, MQ_BITS) <= 1.02 * coded_bits(hb, tb, PROB_BITS) ? 1 : 0;
+            }
+        }
+        // pass 3: the LITQ symbols of every segment
+        if (q_mode == 1) parallel_for(n_segs, threads, [&](uint64_t si) {
+            Seg& s = segs[si];
+            uint64_t pos = s.out_start, lq = 0;
+            for (const Cmd& c : s.cmds) {
+                if (c.lit_len >= q_min) {
+                    const uint8_t* r = s.lit_q.data() + lq;
+                    const uint64_t end = pos + c.lit_len;
+                    for (uint64_t k = pos >> 1; k <= (end - 1) >> 1; k++) {
+                        const bool in0 = 2 * k >= pos, in1 = 2 * k + 1 < end;
+                        uint8_t v0 = in0 ? r[2 * k - pos] : 0, v1 = in1 ? r[2 * k + 1 - pos] : 0;
+                        if (!in0) v0 = best_lo[v1];
+                        if (!in1) v1 = best_hi[v0];
+                        s.q_sym.push_back((uint16_t)(v0 | v1 << 8));
+                    }
+                    lq += c.lit_len;
+                }
+                pos += (uint64_t)c.lit_len + c.match_len;
+            }
+        });
+    }
+    if (q_mode == 0 && q_min) for (Seg& s : segs) s.q_sym.assign(s.lit_q.begin(), s.lit_q.end());
+
+    // ---- histograms and byte tables
+    const uint32_t n_tables = 4 + W;
+    std::vector<std::vector<uint64_t>> H(n_tables, std::vector<uint64_t>(256, 0));
+    uint64_t tot_lit = 0, tot_mb = 0, tot_m = 0, tot_c = 0; uint32_t max_level = 0, max_cmds = 0;
+    for (const Seg& s : segs) {
+        for (const Cmd& c : s.cmds) {
+            H[0][std::min<uint32_t>(c.lit_len, 255)]++;
+            if (c.match_len) {
+                H[1][std::min<uint32_t>(c.match_len - o.min_match, 255)]++;
+                for (uint32_t p = 0; p < W; p++) H[2 + p][(c.off >> (8 * p)) & 0xff]++;
+                tot_m++; tot_mb += c.match_len;
+            }
+        }
+        for (uint8_t v : s.lit_a) H[2 + W][v]++;
+        if (q_mode == 0) for (uint8_t v : s.lit_q) H[3 + W][v]++;
+        tot_lit += s.lit_a.size() + s.lit_q.size(); tot_c += s.cmds.size();
+        max_cmds = std::max<uint32_t>(max_cmds, (uint32_t)s.cmds.size());
+    }
+    for (const Block& B : e.blocks) max_level = std::max<uint32_t>(max_level, B.level);
+    std::vector<Table> T(n_tables);
+    for (uint32_t t = 0; t < n_tables; t++) {
+        normalise(H[t], PROB_BITS, T[t]);
+        if (t >= 2 && t < 2 + W) { // raw if coding would save < 3 %
+            uint64_t n = 0;
+            for (int s = 0; s < 256; s++) n += H[t][s];
+            if (n && coded_bits(H[t], T[t], PROB_BITS) > 0.97 * 8.0 * (double)n) { T[t].mode = 1; T[t].freq.assign(256, 0); }
+        }
+    }
+    if (q_min == 0 || q_mode == 1 || tot_litq == 0) { T[3 + W].mode = (q_min == 0 || q_mode == 1) ? 2 : 0; if (T[3 + W].mode == 2) T[3 + W].freq.assign(256, 0); }
+
     // ---- encode payloads
-    std::vector<std::vector<uint8_t>> pay(e.n_blocks);
-    std::vector<uint32_t> n_words(e.n_blocks);
-    std::vector<uint64_t> fnv(e.n_blocks);
-    parallel_for(e.n_blocks, threads, [&](uint64_t bi) {
-        Block& B = e.blocks[bi];
-        std::vector<uint8_t> sym, tid;
-        size_t nm = B.off.size();
-        sym.reserve(B.cmd.size() + nm * (1 + W) + B.lit.size()); tid.reserve(sym.capacity());
-        for (uint8_t v : B.cmd) { sym.push_back(v); tid.push_back(0); }
-        for (uint8_t v : B.mlen) { sym.push_back(v); tid.push_back(1); }
+    std::vector<std::vector<uint8_t>> pay(n_segs);
+    std::vector<uint32_t> n_words(n_segs), n_ext(n_segs);
+    parallel_for(n_segs, threads, [&](uint64_t si) {
+        const Seg& s = segs[si];
+        std::vector<Sym> sym;
+        std::vector<uint32_t> ext_c, ext_m;
+        size_t nm = 0;
+        for (const Cmd& c : s.cmds) nm += c.match_len != 0;
+        sym.reserve(s.cmds.size() + nm * (1 + W) + s.lit_a.size() + s.q_sym.size());
+        auto put = [&](const Table& t, uint32_t v, uint32_t pb) { sym.push_back(Sym{t.freq[v], t.cum[v], (uint8_t)pb}); };
+        for (const Cmd& c : s.cmds) { put(T[0], std::min<uint32_t>(c.lit_len, 255), PROB_BITS); if (c.lit_len >= 255) ext_c.push_back(c.lit_len - 255); }
+        for (const Cmd& c : s.cmds) if (c.match_len) {
+            uint32_t t = c.match_len - o.min_match;
+            put(T[1], std::min<uint32_t>(t, 255), PROB_BITS); if (t >= 255) ext_m.push_back(t - 255);
+        }
         for (int p = (int)W - 1; p >= 0; p--) if (T[2 + p].mode == 0)
-            for (uint64_t v : B.off) { sym.push_back((uint8_t)(v >> (8 * p))); tid.push_back((uint8_t)(2 + p)); }
-        for (uint8_t v : B.lit) { sym.push_back(v); tid.push_back((uint8_t)(2 + W)); }
+            for (const Cmd& c : s.cmds) if (c.match_len) put(T[2 + p], (uint8_t)(c.off >> (8 * p)), PROB_BITS);
+        for (uint8_t v : s.lit_a) put(T[2 + W], v, PROB_BITS);
+        if (q_mode == 1) for (uint16_t v : s.q_sym) put(TQ, qindex[v], MQ_BITS);
+        else for (uint16_t v : s.q_sym) put(T[3 + W], v, PROB_BITS);
         uint32_t X[32]; std::vector<uint16_t> words[32];
-        rans_block(sym, tid, T, X, words);
+        rans_segment(sym, X, words);
         Out o2;
         uint32_t woff = 0;
         for (int k = 0; k < 32; k++) { o2.u32(X[k]); o2.u32(woff); woff += (uint32_t)words[k].size(); }   // head
-        for (int k = 0; k < 32; k++) for (uint16_t w : words[k]) { o2.b.push_back((uint8_t)w); o2.b.push_back((uint8_t)(w >> 8)); }
+        for (int k = 0; k < 32; k++) for (uint16_t w : words[k]) o2.u16(w);
         o2.pad(4);
-        for (uint32_t v : B.ext_cmd) o2.u32(v);
-        for (uint32_t v : B.ext_mlen) o2.u32(v);
-        for (uint32_t p = 0; p < W; p++) if (T[2 + p].mode == 1) for (uint64_t v : B.off) o2.b.push_back((uint8_t)(v >> (8 * p)));
+        for (uint32_t v : ext_c) o2.u32(v);
+        for (uint32_t v : ext_m) o2.u32(v);
+        for (uint32_t p = 0; p < W; p++) if (T[2 + p].mode == 1) for (const Cmd& c : s.cmds) if (c.match_len) o2.b.push_back((uint8_t)(c.off >> (8 * p)));
         o2.pad(16);
-        pay[bi].swap(o2.b); n_words[bi] = woff;
+        pay[si].swap(o2.b); n_words[si] = woff; n_ext[si] = (uint32_t)(ext_c.size() + ext_m.size());
+    });
+    for (uint64_t si = 0; si < n_segs; si++) if (n_words[si] > 65535 || n_ext[si] > 65535) return -4;
+    std::vector<uint64_t> fnv(e.n_blocks);
+    if (o.with_fnv) parallel_for(e.n_blocks, threads, [&](uint64_t bi) {
         uint64_t h = 0xcbf29ce484222325ull, a = bi * e.BS, b = std::min(N, a + e.BS);
         for (uint64_t q = a; q < b; q++) { h ^= in[q]; h *= 0x100000001b3ull; }
         fnv[bi] = h;
     });
     // ---- layout
-    uint64_t tables_off = 160, dir_off = tables_off + 528ull * n_tables, fnv_off = dir_off + 32 * e.n_blocks;
-    uint64_t payload_off = fnv_off + (o.with_fnv ? 8 * e.n_blocks : 0);
-    payload_off = (payload_off + 15) & ~15ull;
+    auto al16 = [](uint64_t v) { return (v + 15) & ~15ull; };
+    const uint32_t n_qpairs = q_mode == 1 ? (uint32_t)qpair_of.size() : 0;
+    uint64_t tables_off = 192, qtab_off = tables_off + 528ull * n_tables, blocktab_off = al16(qtab_off + 4ull * n_qpairs);
+    uint64_t dir_off = al16(blocktab_off + 8 * (e.n_blocks + 1)), fnv_off = dir_off + 32 * n_segs;
+    uint64_t payload_off = al16(fnv_off + (o.with_fnv ? 8 * e.n_blocks : 0));
     uint64_t total = payload_off;
     for (auto& p : pay) total += p.size();
+    total += TAIL_PAD;
     uint8_t* buf = (uint8_t*)calloc(total ? total : 1, 1);
     if (!buf) return -2;
     Out h;
     const uint8_t magic[8] = {0x41, 0x43, 0x58, 0x42, 0x32, 0x30, 0x30, 0x00};
     h.b.insert(h.b.end(), magic, magic + 8);
-    h.u32(2); h.u32(160); h.u64(N); h.u64(e.n_blocks); h.u32(o.log2_bs); h.u32(o.min_match); h.u32(W); h.u32(PROB_BITS);
-    h.u32(n_tables); h.u32(max_level); h.u32(max_cmds); h.u32(o.with_fnv ? 1 : 0);
-    h.u64(tables_off); h.u64(dir_off); h.u64(o.with_fnv ? fnv_off : 0); h.u64(payload_off); h.u64(total);
-    h.u64(tot_lit); h.u64(tot_mb); h.u64(tot_m); h.u64(tot_c); h.u64(o.src_window); h.u64(0); h.u64(0);
-    memcpy(buf, h.b.data(), 160);
+    h.u32(3); h.u32(192); h.u64(N); h.u64(e.n_blocks); h.u64(n_segs);
+    h.u32(o.log2_bs); h.u32(o.min_match); h.u32(W); h.u32(PROB_BITS); h.u32(n_tables); h.u32(max_level); h.u32(max_cmds); h.u32(o.with_fnv ? 1 : 0);
+    h.u32(o.log2_seg); h.u32(q_min); h.u32(q_mode); h.u32(n_qpairs);
+    h.u64(tables_off); h.u64(qtab_off); h.u64(blocktab_off); h.u64(dir_off); h.u64(o.with_fnv ? fnv_off : 0); h.u64(payload_off); h.u64(total);
+    h.u64(tot_lit); h.u64(tot_mb); h.u64(tot_m); h.u64(tot_c); h.u64(tot_litq); h.u64(o.src_window);
+    memcpy(buf, h.b.data(), 192);
     for (uint32_t t = 0; t < n_tables; t++) {
         uint8_t* p = buf + tables_off + 528ull * t;
         memcpy(p, &T[t].mode, 4);
-        memcpy(p + 16, T[t].freq, 512);
+        memcpy(p + 16, T[t].freq.data(), 512);
+    }
+    for (uint32_t i = 0; i < n_qpairs; i++) { uint16_t v[2] = {qpair_of[i], TQ.freq[i]}; memcpy(buf + qtab_off + 4ull * i, v, 4); }
+    for (uint64_t bi = 0; bi <= e.n_blocks; bi++) {
+        uint8_t* d = buf + blocktab_off + 8 * bi;
+        uint16_t lv = bi < e.n_blocks ? e.blocks[bi].level : 0;
+        memcpy(d, &first_seg[bi], 4); memcpy(d + 4, &lv, 2);
     }
     uint64_t po = payload_off;
-    for (uint64_t bi = 0; bi < e.n_blocks; bi++) {
-        Block& B = e.blocks[bi];
-        uint8_t* d = buf + dir_off + 32 * bi;
-        uint32_t v32[5] = {(uint32_t)B.cmd.size(), (uint32_t)B.off.size(), (uint32_t)B.lit.size(), n_words[bi],
-                           (uint32_t)(B.ext_cmd.size() + B.ext_mlen.size())};
-        memcpy(d, &po, 8); memcpy(d + 8, v32, 20); memcpy(d + 28, &B.level, 2);
-        if (o.with_fnv) memcpy(buf + fnv_off + 8 * bi, &fnv[bi], 8);
-        memcpy(buf + po, pay[bi].data(), pay[bi].size());
-        po += pay[bi].size();
+    for (uint64_t si = 0; si < n_segs; si++) {
+        const Seg& s = segs[si];
+        uint8_t* d = buf + dir_off + 32 * si;
+        uint32_t nm = 0;
+        for (const Cmd& c : s.cmds) nm += c.match_len != 0;
+        uint16_t v16[8] = {(uint16_t)s.cmds.size(), (uint16_t)nm, (uint16_t)s.lit_a.size(), (uint16_t)s.lit_q.size(), (uint16_t)s.q_sym.size(),
+                           (uint16_t)n_words[si], (uint16_t)n_ext[si], e.blocks[s.block].level};
+        memcpy(d, &po, 8); memcpy(d + 8, &s.out_start, 8); memcpy(d + 16, v16, 16);
+        memcpy(buf + po, pay[si].data(), pay[si].size());
+        po += pay[si].size();
     }
+    if (o.with_fnv) memcpy(buf + fnv_off, fnv.data(), 8 * e.n_blocks);
     *out = buf; *out_bytes = total;
     return 0;
 }
