@@ -56,14 +56,18 @@ typedef struct {
     uint64_t total_matches;
     uint64_t total_cmds;
     uint64_t workspace_bytes;    /* device scratch the decode calls need (aceapex_set_workspace) */
-    uint32_t max_level;          /* FORMAT.md §3: number of match waves - 1                      */
+    uint64_t n_segments;         /* FORMAT.md 1.5: entropy-coded units (one warp each)           */
+    uint64_t total_litq_bytes;   /* literal bytes of the class LITQ (runs of q_min bytes or more) */
+    uint32_t max_level;          /* FORMAT.md 3: number of match waves - 1                       */
     uint32_t offset_width;       /* W                                                            */
     uint32_t min_match;
-    uint32_t max_cmds;           /* largest per-block command count                              */
+    uint32_t max_cmds;           /* largest per-segment command count                            */
     uint32_t n_coded_planes;     /* offset planes that are rANS-coded (the rest are raw)         */
     uint32_t has_fnv;            /* per-block FNV-1a 64 section present                          */
     uint32_t resident_warps;     /* warps of the persistent decode grid                          */
-    uint32_t reserved;
+    uint32_t segment_size;       /* SEG                                                          */
+    uint32_t q_min;              /* FORMAT.md 1.6                                                */
+    uint32_t q_mode;             /* FORMAT.md 1.7: 0 = LITQ bytes, 1 = LITQ aligned pairs        */
 } aceapex_info_t;
 
 /* Opens an archive that already resides in device memory ("H2D staging ... outside the timer").

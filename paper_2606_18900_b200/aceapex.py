@@ -21,9 +21,10 @@ class AceapexError(RuntimeError):
 
 class Info(ctypes.Structure):
     _fields_ = [(k, ctypes.c_uint64) for k in ("raw_bytes", "archive_bytes", "n_blocks", "block_size", "total_lit_bytes",
-                                               "total_match_bytes", "total_matches", "total_cmds", "workspace_bytes")] + \
+                                               "total_match_bytes", "total_matches", "total_cmds", "workspace_bytes",
+                                               "n_segments", "total_litq_bytes")] + \
                [(k, ctypes.c_uint32) for k in ("max_level", "offset_width", "min_match", "max_cmds", "n_coded_planes",
-                                               "has_fnv", "resident_warps", "reserved")]
+                                               "has_fnv", "resident_warps", "segment_size", "q_min", "q_mode")]
 
 
 def lib_path():

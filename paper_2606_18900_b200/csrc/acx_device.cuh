@@ -1,5 +1,5 @@
-// Device side of the ACX-B200 decoder (FORMAT.md): per-block entropy decode (A1), command scan (A2), literal
-// placement (A3) and match resolution (A4) — SURVEY §8(a).  One warp owns one block at a time.
+// Device side of the ACX-B200 decoder (FORMAT.md version 3): shared declarations, the rANS step (A1) and the byte copies
+// (A3/A4) — SURVEY §8(a).  One warp owns one segment at a time.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -7,78 +7,79 @@
 namespace acx {
 
 constexpr int PROB_BITS = 11;
-constexpr int LUT_SIZE = 1 << PROB_BITS;          // u32 entries per coded table: sym | bias << 8 | freq << 20
+constexpr int LUT_SIZE = 1 << PROB_BITS;          // u32 entries per byte table: sym | bias << 8 | freq << 20
+constexpr int QPROB_BITS = 12;
+constexpr int QLUT_SIZE = 1 << QPROB_BITS;        // uint2 entries of the pair table: {pair | freq << 16, bias}
 constexpr int RING_BYTES = 2048;                  // per warp: 32 lanes x 64-byte ring of rANS words in shared memory
 constexpr int MAX_W = 8;
 constexpr int MAX_RESIDENT = 8;
+constexpr uint32_t MAX_SEG_CMDS = 510;            // FORMAT.md §1.5
+constexpr uint32_t MAX_SEG_LITS = 16384;
+constexpr uint32_t TOK_STRIDE = 512;              // per-warp token arrays hold one segment's commands
 
 enum : uint32_t { DF_RANS = 1, DF_OFFSET = 2, DF_LENGTH = 4, DF_TIMEOUT = 8, DF_STACK = 16 };
 
-struct DirEntry {            // FORMAT.md §1.3, 32 bytes
-    uint64_t payload_off;
-    uint32_t n_cmd, n_match, n_lit, n_words, n_ext;
-    uint16_t level, flags;
+struct SegEntry {            // FORMAT.md §1.5, 32 bytes
+    uint64_t payload_off, out_start;
+    uint16_t n_cmd, n_match, n_lit_a, n_lit_q, n_sym_q, n_words, n_ext, level;
 };
 
 struct Resident { uint64_t lo, hi; const uint8_t* ptr; };
 
-// "materialise original bytes [pos, pos + len) at out2[dst ..)"; never crosses a block boundary; len == 0: served
+// "materialise original bytes [pos, pos + len) at out2[dst ..)"; never crosses a segment boundary; len == 0: served
 struct Demand { uint64_t pos; uint64_t dst; uint64_t len; };
 
-// Aggregated demands (range decode).  Records are appended unsorted while a per-block counter counts them; before they
-// are served they are bucketed by SOURCE block (k_plan + k_scatter), so one parse of a block serves its whole bucket and a
-// hot block (thousands of records) is cut into work items of GL_ITEM records that different warps take.
-struct GDemand { uint64_t pos; uint64_t dst; uint32_t len; uint32_t pad; };
+// Aggregated demands (range decode).  Records are appended unsorted while a per-segment counter counts them; before they
+// are served they are bucketed by SOURCE segment (plan + scatter), so one parse of a segment serves its whole bucket and a
+// hot segment (thousands of records) is cut into work items of GL_ITEM records that different warps take.
+struct GDemand { uint64_t pos; uint64_t dst; uint32_t len; uint32_t seg; };
 constexpr uint32_t GL_ITEM = 32;
 struct GList {
     GDemand* rec;            // cap records, in order of arrival
-    GDemand* sorted;         // the same records bucketed by block (written by k_scatter)
-    uint32_t* cnt;           // per block: records appended; after k_plan: fill pointer of the block's bucket; 0 when idle
-    uint32_t* touched;       // blocks with at least one record, in order of first touch
-    unsigned long long* work;// work items written by k_plan: block << 32 | first record, then the record count in work_n
+    GDemand* sorted;         // the same records bucketed by segment (written by the scatter phase)
+    uint32_t* cnt;           // per segment: records appended; after the plan phase: fill pointer of its bucket; 0 when idle
+    uint32_t* touched;       // segments with at least one record, in order of first touch
+    unsigned long long* work;// work items written by the plan phase: segment << 32 | first record, the record count in work_n
     uint32_t* work_n;
-    uint32_t* count;         // [0] = records appended, [1] = blocks touched, [2] = work items, [3] = records given a bucket
+    uint32_t* count;         // [0] = records appended, [1] = segments touched, [2] = work items, [3] = records given a bucket
     uint32_t cap, touched_cap, work_cap;
 };
 
-
 struct Params {
     const uint8_t* archive;      // device archive
-    uint64_t archive_bytes;
-    const DirEntry* dir;         // = archive + dir_off
+    const SegEntry* dir;         // = archive + dir_off
     const uint32_t* luts;        // n_coded_tables x LUT_SIZE
+    const uint2* lutq;           // QLUT_SIZE entries (pair mode)
     const uint16_t* levels;      // level per block
-    uint64_t N;
-    uint32_t log2_bs, min_match, W, n_coded_tables;
+    const uint32_t* first_seg;   // n_blocks + 1 entries (FORMAT.md §1.4)
+    uint64_t N, n_segs;
+    uint32_t log2_bs, log2_seg, min_match, W, n_coded_tables, q_min, q_mode;
     int8_t plane_lut[MAX_W];     // coded OFF plane p -> lut index, -1 if raw
-    int8_t plane_raw[MAX_W];     // raw OFF plane p -> index among raw planes, -1 if coded
     uint32_t n_coded_planes, n_raw_planes;
     uint8_t coded_shift[MAX_W];  // bit position of the k-th coded plane in decode order (high plane first)
     uint8_t raw_shift[MAX_W];    // bit position of the r-th raw plane (ascending p)
-    uint32_t lut_cmd, lut_mlen, lut_lit;
+    uint32_t lut_cmd, lut_mlen, lut_lita, lut_litq;
     // work
-    uint64_t first_block, n_work;       // FULL mode: blocks [first_block, first_block + n_work)
-    uint8_t* out;                        // FULL mode: byte at absolute position p is out[p - out_pos0]
+    uint64_t first_work, n_work;         // work items: segments first_work + i, or seg_list[i]
+    const uint32_t* seg_list;
+    uint8_t* out;                        // byte at absolute position p is out[p - out_pos0]
     uint64_t out_pos0, win_end;          // out holds the original bytes [out_pos0, win_end) (the window; block aligned start)
-    const Demand* demands; uint8_t* out2; // span mode (1): top-level work items, destination buffer of every demand
+    uint32_t out_odd;                    // (out - out_pos0) is an odd address: pair stores fall back to byte stores
+    const Demand* demands; uint8_t* out2; // span mode: top-level work items, destination buffer of every demand
     Demand inline_dem[4]; uint32_t n_inline; // span mode with at most four items: they travel in the kernel arguments
     Resident res[MAX_RESIDENT];
     // workspace
-    uint32_t* flags;                     // per block: 2 * epoch = literals placed, 2 * epoch + 1 = complete
-    uint32_t epoch;
+    uint32_t* done;                      // per block: segments completed by the current flag-driven launch
     unsigned long long* ticket;          // work counter of this launch (zero when the kernel starts)
     unsigned long long* ticket_next;     // the other slot: every kernel clears it for the launch that follows
     uint32_t* err;
-    uint8_t* scratch; uint64_t scratch_per_warp; uint32_t max_cmds;
+    uint8_t* scratch; uint64_t scratch_per_warp;
     Demand* stacks; uint32_t stack_cap;  // per-warp LIFO of pending demands
-    uint32_t mode;                       // 0 = whole blocks with flags, 1 = spans (demands), 2 = literal launch, 3 = match wave,
-                                         // 4 = all match waves with flags
-    const uint32_t* level_list;          // block ids to process (n_work entries), null = first_block + i
     GList gl_cur, gl_nxt;                // range decode: demands being served / being collected
-    uint2* pairs;                        // whole-file decode, left by k_literals for k_copy: (dst_rel, len) of every match,
-                                         // block b at pairs[match_prefix[b] ..]
-    uint8_t* cplanes;                    // ... and its decoded coded offset planes: n_coded_planes x n_match bytes per block
-    const uint64_t* match_prefix;        // n_blocks + 1 entries
+    uint2* pairs;                        // left by the literal launch for the match launch: (dst_rel, len) of every match,
+                                         // segment s at pairs[match_prefix[s] ..]
+    uint8_t* cplanes;                    // ... and its decoded coded offset planes: n_coded_planes x n_match bytes per segment
+    const uint64_t* match_prefix;        // n_segs + 1 entries
 };
 
 __device__ __forceinline__ uint32_t lane_id() { return threadIdx.x & 31; }
@@ -86,34 +87,34 @@ __device__ __forceinline__ uint32_t lanemask_lt() { uint32_t m; asm("mov.u32 %0,
 
 // Flag poll.  Relaxed on purpose: an acquire load makes ptxas invalidate the whole L1 (CCTL.IVALL) on every poll.
 // wait_block issues ONE fence.acq_rel.gpu after the loop has seen the value (PTX memory model: the relaxed load that
-// observed the release store, followed by the fence, synchronises with the writer); the guarded data is read with
+// observed the release, followed by the fence, synchronises with the writer); the guarded data is read with
 // ld.cg / cp.async.cg (L2, the coherence point) after that fence.
 __device__ __forceinline__ uint32_t ld_flag(const uint32_t* p) {
     uint32_t v; asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory"); return v;
 }
-__device__ __forceinline__ void st_release(uint32_t* p, uint32_t v) {
-    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
-}
 // data that other SMs may have written during this kernel: read at L2, never from a stale L1 line
 __device__ __forceinline__ uint8_t ldcg8(const uint8_t* p) { return __ldcg(p); }
-// predicated byte load at L2; the result is unspecified (0) when pred is false
-__device__ __forceinline__ uint32_t ldcg8_if(const uint8_t* p, bool pred) {
-    uint32_t v = 0;
-    asm volatile("{ .reg .pred q; setp.ne.u32 q, %2, 0; @q ld.global.cg.u8 %0, [%1]; }" : "+r"(v) : "l"(p), "r"((uint32_t)pred) : "memory");
-    return v;
-}
 __device__ __forceinline__ uint64_t ldcg64(const uint8_t* p) { return __ldcg(reinterpret_cast<const unsigned long long*>(p)); }
 
-
 // ------------------------------------------------------------------------------------------------ rANS ----------
-// FORMAT.md §1.5 (version 2).  32 states, one per lane; symbol i lives on lane i & 31; every state renormalises from
-// its OWN word stream, so the decode step needs no ballot, no prefix and no shared cursor.  Each lane stages its stream
-// through a private 64-byte ring in shared memory (four 16-byte chunks, filled with cp.async two chunks ahead of their
-// use).  Every table (8 KB aligned) and every ring (64 B aligned) sits at an aligned shared address so that an index
-// folds into an address with one LOP3.
+// FORMAT.md §1.7.  32 states, one per lane; symbol i lives on lane i & 31; every state renormalises from its OWN word
+// stream, so the decode step needs no ballot, no prefix and no shared cursor.  Each lane stages its stream through a
+// private 64-byte ring in shared memory (four 16-byte chunks, filled with cp.async two chunks ahead of their use).
+// The archive ends with a 128-byte pad (FORMAT.md §1), so the refill never tests the archive end.
 __device__ __forceinline__ uint32_t lds32(uint32_t a) { uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a)); return v; }
 __device__ __forceinline__ uint32_t lds8(uint32_t a) { uint32_t v; asm volatile("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(a)); return v; }
 __device__ __forceinline__ uint32_t lds16(uint32_t a) { uint32_t v; asm volatile("ld.shared.u16 %0, [%1];" : "=r"(v) : "r"(a)); return v; }
+__device__ __forceinline__ uint2 lds64(uint32_t a) {
+    uint2 v; asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(a)); return v;
+}
+__device__ __forceinline__ uint4 lds128(uint32_t a) {
+    uint4 v; asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a)); return v;
+}
+__device__ __forceinline__ void sts32(uint32_t a, uint32_t v) { asm volatile("st.shared.u32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
+__device__ __forceinline__ void sts16(uint32_t a, uint32_t v) { asm volatile("st.shared.u16 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
+__device__ __forceinline__ void sts128(uint32_t a, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
+    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
+}
 __device__ __forceinline__ void cp_async16s(uint32_t saddr, const void* gmem) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(saddr), "l"(gmem) : "memory");
 }
@@ -127,14 +128,10 @@ struct Rans {
     uint32_t ring;           // shared address of this lane's ring, 64-byte aligned
     uint32_t end;            // rp after the lane's last word (integrity check)
     const uint8_t* gbase;    // 16-byte aligned global address that offsets are relative to
-    uint32_t lim;            // archive end relative to gbase, saturated (loads are clamped)
 
-    __device__ __forceinline__ void fetch() {
-        if (fp + 16 <= lim) cp_async16s(ring | (fp & 63), gbase + fp);
-        fp += 16;
-    }
-    // payload: [32 x (u32 state, u32 word_off)][words]; n_words = total words of the block
-    __device__ __forceinline__ void init(const uint8_t* payload, uint32_t n_words, const uint8_t* lim_end, uint32_t ring_warp) {
+    __device__ __forceinline__ void fetch() { cp_async16s(ring | (fp & 63), gbase + fp); fp += 16; }
+    // payload: [32 x (u32 state, u32 word_off)][words]; n_words = total words of the segment
+    __device__ __forceinline__ void init(const uint8_t* payload, uint32_t n_words, uint32_t ring_warp) {
         const uint32_t lane = lane_id();
         uint2 h = __ldg(reinterpret_cast<const uint2*>(payload) + lane);
         x = h.x;
@@ -148,8 +145,7 @@ struct Rans {
         end = rp + 2u * (next - h.y);
         fp = bias;
         ring = ring_warp + 64u * lane;
-        this->lim = (uint32_t)min((unsigned long long)(lim_end - gbase), 0xfffffff0ull);
-        cp_async_wait_group<0>();            // chunks still in flight from the previous block must not land after ours
+        cp_async_wait_group<0>();            // chunks still in flight from the previous segment must not land after ours
         fetch(); cp_async_commit(); fetch(); cp_async_commit(); fetch(); cp_async_commit(); fetch(); cp_async_commit();
     }
     // Call before every group of <= 8 symbols per lane (<= 16 B of words).  Invariant after the call: fp - rp >= 50 and
@@ -159,64 +155,78 @@ struct Rans {
         cp_async_commit();
         cp_async_wait_group<2>();
     }
-    // one symbol on this lane.  lut = shared address of the table (8 KB aligned).  Returns the table entry
-    // (sym | bias << 8 | freq << 20).  The ring is read only by the lanes that renormalise (a predicated load: about one
-    // lane in four on quality strings), which costs the step a dependent shared-memory read but takes ~1.7 of ~8.4
-    // wavefronts per 32-symbol round off the shared-memory pipe (k_literals 0.844 -> 0.827 ms on configs[1]).
-    __device__ __forceinline__ uint32_t step_full(uint32_t lut) {
-        uint32_t e = lds32(lut | ((x << 2) & (4 * LUT_SIZE - 4)));
-        x = (e >> 20) * (x >> PROB_BITS) + ((e >> 8) & 0xfff);
+    __device__ __forceinline__ void renorm() {
         if (x < 65536u) { x = (x << 16) | lds16(ring | (rp & 63)); rp += 2; }
+    }
+    // one symbol on this lane.  lut = shared address of a byte table.  Returns the table entry (sym | bias << 8 |
+    // freq << 20).  The ring is read only by the lanes that renormalise (a predicated load).
+    __device__ __forceinline__ uint32_t step_full(uint32_t lut) {
+        uint32_t e = lds32(lut + 4u * (x & (LUT_SIZE - 1)));
+        x = (e >> 20) * (x >> PROB_BITS) + ((e >> 8) & 0xfff);
+        renorm();
         return e;
     }
     // one symbol on the lanes with active == true
     __device__ __forceinline__ uint32_t step(uint32_t lut, bool active) {
-        uint32_t e = lds32(lut | ((x << 2) & (4 * LUT_SIZE - 4)));
+        uint32_t e = lds32(lut + 4u * (x & (LUT_SIZE - 1)));
         uint32_t nx = (e >> 20) * (x >> PROB_BITS) + ((e >> 8) & 0xfff);
-        if (active) {
-            x = nx;
-            if (x < 65536u) { x = (x << 16) | lds16(ring | (rp & 63)); rp += 2; }
-        }
+        if (active) { x = nx; renorm(); }
         return e;
+    }
+    // one PAIR symbol (FORMAT.md §1.7, pb = 12): entry = {pair | freq << 16, bias}; returns the low word
+    __device__ __forceinline__ uint32_t step_pair_full(uint32_t lutq) {
+        uint2 e = lds64(lutq + 8u * (x & (QLUT_SIZE - 1)));
+        x = (e.x >> 16) * (x >> QPROB_BITS) + e.y;
+        renorm();
+        return e.x;
+    }
+    __device__ __forceinline__ uint32_t step_pair(uint32_t lutq, bool active) {
+        uint2 e = lds64(lutq + 8u * (x & (QLUT_SIZE - 1)));
+        uint32_t nx = (e.x >> 16) * (x >> QPROB_BITS) + e.y;
+        if (active) { x = nx; renorm(); }
+        return e.x;
     }
     __device__ __forceinline__ bool finished() const { return x == 65536u && rp == end; }
 };
 
 // Decodes `count` symbols whose global symbol indices start at i0, storing them to dst[0..count) (byte stores,
-// consecutive lanes -> consecutive bytes).  Returns the number of symbols equal to 255 when COUNT_ESC.
-// Table entries: sym | bias << 8 | freq << 20  (the low byte is what gets stored).
-template <bool COUNT_ESC>
+// consecutive lanes -> consecutive bytes; PAIR: 16-bit stores to a 2-byte aligned dst).  Returns the number of symbols
+// equal to 255 when COUNT_ESC.  dst == nullptr: decode without storing.
+template <bool COUNT_ESC, bool PAIR = false>
 __device__ __forceinline__ uint32_t rans_region(Rans& r, uint32_t lut, uint32_t i0, uint32_t count, uint8_t* dst) {
     uint32_t esc = 0;
     if (count == 0) return 0;
     const uint32_t i1 = i0 + count, lane = lane_id();
+    const bool store = dst != nullptr;
+    constexpr uint32_t S = PAIR ? 2 : 1;
     uint32_t base = i0 & ~31u;
-    uint8_t* p = dst + lane - (i0 - base);           // address of symbol base + lane
+    uint8_t* p = dst + (int64_t)S * ((int64_t)lane - (int64_t)(i0 - base));     // address of symbol base + lane
+    auto put = [&](uint8_t* q, uint32_t e) { if (PAIR) *reinterpret_cast<uint16_t*>(q) = (uint16_t)e; else *q = (uint8_t)e; };
     if (base != i0) {                                // ragged first round
         uint32_t i = base + lane;
         bool active = i >= i0 && i < i1;
         r.prepare8();
-        uint32_t e = r.step(lut, active);
-        if (active) *p = (uint8_t)e;
+        uint32_t e = PAIR ? r.step_pair(lut, active) : r.step(lut, active);
+        if (active && store) put(p, e);
         if (COUNT_ESC) esc += __popc(__ballot_sync(0xffffffffu, active && (e & 0xff) == 255));
-        base += 32; p += 32;
+        base += 32; p += 32 * S;
     }
     while (base + 256 <= i1) {                       // eight full rounds per ring check
         r.prepare8();
 #pragma unroll
         for (int k = 0; k < 8; k++) {
-            uint32_t e = r.step_full(lut);
-            p[32 * k] = (uint8_t)e;
+            uint32_t e = PAIR ? r.step_pair_full(lut) : r.step_full(lut);
+            if (store) put(p + 32 * S * k, e);
             if (COUNT_ESC) esc += __popc(__ballot_sync(0xffffffffu, (e & 0xff) == 255));
         }
-        base += 256; p += 256;
+        base += 256; p += 256 * S;
     }
     if (base < i1) {                                 // fewer than eight rounds left, the last may be ragged
         r.prepare8();
-        for (; base < i1; base += 32, p += 32) {
+        for (; base < i1; base += 32, p += 32 * S) {
             bool active = base + lane < i1;
-            uint32_t e = r.step(lut, active);
-            if (active) *p = (uint8_t)e;
+            uint32_t e = PAIR ? r.step_pair(lut, active) : r.step(lut, active);
+            if (active && store) put(p, e);
             if (COUNT_ESC) esc += __popc(__ballot_sync(0xffffffffu, active && (e & 0xff) == 255));
         }
     }
@@ -249,20 +259,10 @@ __device__ __forceinline__ void st_small(uint8_t* d, uint64_t v, uint32_t n) {
     if (n) *d = (uint8_t)v;
 }
 
-// dst/src may have any alignment.  `period` = dst position - src position for a match (UINT64_MAX when the two
-// buffers are unrelated).  period >= len (non-overlapping): loads are issued ahead of the stores that depend on
-// them, 8 bytes at a time.  Self-overlap: ascending 8-byte steps when period >= 8, else the byte-serial copy that
-// is the definition (FORMAT.md §2).
+// dst/src may have any alignment and must not overlap: loads are issued ahead of the stores that depend on them,
+// 8 bytes at a time.
 template <bool SRC_CG>
-__device__ __forceinline__ void copy_bytes(uint8_t* dst, const uint8_t* src, uint32_t len, uint64_t period) {
-    if (period < len) {   // self-overlapping match (src + len > dst): ascending order matters
-        if (period < 8) { for (uint32_t i = 0; i < len; i++) dst[i] = SRC_CG ? ldcg8(src + i) : src[i]; return; }
-        for (uint32_t i = 0; i < len; i += 8) {   // bytes [src+i, src+i+8) lie below dst+i: already written
-            uint32_t n = len - i < 8 ? len - i : 8;
-            st_small(dst + i, ld64u<SRC_CG>(src + i, n), n);
-        }
-        return;
-    }
+__device__ __forceinline__ void copy_bytes(uint8_t* dst, const uint8_t* src, uint32_t len) {
     if (len <= 16) {
         uint64_t lo = ld64u<SRC_CG>(src, len < 8 ? len : 8);
         uint64_t hi = len > 8 ? ld64u<SRC_CG>(src + 8, len - 8) : 0;
@@ -326,7 +326,5 @@ __device__ __forceinline__ void warp_copy(uint8_t* dst, const uint8_t* src, uint
     uint32_t done = head + body;
     if (done + lane < len) dst[done + lane] = SRC_CG ? ldcg8(src + done + lane) : src[done + lane];
 }
-
-__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
 } // namespace acx

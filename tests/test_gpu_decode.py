@@ -32,6 +32,25 @@ HAND = [
 ]
 
 
+# version 3 of the format: segments, literal classes, pair symbols (the archives of tests/test_oracle_handbuilt.py)
+SEGS3 = [[(b"ABCDEFGHIJ", None)], [(b"KL", (0, 3)), (b"mn", (2, 4))], [(b"", (8, 4)), (b"wxyz123", None)]]
+QCMDS = [(b"ab", (0, 2)), (b"QQQQQ", (4, 3)), (b"XY", (4, 4)), (b"RSTUVW", (12, 2)), (b"!", None)]
+QFIRST = [(b"a" + bytes(range(98, 98 + 30)) + b"~", None)]
+QPAIR = [QFIRST, [(b"p", (0, 2)), (b"HIJKL", (35, 2)), (b"MNOPQ", (0, 2)), (b"xyzw", None)]]
+HAND += [
+    ([SEGS3], 32, 5, dict(log2_seg=3, min_match=2)),
+    ([SEGS3, [(b"", (0, 8))]], 40, 5, dict(log2_seg=3, min_match=2)),
+    ([QCMDS], 27, 5, dict(min_match=2, q_min=4)),
+    ([QCMDS], 27, 5, dict(min_match=2, q_min=4, q_mode=1)),
+    ([QCMDS], 27, 5, dict(min_match=2, q_min=2, q_mode=1)),
+    (QPAIR, 53, 5, dict(min_match=2, q_min=4, q_mode=1)),
+    (QPAIR, 53, 5, dict(min_match=2, q_min=4, q_mode=1, filler=0)),
+    (QPAIR, 53, 5, dict(min_match=2, q_min=4, q_mode=0)),
+    ([[[(b"ab", None)], [(b"ab", (2, 4))]]], 8, 3, dict(min_match=2)),
+    ([[(b"xab", (1, 5))]], 8, 3, dict(min_match=2)),
+]
+
+
 @pytest.mark.parametrize("case", range(len(HAND)))
 @pytest.mark.parametrize("levels", [False, True])
 def test_hand_built(case, levels):
@@ -63,6 +82,32 @@ def test_config0_fastq(fastq_4m, fastq_4m_archive, schedule):
 def test_fasta(fasta_2m, fasta_2m_archive):
     got = gpu_decode(fasta_2m_archive)
     assert np.array_equal(got, fasta_2m)
+
+
+@pytest.mark.parametrize("kw", [dict(q_mode=0), dict(q_mode=1), dict(q_min=0), dict(q_min=2), dict(q_min=2, q_mode=0), dict(q_min=300, q_mode=1),
+                                dict(max_level=3), dict(max_level=3, q_mode=0), dict(block_size=65536, log2_seg=12), dict(block_size=4096, log2_seg=9),
+                                dict(block_size=1 << 18, q_mode=0, max_level=2), dict(block_size=1 << 20, max_level=1)])
+def test_encoder_options_of_version_3(fastq_4m, fasta_2m, kw):
+    """Literal classes, pair symbols, segment sizes and level caps (FORMAT.md 1.5-1.7, 3), every schedule, vs the oracle."""
+    from paper_2606_18900_b200 import encoder
+    for x in (fastq_4m[:(2 << 20) + 4321], fasta_2m[:(1 << 20) + 77]):
+        a = encoder.encode(x, **kw)
+        exp = O.decode(a)
+        assert np.array_equal(exp, x)
+        for sched in (None, "flags", "fused"):
+            assert np.array_equal(gpu_decode(a, schedule=sched), exp), (kw, sched)
+
+
+def test_incompressible_and_huge_runs():
+    """Literal runs and matches longer than a segment: runs cut at segment boundaries, one command of 200,000 match bytes."""
+    from paper_2606_18900_b200 import encoder
+    rng = np.random.default_rng(5)
+    noise = rng.integers(0, 256, 100_000, dtype=np.uint8)
+    x = np.concatenate([noise, np.full(200_000, 65, np.uint8), noise[:50_000], np.tile(noise[:3000], 30)])
+    for bs in (1 << 20, 1 << 16, 1 << 14):
+        a = encoder.encode(x, block_size=bs)
+        for sched in (None, "flags", "fused"):
+            assert np.array_equal(gpu_decode(a, schedule=sched), x), (bs, sched)
 
 
 @pytest.mark.parametrize("bs", [4096, 8192, 65536, 262144, 1 << 20])
@@ -110,7 +155,7 @@ def test_open_errors(fastq_4m_archive):
     assert e.value.name == "E_TRUNCATED"
     bad = fastq_4m_archive.copy()
     h = O.header(fastq_4m_archive)
-    bad[h["dir_off"] + 8:h["dir_off"] + 12] = 0          # n_cmd = 0
+    bad[h["dir_off"] + 16:h["dir_off"] + 18] = 0         # n_cmd = 0
     with pytest.raises(AceapexError) as e:
         Archive(bad)
     assert e.value.name == "E_CORRUPT"
