@@ -103,6 +103,10 @@ class Archive:
             self.set_stream(stream)
 
     # -- plumbing
+    def _chk(self, rc, what=""):
+        if rc:
+            raise AceapexError(rc, "%s (cuda error %d)" % (what, self.L.aceapex_last_cuda_error(self.h)) if rc == -8 else what)
+
     def info(self):
         return {k: int(getattr(self._info, k)) for k, _ in Info._fields_}
 
@@ -154,18 +158,18 @@ class Archive:
         schedule = "levels" if levels else schedule
         f = {None: self.L.aceapex_decode_all, "levels": self.L.aceapex_decode_all, "flags": self.L.aceapex_decode_all_flags,
              "fused": self.L.aceapex_decode_all_fused}[schedule]
-        _chk(f(self.h, out.data_ptr()), "decode_all")
+        self._chk(f(self.h, out.data_ptr()), "decode_all")
         return out[:self.raw_bytes]
 
     def decode_range(self, lo, hi, out=None, vram_budget=0):
         out = self.new_output(hi - lo) if out is None else out
-        _chk(self.L.aceapex_decode_range(self.h, lo, hi, out.data_ptr(), vram_budget), "decode_range")
+        self._chk(self.L.aceapex_decode_range(self.h, lo, hi, out.data_ptr(), vram_budget), "decode_range")
         return out[:hi - lo]
 
     def reads_bytes(self, read_index, read_ids):
         total = ctypes.c_uint64()
         offs = np.zeros(len(read_ids) + 1, dtype=np.uint64)
-        _chk(self.L.aceapex_reads_bytes(read_index.ctypes.data, read_index.size, read_ids.ctypes.data, read_ids.size,
+        self._chk(self.L.aceapex_reads_bytes(read_index.ctypes.data, read_index.size, read_ids.ctypes.data, read_ids.size,
                                         ctypes.byref(total), offs.ctypes.data), "reads_bytes")
         return int(total.value), offs
 
@@ -175,19 +179,19 @@ class Archive:
         if out is None:
             total, _ = self.reads_bytes(read_index, read_ids)
             out = self.new_output(total)
-        _chk(self.L.aceapex_decode_reads(self.h, read_index.ctypes.data, read_index.size, read_ids.ctypes.data,
+        self._chk(self.L.aceapex_decode_reads(self.h, read_index.ctypes.data, read_index.size, read_ids.ctypes.data,
                                          read_ids.size, out.data_ptr()), "decode_reads")
         return out
 
     def set_resident(self, slot, lo, hi, tensor):
-        _chk(self.L.aceapex_set_resident(self.h, slot, lo, hi, tensor.data_ptr() if tensor is not None else None))
+        self._chk(self.L.aceapex_set_resident(self.h, slot, lo, hi, tensor.data_ptr() if tensor is not None else None))
 
     def verify_fnv(self, data, lo=0, hi=None):
         hi = self.raw_bytes if hi is None else hi
         bad = ctypes.c_uint64()
-        _chk(self.L.aceapex_verify_fnv(self.h, data.data_ptr(), lo, hi, ctypes.byref(bad)), "verify_fnv")
+        self._chk(self.L.aceapex_verify_fnv(self.h, data.data_ptr(), lo, hi, ctypes.byref(bad)), "verify_fnv")
         return int(bad.value)
 
     def decode_all_host(self, h_archive, d_stage, h_out):
         """h_archive / h_out: pinned CPU uint8 tensors; d_stage: device uint8 tensor of raw_bytes."""
-        _chk(self.L.aceapex_decode_all_host(self.h, h_archive.data_ptr(), d_stage.data_ptr(), h_out.data_ptr()), "decode_all_host")
+        self._chk(self.L.aceapex_decode_all_host(self.h, h_archive.data_ptr(), d_stage.data_ptr(), h_out.data_ptr()), "decode_all_host")

@@ -47,6 +47,7 @@ struct aceapex_archive {
     // launch geometry
     int sms = 148, threads = 1024;
     size_t smem_entropy = 0, smem_copy = 0, smem_fused = 0;
+    uint32_t runs_bytes = 0, lita_bytes = 0;              // per-warp shared memory of the entropy kernels (acx_kernels.cuh setup_cta)
     uint64_t scratch_per_warp = 0, ctrl_bytes = 0;
     uint64_t done_off = 0, scratch_off = 0, stacks_off = 0, demands_off = 0, list_off = 0, ws_need = 0;
     uint32_t stack_cap = 0, demand_cap = 0;
@@ -130,8 +131,10 @@ void fill_params(const aceapex_archive* ar, Params& P) {
     memcpy(P.plane_lut, ar->plane_lut, MAX_W);
     P.n_coded_planes = ar->n_coded_planes; P.n_raw_planes = ar->n_raw_planes;
     for (int p = (int)ar->W - 1, k = 0; p >= 0; p--) if (ar->plane_lut[p] >= 0) P.coded_shift[k++] = (uint8_t)(8 * p);
+    for (int p = (int)ar->W - 1, k = 0; p >= 0; p--) if (ar->plane_lut[p] >= 0) P.coded_lut[k++] = (uint8_t)ar->plane_lut[p];
     for (uint32_t p = 0, r = 0; p < ar->W; p++) if (ar->plane_lut[p] < 0) P.raw_shift[r++] = (uint8_t)(8 * p);
     P.lut_cmd = ar->lut_cmd; P.lut_mlen = ar->lut_mlen; P.lut_lita = ar->lut_lita; P.lut_litq = ar->lut_litq;
+    P.runs_bytes = ar->runs_bytes; P.lita_bytes = ar->lita_bytes;
     memcpy(P.res, ar->res, sizeof P.res);
     P.err = reinterpret_cast<uint32_t*>(ar->d_ws + 8);
     P.done = reinterpret_cast<uint32_t*>(ar->d_ws + ar->done_off);
@@ -182,9 +185,13 @@ int32_t launch(aceapex_archive* ar, Params& P, Kind kind, uint64_t n_work) {
     take_ticket(ar, P);
     int T; uint32_t g;
     spread(ar, n_work, ar->threads, g, T);
-    const size_t sm_e = entropy_smem(ar->n_coded_tables, ar->q_mode, T), sm_c = (size_t)(T / 32) * COPY_WARP_BYTES + 64;
+    const size_t sm_e = entropy_smem(ar->n_coded_tables, ar->q_mode, ar->runs_bytes + ar->lita_bytes, T), sm_c = (size_t)(T / 32) * COPY_WARP_BYTES + 64;
     switch (kind) {
-        case K_LIT: k_literals<<<g, T, sm_e, ar->stream>>>(P); break;
+        case K_LIT:
+            if (!ar->q_mode) k_literals<0><<<g, T, sm_e, ar->stream>>>(P);
+            else if (!P.out_odd) k_literals<1><<<g, T, sm_e, ar->stream>>>(P);
+            else k_literals<2><<<g, T, sm_e, ar->stream>>>(P);
+            break;
         case K_COPY_TOP: k_copy<false, false, false, true><<<g, T, sm_c, ar->stream>>>(P); break;
         case K_COPY_WAIT: k_copy<true, false, false, false><<<g, T, sm_c, ar->stream>>>(P); break;
         case K_COPY_WIN: k_copy<false, true, false, false><<<g, T, sm_c, ar->stream>>>(P); break;
@@ -373,18 +380,32 @@ int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* 
     int dev = 0; cudaDeviceProp prop;
     CU(cudaGetDevice(&dev)); CU(cudaGetDeviceProperties(&prop, dev));
     ar->sms = prop.multiProcessorCount;
+    // per-warp shared memory besides the word ring: the LITQ run table (a command table of 2 KB in the span-service kernels)
+    // and, with what the tables leave free, a staging area for LITA (up to 4 KB; larger segments stage in global memory)
     ar->threads = 1024;
-    auto smem_max = [&](int T) { return std::max(entropy_smem(ar->n_coded_tables, ar->q_mode, T), (size_t)(T / 32) * COPY_WARP_BYTES + 64); };
-    while (ar->threads > 128 && smem_max(ar->threads) > (size_t)prop.sharedMemPerBlockOptin) ar->threads -= 64;
-    ar->smem_entropy = entropy_smem(ar->n_coded_tables, ar->q_mode, ar->threads);
-    ar->smem_copy = (size_t)(ar->threads / 32) * COPY_WARP_BYTES + 64;
-    ar->smem_fused = smem_max(ar->threads);
+    ar->runs_bytes = runs_bytes_for(ar->q_min);
+    const uint32_t min_area = 4 * (MAX_SEG_CMDS + 2);
+    auto smem_max = [&](int T, uint32_t area) { return std::max(entropy_smem(ar->n_coded_tables, ar->q_mode, area, T), (size_t)(T / 32) * COPY_WARP_BYTES + 64); };
+    while (ar->threads > 128 && smem_max(ar->threads, min_area) > (size_t)prop.sharedMemPerBlockOptin) ar->threads -= 64;
     {
-        const void* fns[] = {(const void*)k_literals, (const void*)k_copy<false, false, false, true>, (const void*)k_copy<true, false, false, false>,
+        const size_t fixed = entropy_smem(ar->n_coded_tables, ar->q_mode, 0, ar->threads);
+        const size_t room = (size_t)prop.sharedMemPerBlockOptin > fixed ? ((size_t)prop.sharedMemPerBlockOptin - fixed) / (ar->threads / 32) : 0;
+        uint32_t area = (uint32_t)std::min<size_t>(room & ~(size_t)15, ar->runs_bytes + 4096);
+        area = std::max(area, min_area);
+        ar->lita_bytes = area - ar->runs_bytes;
+    }
+    ar->smem_entropy = entropy_smem(ar->n_coded_tables, ar->q_mode, ar->runs_bytes + ar->lita_bytes, ar->threads);
+    ar->smem_copy = (size_t)(ar->threads / 32) * COPY_WARP_BYTES + 64;
+    ar->smem_fused = std::max(ar->smem_entropy, ar->smem_copy);
+    {
+        const void* fns[] = {(const void*)k_literals<0>, (const void*)k_literals<1>, (const void*)k_literals<2>, (const void*)k_fused<0>, (const void*)k_fused<1>,
+                             (const void*)k_copy<false, false, false, true>, (const void*)k_copy<true, false, false, false>,
                              (const void*)k_copy<false, true, false, false>, (const void*)k_copy<true, true, false, false>, (const void*)k_copy<false, true, true, false>,
-                             (const void*)k_serve, (const void*)k_spans, (const void*)k_rounds, (const void*)k_fused};
+                             (const void*)k_serve, (const void*)k_spans, (const void*)k_rounds};
         for (const void* f : fns) {
-            CU(cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ar->smem_fused));
+            // the attribute belongs to the function, not to the handle: always the device maximum, so that handles with
+            // different table counts do not lower each other's limit
+            CU(cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prop.sharedMemPerBlockOptin));
             CU(cudaFuncSetAttribute(f, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
         }
     }
@@ -392,7 +413,7 @@ int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* 
         int coop = 0, occ_r = 0, occ_f = 0;
         CU(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
         CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_r, k_rounds, ar->threads, ar->smem_entropy));
-        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_f, k_fused, ar->threads, ar->smem_fused));
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_f, k_fused<1>, ar->threads, ar->smem_fused));
         ar->cooperative = coop && occ_r >= 1 && occ_f >= 1 && !getenv("ACEAPEX_NO_COOPERATIVE");
         ar->use_graphs = !getenv("ACEAPEX_NO_GRAPHS");
         if (occ_r < 1) return ACEAPEX_E_CUDA;
@@ -527,7 +548,7 @@ int32_t aceapex_decode_all_fused(aceapex_archive* ar, void* d_out) {
     CU(cudaMemsetAsync(F.tickets, 0, 32, ar->stream));
     if (F.n_low && (rc = zero_done(ar, 0, ar->n_blocks))) return rc;
     void* args[] = {&P, &F};
-    CU(cudaLaunchCooperativeKernel((const void*)k_fused, dim3(ar->sms), dim3(ar->threads), args, ar->smem_fused, ar->stream));
+    CU(cudaLaunchCooperativeKernel(ar->q_mode ? (const void*)k_fused<1> : (const void*)k_fused<0>, dim3(ar->sms), dim3(ar->threads), args, ar->smem_fused, ar->stream));
     ar->launches++;
     return ACEAPEX_OK;
 }

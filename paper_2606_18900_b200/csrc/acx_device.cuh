@@ -57,8 +57,10 @@ struct Params {
     int8_t plane_lut[MAX_W];     // coded OFF plane p -> lut index, -1 if raw
     uint32_t n_coded_planes, n_raw_planes;
     uint8_t coded_shift[MAX_W];  // bit position of the k-th coded plane in decode order (high plane first)
+    uint8_t coded_lut[MAX_W];    // lut index of the k-th coded plane in decode order
     uint8_t raw_shift[MAX_W];    // bit position of the r-th raw plane (ascending p)
     uint32_t lut_cmd, lut_mlen, lut_lita, lut_litq;
+    uint32_t runs_bytes, lita_bytes;     // per-warp shared memory: LITQ run table / LITA staging (multiples of 16)
     // work
     uint64_t first_work, n_work;         // work items: segments first_work + i, or seg_list[i]
     const uint32_t* seg_list;
@@ -190,9 +192,11 @@ struct Rans {
 };
 
 // Decodes `count` symbols whose global symbol indices start at i0, storing them to dst[0..count) (byte stores,
-// consecutive lanes -> consecutive bytes; PAIR: 16-bit stores to a 2-byte aligned dst).  Returns the number of symbols
-// equal to 255 when COUNT_ESC.  dst == nullptr: decode without storing.
-template <bool COUNT_ESC, bool PAIR = false>
+// consecutive lanes -> consecutive bytes; PAIR: 16-bit stores to a 2-byte aligned dst).  Returns the number of byte symbols
+// equal to 255 (the escape count of a token stream; two instructions per round, ignored by the other streams, so that ONE
+// instance of this loop serves every byte stream of a segment: the kernels are bound by instruction fetch as much as by
+// issue).  dst == nullptr: decode without storing.
+template <bool PAIR>
 __device__ __forceinline__ uint32_t rans_region(Rans& r, uint32_t lut, uint32_t i0, uint32_t count, uint8_t* dst) {
     uint32_t esc = 0;
     if (count == 0) return 0;
@@ -202,32 +206,25 @@ __device__ __forceinline__ uint32_t rans_region(Rans& r, uint32_t lut, uint32_t 
     uint32_t base = i0 & ~31u;
     uint8_t* p = dst + (int64_t)S * ((int64_t)lane - (int64_t)(i0 - base));     // address of symbol base + lane
     auto put = [&](uint8_t* q, uint32_t e) { if (PAIR) *reinterpret_cast<uint16_t*>(q) = (uint16_t)e; else *q = (uint8_t)e; };
-    if (base != i0) {                                // ragged first round
-        uint32_t i = base + lane;
-        bool active = i >= i0 && i < i1;
+    while (base < i1) {
         r.prepare8();
-        uint32_t e = PAIR ? r.step_pair(lut, active) : r.step(lut, active);
-        if (active && store) put(p, e);
-        if (COUNT_ESC) esc += __popc(__ballot_sync(0xffffffffu, active && (e & 0xff) == 255));
-        base += 32; p += 32 * S;
-    }
-    while (base + 256 <= i1) {                       // eight full rounds per ring check
-        r.prepare8();
+        if (base >= i0 && base + 256 <= i1) {           // eight full rounds per ring check
 #pragma unroll
-        for (int k = 0; k < 8; k++) {
-            uint32_t e = PAIR ? r.step_pair_full(lut) : r.step_full(lut);
-            if (store) put(p + 32 * S * k, e);
-            if (COUNT_ESC) esc += __popc(__ballot_sync(0xffffffffu, (e & 0xff) == 255));
-        }
-        base += 256; p += 256 * S;
-    }
-    if (base < i1) {                                 // fewer than eight rounds left, the last may be ragged
-        r.prepare8();
-        for (; base < i1; base += 32, p += 32 * S) {
-            bool active = base + lane < i1;
-            uint32_t e = PAIR ? r.step_pair(lut, active) : r.step(lut, active);
-            if (active && store) put(p, e);
-            if (COUNT_ESC) esc += __popc(__ballot_sync(0xffffffffu, active && (e & 0xff) == 255));
+            for (int k = 0; k < 8; k++) {
+                uint32_t e = PAIR ? r.step_pair_full(lut) : r.step_full(lut);
+                if (store) put(p + 32 * S * k, e);
+                if (!PAIR) esc += __popc(__ballot_sync(0xffffffffu, (e & 0xff) == 255));
+            }
+            base += 256; p += 256 * S;
+        } else {                                       // ragged first round, or fewer than eight rounds left
+#pragma unroll 1
+            for (int k = 0; k < 8 && base < i1 && !(k && base + 256 <= i1); k++, base += 32, p += 32 * S) {   // back to the fast path after a ragged first round
+                const uint32_t i = base + lane;
+                const bool active = i >= i0 && i < i1;
+                uint32_t e = PAIR ? r.step_pair(lut, active) : r.step(lut, active);
+                if (active && store) put(p, e);
+                if (!PAIR) esc += __popc(__ballot_sync(0xffffffffu, active && (e & 0xff) == 255));
+            }
         }
     }
     return esc;

@@ -92,20 +92,27 @@ __device__ __forceinline__ uint64_t match_src(const Params& P, const SegCtx& c, 
     const uint8_t* rp = c.raw_planes + j;
     if (P.W <= 4) {                                          // files up to 4 GiB: 32-bit arithmetic
         uint32_t src = 0;
-        for (uint32_t k = 0; k < P.n_coded_planes; k++, cp += mc) src |= (uint32_t)__ldcg(cp) << P.coded_shift[k];
+        for (uint32_t k = 0; k < P.n_coded_planes; k++, cp += mc) src |= (uint32_t)*cp << P.coded_shift[k];
         for (uint32_t r = 0; r < P.n_raw_planes; r++, rp += c.d.n_match) src |= (uint32_t)__ldg(rp) << P.raw_shift[r];
         return src;
     }
     uint64_t src = 0;
-    for (uint32_t k = 0; k < P.n_coded_planes; k++, cp += mc) src |= (uint64_t)__ldcg(cp) << P.coded_shift[k];
+    for (uint32_t k = 0; k < P.n_coded_planes; k++, cp += mc) src |= (uint64_t)*cp << P.coded_shift[k];
     for (uint32_t r = 0; r < P.n_raw_planes; r++, rp += c.d.n_match) src |= (uint64_t)__ldg(rp) << P.raw_shift[r];
     return src;
 }
 
-// A1 (first part): the CMD, MLEN and coded OFF streams into the warp's scratch (TO_WS: the coded planes go straight to the
-// workspace of the match launch).  Leaves the rANS state at the first LITA symbol (global symbol index *i_lit).
-template <bool TO_WS>
-__device__ __forceinline__ void parse_tokens(const Params& P, uint32_t s_luts, uint32_t ring, SegCtx& c, Rans& r, uint32_t* i_lit) {
+__device__ __forceinline__ void literals_before(const Params& P, const SegCtx& c, uint64_t pend, uint32_t* n_a, uint32_t* n_q);
+
+// A1: the CMD, MLEN and coded OFF streams, then LITA, into the warp's scratch (TO_WS: the coded planes go straight to the
+// workspace of the match launch).  ONE instance of the byte decode loop serves all of them (instruction fetch).
+// UPTO (span service): only the literals in front of output position `pend` are decoded (LITQ follows LITA in the symbol
+// sequence, so needing any of it means decoding all of LITA), and LITQ in byte mode is one more region of the same loop
+// (bytes at lit_q; pair mode: 16-bit pairs at lit_q).  Leaves the rANS state behind the last symbol it decoded;
+// *i_next = index of the first LITQ symbol; *all = every symbol of the segment has been decoded.
+template <bool TO_WS, bool UPTO>
+__device__ __forceinline__ void parse_streams(const Params& P, uint32_t s_luts, uint32_t s_lutq, uint32_t ring, SegCtx& c, Rans& r, uint64_t pend,
+                                              uint32_t* i_next, bool* all) {
     uint32_t mc = TOK_STRIDE;
     c.off_planes = c.off_scratch; c.plane_stride = TOK_STRIDE;
     if (TO_WS) {
@@ -113,17 +120,29 @@ __device__ __forceinline__ void parse_tokens(const Params& P, uint32_t s_luts, u
         c.plane_stride = c.d.n_match; mc = c.d.n_match;
     }
     r.init(c.payload, c.d.n_words, ring);
-    uint32_t i0 = 0;
-    c.n_ext_cmd = rans_region<true>(r, s_luts + P.lut_cmd * (4 * LUT_SIZE), i0, c.d.n_cmd, c.tok_cmd); i0 += c.d.n_cmd;
-    rans_region<false>(r, s_luts + P.lut_mlen * (4 * LUT_SIZE), i0, c.d.n_match, c.tok_mlen); i0 += c.d.n_match;
-    uint32_t k = 0;
-    for (int p = (int)P.W - 1; p >= 0; p--) {
-        const int li = P.plane_lut[p];
-        if (li < 0) continue;
-        rans_region<false>(r, s_luts + li * (4 * LUT_SIZE), i0, c.d.n_match, c.off_planes + k * mc); i0 += c.d.n_match; k++;
+    uint32_t i0 = 0, na = c.d.n_lit_a, nq = UPTO ? c.d.n_sym_q : 0u;
+    const uint32_t n_tok = 2 + P.n_coded_planes, n_reg = n_tok + 1 + ((UPTO && !P.q_mode) ? 1u : 0u);
+#pragma unroll 1
+    for (uint32_t k = 0; k < n_reg; k++) {
+        uint32_t lut, cnt, adv; uint8_t* dst;
+        if (k == 0) { lut = P.lut_cmd; cnt = c.d.n_cmd; dst = c.tok_cmd; }
+        else if (k == 1) { lut = P.lut_mlen; cnt = c.d.n_match; dst = c.tok_mlen; }
+        else if (k < n_tok) { lut = P.coded_lut[k - 2]; cnt = c.d.n_match; dst = c.off_planes + (k - 2) * mc; }
+        else if (k == n_tok) {
+            __syncwarp();                                       // the tokens are complete: the scan below reads them
+            if (UPTO && pend < c.send) { literals_before(P, c, pend, &na, &nq); if (nq) na = c.d.n_lit_a; }
+            lut = P.lut_lita; cnt = na; dst = c.lit_a;
+        } else { lut = P.lut_litq; cnt = nq; dst = c.lit_q; }
+        adv = k == n_tok ? c.d.n_lit_a : cnt;
+        const uint32_t esc = rans_region<false>(r, s_luts + lut * (4 * LUT_SIZE), i0, cnt, dst);
+        if (k == 0) c.n_ext_cmd = esc;
+        i0 += adv;
+        if (UPTO && k == n_tok && nq == 0) break;               // nothing of LITQ is wanted
     }
+    if (UPTO && P.q_mode && nq) rans_region<true>(r, s_lutq, i0, nq, c.lit_q);
     __syncwarp();
-    *i_lit = i0;
+    *i_next = i0;
+    *all = na == c.d.n_lit_a && (UPTO ? nq == c.d.n_sym_q : c.d.n_sym_q == 0);
 }
 
 // FORMAT.md §1.7 integrity check once every symbol of the segment has been decoded
@@ -146,11 +165,17 @@ struct CmdLane {
 };
 __device__ __forceinline__ void scan_init(ScanState& st, const SegCtx& c) { st.lit_base = 0; st.out_base = 0; st.ec = 0; st.em = c.n_ext_cmd; }
 
-__device__ __forceinline__ CmdLane scan_step(const Params& P, const SegCtx& c, ScanState& st, uint32_t c0) {
+// the tokens of the group of 32 commands that starts at c0 (written by this warp earlier in the kernel: plain loads)
+__device__ __forceinline__ uint2 load_tokens(const SegCtx& c, uint32_t c0) {
+    const uint32_t ci = c0 + lane_id();
+    return make_uint2(ci < c.d.n_cmd ? c.tok_cmd[ci] : 0u, ci < c.d.n_match ? c.tok_mlen[ci] : 0u);
+}
+
+__device__ __forceinline__ CmdLane scan_step(const Params& P, const SegCtx& c, ScanState& st, uint32_t c0, uint2 tok) {
     const uint32_t lane = lane_id(), ci = c0 + lane;
     CmdLane L;
     L.valid = ci < c.d.n_cmd; L.has_match = ci < c.d.n_match;
-    const uint32_t tl = L.valid ? __ldcg(c.tok_cmd + ci) : 0u, tm = L.has_match ? __ldcg(c.tok_mlen + ci) : 0u;
+    const uint32_t tl = tok.x, tm = tok.y;
     const uint32_t ml = __ballot_sync(0xffffffffu, L.valid && tl == 255), mm = __ballot_sync(0xffffffffu, L.has_match && tm == 255);
     L.lit_len = tl; L.match_len = L.has_match ? P.min_match + tm : 0;
     if (L.valid && tl == 255) { const uint32_t k = st.ec + __popc(ml & lanemask_lt()); L.lit_len = k < c.d.n_ext ? 255 + __ldg(c.ext + k) : 0xffffffu; }
@@ -188,55 +213,81 @@ __device__ __forceinline__ bool scan_totals_ok(const SegCtx& c, const ScanState&
 }
 
 // ---- A2 + A3 fused into the literal decode ("direct placement") --------------------------------------------------
-// The command scan runs after LITA has been decoded into the warp's scratch and before LITQ is decoded:
+// The command scan runs after LITA has been decoded (into the warp's staging area in shared memory when it fits, else into
+// its scratch in global memory) and before LITQ is decoded:
 //  * LITA runs are short and many (bases between matches, header digits: 207 runs of 4.7 bytes per 16 KB of FASTQ): the lane
-//    that owns the command copies its run from the scratch to the output;
-//  * LITQ runs are long (quality strings): the scan leaves one table entry per run in shared memory,
-//    (last symbol index of the run) | odd_start << 15 | (delta + bias) << 16 | odd_end << 31, and the LITQ decode stores every
-//    symbol straight to its final position: while a 32-symbol round stays inside one run that is a pointer bump; a round
-//    that crosses run boundaries walks the table (one broadcast read per boundary);
+//    that owns the command copies its run to the output (8-byte loads, byte stores: the runs start anywhere);
+//  * LITQ runs are long (quality strings): the scan leaves one entry per run in the warp's run table in shared memory,
+//    (last symbol index of the run) | (delta + bias) << 16, and the LITQ decode stores every symbol straight to its final
+//    position: while a 32-symbol round stays inside one run that is a pointer bump; a round that crosses run boundaries
+//    walks the table (one broadcast read per boundary);
 //  * the match descriptors (dst_rel, len) go to the workspace for k_copy.
-constexpr uint32_t RUNS_CAP = 512;     // entries per warp (2 KB): at most 510 runs + sentinel
+// In pair mode a LITQ symbol is always stored as a whole aligned pair: inside a segment a literal run has a match (or the
+// segment's edge) on either side (a command is a run followed by its match, FORMAT.md §1.6), so the filler half of a run's
+// first / last pair lands on a match byte, which k_copy writes later.  Only symbol 0 and the last symbol can reach outside
+// the segment; q_edge says whether they do.
 constexpr uint32_t QDELTA_BIAS = 1024; // pair mode: delta = (even position of the run's first pair) - 2 * (first symbol) >= -2 * runs
 
-__device__ __forceinline__ bool build_runs(const Params& P, const SegCtx& c, uint32_t runs /* shared address */, uint8_t* out_seg) {
+__host__ __device__ inline uint32_t runs_bytes_for(uint32_t q_min) {   // run table of a warp: one entry per LITQ run + sentinel
+    const uint32_t n = q_min ? (MAX_SEG_LITS / q_min < MAX_SEG_CMDS ? MAX_SEG_LITS / q_min : MAX_SEG_CMDS) : 0;
+    return (4 * (n + 2) + 15) & ~15u;
+}
+
+__device__ __forceinline__ bool build_runs(const Params& P, const SegCtx& c, uint32_t runs /* shared address */, uint8_t* out_seg, uint32_t* q_edge_out) {
     ScanState st; scan_init(st, c);
-    uint32_t n_q = 0, q_bytes = 0;
+    uint32_t n_q = 0, q_bytes = 0, q_edge = 0;
     uint2* const pairs = P.pairs ? P.pairs + __ldg(P.match_prefix + c.s) : nullptr;
     const uint32_t lane = lane_id();
     const uint32_t even0 = (uint32_t)(c.sstart & 1);           // pair addressing is relative to the even position sstart - even0
+    const uint32_t slen = (uint32_t)(c.send - c.sstart), q_cap = P.runs_bytes / 4 - 1;
     bool good = true;
+    uint2 tok = load_tokens(c, 0);
     for (uint32_t c0 = 0; c0 < c.d.n_cmd; c0 += 32) {
-        const CmdLane L = scan_step(P, c, st, c0);
-        good = good && cmd_ok(P, c, L);
+        const uint2 tok_next = load_tokens(c, c0 + 32);        // in flight while this group is scanned
+        const CmdLane L = scan_step(P, c, st, c0, tok);
+        tok = tok_next;
+        const uint32_t mq = __ballot_sync(0xffffffffu, L.is_q);
+        good = good && cmd_ok(P, c, L) && n_q + __popc(mq) <= q_cap;
         if (__any_sync(0xffffffffu, !good)) break;
         if (pairs && L.has_match) pairs[c0 + lane] = make_uint2(L.out_rel + L.lit_len, L.match_len);
-        if (L.valid && !L.is_q && L.lit_len) {                 // a LITA run: this lane copies it (scratch is L2-resident)
-            const uint8_t* s = c.lit_a + L.lit_pos;
-            uint8_t* d = out_seg + L.out_rel;
-            if (L.lit_len <= 8) for (uint32_t i = 0; i < L.lit_len; i++) d[i] = __ldcg(s + i);
-            else copy_bytes<true>(d, s, L.lit_len);
+        const bool a_run = L.valid && !L.is_q && L.lit_len;
+        if (a_run && L.lit_len < 64) {
+            const uint8_t* sa = c.lit_a + L.lit_pos; uint8_t* da = out_seg + L.out_rel;
+            const uint32_t n0 = min(L.lit_len, 8u), n1 = min(L.lit_len - n0, 8u);
+            uint64_t v0 = ld64u<false>(sa, n0), v1 = n1 ? ld64u<false>(sa + 8, n1) : 0;
+#pragma unroll
+            for (int i = 0; i < 8; i++) { if ((uint32_t)i < n0) da[i] = (uint8_t)v0; v0 >>= 8; }
+            if (n1) {
+#pragma unroll
+                for (int i = 0; i < 8; i++) { if ((uint32_t)i < n1) da[8 + i] = (uint8_t)v1; v1 >>= 8; }
+            }
+            for (uint32_t i = 16; i < L.lit_len; i++) da[i] = sa[i];
         }
-        const uint32_t mq = __ballot_sync(0xffffffffu, L.is_q);
+        uint32_t a_long = __ballot_sync(0xffffffffu, a_run && L.lit_len >= 64);   // only archives without a LITQ class have them
+        while (a_long) {
+            const int l = __ffs(a_long) - 1; a_long &= a_long - 1;
+            warp_copy<false>(out_seg + __shfl_sync(0xffffffffu, L.out_rel, l), c.lit_a + __shfl_sync(0xffffffffu, L.lit_pos, l), __shfl_sync(0xffffffffu, L.lit_len, l));
+        }
         if (L.is_q) {
-            const uint32_t k = n_q + __popc(mq & lanemask_lt());
             uint32_t e;
             if (P.q_mode) {
                 const uint32_t d = L.out_rel + even0;          // position relative to the even base
-                e = ((L.lit_pos + L.q_syms - 1) & 0x7fffu) | (d & 1u) << 15 | (((d & ~1u) + QDELTA_BIAS - 2 * L.lit_pos) & 0x7fffu) << 16 |
-                    ((d + L.lit_len) & 1u) << 31;
+                e = ((L.lit_pos + L.q_syms - 1) & 0x7fffu) | (((d & ~1u) + QDELTA_BIAS - 2 * L.lit_pos) & 0x7fffu) << 16;
+                if (L.out_rel == 0 && even0) q_edge |= 1u;
+                if (L.out_rel + L.lit_len == slen && ((d + L.lit_len) & 1u)) q_edge |= 2u;
             } else e = ((L.lit_pos + L.lit_len - 1) & 0x7fffu) | ((L.out_rel - L.lit_pos) & 0x7fffu) << 16;
-            sts32(runs + 4 * k, e);
+            sts32(runs + 4 * (n_q + __popc(mq & lanemask_lt())), e);
             q_bytes += L.lit_len;
         }
         n_q += __popc(mq);
     }
 #pragma unroll
-    for (int o = 16; o >= 1; o >>= 1) q_bytes += __shfl_xor_sync(0xffffffffu, q_bytes, o);
+    for (int o = 16; o >= 1; o >>= 1) { q_bytes += __shfl_xor_sync(0xffffffffu, q_bytes, o); q_edge |= __shfl_xor_sync(0xffffffffu, q_edge, o); }
     good = !__any_sync(0xffffffffu, !good) && scan_totals_ok(c, st) && q_bytes == c.d.n_lit_q;
     if (!good) { if (lane == 0) report(P, DF_LENGTH); return false; }
     if (lane == 0) sts32(runs + 4 * n_q, 0x7fffu);             // sentinel
     __syncwarp();
+    *q_edge_out = q_edge;
     return true;
 }
 
@@ -244,138 +295,89 @@ struct RunCursor {
     uint32_t k;          // shared address of the entry of the run that holds the first symbol of the coming round
     uint32_t last;       // last symbol index of that run
     uint32_t delta;      // out position - symbol position (pair mode: biased, in bytes from the even base)
-    uint32_t first;      // first symbol index of that run
-    uint32_t flags;      // pair mode: bit 0 = odd start, bit 1 = odd end
-    bool edge;           // pair mode: the coming round starts with the first symbol of an odd-start run
-    __device__ __forceinline__ void load(uint32_t e) { last = e & 0x7fffu; delta = (e >> 16) & 0x7fffu; flags = ((e >> 15) & 1u) | ((e >> 30) & 2u); }
-};
-
-// LITQ in byte mode: symbol j of the stream goes to out_seg[j + delta(run of j)].
-__device__ __forceinline__ void decode_q_bytes(Rans& r, uint32_t lut, uint32_t i0, uint32_t n, uint32_t runs, uint8_t* out_seg) {
-    if (n == 0) return;
-    const uint32_t lane = lane_id(), i1 = i0 + n;
-    RunCursor rc; rc.k = runs; rc.load(lds32(runs)); rc.first = 0;
-    // a round whose symbols [.., j_hi] are not all strictly inside run k: walk the cursor over the runs that end inside the
-    // round; returns the delta of this lane's symbol j and leaves the cursor on the run of symbol j_hi + 1
-    auto walk = [&](uint32_t j, uint32_t j_hi) -> uint32_t {
-        uint32_t mine = rc.delta;
-        while (rc.last <= j_hi) {
-            const uint32_t prev = rc.last;
-            rc.k += 4; rc.load(lds32(rc.k));
-            if (j > prev) mine = rc.delta;
+    __device__ __forceinline__ void load(uint32_t e) { last = e & 0x7fffu; delta = (e >> 16) & 0x7fffu; }
+    // A round whose symbols [.., j_hi] are not all strictly inside run k: walk the cursor over the runs that end inside the
+    // round (one broadcast table read per boundary; the table ends with a sentinel whose `last` is 0x7fff).  Returns the
+    // delta of this lane's symbol j and leaves the cursor on the run of symbol j_hi + 1.
+    __device__ __forceinline__ uint32_t walk(uint32_t j, uint32_t j_hi) {
+        uint32_t mine = delta;
+        while (last <= j_hi) {
+            const uint32_t prev = last;
+            k += 4; load(lds32(k));
+            if (j > prev) mine = delta;
         }
         return mine;
-    };
-    uint32_t base = i0 & ~31u;
-    if (base != i0) {                                     // ragged first round
-        const uint32_t i = base + lane;
-        const bool active = i >= i0 && i < i1;
-        r.prepare8();
-        const uint32_t e = r.step(lut, active);
-        const uint32_t d = walk(i - i0, min(base + 31, i1 - 1) - i0);
-        if (active) out_seg[d + (i - i0)] = (uint8_t)e;
-        base += 32;
     }
-    uint8_t* pj = out_seg + (int64_t)((int64_t)base + lane - i0);      // address of symbol (base + lane - i0) if delta were 0
-    while (base + 256 <= i1) {                            // eight full rounds per ring check
-        r.prepare8();
-        uint8_t* pd = pj + rc.delta;
-#pragma unroll
-        for (int q = 0; q < 8; q++) {
-            const uint32_t e = r.step_full(lut);
-            const uint32_t j_hi = base + 32 * q + 31 - i0;
-            if (j_hi < rc.last) pd[32 * q] = (uint8_t)e;   // the whole round lies strictly inside run k: pointer bump
-            else { const uint32_t d = walk(j_hi - 31 + lane, j_hi); pj[32 * q + d] = (uint8_t)e; pd = pj + rc.delta; }
-        }
-        base += 256; pj += 256;
-    }
-    if (base < i1) {                                      // fewer than eight rounds left, the last may be ragged
-        r.prepare8();
-        for (; base < i1; base += 32) {
-            const bool active = base + lane < i1;
-            const uint32_t e = r.step(lut, active);
-            const uint32_t d = walk(base + lane - i0, min(base + 31, i1 - 1) - i0);
-            if (active) out_seg[d + (base + lane - i0)] = (uint8_t)e;
-        }
-    }
-}
+};
 
-// LITQ in pair mode (FORMAT.md §1.7): symbol j of the stream is the pair at the even position even_base + 2 j + delta - bias;
-// the halves that lie outside the run (odd start / odd end) are dropped.  ODD: the output address of an even position is
-// odd (a range-decode window placed at an odd address): byte stores only.
-template <bool ODD>
-__device__ __forceinline__ void decode_q_pairs(Rans& r, uint32_t lutq, uint32_t i0, uint32_t n, uint32_t runs, uint8_t* even_base) {
+// LITQ straight to its positions.  PAIR = false: symbol j of the stream is the byte at zero + j + delta(run of j).
+// PAIR = true (FORMAT.md §1.7): symbol j is the aligned pair at zero + 2 j + delta(run of j), stored whole (see above)
+// except for the halves of symbol 0 / symbol n - 1 that q_edge says lie outside the segment.  ODD: the output address of an
+// even position is odd (a range-decode window placed at an odd address): two byte stores instead of one 16-bit store.
+template <bool PAIR, bool ODD>
+__device__ __forceinline__ void decode_q(Rans& r, uint32_t lut, uint32_t i0, uint32_t n, uint32_t runs, uint8_t* zero, uint32_t q_edge) {
     if (n == 0) return;
+    constexpr uint32_t S = PAIR ? 2 : 1;
     const uint32_t lane = lane_id(), i1 = i0 + n;
-    RunCursor rc; rc.k = runs; rc.load(lds32(runs)); rc.first = 0; rc.edge = rc.flags & 1u;
-    uint8_t* const zero = even_base - QDELTA_BIAS;        // address of symbol 0 if delta were 0
-    auto put_full = [&](uint8_t* p, uint32_t e) {
-        if (ODD) { p[0] = (uint8_t)e; p[1] = (uint8_t)(e >> 8); } else *reinterpret_cast<uint16_t*>(p) = (uint16_t)e;
+    RunCursor rc; rc.k = runs; rc.load(lds32(runs));
+    auto put = [&](uint8_t* p, uint32_t e) {
+        if (!PAIR) *p = (uint8_t)e;
+        else if (ODD) { p[0] = (uint8_t)e; p[1] = (uint8_t)(e >> 8); }
+        else *reinterpret_cast<uint16_t*>(p) = (uint16_t)e;
     };
-    // slow path of a round: every lane finds the run of its symbol j, stores what lies inside the run
-    auto slow = [&](uint32_t j, uint32_t j_hi, bool active, uint32_t e) {
-        uint32_t m_last = rc.last, m_delta = rc.delta, m_first = rc.first, m_flags = rc.flags;
-        while (rc.last <= j_hi) {
-            const uint32_t prev = rc.last;
-            rc.k += 4; rc.load(lds32(rc.k)); rc.first = prev + 1;
-            if (j > prev) { m_last = rc.last; m_delta = rc.delta; m_first = rc.first; m_flags = rc.flags; }
-        }
-        rc.edge = (rc.flags & 1u) && rc.first > j_hi;      // the next round starts with the first symbol of an odd-start run
-        if (active) {
-            uint8_t* p = zero + 2 * j + m_delta;
-            const bool lo = !((m_flags & 1u) && j == m_first), hi = !((m_flags & 2u) && j == m_last);
-            if (lo && hi) put_full(p, e);
-            else { if (lo) p[0] = (uint8_t)e; if (hi) p[1] = (uint8_t)(e >> 8); }
-        }
+    // a round that may hold a run boundary, an inactive lane, symbol 0 or the last symbol
+    auto careful = [&](uint32_t j, uint32_t j_hi, bool active, uint32_t e) {
+        uint8_t* p = zero + S * j + rc.walk(j, j_hi);
+        if (!active) return;
+        if (PAIR && ((j == 0 && (q_edge & 1u)) || (j == n - 1 && (q_edge & 2u)))) { if (j == 0 && (q_edge & 1u)) p[1] = (uint8_t)(e >> 8); else p[0] = (uint8_t)e; }
+        else put(p, e);
     };
     uint32_t base = i0 & ~31u;
-    if (base != i0) {                                     // ragged first round
-        const uint32_t i = base + lane;
-        const bool active = i >= i0 && i < i1;
+    uint8_t* pj = zero + (int64_t)S * ((int64_t)base + lane - i0);      // address of symbol (base + lane - i0) if delta were 0
+#pragma unroll 1
+    while (base < i1) {
         r.prepare8();
-        const uint32_t e = r.step_pair(lutq, active);
-        slow(i - i0, min(base + 31, i1 - 1) - i0, active, e);
-        base += 32;
-    }
-    uint8_t* pj = zero + 2 * (int64_t)((int64_t)base + lane - i0);
-    while (base + 256 <= i1) {                            // eight full rounds per ring check
-        r.prepare8();
-        uint8_t* pd = pj + rc.delta;
+        if (base > i0 && base + 256 < i1) {               // eight full rounds, none of them the first or the last of the stream
+#pragma unroll 1
+            for (int h = 0; h < 2; h++) {                 // two groups of four (code size)
+                uint8_t* pd = pj + rc.delta;
 #pragma unroll
-        for (int q = 0; q < 8; q++) {
-            const uint32_t e = r.step_pair_full(lutq);
-            const uint32_t j_hi = base + 32 * q + 31 - i0;
-            if (j_hi < rc.last && !rc.edge) put_full(pd + 64 * q, e);      // strictly inside run k, no edge symbol: pointer bump
-            else { slow(j_hi - 31 + lane, j_hi, true, e); pd = pj + rc.delta; }
-        }
-        base += 256; pj += 512;
-    }
-    if (base < i1) {                                      // fewer than eight rounds left, the last may be ragged
-        r.prepare8();
-        for (; base < i1; base += 32) {
-            const bool active = base + lane < i1;
-            const uint32_t e = r.step_pair(lutq, active);
-            slow(base + lane - i0, min(base + 31, i1 - 1) - i0, active, e);
+                for (int q = 0; q < 4; q++) {
+                    const uint32_t e = PAIR ? r.step_pair_full(lut) : r.step_full(lut);
+                    const uint32_t j_hi = base + 32 * q + 31 - i0;
+                    if (j_hi < rc.last) put(pd + 32 * S * q, e);       // the whole round lies strictly inside run k: pointer bump
+                    else { put(pj + 32 * S * q + rc.walk(j_hi - 31 + lane, j_hi), e); pd = pj + rc.delta; }
+                }
+                base += 128; pj += 128 * S;
+            }
+        } else {
+#pragma unroll 1
+            for (int k = 0; k < 8 && base < i1 && !(k && base + 256 < i1); k++, base += 32, pj += 32 * S) {
+                const uint32_t i = base + lane;
+                const bool active = i >= i0 && i < i1;
+                const uint32_t e = PAIR ? r.step_pair(lut, active) : r.step(lut, active);
+                careful(i - i0, min(base + 31, i1 - 1) - i0, active, e);
+            }
         }
     }
 }
 
-// A1 + A2 + A3 for one segment: tokens, LITA into the scratch, scan (LITA placement, LITQ run table, match descriptors),
-// LITQ straight to its positions.  out_seg = address of the segment's first output byte.
-__device__ __forceinline__ bool literals_of_segment(const Params& P, uint32_t s_luts, uint32_t s_lutq, uint32_t ring, uint32_t runs, SegCtx& c) {
+// A1 + A2 + A3 for one segment: tokens and LITA, scan (LITA placement, LITQ run table, match descriptors), LITQ straight to
+// its positions.  QM: 0 = LITQ bytes, 1 = aligned pairs, 2 = pairs at an odd address.  lita_stage: the warp's staging area
+// in shared memory (generic pointer); a segment with more LITA bytes than it holds stages them in the global scratch.
+template <int QM>
+__device__ __forceinline__ bool literals_of_segment(const Params& P, uint32_t s_luts, uint32_t s_lutq, uint32_t ring, uint32_t runs, uint8_t* lita_stage, SegCtx& c) {
     if (!load_seg(P, c)) return false;
     uint8_t* const out_seg = P.out + (c.sstart - P.out_pos0);
-    Rans r; uint32_t i0;
-    parse_tokens<true>(P, s_luts, ring, c, r, &i0);
-    rans_region<false>(r, s_luts + P.lut_lita * (4 * LUT_SIZE), i0, c.d.n_lit_a, c.lit_a);
-    __syncwarp();
-    if (!build_runs(P, c, runs, out_seg)) return false;
-    i0 += c.d.n_lit_a;
-    if (P.q_mode) {
-        uint8_t* const even_base = out_seg - (c.sstart & 1);
-        if (P.out_odd) decode_q_pairs<true>(r, s_lutq, i0, c.d.n_sym_q, runs, even_base);
-        else decode_q_pairs<false>(r, s_lutq, i0, c.d.n_sym_q, runs, even_base);
-    } else decode_q_bytes(r, s_luts + P.lut_litq * (4 * LUT_SIZE), i0, c.d.n_sym_q, runs, out_seg);
+    uint8_t* const lit_a_scratch = c.lit_a;
+    if (c.d.n_lit_a <= P.lita_bytes) c.lit_a = lita_stage;
+    Rans r; uint32_t i0, q_edge; bool all;
+    parse_streams<true, false>(P, s_luts, s_lutq, ring, c, r, 0, &i0, &all);
+    const bool ok = build_runs(P, c, runs, out_seg, &q_edge);
+    c.lit_a = lit_a_scratch;
+    if (!ok) return false;
+    if (QM == 0) decode_q<false, false>(r, s_luts + P.lut_litq * (4 * LUT_SIZE), i0, c.d.n_sym_q, runs, out_seg, 0);
+    else decode_q<true, QM == 2>(r, s_lutq, i0, c.d.n_sym_q, runs, out_seg - (c.sstart & 1) - QDELTA_BIAS, q_edge);
     return rans_final_ok(P, r);
 }
 
@@ -694,7 +696,7 @@ __device__ __forceinline__ void literals_before(const Params& P, const SegCtx& c
     ScanState st; scan_init(st, c);
     uint32_t a = 0, q = 0;
     for (uint32_t c0 = 0; c0 < c.d.n_cmd && c.sstart + st.out_base < pend; c0 += 32) {
-        const CmdLane L = scan_step(P, c, st, c0);
+        const CmdLane L = scan_step(P, c, st, c0, load_tokens(c, c0));
         const bool in = L.valid && c.sstart + L.out_rel < pend;
         a += (in && !L.is_q) ? min(L.lit_len, 0xffffu) : 0u; q += in ? L.q_syms : 0u;
     }
@@ -707,19 +709,10 @@ __device__ __forceinline__ void literals_before(const Params& P, const SegCtx& c
 // bytes, or 16-bit pairs, at lit_q).  LITQ follows LITA in the symbol sequence, so needing any of it means decoding all of LITA.
 __device__ __forceinline__ bool parse_segment_upto(const Params& P, uint32_t s_luts, uint32_t s_lutq, uint32_t ring, SegCtx& c, uint64_t pend) {
     if (!load_seg(P, c)) return false;
-    Rans r; uint32_t i0;
-    parse_tokens<false>(P, s_luts, ring, c, r, &i0);
-    uint32_t na = c.d.n_lit_a, nq = c.d.n_sym_q;
-    if (pend < c.send) literals_before(P, c, pend, &na, &nq);
-    if (nq) na = c.d.n_lit_a;
-    rans_region<false>(r, s_luts + P.lut_lita * (4 * LUT_SIZE), i0, na, c.lit_a);
-    i0 += c.d.n_lit_a;
-    if (nq) {
-        if (P.q_mode) rans_region<false, true>(r, s_lutq, i0, nq, c.lit_q);
-        else rans_region<false>(r, s_luts + P.lut_litq * (4 * LUT_SIZE), i0, nq, c.lit_q);
-    }
+    Rans r; uint32_t i0; bool all;
+    parse_streams<false, true>(P, s_luts, s_lutq, ring, c, r, pend, &i0, &all);
     bool ok = true;
-    if (na == c.d.n_lit_a && nq == c.d.n_sym_q) ok = rans_final_ok(P, r);
+    if (all) ok = rans_final_ok(P, r);
     cp_async_wait_group<0>();          // the ring is reused as table space by the callers
     __syncwarp();
     return ok;
@@ -727,17 +720,17 @@ __device__ __forceinline__ bool parse_segment_upto(const Params& P, uint32_t s_l
 
 // byte at absolute position p of a literal run of the parsed segment (run at absolute position d, lit_pos in its stream)
 __device__ __forceinline__ uint32_t lit_byte(const Params& P, const SegCtx& c, bool is_q, uint32_t lit_pos, uint64_t d, uint64_t p) {
-    if (!is_q) return __ldcg(c.lit_a + lit_pos + (p - d));
-    if (!P.q_mode) return __ldcg(c.lit_q + lit_pos + (p - d));
+    if (!is_q) return c.lit_a[lit_pos + (p - d)];
+    if (!P.q_mode) return c.lit_q[lit_pos + (p - d)];
     const uint32_t sym = lit_pos + (uint32_t)((p >> 1) - (d >> 1));
-    return __ldcg(c.lit_q + 2ull * sym + (p & 1));
+    return c.lit_q[2ull * sym + (p & 1)];
 }
 // bytes [a, b) of that run -> dptr
 __device__ __forceinline__ void copy_lit(const Params& P, const SegCtx& c, bool is_q, uint32_t lit_pos, uint64_t d, uint64_t a, uint64_t b, uint8_t* dptr) {
-    if (!is_q) { copy_bytes<true>(dptr, c.lit_a + lit_pos + (a - d), (uint32_t)(b - a)); return; }
-    if (!P.q_mode) { copy_bytes<true>(dptr, c.lit_q + lit_pos + (a - d), (uint32_t)(b - a)); return; }
+    if (!is_q) { copy_bytes<false>(dptr, c.lit_a + lit_pos + (a - d), (uint32_t)(b - a)); return; }
+    if (!P.q_mode) { copy_bytes<false>(dptr, c.lit_q + lit_pos + (a - d), (uint32_t)(b - a)); return; }
     // pairs in the scratch sit at even positions of the OUTPUT: byte p of the run is byte (p - (d & ~1)) of the pair array
-    copy_bytes<true>(dptr, c.lit_q + 2ull * lit_pos + (a - (d & ~1ull)), (uint32_t)(b - a));
+    copy_bytes<false>(dptr, c.lit_q + 2ull * lit_pos + (a - (d & ~1ull)), (uint32_t)(b - a));
 }
 
 // the piece [a, b) (absolute positions) of command L (literal run at absolute position o0) -> out2[dst + (x - pos)]
@@ -767,7 +760,7 @@ __device__ __forceinline__ void emit_span(const Params& P, const SegCtx& c, cons
     ScanState ss; scan_init(ss, c);
     const uint64_t pend = pos + len;
     for (uint32_t c0 = 0; c0 < c.d.n_cmd; c0 += 32) {
-        const CmdLane L = scan_step(P, c, ss, c0);
+        const CmdLane L = scan_step(P, c, ss, c0, load_tokens(c, c0));
         if (__any_sync(0xffffffffu, !cmd_ok(P, c, L))) { if (lane_id() == 0) report(P, DF_LENGTH); return; }
         if (c.sstart + ss.out_base <= pos) continue;         // the whole group lies before the span
         if (L.valid) emit_cmd_piece(P, c, st, L.is_q, L.lit_pos, c.sstart + L.out_rel, L.lit_len, L.match_len, L.has_match, c0 + lane_id(), pos, pend, dst);
@@ -782,7 +775,7 @@ __device__ __forceinline__ bool build_cmd_table(const Params& P, const SegCtx& c
     ScanState st; scan_init(st, c);
     bool good = true;
     for (uint32_t c0 = 0; c0 < c.d.n_cmd; c0 += 32) {
-        const CmdLane L = scan_step(P, c, st, c0);
+        const CmdLane L = scan_step(P, c, st, c0, load_tokens(c, c0));
         good = good && cmd_ok(P, c, L) && L.lit_len <= MAX_SEG_LITS;
         if (__any_sync(0xffffffffu, !good)) { if (lane_id() == 0) report(P, DF_LENGTH); return false; }
         if (L.valid) {
@@ -865,16 +858,18 @@ __device__ __forceinline__ void process_demands(const Params& P, uint32_t s_luts
 }
 
 // shared memory of the entropy kernels: [byte tables: n_coded_tables x 8 KB][pair table: 32 KB when q_mode = 1]
-// [rings: warps x 2 KB][run tables: warps x 2 KB][stack tops: warps x 4]   (absolute shared addresses)
-struct CtaSmem { uint32_t luts, lutq, ring, runs, top; };
+// [rings: warps x 2 KB][per warp: run table | LITA staging][stack tops: warps x 4]   (absolute shared addresses).
+// The span-service kernels use the per-warp area as one command table (2 KB at least).
+struct CtaSmem { uint32_t luts, lutq, ring, runs, top; uint8_t* lita; };
 
-__host__ __device__ inline size_t entropy_smem(uint32_t n_coded_tables, uint32_t q_mode, int threads) {
-    return (size_t)n_coded_tables * LUT_SIZE * 4 + (q_mode ? (size_t)QLUT_SIZE * 8 : 0) + (size_t)(threads / 32) * (RING_BYTES + 4 * RUNS_CAP + 4) + 16;
+__host__ __device__ inline size_t entropy_smem(uint32_t n_coded_tables, uint32_t q_mode, uint32_t warp_area, int threads) {
+    return (size_t)n_coded_tables * LUT_SIZE * 4 + (q_mode ? (size_t)QLUT_SIZE * 8 : 0) + (size_t)(threads / 32) * (RING_BYTES + warp_area + 4) + 128;
 }
 
 __device__ __forceinline__ CtaSmem setup_cta(const Params& P, uint8_t* smem_raw) {
-    const uint32_t smem0 = ((uint32_t)__cvta_generic_to_shared(smem_raw) + 15u) & ~15u;
-    uint8_t* base_ptr = smem_raw + (smem0 - (uint32_t)__cvta_generic_to_shared(smem_raw));
+    const uint32_t raw0 = (uint32_t)__cvta_generic_to_shared(smem_raw);
+    const uint32_t smem0 = (raw0 + 15u) & ~15u;
+    uint8_t* base_ptr = smem_raw + (smem0 - raw0);
     const uint32_t n_lut_words = P.n_coded_tables * LUT_SIZE;
     {
         uint4* dstv = reinterpret_cast<uint4*>(base_ptr);
@@ -885,14 +880,16 @@ __device__ __forceinline__ CtaSmem setup_cta(const Params& P, uint8_t* smem_raw)
         }
     }
     __syncthreads();
-    const uint32_t warp = threadIdx.x >> 5, warps = blockDim.x >> 5;
+    const uint32_t warp = threadIdx.x >> 5, warps = blockDim.x >> 5, area = P.runs_bytes + P.lita_bytes;
     CtaSmem m;
     m.luts = smem0;
     m.lutq = smem0 + n_lut_words * 4;
     uint32_t base = m.lutq + (P.q_mode ? QLUT_SIZE * 8 : 0);
     base = (base + 63u) & ~63u;                                // rings are 64-byte aligned (ring | slot)
     m.ring = base + warp * RING_BYTES; base += warps * RING_BYTES;
-    m.runs = base + warp * (4 * RUNS_CAP); base += warps * (4 * RUNS_CAP);
+    m.runs = base + warp * area;
+    m.lita = smem_raw + (m.runs + P.runs_bytes - raw0);
+    base += warps * area;
     m.top = base + 4 * warp;
     return m;
 }
@@ -911,6 +908,7 @@ __device__ __forceinline__ bool next_ticket(const Params& P, unsigned long long&
 }
 
 // The literal launch: A1 + A2 + A3 for every segment of the work list, no dependencies.
+template <int QM>
 __global__ void __launch_bounds__(1024, 1) k_literals(const Params P) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
     clear_next_ticket(P);
@@ -920,7 +918,7 @@ __global__ void __launch_bounds__(1024, 1) k_literals(const Params P) {
     unsigned long long t;
     while (next_ticket(P, t)) {
         c.s = P.seg_list ? (uint64_t)P.seg_list[t] : P.first_work + t;
-        literals_of_segment(P, m.luts, m.lutq, m.ring, m.runs, c);
+        literals_of_segment<QM>(P, m.luts, m.lutq, m.ring, m.runs, m.lita, c);
     }
 }
 
@@ -936,6 +934,7 @@ __global__ void __launch_bounds__(1024, 1) k_copy(const Params P) {
 // every segment, a grid-wide barrier, then the match waves: one flag-driven pass over the segments below the top level
 // (when there are any) and one wait-free pass over the top level.  tickets[0..2] are zero at launch.
 struct FusedArgs { uint64_t n_low, n_top; const uint32_t* low_list; const uint32_t* top_list; unsigned long long* tickets; };
+template <int QM>
 __global__ void __launch_bounds__(1024, 1) k_fused(Params P, const FusedArgs F) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
     cooperative_groups::grid_group grid = cooperative_groups::this_grid();
@@ -945,7 +944,7 @@ __global__ void __launch_bounds__(1024, 1) k_fused(Params P, const FusedArgs F) 
         bind_scratch(P, blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), c);
         P.ticket = F.tickets; P.seg_list = nullptr; P.first_work = 0; P.n_work = P.n_segs;
         unsigned long long t;
-        while (next_ticket(P, t)) { c.s = t; literals_of_segment(P, m.luts, m.lutq, m.ring, m.runs, c); }
+        while (next_ticket(P, t)) { c.s = t; literals_of_segment<QM>(P, m.luts, m.lutq, m.ring, m.runs, m.lita, c); }
     }
     __threadfence();
     grid.sync();

@@ -147,6 +147,12 @@ HAND = [
     ([[(b"abc", (0, 10)), (b"XYZ", None)], [(b"", (1, 9)), (b"0123456", None)]], 32, 4, dict(levels=[0, 1])),
     ([[(b"01234567", None)], [(b"89ab", (6, 4))], [(b"", (6, 5)), (b"!!!", None)]], 24, 3, {}),
     ([[(b"ABCDEFGH", None)], [(b"", (0, 8))], [(b"", (8, 8))]], 24, 3, dict(levels=[0, 0, 1])),
+    ([[[(b"ABCDEFGHIJ", None)], [(b"KL", (0, 3)), (b"mn", (2, 4))], [(b"", (8, 4)), (b"wxyz123", None)]], [(b"", (0, 8))]], 40, 5,
+     dict(log2_seg=3, min_match=2)),
+    ([[(b"a" + bytes(range(98, 98 + 30)) + b"~", None)], [(b"p", (0, 2)), (b"HIJKL", (35, 2)), (b"MNOPQ", (0, 2)), (b"xyzw", None)]], 53, 5,
+     dict(min_match=2, q_min=4, q_mode=1)),
+    ([[(b"a" + bytes(range(98, 98 + 30)) + b"~", None)], [(b"p", (0, 2)), (b"HIJKL", (35, 2)), (b"MNOPQ", (0, 2)), (b"xyzw", None)]], 53, 5,
+     dict(min_match=2, q_min=4, q_mode=0)),
 ]
 
 
@@ -188,16 +194,35 @@ def test_large_windows_with_foreign_sources(big):
             check_range(ar, x, lo, min(hi, N))
 
 
-def test_large_windows_token_path(monkeypatch):
-    """ACEAPEX_WIN_TOKENS=1 (read at open): the collect and match launches of a window re-decode the block's tokens
-    (k_matches) instead of reading the descriptors the literal launch left (k_copy); same bytes either way."""
+@pytest.mark.parametrize("kw", [dict(max_level=3), dict(max_level=2, q_mode=0), dict(block_size=1 << 20, max_level=3), dict(block_size=65536),
+                                dict(block_size=4096, q_min=0), dict(block_size=1 << 18, log2_seg=12, max_level=1)])
+def test_large_windows_levels_and_segments(kw):
+    """Archives with dependency levels (demand rounds recurse, the window's match launch is flag-driven) and with several
+    segments per block: windows, ragged ends, reads; also a window placed at an ODD device address (pair stores fall back
+    to byte stores)."""
     from paper_2606_18900_b200 import datagen, encoder
     from paper_2606_18900_b200.aceapex import Archive
-    monkeypatch.setenv("ACEAPEX_WIN_TOKENS", "1")
     x = datagen.fastq(7, 6 << 20, 300_000)
-    ar = Archive(encoder.encode(x, block_size=16384))
-    for lo, hi in ((100 * 16384, 380 * 16384), (x.size - 300 * 16384 - 5, x.size), (0, 256 * 16384)):
+    ar = Archive(encoder.encode(x, **kw))
+    for lo, hi in ((100 * 16384, 380 * 16384), (x.size - 300 * 16384 - 5, x.size), (0, 256 * 16384), (1 << 20, (1 << 20) + 1), (3_000_001, 5_500_003)):
         check_range(ar, x, lo, hi)
+    buf = ar.new_output((2 << 20) + 64)
+    for shift in (1, 3, 8):
+        lo, hi = (2 << 20) + 5, (4 << 20) + 5
+        got = ar.decode_range(lo, hi, out=buf[shift:])
+        ar.check()
+        assert got.cpu().numpy().tobytes() == x[lo:hi].tobytes(), shift
+    idx = datagen.fastq_index(x.size)
+    rng = np.random.default_rng(3)
+    off, ln = (idx & np.uint64((1 << 40) - 1)).astype(np.int64), (idx >> np.uint64(40)).astype(np.int64)
+    for n in (1, 40, 3000):
+        ids = rng.integers(0, idx.size, n).astype(np.uint64)
+        got = ar.decode_reads(idx, ids).cpu().numpy()
+        ar.check()
+        _, offs = ar.reads_bytes(idx, ids)
+        for k in range(0, n, 7):
+            r = int(ids[k])
+            assert got[int(offs[k]):int(offs[k]) + ln[r]].tobytes() == x[off[r]:off[r] + ln[r]].tobytes(), (n, k)
     ar.close()
 
 
