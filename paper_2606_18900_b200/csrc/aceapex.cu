@@ -188,9 +188,10 @@ int32_t launch(aceapex_archive* ar, Params& P, Kind kind, uint64_t n_work) {
     const size_t sm_e = entropy_smem(ar->n_coded_tables, ar->q_mode, ar->runs_bytes + ar->lita_bytes, T), sm_c = (size_t)(T / 32) * COPY_WARP_BYTES + 64;
     switch (kind) {
         case K_LIT:
-            if (!ar->q_mode) k_literals<0><<<g, T, sm_e, ar->stream>>>(P);
-            else if (!P.out_odd) k_literals<1><<<g, T, sm_e, ar->stream>>>(P);
-            else k_literals<2><<<g, T, sm_e, ar->stream>>>(P);
+            if (!ar->q_mode) { if (ar->q_min >= 64) k_literals<3><<<g, T, sm_e, ar->stream>>>(P); else k_literals<0><<<g, T, sm_e, ar->stream>>>(P); }
+            else if (P.out_odd) k_literals<2><<<g, T, sm_e, ar->stream>>>(P);
+            else if (ar->q_min >= 64) k_literals<4><<<g, T, sm_e, ar->stream>>>(P);
+            else k_literals<1><<<g, T, sm_e, ar->stream>>>(P);
             break;
         case K_COPY_TOP: k_copy<false, false, false, true><<<g, T, sm_c, ar->stream>>>(P); break;
         case K_COPY_WAIT: k_copy<true, false, false, false><<<g, T, sm_c, ar->stream>>>(P); break;
@@ -398,7 +399,8 @@ int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* 
     ar->smem_copy = (size_t)(ar->threads / 32) * COPY_WARP_BYTES + 64;
     ar->smem_fused = std::max(ar->smem_entropy, ar->smem_copy);
     {
-        const void* fns[] = {(const void*)k_literals<0>, (const void*)k_literals<1>, (const void*)k_literals<2>, (const void*)k_fused<0>, (const void*)k_fused<1>,
+        const void* fns[] = {(const void*)k_literals<0>, (const void*)k_literals<1>, (const void*)k_literals<2>, (const void*)k_literals<3>, (const void*)k_literals<4>,
+                             (const void*)k_fused<0>, (const void*)k_fused<1>, (const void*)k_fused<3>, (const void*)k_fused<4>,
                              (const void*)k_copy<false, false, false, true>, (const void*)k_copy<true, false, false, false>,
                              (const void*)k_copy<false, true, false, false>, (const void*)k_copy<true, true, false, false>, (const void*)k_copy<false, true, true, false>,
                              (const void*)k_serve, (const void*)k_spans, (const void*)k_rounds};
@@ -548,7 +550,8 @@ int32_t aceapex_decode_all_fused(aceapex_archive* ar, void* d_out) {
     CU(cudaMemsetAsync(F.tickets, 0, 32, ar->stream));
     if (F.n_low && (rc = zero_done(ar, 0, ar->n_blocks))) return rc;
     void* args[] = {&P, &F};
-    CU(cudaLaunchCooperativeKernel(ar->q_mode ? (const void*)k_fused<1> : (const void*)k_fused<0>, dim3(ar->sms), dim3(ar->threads), args, ar->smem_fused, ar->stream));
+    const void* kf = ar->q_mode ? (ar->q_min >= 64 ? (const void*)k_fused<4> : (const void*)k_fused<1>) : (ar->q_min >= 64 ? (const void*)k_fused<3> : (const void*)k_fused<0>);
+    CU(cudaLaunchCooperativeKernel(kf, dim3(ar->sms), dim3(ar->threads), args, ar->smem_fused, ar->stream));
     ar->launches++;
     return ACEAPEX_OK;
 }

@@ -129,6 +129,7 @@ struct Rans {
     uint32_t fp;             // bytes of the stream requested into the ring so far (relative to gbase, multiple of 16)
     uint32_t ring;           // shared address of this lane's ring, 64-byte aligned
     uint32_t end;            // rp after the lane's last word (integrity check)
+    uint32_t w;              // the word at rp, read ahead: a renormalisation does not wait for shared memory
     const uint8_t* gbase;    // 16-byte aligned global address that offsets are relative to
 
     __device__ __forceinline__ void fetch() { cp_async16s(ring | (fp & 63), gbase + fp); fp += 16; }
@@ -149,16 +150,19 @@ struct Rans {
         ring = ring_warp + 64u * lane;
         cp_async_wait_group<0>();            // chunks still in flight from the previous segment must not land after ours
         fetch(); cp_async_commit(); fetch(); cp_async_commit(); fetch(); cp_async_commit(); fetch(); cp_async_commit();
+        cp_async_wait_group<2>();            // the first two chunks: at least 16 bytes from rp on
+        w = lds16(ring | (rp & 63));
     }
     // Call before every group of <= 8 symbols per lane (<= 16 B of words).  Invariant after the call: fp - rp >= 50 and
-    // everything but the two most recent chunks has landed, so the next 16 bytes are readable.
+    // everything but the two most recent chunks has landed, so the next 18 bytes are readable: 8 words and the one read
+    // ahead (a read past the lane's last word sees the next lane's stream or the archive's tail pad, and is never used).
     __device__ __forceinline__ void prepare8() {
         if (fp - rp <= 48) fetch();          // the slot being refilled holds bytes below rp
         cp_async_commit();
         cp_async_wait_group<2>();
     }
     __device__ __forceinline__ void renorm() {
-        if (x < 65536u) { x = (x << 16) | lds16(ring | (rp & 63)); rp += 2; }
+        if (x < 65536u) { x = (x << 16) | w; rp += 2; w = lds16(ring | (rp & 63)); }
     }
     // one symbol on this lane.  lut = shared address of a byte table.  Returns the table entry (sym | bias << 8 |
     // freq << 20).  The ring is read only by the lanes that renormalise (a predicated load).
@@ -206,27 +210,38 @@ __device__ __forceinline__ uint32_t rans_region(Rans& r, uint32_t lut, uint32_t 
     uint32_t base = i0 & ~31u;
     uint8_t* p = dst + (int64_t)S * ((int64_t)lane - (int64_t)(i0 - base));     // address of symbol base + lane
     auto put = [&](uint8_t* q, uint32_t e) { if (PAIR) *reinterpret_cast<uint16_t*>(q) = (uint16_t)e; else *q = (uint8_t)e; };
-    while (base < i1) {
+    auto ragged = [&]() {                                // one round in which some lanes have no symbol
+        const uint32_t i = base + lane;
+        const bool active = i >= i0 && i < i1;
         r.prepare8();
-        if (base >= i0 && base + 256 <= i1) {           // eight full rounds per ring check
+        const uint32_t e = PAIR ? r.step_pair(lut, active) : r.step(lut, active);
+        if (active && store) put(p, e);
+        if (!PAIR) esc += __popc(__ballot_sync(0xffffffffu, active && (e & 0xff) == 255));
+        base += 32; p += 32 * S;
+    };
+    if (base != i0) ragged();
+    uint32_t full = i1 > base ? (i1 - base) >> 5 : 0;     // complete rounds
+    base += 32 * full;
+    for (; full >= 8; full -= 8) {                       // eight rounds per ring check
+        r.prepare8();
 #pragma unroll
-            for (int k = 0; k < 8; k++) {
-                uint32_t e = PAIR ? r.step_pair_full(lut) : r.step_full(lut);
-                if (store) put(p + 32 * S * k, e);
-                if (!PAIR) esc += __popc(__ballot_sync(0xffffffffu, (e & 0xff) == 255));
-            }
-            base += 256; p += 256 * S;
-        } else {                                       // ragged first round, or fewer than eight rounds left
+        for (int k = 0; k < 8; k++) {
+            const uint32_t e = PAIR ? r.step_pair_full(lut) : r.step_full(lut);
+            if (store) put(p + 32 * S * k, e);
+            if (!PAIR) esc += __popc(__ballot_sync(0xffffffffu, (e & 0xff) == 255));
+        }
+        p += 256 * S;
+    }
+    if (full) {
+        r.prepare8();
 #pragma unroll 1
-            for (int k = 0; k < 8 && base < i1 && !(k && base + 256 <= i1); k++, base += 32, p += 32 * S) {   // back to the fast path after a ragged first round
-                const uint32_t i = base + lane;
-                const bool active = i >= i0 && i < i1;
-                uint32_t e = PAIR ? r.step_pair(lut, active) : r.step(lut, active);
-                if (active && store) put(p, e);
-                if (!PAIR) esc += __popc(__ballot_sync(0xffffffffu, active && (e & 0xff) == 255));
-            }
+        for (; full; full--, p += 32 * S) {
+            const uint32_t e = PAIR ? r.step_pair_full(lut) : r.step_full(lut);
+            if (store) put(p, e);
+            if (!PAIR) esc += __popc(__ballot_sync(0xffffffffu, (e & 0xff) == 255));
         }
     }
+    if (base < i1) ragged();
     return esc;
 }
 

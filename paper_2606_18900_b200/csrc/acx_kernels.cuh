@@ -251,22 +251,36 @@ __device__ __forceinline__ bool build_runs(const Params& P, const SegCtx& c, uin
         if (__any_sync(0xffffffffu, !good)) break;
         if (pairs && L.has_match) pairs[c0 + lane] = make_uint2(L.out_rel + L.lit_len, L.match_len);
         const bool a_run = L.valid && !L.is_q && L.lit_len;
-        if (a_run && L.lit_len < 64) {
+        {   // LITA runs of this group: up to eight bytes by the lane that owns the command (two aligned 32-bit loads and a
+            // funnel shift per four bytes, byte stores: the runs start anywhere); longer ones by the whole warp, coalesced
             const uint8_t* sa = c.lit_a + L.lit_pos; uint8_t* da = out_seg + L.out_rel;
-            const uint32_t n0 = min(L.lit_len, 8u), n1 = min(L.lit_len - n0, 8u);
-            uint64_t v0 = ld64u<false>(sa, n0), v1 = n1 ? ld64u<false>(sa + 8, n1) : 0;
-#pragma unroll
-            for (int i = 0; i < 8; i++) { if ((uint32_t)i < n0) da[i] = (uint8_t)v0; v0 >>= 8; }
-            if (n1) {
-#pragma unroll
-                for (int i = 0; i < 8; i++) { if ((uint32_t)i < n1) da[8 + i] = (uint8_t)v1; v1 >>= 8; }
+            const uint32_t n = (a_run && L.lit_len <= 8) ? L.lit_len : 0u;
+            if (__any_sync(0xffffffffu, n != 0)) {
+                const uint32_t sh = 8u * ((uint32_t)reinterpret_cast<uintptr_t>(sa) & 3u);
+                const uint32_t* wa = reinterpret_cast<const uint32_t*>(sa - (sh >> 3));
+                if (n) {
+                    const uint32_t w0 = wa[0], w1 = (sh + 8 * n > 32) ? wa[1] : 0u, w2 = (sh + 8 * n > 64) ? wa[2] : 0u;
+                    const uint32_t v0 = __funnelshift_r(w0, w1, sh), v1 = __funnelshift_r(w1, w2, sh);
+                    da[0] = (uint8_t)v0;
+                    if (n > 1) da[1] = (uint8_t)(v0 >> 8);
+                    if (n > 2) da[2] = (uint8_t)(v0 >> 16);
+                    if (n > 3) da[3] = (uint8_t)(v0 >> 24);
+                    if (n > 4) da[4] = (uint8_t)v1;
+                    if (n > 5) da[5] = (uint8_t)(v1 >> 8);
+                    if (n > 6) da[6] = (uint8_t)(v1 >> 16);
+                    if (n > 7) da[7] = (uint8_t)(v1 >> 24);
+                }
             }
-            for (uint32_t i = 16; i < L.lit_len; i++) da[i] = sa[i];
-        }
-        uint32_t a_long = __ballot_sync(0xffffffffu, a_run && L.lit_len >= 64);   // only archives without a LITQ class have them
-        while (a_long) {
-            const int l = __ffs(a_long) - 1; a_long &= a_long - 1;
-            warp_copy<false>(out_seg + __shfl_sync(0xffffffffu, L.out_rel, l), c.lit_a + __shfl_sync(0xffffffffu, L.lit_pos, l), __shfl_sync(0xffffffffu, L.lit_len, l));
+            uint32_t a_long = __ballot_sync(0xffffffffu, a_run && L.lit_len > 8);
+            while (a_long) {
+                const int l = __ffs(a_long) - 1; a_long &= a_long - 1;
+                const uint32_t m = __shfl_sync(0xffffffffu, L.lit_len, l), lp = __shfl_sync(0xffffffffu, L.lit_pos, l), orl = __shfl_sync(0xffffffffu, L.out_rel, l);
+                if (m >= 64) warp_copy<false>(out_seg + orl, c.lit_a + lp, m);       // only archives without a LITQ class have them
+                else {
+                    if (lane < m) out_seg[orl + lane] = c.lit_a[lp + lane];
+                    if (lane + 32 < m) out_seg[orl + lane + 32] = c.lit_a[lp + lane + 32];
+                }
+            }
         }
         if (L.is_q) {
             uint32_t e;
@@ -314,7 +328,8 @@ struct RunCursor {
 // PAIR = true (FORMAT.md §1.7): symbol j is the aligned pair at zero + 2 j + delta(run of j), stored whole (see above)
 // except for the halves of symbol 0 / symbol n - 1 that q_edge says lie outside the segment.  ODD: the output address of an
 // even position is odd (a range-decode window placed at an odd address): two byte stores instead of one 16-bit store.
-template <bool PAIR, bool ODD>
+// SIMPLE: every run has at least 32 symbols (q_min >= 64), so a full round holds at most one run boundary.
+template <bool PAIR, bool ODD, bool SIMPLE>
 __device__ __forceinline__ void decode_q(Rans& r, uint32_t lut, uint32_t i0, uint32_t n, uint32_t runs, uint8_t* zero, uint32_t q_edge) {
     if (n == 0) return;
     constexpr uint32_t S = PAIR ? 2 : 1;
@@ -346,7 +361,12 @@ __device__ __forceinline__ void decode_q(Rans& r, uint32_t lut, uint32_t i0, uin
                     const uint32_t e = PAIR ? r.step_pair_full(lut) : r.step_full(lut);
                     const uint32_t j_hi = base + 32 * q + 31 - i0;
                     if (j_hi < rc.last) put(pd + 32 * S * q, e);       // the whole round lies strictly inside run k: pointer bump
-                    else { put(pj + 32 * S * q + rc.walk(j_hi - 31 + lane, j_hi), e); pd = pj + rc.delta; }
+                    else if (SIMPLE) {                                 // run k ends in this round, run k + 1 goes on beyond it
+                        const uint32_t prev = rc.last, old_delta = rc.delta;
+                        rc.k += 4; rc.load(lds32(rc.k));
+                        put(pj + 32 * S * q + (j_hi - 31 + lane > prev ? rc.delta : old_delta), e);
+                        pd = pj + rc.delta;
+                    } else { put(pj + 32 * S * q + rc.walk(j_hi - 31 + lane, j_hi), e); pd = pj + rc.delta; }
                 }
                 base += 128; pj += 128 * S;
             }
@@ -376,8 +396,11 @@ __device__ __forceinline__ bool literals_of_segment(const Params& P, uint32_t s_
     const bool ok = build_runs(P, c, runs, out_seg, &q_edge);
     c.lit_a = lit_a_scratch;
     if (!ok) return false;
-    if (QM == 0) decode_q<false, false>(r, s_luts + P.lut_litq * (4 * LUT_SIZE), i0, c.d.n_sym_q, runs, out_seg, 0);
-    else decode_q<true, QM == 2>(r, s_lutq, i0, c.d.n_sym_q, runs, out_seg - (c.sstart & 1) - QDELTA_BIAS, q_edge);
+    // QM: 0 / 1 / 2 as above with run tables of any shape; 3 = bytes, 4 = pairs when every LITQ run has 32 symbols or more
+    if (QM == 0) decode_q<false, false, false>(r, s_luts + P.lut_litq * (4 * LUT_SIZE), i0, c.d.n_sym_q, runs, out_seg, 0);
+    else if (QM == 3) decode_q<false, false, true>(r, s_luts + P.lut_litq * (4 * LUT_SIZE), i0, c.d.n_sym_q, runs, out_seg, 0);
+    else if (QM == 4) decode_q<true, false, true>(r, s_lutq, i0, c.d.n_sym_q, runs, out_seg - (c.sstart & 1) - QDELTA_BIAS, q_edge);
+    else decode_q<true, QM == 2, false>(r, s_lutq, i0, c.d.n_sym_q, runs, out_seg - (c.sstart & 1) - QDELTA_BIAS, q_edge);
     return rans_final_ok(P, r);
 }
 
