@@ -19,6 +19,7 @@ struct SegCtx {
     uint32_t n_ext_cmd;             // number of CMD escapes (they come first in EXT)
     // per-warp scratch
     uint8_t *tok_cmd, *tok_mlen, *off_planes, *lit_a, *lit_q;
+    uint16_t* side;                 // span service: position of every command's literal run in its stream
     uint8_t* off_scratch;           // the warp's own buffer for the coded offset planes
     uint32_t plane_stride;          // bytes between two coded planes at off_planes
 };
@@ -26,9 +27,9 @@ struct SegCtx {
 __device__ __forceinline__ void report(const Params& P, uint32_t bit) { atomicOr(P.err, bit); }
 
 // Scratch layout per warp: [tok_cmd: 512][tok_mlen: 512][off planes: n_coded x 512][lit_a: 16384 + 64][lit_q: 17536 (bytes, or u16 pairs)]
-constexpr uint64_t SCRATCH_LIT_A = MAX_SEG_LITS + 64, SCRATCH_LIT_Q = 2 * (MAX_SEG_LITS / 2 + MAX_SEG_CMDS + 2) + 64;
+constexpr uint64_t SCRATCH_LIT_A = MAX_SEG_LITS + 64, SCRATCH_LIT_Q = 2 * (MAX_SEG_LITS / 2 + MAX_SEG_CMDS + 2) + 64, SCRATCH_SIDE = 2 * TOK_STRIDE;
 __host__ __device__ inline uint64_t scratch_bytes(uint32_t n_coded_planes) {
-    return ((uint64_t)TOK_STRIDE * (2 + n_coded_planes) + SCRATCH_LIT_A + SCRATCH_LIT_Q + 255) & ~255ull;
+    return ((uint64_t)TOK_STRIDE * (2 + n_coded_planes) + SCRATCH_LIT_A + SCRATCH_LIT_Q + SCRATCH_SIDE + 255) & ~255ull;
 }
 __device__ __forceinline__ void bind_scratch(const Params& P, uint32_t warp_global, SegCtx& c) {
     uint8_t* s = P.scratch + (uint64_t)warp_global * P.scratch_per_warp;
@@ -36,7 +37,8 @@ __device__ __forceinline__ void bind_scratch(const Params& P, uint32_t warp_glob
     c.tok_mlen = s; s += TOK_STRIDE;
     c.off_planes = s; c.off_scratch = s; c.plane_stride = TOK_STRIDE; s += (uint64_t)TOK_STRIDE * P.n_coded_planes;
     c.lit_a = s; s += SCRATCH_LIT_A;
-    c.lit_q = s;
+    c.lit_q = s; s += SCRATCH_LIT_Q;
+    c.side = reinterpret_cast<uint16_t*>(s);
 }
 
 // ---- segment geometry (FORMAT.md §1.4, §1.5) ---------------------------------------------------------------------------
@@ -102,47 +104,28 @@ __device__ __forceinline__ uint64_t match_src(const Params& P, const SegCtx& c, 
     return src;
 }
 
-__device__ __forceinline__ void literals_before(const Params& P, const SegCtx& c, uint64_t pend, uint32_t* n_a, uint32_t* n_q);
-
-// A1: the CMD, MLEN and coded OFF streams, then LITA, into the warp's scratch (TO_WS: the coded planes go straight to the
-// workspace of the match launch).  ONE instance of the byte decode loop serves all of them (instruction fetch).
-// UPTO (span service): only the literals in front of output position `pend` are decoded (LITQ follows LITA in the symbol
-// sequence, so needing any of it means decoding all of LITA), and LITQ in byte mode is one more region of the same loop
-// (bytes at lit_q; pair mode: 16-bit pairs at lit_q).  Leaves the rANS state behind the last symbol it decoded;
-// *i_next = index of the first LITQ symbol; *all = every symbol of the segment has been decoded.
-template <bool TO_WS, bool UPTO>
-__device__ __forceinline__ void parse_streams(const Params& P, uint32_t s_luts, uint32_t s_lutq, uint32_t ring, SegCtx& c, Rans& r, uint64_t pend,
-                                              uint32_t* i_next, bool* all) {
-    uint32_t mc = TOK_STRIDE;
-    c.off_planes = c.off_scratch; c.plane_stride = TOK_STRIDE;
-    if (TO_WS) {
-        c.off_planes = P.cplanes + (uint64_t)P.n_coded_planes * __ldg(P.match_prefix + c.s);
-        c.plane_stride = c.d.n_match; mc = c.d.n_match;
-    }
+// A1 for the literal launch: the CMD, MLEN and coded OFF streams and LITA.  Tokens go to the warp's scratch, the coded planes
+// straight to the workspace of the match launch, LITA to c.lit_a.  ONE instance of the byte decode loop serves all of them
+// (instruction fetch).  Leaves the rANS state at the first LITQ symbol (global symbol index *i_next).
+__device__ __forceinline__ void parse_streams(const Params& P, uint32_t s_luts, uint32_t ring, SegCtx& c, Rans& r, uint32_t* i_next) {
+    c.off_planes = P.cplanes + (uint64_t)P.n_coded_planes * __ldg(P.match_prefix + c.s);
+    c.plane_stride = c.d.n_match;
     r.init(c.payload, c.d.n_words, ring);
-    uint32_t i0 = 0, na = c.d.n_lit_a, nq = UPTO ? c.d.n_sym_q : 0u;
-    const uint32_t n_tok = 2 + P.n_coded_planes, n_reg = n_tok + 1 + ((UPTO && !P.q_mode) ? 1u : 0u);
+    uint32_t i0 = 0;
+    const uint32_t n_reg = 3 + P.n_coded_planes;
 #pragma unroll 1
     for (uint32_t k = 0; k < n_reg; k++) {
-        uint32_t lut, cnt, adv; uint8_t* dst;
+        uint32_t lut, cnt; uint8_t* dst;
         if (k == 0) { lut = P.lut_cmd; cnt = c.d.n_cmd; dst = c.tok_cmd; }
         else if (k == 1) { lut = P.lut_mlen; cnt = c.d.n_match; dst = c.tok_mlen; }
-        else if (k < n_tok) { lut = P.coded_lut[k - 2]; cnt = c.d.n_match; dst = c.off_planes + (k - 2) * mc; }
-        else if (k == n_tok) {
-            __syncwarp();                                       // the tokens are complete: the scan below reads them
-            if (UPTO && pend < c.send) { literals_before(P, c, pend, &na, &nq); if (nq) na = c.d.n_lit_a; }
-            lut = P.lut_lita; cnt = na; dst = c.lit_a;
-        } else { lut = P.lut_litq; cnt = nq; dst = c.lit_q; }
-        adv = k == n_tok ? c.d.n_lit_a : cnt;
+        else if (k + 1 < n_reg) { lut = P.coded_lut[k - 2]; cnt = c.d.n_match; dst = c.off_planes + (k - 2) * c.d.n_match; }
+        else { lut = P.lut_lita; cnt = c.d.n_lit_a; dst = c.lit_a; }
         const uint32_t esc = rans_region<false>(r, s_luts + lut * (4 * LUT_SIZE), i0, cnt, dst);
         if (k == 0) c.n_ext_cmd = esc;
-        i0 += adv;
-        if (UPTO && k == n_tok && nq == 0) break;               // nothing of LITQ is wanted
+        i0 += cnt;
     }
-    if (UPTO && P.q_mode && nq) rans_region<true>(r, s_lutq, i0, nq, c.lit_q);
     __syncwarp();
     *i_next = i0;
-    *all = na == c.d.n_lit_a && (UPTO ? nq == c.d.n_sym_q : c.d.n_sym_q == 0);
 }
 
 // FORMAT.md §1.7 integrity check once every symbol of the segment has been decoded
@@ -391,8 +374,8 @@ __device__ __forceinline__ bool literals_of_segment(const Params& P, uint32_t s_
     uint8_t* const out_seg = P.out + (c.sstart - P.out_pos0);
     uint8_t* const lit_a_scratch = c.lit_a;
     if (c.d.n_lit_a <= P.lita_bytes) c.lit_a = lita_stage;
-    Rans r; uint32_t i0, q_edge; bool all;
-    parse_streams<true, false>(P, s_luts, s_lutq, ring, c, r, 0, &i0, &all);
+    Rans r; uint32_t i0, q_edge;
+    parse_streams(P, s_luts, ring, c, r, &i0);
     const bool ok = build_runs(P, c, runs, out_seg, &q_edge);
     c.lit_a = lit_a_scratch;
     if (!ok) return false;
@@ -461,9 +444,20 @@ __device__ __forceinline__ void push_span(const Params& P, const Stack& st, uint
     }
 }
 
+// one out-of-line copy routine for the span-service paths (their code must stay small: the kernels that serve spans were
+// bound by instruction fetch, 5.3 stalled warps per issue, when everything was inlined)
+__device__ __noinline__ void copy_any(uint8_t* dst, const uint8_t* src, uint32_t len) {
+#pragma unroll 1
+    for (uint32_t i = 0; i < len; i += 8) {                 // sources may have been written by other SMs: ld.cg
+        const uint32_t n = min(len - i, 8u);
+        st_small(dst + i, ld64u<true>(src + i, n), n);
+    }
+}
+
 // n contiguous original bytes from absolute position sp -> out2 + dst_off.  Window bytes and resident slots are copied
 // (unless policy SKIP_KNOWN), the rest becomes demands (unless policy SKIP_UNKNOWN).
-__device__ __forceinline__ void fetch_source(const Params& P, const Stack& st, uint64_t sp, uint64_t n, uint64_t dst_off) {
+template <bool COPY_INLINE>
+__device__ __forceinline__ void fetch_source_body(const Params& P, const Stack& st, uint64_t sp, uint64_t n, uint64_t dst_off) {
     while (n) {
         uint64_t m = n;
         const uint8_t* from = nullptr;
@@ -484,12 +478,16 @@ __device__ __forceinline__ void fetch_source(const Params& P, const Stack& st, u
             if (!(st.policy & SKIP_KNOWN)) {
                 uint8_t* d = P.out2 + dst_off;
                 uint64_t left = m; const uint8_t* f = from;
-                while (left) { uint32_t k = (uint32_t)min((unsigned long long)left, 1ull << 30); copy_bytes<true>(d, f, k); d += k; f += k; left -= k; }
+                while (left) { uint32_t k = (uint32_t)min((unsigned long long)left, 1ull << 30); if (COPY_INLINE) copy_bytes<true>(d, f, k); else copy_any(d, f, k); d += k; f += k; left -= k; }
             }
         } else if (!(st.policy & SKIP_UNKNOWN)) push_span(P, st, sp, m, dst_off);
         sp += m; dst_off += m; n -= m;
     }
 }
+
+// the match kernels inline it (a call in their inner loop costs more than the code), the span-service kernels call it
+__device__ __forceinline__ void fetch_source_inl(const Params& P, const Stack& st, uint64_t sp, uint64_t n, uint64_t dst_off) { fetch_source_body<true>(P, st, sp, n, dst_off); }
+__device__ __noinline__ void fetch_source(const Params& P, const Stack st, uint64_t sp, uint64_t n, uint64_t dst_off) { fetch_source_body<false>(P, st, sp, n, dst_off); }
 
 // Where the bytes [src, src + n) live if one known buffer holds them all: the window, or a resident slot (range decode).
 // *end = end of that buffer.  Null when they are unknown or spread over several buffers.
@@ -519,20 +517,22 @@ constexpr uint32_t COPY_WARP_BYTES = 2 * (MTAB_BYTES + 16 * STAGE_CHUNKS);
 static_assert(LONG_MATCH < 256 && (15 + LONG_MATCH + 15) / 16 <= STAGE_CHUNKS, "a short match fits the stage");
 static_assert(COPY_WARP_BYTES % 16 == 0, "tables and stages are 16-byte aligned");
 
+struct Work { unsigned long long* ticket; const uint32_t* seg_list; uint64_t first_work, n_work; };
+
 template <bool WAIT, bool WIN, bool COLLECT, bool REVERSE>
-__device__ __forceinline__ void copy_body(const Params& P, uint32_t smem_warp /* shared address of this warp's COPY_WARP_BYTES */) {
+__device__ __forceinline__ void copy_body(const Params& P, const Work W, uint32_t smem_warp /* shared address of this warp's COPY_WARP_BYTES */) {
     const uint32_t lane = lane_id();
     const uint32_t sbase = smem_warp;
     const uint8_t* const out_end = P.out + (P.win_end - P.out_pos0);
     for (;;) {
         unsigned long long t = 0;
-        if (lane == 0) t = atomicAdd(P.ticket, 1ull);
+        if (lane == 0) t = atomicAdd(W.ticket, 1ull);
         t = __shfl_sync(0xffffffffu, t, 0);
-        if (t >= P.n_work) break;
+        if (t >= W.n_work) break;
         // The wait-free launch of the whole file takes the last segments first: their literals and descriptors are what
         // k_literals wrote last, so the first ~100 MB of the launch's destination sectors and descriptors are still in L2.
-        const unsigned long long tt = REVERSE ? P.n_work - 1 - t : t;
-        const uint64_t s = P.seg_list ? (uint64_t)P.seg_list[tt] : P.first_work + tt;
+        const unsigned long long tt = REVERSE ? W.n_work - 1 - t : t;
+        const uint64_t s = W.seg_list ? (uint64_t)W.seg_list[tt] : W.first_work + tt;
         const uint64_t mp0 = __ldg(P.match_prefix + s);
         const uint4* d4 = reinterpret_cast<const uint4*>(P.dir + s);
         const uint4 da = __ldg(d4), dq = __ldg(d4 + 1);       // FORMAT.md §1.5
@@ -604,7 +604,7 @@ __device__ __forceinline__ void copy_body(const Params& P, uint32_t smem_warp /*
                         if (g0 < n) { load_desc(g0 + lane, npr, nv); have = true; }
                         if (good && !sb) {
                             const Stack sk{nullptr, 0, 0, &P.gl_nxt, SKIP_KNOWN};
-                            fetch_source(P, sk, src, seed_len, dst - P.out_pos0);
+                            fetch_source_inl(P, sk, src, seed_len, dst - P.out_pos0);
                         }
                         continue;
                     }
@@ -618,7 +618,7 @@ __device__ __forceinline__ void copy_body(const Params& P, uint32_t smem_warp /*
                     const bool known = good && sb != nullptr;
                     if (WIN && good && !sb) {                             // seed spread over several buffers or (partly) delivered by the demand rounds
                         const Stack sk{nullptr, 0, 0, nullptr, SKIP_UNKNOWN};
-                        fetch_source(P, sk, src, seed_len, dst - P.out_pos0);   // the known pieces of the seed
+                        fetch_source_inl(P, sk, src, seed_len, dst - P.out_pos0);   // the known pieces of the seed
                     }
                     sp = reinterpret_cast<uint64_t>(sb);
                     mis = (uint32_t)sp & 15u;
@@ -712,178 +712,10 @@ __device__ __forceinline__ void copy_body(const Params& P, uint32_t smem_warp /*
     }
 }
 
-// ---- A5-A7: serving spans of a parsed segment ------------------------------------------------------------------------------
-// LITA bytes / LITQ symbols of the parsed segment in front of output position `pend` (counting the whole literal run of a
-// command that starts before pend): the literal streams have to be decoded only that far to serve spans ending at pend.
-__device__ __forceinline__ void literals_before(const Params& P, const SegCtx& c, uint64_t pend, uint32_t* n_a, uint32_t* n_q) {
-    ScanState st; scan_init(st, c);
-    uint32_t a = 0, q = 0;
-    for (uint32_t c0 = 0; c0 < c.d.n_cmd && c.sstart + st.out_base < pend; c0 += 32) {
-        const CmdLane L = scan_step(P, c, st, c0, load_tokens(c, c0));
-        const bool in = L.valid && c.sstart + L.out_rel < pend;
-        a += (in && !L.is_q) ? min(L.lit_len, 0xffffu) : 0u; q += in ? L.q_syms : 0u;
-    }
-#pragma unroll
-    for (int o = 16; o >= 1; o >>= 1) { a += __shfl_xor_sync(0xffffffffu, a, o); q += __shfl_xor_sync(0xffffffffu, q, o); }
-    *n_a = min(a, (uint32_t)c.d.n_lit_a); *n_q = min(q, (uint32_t)c.d.n_sym_q);
-}
-
-// A1 for span service: tokens, then the literals in front of `pend` into the warp's scratch (LITA bytes at lit_a; LITQ
-// bytes, or 16-bit pairs, at lit_q).  LITQ follows LITA in the symbol sequence, so needing any of it means decoding all of LITA.
-__device__ __forceinline__ bool parse_segment_upto(const Params& P, uint32_t s_luts, uint32_t s_lutq, uint32_t ring, SegCtx& c, uint64_t pend) {
-    if (!load_seg(P, c)) return false;
-    Rans r; uint32_t i0; bool all;
-    parse_streams<false, true>(P, s_luts, s_lutq, ring, c, r, pend, &i0, &all);
-    bool ok = true;
-    if (all) ok = rans_final_ok(P, r);
-    cp_async_wait_group<0>();          // the ring is reused as table space by the callers
-    __syncwarp();
-    return ok;
-}
-
-// byte at absolute position p of a literal run of the parsed segment (run at absolute position d, lit_pos in its stream)
-__device__ __forceinline__ uint32_t lit_byte(const Params& P, const SegCtx& c, bool is_q, uint32_t lit_pos, uint64_t d, uint64_t p) {
-    if (!is_q) return c.lit_a[lit_pos + (p - d)];
-    if (!P.q_mode) return c.lit_q[lit_pos + (p - d)];
-    const uint32_t sym = lit_pos + (uint32_t)((p >> 1) - (d >> 1));
-    return c.lit_q[2ull * sym + (p & 1)];
-}
-// bytes [a, b) of that run -> dptr
-__device__ __forceinline__ void copy_lit(const Params& P, const SegCtx& c, bool is_q, uint32_t lit_pos, uint64_t d, uint64_t a, uint64_t b, uint8_t* dptr) {
-    if (!is_q) { copy_bytes<false>(dptr, c.lit_a + lit_pos + (a - d), (uint32_t)(b - a)); return; }
-    if (!P.q_mode) { copy_bytes<false>(dptr, c.lit_q + lit_pos + (a - d), (uint32_t)(b - a)); return; }
-    // pairs in the scratch sit at even positions of the OUTPUT: byte p of the run is byte (p - (d & ~1)) of the pair array
-    copy_bytes<false>(dptr, c.lit_q + 2ull * lit_pos + (a - (d & ~1ull)), (uint32_t)(b - a));
-}
-
-// the piece [a, b) (absolute positions) of command L (literal run at absolute position o0) -> out2[dst + (x - pos)]
-__device__ __forceinline__ void emit_cmd_piece(const Params& P, const SegCtx& c, const Stack& st, bool is_q, uint32_t lit_pos, uint64_t o0,
-                                               uint32_t lit_len, uint32_t match_len, bool has_match, uint32_t ci,
-                                               uint64_t pos, uint64_t pend, uint64_t dst) {
-    uint64_t a = max((unsigned long long)o0, (unsigned long long)pos), b = min((unsigned long long)(o0 + lit_len), (unsigned long long)pend);
-    if (a < b) copy_lit(P, c, is_q, lit_pos, o0, a, b, P.out2 + dst + (a - pos));
-    const uint64_t md = o0 + lit_len;
-    a = max((unsigned long long)md, (unsigned long long)pos); b = min((unsigned long long)(md + match_len), (unsigned long long)pend);
-    if (has_match && a < b) {
-        const uint64_t src = match_src(P, c, ci);
-        const uint64_t period = md - src;
-        if (src >= md) report(P, DF_OFFSET);
-        else if (period >= match_len) fetch_source(P, st, src + (a - md), b - a, dst + (a - pos));
-        else if (period > lit_len) report(P, DF_OFFSET);      // FORMAT.md §3 (c): the seed is the tail of this literal run
-        else {                                                // byte i of the match = seed[i mod period]
-            uint8_t* d = P.out2 + dst + (a - pos);
-            uint32_t r = (uint32_t)((a - md) % period);
-            for (uint32_t k = 0; k < (uint32_t)(b - a); k++) { d[k] = (uint8_t)lit_byte(P, c, is_q, lit_pos, o0, src + r); if (++r == period) r = 0; }
-        }
-    }
-}
-
-// Emit the bytes [pos, pos + len) of the parsed segment c to out2[dst..): the whole warp walks the commands, a lane per command.
-__device__ __forceinline__ void emit_span(const Params& P, const SegCtx& c, const Stack& st, uint64_t pos, uint64_t len, uint64_t dst) {
-    ScanState ss; scan_init(ss, c);
-    const uint64_t pend = pos + len;
-    for (uint32_t c0 = 0; c0 < c.d.n_cmd; c0 += 32) {
-        const CmdLane L = scan_step(P, c, ss, c0, load_tokens(c, c0));
-        if (__any_sync(0xffffffffu, !cmd_ok(P, c, L))) { if (lane_id() == 0) report(P, DF_LENGTH); return; }
-        if (c.sstart + ss.out_base <= pos) continue;         // the whole group lies before the span
-        if (L.valid) emit_cmd_piece(P, c, st, L.is_q, L.lit_pos, c.sstart + L.out_rel, L.lit_len, L.match_len, L.has_match, c0 + lane_id(), pos, pend, dst);
-        if (c.sstart + ss.out_base >= pend) break;           // uniform: nothing after this group is wanted
-    }
-}
-
-// Command table of a parsed segment (demand rounds): word ci = segment-relative output position of command ci (15 bits) |
-// lit_len << 15 (15 bits) | LITQ class << 30; the 16-bit side table holds the position of the run in its stream.  Word n_cmd
-// is a sentinel (position 0x7fff).  The words live in the warp's run-table area, the side table in its (idle) word ring.
-__device__ __forceinline__ bool build_cmd_table(const Params& P, const SegCtx& c, uint32_t tab, uint32_t side) {
-    ScanState st; scan_init(st, c);
-    bool good = true;
-    for (uint32_t c0 = 0; c0 < c.d.n_cmd; c0 += 32) {
-        const CmdLane L = scan_step(P, c, st, c0, load_tokens(c, c0));
-        good = good && cmd_ok(P, c, L) && L.lit_len <= MAX_SEG_LITS;
-        if (__any_sync(0xffffffffu, !good)) { if (lane_id() == 0) report(P, DF_LENGTH); return false; }
-        if (L.valid) {
-            sts32(tab + 4 * (c0 + lane_id()), L.out_rel | L.lit_len << 15 | (L.is_q ? 1u << 30 : 0u));
-            sts16(side + 2 * (c0 + lane_id()), L.lit_pos);
-        }
-    }
-    if (!scan_totals_ok(c, st)) { if (lane_id() == 0) report(P, DF_LENGTH); return false; }
-    if (lane_id() == 0) sts32(tab + 4 * c.d.n_cmd, 0x7fffu);
-    __syncwarp();
-    return true;
-}
-
-constexpr uint32_t ITEM_LANE_MAX = 96;   // spans up to this many bytes are served by one lane each
-
-// The records of a work item, one per lane: lane l emits bytes [pos, pos + len) of the parsed segment c to out2[dst ..).
-// A binary search in the command table finds the first command of the span; the lane then walks its commands (one to
-// three for a 32-byte span): literal bytes come from the warp's scratch, match pieces are forwarded to their sources.
-__device__ __forceinline__ void emit_item(const Params& P, const SegCtx& c, const Stack& st, uint32_t tab, uint32_t side, bool have,
-                                          uint64_t pos, uint32_t len, uint64_t dst) {
-    if (!have || len == 0) return;
-    const uint32_t pr = (uint32_t)(pos - c.sstart), pe = pr + len, slen = (uint32_t)(c.send - c.sstart);
-    uint32_t lo = 0, hi = c.d.n_cmd;
-    while (hi - lo > 1) { const uint32_t mid = (lo + hi) >> 1; if ((lds32(tab + 4 * mid) & 0x7fffu) <= pr) lo = mid; else hi = mid; }
-    for (uint32_t k = lo; k < c.d.n_cmd; k++) {
-        const uint32_t e = lds32(tab + 4 * k);
-        const uint32_t o0 = e & 0x7fffu, lit_len = (e >> 15) & 0x7fffu;
-        if (o0 >= pe) break;
-        const uint32_t nx = k + 1 < c.d.n_cmd ? lds32(tab + 4 * k + 4) & 0x7fffu : slen;
-        const uint32_t match_len = nx - o0 - lit_len;
-        emit_cmd_piece(P, c, st, (e >> 30) & 1u, lds16(side + 2 * k), c.sstart + o0, lit_len, match_len, k < c.d.n_match, k, pos, pos + len, dst);
-    }
-}
-
-// Serve every pending demand of the warp's stack (depth-first; all demands of one segment from one parse).
-__device__ __forceinline__ void process_demands(const Params& P, uint32_t s_luts, uint32_t s_lutq, uint32_t ring, SegCtx& c, const Stack& st) {
-    const uint32_t lane = lane_id();
-    for (;;) {
-        __syncwarp();
-        uint32_t top = min(lds_top(st), st.cap);
-        while (top > 0 && st.base[top - 1].len == 0) top--;  // drop served entries
-        __syncwarp();
-        if (lane == 0) sts32(st.top, top);
-        __syncwarp();
-        if (top == 0) return;
-        const uint64_t p0 = st.base[top - 1].pos;
-        if (p0 >= P.N) { if (lane == 0) { report(P, DF_OFFSET); st.base[top - 1].len = 0; } continue; }
-        c.s = seg_of(P, p0);
-        const uint64_t b0 = p0 >> P.log2_bs, lo = __ldg(&P.dir[c.s].out_start), hi = seg_end(P, c.s, b0);
-        uint64_t pend = 0;                                   // the literals are needed up to the last pending span of this segment
-        for (uint32_t i0 = 0; i0 < top; i0 += 32) {
-            const uint32_t idx = i0 + lane;
-            if (idx < top && st.base[idx].len != 0 && st.base[idx].pos >= lo && st.base[idx].pos < hi)
-                pend = max((unsigned long long)pend, (unsigned long long)(st.base[idx].pos + st.base[idx].len));
-        }
-#pragma unroll
-        for (int o = 16; o >= 1; o >>= 1) pend = max((unsigned long long)pend, (unsigned long long)__shfl_xor_sync(0xffffffffu, pend, o));
-        const bool ok = parse_segment_upto(P, s_luts, s_lutq, ring, c, pend);
-        bool found = true;
-        while (found) {                                      // emit_span may push more demands for this same segment
-            found = false;
-            const uint32_t n = min(lds_top(st), st.cap);
-            for (uint32_t i0 = 0; i0 < n; i0 += 32) {
-                const uint32_t idx = i0 + lane;
-                const bool mine = idx < n && st.base[idx].len != 0 && st.base[idx].pos >= lo && st.base[idx].pos < hi;
-                uint32_t m = __ballot_sync(0xffffffffu, mine);
-                while (m) {
-                    const uint32_t e = i0 + __ffs(m) - 1; m &= m - 1;
-                    const uint64_t pos = st.base[e].pos, len = st.base[e].len, dst = st.base[e].dst;
-                    __syncwarp();
-                    if (lane == 0) st.base[e].len = 0;
-                    __syncwarp();
-                    if (ok && pos + len <= hi) emit_span(P, c, st, pos, len, dst);
-                    found = true;
-                }
-            }
-            __syncwarp();
-        }
-    }
-}
-
 // shared memory of the entropy kernels: [byte tables: n_coded_tables x 8 KB][pair table: 32 KB when q_mode = 1]
 // [rings: warps x 2 KB][per warp: run table | LITA staging][stack tops: warps x 4]   (absolute shared addresses).
 // The span-service kernels use the per-warp area as one command table (2 KB at least).
-struct CtaSmem { uint32_t luts, lutq, ring, runs, top; uint8_t* lita; };
+struct CtaSmem { uint32_t luts, lutq, ring, runs, top; uint8_t* lita; uint8_t* area; };   // area: generic pointer of `runs`
 
 __host__ __device__ inline size_t entropy_smem(uint32_t n_coded_tables, uint32_t q_mode, uint32_t warp_area, int threads) {
     return (size_t)n_coded_tables * LUT_SIZE * 4 + (q_mode ? (size_t)QLUT_SIZE * 8 : 0) + (size_t)(threads / 32) * (RING_BYTES + warp_area + 4) + 128;
@@ -911,10 +743,211 @@ __device__ __forceinline__ CtaSmem setup_cta(const Params& P, uint8_t* smem_raw)
     base = (base + 63u) & ~63u;                                // rings are 64-byte aligned (ring | slot)
     m.ring = base + warp * RING_BYTES; base += warps * RING_BYTES;
     m.runs = base + warp * area;
-    m.lita = smem_raw + (m.runs + P.runs_bytes - raw0);
+    m.area = smem_raw + (m.runs - raw0);
+    m.lita = m.area + P.runs_bytes;
     base += warps * area;
     m.top = base + 4 * warp;
     return m;
+}
+
+// ---- A5-A7: serving spans of a parsed segment ------------------------------------------------------------------------------
+// Command table of a parsed segment: word ci = segment-relative output position of command ci (15 bits) | lit_len << 15
+// (15 bits) | LITQ class << 30; c.side[ci] = position of the run in its stream.  Word n_cmd is a sentinel (position 0x7fff).
+// The words live in the warp's area in shared memory (tab), the side table behind them when it fits, else in the scratch.
+__device__ __forceinline__ bool build_cmd_table(const Params& P, SegCtx& c, uint32_t tab, uint8_t* area, uint32_t area_bytes) {
+    const uint32_t words = 4 * (c.d.n_cmd + 1);
+    if (words + 2 * c.d.n_cmd <= area_bytes) c.side = reinterpret_cast<uint16_t*>(area + words);
+    ScanState st; scan_init(st, c);
+    bool good = true;
+    for (uint32_t c0 = 0; c0 < c.d.n_cmd; c0 += 32) {
+        const CmdLane L = scan_step(P, c, st, c0, load_tokens(c, c0));
+        good = good && cmd_ok(P, c, L) && L.lit_len <= MAX_SEG_LITS;
+        if (__any_sync(0xffffffffu, !good)) { if (lane_id() == 0) report(P, DF_LENGTH); return false; }
+        if (L.valid) {
+            sts32(tab + 4 * (c0 + lane_id()), L.out_rel | L.lit_len << 15 | (L.is_q ? 1u << 30 : 0u));
+            c.side[c0 + lane_id()] = (uint16_t)L.lit_pos;
+        }
+    }
+    if (!scan_totals_ok(c, st)) { if (lane_id() == 0) report(P, DF_LENGTH); return false; }
+    if (lane_id() == 0) sts32(tab + 4 * c.d.n_cmd, 0x7fffu);
+    __syncwarp();
+    return true;
+}
+
+// LITA bytes / LITQ symbols in front of segment-relative output position `pend_rel`, from the command table (counting the
+// whole literal run of a command that starts before it): the literal streams are decoded only that far.
+__device__ __forceinline__ void literals_before(const Params& P, const SegCtx& c, uint32_t tab, uint32_t pend_rel, uint32_t* n_a, uint32_t* n_q) {
+    uint32_t a = 0, q = 0;
+    for (uint32_t ci = lane_id(); ci < c.d.n_cmd; ci += 32) {
+        const uint32_t e = lds32(tab + 4 * ci), o0 = e & 0x7fffu, ll = (e >> 15) & 0x7fffu;
+        if (o0 < pend_rel) {
+            if ((e >> 30) & 1u) { const uint64_t d = c.sstart + o0; q += P.q_mode ? (uint32_t)(((d + ll - 1) >> 1) - (d >> 1) + 1) : ll; }
+            else a += ll;
+        }
+    }
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) { a += __shfl_xor_sync(0xffffffffu, a, o); q += __shfl_xor_sync(0xffffffffu, q, o); }
+    *n_a = min(a, (uint32_t)c.d.n_lit_a); *n_q = min(q, (uint32_t)c.d.n_sym_q);
+}
+
+// A1 + A2 for span service: tokens, the command table, then the literals in front of `pend` into the warp's scratch (LITA
+// bytes at lit_a; LITQ bytes, or 16-bit pairs, at lit_q).  LITQ follows LITA in the symbol sequence, so needing any of it
+// means decoding all of LITA.  One instance of the byte decode loop.
+__device__ __forceinline__ bool parse_for_spans(const Params& P, uint32_t s_luts, uint32_t s_lutq, uint32_t ring, uint32_t tab, uint8_t* area, SegCtx& c, uint64_t pend) {
+    if (!load_seg(P, c)) return false;
+    c.off_planes = c.off_scratch; c.plane_stride = TOK_STRIDE;
+    Rans r;
+    r.init(c.payload, c.d.n_words, ring);
+    uint32_t i0 = 0, na = c.d.n_lit_a, nq = c.d.n_sym_q;
+    const uint32_t n_tok = 2 + P.n_coded_planes, n_reg = n_tok + 1 + (P.q_mode ? 0u : 1u);
+    bool ok = true;
+#pragma unroll 1
+    for (uint32_t k = 0; k < n_reg; k++) {
+        uint32_t lut, cnt, adv; uint8_t* dst;
+        if (k == 0) { lut = P.lut_cmd; cnt = c.d.n_cmd; dst = c.tok_cmd; }
+        else if (k == 1) { lut = P.lut_mlen; cnt = c.d.n_match; dst = c.tok_mlen; }
+        else if (k < n_tok) { lut = P.coded_lut[k - 2]; cnt = c.d.n_match; dst = c.off_planes + (k - 2) * TOK_STRIDE; }
+        else if (k == n_tok) {
+            __syncwarp();                                       // the tokens are complete: the scan reads them
+            ok = build_cmd_table(P, c, tab, area, P.runs_bytes + P.lita_bytes);
+            if (!ok) break;
+            if (pend < c.send) { literals_before(P, c, tab, (uint32_t)(pend - c.sstart), &na, &nq); if (nq) na = c.d.n_lit_a; }
+            lut = P.lut_lita; cnt = na; dst = c.lit_a;
+        } else { lut = P.lut_litq; cnt = nq; dst = c.lit_q; }
+        adv = k == n_tok ? c.d.n_lit_a : cnt;
+        const uint32_t esc = rans_region<false>(r, s_luts + lut * (4 * LUT_SIZE), i0, cnt, dst);
+        if (k == 0) c.n_ext_cmd = esc;
+        i0 += adv;
+        if (k == n_tok && nq == 0) break;                       // nothing of LITQ is wanted
+    }
+    if (ok && P.q_mode && nq) rans_region<true>(r, s_lutq, i0, nq, c.lit_q);
+    if (ok && na == c.d.n_lit_a && nq == c.d.n_sym_q) ok = rans_final_ok(P, r);
+    cp_async_wait_group<0>();
+    __syncwarp();
+    return ok;
+}
+
+// byte at absolute position p of a literal run of the parsed segment (run at absolute position d, lit_pos in its stream)
+__device__ __forceinline__ uint32_t lit_byte(const Params& P, const SegCtx& c, bool is_q, uint32_t lit_pos, uint64_t d, uint64_t p) {
+    if (!is_q) return c.lit_a[lit_pos + (p - d)];
+    if (!P.q_mode) return c.lit_q[lit_pos + (p - d)];
+    const uint32_t sym = lit_pos + (uint32_t)((p >> 1) - (d >> 1));
+    return c.lit_q[2ull * sym + (p & 1)];
+}
+
+// the piece [pos, pend) (absolute positions) of a command (literal run at absolute position o0) -> out2[dst + (x - pos)]
+__device__ __forceinline__ void emit_cmd_piece(const Params& P, const SegCtx& c, const Stack& st, bool is_q, uint32_t lit_pos, uint64_t o0,
+                                            uint32_t lit_len, uint32_t match_len, bool has_match, uint32_t ci,
+                                            uint64_t pos, uint64_t pend, uint64_t dst) {
+    uint64_t a = max((unsigned long long)o0, (unsigned long long)pos), b = min((unsigned long long)(o0 + lit_len), (unsigned long long)pend);
+    if (a < b) {
+        // bytes [a, b) of the run; pairs in the scratch sit at even positions of the OUTPUT: byte p of the run is byte
+        // (p - (o0 & ~1)) of the pair array that starts at symbol lit_pos
+        const uint8_t* src = !is_q ? c.lit_a + lit_pos + (a - o0) : !P.q_mode ? c.lit_q + lit_pos + (a - o0) : c.lit_q + 2ull * lit_pos + (a - (o0 & ~1ull));
+        copy_any(P.out2 + dst + (a - pos), src, (uint32_t)(b - a));
+    }
+    const uint64_t md = o0 + lit_len;
+    a = max((unsigned long long)md, (unsigned long long)pos); b = min((unsigned long long)(md + match_len), (unsigned long long)pend);
+    if (has_match && a < b) {
+        const uint64_t src = match_src(P, c, ci);
+        const uint64_t period = md - src;
+        if (src >= md) report(P, DF_OFFSET);
+        else if (period >= match_len) fetch_source(P, st, src + (a - md), b - a, dst + (a - pos));
+        else if (period > lit_len) report(P, DF_OFFSET);      // FORMAT.md §3 (c): the seed is the tail of this literal run
+        else {                                                // byte i of the match = seed[i mod period]
+            uint8_t* d = P.out2 + dst + (a - pos);
+            uint32_t r = (uint32_t)((a - md) % period);
+            for (uint32_t k = 0; k < (uint32_t)(b - a); k++) { d[k] = (uint8_t)lit_byte(P, c, is_q, lit_pos, o0, src + r); if (++r == period) r = 0; }
+        }
+    }
+}
+
+constexpr uint32_t ITEM_LANE_MAX = 96;   // spans up to this many bytes are served by one lane each
+constexpr uint32_t WIDE_PIECE = 64;      // longer ones are cut into pieces of this size, a lane per piece
+
+// Records of the parsed segment c, one per lane (have == false: none): lane l emits bytes [pos, pos + len) to out2[dst ..).
+// A binary search in the command table finds the first command of the span; the lane then walks its commands (one to
+// three for a 32-byte span): literal bytes come from the warp's scratch, match pieces are forwarded to their sources.
+// A record longer than ITEM_LANE_MAX is cut into pieces that all lanes serve together, 32 pieces at a time.  The loop is
+// written so that the body exists once in the code (the kernels that serve spans are sensitive to instruction fetch).
+__device__ __forceinline__ void emit_records(const Params& P, const SegCtx& c, const Stack& st, uint32_t tab, bool have,
+                                             uint64_t pos, uint32_t len, uint64_t dst) {
+    const uint32_t lane = lane_id(), slen = (uint32_t)(c.send - c.sstart);
+    have = have && len != 0;
+    uint32_t wides = __ballot_sync(0xffffffffu, have && len > ITEM_LANE_MAX);
+    uint64_t wpos = 0, wdst = 0; uint32_t wlen = 0, q = 0;
+    for (uint32_t pass = 0;; pass++) {
+        bool mine; uint64_t mpos, mdst; uint32_t mlen;
+        if (pass == 0) { mine = have && len <= ITEM_LANE_MAX; mpos = pos; mlen = len; mdst = dst; }
+        else {
+            if (q == 0) {
+                if (!wides) break;
+                const int l = __ffs(wides) - 1; wides &= wides - 1;
+                wpos = __shfl_sync(0xffffffffu, pos, l); wlen = __shfl_sync(0xffffffffu, len, l); wdst = __shfl_sync(0xffffffffu, dst, l);
+            }
+            const uint32_t off = WIDE_PIECE * (lane + 32u * q);
+            mine = off < wlen; mpos = wpos + off; mlen = mine ? min(WIDE_PIECE, wlen - off) : 0u; mdst = wdst + off;
+            q = (WIDE_PIECE * 32u * (q + 1) < wlen) ? q + 1 : 0u;
+        }
+        if (mine) {
+            const uint32_t pr = (uint32_t)(mpos - c.sstart), pe = pr + mlen;
+            uint32_t lo = 0, hi = c.d.n_cmd;
+            while (hi - lo > 1) { const uint32_t mid = (lo + hi) >> 1; if ((lds32(tab + 4 * mid) & 0x7fffu) <= pr) lo = mid; else hi = mid; }
+            for (uint32_t k = lo; k < c.d.n_cmd; k++) {
+                const uint32_t e = lds32(tab + 4 * k);
+                const uint32_t o0 = e & 0x7fffu, lit_len = (e >> 15) & 0x7fffu;
+                if (o0 >= pe) break;
+                const uint32_t nx = k + 1 < c.d.n_cmd ? lds32(tab + 4 * k + 4) & 0x7fffu : slen;
+                emit_cmd_piece(P, c, st, (e >> 30) & 1u, c.side[k], c.sstart + o0, lit_len, nx - o0 - lit_len, k < c.d.n_match, k, mpos, mpos + mlen, mdst);
+            }
+        }
+        __syncwarp();
+    }
+}
+
+// Serve every pending demand of the warp's stack (depth-first; all demands of one segment from one parse).
+__device__ __forceinline__ void process_demands(const Params& P, const CtaSmem& m, SegCtx& c, const Stack& st) {
+    const uint32_t lane = lane_id();
+    for (;;) {
+        __syncwarp();
+        uint32_t top = min(lds_top(st), st.cap);
+        while (top > 0 && st.base[top - 1].len == 0) top--;  // drop served entries
+        __syncwarp();
+        if (lane == 0) sts32(st.top, top);
+        __syncwarp();
+        if (top == 0) return;
+        const uint64_t p0 = st.base[top - 1].pos;
+        if (p0 >= P.N) { if (lane == 0) { report(P, DF_OFFSET); st.base[top - 1].len = 0; } continue; }
+        c.s = seg_of(P, p0);
+        const uint64_t b0 = p0 >> P.log2_bs, lo = __ldg(&P.dir[c.s].out_start), hi = seg_end(P, c.s, b0);
+        uint64_t pend = 0;                                   // the literals are needed up to the last pending span of this segment
+        for (uint32_t i0 = 0; i0 < top; i0 += 32) {
+            const uint32_t idx = i0 + lane;
+            if (idx < top && st.base[idx].len != 0 && st.base[idx].pos >= lo && st.base[idx].pos < hi)
+                pend = max((unsigned long long)pend, (unsigned long long)(st.base[idx].pos + st.base[idx].len));
+        }
+#pragma unroll
+        for (int o = 16; o >= 1; o >>= 1) pend = max((unsigned long long)pend, (unsigned long long)__shfl_xor_sync(0xffffffffu, pend, o));
+        uint16_t* const side0 = c.side;
+        const bool ok = parse_for_spans(P, m.luts, m.lutq, m.ring, m.runs, m.area, c, pend);
+        bool found = true;
+        while (found) {                                      // serving may push more demands for this same segment
+            found = false;
+            const uint32_t n = min(lds_top(st), st.cap);
+            for (uint32_t i0 = 0; i0 < n; i0 += 32) {
+                const uint32_t idx = i0 + lane;
+                const bool mine = idx < n && st.base[idx].len != 0 && st.base[idx].pos >= lo && st.base[idx].pos < hi;
+                uint64_t pos = 0, len = 0, dst = 0;
+                if (mine) { pos = st.base[idx].pos; len = st.base[idx].len; dst = st.base[idx].dst; st.base[idx].len = 0; }
+                if (!__any_sync(0xffffffffu, mine)) continue;
+                __syncwarp();
+                emit_records(P, c, st, m.runs, ok && mine && pos + len <= hi, pos, (uint32_t)len, dst);
+                found = true;
+            }
+            __syncwarp();
+        }
+        c.side = side0;
+    }
 }
 
 // Two ticket slots alternate between consecutive launches of a handle: a kernel draws from its own slot and clears the
@@ -932,7 +965,7 @@ __device__ __forceinline__ bool next_ticket(const Params& P, unsigned long long&
 
 // The literal launch: A1 + A2 + A3 for every segment of the work list, no dependencies.
 template <int QM>
-__global__ void __launch_bounds__(1024, 1) k_literals(const Params P) {
+__global__ void __launch_bounds__(1024, 1) k_literals(const __grid_constant__ Params P) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
     clear_next_ticket(P);
     const CtaSmem m = setup_cta(P, smem_raw);
@@ -946,11 +979,11 @@ __global__ void __launch_bounds__(1024, 1) k_literals(const Params P) {
 }
 
 template <bool WAIT, bool WIN, bool COLLECT, bool REVERSE>
-__global__ void __launch_bounds__(1024, 1) k_copy(const Params P) {
+__global__ void __launch_bounds__(1024, 1) k_copy(const __grid_constant__ Params P) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
     clear_next_ticket(P);
     const uint32_t smem0 = ((uint32_t)__cvta_generic_to_shared(smem_raw) + 15u) & ~15u;
-    copy_body<WAIT, WIN, COLLECT, REVERSE>(P, smem0 + (threadIdx.x >> 5) * COPY_WARP_BYTES);
+    copy_body<WAIT, WIN, COLLECT, REVERSE>(P, Work{P.ticket, P.seg_list, P.first_work, P.n_work}, smem0 + (threadIdx.x >> 5) * COPY_WARP_BYTES);
 }
 
 // The whole wavefront in ONE cooperative launch (a single persistent kernel): the literal wave over
@@ -958,29 +991,32 @@ __global__ void __launch_bounds__(1024, 1) k_copy(const Params P) {
 // (when there are any) and one wait-free pass over the top level.  tickets[0..2] are zero at launch.
 struct FusedArgs { uint64_t n_low, n_top; const uint32_t* low_list; const uint32_t* top_list; unsigned long long* tickets; };
 template <int QM>
-__global__ void __launch_bounds__(1024, 1) k_fused(Params P, const FusedArgs F) {
+__global__ void __launch_bounds__(1024, 1) k_fused(const __grid_constant__ Params P, const FusedArgs F) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
     cooperative_groups::grid_group grid = cooperative_groups::this_grid();
     {
         const CtaSmem m = setup_cta(P, smem_raw);
         SegCtx c;
         bind_scratch(P, blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), c);
-        P.ticket = F.tickets; P.seg_list = nullptr; P.first_work = 0; P.n_work = P.n_segs;
-        unsigned long long t;
-        while (next_ticket(P, t)) { c.s = t; literals_of_segment<QM>(P, m.luts, m.lutq, m.ring, m.runs, m.lita, c); }
+        for (;;) {
+            unsigned long long t = 0;
+            if (lane_id() == 0) t = atomicAdd(F.tickets, 1ull);
+            t = __shfl_sync(0xffffffffu, t, 0);
+            if (t >= P.n_segs) break;
+            c.s = t;
+            literals_of_segment<QM>(P, m.luts, m.lutq, m.ring, m.runs, m.lita, c);
+        }
     }
     __threadfence();
     grid.sync();
     const uint32_t smem0 = ((uint32_t)__cvta_generic_to_shared(smem_raw) + 15u) & ~15u;
     const uint32_t mine = smem0 + (threadIdx.x >> 5) * COPY_WARP_BYTES;
     if (F.n_low) {
-        P.ticket = F.tickets + 1; P.seg_list = F.low_list; P.n_work = F.n_low;
-        copy_body<true, false, false, false>(P, mine);
+        copy_body<true, false, false, false>(P, Work{F.tickets + 1, F.low_list, 0, F.n_low}, mine);
         __threadfence();
         grid.sync();
     }
-    P.ticket = F.tickets + 2; P.seg_list = F.top_list; P.n_work = F.n_top;
-    copy_body<false, false, false, true>(P, mine);
+    copy_body<false, false, false, true>(P, Work{F.tickets + 2, F.top_list, 0, F.n_top}, mine);
 }
 
 // ---- demand rounds ---------------------------------------------------------------------------------------------------
@@ -1022,7 +1058,7 @@ __device__ __forceinline__ void plan_body(const GList& g, uint32_t warp_global, 
     }
 }
 
-__global__ void __launch_bounds__(1024, 1) k_plan(const Params P) {
+__global__ void __launch_bounds__(1024, 1) k_plan(const __grid_constant__ Params P) {
     plan_body(P.gl_cur, blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), gridDim.x * (blockDim.x >> 5));
 }
 
@@ -1035,7 +1071,7 @@ __device__ __forceinline__ void scatter_body(const GList& g, uint32_t tid, uint3
     }
 }
 
-__global__ void __launch_bounds__(256) k_scatter(const Params P) {
+__global__ void __launch_bounds__(256) k_scatter(const __grid_constant__ Params P) {
     scatter_body(P.gl_cur, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
 }
 
@@ -1063,24 +1099,18 @@ __device__ __forceinline__ void serve_body(const Params& P, const CtaSmem& m, Se
         uint64_t pend = have ? d.pos + d.len : 0;             // the literals are needed up to the last span of the item
 #pragma unroll
         for (int o = 16; o >= 1; o >>= 1) pend = max((unsigned long long)pend, (unsigned long long)__shfl_xor_sync(0xffffffffu, pend, o));
-        if (!parse_segment_upto(P, m.luts, m.lutq, m.ring, c, pend)) continue;
-        const bool inside = have && d.pos >= c.sstart && d.pos + d.len <= c.send;
-        if (have && !inside) report(P, DF_LENGTH);
-        if (!build_cmd_table(P, c, m.runs, m.ring)) continue;
-        // a long span covers many commands: the whole warp walks it (a lane per command) instead of one lane
-        const bool wide = inside && d.len > ITEM_LANE_MAX;
-        emit_item(P, c, sk, m.runs, m.ring, inside && !wide, d.pos, d.len, d.dst);
-        __syncwarp();
-        uint32_t wides = __ballot_sync(0xffffffffu, wide);
-        while (wides) {
-            const int l = __ffs(wides) - 1; wides &= wides - 1;
-            emit_span(P, c, sk, __shfl_sync(0xffffffffu, d.pos, l), __shfl_sync(0xffffffffu, d.len, l), __shfl_sync(0xffffffffu, d.dst, l));
+        uint16_t* const side0 = c.side;
+        if (parse_for_spans(P, m.luts, m.lutq, m.ring, m.runs, m.area, c, pend)) {
+            const bool inside = have && d.pos >= c.sstart && d.pos + d.len <= c.send;
+            if (have && !inside) report(P, DF_LENGTH);
+            emit_records(P, c, sk, m.runs, inside, d.pos, d.len, d.dst);
         }
+        c.side = side0;
         __syncwarp();
     }
 }
 
-__global__ void __launch_bounds__(1024, 1) k_serve(const Params P) {
+__global__ void __launch_bounds__(1024, 1) k_serve(const __grid_constant__ Params P) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
     clear_next_ticket(P);
     const CtaSmem m = setup_cta(P, smem_raw);
@@ -1093,7 +1123,7 @@ __global__ void __launch_bounds__(1024, 1) k_serve(const Params P) {
 // serve): a seek or the ragged ends of a range need a handful of records per round, and one launch instead of three per
 // round, with an exit as soon as a round leaves nothing, is what their latency is made of.  P.gl_cur = the filled list,
 // P.gl_nxt = the other one; round_tickets = one zeroed counter per round.
-__global__ void __launch_bounds__(1024, 1) k_rounds(const Params P, unsigned long long* round_tickets, uint32_t rounds) {
+__global__ void __launch_bounds__(1024, 1) k_rounds(const __grid_constant__ Params P, unsigned long long* round_tickets, uint32_t rounds) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
     cooperative_groups::grid_group grid = cooperative_groups::this_grid();
     const CtaSmem m = setup_cta(P, smem_raw);
@@ -1119,7 +1149,7 @@ __global__ void __launch_bounds__(1024, 1) k_rounds(const Params P, unsigned lon
 }
 
 // top-level spans (ragged ends of a range, reads of a batch) enter the demand lists like any other record
-__global__ void k_seed(const Params P, uint32_t n) {
+__global__ void k_seed(const __grid_constant__ Params P, uint32_t n) {
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) {
         const Demand d = P.n_inline ? P.inline_dem[i] : P.demands[i];
@@ -1132,7 +1162,7 @@ __global__ void k_assert_empty(const uint32_t* count, uint32_t* err) { if (*coun
 
 // Read access by recursion inside one warp: one top-level span per ticket; the warp parses the segment that holds it,
 // emits the span, and serves the source spans it pushed on its own stack until the stack is empty.
-__global__ void __launch_bounds__(1024, 1) k_spans(const Params P) {
+__global__ void __launch_bounds__(1024, 1) k_spans(const __grid_constant__ Params P) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
     clear_next_ticket(P);
     const CtaSmem m = setup_cta(P, smem_raw);
@@ -1149,7 +1179,7 @@ __global__ void __launch_bounds__(1024, 1) k_spans(const Params P) {
             const Demand d = P.n_inline ? P.inline_dem[t] : P.demands[t];
             push_span(P, st, d.pos, d.len, d.dst);
         }
-        process_demands(P, m.luts, m.lutq, m.ring, c, st);
+        process_demands(P, m, c, st);
     }
 }
 
