@@ -1093,17 +1093,21 @@ __device__ __forceinline__ void serve_body(const Params& P, const CtaSmem& m, Se
         c.s = item >> 32;
         if (c.s >= P.n_segs) { if (lane == 0) report(P, DF_OFFSET); continue; }
         if (lane == 0) cur.cnt[c.s] = 0;                      // every item of the segment writes the same value: the array is idle again
-        const bool have = lane < cnt && first + lane < cur.cap;
-        GDemand d; d.pos = 0; d.len = 0; d.dst = 0; d.seg = 0;
-        if (have) d = ld_demand(cur.sorted + first + lane);
-        uint64_t pend = have ? d.pos + d.len : 0;             // the literals are needed up to the last span of the item
+        uint64_t pend = 0;                                    // the literals are needed up to the last span of the item
+        for (uint32_t r0 = 0; r0 < cnt; r0 += 32)
+            if (r0 + lane < cnt && first + r0 + lane < cur.cap) { const GDemand d = ld_demand(cur.sorted + first + r0 + lane); pend = max((unsigned long long)pend, (unsigned long long)(d.pos + d.len)); }
 #pragma unroll
         for (int o = 16; o >= 1; o >>= 1) pend = max((unsigned long long)pend, (unsigned long long)__shfl_xor_sync(0xffffffffu, pend, o));
         uint16_t* const side0 = c.side;
         if (parse_for_spans(P, m.luts, m.lutq, m.ring, m.runs, m.area, c, pend)) {
-            const bool inside = have && d.pos >= c.sstart && d.pos + d.len <= c.send;
-            if (have && !inside) report(P, DF_LENGTH);
-            emit_records(P, c, sk, m.runs, inside, d.pos, d.len, d.dst);
+            for (uint32_t r0 = 0; r0 < cnt; r0 += 32) {
+                const bool have = r0 + lane < cnt && first + r0 + lane < cur.cap;
+                GDemand d; d.pos = 0; d.len = 0; d.dst = 0; d.seg = 0;
+                if (have) d = ld_demand(cur.sorted + first + r0 + lane);
+                const bool inside = have && d.pos >= c.sstart && d.pos + d.len <= c.send;
+                if (have && !inside) report(P, DF_LENGTH);
+                emit_records(P, c, sk, m.runs, inside, d.pos, d.len, d.dst);
+            }
         }
         c.side = side0;
         __syncwarp();
