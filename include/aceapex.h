@@ -132,6 +132,39 @@ int32_t aceapex_reads_bytes(const uint64_t* h_read_index, uint64_t n_index, cons
  * and d_ptr must be 8-byte aligned. */
 int32_t aceapex_set_resident(aceapex_archive* ar, uint32_t slot, uint64_t pos_lo, uint64_t pos_hi, const void* d_ptr);
 
+/* Range decode of [byte_lo, byte_hi) through a bounded device ring (section 5: the range decoder "processes
+ * the archive in chunks, never materializing the full output at once"; BASELINE.json north_star (6)).  The library owns the
+ * window order, the slot rotation and the resident registration (aceapex_set_resident); the caller owns the memory.
+ *   d_ring / ring_bytes: device buffer, 16-byte aligned; it is cut into n_slots = min(8, ring_bytes / window_bytes) slots.
+ *   window_bytes: multiple of the block size (the last window may be shorter); byte_lo must be a multiple of it too.
+ *   Window w is decoded into slot w % n_slots.  Before a slot is overwritten its registration is cleared; after the decode
+ *   has been queued it is registered again, so that later windows find its bytes as match sources instead of rebuilding
+ *   them.  Everything runs on the handle's stream, in order: the decode of window w + n_slots, which overwrites the slot
+ *   of window w, is queued after whatever the consumer queued for window w.
+ *   consumer_or_null(user, window_index, window_lo, window_hi, d_window, cuda_stream) is called on the host once per
+ *   window, after its decode has been queued; it may queue device work that reads d_window on cuda_stream (any other
+ *   stream must be ordered by the consumer itself) and returns 0 to go on, anything else to stop (E_ARG is returned).
+ *   With a null consumer and an FNV section in the archive the library's own consumer checks every block of every window
+ *   on the device and reports the number of bad blocks in stats.
+ *   vram_budget: as in aceapex_decode_range.  stats_or_null receives the figures below.  Synchronous: returns after the
+ *   last window has completed.  Resident slots set by the caller before the call are overwritten and cleared. */
+typedef int32_t (*aceapex_window_fn)(void* user, uint64_t window_index, uint64_t window_lo, uint64_t window_hi, const void* d_window,
+                                     void* cuda_stream);
+typedef struct {
+    uint64_t n_windows;          /* windows decoded                                                            */
+    uint64_t n_slots;            /* ring slots used                                                            */
+    uint64_t bytes;              /* output bytes produced                                                      */
+    uint64_t bad_blocks;         /* built-in consumer only: blocks whose FNV-1a differs                       */
+    uint64_t peak_device_bytes;  /* archive + ring + workspace: everything the decode needs resident in VRAM  */
+    float device_ms;             /* CUDA-event time from the first launch to the last                          */
+    float min_window_gbs;        /* slowest / fastest window (10^9 B/s of output, CUDA events per window)     */
+    float max_window_gbs;
+    uint32_t reserved;
+} aceapex_stream_stats_t;
+int32_t aceapex_decode_stream(aceapex_archive* ar, uint64_t byte_lo, uint64_t byte_hi, void* d_ring, uint64_t ring_bytes,
+                              uint64_t window_bytes, aceapex_window_fn consumer_or_null, void* user, uint64_t vram_budget,
+                              aceapex_stream_stats_t* stats_or_null);
+
 /* Device FNV-1a 64 of each block of d_data (= decompressed bytes [byte_lo, byte_hi), byte_lo block aligned) compared
  * with the archive's FNV section ("FNV for device-resident GPU paths").  Synchronous; *n_bad = number
  * of mismatching blocks.  E_ARG when the archive has no FNV section. */

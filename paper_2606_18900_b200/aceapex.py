@@ -27,6 +27,14 @@ class Info(ctypes.Structure):
                                                "has_fnv", "resident_warps", "segment_size", "q_min", "q_mode")]
 
 
+class StreamStats(ctypes.Structure):
+    _fields_ = [(k, ctypes.c_uint64) for k in ("n_windows", "n_slots", "bytes", "bad_blocks", "peak_device_bytes")] + \
+               [(k, ctypes.c_float) for k in ("device_ms", "min_window_gbs", "max_window_gbs")] + [("reserved", ctypes.c_uint32)]
+
+
+WINDOW_FN = ctypes.CFUNCTYPE(ctypes.c_int32, ctypes.c_void_p, ctypes.c_uint64, ctypes.c_uint64, ctypes.c_uint64, ctypes.c_void_p, ctypes.c_void_p)
+
+
 def lib_path():
     return os.path.join(_PKG, "libaceapex.so")
 
@@ -51,6 +59,7 @@ def load():
             "aceapex_decode_all_fused": ([p, p], i32),
             "aceapex_decode_range": ([p, u64, u64, p, u64], i32),
             "aceapex_decode_reads": ([p, p, u64, p, u64, p], i32),
+            "aceapex_decode_stream": ([p, u64, u64, p, u64, u64, WINDOW_FN, p, u64, ctypes.POINTER(StreamStats)], i32),
             "aceapex_reads_bytes": ([p, u64, p, u64, ctypes.POINTER(u64), p], i32),
             "aceapex_set_resident": ([p, u32, u64, u64, p], i32),
             "aceapex_verify_fnv": ([p, p, u64, u64, ctypes.POINTER(u64)], i32),
@@ -182,6 +191,15 @@ class Archive:
         self._chk(self.L.aceapex_decode_reads(self.h, read_index.ctypes.data, read_index.size, read_ids.ctypes.data,
                                          read_ids.size, out.data_ptr()), "decode_reads")
         return out
+
+    def decode_stream(self, lo, hi, ring, window_bytes, consumer=None, vram_budget=0):
+        """Range decode through the ring tensor (aceapex_decode_stream).  consumer(window_index, lo, hi, d_window_ptr, stream_ptr)
+        -> 0 to go on; None: the library's device FNV consumer.  Returns the statistics as a dict."""
+        st = StreamStats()
+        cb = WINDOW_FN(lambda user, w, a, b, ptr, stream: int(consumer(w, a, b, ptr, stream) or 0)) if consumer else WINDOW_FN()
+        self._chk(self.L.aceapex_decode_stream(self.h, lo, hi, ring.data_ptr(), ring.numel(), window_bytes, cb, None, vram_budget,
+                                               ctypes.byref(st)), "decode_stream")
+        return {k: getattr(st, k) for k, _ in StreamStats._fields_ if k != "reserved"}
 
     def set_resident(self, slot, lo, hi, tensor):
         self._chk(self.L.aceapex_set_resident(self.h, slot, lo, hi, tensor.data_ptr() if tensor is not None else None))

@@ -768,6 +768,61 @@ int32_t aceapex_set_resident(aceapex_archive* ar, uint32_t slot, uint64_t lo, ui
     return ACEAPEX_OK;
 }
 
+int32_t aceapex_decode_stream(aceapex_archive* ar, uint64_t lo, uint64_t hi, void* d_ring, uint64_t ring_bytes, uint64_t window,
+                              aceapex_window_fn consumer, void* user, uint64_t budget, aceapex_stream_stats_t* stats) {
+    if (!ar) return ACEAPEX_E_ARG;
+    if (lo > hi || hi > ar->N) return ACEAPEX_E_RANGE;
+    const uint64_t BS = 1ull << ar->log2_bs;
+    if (!d_ring || (reinterpret_cast<uintptr_t>(d_ring) & 15) || window == 0 || window % BS || lo % window || ring_bytes < window) return ACEAPEX_E_ARG;
+    const uint64_t n_slots = std::min<uint64_t>(MAX_RESIDENT, ring_bytes / window), n_win = (hi - lo + window - 1) / window;
+    aceapex_stream_stats_t st; memset(&st, 0, sizeof st);
+    st.n_slots = n_slots; st.peak_device_bytes = ar->archive_bytes + n_slots * window + ar->ws_need;
+    int32_t rc = prepare_ws(ar);
+    if (rc) return rc;
+    for (uint32_t s = 0; s < MAX_RESIDENT; s++) ar->res[s].lo = ar->res[s].hi = 0;
+    const bool own_check = !consumer && (ar->flags & 1);
+    unsigned long long* bad = reinterpret_cast<unsigned long long*>(ar->d_ws + 16);
+    if (own_check) CU(cudaMemsetAsync(bad, 0, 8, ar->stream));
+    std::vector<cudaEvent_t> ev(n_win + 1);
+    for (auto& e : ev) CU(cudaEventCreate(&e));
+    CU(cudaEventRecord(ev[0], ar->stream));
+    for (uint64_t w = 0; w < n_win && !rc; w++) {
+        const uint64_t wlo = lo + w * window, whi = std::min<uint64_t>(hi, wlo + window);
+        const uint32_t slot = (uint32_t)(w % n_slots);
+        uint8_t* d_win = static_cast<uint8_t*>(d_ring) + slot * window;
+        ar->res[slot].lo = ar->res[slot].hi = 0;               // cleared BEFORE its buffer is overwritten
+        rc = aceapex_decode_range(ar, wlo, whi, d_win, budget);
+        if (rc) break;
+        ar->res[slot].lo = wlo; ar->res[slot].hi = whi; ar->res[slot].ptr = d_win;
+        if (own_check) {
+            const uint64_t nb = (whi - wlo + BS - 1) >> ar->log2_bs;
+            const uint64_t* expect = reinterpret_cast<const uint64_t*>(ar->d_archive + ar->fnv_off) + (wlo >> ar->log2_bs);
+            k_fnv<<<(unsigned)((nb + 127) / 128), 128, 0, ar->stream>>>(d_win, whi - wlo, ar->log2_bs, expect, bad);
+            ar->launches++;
+        } else if (consumer && consumer(user, w, wlo, whi, d_win, ar->stream)) rc = ACEAPEX_E_ARG;
+        cudaEventRecord(ev[w + 1], ar->stream);
+        st.n_windows++; st.bytes += whi - wlo;
+    }
+    cudaError_t ce = cudaStreamSynchronize(ar->stream);
+    for (uint32_t s = 0; s < MAX_RESIDENT; s++) ar->res[s].lo = ar->res[s].hi = 0;
+    if (!rc && ce == cudaSuccess && st.n_windows) {
+        cudaEventElapsedTime(&st.device_ms, ev[0], ev[st.n_windows]);
+        st.min_window_gbs = 1e30f;
+        for (uint64_t w = 0; w < st.n_windows; w++) {
+            float ms = 0; cudaEventElapsedTime(&ms, ev[w], ev[w + 1]);
+            const uint64_t wlo = lo + w * window, whi = std::min<uint64_t>(hi, wlo + window);
+            const float g = ms > 0 ? (float)((whi - wlo) / (ms * 1e6)) : 0.f;
+            st.min_window_gbs = std::min(st.min_window_gbs, g); st.max_window_gbs = std::max(st.max_window_gbs, g);
+        }
+        if (own_check) { unsigned long long h = 0; ce = cudaMemcpy(&h, bad, 8, cudaMemcpyDeviceToHost); st.bad_blocks = h; }
+    }
+    for (auto& e : ev) cudaEventDestroy(e);
+    if (stats) *stats = st;
+    if (rc) return rc;
+    CU(ce);
+    return ACEAPEX_OK;
+}
+
 int32_t aceapex_verify_fnv(aceapex_archive* ar, const void* d_data, uint64_t lo, uint64_t hi, uint64_t* n_bad) {
     if (!ar || !n_bad || !(ar->flags & 1) || (lo & ((1ull << ar->log2_bs) - 1)) || lo > hi || hi > ar->N) return ACEAPEX_E_ARG;
     int32_t rc = prepare_ws(ar);

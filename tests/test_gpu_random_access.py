@@ -295,3 +295,62 @@ def test_small_vram_budget_means_more_sub_windows_not_failure(big):
         assert got.cpu().numpy().tobytes() == x[lo:hi].tobytes(), budget
         served += 1
     assert served >= 3
+
+
+def test_decode_stream_ring_in_the_library(big):
+    """aceapex_decode_stream: the library owns window order, slot rotation and resident registration.  A
+    file larger than the ring, (a) checked by the library's own device FNV consumer, (b) handed window by window to a
+    consumer that only counts callbacks and compares each window with the original bytes, (c) stopped by the consumer."""
+    import ctypes
+    from paper_2606_18900_b200.aceapex import AceapexError
+    for ar, x in big:
+        N = x.size
+        W = 64 * 16384                                    # 1 MiB windows
+        ring = ar.new_output(3 * W + 4096)                # three slots (and some slack the library must not need)
+        st = ar.decode_stream(0, N, ring, W)
+        assert st["n_windows"] == (N + W - 1) // W and st["n_slots"] == 3 and st["bytes"] == N and st["bad_blocks"] == 0
+        assert st["device_ms"] > 0 and 0 < st["min_window_gbs"] <= st["max_window_gbs"]
+        assert st["peak_device_bytes"] == ar.info()["archive_bytes"] + 3 * W + ar.info()["workspace_bytes"]
+        seen = []
+
+        errors0 = []
+
+        def consumer(w, lo, hi, ptr, stream):
+            try:
+                torch.cuda.synchronize()                   # a real consumer would queue device work on `stream`
+                off = ptr - ring.data_ptr()
+                assert off % W == 0 and off // W == w % 3   # slot rotation
+                assert ring[off:off + hi - lo].cpu().numpy().tobytes() == x[lo:hi].tobytes(), w
+            except Exception as exc:
+                errors0.append(exc)
+            seen.append((w, lo, hi))
+            return 0
+        st = ar.decode_stream(0, N, ring, W, consumer=consumer)
+        assert not errors0, errors0
+        assert [s[0] for s in seen] == list(range(st["n_windows"])) and seen[-1][2] == N and st["bad_blocks"] == 0
+        # a sub-range that starts at a window boundary in the middle of the file, two slots
+        seen.clear()
+        ring2 = ar.new_output(2 * W)
+        lo0 = 5 * W
+
+        errors = []
+
+        def consumer2(w, lo, hi, ptr, stream):
+            try:                                           # an exception inside a ctypes callback would be swallowed
+                torch.cuda.synchronize()
+                off = ptr - ring2.data_ptr()
+                assert lo == lo0 + w * W and ring2[off:off + hi - lo].cpu().numpy().tobytes() == x[lo:hi].tobytes(), w
+            except Exception as exc:
+                errors.append(exc)
+            seen.append(w)
+            return 1 if w == 1 else 0                     # the consumer stops the stream
+        with pytest.raises(AceapexError) as e:
+            ar.decode_stream(lo0, N, ring2, W, consumer=consumer2)
+        assert not errors, errors
+        assert e.value.name == "E_ARG" and seen == [0, 1]
+        ar.check()
+        for bad_args in ((0, N, ring, W + 1), (W // 2, N, ring, W), (0, N, ring[:W // 2], W)):
+            with pytest.raises(AceapexError):
+                ar.decode_stream(*bad_args)
+        # the stream left no resident slot behind: a plain range decode afterwards rebuilds its sources itself
+        check_range(ar, x, 5 * W + 3, min(N, 7 * W + 5))
