@@ -192,6 +192,10 @@ int32_t aceapex_phase_times(aceapex_archive* ar, float* ms3);
 
 /* Number of kernel launches the library issued on this handle so far (bench.py "gpu_launches"). */
 uint64_t aceapex_launch_count(const aceapex_archive* ar);
+/* Number of those that went out as nodes of a replayed CUDA graph: aceapex_decode_range calls of up to 8 MiB on a level-0
+ * archive record their launch sequence once and replay it with updated node parameters (seek latency is
+ * launch overhead).  ACEAPEX_NO_GRAPHS in the environment at open switches that off. */
+uint64_t aceapex_graph_launch_count(const aceapex_archive* ar);
 
 enum {
     ACEAPEX_DF_RANS = 1,      /* final rANS state / word count mismatch         */

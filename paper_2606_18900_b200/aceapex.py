@@ -69,6 +69,7 @@ def load():
             "aceapex_last_cuda_error": ([p], i32),
             "aceapex_strerror": ([i32], ctypes.c_char_p),
             "aceapex_launch_count": ([p], u64),
+            "aceapex_graph_launch_count": ([p], u64),
             "aceapex_set_phase_timing": ([p, i32], i32),
             "aceapex_phase_times": ([p, ctypes.POINTER(ctypes.c_float)], i32),
         }
@@ -147,6 +148,9 @@ class Archive:
 
     def launch_count(self):
         return int(self.L.aceapex_launch_count(self.h))
+
+    def graph_launch_count(self):
+        return int(self.L.aceapex_graph_launch_count(self.h))
 
     def close(self):
         if self.h:

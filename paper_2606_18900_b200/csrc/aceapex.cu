@@ -14,9 +14,19 @@ using namespace acx;
 
 // ====================================================================================================== host =====
 
-struct SeekGraph {                                      // a captured launch sequence (aceapex_decode_range / _reads, see "graphs")
-    cudaGraphExec_t exec = nullptr;
-    uint64_t key = ~0ull;                               // what the captured sequence depends on
+// A launch sequence kept as a CUDA graph (seek latency "dominated by fixed kernel-launch
+// overhead").  A seek issues the same kernels in the same order every time, only their arguments differ: the calls are
+// recorded instead of launched, the node parameters of the instantiated graph are updated in place, and one
+// cudaGraphLaunch replaces six to ten launches and memsets.
+struct GNode {
+    const void* func = nullptr;                         // null: a memset node
+    dim3 grid, block; size_t smem = 0; bool coop = false;
+    std::vector<uint8_t> blob; std::vector<size_t> arg_off;   // kernel arguments, copied
+    void* ptr = nullptr; size_t bytes = 0;              // memset
+};
+struct SeekGraph {
+    cudaGraph_t graph = nullptr; cudaGraphExec_t exec = nullptr;
+    std::vector<cudaGraphNode_t> nodes; std::vector<const void*> sig;
 };
 
 struct aceapex_archive {
@@ -60,8 +70,10 @@ struct aceapex_archive {
     bool phase_timing = false; cudaEvent_t ev_phase[4] = {nullptr, nullptr, nullptr, nullptr};   // aceapex_set_phase_timing
     std::vector<uint32_t> h_list; std::vector<Demand> h_demands;   // host staging for range / read calls
     // CUDA graphs of the seek / single-read paths
-    bool use_graphs = true; bool capturing = false;
-    SeekGraph g_seek, g_read;
+    bool use_graphs = true; bool capturing = false;     // capturing: launches are recorded into `rec` instead of issued
+    std::vector<GNode> rec;
+    SeekGraph g_seek;
+    uint64_t graph_launches = 0, graph_rebuilds = 0;
     // status
     int32_t last_cuda = 0; uint32_t dev_flags = 0; uint64_t launches = 0;
 };
@@ -155,7 +167,6 @@ void set_out(Params& P, uint8_t* out, uint64_t pos0, uint64_t end) {
 int32_t prepare_ws(aceapex_archive* ar) {
     if (!ar->d_ws || ar->ws_bytes < ar->ws_need) return ACEAPEX_E_WORKSPACE;
     if (!ar->ws_clean) {
-        if (ar->capturing) return ACEAPEX_E_ARG;
         CU(cudaMemsetAsync(ar->d_ws, 0, ar->scratch_off, ar->stream));
         for (int k = 0; k < 2; k++) CU(cudaMemsetAsync(ar->d_ws + ar->gl_cnt_off[k], 0, 4 * ar->n_segs + 4, ar->stream));
         ar->ws_clean = true; ar->ticket_slot = 0;
@@ -177,6 +188,85 @@ void take_ticket(aceapex_archive* ar, Params& P) {
     ar->ticket_slot ^= 1;
 }
 
+constexpr int32_t NOT_GRAPHABLE = 1;                    // internal: the call needs something a recorded sequence cannot hold
+
+struct KArg { const void* p; size_t n; };
+int32_t submit_kernel(aceapex_archive* ar, const void* func, dim3 grid, dim3 block, size_t smem, bool coop, std::initializer_list<KArg> args) {
+    if (ar->capturing) {
+        GNode nd; nd.func = func; nd.grid = grid; nd.block = block; nd.smem = smem; nd.coop = coop;
+        for (const KArg& a : args) {
+            const size_t off = (nd.blob.size() + 15) & ~(size_t)15;
+            nd.blob.resize(off + a.n); memcpy(nd.blob.data() + off, a.p, a.n); nd.arg_off.push_back(off);
+        }
+        ar->rec.push_back(std::move(nd));
+        ar->launches++;
+        return ACEAPEX_OK;
+    }
+    void* argv[4]; int k = 0;
+    for (const KArg& a : args) argv[k++] = const_cast<void*>(a.p);
+    if (coop) CU(cudaLaunchCooperativeKernel(func, grid, block, argv, smem, ar->stream));
+    else CU(cudaLaunchKernel(func, grid, block, argv, smem, ar->stream));
+    ar->launches++;
+    return ACEAPEX_OK;
+}
+int32_t submit_memset(aceapex_archive* ar, void* ptr, size_t bytes) {
+    if (ar->capturing) { GNode nd; nd.ptr = ptr; nd.bytes = bytes; ar->rec.push_back(std::move(nd)); return ACEAPEX_OK; }
+    CU(cudaMemsetAsync(ptr, 0, bytes, ar->stream));
+    return ACEAPEX_OK;
+}
+
+// launches the recorded sequence as a graph: same sequence of kernels as the instantiated one -> parameters updated in place
+int32_t replay(aceapex_archive* ar) {
+    SeekGraph& G = ar->g_seek;
+    std::vector<const void*> sig;
+    for (const GNode& n : ar->rec) sig.push_back(n.func);
+    std::vector<std::vector<void*>> argv(ar->rec.size());
+    auto kparams = [&](size_t i) {
+        GNode& n = ar->rec[i];
+        cudaKernelNodeParams kp; memset(&kp, 0, sizeof kp);
+        for (size_t off : n.arg_off) argv[i].push_back(n.blob.data() + off);
+        kp.func = const_cast<void*>(n.func); kp.gridDim = n.grid; kp.blockDim = n.block; kp.sharedMemBytes = (unsigned)n.smem; kp.kernelParams = argv[i].data();
+        return kp;
+    };
+    auto mparams = [&](size_t i) {
+        cudaMemsetParams mp; memset(&mp, 0, sizeof mp);
+        mp.dst = ar->rec[i].ptr; mp.value = 0; mp.elementSize = 1; mp.width = ar->rec[i].bytes; mp.height = 1; mp.pitch = ar->rec[i].bytes;
+        return mp;
+    };
+    bool ok = G.exec && sig == G.sig;
+    if (ok) {
+        for (size_t i = 0; i < ar->rec.size() && ok; i++) {
+            if (ar->rec[i].func) { cudaKernelNodeParams kp = kparams(i); ok = cudaGraphExecKernelNodeSetParams(G.exec, G.nodes[i], &kp) == cudaSuccess; }
+            else { cudaMemsetParams mp = mparams(i); ok = cudaGraphExecMemsetNodeSetParams(G.exec, G.nodes[i], &mp) == cudaSuccess; }
+        }
+        if (!ok) cudaGetLastError();
+    }
+    if (!ok) {                                           // first use, or another sequence: build and instantiate
+        if (G.exec) { cudaGraphExecDestroy(G.exec); G.exec = nullptr; }
+        if (G.graph) { cudaGraphDestroy(G.graph); G.graph = nullptr; }
+        for (auto& v : argv) v.clear();
+        CU(cudaGraphCreate(&G.graph, 0));
+        G.nodes.assign(ar->rec.size(), nullptr);
+        for (size_t i = 0; i < ar->rec.size(); i++) {
+            const cudaGraphNode_t* dep = i ? &G.nodes[i - 1] : nullptr;
+            if (ar->rec[i].func) {
+                cudaKernelNodeParams kp = kparams(i);
+                CU(cudaGraphAddKernelNode(&G.nodes[i], G.graph, dep, i ? 1 : 0, &kp));
+                if (ar->rec[i].coop) {
+                    cudaKernelNodeAttrValue v; memset(&v, 0, sizeof v); v.cooperative = 1;
+                    CU(cudaGraphKernelNodeSetAttribute(G.nodes[i], cudaKernelNodeAttributeCooperative, &v));
+                }
+            } else { cudaMemsetParams mp = mparams(i); CU(cudaGraphAddMemsetNode(&G.nodes[i], G.graph, dep, i ? 1 : 0, &mp)); }
+        }
+        CU(cudaGraphInstantiate(&G.exec, G.graph, 0));
+        G.sig = sig;
+        ar->graph_rebuilds++;
+    }
+    CU(cudaGraphLaunch(G.exec, ar->stream));
+    ar->graph_launches++;
+    return ACEAPEX_OK;
+}
+
 enum Kind { K_LIT, K_COPY_TOP, K_COPY_WAIT, K_COPY_WIN, K_COPY_WIN_WAIT, K_COLLECT, K_SERVE, K_SPANS };
 
 int32_t launch(aceapex_archive* ar, Params& P, Kind kind, uint64_t n_work) {
@@ -186,30 +276,26 @@ int32_t launch(aceapex_archive* ar, Params& P, Kind kind, uint64_t n_work) {
     int T; uint32_t g;
     spread(ar, n_work, ar->threads, g, T);
     const size_t sm_e = entropy_smem(ar->n_coded_tables, ar->q_mode, ar->runs_bytes + ar->lita_bytes, T), sm_c = (size_t)(T / 32) * COPY_WARP_BYTES + 64;
+    const void* f = nullptr; size_t sm = sm_c; dim3 gd(g), bd(T);
     switch (kind) {
         case K_LIT:
-            if (!ar->q_mode) { if (ar->q_min >= 64) k_literals<3><<<g, T, sm_e, ar->stream>>>(P); else k_literals<0><<<g, T, sm_e, ar->stream>>>(P); }
-            else if (P.out_odd) k_literals<2><<<g, T, sm_e, ar->stream>>>(P);
-            else if (ar->q_min >= 64) k_literals<4><<<g, T, sm_e, ar->stream>>>(P);
-            else k_literals<1><<<g, T, sm_e, ar->stream>>>(P);
+            sm = sm_e;
+            if (!ar->q_mode) f = ar->q_min >= 64 ? (const void*)k_literals<3> : (const void*)k_literals<0>;
+            else if (P.out_odd) f = (const void*)k_literals<2>;
+            else f = ar->q_min >= 64 ? (const void*)k_literals<4> : (const void*)k_literals<1>;
             break;
-        case K_COPY_TOP: k_copy<false, false, false, true><<<g, T, sm_c, ar->stream>>>(P); break;
-        case K_COPY_WAIT: k_copy<true, false, false, false><<<g, T, sm_c, ar->stream>>>(P); break;
-        case K_COPY_WIN: k_copy<false, true, false, false><<<g, T, sm_c, ar->stream>>>(P); break;
-        case K_COPY_WIN_WAIT: k_copy<true, true, false, false><<<g, T, sm_c, ar->stream>>>(P); break;
-        case K_COLLECT: k_copy<false, true, true, false><<<g, T, sm_c, ar->stream>>>(P); break;
-        case K_SERVE: k_serve<<<ar->sms, ar->threads, ar->smem_entropy, ar->stream>>>(P); break;
-        case K_SPANS: k_spans<<<g, T, sm_e, ar->stream>>>(P); break;
+        case K_COPY_TOP: f = (const void*)k_copy<false, false, false, true>; break;
+        case K_COPY_WAIT: f = (const void*)k_copy<true, false, false, false>; break;
+        case K_COPY_WIN: f = (const void*)k_copy<false, true, false, false>; break;
+        case K_COPY_WIN_WAIT: f = (const void*)k_copy<true, true, false, false>; break;
+        case K_COLLECT: f = (const void*)k_copy<false, true, true, false>; break;
+        case K_SERVE: f = (const void*)k_serve; sm = ar->smem_entropy; gd = dim3(ar->sms); bd = dim3(ar->threads); break;
+        case K_SPANS: f = (const void*)k_spans; sm = sm_e; break;
     }
-    CU(cudaGetLastError());
-    ar->launches++;
-    return ACEAPEX_OK;
+    return submit_kernel(ar, f, gd, bd, sm, false, {{&P, sizeof P}});
 }
 
-int32_t zero_done(aceapex_archive* ar, uint64_t b0, uint64_t nb) {
-    CU(cudaMemsetAsync(ar->d_ws + ar->done_off + 4 * b0, 0, 4 * nb, ar->stream));
-    return ACEAPEX_OK;
-}
+int32_t zero_done(aceapex_archive* ar, uint64_t b0, uint64_t nb) { return submit_memset(ar, ar->d_ws + ar->done_off + 4 * b0, 4 * nb); }
 
 } // namespace
 
@@ -440,7 +526,8 @@ int32_t aceapex_close(aceapex_archive* ar) {
     for (cudaEvent_t e : ar->ev_h2d) cudaEventDestroy(e);
     for (cudaEvent_t e : ar->ev_dec) cudaEventDestroy(e);
     for (cudaEvent_t e : ar->ev_phase) if (e) cudaEventDestroy(e);
-    for (SeekGraph* g : {&ar->g_seek, &ar->g_read}) if (g->exec) cudaGraphExecDestroy(g->exec);
+    if (ar->g_seek.exec) cudaGraphExecDestroy(ar->g_seek.exec);
+    if (ar->g_seek.graph) cudaGraphDestroy(ar->g_seek.graph);
     if (ar->s_h2d) cudaStreamDestroy(ar->s_h2d);
     if (ar->s_d2h) cudaStreamDestroy(ar->s_d2h);
     delete ar;
@@ -462,7 +549,6 @@ int32_t aceapex_info(const aceapex_archive* ar, aceapex_info_t* o) {
 int32_t aceapex_set_workspace(aceapex_archive* ar, void* d_ws, uint64_t bytes) {
     if (!ar || (reinterpret_cast<uintptr_t>(d_ws) & 255)) return ACEAPEX_E_ARG;
     ar->d_ws = static_cast<uint8_t*>(d_ws); ar->ws_bytes = bytes; ar->ws_clean = false;
-    for (SeekGraph* g : {&ar->g_seek, &ar->g_read}) if (g->exec) { cudaGraphExecDestroy(g->exec); g->exec = nullptr; g->key = ~0ull; }
     return (d_ws && bytes >= ar->ws_need) ? ACEAPEX_OK : ACEAPEX_E_WORKSPACE;
 }
 
@@ -567,23 +653,22 @@ static void add_demands(aceapex_archive* ar, uint64_t pos, uint64_t len, uint64_
 // Serves the demand list g[0] (filled by the caller) in at most `rounds` rounds; the list left by the last round must be
 // empty.  One cooperative launch (k_rounds) where the device supports it, else three launches per round.
 static int32_t serve_rounds(aceapex_archive* ar, Params Q, const GList g[2], uint32_t rounds) {
+    int32_t rc;
     if (ar->cooperative && rounds <= 16) {
         unsigned long long* tickets = reinterpret_cast<unsigned long long*>(ar->d_ws + 128);     // 16 counters in the control area
-        CU(cudaMemsetAsync(tickets, 0, 128, ar->stream));
+        if ((rc = submit_memset(ar, tickets, 128))) return rc;
         Q.gl_cur = g[0]; Q.gl_nxt = g[1];
-        void* args[] = {&Q, &tickets, &rounds};
-        CU(cudaLaunchCooperativeKernel((const void*)k_rounds, dim3(ar->sms), dim3(ar->threads), args, ar->smem_entropy, ar->stream));
-        ar->launches++;
-        return ACEAPEX_OK;
+        return submit_kernel(ar, (const void*)k_rounds, dim3(ar->sms), dim3(ar->threads), ar->smem_entropy, true,
+                             {{&Q, sizeof Q}, {&tickets, sizeof tickets}, {&rounds, sizeof rounds}});
     }
+    if (ar->capturing) return NOT_GRAPHABLE;
     for (uint32_t r = 0; r < rounds; r++) {
         Q.gl_cur = g[r & 1]; Q.gl_nxt = g[(r + 1) & 1];
         CU(cudaMemsetAsync(Q.gl_nxt.count, 0, 16, ar->stream));
         k_plan<<<ar->sms, 256, 0, ar->stream>>>(Q);          // bucket offsets + work items
         k_scatter<<<4 * ar->sms, 256, 0, ar->stream>>>(Q);
         ar->launches += 2;
-        int32_t rc = launch(ar, Q, K_SERVE, 1);
-        if (rc) return rc;
+        if ((rc = launch(ar, Q, K_SERVE, 1))) return rc;
     }
     k_assert_empty<<<1, 1, 0, ar->stream>>>(g[rounds & 1].count, Q.err);
     CU(cudaGetLastError());
@@ -611,7 +696,7 @@ static int32_t range_launches(aceapex_archive* ar, uint64_t lo, uint64_t hi, uin
         for (uint64_t w0 = s0; w0 < s1;) {                  // sub-windows whose demands fit the lists
             uint64_t w1 = w0 + 1;
             while (w1 < s1 && ar->h_match_prefix[w1 + 1] - ar->h_match_prefix[w0] <= ar->gl_eff / 3) w1++;
-            CU(cudaMemsetAsync(g[0].count, 0, 32, ar->stream));
+            if ((rc = submit_memset(ar, g[0].count, 32))) return rc;
             P.seg_list = nullptr; P.first_work = w0; P.gl_nxt = g[0];
             if ((rc = launch(ar, P, K_COLLECT, w1 - w0))) return rc;
             Params Q = P;                                   // serving knows no window: sources of foreign bytes precede it
@@ -626,7 +711,7 @@ static int32_t range_launches(aceapex_archive* ar, uint64_t lo, uint64_t hi, uin
         } else {
             // its segments sorted by (level, index) in one flag-driven launch (a segment waits for lower-level source
             // blocks of the window only; everything outside the window is final)
-            if (ar->capturing) return ACEAPEX_E_ARG;
+            if (ar->capturing) return NOT_GRAPHABLE;
             std::vector<uint32_t>& L = ar->h_list;
             L.resize(ns);
             std::vector<uint64_t> cnt(ar->max_level + 2, 0);
@@ -650,17 +735,18 @@ static int32_t range_launches(aceapex_archive* ar, uint64_t lo, uint64_t hi, uin
     if (!ar->h_demands.empty()) {
         const GList g[2] = {glist(ar, 0), glist(ar, 1)};
         const uint32_t n = (uint32_t)ar->h_demands.size();      // at most a handful: two spans cut at block boundaries
-        CU(cudaMemsetAsync(g[0].count, 0, 32, ar->stream));
+        if ((rc = submit_memset(ar, g[0].count, 32))) return rc;
         Params Q = P;
         if (alo >= ahi) { Q.out_pos0 = 0; Q.win_end = 0; }
         Q.out2 = out; Q.gl_nxt = g[0];
         Demand* d_dem = reinterpret_cast<Demand*>(ar->d_ws + ar->demands_off);
         Q.demands = d_dem; Q.n_inline = 0;
         if (n <= 4) { Q.n_inline = n; for (uint32_t i = 0; i < n; i++) Q.inline_dem[i] = ar->h_demands[i]; }
-        else CU(cudaMemcpyAsync(d_dem, ar->h_demands.data(), n * sizeof(Demand), cudaMemcpyHostToDevice, ar->stream));
-        k_seed<<<(n + 127) / 128, 128, 0, ar->stream>>>(Q, n);
-        CU(cudaGetLastError());
-        ar->launches++;
+        else {
+            if (ar->capturing) return NOT_GRAPHABLE;
+            CU(cudaMemcpyAsync(d_dem, ar->h_demands.data(), n * sizeof(Demand), cudaMemcpyHostToDevice, ar->stream));
+        }
+        if ((rc = submit_kernel(ar, (const void*)k_seed, dim3((n + 127) / 128), dim3(128), 0, false, {{&Q, sizeof Q}, {&n, sizeof n}}))) return rc;
         if ((rc = serve_rounds(ar, Q, g, ar->max_level + 3))) return rc;   // one more round: the span's own segment comes first
     }
     return ACEAPEX_OK;
@@ -682,8 +768,20 @@ int32_t aceapex_decode_range(aceapex_archive* ar, uint64_t lo, uint64_t hi, void
     }
     int32_t rc = prepare_ws(ar);
     if (rc) return rc;
+    // a seek (up to a few hundred blocks): the launch sequence is replayed as a CUDA graph
+    if (ar->use_graphs && ar->cooperative && hi - lo <= (8ull << 20)) {
+        const uint64_t l0 = ar->launches; const uint32_t slot0 = ar->ticket_slot;
+        ar->capturing = true; ar->rec.clear();
+        rc = range_launches(ar, lo, hi, static_cast<uint8_t*>(d_out));
+        ar->capturing = false;
+        if (rc == ACEAPEX_OK) return ar->rec.empty() ? ACEAPEX_OK : replay(ar);
+        if (rc != NOT_GRAPHABLE) return rc;
+        ar->launches = l0; ar->ticket_slot = slot0;       // nothing was issued: do it again with plain launches
+    }
     return range_launches(ar, lo, hi, static_cast<uint8_t*>(d_out));
 }
+
+uint64_t aceapex_graph_launch_count(const aceapex_archive* ar) { return ar ? ar->graph_launches : 0; }
 
 int32_t aceapex_reads_bytes(const uint64_t* idx, uint64_t n_index, const uint64_t* ids, uint64_t n, uint64_t* total, uint64_t* offs) {
     if ((!idx && n_index) || (!ids && n) || !total) return ACEAPEX_E_ARG;
@@ -746,14 +844,12 @@ int32_t aceapex_decode_reads(aceapex_archive* ar, const uint64_t* idx, uint64_t 
         const size_t chunk = std::max<size_t>(1, std::min<size_t>(ar->demand_cap, ar->gl_cap / 8));
         for (size_t i = 0; i < ar->h_demands.size(); i += chunk) {
             const uint32_t m = (uint32_t)std::min<size_t>(chunk, ar->h_demands.size() - i);
-            CU(cudaMemsetAsync(g[0].count, 0, 32, ar->stream));
+            if ((rc = submit_memset(ar, g[0].count, 32))) return rc;
             Params Q = P;
             Q.gl_nxt = g[0]; Q.demands = d_dem; Q.n_inline = 0;
             if (m <= 4) { Q.n_inline = m; for (uint32_t k = 0; k < m; k++) Q.inline_dem[k] = ar->h_demands[i + k]; }
             else CU(cudaMemcpyAsync(d_dem, ar->h_demands.data() + i, m * sizeof(Demand), cudaMemcpyHostToDevice, ar->stream));
-            k_seed<<<(m + 127) / 128, 128, 0, ar->stream>>>(Q, m);
-            CU(cudaGetLastError());
-            ar->launches++;
+            if ((rc = submit_kernel(ar, (const void*)k_seed, dim3((m + 127) / 128), dim3(128), 0, false, {{&Q, sizeof Q}, {&m, sizeof m}}))) return rc;
             if ((rc = serve_rounds(ar, Q, g, ar->max_level + 3))) return rc;
             if (i + chunk < ar->h_demands.size()) CU(cudaStreamSynchronize(ar->stream));   // the staging area is reused
         }

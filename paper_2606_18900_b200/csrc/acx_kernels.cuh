@@ -77,6 +77,9 @@ __device__ __forceinline__ bool load_seg(const Params& P, SegCtx& c) {
     c.send = seg_end(P, c.s, c.b);
     c.payload = P.archive + c.d.payload_off;
     const uint64_t rans_bytes = 256 + 2ull * c.d.n_words;
+    // the whole payload towards L2 now: a warp that is alone on its SM (a seek, a read) would otherwise meet DRAM latency at
+    // every ring refill; in a full launch the lines arrive a little earlier than their first use
+    for (uint64_t o = 128ull * lane_id(); o < rans_bytes; o += 4096) asm volatile("prefetch.global.L2 [%0];" ::"l"(c.payload + o));
     c.ext = reinterpret_cast<const uint32_t*>(c.payload + ((rans_bytes + 3) & ~3ull));
     c.raw_planes = reinterpret_cast<const uint8_t*>(c.ext + c.d.n_ext);
     // the host validated the directory at open (counts within FORMAT.md §1.5, payload inside the archive); these are the
@@ -430,8 +433,10 @@ __device__ __forceinline__ void gl_append(const Params& P, const GList& gl, uint
 __device__ __forceinline__ void push_span(const Params& P, const Stack& st, uint64_t pos, uint64_t len, uint64_t dst) {
     while (len) {                                   // a demand never crosses a segment boundary
         if (pos >= P.N) { report(P, DF_OFFSET); return; }
-        const uint32_t seg = seg_of(P, pos);
-        const uint64_t send = seg_end(P, seg, pos >> P.log2_bs);
+        const uint64_t pb = pos >> P.log2_bs;
+        uint32_t seg = __ldg(P.first_seg + pb);
+        uint64_t send = block_end(P, pb);
+        if (__ldg(P.first_seg + pb + 1) - seg > 1) { seg = seg_of(P, pos); send = seg_end(P, seg, pb); }   // several segments in the block
         const uint64_t n = min((unsigned long long)len, (unsigned long long)(send - pos));
         if (st.gl) gl_append(P, *st.gl, pos, (uint32_t)n, dst, seg);
         else {
