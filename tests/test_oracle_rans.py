@@ -170,3 +170,46 @@ def test_tables_of_precision_11_and_12_interleaved_on_the_same_states():
     ideal = sum(-math.log2(fa[v] / 2048) for v in a) + sum(-math.log2(fb[v] / 4096) for v in b)
     bits = 16 * sum(len(s) for s in streams) + sum(math.log2(x) - 16 for x in states)
     assert abs(bits - ideal) < 64
+
+
+# ---- the row coder of the entropy micro-benchmark (oracle/acx_rans_rows.c) ----------------
+
+def exponential_rows(n_rows, row_bytes, seed=6, scale=12.0):
+    """The micro-benchmark's data shape: exponentially distributed byte values ("256 MB exponential")."""
+    rng = np.random.default_rng(seed)
+    return np.minimum(rng.exponential(scale=scale, size=(n_rows, row_bytes)), 255).astype(np.uint8)
+
+
+@pytest.mark.parametrize("row_bytes", [1, 31, 32, 33, 1000, 4096])
+def test_row_encoder_matches_the_python_encoder_word_for_word(row_bytes):
+    from oracle import acx_rans_rows as R
+    rows = exponential_rows(3, row_bytes, seed=row_bytes)
+    freq = normalise(np.bincount(rows.ravel(), minlength=256).tolist())
+    enc, sizes = R.encode(rows, freq)
+    for r in range(rows.shape[0]):
+        states, streams = rans_encode(rows[r].tolist(), [0] * row_bytes, [freq])
+        words = [w for st in streams for w in st]
+        assert sizes[r] == 256 + 2 * len(words)
+        head = np.frombuffer(enc[r, :256].tobytes(), dtype="<u4").reshape(32, 2)
+        assert head[:, 0].tolist() == states
+        assert head[:, 1].tolist() == np.concatenate([[0], np.cumsum([len(st) for st in streams])[:-1]]).tolist()
+        assert np.frombuffer(enc[r, 256:sizes[r]].tobytes(), dtype="<u2").tolist() == words
+        # and the oracle's own decoder (FORMAT.md 1.7) reads it back
+        sym, final, used = O.rans_decode(np.array([freq], np.uint16), np.zeros(row_bytes, np.uint8), np.array(states, np.uint32), streams)
+        assert sym.tolist() == rows[r].tolist() and (final == 65536).all()
+    assert np.array_equal(R.decode(enc, sizes, row_bytes, freq), rows)
+
+
+def test_row_coder_size_is_the_entropy_bound():
+    from oracle import acx_rans_rows as R
+    rows = exponential_rows(8, 65536)
+    freq = normalise(np.bincount(rows.ravel(), minlength=256).tolist())
+    enc, sizes = R.encode(rows, freq)
+    ideal_bits = sum(-math.log2(freq[v] / M) for v in rows.ravel())
+    got_bits = 8 * (int(sizes.sum()) - 256 * 8)                       # payload words only
+    assert abs(got_bits - ideal_bits) < 8 * 32 * 32 + 0.001 * ideal_bits   # at most ~one word per state and row, 0.1 % slack
+    assert np.array_equal(R.decode(enc, sizes, 65536, freq), rows)
+    bad = enc.copy()
+    bad[3, 300] ^= 0x40
+    with pytest.raises(ValueError):
+        R.decode(bad, sizes, 65536, freq)
