@@ -197,6 +197,30 @@ uint64_t aceapex_launch_count(const aceapex_archive* ar);
  * launch overhead).  ACEAPEX_NO_GRAPHS in the environment at open switches that off. */
 uint64_t aceapex_graph_launch_count(const aceapex_archive* ar);
 
+/* ---- The entropy stage alone (section 6.4: DietGPU ANS on "256 MB exponential, batch 4096 x 64 KB", encode 364.9 /
+ * decode 592.5 GB/s on the H100).  A batch is n_rows rows of row_bytes byte symbols, row r at d_in + r * row_bytes.  Every row
+ * is coded on its own with ONE static table (256 frequencies summing to 2^11) as a rANS section of FORMAT.md 1.7: row r at
+ * d_enc + r * row_capacity = [32 x (u32 initial state, u32 word_off)][u16 words], d_row_sizes[r] = 256 + 2 * words bytes.
+ * One warp per row.  All pointers but h_freq are device memory owned by the caller; the calls are asynchronous on
+ * cuda_stream unless stated.
+ *   aceapex_rans_row_capacity(row_bytes): bytes to reserve per encoded row (the worst case, a multiple of 16).
+ *   aceapex_rans_table_bytes(): size of the device table buffer; aceapex_rans_tables builds the encode and decode tables
+ *     from h_freq and uploads them (synchronous).  E_ARG when the frequencies do not sum to 2^11.
+ *   aceapex_rans_scratch_bytes(row_bytes): device scratch both kernels need (word staging of the encoder, counters).
+ *   aceapex_rans_encode: rows -> encoded rows + sizes.  Every symbol of the input must have a non-zero frequency.
+ *   aceapex_rans_decode: encoded rows -> rows; a row whose states do not end at 2^16 with every word stream consumed
+ *     exactly latches bit 0 of the status word that aceapex_rans_status reads back (synchronous).  The decoder prefetches
+ *     up to 128 bytes past the words of a row: d_enc must be that much longer than n_rows * row_capacity. */
+uint64_t aceapex_rans_row_capacity(uint64_t row_bytes);
+uint64_t aceapex_rans_table_bytes(void);
+uint64_t aceapex_rans_scratch_bytes(uint64_t row_bytes);
+int32_t aceapex_rans_tables(const uint16_t* h_freq, void* d_tables, void* cuda_stream);
+int32_t aceapex_rans_encode(const void* d_in, uint64_t n_rows, uint64_t row_bytes, const void* d_tables, void* d_enc, uint64_t row_capacity,
+                            uint32_t* d_row_sizes, void* d_scratch, uint64_t scratch_bytes, void* cuda_stream);
+int32_t aceapex_rans_decode(const void* d_enc, uint64_t n_rows, uint64_t row_bytes, uint64_t row_capacity, const uint32_t* d_row_sizes,
+                            const void* d_tables, void* d_out, void* d_scratch, uint64_t scratch_bytes, void* cuda_stream);
+int32_t aceapex_rans_status(const void* d_scratch, void* cuda_stream, uint32_t* status);
+
 enum {
     ACEAPEX_DF_RANS = 1,      /* final rANS state / word count mismatch         */
     ACEAPEX_DF_OFFSET = 2,    /* src >= dst or match leaves the block           */

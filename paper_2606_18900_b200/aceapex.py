@@ -70,6 +70,13 @@ def load():
             "aceapex_strerror": ([i32], ctypes.c_char_p),
             "aceapex_launch_count": ([p], u64),
             "aceapex_graph_launch_count": ([p], u64),
+            "aceapex_rans_row_capacity": ([u64], u64),
+            "aceapex_rans_table_bytes": ([], u64),
+            "aceapex_rans_scratch_bytes": ([u64], u64),
+            "aceapex_rans_tables": ([p, p, p], i32),
+            "aceapex_rans_encode": ([p, u64, u64, p, p, u64, p, p, u64, p], i32),
+            "aceapex_rans_decode": ([p, u64, u64, u64, p, p, p, p, u64, p], i32),
+            "aceapex_rans_status": ([p, p, ctypes.POINTER(u32)], i32),
             "aceapex_set_phase_timing": ([p, i32], i32),
             "aceapex_phase_times": ([p, ctypes.POINTER(ctypes.c_float)], i32),
         }
@@ -217,3 +224,45 @@ class Archive:
     def decode_all_host(self, h_archive, d_stage, h_out):
         """h_archive / h_out: pinned CPU uint8 tensors; d_stage: device uint8 tensor of raw_bytes."""
         self._chk(self.L.aceapex_decode_all_host(self.h, h_archive.data_ptr(), d_stage.data_ptr(), h_out.data_ptr()), "decode_all_host")
+
+
+class RansBatch:
+    """The entropy stage alone (include/aceapex.h, aceapex_rans_*): rows of byte symbols coded with one static
+    table.  Marshalling only: tables, encode and decode run in the CUDA library."""
+
+    def __init__(self, freq, row_bytes, device="cuda:0"):
+        import torch
+        self._torch, self.L, self.row_bytes = torch, load(), int(row_bytes)
+        self.device = torch.device(device)
+        self.stream = torch.cuda.current_stream(self.device)
+        freq = np.ascontiguousarray(freq, dtype=np.uint16)
+        self.row_cap = int(self.L.aceapex_rans_row_capacity(self.row_bytes))
+        self.tables = torch.empty(int(self.L.aceapex_rans_table_bytes()), dtype=torch.uint8, device=self.device)
+        with torch.cuda.device(self.device):
+            self.scratch = torch.empty(int(self.L.aceapex_rans_scratch_bytes(self.row_bytes)), dtype=torch.uint8, device=self.device)
+            _chk(self.L.aceapex_rans_tables(freq.ctypes.data, self.tables.data_ptr(), ctypes.c_void_p(self.stream.cuda_stream)), "rans_tables")
+
+    def new_encoded(self, n_rows):
+        t = self._torch
+        return (t.empty(n_rows * self.row_cap + 128, dtype=t.uint8, device=self.device), t.empty(n_rows, dtype=t.int32, device=self.device))
+
+    def encode(self, rows, enc=None, sizes=None):
+        """rows: CUDA uint8 tensor (n_rows, row_bytes).  Returns (encoded buffer, int32 sizes per row); asynchronous."""
+        n = rows.shape[0]
+        if enc is None:
+            enc, sizes = self.new_encoded(n)
+        _chk(self.L.aceapex_rans_encode(rows.data_ptr(), n, self.row_bytes, self.tables.data_ptr(), enc.data_ptr(), self.row_cap, sizes.data_ptr(),
+                                        self.scratch.data_ptr(), self.scratch.numel(), ctypes.c_void_p(self.stream.cuda_stream)), "rans_encode")
+        return enc, sizes
+
+    def decode(self, enc, sizes, n_rows, out=None):
+        t = self._torch
+        out = t.empty((n_rows, self.row_bytes), dtype=t.uint8, device=self.device) if out is None else out
+        _chk(self.L.aceapex_rans_decode(enc.data_ptr(), n_rows, self.row_bytes, self.row_cap, sizes.data_ptr(), self.tables.data_ptr(), out.data_ptr(),
+                                        self.scratch.data_ptr(), self.scratch.numel(), ctypes.c_void_p(self.stream.cuda_stream)), "rans_decode")
+        return out
+
+    def status(self):
+        v = ctypes.c_uint32()
+        _chk(self.L.aceapex_rans_status(self.scratch.data_ptr(), ctypes.c_void_p(self.stream.cuda_stream), ctypes.byref(v)), "rans_status")
+        return int(v.value)
