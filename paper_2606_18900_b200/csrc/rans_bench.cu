@@ -35,11 +35,20 @@ __global__ void __launch_bounds__(1024, 1) k_rans_encode(const uint8_t* __restri
         if (row >= n_rows) break;
         const uint8_t* src = in + row * row_bytes;
         uint32_t x = 1u << 16, cnt = 0;
-        // symbols in reverse order: round r holds symbols 32 r + lane
-        for (int64_t r = (int64_t)per - 1; r >= 0; r--) {
-            const uint32_t i = 32u * (uint32_t)r + lane;
-            if (i < row_bytes) {
-                const EncSym e = s_tab[__ldg(src + i)];
+        // symbols in reverse order: round r holds symbols 32 r + lane.  Eight rounds at a time: their symbol loads are issued
+        // together, ahead of the eight dependent coding steps
+        for (int64_t r0 = (int64_t)per - 1; r0 >= 0; r0 -= 8) {
+            uint32_t sym[8];
+#pragma unroll
+            for (int k = 0; k < 8; k++) {
+                const int64_t r = r0 - k;
+                const uint32_t i = 32u * (uint32_t)r + lane;
+                sym[k] = (r >= 0 && i < row_bytes) ? (uint32_t)__ldg(src + i) : 0xffffffffu;
+            }
+#pragma unroll
+            for (int k = 0; k < 8; k++) {
+                if (sym[k] == 0xffffffffu) continue;
+                const EncSym e = s_tab[sym[k]];
                 if (x >= e.x_max && e.x_max) { cnt++; my[per - cnt] = (uint16_t)x; x >>= 16; }      // x_max = 0 stands for 2^32 (freq = 2^11): never
                 uint32_t q = __umulhi(x, e.rcp), rem = x - q * e.freq;
                 if (rem >= e.freq) { q++; rem -= e.freq; }
@@ -95,10 +104,14 @@ extern "C" {
 uint64_t aceapex_rans_row_capacity(uint64_t row_bytes) { return (256 + 2 * row_bytes + 15) / 16 * 16; }
 uint64_t aceapex_rans_table_bytes(void) { return ENC_TABLE_BYTES + DEC_TABLE_BYTES + 64; }
 
-static int rans_geometry(int* sms) {
-    int dev = 0; cudaDeviceProp prop;
-    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return -1;
-    *sms = prop.multiProcessorCount;
+static int rans_geometry(int* sms) {                     // one attribute query per process (cudaGetDeviceProperties takes milliseconds)
+    static int cached = 0;
+    if (!cached) {
+        int dev = 0, n = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) return -1;
+        cached = n;
+    }
+    *sms = cached;
     return 0;
 }
 
