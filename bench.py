@@ -81,33 +81,25 @@ def oracle_sample(archive, n_bytes_total, target_s=12.0):
 
 def range_and_reads(torch, ar, x, stream):
     """The other two access modes of the metric on the same archive: range decode of the whole file as 64 MiB windows
-    through a two-slot ring (earlier window resident as a source), and read-level access by index (batch 1, batch 4096)."""
+    through a two-slot ring held by the library (aceapex_decode_stream: earlier window resident as a source), and read-level
+    access by index (batch 1, batch 4096)."""
     from paper_2606_18900_b200 import datagen
     N = x.size
     W = min(64 << 20, max(1 << 20, N // 16))
-    ring = [ar.new_output(W) for _ in range(2)]
-    nwin, ok = (N + W - 1) // W, True
-    best = None
-    for rep in range(2):
-        tot = 0.0
-        for s in range(2):
-            ar.set_resident(s, 0, 0, None)
-        for w in range(nwin):
-            lo, hi = w * W, min(N, (w + 1) * W)
-            s = w % 2
-            ar.set_resident(s, 0, 0, None)
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record(stream)
-            ar.decode_range(lo, hi, out=ring[s])
-            e1.record(stream)
+    ring = ar.new_output(2 * W)
+    st = ar.decode_stream(0, N, ring, W)                     # the library's device FNV consumer checks every block
+    ok = st["bad_blocks"] == 0 and st["bytes"] == N
+    seen = []
+
+    def consumer(w, lo, hi, ptr, cuda_stream):               # a second pass handing three windows to the host for a byte compare
+        if w in (0, st["n_windows"] // 2, st["n_windows"] - 1):
             torch.cuda.synchronize()
-            tot += e0.elapsed_time(e1)
-            if rep == 0 and w in (0, nwin // 2, nwin - 1):
-                ok = ok and bool(torch.equal(ring[s][:hi - lo].cpu(), torch.from_numpy(x[lo:hi])))
-            ar.set_resident(s, lo, hi, ring[s])
-        best = tot if best is None else min(best, tot)
-    for s in range(2):
-        ar.set_resident(s, 0, 0, None)
+            off = ptr - ring.data_ptr()
+            seen.append(bool(torch.equal(ring[off:off + hi - lo].cpu(), torch.from_numpy(x[lo:hi]))))
+        return 0
+    ar.decode_stream(0, N, ring, W, consumer=consumer)
+    ok = ok and len(seen) == 3 and all(seen)
+    best = min(ar.decode_stream(0, N, ring, W, consumer=lambda *a_: 0)["device_ms"] for _ in range(3))   # timed: a consumer that does nothing
     ar.check()
     idx = datagen.fastq_index(N)
     off = (idx & np.uint64((1 << 40) - 1)).astype(np.int64)
@@ -131,12 +123,96 @@ def range_and_reads(torch, ar, x, stream):
         ar.decode_reads(idx, bi, out=out)
         if k >= 1:
             bms.append((time.perf_counter() - t0) * 1e3)
+    # seeks (Table 3): one block and 100 blocks at random block-aligned positions, nothing resident
+    BS = ar.info()["block_size"]
+    seeks = {}
+    sbuf = ar.new_output(100 * BS)
+    for blocks in (1, 100):
+        sl = []
+        for k in range(120):
+            b = int(rng.integers(0, N // BS - blocks))
+            t0 = time.perf_counter()
+            ar.decode_range(b * BS, (b + blocks) * BS, out=sbuf)
+            torch.cuda.synchronize()
+            if k >= 20:
+                sl.append((time.perf_counter() - t0) * 1e3)
+        seeks["%d_blocks_ms_median" % blocks] = float(np.median(sl))
     ar.check()
-    return {"range_decode": {"value": N / best / 1e6, "unit": "GB/s", "window_bytes": W, "ring_bytes": 2 * W, "windows": nwin, "ms": best},
+    return {"range_decode": {"value": N / best / 1e6, "unit": "GB/s", "window_bytes": W, "ring_bytes": 2 * W, "windows": st["n_windows"], "ms": best,
+                             "min_window_gbs": st["min_window_gbs"], "max_window_gbs": st["max_window_gbs"], "peak_device_bytes": st["peak_device_bytes"],
+                             "through": "aceapex_decode_stream (ring inside the library; every block checked by its device FNV consumer in an untimed pass: %.2f ms with it)" % st["device_ms"]},
             "random_read_latency": {"batch1_ms_median": float(np.median(lat)), "batch1_ms_p99": float(np.percentile(lat, 99)),
                                     "batch4096_ms": float(np.median(bms)), "batch4096_us_per_read": float(np.median(bms)) * 1e3 / 4096,
                                     "reads_in_index": int(idx.size), "timer": "host wall clock around the synchronous C-ABI call"},
+            "seek_latency": dict(seeks, graph_launches=ar.graph_launch_count(), timer="host wall clock around aceapex_decode_range + synchronize"),
             "bit_exact": ok}
+
+
+def entropy_microbench(torch):
+    """SURVEY.md 8(f) rank 1 / PAPER.md:135: the rANS stage alone on 256 MiB of exponentially distributed bytes, 4096 rows of 64 KB
+    (the paper's DietGPU shape), through aceapex_rans_encode / aceapex_rans_decode; decode(encode(x)) == x is checked."""
+    from paper_2606_18900_b200.aceapex import RansBatch
+    rng = np.random.default_rng(6)
+    rows = np.minimum(rng.exponential(scale=12.0, size=(4096, 65536)), 255).astype(np.uint8)
+    hist = np.bincount(rows.ravel(), minlength=256).astype(np.int64)
+    freq = np.maximum((hist * 2048) // hist.sum(), (hist > 0).astype(np.int64))      # 2^11 slots, every present symbol >= 1
+    while freq.sum() != 2048:
+        freq[int(np.argmax(freq))] += 1 if freq.sum() < 2048 else -1
+    rb = RansBatch(freq.astype(np.uint16), 65536)
+    d = torch.from_numpy(rows).cuda()
+    enc, sizes = rb.new_encoded(4096)
+    out = torch.empty_like(d)
+    st = torch.cuda.current_stream()
+    res = {}
+    for name, fn in (("encode", lambda: rb.encode(d, enc, sizes)), ("decode", lambda: rb.decode(enc, sizes, 4096, out))):
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(st)
+        for _ in range(10):
+            fn()
+        e1.record(st)
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / 10
+        res[name] = {"ms": ms, "value": rows.size / ms / 1e6, "unit": "GB/s of symbols"}
+    res["bit_exact"] = bool(torch.equal(out, d)) and rb.status() == 0
+    res["ratio"] = rows.size / float(sizes.sum().item())
+    res["shape"] = "4096 rows x 64 KB, exponential bytes (scale 12), one static table, 32 interleaved states per row"
+    res["context"] = "DietGPU on one H100: encode 364.9, decode 592.5 GB/s (PAPER.md:135); not on this box"
+    return res
+
+
+def launch_overhead(torch, stream):
+    """SURVEY.md 8(c) S19 ("launch-overhead floor near 270 us"): the schedule of decode_all on an archive of one
+    8-byte block: nothing to decode, so the time of a step is what its launches cost."""
+    from paper_2606_18900_b200 import encoder
+    from paper_2606_18900_b200.aceapex import Archive
+    ar = Archive(encoder.encode(np.frombuffer(b"ACGTACGT", dtype=np.uint8), block_size=16384))
+    ar.set_stream(stream)
+    out = ar.new_output()
+    res = {}
+    for sched in (None, "fused"):
+        for _ in range(5):
+            ar.decode_all(out, schedule=sched)
+        torch.cuda.synchronize()
+        l0 = ar.launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(200):
+            ar.decode_all(out, schedule=sched)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        n = (ar.launch_count() - l0) / 200
+        t0 = time.perf_counter()
+        for _ in range(200):
+            ar.decode_all(out, schedule=sched)
+            torch.cuda.synchronize()
+        wall = (time.perf_counter() - t0) / 200 * 1e3
+        res[sched or "default"] = {"launches_per_step": n, "empty_step_ms_device": e0.elapsed_time(e1) / 200, "empty_step_ms_wall_with_sync": wall,
+                                   "per_launch_us": e0.elapsed_time(e1) / 200 / max(n, 1) * 1e3}
+    ar.close()
+    return res
 
 
 def max_over_ranks(dist, value, device):
@@ -219,6 +295,10 @@ def run_ours(args):
     barrier()
     launches = ar.launch_count() - l0
     total_ms = e0.elapsed_time(e1)
+    if args.step_only:
+        ar.check()
+        print(json.dumps({"step_only": True, "ms_per_step": total_ms / args.steps, "bit_exact": bool(torch.equal(out[:x.size].cpu(), torch.from_numpy(x)))}))
+        return
     kernel_ms = sum(p.elapsed_time(q) for p, q in per_step) / args.steps
     ar.check()
     ok = bool(torch.equal(out[:x.size].cpu(), torch.from_numpy(x)))
@@ -296,9 +376,13 @@ def run_ours(args):
     extra = range_and_reads(torch, ar, x, stream) if world == 1 else None
     if extra is not None:
         ok = ok and extra["bit_exact"]
+    micro = entropy_microbench(torch) if world == 1 and rank == 0 else None
+    if micro is not None:
+        ok = ok and micro["bit_exact"]
+    lo_info = launch_overhead(torch, stream) if world == 1 and rank == 0 else None
     if rank != 0:
         return
-    # ---- roofline of the step's kernels (k_literals 59 %, k_copy 41 %): algorithmic bytes C + M + N per step / measured time of its launches
+    # ---- roofline of the step's kernels: algorithmic bytes C + M + N per step / measured time of its launches
     peaks = {}
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
@@ -307,27 +391,35 @@ def run_ours(args):
     peak = float(peaks.get("hbm_gbs", 6650.0))
     alg_bytes = info["archive_bytes"] + info["total_match_bytes"] + info["raw_bytes"]
     achieved = alg_bytes / (kernel_ms * 1e-3) / 1e9
-    traffic = None                         # dram__bytes_read.sum + dram__bytes_write.sum of one step, from the committed ncu capture
+    # dram__bytes_read.sum + dram__bytes_write.sum of one step and what bounds each kernel, from the committed summary of one
+    # ncu --set full capture (profiles/step_capture.json, written by paper_2606_18900_b200/ncu_summary.py); it names the
+    # hash of the CUDA sources it was taken on, and is ignored when those have changed since
+    cap = {}
     try:
-        for ln_ in open(os.path.join(ROOT, "profiles", "traffic.txt")):
-            if ln_.startswith("dram_bytes_per_step"):
-                traffic = int(ln_.split()[1])
+        from paper_2606_18900_b200 import ncu_summary
+        cap = json.load(open(os.path.join(ROOT, "profiles", "step_capture.json")))
+        if cap.get("source_hash") != ncu_summary.source_hash():
+            cap = {"stale": "the CUDA sources changed after profiles/step_capture.json was taken"}
     except Exception:
         pass
+    kern = cap.get("kernels", {})
+    traffic = cap.get("dram_bytes_per_step")
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
                 "peak_source": "MEASURED_PEAKS.json hbm_gbs (measured)" if peaks else "fallback 6650 GB/s",
-                "kernel": "k_literals + k_copy (the three launches of one decode_all step)", "kernel_ms": kernel_ms,
-                "algorithmic_bytes": {"C": info["archive_bytes"], "M": info["total_match_bytes"], "N": info["raw_bytes"]}}
+                "kernel": "k_literals + k_copy (the launches of one decode_all step)", "kernel_ms": kernel_ms,
+                "algorithmic_bytes": {"C": info["archive_bytes"], "M": info["total_match_bytes"], "N": info["raw_bytes"]},
+                "capture": cap.get("stale") or cap.get("command")}
     # the dominant kernel on its own: k_literals reads the archive and writes the literal bytes; k_copy reads and writes
     # the match bytes
     lit_bytes = info["archive_bytes"] + info["total_lit_bytes"]
     cp_bytes = 2 * info["total_match_bytes"]
+    t_copy = phase[1] + phase[2]
     roofline["per_kernel"] = [
         {"kernel": "k_literals", "ms": phase[0], "share_of_step": phase[0] / max(sum(phase), 1e-9), "algorithmic_bytes": lit_bytes,
-         "achieved": lit_bytes / (phase[0] * 1e-3) / 1e9, "frac": lit_bytes / (phase[0] * 1e-3) / 1e9 / peak, "bound_observed": "instruction issue 81 % (shared-memory wavefronts 75 %) (profiles/r1f_kernels.md)"},
-        {"kernel": "k_copy (lower levels + top level)", "ms": phase[1] + phase[2], "share_of_step": (phase[1] + phase[2]) / max(sum(phase), 1e-9),
-         "algorithmic_bytes": cp_bytes, "achieved": cp_bytes / ((phase[1] + phase[2]) * 1e-3) / 1e9,
-         "frac": cp_bytes / ((phase[1] + phase[2]) * 1e-3) / 1e9 / peak, "bound_observed": "scattered 32-byte DRAM sectors (1.96 GB in 0.53 ms) + shared-memory pipe; responds to L2 residency, not to copy-loop stalls (profiles/r1f_kernels.md)"}]
+         "achieved": lit_bytes / (phase[0] * 1e-3) / 1e9, "frac": lit_bytes / (phase[0] * 1e-3) / 1e9 / peak, "bound_observed": kern.get("k_literals", {}).get("bound_observed")},
+        {"kernel": "k_copy", "ms": t_copy, "share_of_step": t_copy / max(sum(phase), 1e-9),
+         "algorithmic_bytes": cp_bytes, "achieved": cp_bytes / (t_copy * 1e-3) / 1e9,
+         "frac": cp_bytes / (t_copy * 1e-3) / 1e9 / peak, "bound_observed": kern.get("k_copy", {}).get("bound_observed")}]
     cpu, cpu_mt = None, None
     if args.cpu_baseline:
         got, dt, sample = oracle_sample(a, x.size)
@@ -349,12 +441,14 @@ def run_ours(args):
             "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8",
             "data": "synthetic",
             "config": {"workload": WORKLOAD, "size_bytes": int(x.size), "archive_bytes": int(a.size),
-                       "ratio": x.size / a.size, "n_blocks": info["n_blocks"], "max_level": info["max_level"],
+                       "ratio": x.size / a.size, "n_blocks": info["n_blocks"], "n_segments": info["n_segments"], "max_level": info["max_level"],
+                       "format": "ACX-B200 v3: q_min %d, LITQ %s, %.0f %% of the literal bytes in LITQ" % (info["q_min"], "aligned pairs" if info["q_mode"] else "bytes", 100.0 * info["total_litq_bytes"] / max(info["total_lit_bytes"], 1)),
                        "l2": "output (1 GiB) and archive are larger than the 126 MB L2; no flush needed",
                        "parallelism": "replicas only" if world > 1 else "1 GPU", "resident_warps": info["resident_warps"]},
             "bit_exact": ok and fnv_bad == 0,
             "clocks": dict(sampler.summary(), sustained_ms_per_step=sustained_ms, sustained_steps=n_sus), "e2e": e2e, "gpu_launches": int(launches),
-            "roofline": roofline, "cpu_baseline": cpu, "cpu_multithreaded": cpu_mt, "range_and_reads": extra, "flag_schedule": levels_info, "fused_schedule": fused_info}
+            "roofline": roofline, "cpu_baseline": cpu, "cpu_multithreaded": cpu_mt, "range_and_reads": extra, "flag_schedule": levels_info, "fused_schedule": fused_info,
+            "entropy_microbench": micro, "launch_overhead": lo_info}
     print(json.dumps(line))
     if not (ok and fnv_bad == 0):
         sys.exit(1)
@@ -368,6 +462,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--size", type=int, default=1 << 30, help="bytes of FASTQ (default: configs[1], 1 GiB)")
     ap.add_argument("--no-cpu-baseline", dest="cpu_baseline", action="store_false")
+    ap.add_argument("--step-only", action="store_true", help="only the timed decode_all steps (for ncu captures); prints a short line")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

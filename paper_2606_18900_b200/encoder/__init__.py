@@ -31,7 +31,7 @@ def encode(data, block_size=16384, **kw):
 
     Options (encoder.cpp acx_enc_opts): min_match, max_level (default 0), threads, src_window, chunk_log2, batch_chunks,
     chain_depth, hash_log2, with_fnv, log2_seg (segment size, default min(block, 16 KB)), q_min (literal runs of this many
-    bytes or more form the stream LITQ; default 64, 0 = one literal class), q_mode (0 bytes, 1 pairs, 2 = the smaller)."""
+    bytes or more form the stream LITQ; default 64, 0 = one literal class), q_mode (0 bytes, 1 pairs = default, 2 = the smaller)."""
     lib = _load()
     data = np.ascontiguousarray(np.frombuffer(data, dtype=np.uint8) if isinstance(data, (bytes, bytearray)) else data)
     assert data.dtype == np.uint8
