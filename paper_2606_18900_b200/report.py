@@ -4,7 +4,9 @@
   python -m paper_2606_18900_b200.report --config 1            # 1 GiB FASTQ: whole-file, range windows, reads
   python -m paper_2606_18900_b200.report --config 2            # 3.1 GB FASTA + 10^6 region reads (batch 1 / 4096)
   python -m paper_2606_18900_b200.report --config 3 --size N   # N bytes of FASTA (default 50 GiB) through an 8 GiB ring
-  python -m paper_2606_18900_b200.report --config 4            # block-size sweep on the configs[1] FASTQ
+  python -m paper_2606_18900_b200.report --config 4            # block-size sweep on the configs[1] FASTQ, launch overhead
+  python -m paper_2606_18900_b200.report --config 5            # the rANS stage alone (PAPER.md:135 shape)
+  python -m paper_2606_18900_b200.report --config 6            # encoder options (level cap, source window, LITQ mode) vs speed
 
 Everything is verified against the ORIGINAL bytes (direct compare where the data fits, per-block FNV-1a otherwise).
 Timing: CUDA events on the handle's stream around the C-ABI calls, after warm-up; GB = 10^9 bytes.
@@ -84,46 +86,37 @@ def whole_file(torch, ar, x, label, reps=5):
 
 
 def windows(torch, ar, x, label, window, ring_slots, reps=1, sample_check=None):
-    """Whole file as consecutive windows through a ring of `ring_slots` buffers that stay resident as sources."""
+    """Whole file as consecutive windows through a ring of `ring_slots` slots: aceapex_decode_stream owns the window order, the
+    slot rotation and the resident registration.  Pass 1: the library's device FNV consumer checks every block; pass 2:
+    a consumer that compares sampled windows with the original bytes; then `reps` timed passes with a consumer that does
+    nothing."""
     stream = torch.cuda.current_stream()
     ar.set_stream(stream)
     info = ar.info()
     N = info["raw_bytes"]
-    ring = [ar.new_output(window) for _ in range(ring_slots)]
-    nwin = (N + window - 1) // window
-    per_win, bad = [], 0
-    for rep in range(reps + 1):
-        for s in range(ring_slots):
-            ar.set_resident(s, 0, 0, None)
-        t_all = 0.0
-        per_win = []
-        for w in range(nwin):
-            lo, hi = w * window, min(N, (w + 1) * window)
-            s = w % ring_slots
-            ar.set_resident(s, 0, 0, None)             # about to be overwritten
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record(stream)
-            ar.decode_range(lo, hi, out=ring[s])
-            e1.record(stream)
+    ring = ar.new_output(window * ring_slots)
+    st = ar.decode_stream(0, N, ring, window)
+    bad = st["bad_blocks"] if info["has_fnv"] else 0
+    mism = []
+
+    def consumer(w, lo, hi, ptr, cuda_stream):
+        if x is not None and (sample_check is None or w in sample_check):
             torch.cuda.synchronize()
-            ms = e0.elapsed_time(e1)
-            t_all += ms
-            per_win.append((hi - lo) / ms / 1e6)
-            if rep == 0:                                # verify once (the consumer of the ring)
-                ar.check()
-                if info["has_fnv"]:
-                    bad += ar.verify_fnv(ring[s], lo, hi)
-                if x is not None and (sample_check is None or w in sample_check):
-                    if not torch.equal(ring[s][:hi - lo].cpu(), torch.from_numpy(x[lo:hi])):
-                        bad += 1
-            ar.set_resident(s, lo, hi, ring[s])
-    for s in range(ring_slots):
-        ar.set_resident(s, 0, 0, None)
-    emit(config=label, what="range_windows_through_ring", window_bytes=window, ring_bytes=window * ring_slots, windows=nwin,
-         total_ms=t_all, GBps=N / t_all / 1e6, GBps_min=min(per_win), GBps_max=max(per_win),
-         GBps_first_mid_last=[per_win[0], per_win[len(per_win) // 2], per_win[-1]], bad=bad,
-         roofline=roofline(info, t_all), peak_vram_bytes=int(torch.cuda.max_memory_allocated()))
-    return bad
+            off = ptr - ring.data_ptr()
+            if not torch.equal(ring[off:off + hi - lo].cpu(), torch.from_numpy(x[lo:hi])):
+                mism.append(w)
+        return 0
+    ar.decode_stream(0, N, ring, window, consumer=consumer)
+    best = None
+    for _ in range(max(reps, 1)):
+        t = ar.decode_stream(0, N, ring, window, consumer=lambda *a_: 0)
+        best = t if best is None or t["device_ms"] < best["device_ms"] else best
+    ar.check()
+    emit(config=label, what="range_windows_through_ring", window_bytes=window, ring_bytes=window * ring_slots, windows=best["n_windows"],
+         total_ms=best["device_ms"], GBps=N / best["device_ms"] / 1e6, GBps_min=best["min_window_gbs"], GBps_max=best["max_window_gbs"],
+         total_ms_with_fnv_consumer=st["device_ms"], bad=int(bad) + len(mism), roofline=roofline(info, best["device_ms"]),
+         peak_device_bytes=best["peak_device_bytes"], torch_peak_bytes=int(torch.cuda.max_memory_allocated()))
+    return int(bad) + len(mism)
 
 
 def isolated_windows(torch, ar, x, label, window):
@@ -279,40 +272,73 @@ def main():
         ar.close()
     elif args.config == 5:
         # the entropy stage alone on the workload shape of PAPER.md:135 (DietGPU: 256 MB of
-        # exponentially distributed bytes, 4096 x 64 KB).  Random bytes have no matches, so decode_all = rANS literal decode.
-        size = args.size or (256 << 20)
-        rng = np.random.default_rng(6)
-        x = np.minimum(rng.exponential(scale=12.0, size=size), 255).astype(np.uint8)
-        for bs in (65536, 16384):
-            a = encoder.encode(x, block_size=bs)
-            ar = Archive(a)
-            info = ar.info()
-            res = whole_file(torch, ar, x, "5/bs=%d" % bs, reps=10)
-            emit(config=5, what="rans_microbench", block_size=bs, n_blocks=info["n_blocks"], ratio=x.size / a.size,
-                 literal_fraction=info["total_lit_bytes"] / max(info["raw_bytes"], 1), GBps=res["default"]["GBps"],
-                 compressed_GBps=res["default"]["GBps"] * a.size / x.size,
-                 context="DietGPU on H100: decode 592.5 GB/s (PAPER.md:135); not on this box")
-            ar.close()
+        # exponentially distributed bytes, 4096 x 64 KB): aceapex_rans_encode / aceapex_rans_decode, one warp per row
+        sys.path.insert(0, ROOT)
+        import bench
+        emit(config=5, what="rans_microbench", **bench.entropy_microbench(torch))
     elif args.config == 4:
         size = args.size or (1 << 30)
         x = datagen.fastq(2, size, 50_000_000)
+        sys.path.insert(0, ROOT)
+        import bench
+        emit(config=4, what="launch_overhead", note="SURVEY.md 8(c) S19 (c): the schedule of decode_all on an archive of one 8-byte block",
+             **bench.launch_overhead(torch, torch.cuda.current_stream()))
         for bs in (4096, 8192, 16384, 65536, 262144, 1 << 20):
+            for max_level in ((0, 3) if bs == 16384 else (0,)):
+                t = time.time()
+                a = encoder.encode(x, block_size=bs, max_level=max_level)
+                enc_s = time.time() - t
+                ar = Archive(a)
+                info = ar.info()
+                res = whole_file(torch, ar, x, "4/bs=%d/max_level=%d" % (bs, max_level), reps=3)
+                n_blocks, bt_off = int(a[24:32].view(np.uint64)[0]), int(a[104:112].view(np.uint64)[0])   # FORMAT.md §1.1
+                lv = np.frombuffer(a[bt_off:bt_off + 8 * n_blocks].tobytes(), dtype=np.uint16).reshape(-1, 4)[:, 2]   # §1.4 level
+                # S19 (a), (b): launches per decode; time of a call not covered by its kernels, per launch (phase timers = CUDA events
+                # around each launch; the rest of the call is launch gaps)
+                ar.set_phase_timing(True)
+                ms_call = timed(torch, torch.cuda.current_stream(), lambda: ar.decode_all(res_out(ar)), 3)
+                ph = ar.phase_times()
+                ar.set_phase_timing(False)
+                emit(config=4, what="block_size_point", block_size=bs, encoder_max_level=max_level, ratio=x.size / a.size, encode_seconds=enc_s,
+                     n_segments=info["n_segments"], GBps=res["default"]["GBps"], ms=res["default"]["ms"], mean_level=float(lv.mean()), max_level=int(lv.max()),
+                     wavefront_depth=int(lv.max()) + 1, launches_default=res["default"]["launches"], ms_flags=res["flags"]["ms"], ms_fused=res["fused"]["ms"],
+                     call_ms=ms_call, kernels_ms=float(sum(ph)), gap_per_launch_us=(ms_call - float(sum(ph))) * 1e3 / max(res["default"]["launches"], 1))
+                if bs == 16384 and max_level == 0:
+                    seeks(torch, ar, x, "4/bs=16384")
+                ar.close()
+                del ar
+                torch.cuda.empty_cache()
+    elif args.config == 6:
+        # encoder options against range-decode speed (measure, do not dismiss): level cap, source window, LITQ mode
+        size = args.size or (1 << 30)
+        x = datagen.fastq(2, size, 50_000_000)
+        for kw in (dict(), dict(max_level=3), dict(q_mode=0), dict(q_min=0), dict(src_window=256 << 20), dict(src_window=64 << 20), dict(log2_seg=12)):
             t = time.time()
-            a = encoder.encode(x, block_size=bs)
-            enc_s = time.time() - t
+            a = encoder.encode(x, block_size=16384, **kw)
             ar = Archive(a)
-            res = whole_file(torch, ar, x, "4/bs=%d" % bs, reps=3)
-            n_blocks, dir_off = int(a[24:32].view(np.uint64)[0]), int(a[72:80].view(np.uint64)[0])   # FORMAT.md §1.1
-            lv = np.frombuffer(a[dir_off:dir_off + 32 * n_blocks].tobytes(), dtype=np.uint16).reshape(-1, 16)[:, 14]   # §1.3 level
-            # per-launch overhead (S19): level schedule time minus the two-launch time, per extra launch
-            extra = res["default"]["launches"] - res["flags"]["launches"]
-            emit(config=4, what="block_size_point", block_size=bs, ratio=x.size / a.size, encode_seconds=enc_s,
-                 GBps=res["default"]["GBps"], ms=res["default"]["ms"], mean_level=float(lv.mean()), max_level=int(lv.max()),
-                 launches_default=res["default"]["launches"], launches_flags=res["flags"]["launches"],
-                 ms_flags=res["flags"]["ms"], per_launch_overhead_ms=(res["default"]["ms"] - res["flags"]["ms"]) / max(extra, 1))
+            res = whole_file(torch, ar, x, "6/%s" % kw, reps=3)
+            win = min(64 << 20, max(1 << 20, size // 16))
+            ring = ar.new_output(2 * win)
+            st = min((ar.decode_stream(0, size, ring, win, consumer=lambda *a_: 0) for _ in range(2)), key=lambda q: q["device_ms"])
+            bad = ar.decode_stream(0, size, ring, win)["bad_blocks"]
+            emit(config=6, what="encoder_option", options=kw, ratio=x.size / a.size, encode_seconds=time.time() - t, decode_all_GBps=res["default"]["GBps"],
+                 ring_GBps=size / st["device_ms"] / 1e6, ring_min_window_GBps=st["min_window_gbs"], bad_blocks=int(bad))
+            seeks(torch, ar, x, "6/%s" % kw, n=100)
             ar.close()
-            del ar
+            del ar, ring
             torch.cuda.empty_cache()
+
+
+_OUT = {}
+
+
+def res_out(ar):
+    """one output buffer per archive handle (timing helper)"""
+    k = id(ar)
+    if k not in _OUT:
+        _OUT.clear()
+        _OUT[k] = ar.new_output()
+    return _OUT[k]
 
 
 if __name__ == "__main__":
