@@ -275,7 +275,7 @@ int32_t launch(aceapex_archive* ar, Params& P, Kind kind, uint64_t n_work) {
     take_ticket(ar, P);
     int T; uint32_t g;
     spread(ar, n_work, ar->threads, g, T);
-    const size_t sm_e = entropy_smem(ar->n_coded_tables, ar->q_mode, ar->runs_bytes + ar->lita_bytes, T), sm_c = (size_t)(T / 32) * COPY_WARP_BYTES + 64;
+    const size_t sm_e = entropy_smem(ar->n_coded_tables, ar->q_mode, ar->runs_bytes + ALIST_BYTES + ar->lita_bytes, T), sm_c = (size_t)(T / 32) * COPY_WARP_BYTES + 64;
     const void* f = nullptr; size_t sm = sm_c; dim3 gd(g), bd(T);
     switch (kind) {
         case K_LIT:
@@ -471,17 +471,17 @@ int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* 
     // and, with what the tables leave free, a staging area for LITA (up to 4 KB; larger segments stage in global memory)
     ar->threads = 1024;
     ar->runs_bytes = runs_bytes_for(ar->q_min);
-    const uint32_t min_area = 4 * (MAX_SEG_CMDS + 2);
+    const uint32_t min_area = std::max<uint32_t>(4 * (MAX_SEG_CMDS + 2), ar->runs_bytes + ALIST_BYTES);
     auto smem_max = [&](int T, uint32_t area) { return std::max(entropy_smem(ar->n_coded_tables, ar->q_mode, area, T), (size_t)(T / 32) * COPY_WARP_BYTES + 64); };
     while (ar->threads > 128 && smem_max(ar->threads, min_area) > (size_t)prop.sharedMemPerBlockOptin) ar->threads -= 64;
     {
         const size_t fixed = entropy_smem(ar->n_coded_tables, ar->q_mode, 0, ar->threads);
         const size_t room = (size_t)prop.sharedMemPerBlockOptin > fixed ? ((size_t)prop.sharedMemPerBlockOptin - fixed) / (ar->threads / 32) : 0;
-        uint32_t area = (uint32_t)std::min<size_t>(room & ~(size_t)15, ar->runs_bytes + 4096);
+        uint32_t area = (uint32_t)std::min<size_t>(room & ~(size_t)15, ar->runs_bytes + ALIST_BYTES + 4096);
         area = std::max(area, min_area);
-        ar->lita_bytes = area - ar->runs_bytes;
+        ar->lita_bytes = area - ar->runs_bytes - ALIST_BYTES;
     }
-    ar->smem_entropy = entropy_smem(ar->n_coded_tables, ar->q_mode, ar->runs_bytes + ar->lita_bytes, ar->threads);
+    ar->smem_entropy = entropy_smem(ar->n_coded_tables, ar->q_mode, ar->runs_bytes + ALIST_BYTES + ar->lita_bytes, ar->threads);
     ar->smem_copy = (size_t)(ar->threads / 32) * COPY_WARP_BYTES + 64;
     ar->smem_fused = std::max(ar->smem_entropy, ar->smem_copy);
     {

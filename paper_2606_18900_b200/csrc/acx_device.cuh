@@ -113,6 +113,7 @@ __device__ __forceinline__ uint4 lds128(uint32_t a) {
     uint4 v; asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a)); return v;
 }
 __device__ __forceinline__ void sts32(uint32_t a, uint32_t v) { asm volatile("st.shared.u32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
+__device__ __forceinline__ void sts64(uint32_t a, uint32_t x, uint32_t y) { asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(a), "r"(x), "r"(y) : "memory"); }
 __device__ __forceinline__ void sts16(uint32_t a, uint32_t v) { asm volatile("st.shared.u16 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
 __device__ __forceinline__ void sts128(uint32_t a, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
     asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
@@ -162,7 +163,7 @@ struct Rans {
         cp_async_wait_group<2>();
     }
     __device__ __forceinline__ void renorm() {
-        if (x < 65536u) { x = (x << 16) | w; rp += 2; w = lds16(ring | (rp & 63)); }
+        if (x < 65536u) { x = (x << 16) + w; rp += 2; w = lds16(ring | (rp & 63)); }      // + : one IMAD
     }
     // one symbol on this lane.  lut = shared address of a byte table.  Returns the table entry (sym | bias << 8 |
     // freq << 20).  The ring is read only by the lanes that renormalise (a predicated load).
@@ -216,7 +217,7 @@ __device__ __forceinline__ uint32_t rans_region(Rans& r, uint32_t lut, uint32_t 
         r.prepare8();
         const uint32_t e = PAIR ? r.step_pair(lut, active) : r.step(lut, active);
         if (active && store) put(p, e);
-        if (!PAIR) esc += __popc(__ballot_sync(0xffffffffu, active && (e & 0xff) == 255));
+        if (!PAIR && active && (~e & 0xffu) == 0) esc++;
         base += 32; p += 32 * S;
     };
     if (base != i0) ragged();
@@ -228,7 +229,7 @@ __device__ __forceinline__ uint32_t rans_region(Rans& r, uint32_t lut, uint32_t 
         for (int k = 0; k < 8; k++) {
             const uint32_t e = PAIR ? r.step_pair_full(lut) : r.step_full(lut);
             if (store) put(p + 32 * S * k, e);
-            if (!PAIR) esc += __popc(__ballot_sync(0xffffffffu, (e & 0xff) == 255));
+            if (!PAIR && (~e & 0xffu) == 0) esc++;
         }
         p += 256 * S;
     }
@@ -238,11 +239,11 @@ __device__ __forceinline__ uint32_t rans_region(Rans& r, uint32_t lut, uint32_t 
         for (; full; full--, p += 32 * S) {
             const uint32_t e = PAIR ? r.step_pair_full(lut) : r.step_full(lut);
             if (store) put(p, e);
-            if (!PAIR) esc += __popc(__ballot_sync(0xffffffffu, (e & 0xff) == 255));
+            if (!PAIR && (~e & 0xffu) == 0) esc++;
         }
     }
     if (base < i1) ragged();
-    return esc;
+    return PAIR ? 0u : __reduce_add_sync(0xffffffffu, esc);    // per-lane counts, one REDUX per region
 }
 
 // ------------------------------------------------------------------------------------------------ copies --------

@@ -221,6 +221,7 @@ __host__ __device__ inline uint32_t runs_bytes_for(uint32_t q_min) {   // run ta
 
 __device__ __forceinline__ bool build_runs(const Params& P, const SegCtx& c, uint32_t runs /* shared address */, uint8_t* out_seg, uint32_t* q_edge_out) {
     ScanState st; scan_init(st, c);
+    const uint32_t alist = runs + P.runs_bytes;                // 32 x 8 bytes behind the run table
     uint32_t n_q = 0, q_bytes = 0, q_edge = 0;
     uint2* const pairs = P.pairs ? P.pairs + __ldg(P.match_prefix + c.s) : nullptr;
     const uint32_t lane = lane_id();
@@ -257,15 +258,38 @@ __device__ __forceinline__ bool build_runs(const Params& P, const SegCtx& c, uin
                     if (n > 7) da[7] = (uint8_t)(v1 >> 24);
                 }
             }
-            uint32_t a_long = __ballot_sync(0xffffffffu, a_run && L.lit_len > 8);
+            // runs of 9..63 bytes: compacted into a list in shared memory, then four runs at a time, eight lanes per run
+            // (lane sub copies bytes sub, sub + 8, ..): one pass of predicated byte copies serves four runs
+            const bool a_mid = a_run && L.lit_len > 8 && L.lit_len < 64;
+            const uint32_t m_mid = __ballot_sync(0xffffffffu, a_mid);
+            if (m_mid) {
+                if (a_mid) sts64(alist + 8 * __popc(m_mid & lanemask_lt()), L.lit_pos | L.lit_len << 16, L.out_rel);
+                __syncwarp();
+                const uint32_t n_mid = __popc(m_mid), sub = lane & 7u;
+                for (uint32_t k = lane >> 3; k < ((n_mid + 3u) & ~3u); k += 4) {
+                    uint2 e = make_uint2(0u, 0u);
+                    if (k < n_mid) e = lds64(alist + 8 * k);
+                    const uint32_t m = e.x >> 16;
+                    const uint8_t* sp = c.lit_a + (e.x & 0xffffu) + sub; uint8_t* dp = out_seg + e.y + sub;
+                    uint32_t v[4];
+#pragma unroll
+                    for (int j = 0; j < 4; j++) if (sub + 8 * j < m) v[j] = sp[8 * j];
+#pragma unroll
+                    for (int j = 0; j < 4; j++) if (sub + 8 * j < m) dp[8 * j] = (uint8_t)v[j];
+                    if (__any_sync(0xffffffffu, m > 32)) {
+#pragma unroll
+                        for (int j = 4; j < 8; j++) if (sub + 8 * j < m) v[j - 4] = sp[8 * j];
+#pragma unroll
+                        for (int j = 4; j < 8; j++) if (sub + 8 * j < m) dp[8 * j] = (uint8_t)v[j - 4];
+                    }
+                }
+                __syncwarp();                                   // the list is rewritten by the next group
+            }
+            uint32_t a_long = __ballot_sync(0xffffffffu, a_run && L.lit_len >= 64);      // only archives without a LITQ class have them
             while (a_long) {
                 const int l = __ffs(a_long) - 1; a_long &= a_long - 1;
                 const uint32_t m = __shfl_sync(0xffffffffu, L.lit_len, l), lp = __shfl_sync(0xffffffffu, L.lit_pos, l), orl = __shfl_sync(0xffffffffu, L.out_rel, l);
-                if (m >= 64) warp_copy<false>(out_seg + orl, c.lit_a + lp, m);       // only archives without a LITQ class have them
-                else {
-                    if (lane < m) out_seg[orl + lane] = c.lit_a[lp + lane];
-                    if (lane + 32 < m) out_seg[orl + lane + 32] = c.lit_a[lp + lane + 32];
-                }
+                warp_copy<false>(out_seg + orl, c.lit_a + lp, m);
             }
         }
         if (L.is_q) {
@@ -339,22 +363,29 @@ __device__ __forceinline__ void decode_q(Rans& r, uint32_t lut, uint32_t i0, uin
     while (base < i1) {
         r.prepare8();
         if (base > i0 && base + 256 < i1) {               // eight full rounds, none of them the first or the last of the stream
+            // pd = address of this lane's symbol of round 0 under the current run's delta; lim = symbols of the group's
+            // first position up to the run's last one: a round q lies strictly inside the run iff 32 q + 31 < lim
+            uint8_t* pd = pj + rc.delta;
+            uint32_t lim = rc.last - (base - i0);
 #pragma unroll 1
             for (int h = 0; h < 2; h++) {                 // two groups of four (code size)
-                uint8_t* pd = pj + rc.delta;
 #pragma unroll
                 for (int q = 0; q < 4; q++) {
                     const uint32_t e = PAIR ? r.step_pair_full(lut) : r.step_full(lut);
-                    const uint32_t j_hi = base + 32 * q + 31 - i0;
-                    if (j_hi < rc.last) put(pd + 32 * S * q, e);       // the whole round lies strictly inside run k: pointer bump
+                    if (32u * q + 31u < lim) put(pd + 32 * S * q, e);        // pointer bump
                     else if (SIMPLE) {                                 // run k ends in this round, run k + 1 goes on beyond it
-                        const uint32_t prev = rc.last, old_delta = rc.delta;
+                        const uint32_t old_delta = rc.delta;
                         rc.k += 4; rc.load(lds32(rc.k));
-                        put(pj + 32 * S * q + (j_hi - 31 + lane > prev ? rc.delta : old_delta), e);
-                        pd = pj + rc.delta;
-                    } else { put(pj + 32 * S * q + rc.walk(j_hi - 31 + lane, j_hi), e); pd = pj + rc.delta; }
+                        const int32_t dd = (int32_t)(rc.delta - old_delta);
+                        put(pd + 32 * S * q + (32u * q + lane > lim ? dd : 0), e);
+                        pd += dd; lim = rc.last - (base - i0);
+                    } else {
+                        const uint32_t old_delta = rc.delta, j_hi = base + 32 * q + 31 - i0;
+                        put(pj + 32 * S * q + rc.walk(j_hi - 31 + lane, j_hi), e);
+                        pd += (int32_t)(rc.delta - old_delta); lim = rc.last - (base - i0);
+                    }
                 }
-                base += 128; pj += 128 * S;
+                base += 128; pj += 128 * S; pd += 128 * S; lim -= 128;
             }
         } else {
 #pragma unroll 1
@@ -718,9 +749,10 @@ __device__ __forceinline__ void copy_body(const Params& P, const Work W, uint32_
 }
 
 // shared memory of the entropy kernels: [byte tables: n_coded_tables x 8 KB][pair table: 32 KB when q_mode = 1]
-// [rings: warps x 2 KB][per warp: run table | LITA staging][stack tops: warps x 4]   (absolute shared addresses).
+// [rings: warps x 2 KB][per warp: run table | list of 32 runs | LITA staging][stack tops: warps x 4]   (absolute shared addresses).
 // The span-service kernels use the per-warp area as one command table (2 KB at least).
 struct CtaSmem { uint32_t luts, lutq, ring, runs, top; uint8_t* lita; uint8_t* area; };   // area: generic pointer of `runs`
+constexpr uint32_t ALIST_BYTES = 256;       // k_literals: list of the mid-length LITA runs of a command group, behind the run table
 
 __host__ __device__ inline size_t entropy_smem(uint32_t n_coded_tables, uint32_t q_mode, uint32_t warp_area, int threads) {
     return (size_t)n_coded_tables * LUT_SIZE * 4 + (q_mode ? (size_t)QLUT_SIZE * 8 : 0) + (size_t)(threads / 32) * (RING_BYTES + warp_area + 4) + 128;
@@ -740,7 +772,7 @@ __device__ __forceinline__ CtaSmem setup_cta(const Params& P, uint8_t* smem_raw)
         }
     }
     __syncthreads();
-    const uint32_t warp = threadIdx.x >> 5, warps = blockDim.x >> 5, area = P.runs_bytes + P.lita_bytes;
+    const uint32_t warp = threadIdx.x >> 5, warps = blockDim.x >> 5, area = P.runs_bytes + ALIST_BYTES + P.lita_bytes;
     CtaSmem m;
     m.luts = smem0;
     m.lutq = smem0 + n_lut_words * 4;
@@ -749,7 +781,7 @@ __device__ __forceinline__ CtaSmem setup_cta(const Params& P, uint8_t* smem_raw)
     m.ring = base + warp * RING_BYTES; base += warps * RING_BYTES;
     m.runs = base + warp * area;
     m.area = smem_raw + (m.runs - raw0);
-    m.lita = m.area + P.runs_bytes;
+    m.lita = m.area + P.runs_bytes + ALIST_BYTES;
     base += warps * area;
     m.top = base + 4 * warp;
     return m;
@@ -814,7 +846,7 @@ __device__ __forceinline__ bool parse_for_spans(const Params& P, uint32_t s_luts
         else if (k < n_tok) { lut = P.coded_lut[k - 2]; cnt = c.d.n_match; dst = c.off_planes + (k - 2) * TOK_STRIDE; }
         else if (k == n_tok) {
             __syncwarp();                                       // the tokens are complete: the scan reads them
-            ok = build_cmd_table(P, c, tab, area, P.runs_bytes + P.lita_bytes);
+            ok = build_cmd_table(P, c, tab, area, P.runs_bytes + ALIST_BYTES + P.lita_bytes);
             if (!ok) break;
             if (pend < c.send) { literals_before(P, c, tab, (uint32_t)(pend - c.sstart), &na, &nq); if (nq) na = c.d.n_lit_a; }
             lut = P.lut_lita; cnt = na; dst = c.lit_a;

@@ -29,7 +29,7 @@ def _load():
 def encode(data, block_size=16384, **kw):
     """data: uint8 numpy array (or bytes).  Returns the archive as a uint8 numpy array.
 
-    Options (encoder.cpp acx_enc_opts): min_match, max_level (default 0), threads, src_window, chunk_log2, batch_chunks,
+    Options (encoder.cpp acx_enc_opts): min_match, max_level (default 2), threads, src_window, chunk_log2, batch_chunks,
     chain_depth, hash_log2, with_fnv, log2_seg (segment size, default min(block, 16 KB)), q_min (literal runs of this many
     bytes or more form the stream LITQ; default 64, 0 = one literal class), q_mode (0 bytes, 1 pairs = default, 2 = the smaller)."""
     lib = _load()

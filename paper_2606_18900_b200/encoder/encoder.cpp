@@ -330,7 +330,7 @@ struct acx_enc_opts {
 // log2_seg 0 = min(log2_bs, 14).  q_min 0 = one literal class.
 void acx_enc_default_opts(acx_enc_opts* o) {
     memset(o, 0, sizeof *o);
-    o->log2_bs = 14; o->min_match = 4; o->max_level = 0; o->threads = 0; o->src_window = 0;
+    o->log2_bs = 14; o->min_match = 4; o->max_level = 2; o->threads = 0; o->src_window = 0;
     o->chunk_log2 = 22; o->batch_chunks = 16; o->chain_depth = 2; o->hash_log2 = 0; o->with_fnv = 1;
     o->log2_seg = 0; o->q_min = 64; o->q_mode = 1;
 }
