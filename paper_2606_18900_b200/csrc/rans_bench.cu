@@ -23,11 +23,15 @@ __global__ void __launch_bounds__(1024, 1) k_rans_encode(const uint8_t* __restri
                                                           uint8_t* __restrict__ out, uint64_t row_cap, uint32_t* __restrict__ row_sizes, uint16_t* __restrict__ stage,
                                                           unsigned long long* ticket) {
     __shared__ EncSym s_tab[256];
+    __shared__ __align__(16) uint16_t s_grp[32][32][8];          // per warp and lane: the eight words being collected
     for (uint32_t i = threadIdx.x; i < 256; i += blockDim.x) s_tab[i] = table[i];
     __syncthreads();
     const uint32_t lane = threadIdx.x & 31;
-    const uint32_t per = (row_bytes + 31) / 32;                // a state emits at most one word per symbol
-    uint16_t* const my = stage + ((uint64_t)(blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5)) * 32 + lane) * per;   // this lane's words, written from the end
+    const uint32_t per = ((row_bytes + 31) / 32 + 7) & ~7u;   // a state emits at most one word per symbol; whole groups of eight
+    // this lane's words, written from the end in groups of eight (one 16-byte store per group instead of eight 2-byte stores
+    // to eight different sectors per warp: the scattered stores, not the arithmetic, set the pace of this kernel)
+    uint16_t* const my = stage + ((uint64_t)(blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5)) * 32 + lane) * per;
+    const uint32_t grp = (uint32_t)__cvta_generic_to_shared(&s_grp[threadIdx.x >> 5][lane][0]);
     for (;;) {
         unsigned long long row = 0;
         if (lane == 0) row = atomicAdd(ticket, 1ull);
@@ -37,25 +41,37 @@ __global__ void __launch_bounds__(1024, 1) k_rans_encode(const uint8_t* __restri
         uint32_t x = 1u << 16, cnt = 0;
         // symbols in reverse order: round r holds symbols 32 r + lane.  Eight rounds at a time: their symbol loads are issued
         // together, ahead of the eight dependent coding steps
-        for (int64_t r0 = (int64_t)per - 1; r0 >= 0; r0 -= 8) {
-            uint32_t sym[8];
+        auto load8 = [&](int64_t r0, uint32_t (&sym)[8]) {
 #pragma unroll
             for (int k = 0; k < 8; k++) {
                 const int64_t r = r0 - k;
                 const uint32_t i = 32u * (uint32_t)r + lane;
                 sym[k] = (r >= 0 && i < row_bytes) ? (uint32_t)__ldg(src + i) : 0xffffffffu;
             }
+        };
+        uint32_t nxt[8];
+        load8((int64_t)((row_bytes + 31) / 32) - 1, nxt);
+        for (int64_t r0 = (int64_t)((row_bytes + 31) / 32) - 1; r0 >= 0; r0 -= 8) {
+            uint32_t sym[8];
+#pragma unroll
+            for (int k = 0; k < 8; k++) sym[k] = nxt[k];
+            load8(r0 - 8, nxt);                                // the next eight rounds' symbols travel while these are coded
 #pragma unroll
             for (int k = 0; k < 8; k++) {
                 if (sym[k] == 0xffffffffu) continue;
                 const EncSym e = s_tab[sym[k]];
-                if (x >= e.x_max && e.x_max) { cnt++; my[per - cnt] = (uint16_t)x; x >>= 16; }      // x_max = 0 stands for 2^32 (freq = 2^11): never
+                if (x >= e.x_max && e.x_max) {                 // x_max = 0 stands for 2^32 (freq = 2^11): never
+                    sts16(grp + 2u * (7u - (cnt & 7u)), x);    // word c of the lane lands at my[per - 1 - c]
+                    x >>= 16; cnt++;
+                    if ((cnt & 7u) == 0) *reinterpret_cast<uint4*>(my + (per - cnt)) = lds128(grp);
+                }
                 uint32_t q = __umulhi(x, e.rcp), rem = x - q * e.freq;
                 if (rem >= e.freq) { q++; rem -= e.freq; }
                 if (e.freq == 1) { q = x; rem = 0; }
                 x = (q << PROB_BITS) + rem + e.cum;
             }
         }
+        if (cnt & 7u) *reinterpret_cast<uint4*>(my + (per - ((cnt + 7u) & ~7u))) = lds128(grp);     // the open group: its low slots are not read
         // head: (state, word_off); then every state's words in the order the decoder consumes them (the reverse of emission)
         uint32_t off = cnt;
 #pragma unroll
@@ -70,7 +86,15 @@ __global__ void __launch_bounds__(1024, 1) k_rans_encode(const uint8_t* __restri
         for (int k = 0; k < 32; k++) {                       // the whole warp copies state k's stream: coalesced on both sides
             const uint32_t n = __shfl_sync(0xffffffffu, cnt, k), o = __shfl_sync(0xffffffffu, off, k);
             const uint16_t* from = reinterpret_cast<const uint16_t*>(__shfl_sync(0xffffffffu, reinterpret_cast<unsigned long long>(my), k)) + (per - n);
-            for (uint32_t j = lane; j < n; j += 32) words[o + j] = from[j];
+            uint32_t j = lane;
+            for (; j + 224 < n; j += 256) {                    // eight loads in flight per lane
+                uint16_t v[8];
+#pragma unroll
+                for (int q = 0; q < 8; q++) v[q] = from[j + 32 * q];
+#pragma unroll
+                for (int q = 0; q < 8; q++) words[o + j + 32 * q] = v[q];
+            }
+            for (; j < n; j += 32) words[o + j] = from[j];
         }
         __syncwarp();
     }
@@ -118,7 +142,7 @@ static int rans_geometry(int* sms) {                     // one attribute query 
 uint64_t aceapex_rans_scratch_bytes(uint64_t row_bytes) {
     int sms = 148;
     rans_geometry(&sms);
-    return (uint64_t)sms * 32 * 32 * ((row_bytes + 31) / 32) * 2 + 64;      // per resident warp: 32 states x one word per symbol at most
+    return (uint64_t)sms * 32 * 32 * (((row_bytes + 31) / 32 + 7) & ~7ull) * 2 + 64;      // per resident warp: 32 states x one word per symbol at most, in groups of eight
 }
 
 int32_t aceapex_rans_tables(const uint16_t* h_freq, void* d_tables, void* stream) {
