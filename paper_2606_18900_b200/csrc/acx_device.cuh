@@ -33,7 +33,7 @@ struct Demand { uint64_t pos; uint64_t dst; uint64_t len; };
 // are served they are bucketed by SOURCE segment (plan + scatter), so one parse of a segment serves its whole bucket and a
 // hot segment (thousands of records) is cut into work items of GL_ITEM records that different warps take.
 struct GDemand { uint64_t pos; uint64_t dst; uint32_t len; uint32_t seg; };
-constexpr uint32_t GL_ITEM = 512;                 // records per work item: one parse of the source segment, then 32 records at a time
+constexpr uint32_t GL_ITEM = 128;                 // records per work item: one parse of the source segment, then 32 records at a time
 struct GList {
     GDemand* rec;            // cap records, in order of arrival
     GDemand* sorted;         // the same records bucketed by segment (written by the scatter phase)

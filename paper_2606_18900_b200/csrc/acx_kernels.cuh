@@ -449,6 +449,8 @@ enum : uint32_t { SKIP_KNOWN = 1, SKIP_UNKNOWN = 2 };
 
 __device__ __forceinline__ uint32_t lds_top(const Stack& st) { return lds32(st.top); }
 
+constexpr uint32_t GL_SPAN_MAX = 96;     // a record of the global lists covers at most this many bytes (= ITEM_LANE_MAX: one lane serves
+                                         // it; a work item of GL_ITEM records is bounded in bytes, not only in records)
 // append "original bytes [pos, pos + len) -> out2[dst ..)" (inside segment seg)
 __device__ __forceinline__ void gl_append(const Params& P, const GList& gl, uint64_t pos, uint32_t len, uint64_t dst, uint32_t seg) {
     const uint32_t idx = atomicAdd(gl.count, 1u);
@@ -468,7 +470,8 @@ __device__ __forceinline__ void push_span(const Params& P, const Stack& st, uint
         uint32_t seg = __ldg(P.first_seg + pb);
         uint64_t send = block_end(P, pb);
         if (__ldg(P.first_seg + pb + 1) - seg > 1) { seg = seg_of(P, pos); send = seg_end(P, seg, pb); }   // several segments in the block
-        const uint64_t n = min((unsigned long long)len, (unsigned long long)(send - pos));
+        uint64_t n = min((unsigned long long)len, (unsigned long long)(send - pos));
+        if (st.gl) n = min((unsigned long long)n, (unsigned long long)GL_SPAN_MAX);   // work items are sized by record count: bound a record's bytes
         if (st.gl) gl_append(P, *st.gl, pos, (uint32_t)n, dst, seg);
         else {
             uint32_t idx;
@@ -484,9 +487,12 @@ __device__ __forceinline__ void push_span(const Params& P, const Stack& st, uint
 // bound by instruction fetch, 5.3 stalled warps per issue, when everything was inlined)
 __device__ __noinline__ void copy_any(uint8_t* dst, const uint8_t* src, uint32_t len) {
 #pragma unroll 1
-    for (uint32_t i = 0; i < len; i += 8) {                 // sources may have been written by other SMs: ld.cg
-        const uint32_t n = min(len - i, 8u);
-        st_small(dst + i, ld64u<true>(src + i, n), n);
+    for (uint32_t i = 0; i < len; i += 32) {                // sources may have been written by other SMs: ld.cg; four loads in flight
+        uint64_t v[4];
+#pragma unroll
+        for (uint32_t q = 0; q < 4; q++) if (i + 8 * q < len) v[q] = ld64u<true>(src + i + 8 * q, min(len - i - 8 * q, 8u));
+#pragma unroll
+        for (uint32_t q = 0; q < 4; q++) if (i + 8 * q < len) st_small(dst + i + 8 * q, v[q], min(len - i - 8 * q, 8u));
     }
 }
 
@@ -894,7 +900,20 @@ __device__ __forceinline__ void emit_cmd_piece(const Params& P, const SegCtx& c,
         else {                                                // byte i of the match = seed[i mod period]
             uint8_t* d = P.out2 + dst + (a - pos);
             uint32_t r = (uint32_t)((a - md) % period);
-            for (uint32_t k = 0; k < (uint32_t)(b - a); k++) { d[k] = (uint8_t)lit_byte(P, c, is_q, lit_pos, o0, src + r); if (++r == period) r = 0; }
+            const uint32_t n = (uint32_t)(b - a);
+            // the seed [src, md) lies in this command's literal run, contiguous in the warp's scratch: copy it piecewise,
+            // wrapping at the period (a FASTA N-run with its newlines has period 61; a byte loop here made one hot source
+            // segment cost milliseconds)
+            const uint8_t* seed = !is_q ? c.lit_a + lit_pos + (src - o0) : !P.q_mode ? c.lit_q + lit_pos + (src - o0) : c.lit_q + 2ull * lit_pos + (src - (o0 & ~1ull));
+            if (period < 8) {                                  // short periods: one byte at a time is as good as it gets per piece
+                for (uint32_t k = 0; k < n; k++) { d[k] = seed[r]; if (++r == (uint32_t)period) r = 0; }
+            } else {
+                for (uint32_t k = 0; k < n;) {
+                    const uint32_t m = min(n - k, (uint32_t)period - r);
+                    copy_any(d + k, seed + r, m);
+                    k += m; r = 0;
+                }
+            }
         }
     }
 }

@@ -47,7 +47,8 @@ struct Seg {
     uint64_t block, out_start;
     std::vector<Cmd> cmds;
     std::vector<uint8_t> lit_a, lit_q;
-    std::vector<uint16_t> q_sym;                                  // LITQ symbols: bytes, or pairs v0 | v1 << 8
+    std::vector<uint16_t> q_sym;                                  // pair mode: LITQ symbols v0 | v1 << 8 (lit_q is released once they exist)
+    uint32_t n_lit_q = 0, n_sym_q = 0;                            // LITQ bytes / LITQ symbols of the segment
     std::vector<uint32_t> q_edge;                                 // pair mode: indices into q_sym of the pairs with a filler half
 };
 
@@ -511,9 +512,11 @@ int acx_encode(const uint8_t* in, uint64_t N, const acx_enc_opts* uo, uint8_t** 
                 }
                 pos += (uint64_t)c.lit_len + c.match_len;
             }
+            s.n_lit_q = (uint32_t)s.lit_q.size(); s.n_sym_q = (uint32_t)s.q_sym.size();
+            std::vector<uint8_t>().swap(s.lit_q);           // 50 GiB inputs: the literals are held once, not twice
         });
     }
-    if (q_mode == 0 && q_min) for (Seg& s : segs) s.q_sym.assign(s.lit_q.begin(), s.lit_q.end());
+    if (q_mode == 0) for (Seg& s : segs) s.n_lit_q = s.n_sym_q = (uint32_t)s.lit_q.size();
 
     // ---- histograms and byte tables
     const uint32_t n_tables = 4 + W;
@@ -530,7 +533,7 @@ int acx_encode(const uint8_t* in, uint64_t N, const acx_enc_opts* uo, uint8_t** 
         }
         for (uint8_t v : s.lit_a) H[2 + W][v]++;
         if (q_mode == 0) for (uint8_t v : s.lit_q) H[3 + W][v]++;
-        tot_lit += s.lit_a.size() + s.lit_q.size(); tot_c += s.cmds.size();
+        tot_lit += s.lit_a.size() + s.n_lit_q; tot_c += s.cmds.size();
         max_cmds = std::max<uint32_t>(max_cmds, (uint32_t)s.cmds.size());
     }
     for (const Block& B : e.blocks) max_level = std::max<uint32_t>(max_level, B.level);
@@ -554,7 +557,7 @@ int acx_encode(const uint8_t* in, uint64_t N, const acx_enc_opts* uo, uint8_t** 
         std::vector<uint32_t> ext_c, ext_m;
         size_t nm = 0;
         for (const Cmd& c : s.cmds) nm += c.match_len != 0;
-        sym.reserve(s.cmds.size() + nm * (1 + W) + s.lit_a.size() + s.q_sym.size());
+        sym.reserve(s.cmds.size() + nm * (1 + W) + s.lit_a.size() + s.n_sym_q);
         auto put = [&](const Table& t, uint32_t v, uint32_t pb) { sym.push_back(Sym{t.freq[v], t.cum[v], (uint8_t)pb}); };
         for (const Cmd& c : s.cmds) { put(T[0], std::min<uint32_t>(c.lit_len, 255), PROB_BITS); if (c.lit_len >= 255) ext_c.push_back(c.lit_len - 255); }
         for (const Cmd& c : s.cmds) if (c.match_len) {
@@ -565,7 +568,7 @@ int acx_encode(const uint8_t* in, uint64_t N, const acx_enc_opts* uo, uint8_t** 
             for (const Cmd& c : s.cmds) if (c.match_len) put(T[2 + p], (uint8_t)(c.off >> (8 * p)), PROB_BITS);
         for (uint8_t v : s.lit_a) put(T[2 + W], v, PROB_BITS);
         if (q_mode == 1) for (uint16_t v : s.q_sym) put(TQ, qindex[v], MQ_BITS);
-        else for (uint16_t v : s.q_sym) put(T[3 + W], v, PROB_BITS);
+        else for (uint8_t v : s.lit_q) put(T[3 + W], v, PROB_BITS);
         uint32_t X[32]; std::vector<uint16_t> words[32];
         rans_segment(sym, X, words);
         Out o2;
@@ -623,7 +626,7 @@ int acx_encode(const uint8_t* in, uint64_t N, const acx_enc_opts* uo, uint8_t** 
         uint8_t* d = buf + dir_off + 32 * si;
         uint32_t nm = 0;
         for (const Cmd& c : s.cmds) nm += c.match_len != 0;
-        uint16_t v16[8] = {(uint16_t)s.cmds.size(), (uint16_t)nm, (uint16_t)s.lit_a.size(), (uint16_t)s.lit_q.size(), (uint16_t)s.q_sym.size(),
+        uint16_t v16[8] = {(uint16_t)s.cmds.size(), (uint16_t)nm, (uint16_t)s.lit_a.size(), (uint16_t)s.n_lit_q, (uint16_t)s.n_sym_q,
                            (uint16_t)n_words[si], (uint16_t)n_ext[si], e.blocks[s.block].level};
         memcpy(d, &po, 8); memcpy(d + 8, &s.out_start, 8); memcpy(d + 16, v16, 16);
         memcpy(buf + po, pay[si].data(), pay[si].size());
