@@ -43,7 +43,8 @@ enum {
     ACEAPEX_E_BUDGET = -6,     /* vram_budget too small for the call                             */
     ACEAPEX_E_WORKSPACE = -7,  /* workspace missing or smaller than aceapex_info.workspace_bytes */
     ACEAPEX_E_CUDA = -8,       /* a CUDA runtime call failed (aceapex_last_cuda_error)           */
-    ACEAPEX_E_ARG = -9         /* null pointer / bad argument                                    */
+    ACEAPEX_E_ARG = -9,        /* null pointer / bad argument                                    */
+    ACEAPEX_E_TOO_LARGE = -10  /* size beyond the fixed maximum of a no-allocation entry point  */
 };
 
 typedef struct {
@@ -220,6 +221,28 @@ int32_t aceapex_rans_encode(const void* d_in, uint64_t n_rows, uint64_t row_byte
 int32_t aceapex_rans_decode(const void* d_enc, uint64_t n_rows, uint64_t row_bytes, uint64_t row_capacity, const uint32_t* d_row_sizes,
                             const void* d_tables, void* d_out, void* d_scratch, uint64_t scratch_bytes, void* cuda_stream);
 int32_t aceapex_rans_status(const void* d_scratch, void* cuda_stream, uint32_t* status);
+
+/* ---- aceapex_rans_encode without any allocation, for callers that cannot call cudaMalloc (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid it): the word staging and the work counter live in ONE file-scope
+ * `static __device__` array of ACEAPEX_RANS_STATIC_SCRATCH_BYTES (+ 256) bytes inside the library, which every GPU that loads
+ * the library holds until the process exits.  Same inputs, outputs, row layout and result (bit for bit) as
+ * aceapex_rans_encode; the caller passes no scratch.  The number of warps at work is what the fixed array holds
+ * (64 KB rows: 256 warps instead of one per row slot of the GPU), so large rows encode slower than through
+ * aceapex_rans_encode.  Limits and rules:
+ *   - row_bytes > ACEAPEX_RANS_STATIC_MAX_ROW_BYTES returns ACEAPEX_E_TOO_LARGE (nothing is launched); other bad arguments
+ *     E_ARG as in aceapex_rans_encode.
+ *   - The call makes no cudaMalloc / cudaFree and calls no allocating library routine: one cudaMemsetAsync of the 8-byte work
+ *     counter (the only part of the array that must start at zero; the staging keeps the previous call's words, which are
+ *     never read before they are rewritten) and one kernel launch on cuda_stream.
+ *   - ALL calls on a device share the array: calls that overlap on the GPU (different streams, or graphs replayed
+ *     concurrently) race on it and produce garbage.  Calls on one stream are ordered and safe.
+ *   - The device address of the array is looked up once per device, with that device current (cudaGetSymbolAddress), by the
+ *     first call on that device or by aceapex_rans_static_setup(), which callers that capture graphs run before capturing. */
+#define ACEAPEX_RANS_STATIC_SCRATCH_BYTES (32ull << 20)
+#define ACEAPEX_RANS_STATIC_MAX_ROW_BYTES 65536ull
+int32_t aceapex_rans_static_setup(void);
+int32_t aceapex_rans_encode_static(const void* d_in, uint64_t n_rows, uint64_t row_bytes, const void* d_tables, void* d_enc, uint64_t row_capacity,
+                                   uint32_t* d_row_sizes, void* cuda_stream);
 
 enum {
     ACEAPEX_DF_RANS = 1,      /* final rANS state / word count mismatch         */

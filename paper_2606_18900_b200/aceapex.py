@@ -9,7 +9,7 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 _lib = None
 
 ERRORS = {0: "OK", -1: "E_MAGIC", -2: "E_VERSION", -3: "E_TRUNCATED", -4: "E_CORRUPT", -5: "E_RANGE", -6: "E_BUDGET",
-          -7: "E_WORKSPACE", -8: "E_CUDA", -9: "E_ARG"}
+          -7: "E_WORKSPACE", -8: "E_CUDA", -9: "E_ARG", -10: "E_TOO_LARGE"}
 
 
 class AceapexError(RuntimeError):
@@ -77,6 +77,8 @@ def load():
             "aceapex_rans_encode": ([p, u64, u64, p, p, u64, p, p, u64, p], i32),
             "aceapex_rans_decode": ([p, u64, u64, u64, p, p, p, p, u64, p], i32),
             "aceapex_rans_status": ([p, p, ctypes.POINTER(u32)], i32),
+            "aceapex_rans_static_setup": ([], i32),
+            "aceapex_rans_encode_static": ([p, u64, u64, p, p, u64, p, p], i32),
             "aceapex_set_phase_timing": ([p, i32], i32),
             "aceapex_phase_times": ([p, ctypes.POINTER(ctypes.c_float)], i32),
         }
@@ -253,6 +255,16 @@ class RansBatch:
             enc, sizes = self.new_encoded(n)
         _chk(self.L.aceapex_rans_encode(rows.data_ptr(), n, self.row_bytes, self.tables.data_ptr(), enc.data_ptr(), self.row_cap, sizes.data_ptr(),
                                         self.scratch.data_ptr(), self.scratch.numel(), ctypes.c_void_p(self.stream.cuda_stream)), "rans_encode")
+        return enc, sizes
+
+    def encode_static(self, rows, enc=None, sizes=None):
+        """encode() through aceapex_rans_encode_static: no scratch passed, nothing allocated by the library (row_bytes <= 65536)."""
+        n = rows.shape[0]
+        if enc is None:
+            enc, sizes = self.new_encoded(n)
+        with self._torch.cuda.device(self.device):
+            _chk(self.L.aceapex_rans_encode_static(rows.data_ptr(), n, self.row_bytes, self.tables.data_ptr(), enc.data_ptr(), self.row_cap,
+                                                   sizes.data_ptr(), ctypes.c_void_p(self.stream.cuda_stream)), "rans_encode_static")
         return enc, sizes
 
     def decode(self, enc, sizes, n_rows, out=None):

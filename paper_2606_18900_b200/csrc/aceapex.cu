@@ -1040,6 +1040,7 @@ const char* aceapex_strerror(int32_t c) {
         case ACEAPEX_E_WORKSPACE: return "workspace missing or too small";
         case ACEAPEX_E_CUDA: return "CUDA runtime error";
         case ACEAPEX_E_ARG: return "bad argument";
+        case ACEAPEX_E_TOO_LARGE: return "size beyond the fixed maximum of the no-allocation entry point";
     }
     return "unknown error";
 }

@@ -5,10 +5,18 @@
 #include "aceapex.h"
 #include "acx_device.cuh"
 
+#include <algorithm>
 #include <cstring>
+#include <mutex>
 #include <vector>
 
 using namespace acx;
+
+// Scratch of aceapex_rans_encode_static (include/aceapex.h): the row encoder for callers that may not allocate.  Every GPU
+// that loads this library holds these 32 MiB + 256 bytes until the process exits.  Layout: [work ticket u64 @0, pad to 256]
+// [word staging of the resident warps].  In HOST code the name below is a host-side stand-in, not a device address: the
+// host gets the address once per device with cudaGetSymbolAddress (static_scratch_of) and passes that to the kernel.
+static __device__ __align__(256) uint8_t g_static_scratch[ACEAPEX_RANS_STATIC_SCRATCH_BYTES + 256];
 
 namespace {
 
@@ -206,6 +214,50 @@ int32_t aceapex_rans_decode(const void* d_enc, uint64_t n_rows, uint64_t row_byt
     k_rans_decode<<<g, T, smem, st>>>(static_cast<const uint8_t*>(d_enc), n_rows, (uint32_t)row_bytes, row_cap, d_row_sizes,
                                       reinterpret_cast<const uint32_t*>(static_cast<const uint8_t*>(d_tables) + ENC_TABLE_BYTES), static_cast<uint8_t*>(d_out),
                                       reinterpret_cast<uint32_t*>(sc + 8), reinterpret_cast<unsigned long long*>(sc));
+    return cudaGetLastError() == cudaSuccess ? ACEAPEX_OK : ACEAPEX_E_CUDA;
+}
+
+// device address of g_static_scratch and SM count of the current device, looked up once per device
+static int32_t static_scratch_of(uint8_t** ptr, int* sms) {
+    static std::mutex mu;
+    static struct { uint8_t* ptr; int sms; } devs[64];
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return ACEAPEX_E_CUDA;
+    std::lock_guard<std::mutex> lk(mu);
+    if (!devs[dev].ptr) {
+        uint8_t* p = nullptr; int n = 0;
+        if (cudaGetSymbolAddress((void**)&p, g_static_scratch) != cudaSuccess || !p) { cudaGetLastError(); return ACEAPEX_E_CUDA; }
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) return ACEAPEX_E_CUDA;
+        devs[dev].sms = n; devs[dev].ptr = p;
+    }
+    *ptr = devs[dev].ptr; *sms = devs[dev].sms;
+    return ACEAPEX_OK;
+}
+
+int32_t aceapex_rans_static_setup(void) {
+    uint8_t* p; int sms;
+    return static_scratch_of(&p, &sms);
+}
+
+int32_t aceapex_rans_encode_static(const void* d_in, uint64_t n_rows, uint64_t row_bytes, const void* d_tables, void* d_out, uint64_t row_cap,
+                                   uint32_t* d_row_sizes, void* stream) {
+    if (!d_in || !d_tables || !d_out || !d_row_sizes || row_bytes == 0 || (row_cap & 15) || (reinterpret_cast<uintptr_t>(d_out) & 15)) return ACEAPEX_E_ARG;
+    if (row_bytes > ACEAPEX_RANS_STATIC_MAX_ROW_BYTES) return ACEAPEX_E_TOO_LARGE;
+    if (row_cap < 256 + 2 * row_bytes) return ACEAPEX_E_ARG;
+    if (n_rows == 0) return ACEAPEX_OK;
+    uint8_t* sc = nullptr; int sms = 0;
+    const int32_t rc = static_scratch_of(&sc, &sms);
+    if (rc) return rc;
+    // as many warps as the fixed staging area holds (a lane stages at most one word per symbol, in groups of eight)
+    const uint64_t per = ((row_bytes + 31) / 32 + 7) & ~7ull, warp_bytes = 32 * per * 2;
+    const uint64_t warps = std::min<uint64_t>(std::min<uint64_t>((uint64_t)sms * 32, n_rows), ACEAPEX_RANS_STATIC_SCRATCH_BYTES / warp_bytes);
+    const uint64_t wps = warps >= (uint64_t)sms ? std::min<uint64_t>(32, warps / sms) : 1;     // warps per CTA
+    const unsigned g = (unsigned)std::min<uint64_t>(sms, warps / wps);                          // g * wps <= warps
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    unsigned long long* ticket = reinterpret_cast<unsigned long long*>(sc);
+    if (cudaMemsetAsync(ticket, 0, 8, st) != cudaSuccess) return ACEAPEX_E_CUDA;                // the one part of the array that must start at zero
+    k_rans_encode<<<g, (unsigned)(32 * wps), 0, st>>>(static_cast<const uint8_t*>(d_in), n_rows, (uint32_t)row_bytes, static_cast<const EncSym*>(d_tables),
+                                                      static_cast<uint8_t*>(d_out), row_cap, d_row_sizes, reinterpret_cast<uint16_t*>(sc + 256), ticket);
     return cudaGetLastError() == cudaSuccess ? ACEAPEX_OK : ACEAPEX_E_CUDA;
 }
 
