@@ -708,10 +708,17 @@ static int32_t range_launches(aceapex_archive* ar, uint64_t lo, uint64_t hi, uin
         if (ar->max_level == 0) {                           // every source is a literal byte: no order among the window's segments
             P.seg_list = nullptr; P.first_work = s0;
             if ((rc = launch(ar, P, K_COPY_WIN, ns))) return rc;
+        } else if (ar->capturing || ns <= 1024) {
+            // A seek: one flag-driven launch over the window's segments in INDEX order.  A segment waits for lower-level
+            // source blocks of the window only, and sources precede their destinations (src < dst), so it only ever waits
+            // for segments whose tickets were drawn before its own: no deadlock, no list to build or upload, and the
+            // sequence can be replayed as a graph.
+            if ((rc = zero_done(ar, b0, b1 - b0))) return rc;
+            P.seg_list = nullptr; P.first_work = s0;
+            if ((rc = launch(ar, P, K_COPY_WIN_WAIT, ns))) return rc;
         } else {
             // its segments sorted by (level, index) in one flag-driven launch (a segment waits for lower-level source
-            // blocks of the window only; everything outside the window is final)
-            if (ar->capturing) return NOT_GRAPHABLE;
+            // blocks of the window only; everything outside the window is final): sorted, almost nobody waits
             std::vector<uint32_t>& L = ar->h_list;
             L.resize(ns);
             std::vector<uint64_t> cnt(ar->max_level + 2, 0);

@@ -164,7 +164,7 @@ def seeks(torch, ar, x, label, n=300, seed=11):
         lat = np.array(lat)
         res["%d_blocks" % blocks] = {"ms_median": float(np.median(lat)), "ms_p99": float(np.percentile(lat, 99)), "ms_min": float(lat.min()),
                                      "bytes": blocks * BS, "bit_exact": ok}
-    emit(config=label, what="seek_latency", n=n, seeks=res)
+    emit(config=label, what="seek_latency", n=n, seeks=res, graph_launches=ar.graph_launch_count())
 
 
 def reads(torch, ar, x, idx, label, n_single=1000, n_batches=20, batch=4096, seed=5):
@@ -218,6 +218,7 @@ def main():
     ap.add_argument("--config", type=int, required=True)
     ap.add_argument("--size", type=int, default=0)
     ap.add_argument("--src-window", type=int, default=0, help="encoder option: sources at most this far back (0 = unlimited)")
+    ap.add_argument("--max-levels", default="", help="config 3: comma-separated encoder level caps to measure (default: the encoder's)")
     args = ap.parse_args()
     import torch
     from paper_2606_18900_b200 import datagen, encoder
@@ -237,6 +238,11 @@ def main():
         isolated_windows(torch, ar, x, args.config, win)
         reads(torch, ar, x, datagen.fastq_index(size), args.config)
         seeks(torch, ar, x, args.config)
+        ar.close()
+        os.environ["ACEAPEX_NO_GRAPHS"] = "1"                  # read at open: the same seeks with plain launches
+        ar = Archive(a)
+        del os.environ["ACEAPEX_NO_GRAPHS"]
+        seeks(torch, ar, x, "%d/plain launches (ACEAPEX_NO_GRAPHS=1)" % args.config)
         ar.close()
     elif args.config == 2:
         size = args.size or 3_100_000_000
@@ -258,18 +264,23 @@ def main():
         t = time.time()
         x = datagen.fasta(4, size)
         emit(config=3, what="generate", seconds=time.time() - t, bytes=size)
-        t = time.time()
-        a = encoder.encode(x, block_size=16384, src_window=args.src_window)
-        emit(config=3, what="encode", src_window=args.src_window, seconds=time.time() - t, MBps=x.size / (time.time() - t) / 1e6, archive_bytes=int(a.size))
-        ar = Archive(a)
-        info = ar.info()
-        emit(config=3, what="archive", raw_bytes=info["raw_bytes"], archive_bytes=info["archive_bytes"], n_blocks=info["n_blocks"],
-             offset_width=info["offset_width"], max_level=info["max_level"], workspace_bytes=info["workspace_bytes"])
-        window = min(1 << 30, max(1 << 24, size // 8))
-        nwin = (size + window - 1) // window
-        windows(torch, ar, x, 3, window, 8, reps=1, sample_check={0, nwin // 2, nwin - 1})
-        isolated_windows(torch, ar, x, 3, window)
-        ar.close()
+        for max_level in ([int(v) for v in args.max_levels.split(",")] if args.max_levels else [None]):
+            kw = {} if max_level is None else {"max_level": max_level}
+            t = time.time()
+            a = encoder.encode(x, block_size=16384, src_window=args.src_window, **kw)
+            emit(config=3, what="encode", src_window=args.src_window, encoder_max_level=max_level, seconds=time.time() - t,
+                 MBps=x.size / (time.time() - t) / 1e6, archive_bytes=int(a.size))
+            ar = Archive(a)
+            info = ar.info()
+            emit(config=3, what="archive", raw_bytes=info["raw_bytes"], archive_bytes=info["archive_bytes"], n_blocks=info["n_blocks"],
+                 offset_width=info["offset_width"], max_level=info["max_level"], workspace_bytes=info["workspace_bytes"])
+            window = min(1 << 30, max(1 << 24, size // 8))
+            nwin = (size + window - 1) // window
+            windows(torch, ar, x, 3, window, 8, reps=1, sample_check={0, nwin // 2, nwin - 1})
+            isolated_windows(torch, ar, x, 3, window)
+            ar.close()
+            del ar, a
+            torch.cuda.empty_cache()
     elif args.config == 5:
         # the entropy stage alone on the workload shape of PAPER.md:135 (DietGPU: 256 MB of
         # exponentially distributed bytes, 4096 x 64 KB): aceapex_rans_encode / aceapex_rans_decode, one warp per row
@@ -284,7 +295,7 @@ def main():
         emit(config=4, what="launch_overhead", note="SURVEY.md 8(c) S19 (c): the schedule of decode_all on an archive of one 8-byte block",
              **bench.launch_overhead(torch, torch.cuda.current_stream()))
         for bs in (4096, 8192, 16384, 65536, 262144, 1 << 20):
-            for max_level in ((0, 3) if bs == 16384 else (0,)):
+            for max_level in ((2, 0, 3) if bs == 16384 else (2,)):          # 2 = the encoder's default
                 t = time.time()
                 a = encoder.encode(x, block_size=bs, max_level=max_level)
                 enc_s = time.time() - t
@@ -303,7 +314,7 @@ def main():
                      n_segments=info["n_segments"], GBps=res["default"]["GBps"], ms=res["default"]["ms"], mean_level=float(lv.mean()), max_level=int(lv.max()),
                      wavefront_depth=int(lv.max()) + 1, launches_default=res["default"]["launches"], ms_flags=res["flags"]["ms"], ms_fused=res["fused"]["ms"],
                      call_ms=ms_call, kernels_ms=float(sum(ph)), gap_per_launch_us=(ms_call - float(sum(ph))) * 1e3 / max(res["default"]["launches"], 1))
-                if bs == 16384 and max_level == 0:
+                if bs == 16384 and max_level == 2:
                     seeks(torch, ar, x, "4/bs=16384")
                 ar.close()
                 del ar
@@ -312,7 +323,7 @@ def main():
         # encoder options against range-decode speed (measure, do not dismiss): level cap, source window, LITQ mode
         size = args.size or (1 << 30)
         x = datagen.fastq(2, size, 50_000_000)
-        for kw in (dict(), dict(max_level=3), dict(q_mode=0), dict(q_min=0), dict(src_window=256 << 20), dict(src_window=64 << 20), dict(log2_seg=12)):
+        for kw in (dict(), dict(max_level=0), dict(max_level=3), dict(q_mode=0), dict(q_min=0), dict(src_window=256 << 20), dict(src_window=64 << 20), dict(log2_seg=12)):
             t = time.time()
             a = encoder.encode(x, block_size=16384, **kw)
             ar = Archive(a)

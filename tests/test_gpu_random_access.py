@@ -263,6 +263,71 @@ def test_large_window_runs_and_overlaps():
     ar.close()
 
 
+def test_hot_source_segment_and_long_period_overlaps_through_the_demand_rounds():
+    """One early segment (an N-run with newlines: self-overlapping matches of period 61) is the source of thousands of later
+    matches, some of them kilobytes long: windows far from it get its bytes through the demand rounds (records of at most
+    96 bytes, work items of 128 records, seeds copied piecewise), single reads through the per-warp recursion.  Every
+    level cap, vs the original bytes and the oracle."""
+    from paper_2606_18900_b200 import encoder
+    from paper_2606_18900_b200.aceapex import Archive
+    rng = np.random.default_rng(9)
+    nrun = (b"N" * 60 + b"\n") * 400                         # 24,400 bytes, period 61
+    odd = (b"ACGTTGCAGGA" * 7 + b"\n") * 200                 # period 78
+    parts = [b">chr1\n", rng.integers(65, 69, 40_000, dtype=np.uint8).tobytes(), nrun, odd]
+    for k in range(1500):
+        parts.append(rng.integers(65, 69, 700 + (k % 13), dtype=np.uint8).tobytes())
+        cut = 61 * (k % 300) + (k % 61)
+        parts.append(nrun[cut:cut + 30 + (k * 37) % 3000])    # pieces of the run, 30 bytes .. 3 KB
+        if k % 5 == 0:
+            parts.append(odd[(k * 7) % 500:(k * 7) % 500 + 200 + k % 900])
+    x = np.frombuffer(b"".join(parts), dtype=np.uint8)
+    N = x.size
+    for ml in (0, 1, 2):
+        a = encoder.encode(x, block_size=16384, max_level=ml)
+        want = O.decode(a)
+        assert np.array_equal(want, x)
+        ar = Archive(a)
+        for lo, hi in ((N // 2, N // 2 + (1 << 20)), (N - (1 << 20) - 12345, N - 7), (N // 3 + 5, N // 3 + 5 + 70_000)):
+            check_range(ar, x, lo, hi)
+        idx = np.array([(N // 2 + 1000 * i) | (1500 << 40) for i in range(600)], dtype=np.uint64)
+        for ids in (np.array([17], dtype=np.uint64), np.arange(600, dtype=np.uint64)):
+            got = ar.decode_reads(idx, ids).cpu().numpy()
+            ar.check()
+            for j, i in enumerate(ids.tolist()):
+                off = N // 2 + 1000 * i
+                assert got[1500 * j:1500 * (j + 1)].tobytes() == x[off:off + 1500].tobytes(), (ml, i)
+        ar.close()
+
+
+def test_seeks_replayed_as_cuda_graphs_match_plain_launches(monkeypatch):
+    """aceapex_decode_range of up to 8 MiB replays its launch sequence as a CUDA graph with updated node parameters
+    (aceapex_graph_launch_count counts the replays); ACEAPEX_NO_GRAPHS=1 at open keeps the plain launches.  Both against
+    the original bytes, for an archive without levels and for the encoder's default (flag-driven window launch)."""
+    from paper_2606_18900_b200 import datagen, encoder
+    from paper_2606_18900_b200.aceapex import Archive
+    x = datagen.fastq(5, 6 << 20, 1_000_000)
+    rng = np.random.default_rng(4)
+    for kw in (dict(max_level=0), dict(), dict(block_size=65536, max_level=3)):
+        a = encoder.encode(x, **kw)
+        ar_g = Archive(a)
+        monkeypatch.setenv("ACEAPEX_NO_GRAPHS", "1")
+        ar_p = Archive(a)
+        monkeypatch.delenv("ACEAPEX_NO_GRAPHS")
+        BS = ar_g.info()["block_size"]
+        n_calls = 0
+        for k in range(40):
+            blocks = (1, 3, 100 if BS == 16384 else 20)[k % 3]
+            lo = int(rng.integers(0, x.size // BS - blocks)) * BS + (0 if k % 4 else 777)      # aligned and ragged
+            hi = min(x.size, lo + blocks * BS - (0 if k % 5 else 13))
+            want = x[lo:hi].tobytes()
+            assert ar_g.decode_range(lo, hi).cpu().numpy().tobytes() == want, (kw, lo, hi)
+            assert ar_p.decode_range(lo, hi).cpu().numpy().tobytes() == want, (kw, lo, hi)
+            n_calls += 1
+        ar_g.check(); ar_p.check()
+        assert ar_g.graph_launch_count() == n_calls and ar_p.graph_launch_count() == 0, kw
+        ar_g.close(); ar_p.close()
+
+
 def test_end_to_end_host_pipeline(big, fq):
     """aceapex_decode_all_host: archive from pinned host memory, output to pinned host memory, chunks pipelined."""
     for ar, x in (big[0], big[1], fq):
