@@ -7,6 +7,7 @@
   python -m paper_2606_18900_b200.report --config 4            # block-size sweep on the configs[1] FASTQ, launch overhead
   python -m paper_2606_18900_b200.report --config 5            # the rANS stage alone (PAPER.md:135 shape)
   python -m paper_2606_18900_b200.report --config 6            # encoder options (level cap, source window, LITQ mode) vs speed
+  python -m paper_2606_18900_b200.report --config 7            # one isolated 64 MiB window of configs[1] (the ncu target of range decode)
 
 Everything is verified against the ORIGINAL bytes (direct compare where the data fits, per-block FNV-1a otherwise).
 Timing: CUDA events on the handle's stream around the C-ABI calls, after warm-up; GB = 10^9 bytes.
@@ -338,6 +339,23 @@ def main():
             ar.close()
             del ar, ring
             torch.cuda.empty_cache()
+    elif args.config == 7:
+        # one isolated 64 MiB window in the middle of configs[1] (nothing resident: every source before it is foreign), three
+        # times: the command profiles/r2_range_window.md captures with ncu
+        size = args.size or (1 << 30)
+        x = datagen.fastq(2, size, 50_000_000)
+        ar = Archive(encoder.encode(x, block_size=16384))
+        W = min(64 << 20, size // 4)
+        lo = (size // 2) & ~(W - 1)
+        buf = ar.new_output(W)
+        for _ in range(3):
+            ar.decode_range(lo, lo + W, out=buf)
+        torch.cuda.synchronize()
+        ar.check()
+        ms = timed(torch, torch.cuda.current_stream(), lambda: ar.decode_range(lo, lo + W, out=buf), 3, warmup=0)
+        emit(config=7, what="isolated_window", lo=lo, hi=lo + W, ms=ms, GBps=W / ms / 1e6, launches=ar.launch_count() // 6,
+             bit_exact=bool(torch.equal(buf[:W].cpu(), torch.from_numpy(x[lo:lo + W]))))
+        ar.close()
 
 
 _OUT = {}
