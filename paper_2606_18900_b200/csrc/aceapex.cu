@@ -470,6 +470,10 @@ int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* 
     // per-warp shared memory besides the word ring: the LITQ run table (a command table of 2 KB in the span-service kernels)
     // and, with what the tables leave free, a staging area for LITA (up to 4 KB; larger segments stage in global memory)
     ar->threads = 1024;
+    if (const char* e = getenv("ACEAPEX_THREADS")) {      // tests: other CTA sizes (other interleavings of the flag-driven launches)
+        const int t = atoi(e);
+        if (t >= 128 && t <= 1024) ar->threads = t / 64 * 64;
+    }
     ar->runs_bytes = runs_bytes_for(ar->q_min);
     const uint32_t min_area = std::max<uint32_t>(4 * (MAX_SEG_CMDS + 2), ar->runs_bytes + ALIST_BYTES);
     auto smem_max = [&](int T, uint32_t area) { return std::max(entropy_smem(ar->n_coded_tables, ar->q_mode, area, T), (size_t)(T / 32) * COPY_WARP_BYTES + 64); };

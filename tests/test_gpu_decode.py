@@ -143,6 +143,38 @@ def test_repeated_calls_and_fnv(fastq_4m, fastq_4m_archive):
     ar.close()
 
 
+def test_flag_schedules_stress(fastq_4m, monkeypatch):
+    """The completion-count protocol (S20) under repetition: compute-sanitizer is refused on this GPU pool, so the
+    flag-driven schedules are run 200 times per CTA size on configs[0] encoded with a deep level structure (max_level 7: most
+    blocks wait for others), every output compared with the original bytes on the device; then flag-driven windows."""
+    from paper_2606_18900_b200 import encoder
+    from paper_2606_18900_b200.aceapex import Archive
+    a = encoder.encode(fastq_4m, block_size=16384, max_level=7)
+    want = torch.from_numpy(fastq_4m).cuda()
+    rng = np.random.default_rng(8)
+    for threads in ("1024", "512", "192"):
+        monkeypatch.setenv("ACEAPEX_THREADS", threads)
+        ar = Archive(a)
+        monkeypatch.delenv("ACEAPEX_THREADS")
+        assert ar.info()["max_level"] >= 5
+        out = ar.new_output()
+        for k in range(200):
+            sched = ("flags", "fused", None)[k % 3]
+            out.fill_(0xA5)
+            ar.decode_all(out, schedule=sched)
+            assert torch.equal(out[:want.numel()], want), (threads, k, sched)
+        ar.check()
+        buf = ar.new_output(1 << 20)
+        for k in range(60):                                      # windows of 3..60 blocks: flag-driven, in index order
+            lo = int(rng.integers(0, 190)) * 16384
+            hi = lo + int(rng.integers(3, 60)) * 16384
+            buf.fill_(0x5A)
+            ar.decode_range(lo, hi, out=buf)
+            assert torch.equal(buf[:hi - lo], want[lo:hi]), (threads, lo, hi)
+        ar.check()
+        ar.close()
+
+
 def test_open_errors(fastq_4m_archive):
     from paper_2606_18900_b200.aceapex import AceapexError, Archive
     bad = fastq_4m_archive.copy()
