@@ -267,7 +267,7 @@ int32_t replay(aceapex_archive* ar) {
     return ACEAPEX_OK;
 }
 
-enum Kind { K_LIT, K_COPY_TOP, K_COPY_WAIT, K_COPY_WIN, K_COPY_WIN_WAIT, K_COLLECT, K_SERVE, K_SPANS };
+enum Kind { K_LIT, K_COPY_TOP, K_COPY_WAIT, K_COPY_WIN, K_COPY_WIN_WAIT, K_COLLECT, K_SERVE, K_SPANS, K_SPANS_CTA };
 
 int32_t launch(aceapex_archive* ar, Params& P, Kind kind, uint64_t n_work) {
     P.n_work = n_work;
@@ -275,6 +275,10 @@ int32_t launch(aceapex_archive* ar, Params& P, Kind kind, uint64_t n_work) {
     take_ticket(ar, P);
     int T; uint32_t g;
     spread(ar, n_work, ar->threads, g, T);
+    // kernels that stage the decode tables (40-70 KB per CTA): a CTA of one or two warps would spend tens of microseconds
+    // loading them; at least eight warps load (the ones without work find no ticket and leave)
+    static const int min_t = getenv("ACEAPEX_MIN_THREADS") ? atoi(getenv("ACEAPEX_MIN_THREADS")) : 256;
+    if ((kind == K_LIT || kind == K_SPANS) && T < min_t) T = std::min(ar->threads, std::max(T, min_t / 32 * 32));
     const size_t sm_e = entropy_smem(ar->n_coded_tables, ar->q_mode, ar->runs_bytes + ALIST_BYTES + ar->lita_bytes, T), sm_c = (size_t)(T / 32) * COPY_WARP_BYTES + 64;
     const void* f = nullptr; size_t sm = sm_c; dim3 gd(g), bd(T);
     switch (kind) {
@@ -291,6 +295,12 @@ int32_t launch(aceapex_archive* ar, Params& P, Kind kind, uint64_t n_work) {
         case K_COLLECT: f = (const void*)k_copy<false, true, true, false>; break;
         case K_SERVE: f = (const void*)k_serve; sm = ar->smem_entropy; gd = dim3(ar->sms); bd = dim3(ar->threads); break;
         case K_SPANS: f = (const void*)k_spans; sm = sm_e; break;
+        case K_SPANS_CTA: {                                    // one CTA of up to 16 warps that share the read's queue of spans
+            const int Tc = std::max(128, std::min(ar->threads, 512));
+            f = (const void*)k_spans_cta; gd = dim3(1); bd = dim3(Tc);
+            sm = entropy_smem(ar->n_coded_tables, ar->q_mode, ar->runs_bytes + ALIST_BYTES + ar->lita_bytes, Tc);
+            break;
+        }
     }
     return submit_kernel(ar, f, gd, bd, sm, false, {{&P, sizeof P}});
 }
@@ -493,7 +503,7 @@ int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* 
                              (const void*)k_fused<0>, (const void*)k_fused<1>, (const void*)k_fused<3>, (const void*)k_fused<4>,
                              (const void*)k_copy<false, false, false, true>, (const void*)k_copy<true, false, false, false>,
                              (const void*)k_copy<false, true, false, false>, (const void*)k_copy<true, true, false, false>, (const void*)k_copy<false, true, true, false>,
-                             (const void*)k_serve, (const void*)k_spans, (const void*)k_rounds};
+                             (const void*)k_serve, (const void*)k_spans, (const void*)k_spans_cta, (const void*)k_rounds};
         for (const void* f : fns) {
             // the attribute belongs to the function, not to the handle: always the device maximum, so that handles with
             // different table counts do not lower each other's limit
@@ -814,7 +824,8 @@ static int32_t run_spans(aceapex_archive* ar, Params& P) {
     if (ar->h_demands.size() <= 4) {                   // a single read: the items travel in the kernel arguments, no copy
         P.n_inline = (uint32_t)ar->h_demands.size();
         for (uint32_t i = 0; i < P.n_inline; i++) P.inline_dem[i] = ar->h_demands[i];
-        return launch(ar, P, K_SPANS, P.n_inline);
+        static const bool one_warp = getenv("ACEAPEX_READ_ONE_WARP") != nullptr;      // the earlier path, for comparison
+        return launch(ar, P, one_warp ? K_SPANS : K_SPANS_CTA, P.n_inline);
     }
     for (size_t i = 0; i < ar->h_demands.size(); i += ar->demand_cap) {
         size_t n = std::min<size_t>(ar->demand_cap, ar->h_demands.size() - i);

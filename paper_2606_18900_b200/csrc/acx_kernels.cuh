@@ -476,7 +476,7 @@ __device__ __forceinline__ void push_span(const Params& P, const Stack& st, uint
         else {
             uint32_t idx;
             asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(idx) : "r"(st.top) : "memory");
-            if (idx < st.cap) { st.base[idx].pos = pos; st.base[idx].dst = dst; st.base[idx].len = n; }
+            if (idx < st.cap) { st.base[idx].pos = pos; st.base[idx].dst = dst; __threadfence_block(); st.base[idx].len = n; }   // len last: k_spans_cta polls it
             else report(P, DF_STACK);
         }
         pos += n; dst += n; len -= n;
@@ -1240,6 +1240,75 @@ __global__ void __launch_bounds__(1024, 1) k_spans(const __grid_constant__ Param
             push_span(P, st, d.pos, d.len, d.dst);
         }
         process_demands(P, m, c, st);
+    }
+}
+
+// A single read (at most four top-level spans): ONE CTA whose warps share a queue of spans in place of the per-warp stack of
+// k_spans, so that the source segments of a span (five or so for a FASTQ record, then theirs) are parsed side by side by
+// different warps instead of one after the other by one warp: the latency of a read is its recursion depth
+// (<= max_level + 2 parses), not its number of source segments.  Queue = the CTA's first stack area in the workspace;
+// shared counters: tail (entries pushed; push_span adds), head (entries claimed), done (entries served).  An entry is
+// published by its `len` (written last, zero before); a warp leaves when everything pushed so far has been served (then
+// nobody can push any more).  Every demand is served from its own parse of its segment and written straight to its
+// destination: there are no data dependencies between entries.  All waits are bounded (DF_TIMEOUT).
+__global__ void __launch_bounds__(1024, 1) k_spans_cta(const __grid_constant__ Params P) {
+    extern __shared__ __align__(16) uint8_t smem_raw[];
+    clear_next_ticket(P);
+    const CtaSmem m = setup_cta(P, smem_raw);
+    const uint32_t lane = lane_id(), warps = blockDim.x >> 5;
+    // tail, head, done: the stack-top words of the CTA's first three warps (the CTA has at least four; no static shared
+    // memory: the kernel uses the whole opt-in maximum of dynamic shared memory like the others)
+    const uint32_t a_tail = m.top - 4u * (threadIdx.x >> 5);
+    uint32_t* const s_q = reinterpret_cast<uint32_t*>(smem_raw + (a_tail - (uint32_t)__cvta_generic_to_shared(smem_raw)));
+    Demand* const queue = P.stacks + (uint64_t)blockIdx.x * warps * P.stack_cap;
+    const uint32_t cap = P.stack_cap;
+    for (uint32_t i = threadIdx.x; i < cap; i += blockDim.x) queue[i].len = 0;
+    if (threadIdx.x < 3) s_q[threadIdx.x] = 0;
+    __threadfence_block();
+    __syncthreads();
+    SegCtx c;
+    bind_scratch(P, blockIdx.x * warps + (threadIdx.x >> 5), c);
+    Stack st;
+    st.base = queue; st.cap = cap; st.top = a_tail; st.gl = nullptr; st.policy = 0;
+    if (threadIdx.x == 0)
+        for (uint32_t i = 0; i < P.n_inline; i++) push_span(P, st, P.inline_dem[i].pos, P.inline_dem[i].len, P.inline_dem[i].dst);
+    __syncthreads();                                         // nobody looks at the counters before the read's own spans are in
+    volatile uint32_t* const q = s_q;
+    constexpr uint32_t LEAVE = 0xffffffffu;
+    for (;;) {
+        uint32_t h = LEAVE;
+        if (lane == 0) {
+            for (uint32_t spins = 0;; spins++) {
+                const uint32_t done = q[2];                  // read BEFORE tail: done == tail then means that nothing is in flight
+                const uint32_t tail = min(q[0], cap), head = q[1];
+                if (head < tail) { if (atomicCAS(&s_q[1], head, head + 1) == head) { h = head; break; } continue; }
+                if (done >= tail) break;
+                if (spins > (1u << 22)) { report(P, DF_TIMEOUT); break; }
+                __nanosleep(64);
+            }
+        }
+        h = __shfl_sync(0xffffffffu, h, 0);
+        if (h == LEAVE) break;
+        Demand d; d.pos = 0; d.dst = 0; d.len = 0;
+        {
+            volatile Demand* const e = queue + h;
+            for (uint32_t spins = 0; (d.len = e->len) == 0 && spins < (1u << 22); spins++) __nanosleep(32);
+            __threadfence_block();
+            d.pos = e->pos; d.dst = e->dst;
+        }
+        if (d.len == 0) { if (lane == 0) report(P, DF_TIMEOUT); }
+        else if (d.pos >= P.N) { if (lane == 0) report(P, DF_OFFSET); }
+        else {
+            c.s = seg_of(P, d.pos);
+            uint16_t* const side0 = c.side;
+            const bool ok = parse_for_spans(P, m.luts, m.lutq, m.ring, m.runs, m.area, c, d.pos + d.len);
+            const bool inside = d.pos >= c.sstart && d.pos + d.len <= c.send;
+            if (ok && !inside && lane == 0) report(P, DF_LENGTH);
+            emit_records(P, c, st, m.runs, ok && inside && lane == 0, d.pos, (uint32_t)d.len, d.dst);
+            c.side = side0;
+        }
+        __syncwarp();
+        if (lane == 0) { __threadfence_block(); atomicAdd(&s_q[2], 1u); }
     }
 }
 

@@ -104,6 +104,27 @@ def test_reads_fastq(fq):
     assert got[:exp.size].tobytes() == exp.tobytes()
 
 
+def test_single_reads_one_cta_many_warps():
+    """A single read goes through k_spans_cta (one CTA, a shared queue of spans, many warps): 400 single reads on FASTQ and
+    FASTA archives with 0, 2 and 7 dependency levels, long reads (32 KB, several segments) included, vs the original bytes."""
+    from paper_2606_18900_b200 import datagen, encoder
+    from paper_2606_18900_b200.aceapex import Archive
+    rng = np.random.default_rng(12)
+    for x in (datagen.fastq(7, 3 << 20, 1_000_000), datagen.fasta(8, 2 << 20)):
+        for ml in (0, 2, 7):
+            ar = Archive(encoder.encode(x, block_size=16384, max_level=ml))
+            offs = rng.integers(0, x.size - 40_000, 400).astype(np.uint64)
+            lens = np.where(np.arange(400) % 50 == 0, 32_768, rng.integers(1, 700, 400)).astype(np.uint64)
+            idx = offs | (lens << np.uint64(40))
+            out = ar.new_output(40_000)
+            for i in range(400):
+                ar.decode_reads(idx, np.array([i], dtype=np.uint64), out=out)
+                o, ln = int(offs[i]), int(lens[i])
+                assert out[:ln].cpu().numpy().tobytes() == x[o:o + ln].tobytes(), (ml, i, o, ln)
+            ar.check()
+            ar.close()
+
+
 def test_reads_regions_fasta(fa):
     from paper_2606_18900_b200 import datagen
     ar, x = fa
