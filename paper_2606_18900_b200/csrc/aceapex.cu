@@ -152,7 +152,7 @@ void fill_params(const aceapex_archive* ar, Params& P) {
     P.done = reinterpret_cast<uint32_t*>(ar->d_ws + ar->done_off);
     P.scratch = ar->d_ws + ar->scratch_off;
     P.scratch_per_warp = ar->scratch_per_warp;
-    P.out_pos0 = 0; P.win_end = ar->N;
+    P.out_pos0 = 0; P.win_end = ar->N; P.copy_parts = 1;
     P.stacks = reinterpret_cast<Demand*>(ar->d_ws + ar->stacks_off); P.stack_cap = ar->stack_cap;
     P.pairs = reinterpret_cast<uint2*>(ar->d_ws + ar->desc_off);
     P.cplanes = ar->d_ws + ar->cplanes_off;
@@ -270,9 +270,17 @@ int32_t replay(aceapex_archive* ar) {
 enum Kind { K_LIT, K_COPY_TOP, K_COPY_WAIT, K_COPY_WIN, K_COPY_WIN_WAIT, K_COLLECT, K_SERVE, K_SPANS, K_SPANS_CTA };
 
 int32_t launch(aceapex_archive* ar, Params& P, Kind kind, uint64_t n_work) {
-    P.n_work = n_work;
+    P.n_work = n_work; P.copy_parts = 1;
     if (n_work == 0) return ACEAPEX_OK;
     take_ticket(ar, P);
+    if (kind == K_COPY_TOP || kind == K_COPY_WAIT || kind == K_COPY_WIN || kind == K_COPY_WIN_WAIT || kind == K_COLLECT) {
+        // a seek: far fewer segments than resident warps; every segment's matches are shared out among up to eight warps
+        static const uint32_t max_parts = getenv("ACEAPEX_COPY_PARTS") ? (uint32_t)atoi(getenv("ACEAPEX_COPY_PARTS")) : 8;
+        const uint64_t resident = (uint64_t)ar->sms * (ar->threads / 32);
+        uint32_t parts = 1;
+        while (parts < max_parts && n_work * parts * 2 <= resident / 2) parts *= 2;
+        P.copy_parts = parts; P.n_work = n_work * parts; n_work = P.n_work;
+    }
     int T; uint32_t g;
     spread(ar, n_work, ar->threads, g, T);
     // kernels that stage the decode tables (40-70 KB per CTA): a CTA of one or two warps would spend tens of microseconds

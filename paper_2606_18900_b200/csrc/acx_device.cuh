@@ -63,6 +63,7 @@ struct Params {
     uint32_t runs_bytes, lita_bytes;     // per-warp shared memory: LITQ run table / LITA staging (multiples of 16)
     // work
     uint64_t first_work, n_work;         // work items: segments first_work + i, or seg_list[i]
+    uint32_t copy_parts;                 // k_copy: shares per segment (n_work = segments x copy_parts); 1 in every other kernel
     const uint32_t* seg_list;
     uint8_t* out;                        // byte at absolute position p is out[p - out_pos0]
     uint64_t out_pos0, win_end;          // out holds the original bytes [out_pos0, win_end) (the window; block aligned start)

@@ -425,7 +425,7 @@ __device__ __forceinline__ bool literals_of_segment(const Params& P, uint32_t s_
 // done[S] counts the segments of block S completed by the current flag-driven launch (zeroed before it).
 __device__ __forceinline__ void wait_block(const Params& P, uint64_t S) {
     const uint32_t* f = P.done + S;
-    const uint32_t want = __ldg(P.first_seg + S + 1) - __ldg(P.first_seg + S);
+    const uint32_t want = (__ldg(P.first_seg + S + 1) - __ldg(P.first_seg + S)) * P.copy_parts;   // every share of every segment
     uint32_t spins = 0, ns = 128;
     while (ld_flag(f) < want) {
         __nanosleep(ns);
@@ -559,7 +559,9 @@ constexpr uint32_t COPY_WARP_BYTES = 2 * (MTAB_BYTES + 16 * STAGE_CHUNKS);
 static_assert(LONG_MATCH < 256 && (15 + LONG_MATCH + 15) / 16 <= STAGE_CHUNKS, "a short match fits the stage");
 static_assert(COPY_WARP_BYTES % 16 == 0, "tables and stages are 16-byte aligned");
 
-struct Work { unsigned long long* ticket; const uint32_t* seg_list; uint64_t first_work, n_work; };
+// parts: a small launch (a seek) cuts every segment's matches into `parts` interleaved shares of 32-match groups, a work item
+// each (no match reads match bytes of its own block, so the shares are independent): a lone warp per segment is all latency
+struct Work { unsigned long long* ticket; const uint32_t* seg_list; uint64_t first_work, n_work; uint32_t parts; };
 
 template <bool WAIT, bool WIN, bool COLLECT, bool REVERSE>
 __device__ __forceinline__ void copy_body(const Params& P, const Work W, uint32_t smem_warp /* shared address of this warp's COPY_WARP_BYTES */) {
@@ -573,7 +575,10 @@ __device__ __forceinline__ void copy_body(const Params& P, const Work W, uint32_
         if (t >= W.n_work) break;
         // The wait-free launch of the whole file takes the last segments first: their literals and descriptors are what
         // k_literals wrote last, so the first ~100 MB of the launch's destination sectors and descriptors are still in L2.
-        const unsigned long long tt = REVERSE ? W.n_work - 1 - t : t;
+        unsigned long long tt = REVERSE ? W.n_work - 1 - t : t;
+        uint32_t part = 0;
+        if (W.parts > 1) { part = (uint32_t)(tt % W.parts); tt /= W.parts; }
+        const uint32_t g_step = 32u * W.parts;
         const uint64_t s = W.seg_list ? (uint64_t)W.seg_list[tt] : W.first_work + tt;
         const uint64_t mp0 = __ldg(P.match_prefix + s);
         const uint4* d4 = reinterpret_cast<const uint4*>(P.dir + s);
@@ -586,7 +591,7 @@ __device__ __forceinline__ void copy_body(const Params& P, const Work W, uint32_
         const uint32_t slen = (uint32_t)(seg_end(P, s, b) - sstart);
         const uint32_t lvl = dq.w >> 16;
         uint8_t* const out_seg = P.out + (sstart - P.out_pos0);
-        uint32_t g0 = 0, pending = 0, mis = 0, len = 0, dst_rel = 0;
+        uint32_t g0 = 32u * part, pending = 0, mis = 0, len = 0, dst_rel = 0;
         uint64_t sp = 0;
         bool done = n == 0;
         // (dst_rel, len) from k_literals, the offset bytes from its decoded coded planes and the raw planes of the payload.
@@ -632,7 +637,7 @@ __device__ __forceinline__ void copy_body(const Params& P, const Work W, uint32_
                     const uint64_t src = desc_src(nv), dst = sstart + npr.x;
                     dst_rel = npr.x; len = npr.y;
                     const bool has = g0 + lane < n;
-                    g0 += 32;
+                    g0 += g_step;
                     const bool good = has && src < dst && (uint64_t)dst_rel + len <= slen && len != 0;
                     if (has && !good) report(P, src < dst ? DF_LENGTH : DF_OFFSET);
                     const bool ovl = good && src + len > dst;
@@ -1039,7 +1044,7 @@ __global__ void __launch_bounds__(1024, 1) k_copy(const __grid_constant__ Params
     extern __shared__ __align__(16) uint8_t smem_raw[];
     clear_next_ticket(P);
     const uint32_t smem0 = ((uint32_t)__cvta_generic_to_shared(smem_raw) + 15u) & ~15u;
-    copy_body<WAIT, WIN, COLLECT, REVERSE>(P, Work{P.ticket, P.seg_list, P.first_work, P.n_work}, smem0 + (threadIdx.x >> 5) * COPY_WARP_BYTES);
+    copy_body<WAIT, WIN, COLLECT, REVERSE>(P, Work{P.ticket, P.seg_list, P.first_work, P.n_work, P.copy_parts}, smem0 + (threadIdx.x >> 5) * COPY_WARP_BYTES);
 }
 
 // The whole wavefront in ONE cooperative launch (a single persistent kernel): the literal wave over
@@ -1068,11 +1073,11 @@ __global__ void __launch_bounds__(1024, 1) k_fused(const __grid_constant__ Param
     const uint32_t smem0 = ((uint32_t)__cvta_generic_to_shared(smem_raw) + 15u) & ~15u;
     const uint32_t mine = smem0 + (threadIdx.x >> 5) * COPY_WARP_BYTES;
     if (F.n_low) {
-        copy_body<true, false, false, false>(P, Work{F.tickets + 1, F.low_list, 0, F.n_low}, mine);
+        copy_body<true, false, false, false>(P, Work{F.tickets + 1, F.low_list, 0, F.n_low, 1u}, mine);
         __threadfence();
         grid.sync();
     }
-    copy_body<false, false, false, true>(P, Work{F.tickets + 2, F.top_list, 0, F.n_top}, mine);
+    copy_body<false, false, false, true>(P, Work{F.tickets + 2, F.top_list, 0, F.n_top, 1u}, mine);
 }
 
 // ---- demand rounds ---------------------------------------------------------------------------------------------------
