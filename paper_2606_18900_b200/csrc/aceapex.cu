@@ -267,7 +267,7 @@ int32_t replay(aceapex_archive* ar) {
     return ACEAPEX_OK;
 }
 
-enum Kind { K_LIT, K_COPY_TOP, K_COPY_WAIT, K_COPY_WIN, K_COPY_WIN_WAIT, K_COLLECT, K_SERVE, K_SPANS, K_SPANS_CTA };
+enum Kind { K_LIT, K_LIT_COLLECT, K_COPY_TOP, K_COPY_WAIT, K_COPY_WIN, K_COPY_WIN_WAIT, K_COLLECT, K_SERVE, K_SPANS, K_SPANS_CTA };
 
 int32_t launch(aceapex_archive* ar, Params& P, Kind kind, uint64_t n_work) {
     P.n_work = n_work; P.copy_parts = 1;
@@ -286,7 +286,7 @@ int32_t launch(aceapex_archive* ar, Params& P, Kind kind, uint64_t n_work) {
     // kernels that stage the decode tables (40-70 KB per CTA): a CTA of one or two warps would spend tens of microseconds
     // loading them; at least eight warps load (the ones without work find no ticket and leave)
     static const int min_t = getenv("ACEAPEX_MIN_THREADS") ? atoi(getenv("ACEAPEX_MIN_THREADS")) : 256;
-    if ((kind == K_LIT || kind == K_SPANS) && T < min_t) T = std::min(ar->threads, std::max(T, min_t / 32 * 32));
+    if ((kind == K_LIT || kind == K_LIT_COLLECT || kind == K_SPANS) && T < min_t) T = std::min(ar->threads, std::max(T, min_t / 32 * 32));
     const size_t sm_e = entropy_smem(ar->n_coded_tables, ar->q_mode, ar->runs_bytes + ALIST_BYTES + ar->lita_bytes, T), sm_c = (size_t)(T / 32) * COPY_WARP_BYTES + 64;
     const void* f = nullptr; size_t sm = sm_c; dim3 gd(g), bd(T);
     switch (kind) {
@@ -295,6 +295,12 @@ int32_t launch(aceapex_archive* ar, Params& P, Kind kind, uint64_t n_work) {
             if (!ar->q_mode) f = ar->q_min >= 64 ? (const void*)k_literals<3> : (const void*)k_literals<0>;
             else if (P.out_odd) f = (const void*)k_literals<2>;
             else f = ar->q_min >= 64 ? (const void*)k_literals<4> : (const void*)k_literals<1>;
+            break;
+        case K_LIT_COLLECT:                                    // a window: literal pass and collect pass in one launch
+            sm = sm_e;
+            if (!ar->q_mode) f = ar->q_min >= 64 ? (const void*)k_literals<3, true> : (const void*)k_literals<0, true>;
+            else if (P.out_odd) f = (const void*)k_literals<2, true>;
+            else f = ar->q_min >= 64 ? (const void*)k_literals<4, true> : (const void*)k_literals<1, true>;
             break;
         case K_COPY_TOP: f = (const void*)k_copy<false, false, false, true>; break;
         case K_COPY_WAIT: f = (const void*)k_copy<true, false, false, false>; break;
@@ -507,7 +513,8 @@ int32_t aceapex_open(const void* d_archive, uint64_t archive_bytes, const void* 
     ar->smem_copy = (size_t)(ar->threads / 32) * COPY_WARP_BYTES + 64;
     ar->smem_fused = std::max(ar->smem_entropy, ar->smem_copy);
     {
-        const void* fns[] = {(const void*)k_literals<0>, (const void*)k_literals<1>, (const void*)k_literals<2>, (const void*)k_literals<3>, (const void*)k_literals<4>,
+        const void* fns[] = {(const void*)k_literals<0, true>, (const void*)k_literals<1, true>, (const void*)k_literals<2, true>, (const void*)k_literals<3, true>, (const void*)k_literals<4, true>,
+                             (const void*)k_literals<0>, (const void*)k_literals<1>, (const void*)k_literals<2>, (const void*)k_literals<3>, (const void*)k_literals<4>,
                              (const void*)k_fused<0>, (const void*)k_fused<1>, (const void*)k_fused<3>, (const void*)k_fused<4>,
                              (const void*)k_copy<false, false, false, true>, (const void*)k_copy<true, false, false, false>,
                              (const void*)k_copy<false, true, false, false>, (const void*)k_copy<true, true, false, false>, (const void*)k_copy<false, true, true, false>,
@@ -712,15 +719,26 @@ static int32_t range_launches(aceapex_archive* ar, uint64_t lo, uint64_t hi, uin
         set_out(P, out + (alo - lo), alo, ahi); P.out2 = P.out;
         // (1) literals of the window; (2) foreign seed bytes of its matches -> demand lists, served in rounds, every
         // source segment parsed once per round; (3) matches of the window
-        P.seg_list = nullptr; P.first_work = s0;
-        if ((rc = launch(ar, P, K_LIT, ns))) return rc;
         const GList g[2] = {glist(ar, 0), glist(ar, 1)};
+        // the demands of the whole window fit the lists: its literal launch does the collect pass too
+        static const bool no_merge = getenv("ACEAPEX_NO_COLLECT_MERGE") != nullptr;
+        // (not for a seek: there the separate collect launch shares every segment's matches out among eight warps)
+        const bool merged = !no_merge && ns >= 1024 && ar->h_match_prefix[s1] - ar->h_match_prefix[s0] <= ar->gl_eff / 3;
+        P.seg_list = nullptr; P.first_work = s0;
+        if (merged) {
+            if ((rc = submit_memset(ar, g[0].count, 32))) return rc;
+            P.gl_nxt = g[0];
+        }
+        if ((rc = launch(ar, P, merged ? K_LIT_COLLECT : K_LIT, ns))) return rc;
         for (uint64_t w0 = s0; w0 < s1;) {                  // sub-windows whose demands fit the lists
             uint64_t w1 = w0 + 1;
             while (w1 < s1 && ar->h_match_prefix[w1 + 1] - ar->h_match_prefix[w0] <= ar->gl_eff / 3) w1++;
-            if ((rc = submit_memset(ar, g[0].count, 32))) return rc;
-            P.seg_list = nullptr; P.first_work = w0; P.gl_nxt = g[0];
-            if ((rc = launch(ar, P, K_COLLECT, w1 - w0))) return rc;
+            if (merged) w1 = s1;
+            else {
+                if ((rc = submit_memset(ar, g[0].count, 32))) return rc;
+                P.seg_list = nullptr; P.first_work = w0; P.gl_nxt = g[0];
+                if ((rc = launch(ar, P, K_COLLECT, w1 - w0))) return rc;
+            }
             Params Q = P;                                   // serving knows no window: sources of foreign bytes precede it
             Q.out_pos0 = 0; Q.win_end = 0;
             // a seed byte is found after at most max_level + 1 source blocks (FORMAT.md §3): one round each

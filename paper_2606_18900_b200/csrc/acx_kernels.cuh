@@ -219,6 +219,11 @@ __host__ __device__ inline uint32_t runs_bytes_for(uint32_t q_min) {   // run ta
     return (4 * (n + 2) + 15) & ~15u;
 }
 
+// COLLECT (a window of a range decode whose demands fit the lists in one go): the scan also does the collect pass of the
+// window, i.e. appends the unknown seed bytes of every match to the demand lists (defined behind resolve_src)
+__device__ __forceinline__ void collect_match(const Params& P, const SegCtx& c, uint64_t src, uint64_t dst, uint32_t len);
+
+template <bool COLLECT>
 __device__ __forceinline__ bool build_runs(const Params& P, const SegCtx& c, uint32_t runs /* shared address */, uint8_t* out_seg, uint32_t* q_edge_out) {
     ScanState st; scan_init(st, c);
     const uint32_t alist = runs + P.runs_bytes;                // 32 x 8 bytes behind the run table
@@ -237,6 +242,7 @@ __device__ __forceinline__ bool build_runs(const Params& P, const SegCtx& c, uin
         good = good && cmd_ok(P, c, L) && n_q + __popc(mq) <= q_cap;
         if (__any_sync(0xffffffffu, !good)) break;
         if (pairs && L.has_match) pairs[c0 + lane] = make_uint2(L.out_rel + L.lit_len, L.match_len);
+        if (COLLECT && L.has_match) collect_match(P, c, match_src(P, c, c0 + lane), c.sstart + L.out_rel + L.lit_len, L.match_len);
         const bool a_run = L.valid && !L.is_q && L.lit_len;
         {   // LITA runs of this group: up to eight bytes by the lane that owns the command (two aligned 32-bit loads and a
             // funnel shift per four bytes, byte stores: the runs start anywhere); longer ones by the whole warp, coalesced
@@ -402,7 +408,7 @@ __device__ __forceinline__ void decode_q(Rans& r, uint32_t lut, uint32_t i0, uin
 // A1 + A2 + A3 for one segment: tokens and LITA, scan (LITA placement, LITQ run table, match descriptors), LITQ straight to
 // its positions.  QM: 0 = LITQ bytes, 1 = aligned pairs, 2 = pairs at an odd address.  lita_stage: the warp's staging area
 // in shared memory (generic pointer); a segment with more LITA bytes than it holds stages them in the global scratch.
-template <int QM>
+template <int QM, bool COLLECT = false>
 __device__ __forceinline__ bool literals_of_segment(const Params& P, uint32_t s_luts, uint32_t s_lutq, uint32_t ring, uint32_t runs, uint8_t* lita_stage, SegCtx& c) {
     if (!load_seg(P, c)) return false;
     uint8_t* const out_seg = P.out + (c.sstart - P.out_pos0);
@@ -410,7 +416,7 @@ __device__ __forceinline__ bool literals_of_segment(const Params& P, uint32_t s_
     if (c.d.n_lit_a <= P.lita_bytes) c.lit_a = lita_stage;
     Rans r; uint32_t i0, q_edge;
     parse_streams(P, s_luts, ring, c, r, &i0);
-    const bool ok = build_runs(P, c, runs, out_seg, &q_edge);
+    const bool ok = build_runs<COLLECT>(P, c, runs, out_seg, &q_edge);
     c.lit_a = lit_a_scratch;
     if (!ok) return false;
     // QM: 0 / 1 / 2 as above with run tables of any shape; 3 = bytes, 4 = pairs when every LITQ run has 32 symbols or more
@@ -539,6 +545,19 @@ __device__ __forceinline__ const uint8_t* resolve_src(const Params& P, uint64_t 
     for (int r = 0; r < MAX_RESIDENT; r++)
         if (src >= P.res[r].lo && src + n <= P.res[r].hi) { *end = P.res[r].ptr + (P.res[r].hi - P.res[r].lo); return P.res[r].ptr + (src - P.res[r].lo); }
     return nullptr;
+}
+
+// the collect pass for one match (see copy_body<.., COLLECT>): seed bytes that are neither in the window nor in a resident
+// slot become records of the demand list P.gl_nxt; bad offsets are reported by the match launch
+__device__ __forceinline__ void collect_match(const Params& P, const SegCtx& c, uint64_t src, uint64_t dst, uint32_t len) {
+    if (src >= dst || len == 0) return;
+    const bool ovl = src + len > dst;
+    if (ovl && src >= c.sstart) return;                      // FORMAT.md §3 (c): its own literal run
+    const uint32_t seed_len = ovl ? (uint32_t)(dst - src) : len;
+    const uint8_t* end;
+    if (resolve_src(P, src, seed_len, &end)) return;
+    const Stack sk{nullptr, 0, 0, &P.gl_nxt, SKIP_KNOWN};
+    fetch_source_inl(P, sk, src, seed_len, dst - P.out_pos0);
 }
 
 // ---- A4: match resolution from the descriptors the literal launch left ---------------------------------------------------
@@ -1025,7 +1044,7 @@ __device__ __forceinline__ bool next_ticket(const Params& P, unsigned long long&
 }
 
 // The literal launch: A1 + A2 + A3 for every segment of the work list, no dependencies.
-template <int QM>
+template <int QM, bool COLLECT = false>
 __global__ void __launch_bounds__(1024, 1) k_literals(const __grid_constant__ Params P) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
     clear_next_ticket(P);
@@ -1035,7 +1054,7 @@ __global__ void __launch_bounds__(1024, 1) k_literals(const __grid_constant__ Pa
     unsigned long long t;
     while (next_ticket(P, t)) {
         c.s = P.seg_list ? (uint64_t)P.seg_list[t] : P.first_work + t;
-        literals_of_segment<QM>(P, m.luts, m.lutq, m.ring, m.runs, m.lita, c);
+        literals_of_segment<QM, COLLECT>(P, m.luts, m.lutq, m.ring, m.runs, m.lita, c);
     }
 }
 
