@@ -236,6 +236,7 @@ def main():
         whole_file(torch, ar, x, args.config)
         win = min(64 << 20, max(1 << 20, size // 16))
         windows(torch, ar, x, args.config, win, 2)
+        windows(torch, ar, x, args.config, 2 * win, 1)         # the same ring bytes as ONE reused buffer (chunks)
         isolated_windows(torch, ar, x, args.config, win)
         reads(torch, ar, x, datagen.fastq_index(size), args.config)
         seeks(torch, ar, x, args.config)
@@ -329,8 +330,8 @@ def main():
             a = encoder.encode(x, block_size=16384, **kw)
             ar = Archive(a)
             res = whole_file(torch, ar, x, "6/%s" % kw, reps=3)
-            win = min(64 << 20, max(1 << 20, size // 16))
-            ring = ar.new_output(2 * win)
+            win = min(128 << 20, max(1 << 20, size // 8))       # one reused buffer of an eighth of the file
+            ring = ar.new_output(win)
             st = min((ar.decode_stream(0, size, ring, win, consumer=lambda *a_: 0) for _ in range(2)), key=lambda q: q["device_ms"])
             bad = ar.decode_stream(0, size, ring, win)["bad_blocks"]
             emit(config=6, what="encoder_option", options=kw, ratio=x.size / a.size, encode_seconds=time.time() - t, decode_all_GBps=res["default"]["GBps"],
